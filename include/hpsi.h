@@ -1,0 +1,176 @@
+/*
+ * hpsi.h - C ABI of the B200-native effective-Hamiltonian application for two-site QC-DMRG.
+ *
+ * What is computed (BASELINE.json `north_star`; "Numerical procedure" names the step:
+ * "solving a large hermitian eigenvalue problem using e.g. the Lanczos or Davidson method. This step
+ * usually accounts for 80% of the execution time, and scales as O(D^3)"):
+ *
+ *     psi'(l,r) = sum_t  c_t * A_t(l,l') * psi(l',r') * B_t(r,r')^T
+ *
+ * in block-sparse symmetry-sector form, real FP64 (Fig. 1 "FP64"), plain transpose.
+ * Index convention (reading A2):  out[x,y] = sum_{x',y'} A[x,x'] * psi[x',y'] * B[y,y'].
+ *
+ * Layout of psi / out: for left sector i = 0..n_left-1
+ * ascending, if a right sector j with q_left[i] + q_right[j] == target exists, psi holds the dense
+ * d_left[i] x d_right[j] block, row-major, appended to the vector.  hpsi_query(HPSI_Q_PSI_BLOCKS) returns it.
+ *
+ * Pointers: every argument says HOST or DEVICE.  No C++ exception crosses this boundary; every call
+ * returns 0 on success or a negative HPSI_E* code, and hpsi_last_error() gives a thread-local message.
+ * The library has no CPU fallback: without a CUDA device every compute entry point fails with HPSI_ECUDA.
+ */
+#ifndef HPSI_H_
+#define HPSI_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define HPSI_OK       0
+#define HPSI_EINVAL  (-1)   /* malformed sector table / term list / argument                         */
+#define HPSI_ENOMEM  (-2)   /* host or device allocation failed                                      */
+#define HPSI_ECUDA   (-3)   /* CUDA runtime error (message holds cudaGetErrorString)                 */
+#define HPSI_ESTATE  (-4)   /* call not valid in the plan's state (arenas not bound, host-only plan) */
+
+/* hpsi_plan flags */
+#define HPSI_PLAN_HOST_ONLY  (1u << 0)  /* build the schedule on the host only: no CUDA call, no device memory.
+                                           Such a plan serves hpsi_query and hpsi_debug_* ; hpsi_apply -> ESTATE. */
+#define HPSI_PLAN_FIXED_ORDER1 (1u << 1) /* diagnostic: force (A psi) B^T for every task                  */
+#define HPSI_PLAN_FIXED_ORDER2 (1u << 2) /* diagnostic: force A (psi B^T) for every task                  */
+
+typedef struct hpsi_plan hpsi_plan_t;   /* opaque; owns the device schedule and the workspace */
+
+/* "Sector table" (north_star).  All arrays HOST, copied by hpsi_plan. */
+typedef struct {
+  int32_t n_left, n_right;
+  const int32_t* q_left;    /* [n_left][2]  labels (N, 2Sz); unique within the side (else EINVAL) */
+  const int32_t* q_right;   /* [n_right][2]                                                      */
+  const int32_t* d_left;    /* [n_left]  sector dimensions, each >= 1                            */
+  const int32_t* d_right;   /* [n_right]                                                         */
+  int32_t target[2];        /* Q* = (N*, 2Sz*)                                                   */
+} hpsi_sectors_t;
+
+/* One dense operator block: maps sector `col` to sector `row` of its side; rows x cols = d[row] x d[col],
+ * row-major with leading dimension ld >= d[col], starting `offset` doubles into the side's arena. */
+typedef struct {
+  int32_t term, row, col, ld;
+  int64_t offset;
+} hpsi_opblock_t;
+
+/* "Term list" (north_star).  Descriptors and coef are HOST (copied).  a_data / b_data are DEVICE arenas,
+ * caller-owned and BORROWED: they must outlive the plan (no copy is made - at D=8192 they are ~80 GB).
+ * They may be NULL at plan time and bound later with hpsi_bind.  a_len / b_len = arena lengths in doubles
+ * (used to validate descriptors).  Fast path: every block has even `offset` and even `ld` and the arenas
+ * are 16-byte aligned (16-byte cp.async); otherwise a slower 8-byte staging variant of the kernels runs. */
+typedef struct {
+  int32_t n_terms;
+  const double* coef;              /* [n_terms] c_t                                             */
+  int64_t n_a;
+  const hpsi_opblock_t* a_blocks;  /* [n_a] any order; at most one block per (term,row,col)       */
+  int64_t n_b;
+  const hpsi_opblock_t* b_blocks;  /* [n_b]                                                      */
+  const double* a_data;            /* DEVICE (or NULL)                                           */
+  const double* b_data;            /* DEVICE (or NULL)                                           */
+  int64_t a_len, b_len;
+} hpsi_terms_t;
+
+/* Steps 1-4 of SURVEY.md 8(a): psi block table, task enumeration, per-task order choice
+ * (A psi)B^T vs A(psi B^T) by flop count, grouping of all tasks that write one output block, cutting into
+ * CTA work units; uploads the flat schedule and allocates the workspace.  One-off, synchronous. */
+int hpsi_plan(const hpsi_sectors_t* sectors, const hpsi_terms_t* terms, uint32_t flags, hpsi_plan_t** plan_out);
+
+/* (Re)bind the DEVICE operator arenas (same descriptors).  */
+int hpsi_bind(hpsi_plan_t* plan, const double* a_data_dev, const double* b_data_dev);
+
+/* Steps 5-7: out = H psi (overwrite).  psi_dev / out_dev: DEVICE, psi_length doubles each, must not alias.
+ * cuda_stream: a cudaStream_t cast to void* (NULL = default stream).  Enqueue only: no host sync, no
+ * allocation, CUDA-graph capturable.  A plan owns one workspace: do not run it on two streams at once.
+ * Repeated applies on the same inputs are bitwise identical (no atomics on data). */
+int hpsi_apply(hpsi_plan_t* plan, const double* psi_dev, double* out_dev, void* cuda_stream);
+
+/* Same result through HOST buffers: copies psi to the device, applies, copies out back, synchronises the stream.
+ * (End-to-end entry point; operators stay resident in the bound arenas.) */
+int hpsi_apply_host(hpsi_plan_t* plan, const double* psi_host, double* out_host, void* cuda_stream);
+
+/* diag(H) on the psi layout (reading A21): diag[l][x,y] = sum over tasks whose A and B blocks are both
+ * sector-diagonal of c_t * A[x,x] * B[y,y].  diag_dev: DEVICE, psi_length doubles.  Enqueue only. */
+int hpsi_diagonal(hpsi_plan_t* plan, double* diag_dev, void* cuda_stream);
+
+/* Step 8: Davidson-Liu, lowest eigenpair, single root (PAPER.md:62 names the method; A21 gives the
+ * algorithm).  All O(psi_length) work and the small subspace eigenproblem run on the device; the host reads back
+ * one residual norm per iteration to test convergence. */
+typedef struct {
+  double tol;            /* stop when ||H x - theta x|| <= tol                 (default 1e-8) */
+  int32_t max_iter;      /* max matrix-vector products                          (default 200)  */
+  int32_t m_max;         /* max subspace dimension before restart, 2..32        (default 16)   */
+  int32_t precondition;  /* 1: s = r / (diag(H) - theta) with guard; 0: s = r   (default 1)    */
+} hpsi_davidson_params_t;
+
+typedef struct {
+  int32_t n_matvec;      /* hpsi_apply calls made                                             */
+  int32_t converged;     /* 1 if residual <= tol                                              */
+  double residual;       /* last ||H x - theta x||                                            */
+} hpsi_davidson_info_t;
+
+/* psi_inout_dev: DEVICE, psi_length doubles; in = start vector (any non-zero), out = normalised Ritz vector.
+ * eig_host: HOST, receives theta.  params may be NULL (defaults); info may be NULL.  Synchronises the stream. */
+int hpsi_davidson(hpsi_plan_t* plan, double* psi_inout_dev, double* eig_host,
+                  const hpsi_davidson_params_t* params, hpsi_davidson_info_t* info, void* cuda_stream);
+
+/* hpsi_query items.  `out` is HOST; `bytes` must be >= the item's size (else EINVAL). */
+enum {
+  HPSI_Q_PSI_LENGTH = 0,     /* int64: doubles in psi / out                                                  */
+  HPSI_Q_N_PSI_BLOCKS = 1,   /* int64                                                                        */
+  HPSI_Q_PSI_BLOCKS = 2,     /* hpsi_psi_block_t[n_psi_blocks]                                               */
+  HPSI_Q_N_TASKS = 3,        /* int64: realisable (term, A block, B block) triples                            */
+  HPSI_Q_USEFUL_FLOPS = 4,   /* int64: sum over tasks of min(2 m n'(k+n), 2 k n(n'+m))  (A18)        */
+  HPSI_Q_ISSUED_FLOPS = 5,   /* int64: flops of the DMMA instructions the schedule issues (8x8x4 padding incl.) */
+  HPSI_Q_OPERATOR_BYTES = 6, /* int64: 8 * (m k + n n') summed over tasks (bytes streamed once per apply)     */
+  HPSI_Q_WORKSPACE_BYTES = 7,/* int64: device workspace the plan owns                                         */
+  HPSI_Q_N_GROUPS = 8,       /* int64: (source block, destination block) groups                               */
+  HPSI_Q_N_P1_UNITS = 9,     /* int64: CTA work units of the first-GEMM kernel                                */
+  HPSI_Q_N_P2_UNITS = 10,    /* int64: CTA work units of the second-GEMM kernel                               */
+  HPSI_Q_N_ORDER1_TASKS = 11,/* int64: tasks scheduled as (A psi) B^T                                         */
+  HPSI_Q_LAUNCHES_PER_APPLY = 12, /* int64: kernels hpsi_apply enqueues                                       */
+  HPSI_Q_ALIGNED16 = 13,     /* int64: 1 if the 16-byte staging path is used                                  */
+  HPSI_Q_INTERMEDIATE_BYTES = 14, /* int64: bytes of first-GEMM results written (and read back) per apply     */
+  HPSI_Q_ISSUED_FLOPS_P1 = 15,    /* int64: first-GEMM share of HPSI_Q_ISSUED_FLOPS                           */
+  HPSI_Q_TASKS = 16          /* hpsi_task_t[n_tasks], in schedule order                                      */
+};
+
+typedef struct {
+  int32_t left, right;   /* sector indices                     */
+  int32_t rows, cols;    /* d_left[left], d_right[right]       */
+  int64_t offset;        /* start in psi, in doubles           */
+} hpsi_psi_block_t;
+
+typedef struct {
+  int32_t term, a_block, b_block;   /* indices into the term list's a_blocks / b_blocks            */
+  int32_t src_left, dst_left;       /* psi blocks (by left sector) read / written                  */
+  int32_t order;                    /* 1 = (A psi) B^T, 2 = A (psi B^T)                            */
+} hpsi_task_t;
+
+int hpsi_query(const hpsi_plan_t* plan, int what, void* out, size_t bytes);
+
+void hpsi_destroy(hpsi_plan_t* plan);
+
+const char* hpsi_last_error(void);
+
+/* FP64 tensor-pipe microbenchmarks used by bench.py's calibration: run `iters`
+ * dependent-chain rounds of register-resident DMMA.8x8x4 (kind 0), DFMA (kind 1) or both interleaved (kind 2)
+ * on every SM and return the elapsed milliseconds and the flops executed.  HOST outputs. */
+int hpsi_bench_fp64_pipe(int kind, int iters, double* ms_out, double* flops_out);
+
+/* ---- debug / test entry points (HOST memory only; run the *device schedule* with naive loops on the CPU) ----
+ * hpsi_debug_interpret executes exactly the work-unit tables the kernels consume (prep, first GEMM units,
+ * second GEMM units, ordered reduce) so that the planner can be verified on a box without a GPU.
+ * a_host / b_host are HOST copies of the arenas, psi_host / out_host HOST vectors of psi_length doubles. */
+int hpsi_debug_interpret(const hpsi_plan_t* plan, const double* a_host, const double* b_host,
+                         const double* psi_host, double* out_host);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* HPSI_H_ */

@@ -1,0 +1,215 @@
+"""Thin ctypes binding of include/hpsi.h: same names, argument marshalling only (every step of the path runs in
+libhpsi.so's kernels).  Device buffers are passed as torch CUDA tensors (or raw integer addresses); PyTorch is used
+for device memory and streams only.  There is no CPU fallback: if libhpsi.so is missing or CUDA is unavailable
+the calls raise."""
+from __future__ import annotations
+
+import ctypes
+import os
+from typing import Optional
+
+import numpy as np
+
+from .build import LIB, build
+
+HPSI_OK, HPSI_EINVAL, HPSI_ENOMEM, HPSI_ECUDA, HPSI_ESTATE = 0, -1, -2, -3, -4
+HPSI_PLAN_HOST_ONLY = 1 << 0
+HPSI_PLAN_FIXED_ORDER1 = 1 << 1
+HPSI_PLAN_FIXED_ORDER2 = 1 << 2
+
+(HPSI_Q_PSI_LENGTH, HPSI_Q_N_PSI_BLOCKS, HPSI_Q_PSI_BLOCKS, HPSI_Q_N_TASKS, HPSI_Q_USEFUL_FLOPS, HPSI_Q_ISSUED_FLOPS,
+ HPSI_Q_OPERATOR_BYTES, HPSI_Q_WORKSPACE_BYTES, HPSI_Q_N_GROUPS, HPSI_Q_N_P1_UNITS, HPSI_Q_N_P2_UNITS,
+ HPSI_Q_N_ORDER1_TASKS, HPSI_Q_LAUNCHES_PER_APPLY, HPSI_Q_ALIGNED16, HPSI_Q_INTERMEDIATE_BYTES,
+ HPSI_Q_ISSUED_FLOPS_P1, HPSI_Q_TASKS) = range(17)
+
+PSI_BLOCK_DTYPE = np.dtype([("left", "<i4"), ("right", "<i4"), ("rows", "<i4"), ("cols", "<i4"), ("offset", "<i8")],
+                           align=True)
+TASK_DTYPE = np.dtype([("term", "<i4"), ("a_block", "<i4"), ("b_block", "<i4"), ("src_left", "<i4"),
+                       ("dst_left", "<i4"), ("order", "<i4")], align=True)
+
+
+class hpsi_sectors_t(ctypes.Structure):
+    _fields_ = [("n_left", ctypes.c_int32), ("n_right", ctypes.c_int32),
+                ("q_left", ctypes.c_void_p), ("q_right", ctypes.c_void_p),
+                ("d_left", ctypes.c_void_p), ("d_right", ctypes.c_void_p),
+                ("target", ctypes.c_int32 * 2)]
+
+
+class hpsi_terms_t(ctypes.Structure):
+    _fields_ = [("n_terms", ctypes.c_int32), ("coef", ctypes.c_void_p),
+                ("n_a", ctypes.c_int64), ("a_blocks", ctypes.c_void_p),
+                ("n_b", ctypes.c_int64), ("b_blocks", ctypes.c_void_p),
+                ("a_data", ctypes.c_void_p), ("b_data", ctypes.c_void_p),
+                ("a_len", ctypes.c_int64), ("b_len", ctypes.c_int64)]
+
+
+class hpsi_davidson_params_t(ctypes.Structure):
+    _fields_ = [("tol", ctypes.c_double), ("max_iter", ctypes.c_int32), ("m_max", ctypes.c_int32),
+                ("precondition", ctypes.c_int32)]
+
+
+class hpsi_davidson_info_t(ctypes.Structure):
+    _fields_ = [("n_matvec", ctypes.c_int32), ("converged", ctypes.c_int32), ("residual", ctypes.c_double)]
+
+
+class HpsiError(RuntimeError):
+    def __init__(self, code: int, msg: str):
+        super().__init__(f"hpsi error {code}: {msg}")
+        self.code = code
+
+
+_lib = None
+
+
+def lib() -> ctypes.CDLL:
+    """Load libhpsi.so (building it in-tree with nvcc if it is missing or stale).  Raises if that fails."""
+    global _lib
+    if _lib is None:
+        path = build() if not os.environ.get("HPSI_NO_BUILD") else LIB
+        L = ctypes.CDLL(path)
+        vp, i32, i64 = ctypes.c_void_p, ctypes.c_int32, ctypes.c_int64
+        L.hpsi_plan.argtypes = [ctypes.POINTER(hpsi_sectors_t), ctypes.POINTER(hpsi_terms_t), ctypes.c_uint32,
+                                ctypes.POINTER(vp)]
+        L.hpsi_bind.argtypes = [vp, vp, vp]
+        L.hpsi_apply.argtypes = [vp, vp, vp, vp]
+        L.hpsi_apply_host.argtypes = [vp, vp, vp, vp]
+        L.hpsi_diagonal.argtypes = [vp, vp, vp]
+        L.hpsi_davidson.argtypes = [vp, vp, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(hpsi_davidson_params_t),
+                                    ctypes.POINTER(hpsi_davidson_info_t), vp]
+        L.hpsi_query.argtypes = [vp, ctypes.c_int, vp, ctypes.c_size_t]
+        L.hpsi_destroy.argtypes = [vp]
+        L.hpsi_destroy.restype = None
+        L.hpsi_last_error.restype = ctypes.c_char_p
+        L.hpsi_bench_fp64_pipe.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.POINTER(ctypes.c_double),
+                                           ctypes.POINTER(ctypes.c_double)]
+        L.hpsi_debug_interpret.argtypes = [vp, vp, vp, vp, vp]
+        for name in ("hpsi_plan", "hpsi_bind", "hpsi_apply", "hpsi_apply_host", "hpsi_diagonal", "hpsi_davidson",
+                     "hpsi_query", "hpsi_bench_fp64_pipe", "hpsi_debug_interpret"):
+            getattr(L, name).restype = ctypes.c_int
+        del i32, i64
+        _lib = L
+    return _lib
+
+
+def _check(rc: int) -> None:
+    if rc != HPSI_OK:
+        raise HpsiError(rc, lib().hpsi_last_error().decode())
+
+
+def _ptr(x) -> Optional[int]:
+    """Address of a torch tensor / numpy array / int / None."""
+    if x is None:
+        return None
+    if isinstance(x, int):
+        return x
+    if isinstance(x, np.ndarray):
+        assert x.flags.c_contiguous
+        return x.ctypes.data
+    assert x.is_contiguous()
+    return x.data_ptr()
+
+
+def _stream(stream) -> Optional[int]:
+    if stream is None:
+        return None
+    if isinstance(stream, int):
+        return stream or None
+    return stream.cuda_stream or None
+
+
+class Plan:
+    """Opaque hpsi_plan_t* plus the host arrays whose lifetime the caller would otherwise have to manage."""
+
+    def __init__(self, handle: int, keep):
+        self.handle = handle
+        self._keep = keep
+
+    def __del__(self):
+        if getattr(self, "handle", None):
+            lib().hpsi_destroy(self.handle)
+            self.handle = None
+
+
+def hpsi_plan(q_left, q_right, d_left, d_right, target, coef, a_blocks, b_blocks, a_data=None, b_data=None,
+              a_len: int = 0, b_len: int = 0, flags: int = 0) -> Plan:
+    """hpsi_plan(sector table, term list).  Host arrays: numpy; a_blocks/b_blocks: numpy arrays with the 24-byte
+    hpsi_opblock_t layout; a_data/b_data: torch CUDA float64 tensors (or None, to hpsi_bind later)."""
+    q_left = np.ascontiguousarray(q_left, np.int32).reshape(-1, 2)
+    q_right = np.ascontiguousarray(q_right, np.int32).reshape(-1, 2)
+    d_left = np.ascontiguousarray(d_left, np.int32)
+    d_right = np.ascontiguousarray(d_right, np.int32)
+    coef = np.ascontiguousarray(coef, np.float64)
+    a_blocks = np.ascontiguousarray(a_blocks)
+    b_blocks = np.ascontiguousarray(b_blocks)
+    assert a_blocks.dtype.itemsize == 24 and b_blocks.dtype.itemsize == 24
+    sec = hpsi_sectors_t(q_left.shape[0], q_right.shape[0], q_left.ctypes.data, q_right.ctypes.data,
+                         d_left.ctypes.data, d_right.ctypes.data, (ctypes.c_int32 * 2)(int(target[0]), int(target[1])))
+    trm = hpsi_terms_t(coef.shape[0], coef.ctypes.data, a_blocks.shape[0], a_blocks.ctypes.data,
+                       b_blocks.shape[0], b_blocks.ctypes.data, _ptr(a_data), _ptr(b_data), int(a_len), int(b_len))
+    out = ctypes.c_void_p()
+    _check(lib().hpsi_plan(ctypes.byref(sec), ctypes.byref(trm), flags, ctypes.byref(out)))
+    return Plan(out.value, (a_data, b_data))
+
+
+def hpsi_bind(plan: Plan, a_data, b_data) -> None:
+    _check(lib().hpsi_bind(plan.handle, _ptr(a_data), _ptr(b_data)))
+    plan._keep = (a_data, b_data)
+
+
+def hpsi_apply(plan: Plan, psi, out, stream=None) -> None:
+    """out = H psi; psi/out: torch CUDA float64 tensors of psi_length; stream: torch.cuda.Stream or None."""
+    _check(lib().hpsi_apply(plan.handle, _ptr(psi), _ptr(out), _stream(stream)))
+
+
+def hpsi_apply_host(plan: Plan, psi_host, out_host, stream=None) -> None:
+    """Same through HOST buffers (numpy arrays or pinned torch CPU tensors)."""
+    _check(lib().hpsi_apply_host(plan.handle, _ptr(psi_host), _ptr(out_host), _stream(stream)))
+
+
+def hpsi_diagonal(plan: Plan, diag, stream=None) -> None:
+    _check(lib().hpsi_diagonal(plan.handle, _ptr(diag), _stream(stream)))
+
+
+def hpsi_davidson(plan: Plan, psi_inout, tol: float = 1e-8, max_iter: int = 200, m_max: int = 16,
+                  precondition: bool = True, stream=None):
+    """Returns (theta, info dict); psi_inout (torch CUDA tensor) is overwritten with the Ritz vector."""
+    prm = hpsi_davidson_params_t(tol, max_iter, m_max, 1 if precondition else 0)
+    info = hpsi_davidson_info_t()
+    eig = ctypes.c_double()
+    _check(lib().hpsi_davidson(plan.handle, _ptr(psi_inout), ctypes.byref(eig), ctypes.byref(prm),
+                               ctypes.byref(info), _stream(stream)))
+    return eig.value, {"n_matvec": info.n_matvec, "converged": bool(info.converged), "residual": info.residual}
+
+
+def hpsi_query(plan: Plan, what: int):
+    """Scalar items return int; HPSI_Q_PSI_BLOCKS / HPSI_Q_TASKS return structured numpy arrays."""
+    if what in (HPSI_Q_PSI_BLOCKS, HPSI_Q_TASKS):
+        n = hpsi_query(plan, HPSI_Q_N_PSI_BLOCKS if what == HPSI_Q_PSI_BLOCKS else HPSI_Q_N_TASKS)
+        arr = np.zeros(max(n, 1), PSI_BLOCK_DTYPE if what == HPSI_Q_PSI_BLOCKS else TASK_DTYPE)
+        _check(lib().hpsi_query(plan.handle, what, arr.ctypes.data, arr.nbytes))
+        return arr[:n]
+    v = ctypes.c_int64()
+    _check(lib().hpsi_query(plan.handle, what, ctypes.addressof(v), 8))
+    return v.value
+
+
+def hpsi_bench_fp64_pipe(kind: int, iters: int):
+    """(milliseconds, flops) of the register-resident FP64 pipe probe (0 DMMA, 1 DFMA, 2 both)."""
+    ms, fl = ctypes.c_double(), ctypes.c_double()
+    _check(lib().hpsi_bench_fp64_pipe(kind, iters, ctypes.byref(ms), ctypes.byref(fl)))
+    return ms.value, fl.value
+
+
+def hpsi_debug_interpret(plan: Plan, a_host: np.ndarray, b_host: np.ndarray, psi_host: np.ndarray) -> np.ndarray:
+    """Run the device schedule with naive loops on the CPU (planner verification; tests only)."""
+    psi_host = np.ascontiguousarray(psi_host, np.float64)
+    out = np.empty_like(psi_host)
+    _check(lib().hpsi_debug_interpret(plan.handle, _ptr(np.ascontiguousarray(a_host, np.float64)),
+                                      _ptr(np.ascontiguousarray(b_host, np.float64)), _ptr(psi_host), _ptr(out)))
+    return out
+
+
+def plan_problem(p, a_data=None, b_data=None, flags: int = 0) -> Plan:
+    """Marshal a ``workloads.Problem`` (any object with the boundary's fields) into hpsi_plan."""
+    return hpsi_plan(p.q_left, p.q_right, p.d_left, p.d_right, p.target, p.coef, p.a_desc, p.b_desc,
+                     a_data, b_data, p.a_len, p.b_len, flags)

@@ -1,0 +1,240 @@
+// C-ABI entry points of include/hpsi.h (plan / bind / apply / query / destroy / debug).
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "plan_dev.h"
+
+namespace hpsi {
+static thread_local std::string g_err;
+void set_error(const std::string& s) { g_err = s; }
+int cuda_fail(cudaError_t e, const char* what) {
+  g_err = std::string("CUDA error: ") + cudaGetErrorString(e) + " in " + what;
+  cudaGetLastError();
+  return HPSI_ECUDA;
+}
+}  // namespace hpsi
+
+using namespace hpsi;
+
+extern "C" const char* hpsi_last_error(void) { return g_err.c_str(); }
+
+namespace {
+
+template <class T>
+size_t table_bytes(const std::vector<T>& v) { return (v.size() * sizeof(T) + 255) / 256 * 256 + 256; }
+
+template <class T>
+int upload(const std::vector<T>& v, char* base, size_t& cursor, const T** dev_ptr) {
+  *dev_ptr = reinterpret_cast<const T*>(base + cursor);
+  if (!v.empty()) HPSI_CUDA(cudaMemcpy(base + cursor, v.data(), v.size() * sizeof(T), cudaMemcpyHostToDevice));
+  cursor += table_bytes(v);
+  return HPSI_OK;
+}
+
+int upload_schedule(hpsi_plan_t* p) {
+  const Schedule& sc = p->sc;
+  size_t total = table_bytes(sc.blocks) + table_bytes(sc.segs) + table_bytes(sc.groups) + table_bytes(sc.p1) +
+                 table_bytes(sc.runs) + table_bytes(sc.p2) + table_bytes(sc.diag);
+  HPSI_CUDA(cudaMalloc(&p->d_tables, total));
+  cudaError_t e = cudaMalloc(&p->d_ws, (size_t)sc.ws_len * sizeof(double));
+  if (e != cudaSuccess) {
+    cudaGetLastError();
+    char buf[160];
+    snprintf(buf, sizeof buf, "device workspace allocation of %.2f GB failed", sc.ws_len * 8.0 / 1e9);
+    set_error(buf);
+    return HPSI_ENOMEM;
+  }
+  HPSI_CUDA(cudaMemset(p->d_ws, 0, (size_t)sc.ws_len * sizeof(double)));
+  char* base = static_cast<char*>(p->d_tables);
+  size_t cur = 0;
+  int rc;
+  if ((rc = upload(sc.blocks, base, cur, &p->dev.blocks))) return rc;
+  if ((rc = upload(sc.segs, base, cur, &p->dev.segs))) return rc;
+  if ((rc = upload(sc.groups, base, cur, &p->dev.groups))) return rc;
+  if ((rc = upload(sc.p1, base, cur, &p->dev.p1))) return rc;
+  if ((rc = upload(sc.runs, base, cur, &p->dev.runs))) return rc;
+  if ((rc = upload(sc.p2, base, cur, &p->dev.p2))) return rc;
+  if ((rc = upload(sc.diag, base, cur, &p->dev.diag))) return rc;
+  p->dev.ws = p->d_ws;
+  p->dev.n_blocks = (int)sc.blocks.size();
+  p->dev.n_p1 = (int)sc.p1.size();
+  p->dev.n_p2 = (int)sc.p2.size();
+  p->dev.max_block_elems = sc.max_block_elems;
+  if (sc.psi_len > 0) {
+    HPSI_CUDA(cudaMalloc(&p->d_psi_stage, (size_t)sc.psi_len * sizeof(double)));
+    HPSI_CUDA(cudaMalloc(&p->d_out_stage, (size_t)sc.psi_len * sizeof(double)));
+  }
+  return HPSI_OK;
+}
+
+void free_plan(hpsi_plan_t* p) {
+  if (!p) return;
+  if (!p->host_only) {
+    cudaFree(p->d_tables);
+    cudaFree(p->d_ws);
+    cudaFree(p->d_psi_stage);
+    cudaFree(p->d_out_stage);
+    cudaFree(p->d_dav);
+    cudaGetLastError();
+  }
+  delete p;
+}
+
+}  // namespace
+
+extern "C" int hpsi_bind(hpsi_plan_t* p, const double* a_dev, const double* b_dev) {
+  if (!p) { set_error("null plan"); return HPSI_EINVAL; }
+  if (p->host_only) { set_error("host-only plan cannot bind device arenas"); return HPSI_ESTATE; }
+  bool need_a = false, need_b = false;
+  for (const Seg& s : p->sc.segs) { (void)s; need_a = need_b = true; break; }
+  if ((need_a && !a_dev) || (need_b && !b_dev)) { set_error("null operator arena"); return HPSI_EINVAL; }
+  p->dev.a = a_dev;
+  p->dev.b = b_dev;
+  p->aligned16 = p->sc.aligned16 && ((reinterpret_cast<uintptr_t>(a_dev) & 15) == 0) &&
+                 ((reinterpret_cast<uintptr_t>(b_dev) & 15) == 0);
+  p->bound = true;
+  return HPSI_OK;
+}
+
+extern "C" int hpsi_plan(const hpsi_sectors_t* sectors, const hpsi_terms_t* terms, uint32_t flags,
+                         hpsi_plan_t** plan_out) {
+  if (!plan_out) { set_error("null plan_out"); return HPSI_EINVAL; }
+  *plan_out = nullptr;
+  hpsi_plan_t* p = new (std::nothrow) hpsi_plan_t();
+  if (!p) { set_error("out of host memory"); return HPSI_ENOMEM; }
+  p->host_only = (flags & HPSI_PLAN_HOST_ONLY) != 0;
+  int rc = HPSI_OK;
+  try {
+    if (!p->host_only) {
+      int dev = 0;
+      cudaError_t e = cudaGetDevice(&dev);
+      if (e == cudaSuccess) e = cudaDeviceGetAttribute(&p->n_sm, cudaDevAttrMultiProcessorCount, dev);
+      if (e == cudaSuccess) e = kernels_init();
+      if (e != cudaSuccess) {
+        rc = cuda_fail(e, "device initialisation (no CPU fallback exists)");
+        p->host_only = true;   // nothing to free on the device
+        free_plan(p);
+        return rc;
+      }
+    }
+    std::string err;
+    rc = build_schedule(sectors, terms, flags, p->n_sm, &p->sc, &err);
+    if (rc != HPSI_OK) { set_error(err); free_plan(p); return rc; }
+    if (!p->host_only) {
+      rc = upload_schedule(p);
+      if (rc != HPSI_OK) { free_plan(p); return rc; }
+      if (terms->a_data || terms->b_data || p->sc.segs.empty()) {
+        rc = hpsi_bind(p, terms->a_data, terms->b_data);
+        if (rc != HPSI_OK) { free_plan(p); return rc; }
+      }
+    }
+  } catch (const std::bad_alloc&) {
+    set_error("out of host memory while planning");
+    p->host_only = true;
+    free_plan(p);
+    return HPSI_ENOMEM;
+  }
+  *plan_out = p;
+  return HPSI_OK;
+}
+
+extern "C" void hpsi_destroy(hpsi_plan_t* p) { free_plan(p); }
+
+extern "C" int hpsi_apply(hpsi_plan_t* p, const double* psi_dev, double* out_dev, void* cuda_stream) {
+  if (!p) { set_error("null plan"); return HPSI_EINVAL; }
+  if (p->host_only) { set_error("host-only plan: hpsi_apply needs a CUDA device (no CPU fallback)"); return HPSI_ESTATE; }
+  if (!p->bound) { set_error("operator arenas not bound (hpsi_bind)"); return HPSI_ESTATE; }
+  if (p->sc.psi_len == 0) return HPSI_OK;
+  if (!psi_dev || !out_dev) { set_error("null psi/out"); return HPSI_EINVAL; }
+  if (psi_dev == out_dev) { set_error("psi and out must not alias"); return HPSI_EINVAL; }
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  launch_prep(p->dev, psi_dev, st);
+  launch_p1(p->dev, p->aligned16, st);
+  launch_p2(p->dev, p->aligned16, st);
+  launch_reduce(p->dev, out_dev, st);
+  HPSI_CUDA(cudaGetLastError());
+  return HPSI_OK;
+}
+
+extern "C" int hpsi_apply_host(hpsi_plan_t* p, const double* psi_host, double* out_host, void* cuda_stream) {
+  if (!p) { set_error("null plan"); return HPSI_EINVAL; }
+  if (p->host_only) { set_error("host-only plan: hpsi_apply_host needs a CUDA device (no CPU fallback)"); return HPSI_ESTATE; }
+  if (p->sc.psi_len == 0) return HPSI_OK;
+  if (!psi_host || !out_host) { set_error("null psi/out"); return HPSI_EINVAL; }
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  const size_t bytes = (size_t)p->sc.psi_len * sizeof(double);
+  HPSI_CUDA(cudaMemcpyAsync(p->d_psi_stage, psi_host, bytes, cudaMemcpyHostToDevice, st));
+  int rc = hpsi_apply(p, p->d_psi_stage, p->d_out_stage, cuda_stream);
+  if (rc != HPSI_OK) return rc;
+  HPSI_CUDA(cudaMemcpyAsync(out_host, p->d_out_stage, bytes, cudaMemcpyDeviceToHost, st));
+  HPSI_CUDA(cudaStreamSynchronize(st));
+  return HPSI_OK;
+}
+
+extern "C" int hpsi_diagonal(hpsi_plan_t* p, double* diag_dev, void* cuda_stream) {
+  if (!p) { set_error("null plan"); return HPSI_EINVAL; }
+  if (p->host_only) { set_error("host-only plan: hpsi_diagonal needs a CUDA device"); return HPSI_ESTATE; }
+  if (!p->bound) { set_error("operator arenas not bound (hpsi_bind)"); return HPSI_ESTATE; }
+  if (p->sc.psi_len == 0) return HPSI_OK;
+  if (!diag_dev) { set_error("null diag"); return HPSI_EINVAL; }
+  launch_diag(p->dev, diag_dev, static_cast<cudaStream_t>(cuda_stream));
+  HPSI_CUDA(cudaGetLastError());
+  return HPSI_OK;
+}
+
+extern "C" int hpsi_query(const hpsi_plan_t* p, int what, void* out, size_t bytes) {
+  if (!p || !out) { set_error("null argument"); return HPSI_EINVAL; }
+  const Schedule& sc = p->sc;
+  auto put_i64 = [&](int64_t v) -> int {
+    if (bytes < sizeof(int64_t)) { set_error("hpsi_query: buffer too small"); return HPSI_EINVAL; }
+    memcpy(out, &v, sizeof v);
+    return HPSI_OK;
+  };
+  switch (what) {
+    case HPSI_Q_PSI_LENGTH: return put_i64(sc.psi_len);
+    case HPSI_Q_N_PSI_BLOCKS: return put_i64((int64_t)sc.blocks.size());
+    case HPSI_Q_PSI_BLOCKS: {
+      if (bytes < sc.blocks.size() * sizeof(hpsi_psi_block_t)) { set_error("hpsi_query: buffer too small"); return HPSI_EINVAL; }
+      hpsi_psi_block_t* o = static_cast<hpsi_psi_block_t*>(out);
+      for (size_t i = 0; i < sc.blocks.size(); ++i)
+        o[i] = {sc.blocks[i].left, sc.blocks[i].right, sc.blocks[i].rows, sc.blocks[i].cols, sc.blocks[i].off};
+      return HPSI_OK;
+    }
+    case HPSI_Q_N_TASKS: return put_i64((int64_t)sc.segs.size());
+    case HPSI_Q_USEFUL_FLOPS: return put_i64(sc.useful_flops);
+    case HPSI_Q_ISSUED_FLOPS: return put_i64(sc.issued_flops);
+    case HPSI_Q_ISSUED_FLOPS_P1: return put_i64(sc.issued_flops_p1);
+    case HPSI_Q_OPERATOR_BYTES: return put_i64(sc.operator_bytes);
+    case HPSI_Q_WORKSPACE_BYTES: return put_i64(sc.ws_len * 8);
+    case HPSI_Q_N_GROUPS: return put_i64((int64_t)sc.groups.size());
+    case HPSI_Q_N_P1_UNITS: return put_i64((int64_t)sc.p1.size());
+    case HPSI_Q_N_P2_UNITS: return put_i64((int64_t)sc.p2.size());
+    case HPSI_Q_N_ORDER1_TASKS: return put_i64(sc.n_order1);
+    case HPSI_Q_LAUNCHES_PER_APPLY:
+      return put_i64((sc.blocks.empty() ? 0 : 2) + (sc.p1.empty() ? 0 : 1) + (sc.p2.empty() ? 0 : 1));
+    case HPSI_Q_ALIGNED16: return put_i64(p->host_only ? sc.aligned16 : p->aligned16);
+    case HPSI_Q_INTERMEDIATE_BYTES: return put_i64(sc.intermediate_bytes);
+    case HPSI_Q_TASKS: {
+      if (bytes < sc.tasks.size() * sizeof(hpsi_task_t)) { set_error("hpsi_query: buffer too small"); return HPSI_EINVAL; }
+      if (!sc.tasks.empty()) memcpy(out, sc.tasks.data(), sc.tasks.size() * sizeof(hpsi_task_t));
+      return HPSI_OK;
+    }
+    default: set_error("hpsi_query: unknown item"); return HPSI_EINVAL;
+  }
+}
+
+extern "C" int hpsi_debug_interpret(const hpsi_plan_t* p, const double* a_host, const double* b_host,
+                                    const double* psi_host, double* out_host) {
+  if (!p) { set_error("null plan"); return HPSI_EINVAL; }
+  if (p->sc.psi_len > 0 && (!psi_host || !out_host)) { set_error("null psi/out"); return HPSI_EINVAL; }
+  if (!p->sc.segs.empty() && (!a_host || !b_host)) { set_error("null arena"); return HPSI_EINVAL; }
+  try {
+    interpret_schedule(p->sc, a_host, b_host, psi_host, out_host);
+  } catch (const std::bad_alloc&) {
+    set_error("out of host memory in interpreter");
+    return HPSI_ENOMEM;
+  }
+  return HPSI_OK;
+}

@@ -1,0 +1,75 @@
+// Host interpreter of the device schedule (hpsi_debug_interpret): walks exactly the tables the kernels consume
+// - prep (padded psi / psi^T), P1 units, P2 units, ordered reduce - with naive loops, so the planner can be
+// verified against the oracle on a box without a GPU.  Test infrastructure for the planner; not a compute path:
+// hpsi_apply never calls it.
+#include <vector>
+
+#include "plan.h"
+
+namespace hpsi {
+
+void interpret_schedule(const Schedule& sc, const double* a, const double* b, const double* psi, double* out) {
+  std::vector<double> wsv((size_t)sc.ws_len, 0.0);
+  double* ws = wsv.data();
+  // prep
+  for (const PsiBlk& B : sc.blocks)
+    for (int x = 0; x < B.rows; ++x)
+      for (int y = 0; y < B.cols; ++y) {
+        double v = psi[B.off + (int64_t)x * B.cols + y];
+        ws[B.p_off + (int64_t)x * B.ldp + y] = v;
+        ws[B.t_off + (int64_t)y * B.ldt + x] = v;
+      }
+  // P1: C[R, j] = coef(seg of R) * sum_k X[R,k] Y[j,k]
+  for (const P1Unit& u : sc.p1) {
+    const Group& g = sc.groups[u.group];
+    const double* xbase = (g.order == 1) ? a : b;
+    const double* y = ws + g.y1_off;
+    for (int r = 0; r < u.rows_valid; ++r) {
+      const int R = u.R0 + r;
+      const int ti = R / g.rows, x = R % g.rows;
+      const Seg& sg = sc.segs[g.seg0 + ti];
+      const double* xr = xbase + sg.p1_off + (int64_t)x * sg.p1_ld;
+      for (int c = 0; c < u.cols_valid; ++c) {
+        const int j = u.j0 + c;
+        const double* yr = y + (int64_t)j * g.ldy1;
+        double s = 0.0;
+        for (int k = 0; k < g.K1; ++k) s += xr[k] * yr[k];
+        ws[g.ws_off + (int64_t)R * g.ldw + j] = sg.coef * s;
+      }
+    }
+  }
+  // P2: partial[i,j] = sum over runs, segs, k of X[i,k] Y[j,k]
+  for (const P2Unit& u : sc.p2) {
+    for (int r = 0; r < u.rows_valid; ++r)
+      for (int c = 0; c < u.cols_valid; ++c) {
+        double s = 0.0;
+        for (int ri = u.run_begin; ri < u.run_end; ++ri) {
+          const Run& run = sc.runs[ri];
+          for (int si = run.seg_begin; si < run.seg_end; ++si) {
+            const Seg& sg = sc.segs[si];
+            const double *xr, *yr;
+            if (run.order == 1) {
+              xr = ws + sg.ws_off + (int64_t)(u.i0 + r) * run.ldw;
+              yr = b + sg.p2_off + (int64_t)(u.j0 + c) * sg.p2_ld;
+            } else {
+              xr = a + sg.p2_off + (int64_t)(u.i0 + r) * sg.p2_ld;
+              yr = ws + sg.ws_off + (int64_t)(u.j0 + c) * run.ldw;
+            }
+            for (int k = 0; k < run.K; ++k) s += xr[k] * yr[k];
+          }
+        }
+        ws[u.out_off + (int64_t)r * u.ldo + c] = s;
+      }
+  }
+  // ordered reduce
+  for (const PsiBlk& B : sc.blocks)
+    for (int x = 0; x < B.rows; ++x)
+      for (int y = 0; y < B.cols; ++y) {
+        double s = 0.0;
+        for (int sp = 0; sp < B.nsplit; ++sp)
+          s += ws[B.part_off + (int64_t)sp * B.rows * B.ldo + (int64_t)x * B.ldo + y];
+        out[B.off + (int64_t)x * B.cols + y] = s;
+      }
+}
+
+}  // namespace hpsi

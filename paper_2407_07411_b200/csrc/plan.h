@@ -1,0 +1,116 @@
+// Internal schedule format shared by the host planner, the host schedule interpreter and the kernels.
+// Flat POD tables only: the same bytes are uploaded to the device and walked by hpsi_debug_interpret.
+//
+// Vocabulary:
+//   task   = (term t, A block l<-l', B block r<-r') with (l',r') and (l,r) both psi blocks          (8(a)-2)
+//   group  = all tasks with the same (source psi block, destination psi block); they share the dims
+//            (m,k,n',n), hence the order choice, and are STACKED along one GEMM dimension            (8(a)-4)
+//   seg    = one task seen as a K-segment of the second GEMM / a row-segment of the first GEMM
+//   P1     = first GEMM  (order 1: T_t = c_t A_t psi ; order 2: U_t^T = c_t B_t psi^T), stacked over the group's terms
+//   P2     = second GEMM (order 1: out += T_t B_t^T ; order 2: out += A_t U_t), K runs over all segs of all groups
+//            that write one destination block; split-K partials + ordered reduce, no atomics on data.
+// Every GEMM is "NT": C[i,j] = sum_k X[i,k] * Y[j,k] with both operands K-contiguous.
+#pragma once
+#include <cstdint>
+#include <string>
+#include <vector>
+
+#include "../../include/hpsi.h"
+
+namespace hpsi {
+
+constexpr int TILE = 64;      // CTA tile edge (rows and cols), 8 fragments of 8
+constexpr int KT = 16;        // K extent of one staged tile (4 DMMA k-steps)
+
+enum BaseSel : int32_t { BASE_A = 0, BASE_B = 1, BASE_WS = 2 };
+
+struct Seg {                  // one task, in schedule order (by destination, source, term)
+  int64_t p1_off;             // operator block used by P1 (order 1: A_t, order 2: B_t), doubles into its arena
+  int64_t p2_off;             // operator block used by P2 (order 1: B_t, order 2: A_t)
+  int64_t ws_off;             // start of this task's intermediate (rows x ldw) in the workspace
+  int32_t p1_ld, p2_ld;       // leading dimensions of those blocks
+  double coef;                // per-task coefficient (initialised to c_t; reading A4)
+};
+
+struct Group {
+  int32_t order;              // 1 or 2
+  int32_t tcount;             // tasks (terms) in the group
+  int32_t seg0;               // first Seg
+  int32_t rows;               // rows of one task's intermediate (order 1: m, order 2: n)
+  int32_t K1;                 // P1 contraction length (order 1: k, order 2: n')
+  int32_t N1;                 // P1 columns = P2 segment length (order 1: n', order 2: k)
+  int32_t ldw;                // leading dimension of the intermediate (N1 rounded up to even)
+  int32_t ldy1;               // leading dimension of the P1 Y operand (padded psi^T or psi block)
+  int64_t y1_off;             // its offset in the workspace
+  int64_t ws_off;             // start of the stacked intermediate  [(tcount*rows) x ldw]
+  int32_t src, dst;           // psi block indices
+};
+
+struct P1Unit {               // one CTA of the first-GEMM kernel
+  int32_t group;
+  int32_t R0, rows_valid;     // stacked-row tile
+  int32_t j0, cols_valid;     // column tile
+  int32_t pad;
+};
+
+struct Run {                  // consecutive segs of one group inside one P2 unit's K range
+  int32_t seg_begin, seg_end;
+  int32_t K;                  // segment length (group.N1)
+  int32_t ldw;                // ld of the intermediate operand
+  int32_t order;
+  int32_t pad;
+};
+
+struct P2Unit {               // one CTA of the second-GEMM kernel
+  int32_t run_begin, run_end;
+  int32_t i0, rows_valid, j0, cols_valid;
+  int64_t out_off;            // partial buffer offset of element (i0, j0) of this split's m x ldp tile
+  int32_t ldo;
+  int32_t pad;
+};
+
+struct PsiBlk {               // one psi block and its padded copies
+  int64_t off;                // in psi / out (dense rows x cols)
+  int64_t p_off;              // padded copy   rows x ldp   in workspace
+  int64_t t_off;              // padded transpose cols x ldt in workspace
+  int32_t rows, cols, ldp, ldt;
+  int64_t part_off;           // split-K partials: nsplit x (rows x ldo)
+  int32_t nsplit, ldo;
+  int32_t left, right;
+  int32_t diag0, diag1;       // range in the diagonal-task table
+};
+
+struct DiagTask {             // sector-diagonal task (for diag(H))
+  int64_t a_off, b_off;
+  int32_t a_ld, b_ld;
+  double coef;
+};
+
+struct Schedule {
+  std::vector<PsiBlk> blocks;
+  std::vector<Seg> segs;
+  std::vector<Group> groups;
+  std::vector<P1Unit> p1;
+  std::vector<Run> runs;
+  std::vector<P2Unit> p2;
+  std::vector<DiagTask> diag;
+  std::vector<hpsi_task_t> tasks;     // schedule order, for hpsi_query
+  int64_t psi_len = 0;
+  int64_t ws_len = 0;                 // doubles
+  int64_t useful_flops = 0, issued_flops = 0, issued_flops_p1 = 0, operator_bytes = 0, intermediate_bytes = 0;
+  int64_t n_order1 = 0;
+  int32_t max_block_elems = 0;
+  bool aligned16 = true;              // descriptors allow the 16-byte staging path (arena base checked at bind)
+};
+
+// Host planner.  Returns HPSI_OK or an error code with `err` filled.
+int build_schedule(const hpsi_sectors_t* s, const hpsi_terms_t* t, uint32_t flags, int n_sm, Schedule* out,
+                   std::string* err);
+
+// Host interpreter of the schedule (tests only; naive loops).
+void interpret_schedule(const Schedule& sc, const double* a, const double* b, const double* psi, double* out);
+
+inline int even_up(int x) { return x + (x & 1); }
+inline int frags(int x) { return (x + 7) / 8; }
+
+}  // namespace hpsi

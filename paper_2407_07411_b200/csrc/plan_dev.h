@@ -1,0 +1,37 @@
+// The opaque hpsi_plan: host schedule + its device copy + plan-owned device buffers.
+#pragma once
+#include <cuda_runtime.h>
+
+#include <string>
+
+#include "kernels.cuh"
+#include "plan.h"
+
+struct hpsi_plan {
+  hpsi::Schedule sc;
+  bool host_only = false;
+  bool bound = false;
+  bool aligned16 = true;          // descriptors AND arena bases allow 16-byte staging
+  int n_sm = 148;
+  hpsi::DevSchedule dev{};
+  void* d_tables = nullptr;       // one allocation holding every uploaded table
+  double* d_ws = nullptr;
+  // apply_host staging
+  double* d_psi_stage = nullptr;
+  double* d_out_stage = nullptr;
+  // Davidson buffers (allocated on first use)
+  double* d_dav = nullptr;
+  size_t dav_doubles = 0;
+  int dav_mmax = 0;
+};
+
+namespace hpsi {
+void set_error(const std::string& s);
+int cuda_fail(cudaError_t e, const char* what);   // records the message, returns HPSI_ECUDA
+}  // namespace hpsi
+
+#define HPSI_CUDA(call)                                             \
+  do {                                                              \
+    cudaError_t e_ = (call);                                        \
+    if (e_ != cudaSuccess) return hpsi::cuda_fail(e_, #call);       \
+  } while (0)

@@ -1,0 +1,333 @@
+// Host planner: sector table + term list -> flat device schedule.
+//
+//  1. psi block table: left sector i pairs with the unique right sector j with q_left[i]+q_right[j]==Q*.
+//  2. task enumeration: (t, A block l<-l', B block r<-r') with (l',r') and (l,r) both psi blocks.
+//  3. order choice per task by flops: f1 = 2 m n'(k+n) for (A psi)B^T, f2 = 2 k n(n'+m) for A(psi B^T)
+//     (north_star: "orders each term as (A psi)B^T or A(psi B^T) by flop count"); tie -> order 1.
+//  4. grouping: tasks sorted by (destination block, source block, term).  A (source,destination) group shares
+//     all four dims; its first GEMMs are stacked into one tall GEMM, and all groups of one destination form
+//     the K dimension of that block's second GEMM ("groups all tasks that write one output block so accumulation
+//     stays on-chip with no global atomics").  K is cut into chunks of roughly equal DMMA count (split-K partials,
+//     reduced in a fixed order), output blocks into <=64x64 tiles with an even split in units of 8x8 fragments.
+#include <algorithm>
+#include <cstdio>
+#include <numeric>
+#include <unordered_map>
+
+#include "plan.h"
+
+namespace hpsi {
+
+namespace {
+
+struct Tile1D { int start, len; };
+
+// Even split of a dimension into tiles of at most 8 fragments (64), sizes balanced in units of 8.
+std::vector<Tile1D> split_dim(int64_t n) {
+  std::vector<Tile1D> out;
+  if (n <= 0) return out;
+  int64_t F = (n + 7) / 8;
+  int64_t nt = (F + 7) / 8;
+  int64_t base = F / nt, rem = F % nt;
+  int64_t start = 0;
+  for (int64_t i = 0; i < nt; ++i) {
+    int64_t f = base + (i < rem ? 1 : 0);
+    int64_t len = std::min<int64_t>(f * 8, n - start);
+    out.push_back({(int)start, (int)len});
+    start += f * 8;
+  }
+  return out;
+}
+
+int64_t align_up(int64_t x, int64_t a) { return (x + a - 1) / a * a; }
+
+#define FAIL(code, ...)                                   \
+  do {                                                    \
+    char buf_[512];                                       \
+    snprintf(buf_, sizeof buf_, __VA_ARGS__);             \
+    *err = buf_;                                          \
+    return code;                                          \
+  } while (0)
+
+struct RawTask {
+  int32_t term, ia, ib, src, dst;   // src/dst = psi block indices
+};
+
+}  // namespace
+
+int build_schedule(const hpsi_sectors_t* s, const hpsi_terms_t* t, uint32_t flags, int n_sm, Schedule* sc,
+                   std::string* err) {
+  if (!s || !t || !sc) FAIL(HPSI_EINVAL, "null argument");
+  const int nL = s->n_left, nR = s->n_right;
+  if (nL < 0 || nR < 0) FAIL(HPSI_EINVAL, "negative sector count");
+  if ((nL > 0 && (!s->q_left || !s->d_left)) || (nR > 0 && (!s->q_right || !s->d_right)))
+    FAIL(HPSI_EINVAL, "null sector arrays");
+  if (t->n_terms < 0 || t->n_a < 0 || t->n_b < 0) FAIL(HPSI_EINVAL, "negative term/block count");
+  if ((t->n_terms > 0 && !t->coef) || (t->n_a > 0 && !t->a_blocks) || (t->n_b > 0 && !t->b_blocks))
+    FAIL(HPSI_EINVAL, "null term arrays");
+  if ((flags & HPSI_PLAN_FIXED_ORDER1) && (flags & HPSI_PLAN_FIXED_ORDER2))
+    FAIL(HPSI_EINVAL, "both fixed-order flags set");
+
+  // ---- validation of the sector table (reading A22: labels unique per side, dims >= 1)
+  auto check_side = [&](int n, const int32_t* q, const int32_t* d, const char* side) -> int {
+    std::unordered_map<uint64_t, int> seen;
+    for (int i = 0; i < n; ++i) {
+      if (d[i] < 1) FAIL(HPSI_EINVAL, "%s sector %d has dimension %d < 1", side, i, d[i]);
+      uint64_t key = ((uint64_t)(uint32_t)q[2 * i] << 32) | (uint32_t)q[2 * i + 1];
+      if (!seen.emplace(key, i).second) FAIL(HPSI_EINVAL, "duplicate %s sector label (%d,%d)", side, q[2 * i], q[2 * i + 1]);
+    }
+    return HPSI_OK;
+  };
+  if (int rc = check_side(nL, s->q_left, s->d_left, "left")) return rc;
+  if (int rc = check_side(nR, s->q_right, s->d_right, "right")) return rc;
+
+  // ---- step 1: psi block table
+  std::unordered_map<uint64_t, int> right_by_label;
+  for (int j = 0; j < nR; ++j)
+    right_by_label[((uint64_t)(uint32_t)s->q_right[2 * j] << 32) | (uint32_t)s->q_right[2 * j + 1]] = j;
+  std::vector<int> blk_of_left(nL, -1), partner(nL, -1);
+  sc->blocks.clear();
+  int64_t off = 0;
+  for (int i = 0; i < nL; ++i) {
+    int32_t wantN = s->target[0] - s->q_left[2 * i], wantS = s->target[1] - s->q_left[2 * i + 1];
+    auto it = right_by_label.find(((uint64_t)(uint32_t)wantN << 32) | (uint32_t)wantS);
+    if (it == right_by_label.end()) continue;
+    PsiBlk b{};
+    b.left = i;
+    b.right = it->second;
+    b.rows = s->d_left[i];
+    b.cols = s->d_right[it->second];
+    b.off = off;
+    b.ldp = even_up(b.cols);
+    b.ldt = even_up(b.rows);
+    off += (int64_t)b.rows * b.cols;
+    blk_of_left[i] = (int)sc->blocks.size();
+    partner[i] = it->second;
+    sc->blocks.push_back(b);
+  }
+  sc->psi_len = off;
+  const int nB = (int)sc->blocks.size();
+
+  // ---- validation of block descriptors
+  sc->aligned16 = true;
+  auto check_blocks = [&](int64_t n, const hpsi_opblock_t* blk, const int32_t* d, int nsec, int64_t arena_len,
+                          const char* side) -> int {
+    std::unordered_map<uint64_t, int64_t> seen;
+    seen.reserve((size_t)n * 2);
+    for (int64_t i = 0; i < n; ++i) {
+      const hpsi_opblock_t& e = blk[i];
+      if (e.term < 0 || e.term >= t->n_terms) FAIL(HPSI_EINVAL, "%s block %lld: term %d out of range", side, (long long)i, e.term);
+      if (e.row < 0 || e.row >= nsec || e.col < 0 || e.col >= nsec)
+        FAIL(HPSI_EINVAL, "%s block %lld: sector index out of range", side, (long long)i);
+      if (e.ld < d[e.col]) FAIL(HPSI_EINVAL, "%s block %lld: ld %d < cols %d", side, (long long)i, e.ld, d[e.col]);
+      if (e.offset < 0) FAIL(HPSI_EINVAL, "%s block %lld: negative offset", side, (long long)i);
+      int64_t last = e.offset + (int64_t)(d[e.row] - 1) * e.ld + d[e.col];
+      if (arena_len > 0 && last > arena_len)
+        FAIL(HPSI_EINVAL, "%s block %lld: extends past the arena (%lld > %lld)", side, (long long)i, (long long)last, (long long)arena_len);
+      uint64_t key = ((uint64_t)e.term * (uint64_t)nsec + (uint64_t)e.row) * (uint64_t)nsec + (uint64_t)e.col;
+      if (!seen.emplace(key, i).second)
+        FAIL(HPSI_EINVAL, "%s: two blocks for (term %d, row %d, col %d)", side, e.term, e.row, e.col);
+    }
+    return HPSI_OK;
+  };
+  if (int rc = check_blocks(t->n_a, t->a_blocks, s->d_left, nL, t->a_len, "A")) return rc;
+  if (int rc = check_blocks(t->n_b, t->b_blocks, s->d_right, nR, t->b_len, "B")) return rc;
+
+  // ---- step 2: task enumeration
+  std::unordered_map<uint64_t, int64_t> b_index;
+  b_index.reserve((size_t)t->n_b * 2);
+  for (int64_t i = 0; i < t->n_b; ++i) {
+    const hpsi_opblock_t& e = t->b_blocks[i];
+    b_index[((uint64_t)e.term * (uint64_t)nR + (uint64_t)e.row) * (uint64_t)nR + (uint64_t)e.col] = i;
+  }
+  std::vector<RawTask> raw;
+  for (int64_t ia = 0; ia < t->n_a; ++ia) {
+    const hpsi_opblock_t& a = t->a_blocks[ia];
+    int dst = blk_of_left[a.row], src = blk_of_left[a.col];
+    if (dst < 0 || src < 0) continue;
+    uint64_t key = ((uint64_t)a.term * (uint64_t)nR + (uint64_t)partner[a.row]) * (uint64_t)nR + (uint64_t)partner[a.col];
+    auto it = b_index.find(key);
+    if (it == b_index.end()) continue;
+    raw.push_back({a.term, (int32_t)ia, (int32_t)it->second, src, dst});
+  }
+  std::stable_sort(raw.begin(), raw.end(), [](const RawTask& x, const RawTask& y) {
+    if (x.dst != y.dst) return x.dst < y.dst;
+    if (x.src != y.src) return x.src < y.src;
+    return x.term < y.term;
+  });
+
+  // ---- workspace layout part 1: padded psi and psi^T
+  int64_t ws = 0;
+  for (auto& b : sc->blocks) {
+    b.p_off = ws;
+    ws = align_up(ws + (int64_t)b.rows * b.ldp, 16);
+  }
+  for (auto& b : sc->blocks) {
+    b.t_off = ws;
+    ws = align_up(ws + (int64_t)b.cols * b.ldt, 16);
+    sc->max_block_elems = std::max<int32_t>(sc->max_block_elems, b.rows * b.cols);
+  }
+
+  // ---- steps 3+4a: order choice, groups, segs
+  sc->segs.clear(); sc->groups.clear(); sc->tasks.clear(); sc->diag.clear();
+  sc->useful_flops = sc->operator_bytes = sc->intermediate_bytes = 0;
+  sc->n_order1 = 0;
+  std::vector<std::vector<DiagTask>> diag_by_blk(nB);
+  for (size_t i = 0; i < raw.size();) {
+    size_t j = i;
+    while (j < raw.size() && raw[j].dst == raw[i].dst && raw[j].src == raw[i].src) ++j;
+    const PsiBlk& S = sc->blocks[raw[i].src];
+    const PsiBlk& D = sc->blocks[raw[i].dst];
+    const int64_t m = D.rows, n = D.cols, k = S.rows, np = S.cols;
+    const int64_t f1 = 2 * m * np * (k + n), f2 = 2 * k * n * (np + m);
+    int order = (f2 < f1) ? 2 : 1;
+    if (flags & HPSI_PLAN_FIXED_ORDER1) order = 1;
+    if (flags & HPSI_PLAN_FIXED_ORDER2) order = 2;
+    Group g{};
+    g.order = order;
+    g.tcount = (int32_t)(j - i);
+    g.seg0 = (int32_t)sc->segs.size();
+    g.src = raw[i].src;
+    g.dst = raw[i].dst;
+    if (order == 1) { g.rows = (int32_t)m; g.K1 = (int32_t)k; g.N1 = (int32_t)np; g.ldy1 = S.ldt; g.y1_off = S.t_off; }
+    else            { g.rows = (int32_t)n; g.K1 = (int32_t)np; g.N1 = (int32_t)k; g.ldy1 = S.ldp; g.y1_off = S.p_off; }
+    g.ldw = even_up(g.N1);
+    g.ws_off = ws;
+    const int64_t per_task = (int64_t)g.rows * g.ldw;
+    for (size_t q = i; q < j; ++q) {
+      const hpsi_opblock_t& a = t->a_blocks[raw[q].ia];
+      const hpsi_opblock_t& b = t->b_blocks[raw[q].ib];
+      Seg sg{};
+      if (order == 1) { sg.p1_off = a.offset; sg.p1_ld = a.ld; sg.p2_off = b.offset; sg.p2_ld = b.ld; }
+      else            { sg.p1_off = b.offset; sg.p1_ld = b.ld; sg.p2_off = a.offset; sg.p2_ld = a.ld; }
+      sg.ws_off = ws + (int64_t)(q - i) * per_task;
+      sg.coef = t->coef[raw[q].term];
+      sc->segs.push_back(sg);
+      if ((a.offset & 1) || (a.ld & 1) || (b.offset & 1) || (b.ld & 1)) sc->aligned16 = false;
+      sc->tasks.push_back({raw[q].term, raw[q].ia, raw[q].ib, S.left, D.left, order});
+      sc->useful_flops += std::min(f1, f2);
+      sc->operator_bytes += 8 * (m * k + n * np);
+      sc->intermediate_bytes += 8 * (int64_t)g.rows * g.N1;
+      if (order == 1) sc->n_order1++;
+      if (raw[q].src == raw[q].dst)
+        diag_by_blk[raw[q].dst].push_back({a.offset, b.offset, a.ld, b.ld, t->coef[raw[q].term]});
+    }
+    ws = align_up(ws + per_task * g.tcount, 16);
+    sc->groups.push_back(g);
+    i = j;
+  }
+  for (int b = 0; b < nB; ++b) {
+    sc->blocks[b].diag0 = (int32_t)sc->diag.size();
+    sc->diag.insert(sc->diag.end(), diag_by_blk[b].begin(), diag_by_blk[b].end());
+    sc->blocks[b].diag1 = (int32_t)sc->diag.size();
+  }
+
+  // ---- step 4b: P1 units (group-major, row tile, column tile fastest so that tiles sharing operator rows co-run)
+  sc->p1.clear();
+  sc->issued_flops_p1 = 0;
+  for (size_t gi = 0; gi < sc->groups.size(); ++gi) {
+    const Group& g = sc->groups[gi];
+    auto rt = split_dim((int64_t)g.tcount * g.rows);
+    auto ct = split_dim(g.N1);
+    const int64_t ks = (g.K1 + 3) / 4;
+    for (auto& r : rt)
+      for (auto& c : ct) {
+        sc->p1.push_back({(int32_t)gi, r.start, r.len, c.start, c.len, 0});
+        sc->issued_flops_p1 += (int64_t)frags(r.len) * frags(c.len) * ks * 512;
+      }
+  }
+
+  // ---- step 4c: P2 units.  K-space of destination d = all segs of all groups with dst == d, in seg order.
+  struct DstInfo { int g0 = 0, g1 = 0; int64_t ksteps = 0; int64_t nseg = 0; };
+  std::vector<DstInfo> dsts(nB);
+  {
+    size_t gi = 0;
+    for (int d = 0; d < nB; ++d) {
+      dsts[d].g0 = (int)gi;
+      while (gi < sc->groups.size() && sc->groups[gi].dst == d) {
+        dsts[d].ksteps += (int64_t)sc->groups[gi].tcount * ((sc->groups[gi].N1 + 3) / 4);
+        dsts[d].nseg += sc->groups[gi].tcount;
+        ++gi;
+      }
+      dsts[d].g1 = (int)gi;
+    }
+  }
+  int64_t total_p2_dmma = 0;
+  for (int d = 0; d < nB; ++d)
+    total_p2_dmma += (int64_t)frags(sc->blocks[d].rows) * frags(sc->blocks[d].cols) * dsts[d].ksteps;
+  const int64_t slots = (int64_t)std::max(n_sm, 1) * 4 * 8;      // 4 resident CTAs per SM, ~8 waves
+  const int64_t target = std::max<int64_t>(64 * 4 * 24, total_p2_dmma / slots);
+
+  sc->runs.clear(); sc->p2.clear();
+  std::vector<int64_t> unit_cost;
+  int64_t issued_p2 = 0;
+  for (int d = 0; d < nB; ++d) {
+    PsiBlk& D = sc->blocks[d];
+    D.ldo = even_up(D.cols);
+    D.part_off = ws;
+    D.nsplit = 0;
+    if (dsts[d].nseg == 0) continue;
+    auto rt = split_dim(D.rows);
+    auto ct = split_dim(D.cols);
+    int maxf = 0;
+    for (auto& r : rt) for (auto& c : ct) maxf = std::max(maxf, frags(r.len) * frags(c.len));
+    int64_t nsplit = (maxf * dsts[d].ksteps + target - 1) / target;
+    nsplit = std::max<int64_t>(1, std::min<int64_t>(nsplit, dsts[d].nseg));
+    // cut the seg sequence at cumulative k-step boundaries
+    std::vector<std::pair<int, int>> split_runs;   // run index range per split
+    int64_t cum = 0;
+    int gi = dsts[d].g0;
+    int ti = 0;                                    // position inside group gi
+    int realised = 0;
+    for (int64_t sp = 0; sp < nsplit; ++sp) {
+      const int64_t want = dsts[d].ksteps * (sp + 1) / nsplit;
+      int run0 = (int)sc->runs.size();
+      int64_t chunk_ksteps = 0;
+      while (gi < dsts[d].g1 && (cum < want || sp == nsplit - 1)) {
+        const Group& g = sc->groups[gi];
+        const int64_t per = (g.N1 + 3) / 4;
+        int take;
+        if (sp == nsplit - 1) take = g.tcount - ti;
+        else take = (int)std::min<int64_t>(g.tcount - ti, std::max<int64_t>(1, (want - cum + per - 1) / per));
+        if (take > 0) {
+          sc->runs.push_back({g.seg0 + ti, g.seg0 + ti + take, g.N1, g.ldw, g.order, 0});
+          cum += per * take;
+          chunk_ksteps += per * take;
+          ti += take;
+        }
+        if (ti >= g.tcount) { ++gi; ti = 0; }
+      }
+      int run1 = (int)sc->runs.size();
+      if (run1 == run0) continue;                  // empty chunk (rounding): skip
+      for (auto& r : rt)
+        for (auto& c : ct) {
+          P2Unit u{};
+          u.run_begin = run0; u.run_end = run1;
+          u.i0 = r.start; u.rows_valid = r.len; u.j0 = c.start; u.cols_valid = c.len;
+          u.ldo = D.ldo;
+          u.out_off = ws + (int64_t)realised * D.rows * D.ldo + (int64_t)r.start * D.ldo + c.start;
+          sc->p2.push_back(u);
+          int64_t cost = (int64_t)frags(r.len) * frags(c.len) * chunk_ksteps;
+          unit_cost.push_back(cost);
+          issued_p2 += cost * 512;
+        }
+      ++realised;
+    }
+    D.nsplit = realised;
+    ws = align_up(ws + (int64_t)realised * D.rows * D.ldo, 16);
+  }
+  // LPT order (stable: tiles of one (block, split) stay adjacent and share their operands in L2)
+  {
+    std::vector<int> idx(sc->p2.size());
+    std::iota(idx.begin(), idx.end(), 0);
+    std::stable_sort(idx.begin(), idx.end(), [&](int a, int b) { return unit_cost[a] > unit_cost[b]; });
+    std::vector<P2Unit> sorted(sc->p2.size());
+    for (size_t i = 0; i < idx.size(); ++i) sorted[i] = sc->p2[idx[i]];
+    sc->p2.swap(sorted);
+  }
+  sc->issued_flops = sc->issued_flops_p1 + issued_p2;
+  sc->ws_len = std::max<int64_t>(ws, 16);
+  return HPSI_OK;
+}
+
+}  // namespace hpsi
