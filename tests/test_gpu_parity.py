@@ -1,0 +1,195 @@
+"""GPU parity: hpsi_apply / hpsi_diagonal / hpsi_davidson through the C ABI versus the CPU oracle, element by element
+on the same seeded inputs.  Bar (BASELINE.json north_star): relative L2 error <= 1e-12 in FP64."""
+import numpy as np
+import pytest
+
+import oracle
+import workloads
+from workloads.hubbard import hubbard_two_block_problem
+from gpu_util import GpuProblem, rel_l2
+from test_oracle_pins import random_custom
+
+pytestmark = pytest.mark.gpu
+TOL = 1e-12      # north_star: "relative L2 error <= 1e-12 in FP64"
+
+
+@pytest.fixture(scope="module")
+def H():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    import paper_2407_07411_b200 as H
+    return H
+
+
+@pytest.mark.parametrize("flags_name", ["min_flops", "order1", "order2"])
+def test_toy_parity(H, toy, flags_name):
+    flags = {"min_flops": 0, "order1": H.HPSI_PLAN_FIXED_ORDER1, "order2": H.HPSI_PLAN_FIXED_ORDER2}[flags_name]
+    g = GpuProblem(toy, flags)
+    for k in range(3):
+        psi = workloads.make_psi(toy, k)
+        assert rel_l2(g.apply(psi), oracle.apply(toy, psi)) <= TOL
+
+
+@pytest.mark.parametrize("flags_name", ["min_flops", "order1", "order2"])
+def test_small_parity(H, small, flags_name):
+    flags = {"min_flops": 0, "order1": H.HPSI_PLAN_FIXED_ORDER1, "order2": H.HPSI_PLAN_FIXED_ORDER2}[flags_name]
+    g = GpuProblem(small, flags)
+    psi = workloads.make_psi(small)
+    ref = oracle.apply(small, psi)
+    got = g.apply(psi)
+    assert rel_l2(got, ref) <= TOL
+    # worst block, as a diagnostic with the same bar
+    for (i, j, r, c, off) in small.psi_blocks():
+        assert np.linalg.norm(got[off:off + r * c] - ref[off:off + r * c]) <= 1e-11 * np.linalg.norm(ref)
+
+
+def test_small_unaligned_staging(H):
+    """Dense (odd) leading dimensions and an 8-byte-aligned arena: the 8-byte cp.async variant of the kernels."""
+    p = workloads.make_problem("small", pad_even=False, n_terms=60)
+    g = GpuProblem(p, misalign=True)
+    assert g.q(H.HPSI_Q_ALIGNED16) == 0
+    psi = workloads.make_psi(p)
+    assert rel_l2(g.apply(psi), oracle.apply(p, psi)) <= TOL
+    g2 = GpuProblem(workloads.make_problem("small", pad_even=True, n_terms=60), misalign=True)
+    assert g2.q(H.HPSI_Q_ALIGNED16) == 0
+    assert rel_l2(g2.apply(psi), oracle.apply(g2.p, psi)) <= TOL
+
+
+@pytest.mark.parametrize("seed", range(8))
+def test_irregular_parity(H, seed):
+    p = random_custom(seed, grid=(seed < 4))
+    g = GpuProblem(p)
+    psi = np.random.default_rng(seed).standard_normal(p.psi_len)
+    ref = oracle.apply(p, psi)
+    assert np.linalg.norm(g.apply(psi) - ref) <= TOL * max(np.linalg.norm(ref), 1.0)
+
+
+def test_multi_tile_ragged_split_k(H):
+    """Output blocks spanning several 64x64 tiles with ragged tails (150x131, 70x9) and split-K partials."""
+    rng = np.random.default_rng(5)
+    dL, dR = [150, 70], [131, 9]
+    terms = []
+    for _ in range(40):
+        ab = {(r, c): rng.standard_normal((dL[r], dL[c])) for r in range(2) for c in range(2)}
+        bb = {(r, c): rng.standard_normal((dR[r], dR[c])) for r in range(2) for c in range(2)}
+        terms.append((float(rng.standard_normal()), ab, bb))
+    p = workloads.custom_problem([(0, 0), (1, 1)], dL, [(3, 1), (2, 0)], dR, (3, 1), terms, pad_even=True)
+    g = GpuProblem(p)
+    psi = rng.standard_normal(p.psi_len)
+    assert rel_l2(g.apply(psi), oracle.apply(p, psi)) <= TOL
+
+
+def test_single_block_equals_blas(H):
+    """n_L = n_R = 1, one term, c = 1: the result is A @ psi @ B.T (LAPACK/BLAS DGEMM)."""
+    rng = np.random.default_rng(11)
+    A, B = rng.standard_normal((77, 77)), rng.standard_normal((45, 45))
+    p = workloads.custom_problem([(1, 0)], [77], [(2, 0)], [45], (3, 0), [(1.0, {(0, 0): A}, {(0, 0): B})])
+    psi = rng.standard_normal(77 * 45)
+    ref = (A @ psi.reshape(77, 45) @ B.T).ravel()
+    assert rel_l2(GpuProblem(p).apply(psi), ref) <= TOL
+
+
+def test_empty_cases(H):
+    import torch
+    p = workloads.make_problem("toy", n_terms=0)
+    g = GpuProblem(p)
+    assert np.all(g.apply(workloads.make_psi(p)) == 0.0)            # overwrite semantics: zeros, not the NaN prefill
+    # a destination block that no task writes is zero-filled
+    q = workloads.custom_problem([(0, 0), (1, 0)], [3, 2], [(1, 0), (0, 0)], [2, 4], (1, 0),
+                                 [(2.0, {(0, 0): np.ones((3, 3))}, {(0, 0): np.ones((2, 2))})])
+    g = GpuProblem(q)
+    psi = np.arange(1.0, 1.0 + q.psi_len)
+    ref = oracle.apply(q, psi)
+    out = g.apply(psi)
+    assert rel_l2(out, ref) <= TOL and np.all(out[6:] == 0.0)
+    with pytest.raises(H.HpsiError):
+        x = torch.zeros(q.psi_len, dtype=torch.float64, device="cuda")
+        H.hpsi_apply(g.plan, x, x)                                    # aliasing is rejected
+
+
+def test_bitwise_determinism(H, small):
+    g = GpuProblem(small)
+    psi = workloads.make_psi(small, 1)
+    a, b = g.apply(psi), g.apply(psi)
+    assert np.array_equal(a, b)
+    assert np.array_equal(a, GpuProblem(small).apply(psi))           # a fresh plan gives the same bits
+
+
+def test_apply_host_and_graph_capture(H, small):
+    import torch
+    g = GpuProblem(small)
+    psi = workloads.make_psi(small, 2)
+    ref = g.apply(psi)
+    out = np.empty_like(psi)
+    H.hpsi_apply_host(g.plan, psi, out, torch.cuda.current_stream())
+    assert np.array_equal(out, ref)
+    # hpsi_apply only enqueues: it can be captured into a CUDA graph and replayed
+    x = torch.from_numpy(psi).cuda()
+    y = torch.zeros_like(x)
+    s = torch.cuda.Stream()
+    with torch.cuda.stream(s):
+        H.hpsi_apply(g.plan, x, y, s)
+        s.synchronize()
+        graph = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(graph, stream=s):
+            H.hpsi_apply(g.plan, x, y, s)
+        y.zero_()
+        graph.replay()
+        s.synchronize()
+    assert np.array_equal(y.cpu().numpy(), ref)
+
+
+def test_hermiticity_on_gpu(H, small):
+    g = GpuProblem(small)
+    rng = np.random.default_rng(3)
+    x, y = rng.standard_normal(small.psi_len), rng.standard_normal(small.psi_len)
+    Hx, Hy = g.apply(x), g.apply(y)
+    assert abs(x @ Hy - Hx @ y) <= 1e-12 * np.linalg.norm(x) * np.linalg.norm(Hy)
+
+
+def test_diagonal(H, toy):
+    import torch
+    g = GpuProblem(toy)
+    d = torch.empty(g.n, dtype=torch.float64, device="cuda")
+    H.hpsi_diagonal(g.plan, d)
+    torch.cuda.synchronize()
+    ref = oracle.diagonal(toy)
+    assert np.linalg.norm(d.cpu().numpy() - ref) <= 1e-13 * max(np.linalg.norm(ref), 1.0)
+    assert np.allclose(ref, np.diag(oracle.dense_hamiltonian(toy)), atol=1e-13)
+
+
+def _davidson(H, g, v0, **kw):
+    import torch
+    x = torch.from_numpy(np.ascontiguousarray(v0)).cuda()
+    theta, info = H.hpsi_davidson(g.plan, x, **kw)
+    return theta, x.cpu().numpy(), info
+
+
+def test_davidson_toy_vs_dense(H, toy):
+    g = GpuProblem(toy)
+    ev = np.linalg.eigvalsh(oracle.dense_hamiltonian(toy))
+    theta, x, info = _davidson(H, g, workloads.make_psi(toy), tol=1e-9, max_iter=400)
+    assert info["converged"] and abs(theta - ev[0]) <= 1e-10
+    assert np.linalg.norm(oracle.apply(toy, x) - theta * x) <= 1e-8
+    th_o, _, nmv_o, _ = oracle.davidson(toy, workloads.make_psi(toy), tol=1e-9, max_iter=400)
+    assert abs(theta - th_o) <= 1e-10
+    theta2, _, info2 = _davidson(H, g, workloads.make_psi(toy), tol=1e-9, max_iter=400, precondition=False, m_max=8)
+    assert info2["converged"] and abs(theta2 - ev[0]) <= 1e-10
+
+
+def test_davidson_hubbard_closed_forms(H):
+    """Textbook pins (tests/golden/hubbard_closed_forms.txt): dimer (U - sqrt(U^2+16t^2))/2, 4-site chain -2 sqrt(5) t."""
+    dimer = hubbard_two_block_problem(1, 1, 1.0, 3.7, 2, 0)
+    theta, _, info = _davidson(H, GpuProblem(dimer), np.ones(dimer.psi_len), tol=1e-10)
+    assert info["converged"] and abs(theta - (3.7 - np.sqrt(3.7 ** 2 + 16.0)) / 2) <= 1e-10
+    chain = hubbard_two_block_problem(2, 2, 1.0, 0.0, 4, 0)
+    v0 = np.random.default_rng(0).standard_normal(chain.psi_len)
+    theta, _, info = _davidson(H, GpuProblem(chain), v0, tol=1e-10, precondition=False)
+    assert info["converged"] and abs(theta + 2 * np.sqrt(5.0)) <= 1e-9
+
+
+def test_davidson_small(H, small):
+    g = GpuProblem(small)
+    theta, x, info = _davidson(H, g, workloads.make_psi(small), tol=1e-7, max_iter=300)
+    assert info["converged"]
+    assert np.linalg.norm(oracle.apply(small, x) - theta * x) <= 1e-6

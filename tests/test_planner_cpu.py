@@ -1,0 +1,192 @@
+"""CPU-only tests of the product's host side: the C-ABI library loads and exports every declared symbol, the planner
+validates its input, and the *device schedule* (executed by hpsi_debug_interpret with naive loops) reproduces the
+oracle.  No CUDA call is made here (plans are HPSI_PLAN_HOST_ONLY)."""
+import ctypes
+import os
+import re
+
+import numpy as np
+import pytest
+
+import oracle
+import workloads
+import paper_2407_07411_b200 as H
+from test_oracle_pins import random_custom
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def host_plan(p, flags=0):
+    return H.plan_problem(p, flags=H.HPSI_PLAN_HOST_ONLY | flags)
+
+
+def rel(x, ref):
+    return np.linalg.norm(x - ref) / max(np.linalg.norm(ref), 1e-300)
+
+
+# ------------------------------------------------------------------------------------------------ ABI
+def test_library_exports_every_declared_symbol():
+    hdr = open(os.path.join(ROOT, "include", "hpsi.h")).read()
+    hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
+    names = set(re.findall(r"\b(hpsi_[a-z0-9_]+)\s*\(", hdr))
+    assert {"hpsi_plan", "hpsi_apply", "hpsi_apply_host", "hpsi_bind", "hpsi_davidson", "hpsi_query", "hpsi_destroy",
+            "hpsi_last_error", "hpsi_diagonal", "hpsi_debug_interpret", "hpsi_bench_fp64_pipe"} <= names
+    L = H.lib()
+    for n in names:
+        assert hasattr(L, n), n
+
+
+def test_opblock_layout_matches_header():
+    assert workloads.OPBLOCK_DTYPE.itemsize == 24
+    assert [workloads.OPBLOCK_DTYPE.fields[k][1] for k in ("term", "row", "col", "ld", "offset")] == [0, 4, 8, 12, 16]
+
+
+def test_no_cpu_fallback(toy):
+    """Compute entry points refuse to run without a device plan (no CPU fallback exists)."""
+    plan = host_plan(toy)
+    x = np.zeros(H.hpsi_query(plan, H.HPSI_Q_PSI_LENGTH))
+    with pytest.raises(H.HpsiError) as e:
+        H.hpsi_apply(plan, x.ctypes.data, x.ctypes.data + 8, None)
+    assert e.value.code == H.HPSI_ESTATE
+    with pytest.raises(H.HpsiError):
+        H.hpsi_apply_host(plan, x, x.copy(), None)
+
+
+# ------------------------------------------------------------------------------------------ psi table
+def test_psi_blocks_match_oracle_table(toy, small):
+    for p in (toy, small, random_custom(3), random_custom(6, grid=False)):
+        plan = host_plan(p)
+        blocks = H.hpsi_query(plan, H.HPSI_Q_PSI_BLOCKS)
+        partner, offset, n = oracle.psi_table(p)
+        assert H.hpsi_query(plan, H.HPSI_Q_PSI_LENGTH) == n
+        want = [(i, int(partner[i]), int(p.d_left[i]), int(p.d_right[partner[i]]), int(offset[i]))
+                for i in range(len(partner)) if partner[i] >= 0]
+        got = [(int(b["left"]), int(b["right"]), int(b["rows"]), int(b["cols"]), int(b["offset"])) for b in blocks]
+        assert got == want
+
+
+# ------------------------------------------------------------------------- schedule == oracle (CPU)
+@pytest.mark.parametrize("flags", [0, H.HPSI_PLAN_FIXED_ORDER1, H.HPSI_PLAN_FIXED_ORDER2])
+def test_schedule_interpreter_toy(toy, flags):
+    plan = host_plan(toy, flags)
+    for k in range(2):
+        psi = workloads.make_psi(toy, k)
+        assert rel(H.hpsi_debug_interpret(plan, toy.a_data, toy.b_data, psi), oracle.apply(toy, psi)) <= 1e-13
+
+
+def test_schedule_interpreter_small(small):
+    plan = host_plan(small)
+    psi = workloads.make_psi(small)
+    assert rel(H.hpsi_debug_interpret(plan, small.a_data, small.b_data, psi), oracle.apply(small, psi)) <= 1e-13
+
+
+@pytest.mark.parametrize("seed", range(8))
+def test_schedule_interpreter_irregular(seed):
+    """Partner-less sectors, non-shift block patterns, dense (odd) and padded leading dimensions."""
+    p = random_custom(seed, grid=(seed < 4))
+    plan = host_plan(p)
+    psi = np.random.default_rng(seed).standard_normal(p.psi_len)
+    ref = oracle.apply(p, psi)
+    got = H.hpsi_debug_interpret(plan, p.a_data, p.b_data, psi)
+    assert np.linalg.norm(got - ref) <= 1e-13 * max(np.linalg.norm(ref), 1.0)
+    assert H.hpsi_query(plan, H.HPSI_Q_ALIGNED16) == (1 if seed % 2 else 0) or p.a_desc.size == 0
+
+
+def test_schedule_split_k_and_multi_tile():
+    """A problem whose output block spans several 64x64 tiles with a ragged tail and whose K is split."""
+    rng = np.random.default_rng(5)
+    dL, dR = [150, 70], [131, 9]
+    qL, qR = [(0, 0), (1, 1)], [(3, 1), (2, 0)]
+    terms = []
+    for _ in range(40):
+        ab = {(r, c): rng.standard_normal((dL[r], dL[c])) for r in range(2) for c in range(2)}
+        bb = {(r, c): rng.standard_normal((dR[r], dR[c])) for r in range(2) for c in range(2)}
+        terms.append((float(rng.standard_normal()), ab, bb))
+    p = workloads.custom_problem(qL, dL, qR, dR, (3, 1), terms, pad_even=True)
+    plan = host_plan(p)
+    assert H.hpsi_query(plan, H.HPSI_Q_N_P2_UNITS) > 6
+    psi = rng.standard_normal(p.psi_len)
+    assert rel(H.hpsi_debug_interpret(plan, p.a_data, p.b_data, psi), oracle.apply(p, psi)) <= 1e-13
+
+
+# ---------------------------------------------------------------------------------- counts and flops
+def test_flop_and_task_counts(toy, small):
+    for p in (toy, small):
+        plan = host_plan(p)
+        flops, ntask = oracle.useful_flops(p)
+        assert H.hpsi_query(plan, H.HPSI_Q_N_TASKS) == ntask
+        assert H.hpsi_query(plan, H.HPSI_Q_USEFUL_FLOPS) == flops
+        assert H.hpsi_query(plan, H.HPSI_Q_ISSUED_FLOPS) >= flops
+        assert H.hpsi_query(plan, H.HPSI_Q_OPERATOR_BYTES) <= p.operator_bytes()
+        tasks = H.hpsi_query(plan, H.HPSI_Q_TASKS)
+        assert len(tasks) == ntask and set(np.unique(tasks["order"])) <= {1, 2}
+
+
+def test_order_choice_is_min_flops(small):
+    """Per task the planner picks min(2mn'(k+n), 2kn(n'+m)); forcing either order can only cost more DMMA work."""
+    free = H.hpsi_query(host_plan(small), H.HPSI_Q_USEFUL_FLOPS)
+    plan = host_plan(small)
+    partner = small.partner
+    for t in H.hpsi_query(plan, H.HPSI_Q_TASKS):
+        l, lp = int(t["dst_left"]), int(t["src_left"])
+        m, k = int(small.d_left[l]), int(small.d_left[lp])
+        n, n1 = int(small.d_right[partner[l]]), int(small.d_right[partner[lp]])
+        f1, f2 = 2 * m * n1 * (k + n), 2 * k * n * (n1 + m)
+        assert int(t["order"]) == (2 if f2 < f1 else 1)
+    assert free == oracle.useful_flops(small)[0]
+
+
+def test_useful_flops_scale_as_D_cubed():
+    """PAPER.md:62 / :82 - cost O(D^3): doubling every sector dim multiplies the useful flops by exactly 8."""
+    base = workloads.make_problem("toy", fill=False)
+    dbl = workloads.make_problem("toy", fill=False)
+    dbl.d_left = (2 * base.d_left).astype(np.int32)
+    dbl.d_right = (2 * base.d_right).astype(np.int32)
+    dbl.a_desc = dbl.a_desc.copy(); dbl.b_desc = dbl.b_desc.copy()
+    dbl.a_desc["ld"] *= 2; dbl.b_desc["ld"] *= 2
+    dbl.a_desc["offset"] *= 4; dbl.b_desc["offset"] *= 4
+    dbl.a_len *= 4; dbl.b_len *= 4
+    f1 = H.hpsi_query(host_plan(base), H.HPSI_Q_USEFUL_FLOPS)
+    f2 = H.hpsi_query(host_plan(dbl), H.HPSI_Q_USEFUL_FLOPS)
+    assert f2 == 8 * f1
+
+
+# ----------------------------------------------------------------------------------------- validation
+def _expect_einval(p, match):
+    with pytest.raises(H.HpsiError) as e:
+        host_plan(p)
+    assert e.value.code == H.HPSI_EINVAL and match in str(e.value)
+
+
+def test_validation_errors():
+    p = workloads.make_problem("toy")
+    bad = workloads.make_problem("toy"); bad.q_left = bad.q_left.copy(); bad.q_left[1] = bad.q_left[0]
+    _expect_einval(bad, "duplicate")
+    bad = workloads.make_problem("toy"); bad.d_right = bad.d_right.copy(); bad.d_right[2] = 0
+    _expect_einval(bad, "dimension")
+    bad = workloads.make_problem("toy"); bad.a_desc = bad.a_desc.copy(); bad.a_desc["ld"][0] = 0
+    _expect_einval(bad, "ld")
+    bad = workloads.make_problem("toy"); bad.b_desc = bad.b_desc.copy(); bad.b_desc["offset"][-1] = bad.b_len
+    _expect_einval(bad, "arena")
+    bad = workloads.make_problem("toy"); bad.a_desc = np.concatenate([bad.a_desc, bad.a_desc[:1]])
+    _expect_einval(bad, "two blocks")
+    bad = workloads.make_problem("toy"); bad.a_desc = bad.a_desc.copy(); bad.a_desc["term"][0] = p.n_terms
+    _expect_einval(bad, "term")
+
+
+def test_empty_problems():
+    """No terms / no psi blocks are legal: the schedule is empty and the result is zeros."""
+    p = workloads.make_problem("toy", n_terms=0)
+    plan = host_plan(p)
+    assert H.hpsi_query(plan, H.HPSI_Q_N_TASKS) == 0
+    out = H.hpsi_debug_interpret(plan, p.a_data, p.b_data, workloads.make_psi(p))
+    assert np.all(out == 0.0)
+    q = workloads.custom_problem([(0, 0)], [2], [(5, 5)], [3], (1, 1), [(1.0, {(0, 0): np.eye(2)}, {(0, 0): np.eye(3)})])
+    plan = host_plan(q)
+    assert H.hpsi_query(plan, H.HPSI_Q_PSI_LENGTH) == 0 and H.hpsi_query(plan, H.HPSI_Q_N_TASKS) == 0
+
+
+def test_struct_sizes():
+    assert ctypes.sizeof(H.binding.hpsi_sectors_t) == 48
+    assert ctypes.sizeof(H.binding.hpsi_terms_t) == 80
+    assert H.binding.PSI_BLOCK_DTYPE.itemsize == 24 and H.binding.TASK_DTYPE.itemsize == 24
