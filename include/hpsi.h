@@ -161,7 +161,7 @@ const char* hpsi_last_error(void);
 /* FP64 tensor-pipe microbenchmarks used by bench.py's calibration: run `iters`
  * dependent-chain rounds of register-resident DMMA.8x8x4 (kind 0), DFMA (kind 1) or both interleaved (kind 2)
  * on every SM (4 CTAs of 8 warps per SM) and return the elapsed milliseconds and the flops executed; kind 100+w runs
- * the DMMA probe with one CTA of w warps (1..32) per SM (occupancy sensitivity of the pipe).  HOST outputs. */
+ * the DMMA probe with w one-warp CTAs (1..32) per SM (occupancy sensitivity of the pipe).  HOST outputs. */
 int hpsi_bench_fp64_pipe(int kind, int iters, double* ms_out, double* flops_out);
 
 /* ---- debug / test entry points (HOST memory only; run the *device schedule* with naive loops on the CPU) ----

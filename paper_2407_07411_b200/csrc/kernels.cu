@@ -1,5 +1,14 @@
 // sm_100a kernels of hpsi_apply: prep (padded psi, psi^T), P1 (stacked first GEMM), P2 (segmented-K second GEMM
 // with split-K partials), reduce (ordered sum of partials), diag.  See kernels.cuh / plan.h for the vocabulary.
+//
+// GEMM CTA = 1 producer warp + 4 consumer warps (warp-specialised, mbarrier ring of NSTAGE stages):
+//   producer : cp.async (LDGSTS, zero-fill for ragged edges) of a 64 x 16 X tile and a 64 x 16 Y tile per stage,
+//              completion signalled with cp.async.mbarrier.arrive on the stage's "full" barrier;
+//   consumers: 2x2 warps, each <= 4x4 fragments of DMMA.8x8x4 with register accumulators; a warp waits only on the
+//              "full" barrier of its next stage and releases the stage on its "empty" barrier - no CTA-wide barrier
+//              in the main loop.  Measured on B200: one warp issues a DMMA.8x8x4 at most every ~29 clk while the
+//              pipe takes one per 16 clk per SM sub-partition, so >= 2 warps per sub-partition must always be in
+//              their DMMA phase; decoupling the warps is what keeps them there.
 #include "kernels.cuh"
 
 namespace hpsi {
@@ -11,9 +20,30 @@ __device__ __forceinline__ void cp_async_chunk16(uint32_t dst, const void* src, 
 __device__ __forceinline__ void cp_async_chunk8(uint32_t dst, const void* src, int bytes) {
   asm volatile("cp.async.ca.shared.global [%0], [%1], 8, %2;\n" ::"r"(dst), "l"(src), "r"(bytes) : "memory");
 }
-__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::: "memory"); }
-template <int N>
-__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N) : "memory"); }
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;\n" ::: "memory"); }
+
+__device__ __forceinline__ void mbar_init(uint32_t bar, int count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;\n" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+  asm volatile("{\n .reg .b64 st;\n mbarrier.arrive.shared::cta.b64 st, [%0];\n}\n" ::"r"(bar) : "memory");
+}
+// arrive on `bar` once all cp.async issued so far by this thread have landed (does not change the pending count)
+__device__ __forceinline__ void cp_async_mbar_arrive(uint32_t bar) {
+  asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];\n" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ bool mbar_try_wait(uint32_t bar, uint32_t parity) {
+  uint32_t ok;
+  asm volatile(
+      "{\n .reg .pred p;\n mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n selp.u32 %0, 1, 0, p;\n}\n"
+      : "=r"(ok)
+      : "r"(bar), "r"(parity)
+      : "memory");
+  return ok != 0;
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+  while (!mbar_try_wait(bar, parity)) {}
+}
 
 // D(8x8) += A(8x4,row) * B(4x8,col): lane L, g=L>>2, q=L&3 holds a=A[g][q], b=B[q][g], c0,c1=C[g][2q],C[g][2q+1].
 __device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double b) {
@@ -26,20 +56,21 @@ __device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double
 // Stage layout per operand: [k-slab (4)][row (64)][4 doubles]; element (row, kc) at ((kc>>2)*64 + row)*4 + (kc&3).
 // A warp's fragment read (row = r0+g, kc = 4*ks+q) is then 32 consecutive doubles: conflict-free.
 // CH = doubles per cp.async (2: 16-byte chunks, needs 16-byte aligned rows; 1: 8-byte chunks, any FP64 alignment).
+// The producer warp's lane handles chunk column (lane % CPR) of rows (lane / CPR) + p * RPP.
 template <int CH>
 struct Stager {
   static constexpr int CPR = KT / CH;            // chunks per row
-  static constexpr int RPP = NTHREADS / CPR;     // rows per pass
+  static constexpr int RPP = 32 / CPR;           // rows per pass of the producer warp
   static constexpr int PASSES = TILE / RPP;
   int r0, kc;
   uint32_t dst0;                                 // byte offset inside an operand's stage
-  __device__ __forceinline__ Stager(int tid) {
-    const int c = tid % CPR;
-    r0 = tid / CPR;
+  __device__ __forceinline__ Stager(int lane) {
+    const int c = lane % CPR;
+    r0 = lane / CPR;
     kc = c * CH;
     dst0 = (uint32_t)((((kc >> 2) * TILE + r0) * 4 + (kc & 3)) * 8);
   }
-  // rows r0 + p*RPP of the operand; rowptr(p) = pointer to (row, k=0) of that row in global memory
+  // rowptr(p) = pointer to (row r0 + p*RPP, k = 0) in global memory; rows >= rows_valid and k >= K are zero-filled
   template <class RowPtr>
   __device__ __forceinline__ void load(uint32_t s_op, RowPtr rowptr, int rows_valid, const double* safe, int kappa,
                                        int K) const {
@@ -72,34 +103,35 @@ struct WarpTile {
   }
 };
 
-__device__ __forceinline__ void mma_stage(const double* sx, const double* sy, double (&acc)[4][4][2], int nk4,
-                                          const WarpTile& w, int lane) {
-  const double* px = sx + w.wr0 * 4 + lane;
-  const double* py = sy + w.wc0 * 4 + lane;
-  if (w.mi == 4 && w.nj == 4) {
-#pragma unroll 1
-    for (int ks = 0; ks < nk4; ++ks) {
-      double a[4], b[4];
+// One staged K-tile for a warp owning MI x NJ fragments (compile-time, so no predicated DMMA and no WARPSYNC):
+// nk4 k-steps of MI*NJ DMMA.8x8x4; the fragments of step ks+1 are fetched while step ks issues.
+template <int MI, int NJ>
+__device__ __forceinline__ void mma_stage(const double* px, const double* py, double (&acc)[4][4][2], int nk4) {
+  double a[MI], b[NJ];
 #pragma unroll
-      for (int i = 0; i < 4; ++i) { a[i] = px[ks * TILE * 4 + i * 32]; b[i] = py[ks * TILE * 4 + i * 32]; }
+  for (int i = 0; i < MI; ++i) a[i] = px[i * 32];
 #pragma unroll
-      for (int i = 0; i < 4; ++i)
+  for (int j = 0; j < NJ; ++j) b[j] = py[j * 32];
 #pragma unroll
-        for (int j = 0; j < 4; ++j) dmma884(acc[i][j][0], acc[i][j][1], a[i], b[j]);
-    }
-  } else {
-#pragma unroll 1
-    for (int ks = 0; ks < nk4; ++ks) {
-      double a[4], b[4];
+  for (int ks = 0; ks < 4; ++ks) {
+    if (ks < nk4) {
+      double an[MI], bn[NJ];
+      if (ks + 1 < 4) {
 #pragma unroll
-      for (int i = 0; i < 4; ++i) { a[i] = px[ks * TILE * 4 + i * 32]; b[i] = py[ks * TILE * 4 + i * 32]; }
+        for (int i = 0; i < MI; ++i) an[i] = px[(ks + 1) * TILE * 4 + i * 32];
 #pragma unroll
-      for (int i = 0; i < 4; ++i)
-        if (i < w.mi) {
+        for (int j = 0; j < NJ; ++j) bn[j] = py[(ks + 1) * TILE * 4 + j * 32];
+      }
 #pragma unroll
-          for (int j = 0; j < 4; ++j)
-            if (j < w.nj) dmma884(acc[i][j][0], acc[i][j][1], a[i], b[j]);
-        }
+      for (int i = 0; i < MI; ++i)
+#pragma unroll
+        for (int j = 0; j < NJ; ++j) dmma884(acc[i][j][0], acc[i][j][1], a[i], b[j]);
+      if (ks + 1 < 4) {
+#pragma unroll
+        for (int i = 0; i < MI; ++i) a[i] = an[i];
+#pragma unroll
+        for (int j = 0; j < NJ; ++j) b[j] = bn[j];
+      }
     }
   }
 }
@@ -131,68 +163,119 @@ __device__ __forceinline__ void store_tile(double* dst, int ld, int rows_valid, 
   }
 }
 
+// Shared-memory carve-up: NSTAGE stages of [X tile | Y tile], then the barriers and (P1) the row-pointer table.
+struct SmemLayout {
+  uint32_t base;                                   // shared-window address of stage 0
+  __device__ __forceinline__ uint32_t stage(int s) const { return base + s * STAGE_DOUBLES * 8; }
+  __device__ __forceinline__ uint32_t full(int s) const { return base + NSTAGE * STAGE_DOUBLES * 8 + s * 8; }
+  __device__ __forceinline__ uint32_t empty(int s) const { return base + NSTAGE * STAGE_DOUBLES * 8 + (NSTAGE + s) * 8; }
+};
+__device__ __forceinline__ void init_barriers(const SmemLayout& sm, int tid) {
+  if (tid == 0) {
+    for (int s = 0; s < NSTAGE; ++s) { mbar_init(sm.full(s), 32); mbar_init(sm.empty(s), NCONS); }
+    asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
+  }
+  __syncthreads();
+}
+
+
+// Consumer main loop for a warp owning MI x NJ fragments.  seq.next() returns the number of k-steps (1..4) of the
+// next staged K-tile, or 0 when the unit is done.  Idle warps (MI == 0) only hand the stages back.
+template <int MI, int NJ, class Seq>
+__device__ __forceinline__ void consume(const double* smem, const SmemLayout& sm, Seq& seq, double (&acc)[4][4][2],
+                                        const WarpTile& w, int lane) {
+  int stage = 0;
+  uint32_t phase = 0;
+  const int xoff = w.wr0 * 4 + lane, yoff = 4 * TILE * 4 + w.wc0 * 4 + lane;
+  for (int nk4 = seq.next(); nk4 > 0; nk4 = seq.next()) {
+    mbar_wait(sm.full(stage), phase);
+    if (MI > 0) {
+      const double* st = smem + stage * STAGE_DOUBLES;
+      mma_stage<(MI > 0 ? MI : 1), (NJ > 0 ? NJ : 1)>(st + xoff, st + yoff, acc, nk4);
+    }
+    __syncwarp();
+    if (lane == 0) mbar_arrive(sm.empty(stage));
+    if (++stage == NSTAGE) { stage = 0; phase ^= 1; }
+  }
+}
+
+template <class Seq>
+__device__ __forceinline__ void consume_dispatch(const double* smem, const SmemLayout& sm, Seq& seq,
+                                                 double (&acc)[4][4][2], const WarpTile& w, int lane) {
+#define HPSI_CASE(MI, NJ) case MI * 5 + NJ: consume<MI, NJ>(smem, sm, seq, acc, w, lane); break;
+  switch ((w.nj > 0 ? w.mi : 0) * 5 + (w.mi > 0 ? w.nj : 0)) {
+    HPSI_CASE(1, 1) HPSI_CASE(1, 2) HPSI_CASE(1, 3) HPSI_CASE(1, 4)
+    HPSI_CASE(2, 1) HPSI_CASE(2, 2) HPSI_CASE(2, 3) HPSI_CASE(2, 4)
+    HPSI_CASE(3, 1) HPSI_CASE(3, 2) HPSI_CASE(3, 3) HPSI_CASE(3, 4)
+    HPSI_CASE(4, 1) HPSI_CASE(4, 2) HPSI_CASE(4, 3) HPSI_CASE(4, 4)
+    default: consume<0, 0>(smem, sm, seq, acc, w, lane); break;
+  }
+#undef HPSI_CASE
+}
+
 // ------------------------------------------------------------------------------------------------ P1 kernel
 // One CTA = one P1Unit: C[R0.., j0..] = coef(row) * sum_k X[R,k] Y[j,k], X rows stacked over the group's terms
 // (order 1: A_t rows; order 2: B_t rows), Y = padded psi^T (order 1) or padded psi (order 2) block of the source.
 template <int CH>
-__global__ void __launch_bounds__(NTHREADS, 4) p1_kernel(DevSchedule d) {
+__global__ void __launch_bounds__(NTHREADS, 3) p1_kernel(DevSchedule d) {
   extern __shared__ __align__(16) double smem[];
   const P1Unit u = d.p1[blockIdx.x];
   const Group g = d.groups[u.group];
-  const int tid = threadIdx.x, lane = tid & 31;
-  const int warp = ((tid >> 5) + blockIdx.x) & 3;          // rotate so light edge warps spread over the 4 SMSPs
-  const double* xbase = (g.order == 1) ? d.a : d.b;
-  const double* ybase = d.ws + g.y1_off + (int64_t)u.j0 * g.ldy1;
+  const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+  SmemLayout sm{(uint32_t)__cvta_generic_to_shared(smem)};
+  const double** rowtab = reinterpret_cast<const double**>(smem + NSTAGE * STAGE_DOUBLES + 2 * NSTAGE);
+  init_barriers(sm, tid);
+  const int ntiles = (g.K1 + KT - 1) / KT;
 
-  const Stager<CH> st(tid);
-  const double* xrow[Stager<CH>::PASSES];
-#pragma unroll
-  for (int p = 0; p < Stager<CH>::PASSES; ++p) {
-    const int r = st.r0 + p * Stager<CH>::RPP;
-    xrow[p] = ybase;
-    if (r < u.rows_valid) {
-      const int R = u.R0 + r;
-      const int ti = R / g.rows, x = R - ti * g.rows;
-      const Seg* sg = d.segs + g.seg0 + ti;
-      xrow[p] = xbase + sg->p1_off + (int64_t)x * sg->p1_ld;
+  if (wid == NCONS) {
+    // ---------------- producer warp
+    const double* xbase = (g.order == 1) ? d.a : d.b;
+    const double* ybase = d.ws + g.y1_off + (int64_t)u.j0 * g.ldy1;
+    for (int r = lane; r < TILE; r += 32) {                 // row-pointer table of the stacked X rows
+      const double* ptr = ybase;
+      if (r < u.rows_valid) {
+        const int R = u.R0 + r;
+        const int ti = R / g.rows, x = R - ti * g.rows;
+        const Seg* sg = d.segs + g.seg0 + ti;
+        ptr = xbase + sg->p1_off + (int64_t)x * sg->p1_ld;
+      }
+      rowtab[r] = ptr;
     }
+    __syncwarp();
+    const Stager<CH> st(lane);
+    const double* yrow0 = ybase + (int64_t)st.r0 * g.ldy1;
+    const int64_t ystep = (int64_t)Stager<CH>::RPP * g.ldy1;
+    int stage = 0;
+    uint32_t phase = 1;
+    for (int t = 0; t < ntiles; ++t) {
+      mbar_wait(sm.empty(stage), phase);
+      const uint32_t sx = sm.stage(stage), sy = sx + 4 * TILE * 4 * 8;
+      st.load(sx, [&](int p) { return rowtab[st.r0 + p * Stager<CH>::RPP]; }, u.rows_valid, ybase, t * KT, g.K1);
+      st.load(sy, [&](int p) { return yrow0 + p * ystep; }, u.cols_valid, ybase, t * KT, g.K1);
+      cp_async_mbar_arrive(sm.full(stage));
+      if (++stage == NSTAGE) { stage = 0; phase ^= 1; }
+    }
+    cp_async_wait_all();
+    return;
   }
-  const double* yrow0 = ybase + (int64_t)st.r0 * g.ldy1;
-  const int64_t ystep = (int64_t)Stager<CH>::RPP * g.ldy1;
-  const uint32_t s0 = (uint32_t)__cvta_generic_to_shared(smem);
 
-  auto load = [&](int stage, int kappa) {
-    const uint32_t sx = s0 + stage * STAGE_DOUBLES * 8, sy = sx + 4 * TILE * 4 * 8;
-    st.load(sx, [&](int p) { return xrow[p]; }, u.rows_valid, ybase, kappa, g.K1);
-    st.load(sy, [&](int p) { return yrow0 + p * ystep; }, u.cols_valid, ybase, kappa, g.K1);
-  };
-
+  // ------------------ consumer warps
+  const int warp = (wid + blockIdx.x) & 3;                  // rotate so light edge warps spread over the 4 SMSPs
   const WarpTile w(warp, u.rows_valid, u.cols_valid);
   double acc[4][4][2];
 #pragma unroll
   for (int i = 0; i < 4; ++i)
 #pragma unroll
     for (int j = 0; j < 4; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
-
-  const int ntiles = (g.K1 + KT - 1) / KT;
-#pragma unroll
-  for (int s = 0; s < NSTAGE - 1; ++s) {
-    if (s < ntiles) load(s, s * KT);
-    cp_async_commit();
-  }
-  for (int t = 0; t < ntiles; ++t) {
-    cp_async_wait<NSTAGE - 2>();
-    __syncthreads();
-    const int nt = t + NSTAGE - 1;
-    if (nt < ntiles) load(nt % NSTAGE, nt * KT);
-    cp_async_commit();
-    const double* sx = smem + (t % NSTAGE) * STAGE_DOUBLES;
-    int nk4 = (g.K1 - t * KT + 3) >> 2;
-    nk4 = nk4 > 4 ? 4 : nk4;
-    mma_stage(sx, sx + 4 * TILE * 4, acc, nk4, w, lane);
-  }
-  cp_async_wait<0>();
-
+  struct Seq1 {
+    int K, t;
+    __device__ __forceinline__ int next() {
+      int n = (K - t * KT + 3) >> 2;
+      ++t;
+      return n > 4 ? 4 : (n < 0 ? 0 : n);
+    }
+  } seq{g.K1, 0};
+  consume_dispatch(smem, sm, seq, acc, w, lane);
   double* dst = d.ws + g.ws_off + (int64_t)u.R0 * g.ldw + u.j0;
   store_tile(dst, g.ldw, u.rows_valid, u.cols_valid, acc, w, lane, [&](int row) {
     const int ti = (u.R0 + row) / g.rows;
@@ -229,79 +312,75 @@ struct KIter {                 // walks (run, seg, kappa) in K-tile steps
 };
 
 template <int CH>
-__global__ void __launch_bounds__(NTHREADS, 4) p2_kernel(DevSchedule d) {
+__global__ void __launch_bounds__(NTHREADS, 3) p2_kernel(DevSchedule d) {
   extern __shared__ __align__(16) double smem[];
   const P2Unit u = d.p2[blockIdx.x];
-  const int tid = threadIdx.x, lane = tid & 31;
-  const int warp = ((tid >> 5) + blockIdx.x) & 3;
-  const Stager<CH> st(tid);
-  const uint32_t s0 = (uint32_t)__cvta_generic_to_shared(smem);
+  const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+  SmemLayout sm{(uint32_t)__cvta_generic_to_shared(smem)};
+  init_barriers(sm, tid);
+  KIter it(d.runs, u.run_begin, u.run_end);
 
-  KIter prod(d.runs, u.run_begin, u.run_end), cons(d.runs, u.run_begin, u.run_end);
-  const double *xrow0 = nullptr, *yrow0 = nullptr, *xsafe = nullptr, *ysafe = nullptr;
-  int64_t xstep = 0, ystep = 0;
-  auto open_seg = [&]() {
-    const Seg* sg = d.segs + prod.seg;
-    const int64_t p2_off = sg->p2_off, ws_off = sg->ws_off;
-    const int p2_ld = sg->p2_ld;
-    if (prod.order == 1) {
-      xsafe = d.ws + ws_off + (int64_t)u.i0 * prod.ldw;
-      xrow0 = xsafe + (int64_t)st.r0 * prod.ldw;
-      xstep = (int64_t)Stager<CH>::RPP * prod.ldw;
-      ysafe = d.b + p2_off + (int64_t)u.j0 * p2_ld;
-      yrow0 = ysafe + (int64_t)st.r0 * p2_ld;
-      ystep = (int64_t)Stager<CH>::RPP * p2_ld;
-    } else {
-      xsafe = d.a + p2_off + (int64_t)u.i0 * p2_ld;
-      xrow0 = xsafe + (int64_t)st.r0 * p2_ld;
-      xstep = (int64_t)Stager<CH>::RPP * p2_ld;
-      ysafe = d.ws + ws_off + (int64_t)u.j0 * prod.ldw;
-      yrow0 = ysafe + (int64_t)st.r0 * prod.ldw;
-      ystep = (int64_t)Stager<CH>::RPP * prod.ldw;
+  if (wid == NCONS) {
+    // ---------------- producer warp
+    const Stager<CH> st(lane);
+    const double *xrow0 = nullptr, *yrow0 = nullptr, *xsafe = nullptr, *ysafe = nullptr;
+    int64_t xstep = 0, ystep = 0;
+    auto open_seg = [&]() {
+      const Seg* sg = d.segs + it.seg;
+      const int64_t p2_off = sg->p2_off, ws_off = sg->ws_off;
+      const int p2_ld = sg->p2_ld;
+      if (it.order == 1) {
+        xsafe = d.ws + ws_off + (int64_t)u.i0 * it.ldw;
+        xrow0 = xsafe + (int64_t)st.r0 * it.ldw;
+        xstep = (int64_t)Stager<CH>::RPP * it.ldw;
+        ysafe = d.b + p2_off + (int64_t)u.j0 * p2_ld;
+        yrow0 = ysafe + (int64_t)st.r0 * p2_ld;
+        ystep = (int64_t)Stager<CH>::RPP * p2_ld;
+      } else {
+        xsafe = d.a + p2_off + (int64_t)u.i0 * p2_ld;
+        xrow0 = xsafe + (int64_t)st.r0 * p2_ld;
+        xstep = (int64_t)Stager<CH>::RPP * p2_ld;
+        ysafe = d.ws + ws_off + (int64_t)u.j0 * it.ldw;
+        yrow0 = ysafe + (int64_t)st.r0 * it.ldw;
+        ystep = (int64_t)Stager<CH>::RPP * it.ldw;
+      }
+    };
+    if (it.valid) open_seg();
+    int stage = 0;
+    uint32_t phase = 1;
+    while (it.valid) {
+      mbar_wait(sm.empty(stage), phase);
+      const uint32_t sx = sm.stage(stage), sy = sx + 4 * TILE * 4 * 8;
+      st.load(sx, [&](int p) { return xrow0 + p * xstep; }, u.rows_valid, xsafe, it.kappa, it.K);
+      st.load(sy, [&](int p) { return yrow0 + p * ystep; }, u.cols_valid, ysafe, it.kappa, it.K);
+      cp_async_mbar_arrive(sm.full(stage));
+      if (it.advance()) open_seg();
+      if (++stage == NSTAGE) { stage = 0; phase ^= 1; }
     }
-  };
-  auto load = [&](int stage) {
-    const uint32_t sx = s0 + stage * STAGE_DOUBLES * 8, sy = sx + 4 * TILE * 4 * 8;
-    st.load(sx, [&](int p) { return xrow0 + p * xstep; }, u.rows_valid, xsafe, prod.kappa, prod.K);
-    st.load(sy, [&](int p) { return yrow0 + p * ystep; }, u.cols_valid, ysafe, prod.kappa, prod.K);
-  };
+    cp_async_wait_all();
+    return;
+  }
 
+  // ------------------ consumer warps
+  const int warp = (wid + blockIdx.x) & 3;
   const WarpTile w(warp, u.rows_valid, u.cols_valid);
   double acc[4][4][2];
 #pragma unroll
   for (int i = 0; i < 4; ++i)
 #pragma unroll
     for (int j = 0; j < 4; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
-
-  if (prod.valid) open_seg();
-#pragma unroll
-  for (int s = 0; s < NSTAGE - 1; ++s) {
-    if (prod.valid) {
-      load(s);
-      if (prod.advance()) open_seg();
+  struct Seq2 {
+    KIter& it;
+    __device__ __forceinline__ int next() {
+      if (!it.valid) return 0;
+      const int n = it.nk4();
+      it.advance();
+      return n;
     }
-    cp_async_commit();
-  }
-  int stage = 0, pstage = NSTAGE - 1;
-  while (cons.valid) {
-    cp_async_wait<NSTAGE - 2>();
-    __syncthreads();
-    if (prod.valid) {
-      load(pstage);
-      if (prod.advance()) open_seg();
-    }
-    cp_async_commit();
-    const double* sx = smem + stage * STAGE_DOUBLES;
-    mma_stage(sx, sx + 4 * TILE * 4, acc, cons.nk4(), w, lane);
-    cons.advance();
-    stage = (stage + 1 == NSTAGE) ? 0 : stage + 1;
-    pstage = (pstage + 1 == NSTAGE) ? 0 : pstage + 1;
-  }
-  cp_async_wait<0>();
-
+  } seq{it};
+  consume_dispatch(smem, sm, seq, acc, w, lane);
   store_tile(d.ws + u.out_off, u.ldo, u.rows_valid, u.cols_valid, acc, w, lane, [](int) { return 1.0; });
 }
-
 // ------------------------------------------------------------------------------- prep / reduce / diag kernels
 // prep: psi block (rows x cols, dense) -> padded copy (rows x ldp) and padded transpose (cols x ldt) in the workspace.
 __global__ void prep_kernel(DevSchedule d, const double* __restrict__ psi) {

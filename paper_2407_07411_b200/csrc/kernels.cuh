@@ -1,6 +1,6 @@
 // sm_100a kernels of hpsi_apply.  FP64 tensor path = mma.sync.m8n8k4.f64 (SASS DMMA.8x8x4), the only FP64 MMA
 // sm_100a has (tcgen05 has no f64 kind); operands staged HBM/L2 -> shared memory with cp.async (LDGSTS),
-// accumulators in registers.  One CTA = 128 threads = 2x2 warps on a <=64x64 tile, each warp <=4x4 fragments.
+// accumulators in registers.  One CTA = 1 producer warp + 2x2 consumer warps on a <=64x64 tile (<=4x4 fragments each).
 #pragma once
 #include <cuda_runtime.h>
 
@@ -8,11 +8,13 @@
 
 namespace hpsi {
 
-constexpr int NTHREADS = 128;
-constexpr int NSTAGE = 3;
+constexpr int NCONS = 4;                       // consumer (DMMA) warps per CTA, 2 x 2 over the tile
+constexpr int NTHREADS = (NCONS + 1) * 32;     // + 1 producer (cp.async) warp
+constexpr int NSTAGE = 4;
 // one stage: X[4 k-slabs][64 rows][4] and Y[4][64][4] doubles = 2 * 8 KB
 constexpr int STAGE_DOUBLES = 2 * 4 * TILE * 4;
-constexpr int SMEM_BYTES = NSTAGE * STAGE_DOUBLES * 8 + 64;
+// stages | full[NSTAGE], empty[NSTAGE] mbarriers | 64 row pointers (P1)
+constexpr int SMEM_BYTES = NSTAGE * STAGE_DOUBLES * 8 + 2 * NSTAGE * 8 + TILE * 8;
 
 struct DevSchedule {           // device pointers to the uploaded tables
   const PsiBlk* blocks;

@@ -12,7 +12,7 @@ __device__ __forceinline__ void dmma(double& c0, double& c1, double a, double b)
 
 // KIND 0: 16 independent DMMA chains per warp; 1: 32 independent DFMA chains per thread; 2: both interleaved.
 template <int KIND>
-__global__ void __launch_bounds__(1024) pipe_kernel(int iters, double* sink, double a0, double b0) {
+__global__ void __launch_bounds__(256) pipe_kernel(int iters, double* sink, double a0, double b0) {
   double c[16][2], f[16];
 #pragma unroll
   for (int i = 0; i < 16; ++i) { c[i][0] = c[i][1] = 0.0; f[i] = threadIdx.x * 1e-9 + i; }
@@ -47,7 +47,7 @@ extern "C" int hpsi_bench_fp64_pipe(int kind, int iters, double* ms_out, double*
   cudaEvent_t e0, e1;
   HPSI_CUDA(cudaEventCreate(&e0));
   HPSI_CUDA(cudaEventCreate(&e1));
-  const int grid = wps ? n_sm : n_sm * 4, threads = wps ? wps * 32 : 256;
+  const int grid = wps ? n_sm * wps : n_sm * 4, threads = wps ? 32 : 256;   // w one-warp CTAs per SM
   auto run = [&](int n) {
     if (kind == 0) pipe_kernel<0><<<grid, threads>>>(n, sink, 1.0, 1e-9);
     else if (kind == 1) pipe_kernel<1><<<grid, threads>>>(n, sink, 1.0, 1e-9);

@@ -259,7 +259,8 @@ int build_schedule(const hpsi_sectors_t* s, const hpsi_terms_t* t, uint32_t flag
   const int64_t target = std::max<int64_t>(64 * 4 * 24, total_p2_dmma / slots);
 
   sc->runs.clear(); sc->p2.clear();
-  std::vector<int64_t> unit_cost;
+  std::vector<int> unit_bundle;            // (block, split) bundle of each unit
+  std::vector<int64_t> bundle_cost;        // heaviest tile of the bundle, in DMMA count
   int64_t issued_p2 = 0;
   for (int d = 0; d < nB; ++d) {
     PsiBlk& D = sc->blocks[d];
@@ -299,6 +300,7 @@ int build_schedule(const hpsi_sectors_t* s, const hpsi_terms_t* t, uint32_t flag
       }
       int run1 = (int)sc->runs.size();
       if (run1 == run0) continue;                  // empty chunk (rounding): skip
+      int64_t bundle_max = 0;
       for (auto& r : rt)
         for (auto& c : ct) {
           P2Unit u{};
@@ -308,19 +310,25 @@ int build_schedule(const hpsi_sectors_t* s, const hpsi_terms_t* t, uint32_t flag
           u.out_off = ws + (int64_t)realised * D.rows * D.ldo + (int64_t)r.start * D.ldo + c.start;
           sc->p2.push_back(u);
           int64_t cost = (int64_t)frags(r.len) * frags(c.len) * chunk_ksteps;
-          unit_cost.push_back(cost);
+          unit_bundle.push_back((int)bundle_cost.size());
+          bundle_max = std::max(bundle_max, cost);
           issued_p2 += cost * 512;
         }
+      bundle_cost.push_back(bundle_max);
       ++realised;
     }
     D.nsplit = realised;
     ws = align_up(ws + (int64_t)realised * D.rows * D.ldo, 16);
   }
-  // LPT order (stable: tiles of one (block, split) stay adjacent and share their operands in L2)
+  // LPT order over (block, split) bundles: the tiles of one bundle read the same operand segments, so they stay
+  // adjacent in launch order (co-resident CTAs -> the second reader hits L2); bundles go heaviest tile first.
   {
     std::vector<int> idx(sc->p2.size());
     std::iota(idx.begin(), idx.end(), 0);
-    std::stable_sort(idx.begin(), idx.end(), [&](int a, int b) { return unit_cost[a] > unit_cost[b]; });
+    std::stable_sort(idx.begin(), idx.end(), [&](int a, int b) {
+      if (bundle_cost[unit_bundle[a]] != bundle_cost[unit_bundle[b]]) return bundle_cost[unit_bundle[a]] > bundle_cost[unit_bundle[b]];
+      return unit_bundle[a] < unit_bundle[b];
+    });
     std::vector<P2Unit> sorted(sc->p2.size());
     for (size_t i = 0; i < idx.size(); ++i) sorted[i] = sc->p2[idx[i]];
     sc->p2.swap(sorted);
