@@ -1,0 +1,358 @@
+#!/usr/bin/env python
+"""bench.py - H_eff*psi sustained FP64 TFLOPS on B200 (BASELINE.json metric), one JSON line on stdout.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config cyp] [--impl ours|reference]
+
+A *step* is one pass of the whole hot path (hpsi_apply: prep, first GEMM, second GEMM, reduce) over one seeded
+synthetic psi of the named config (default ``cyp`` = BASELINE.json configs[2], the D=4096 config the metric is
+quoted on).  ``value`` = useful flops (A18: sum over tasks of min(f1, f2)) x steps / device time, inputs
+resident in HBM; ``e2e`` = the same through hpsi_apply_host with pinned HOST psi/out buffers (H2D + D2H inside the
+timed region).  N > 1 (torchrun): the term list is sharded over ranks (operators are the big object), psi is
+replicated and one NCCL all-reduce of psi' per step is inside the timed region; total work is fixed -> "strong".
+``--impl reference`` times the CPU oracle (oracle/, as it stands) on a bounded sample of the same config.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+import workloads  # noqa: E402
+
+METRIC = "H_eff*psi sustained FP64 TFLOPS on 1 B200 (% of measured FP64 TC peak)"
+CONFIG_DESC = {
+    "toy": "configs[0] toy", "small": "configs[1] small QC-like D=1024", "cyp": "configs[2] CYP-shaped D=4096",
+    "femoco": "configs[3] FeMoco-shaped D=8192", "stress": "configs[4] load-imbalance stress D=4096",
+}
+
+
+def log(*a):
+    print(*a, file=sys.stderr, flush=True)
+
+
+# --------------------------------------------------------------------------------------------- clocks sampling
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled every 200 ms while the timed region runs."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.rows, self.proc, self.index = [], None, index
+
+    def __enter__(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "200"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._pump, daemon=True)
+            self.thread.start()
+        except OSError:
+            self.proc = None
+        return self
+
+    def _pump(self):
+        for line in self.proc.stdout:
+            self.rows.append([x.strip() for x in line.split(",")])
+
+    def __exit__(self, *exc):
+        if self.proc is not None:
+            time.sleep(0.25)
+            self.proc.terminate()
+            self.thread.join(timeout=2)
+
+    def summary(self):
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            try:
+                sm.append(float(r[0])); mx.append(float(r[1]))
+            except (ValueError, IndexError):
+                continue
+            for n, v in zip(names, r[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        return {"sm_mhz": float(np.median(sm)), "sm_max_mhz": float(max(mx)), "reasons": sorted(reasons),
+                "samples": len(sm)}
+
+
+# ------------------------------------------------------------------------------------------------ calibration
+def dgemm_calibration(torch, secs=1.0):
+    """Same-run FP64 tensor-core peak: cuBLAS DGEMM (torch.matmul on float64), best sustained 2N^3/t (north_star)."""
+    best, detail = 0.0, {}
+    for N in (4096, 8192):
+        a = torch.randn(N, N, dtype=torch.float64, device="cuda")
+        b = torch.randn(N, N, dtype=torch.float64, device="cuda")
+        c = torch.empty_like(a)
+        for _ in range(2):
+            torch.matmul(a, b, out=c)
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        reps, t0 = 0, time.time()
+        e0.record()
+        while True:
+            for _ in range(3):
+                torch.matmul(a, b, out=c)
+            reps += 3
+            torch.cuda.synchronize()
+            if time.time() - t0 > secs:
+                break
+        e1.record()
+        torch.cuda.synchronize()
+        tf = 2.0 * N ** 3 * reps / (e0.elapsed_time(e1) * 1e-3) / 1e12
+        detail[f"dgemm_{N}"] = round(tf, 3)
+        best = max(best, tf)
+        del a, b, c
+    return best, detail
+
+
+def sample_points(p, n, seed=1):
+    rng = np.random.default_rng(seed)
+    blocks = p.psi_blocks()
+    bi = rng.integers(0, len(blocks), n)
+    sl = np.array([blocks[b][0] for b in bi], np.int32)
+    sx = np.array([rng.integers(0, blocks[b][2]) for b in bi], np.int32)
+    sy = np.array([rng.integers(0, blocks[b][3]) for b in bi], np.int32)
+    idx = np.array([blocks[b][4] + x * blocks[b][3] + y for b, x, y in zip(bi, sx, sy)], np.int64)
+    return sl, sx, sy, idx
+
+
+def cpu_baseline(cfg, budget_s=15.0):
+    """The oracle as it stands, timed on this box's host cores on a bounded sample: the first n base terms (and their
+    adjoints) of the config, n sized from a 1-term probe so that one apply takes about ``budget_s`` seconds."""
+    import oracle
+    half = workloads.config_params(cfg)["n_terms"] // 2
+
+    def run(n):
+        sp = workloads.make_problem(cfg, base_terms=np.arange(min(n, half)))
+        psi = workloads.make_psi(sp)
+        t0 = time.time()
+        oracle.apply(sp, psi)
+        dt = time.time() - t0
+        return oracle.useful_flops(sp)[0], dt, sp.n_terms
+
+    n = 1
+    fl, dt, _ = run(n)
+    for _ in range(3):                          # grow the sample until one apply takes a sizeable part of the budget
+        if dt >= budget_s / 3 or n >= half:
+            break
+        n = int(max(n + 1, min(half, n * budget_s / max(dt, 1e-3))))
+        fl, dt, _ = run(n)
+    return {"value": fl / dt / 1e12, "unit": "TFLOPS", "cores": oracle.num_threads(), "kind": "oracle",
+            "sample": f"one oracle.apply on the first {n} of {half} base terms + adjoints of {cfg} "
+                      f"({fl / 1e9:.2f} useful GF in {dt:.2f} s)"}, fl, dt
+
+
+# ------------------------------------------------------------------------------------------- reference arm
+def run_reference(args, rank):
+    """bench.py --impl reference: the CPU oracle on host cores, bounded sample per step (rank 0 only)."""
+    if rank != 0:
+        return
+    import oracle
+    half = workloads.config_params(args.config)["n_terms"] // 2
+    total_budget = 150.0
+    per_step = total_budget / (args.steps + args.warmup)
+    probe = workloads.make_problem(args.config, base_terms=np.arange(1))
+    psi = workloads.make_psi(probe)
+    t0 = time.time()
+    oracle.apply(probe, psi)
+    dt1 = max(time.time() - t0, 1e-4)
+    n = int(max(1, min(half, per_step / dt1)))
+    sp = workloads.make_problem(args.config, base_terms=np.arange(n))
+    psi = workloads.make_psi(sp)
+    flops = oracle.useful_flops(sp)[0]
+    for _ in range(args.warmup):
+        oracle.apply(sp, psi)
+    t0 = time.time()
+    for _ in range(args.steps):
+        oracle.apply(sp, psi)
+    dt = time.time() - t0
+    val = flops * args.steps / dt / 1e12
+    sample = f"each step = one oracle.apply on the first {n} of {half} base terms + adjoints ({flops / 1e9:.2f} useful GF)"
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": val, "unit": "TFLOPS", "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt / args.steps * 1e3, "higher_is_better": True,
+        "scaling": "strong", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": CONFIG_DESC[args.config], "sample": sample},
+        "cpu_baseline": {"value": val, "unit": "TFLOPS", "cores": oracle.num_threads(), "kind": "oracle", "sample": sample},
+        "e2e": {"value": val, "unit": "TFLOPS", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }), flush=True)
+
+
+# ------------------------------------------------------------------------------------------------- our arm
+def run_ours(args, rank, world, local_rank):
+    import torch
+    import torch.distributed as dist
+    import paper_2407_07411_b200 as H
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the product has no CPU fallback)")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    H.lib()
+
+    cfg = args.config
+    half = workloads.config_params(cfg)["n_terms"] // 2
+    t0 = time.time()
+    shard = None if world == 1 else np.arange(rank, half, world)
+    p = workloads.make_problem(cfg, base_terms=shard)
+    gen_s = time.time() - t0
+    a = torch.from_numpy(p.a_data).to(dev)
+    b = torch.from_numpy(p.b_data).to(dev)
+    t0 = time.time()
+    plan = H.plan_problem(p, a, b)
+    plan_s = time.time() - t0
+    q = lambda w: H.hpsi_query(plan, w)  # noqa: E731
+    n = q(H.HPSI_Q_PSI_LENGTH)
+    useful = torch.tensor([q(H.HPSI_Q_USEFUL_FLOPS), q(H.HPSI_Q_OPERATOR_BYTES), q(H.HPSI_Q_N_TASKS)],
+                          dtype=torch.int64, device=dev)
+    if world > 1:
+        dist.all_reduce(useful)
+    useful_flops, operator_bytes, n_tasks = (int(v) for v in useful.tolist())
+    log(f"[rank {rank}] {cfg}: gen {gen_s:.1f}s plan {plan_s:.2f}s tasks {q(H.HPSI_Q_N_TASKS)} "
+        f"useful {q(H.HPSI_Q_USEFUL_FLOPS) / 1e9:.1f} GF issued {q(H.HPSI_Q_ISSUED_FLOPS) / 1e9:.1f} GF "
+        f"operators {q(H.HPSI_Q_OPERATOR_BYTES) / 1e9:.2f} GB workspace {q(H.HPSI_Q_WORKSPACE_BYTES) / 1e9:.2f} GB")
+
+    dgemm_peak, calib = dgemm_calibration(torch)
+    ms_pipe, fl_pipe = H.hpsi_bench_fp64_pipe(0, 20000)
+    calib["dmma_pipe_probe"] = round(fl_pipe / ms_pipe / 1e9, 3)
+
+    stream = torch.cuda.current_stream()
+    n_psi = 10 if cfg == "femoco" else 1                      # A17: 10 different psi's for the FeMoco config
+    psis = [torch.from_numpy(workloads.make_psi(p, k)).to(dev) for k in range(n_psi)]
+    out = torch.empty(n, dtype=torch.float64, device=dev)
+
+    def step(i):
+        H.hpsi_apply(plan, psis[i % n_psi], out, stream)
+        if world > 1:
+            dist.all_reduce(out)
+
+    def sync_all():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for i in range(args.warmup):
+        step(i)
+    sync_all()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    with ClockSampler(local_rank) as clk:
+        e0.record(stream)
+        for i in range(args.steps):
+            step(i)
+        e1.record(stream)
+        sync_all()
+    ms = torch.tensor([e0.elapsed_time(e1)], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(ms, op=dist.ReduceOp.MAX)
+    ms_total = float(ms.item())
+    value = useful_flops * args.steps / (ms_total * 1e-3) / 1e12
+
+    # ---- end to end: pinned HOST psi / out, H2D + D2H inside the timed region
+    hpsi_in = [torch.from_numpy(workloads.make_psi(p, k)).pin_memory() for k in range(n_psi)]
+    hout = torch.empty(n, dtype=torch.float64).pin_memory()
+    xdev = torch.empty(n, dtype=torch.float64, device=dev)
+
+    def e2e_step(i):
+        if world == 1:
+            H.hpsi_apply_host(plan, hpsi_in[i % n_psi], hout, stream)       # the C-ABI call with HOST buffers
+        else:
+            xdev.copy_(hpsi_in[i % n_psi], non_blocking=True)
+            H.hpsi_apply(plan, xdev, out, stream)
+            dist.all_reduce(out)
+            hout.copy_(out, non_blocking=True)
+            torch.cuda.synchronize()
+
+    for i in range(min(args.warmup, 3)):
+        e2e_step(i)
+    sync_all()
+    e0.record(stream)
+    for i in range(args.steps):
+        e2e_step(i)
+    e1.record(stream)
+    sync_all()
+    ms2 = torch.tensor([e0.elapsed_time(e1)], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(ms2, op=dist.ReduceOp.MAX)
+    e2e_value = useful_flops * args.steps / (float(ms2.item()) * 1e-3) / 1e12
+
+    # ---- roofline of the dominant kernel (live CUDA events between the kernels of an apply)
+    prof = np.zeros(4)
+    for i in range(3):
+        prof += np.array(H.hpsi_apply_profiled(plan, psis[0], out, stream))
+    prof /= 3
+    names = ["prep_kernel", "p1_kernel (first GEMM)", "p2_kernel (second GEMM)", "reduce_kernel"]
+    fl_p1 = q(H.HPSI_Q_USEFUL_FLOPS_P1)
+    fl = [0, fl_p1, q(H.HPSI_Q_USEFUL_FLOPS) - fl_p1, 0]
+    dom = int(np.argmax(prof))
+    achieved = fl[dom] / (prof[dom] * 1e-3) / 1e12 if prof[dom] > 0 else 0.0
+    roofline = {"bound": "tensor", "kernel": names[dom], "achieved": achieved, "peak": dgemm_peak, "unit": "TFLOP/s",
+                "frac": achieved / dgemm_peak, "traffic": None,
+                "peak_source": "same-run cuBLAS DGEMM calibration (north_star); DMMA.8x8x4 pipe probe "
+                               f"{calib['dmma_pipe_probe']} TFLOP/s",
+                "kernel_ms": {k: round(float(v), 4) for k, v in zip(names, prof)},
+                "useful_flops_per_launch": int(fl[dom])}
+
+    res = {
+        "metric": METRIC, "value": value, "unit": "TFLOPS", "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": ms_total / args.steps, "higher_is_better": True, "scaling": "strong",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "pct_of_fp64_tc_peak": 100.0 * value / (dgemm_peak * world),
+        "config": {"workload": CONFIG_DESC[cfg], "sectors_per_side": int(p.q_left.shape[0]),
+                   "D": int(p.d_left.sum()), "terms": int(workloads.config_params(cfg)["n_terms"]), "tasks": n_tasks,
+                   "useful_flops_per_step": useful_flops, "operator_bytes": operator_bytes, "psi_length": n,
+                   "parallelism": "1 GPU" if world == 1 else f"term-sharded x{world} + NCCL all-reduce of psi'",
+                   "l2": "inputs larger than L2 (operators streamed once per step)"},
+        "calibration": {"fp64_tc_peak_tflops": dgemm_peak, **calib},
+        "clocks": clk.summary(),
+        "e2e": {"value": e2e_value, "unit": "TFLOPS", "h2d_bytes_per_step": 8 * n, "d2h_bytes_per_step": 8 * n},
+        "gpu_launches": int(q(H.HPSI_Q_LAUNCHES_PER_APPLY)) * args.steps,
+        "roofline": roofline,
+    }
+    if rank == 0 and world == 1:
+        import oracle
+        # parity spot check on sampled outputs the oracle computes one by one
+        sl, sx, sy, idx = sample_points(p, 32)
+        psi0 = workloads.make_psi(p, 0)
+        H.hpsi_apply(plan, psis[0], out, stream)
+        torch.cuda.synchronize()
+        got = out.cpu().numpy()[idx]
+        ref = oracle.apply_samples(p, psi0, sl, sx, sy)
+        res["parity_sample_rel_err"] = float(np.linalg.norm(got - ref) / np.linalg.norm(ref))
+        del a, b
+        res["cpu_baseline"], _, _ = cpu_baseline(cfg)
+    if rank == 0:
+        print(json.dumps(res), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", default="cyp", choices=list(CONFIG_DESC))
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    args = ap.parse_args()
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.impl == "reference":
+        run_reference(args, rank)
+    else:
+        run_ours(args, rank, world, local_rank)
+
+
+if __name__ == "__main__":
+    main()

@@ -90,6 +90,10 @@ int hpsi_bind(hpsi_plan_t* plan, const double* a_data_dev, const double* b_data_
  * Repeated applies on the same inputs are bitwise identical (no atomics on data). */
 int hpsi_apply(hpsi_plan_t* plan, const double* psi_dev, double* out_dev, void* cuda_stream);
 
+/* hpsi_apply with a CUDA event between its kernels: ms_host (HOST, 4 floats) receives the device time of
+ * [prep, first-GEMM kernel, second-GEMM kernel, reduce].  Synchronises the stream.  For bench.py's roofline object. */
+int hpsi_apply_profiled(hpsi_plan_t* plan, const double* psi_dev, double* out_dev, void* cuda_stream, float* ms_host);
+
 /* Same result through HOST buffers: copies psi to the device, applies, copies out back, synchronises the stream.
  * (End-to-end entry point; operators stay resident in the bound arenas.) */
 int hpsi_apply_host(hpsi_plan_t* plan, const double* psi_host, double* out_host, void* cuda_stream);
@@ -137,7 +141,8 @@ enum {
   HPSI_Q_ALIGNED16 = 13,     /* int64: 1 if the 16-byte staging path is used                                  */
   HPSI_Q_INTERMEDIATE_BYTES = 14, /* int64: bytes of first-GEMM results written (and read back) per apply     */
   HPSI_Q_ISSUED_FLOPS_P1 = 15,    /* int64: first-GEMM share of HPSI_Q_ISSUED_FLOPS                           */
-  HPSI_Q_TASKS = 16          /* hpsi_task_t[n_tasks], in schedule order                                      */
+  HPSI_Q_TASKS = 16,         /* hpsi_task_t[n_tasks], in schedule order                                      */
+  HPSI_Q_USEFUL_FLOPS_P1 = 17 /* int64: first-GEMM share of HPSI_Q_USEFUL_FLOPS                                */
 };
 
 typedef struct {

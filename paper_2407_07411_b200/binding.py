@@ -20,7 +20,7 @@ HPSI_PLAN_FIXED_ORDER2 = 1 << 2
 (HPSI_Q_PSI_LENGTH, HPSI_Q_N_PSI_BLOCKS, HPSI_Q_PSI_BLOCKS, HPSI_Q_N_TASKS, HPSI_Q_USEFUL_FLOPS, HPSI_Q_ISSUED_FLOPS,
  HPSI_Q_OPERATOR_BYTES, HPSI_Q_WORKSPACE_BYTES, HPSI_Q_N_GROUPS, HPSI_Q_N_P1_UNITS, HPSI_Q_N_P2_UNITS,
  HPSI_Q_N_ORDER1_TASKS, HPSI_Q_LAUNCHES_PER_APPLY, HPSI_Q_ALIGNED16, HPSI_Q_INTERMEDIATE_BYTES,
- HPSI_Q_ISSUED_FLOPS_P1, HPSI_Q_TASKS) = range(17)
+ HPSI_Q_ISSUED_FLOPS_P1, HPSI_Q_TASKS, HPSI_Q_USEFUL_FLOPS_P1) = range(18)
 
 PSI_BLOCK_DTYPE = np.dtype([("left", "<i4"), ("right", "<i4"), ("rows", "<i4"), ("cols", "<i4"), ("offset", "<i8")],
                            align=True)
@@ -73,6 +73,7 @@ def lib() -> ctypes.CDLL:
         L.hpsi_bind.argtypes = [vp, vp, vp]
         L.hpsi_apply.argtypes = [vp, vp, vp, vp]
         L.hpsi_apply_host.argtypes = [vp, vp, vp, vp]
+        L.hpsi_apply_profiled.argtypes = [vp, vp, vp, vp, ctypes.POINTER(ctypes.c_float)]
         L.hpsi_diagonal.argtypes = [vp, vp, vp]
         L.hpsi_davidson.argtypes = [vp, vp, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(hpsi_davidson_params_t),
                                     ctypes.POINTER(hpsi_davidson_info_t), vp]
@@ -83,7 +84,7 @@ def lib() -> ctypes.CDLL:
         L.hpsi_bench_fp64_pipe.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.POINTER(ctypes.c_double),
                                            ctypes.POINTER(ctypes.c_double)]
         L.hpsi_debug_interpret.argtypes = [vp, vp, vp, vp, vp]
-        for name in ("hpsi_plan", "hpsi_bind", "hpsi_apply", "hpsi_apply_host", "hpsi_diagonal", "hpsi_davidson",
+        for name in ("hpsi_plan", "hpsi_bind", "hpsi_apply", "hpsi_apply_host", "hpsi_apply_profiled", "hpsi_diagonal", "hpsi_davidson",
                      "hpsi_query", "hpsi_bench_fp64_pipe", "hpsi_debug_interpret"):
             getattr(L, name).restype = ctypes.c_int
         del i32, i64
@@ -159,6 +160,13 @@ def hpsi_bind(plan: Plan, a_data, b_data) -> None:
 def hpsi_apply(plan: Plan, psi, out, stream=None) -> None:
     """out = H psi; psi/out: torch CUDA float64 tensors of psi_length; stream: torch.cuda.Stream or None."""
     _check(lib().hpsi_apply(plan.handle, _ptr(psi), _ptr(out), _stream(stream)))
+
+
+def hpsi_apply_profiled(plan: Plan, psi, out, stream=None):
+    """hpsi_apply with per-kernel device times: returns [prep, first GEMM, second GEMM, reduce] in milliseconds."""
+    ms = (ctypes.c_float * 4)()
+    _check(lib().hpsi_apply_profiled(plan.handle, _ptr(psi), _ptr(out), _stream(stream), ms))
+    return list(ms)
 
 
 def hpsi_apply_host(plan: Plan, psi_host, out_host, stream=None) -> None:

@@ -158,6 +158,31 @@ extern "C" int hpsi_apply(hpsi_plan_t* p, const double* psi_dev, double* out_dev
   return HPSI_OK;
 }
 
+extern "C" int hpsi_apply_profiled(hpsi_plan_t* p, const double* psi_dev, double* out_dev, void* cuda_stream,
+                                   float* ms_host) {
+  if (!p || !ms_host) { set_error("null argument"); return HPSI_EINVAL; }
+  if (p->host_only) { set_error("host-only plan: hpsi_apply_profiled needs a CUDA device"); return HPSI_ESTATE; }
+  if (!p->bound) { set_error("operator arenas not bound (hpsi_bind)"); return HPSI_ESTATE; }
+  if (!psi_dev || !out_dev || psi_dev == out_dev) { set_error("bad psi/out"); return HPSI_EINVAL; }
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  cudaEvent_t ev[5];
+  for (auto& e : ev) HPSI_CUDA(cudaEventCreate(&e));
+  HPSI_CUDA(cudaEventRecord(ev[0], st));
+  launch_prep(p->dev, psi_dev, st);
+  HPSI_CUDA(cudaEventRecord(ev[1], st));
+  launch_p1(p->dev, p->aligned16, st);
+  HPSI_CUDA(cudaEventRecord(ev[2], st));
+  launch_p2(p->dev, p->aligned16, st);
+  HPSI_CUDA(cudaEventRecord(ev[3], st));
+  launch_reduce(p->dev, out_dev, st);
+  HPSI_CUDA(cudaEventRecord(ev[4], st));
+  HPSI_CUDA(cudaEventSynchronize(ev[4]));
+  for (int i = 0; i < 4; ++i) HPSI_CUDA(cudaEventElapsedTime(&ms_host[i], ev[i], ev[i + 1]));
+  for (auto& e : ev) cudaEventDestroy(e);
+  HPSI_CUDA(cudaGetLastError());
+  return HPSI_OK;
+}
+
 extern "C" int hpsi_apply_host(hpsi_plan_t* p, const double* psi_host, double* out_host, void* cuda_stream) {
   if (!p) { set_error("null plan"); return HPSI_EINVAL; }
   if (p->host_only) { set_error("host-only plan: hpsi_apply_host needs a CUDA device (no CPU fallback)"); return HPSI_ESTATE; }
@@ -204,6 +229,7 @@ extern "C" int hpsi_query(const hpsi_plan_t* p, int what, void* out, size_t byte
     }
     case HPSI_Q_N_TASKS: return put_i64((int64_t)sc.segs.size());
     case HPSI_Q_USEFUL_FLOPS: return put_i64(sc.useful_flops);
+    case HPSI_Q_USEFUL_FLOPS_P1: return put_i64(sc.useful_flops_p1);
     case HPSI_Q_ISSUED_FLOPS: return put_i64(sc.issued_flops);
     case HPSI_Q_ISSUED_FLOPS_P1: return put_i64(sc.issued_flops_p1);
     case HPSI_Q_OPERATOR_BYTES: return put_i64(sc.operator_bytes);

@@ -106,32 +106,36 @@ struct WarpTile {
 // One staged K-tile for a warp owning MI x NJ fragments (compile-time, so no predicated DMMA and no WARPSYNC):
 // nk4 k-steps of MI*NJ DMMA.8x8x4; the fragments of step ks+1 are fetched while step ks issues.
 template <int MI, int NJ>
+__device__ __forceinline__ void mma_step(const double (&a)[MI], const double (&b)[NJ], double (&acc)[4][4][2]) {
+#pragma unroll
+  for (int i = 0; i < MI; ++i)
+#pragma unroll
+    for (int j = 0; j < NJ; ++j) dmma884(acc[i][j][0], acc[i][j][1], a[i], b[j]);
+}
+template <int MI, int NJ>
+__device__ __forceinline__ void load_frags(const double* px, const double* py, int ks, double (&a)[MI], double (&b)[NJ]) {
+#pragma unroll
+  for (int i = 0; i < MI; ++i) a[i] = px[ks * TILE * 4 + i * 32];
+#pragma unroll
+  for (int j = 0; j < NJ; ++j) b[j] = py[ks * TILE * 4 + j * 32];
+}
+template <int MI, int NJ>
 __device__ __forceinline__ void mma_stage(const double* px, const double* py, double (&acc)[4][4][2], int nk4) {
-  double a[MI], b[NJ];
-#pragma unroll
-  for (int i = 0; i < MI; ++i) a[i] = px[i * 32];
-#pragma unroll
-  for (int j = 0; j < NJ; ++j) b[j] = py[j * 32];
-#pragma unroll
-  for (int ks = 0; ks < 4; ++ks) {
-    if (ks < nk4) {
-      double an[MI], bn[NJ];
-      if (ks + 1 < 4) {
-#pragma unroll
-        for (int i = 0; i < MI; ++i) an[i] = px[(ks + 1) * TILE * 4 + i * 32];
-#pragma unroll
-        for (int j = 0; j < NJ; ++j) bn[j] = py[(ks + 1) * TILE * 4 + j * 32];
-      }
-#pragma unroll
-      for (int i = 0; i < MI; ++i)
-#pragma unroll
-        for (int j = 0; j < NJ; ++j) dmma884(acc[i][j][0], acc[i][j][1], a[i], b[j]);
-      if (ks + 1 < 4) {
-#pragma unroll
-        for (int i = 0; i < MI; ++i) a[i] = an[i];
-#pragma unroll
-        for (int j = 0; j < NJ; ++j) b[j] = bn[j];
-      }
+  double a0[MI], b0[NJ], a1[MI], b1[NJ];
+  load_frags<MI, NJ>(px, py, 0, a0, b0);
+  if (nk4 == 4) {                       // the common case: straight-line, no predication, no WARPSYNC
+    load_frags<MI, NJ>(px, py, 1, a1, b1);
+    mma_step<MI, NJ>(a0, b0, acc);
+    load_frags<MI, NJ>(px, py, 2, a0, b0);
+    mma_step<MI, NJ>(a1, b1, acc);
+    load_frags<MI, NJ>(px, py, 3, a1, b1);
+    mma_step<MI, NJ>(a0, b0, acc);
+    mma_step<MI, NJ>(a1, b1, acc);
+  } else {                              // ragged K tail of a segment (1..3 k-steps)
+    mma_step<MI, NJ>(a0, b0, acc);
+    for (int ks = 1; ks < nk4; ++ks) {
+      load_frags<MI, NJ>(px, py, ks, a0, b0);
+      mma_step<MI, NJ>(a0, b0, acc);
     }
   }
 }

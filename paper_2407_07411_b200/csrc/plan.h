@@ -97,7 +97,7 @@ struct Schedule {
   std::vector<hpsi_task_t> tasks;     // schedule order, for hpsi_query
   int64_t psi_len = 0;
   int64_t ws_len = 0;                 // doubles
-  int64_t useful_flops = 0, issued_flops = 0, issued_flops_p1 = 0, operator_bytes = 0, intermediate_bytes = 0;
+  int64_t useful_flops = 0, useful_flops_p1 = 0, issued_flops = 0, issued_flops_p1 = 0, operator_bytes = 0, intermediate_bytes = 0;
   int64_t n_order1 = 0;
   int32_t max_block_elems = 0;
   bool aligned16 = true;              // descriptors allow the 16-byte staging path (arena base checked at bind)

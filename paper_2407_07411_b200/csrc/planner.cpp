@@ -170,7 +170,7 @@ int build_schedule(const hpsi_sectors_t* s, const hpsi_terms_t* t, uint32_t flag
 
   // ---- steps 3+4a: order choice, groups, segs
   sc->segs.clear(); sc->groups.clear(); sc->tasks.clear(); sc->diag.clear();
-  sc->useful_flops = sc->operator_bytes = sc->intermediate_bytes = 0;
+  sc->useful_flops = sc->useful_flops_p1 = sc->operator_bytes = sc->intermediate_bytes = 0;
   sc->n_order1 = 0;
   std::vector<std::vector<DiagTask>> diag_by_blk(nB);
   for (size_t i = 0; i < raw.size();) {
@@ -206,6 +206,7 @@ int build_schedule(const hpsi_sectors_t* s, const hpsi_terms_t* t, uint32_t flag
       if ((a.offset & 1) || (a.ld & 1) || (b.offset & 1) || (b.ld & 1)) sc->aligned16 = false;
       sc->tasks.push_back({raw[q].term, raw[q].ia, raw[q].ib, S.left, D.left, order});
       sc->useful_flops += std::min(f1, f2);
+      sc->useful_flops_p1 += (f2 < f1) ? 2 * k * np * n : 2 * m * k * np;   // first GEMM of the min-flop order
       sc->operator_bytes += 8 * (m * k + n * np);
       sc->intermediate_bytes += 8 * (int64_t)g.rows * g.N1;
       if (order == 1) sc->n_order1++;

@@ -30,7 +30,7 @@ def test_library_exports_every_declared_symbol():
     hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
     names = set(re.findall(r"\b(hpsi_[a-z0-9_]+)\s*\(", hdr))
     assert {"hpsi_plan", "hpsi_apply", "hpsi_apply_host", "hpsi_bind", "hpsi_davidson", "hpsi_query", "hpsi_destroy",
-            "hpsi_last_error", "hpsi_diagonal", "hpsi_debug_interpret", "hpsi_bench_fp64_pipe"} <= names
+            "hpsi_last_error", "hpsi_diagonal", "hpsi_debug_interpret", "hpsi_bench_fp64_pipe", "hpsi_apply_profiled"} <= names
     L = H.lib()
     for n in names:
         assert hasattr(L, n), n

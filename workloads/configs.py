@@ -66,6 +66,7 @@ class Problem:
     term_a_range: Optional[np.ndarray] = None   # [n_terms, 2] descriptor index range of each term in a_desc
     term_b_range: Optional[np.ndarray] = None
     entry_seed: Optional[Tuple[int, ...]] = None
+    base_term_ids: Optional[np.ndarray] = None  # [n_terms/2] index of each base term in the full config (term shards)
 
     @property
     def n_terms(self) -> int:
@@ -266,7 +267,8 @@ def fill_term(p: Problem, t: int, a_data: np.ndarray, b_data: np.ndarray,
     adjoint blocks are exact transposes (A9).  The stream of term t depends only on (entry_seed, t)."""
     half = p.n_terms // 2
     assert 0 <= t < half
-    rng = np.random.default_rng(list(p.entry_seed) + [t])
+    gid = int(p.base_term_ids[t]) if p.base_term_ids is not None else t      # stream of the term in the full config
+    rng = np.random.default_rng(list(p.entry_seed) + [gid])
     for desc, rng_tab, data, base, dims in ((p.a_desc, p.term_a_range, a_data, a_base, p.d_left),
                                             (p.b_desc, p.term_b_range, b_data, b_base, p.d_right)):
         lo, hi = rng_tab[t]
@@ -286,9 +288,12 @@ def fill_term(p: Problem, t: int, a_data: np.ndarray, b_data: np.ndarray,
 
 
 def make_problem(name: str, seed: Optional[int] = None, fill: bool = True, pad_even: bool = True,
-                 n_terms: Optional[int] = None) -> Problem:
+                 n_terms: Optional[int] = None, base_terms=None) -> Problem:
     """Build config ``name`` (seed defaults to the config index).  ``fill=False`` returns descriptors only
-    (arenas can then be streamed with ``fill_term``).  ``n_terms`` overrides the term count (tests)."""
+    (arenas can then be streamed with ``fill_term``).  ``n_terms`` overrides the term count (tests).
+    ``base_terms`` (indices into the T/2 base terms) keeps only those terms and their adjoints, with the same
+    coefficients, shifts and entries they have in the full config (term shards for multi-GPU runs, bounded
+    samples for the timed CPU baseline); arenas are compacted to the kept terms."""
     par = _PARAMS[name]
     seed = par["index"] if seed is None else seed
     q_left, q_right, d_left, d_right, target, partner = _sector_tables(name, seed)
@@ -300,11 +305,20 @@ def make_problem(name: str, seed: Optional[int] = None, fill: bool = True, pad_e
     base_shift = np.array([SHIFTS[i] for i in pick], np.int32).reshape(half, 2)
     shifts = np.concatenate([base_shift, -base_shift], axis=0)
     c = rng.standard_normal(half)
+    ids = None
+    if base_terms is not None:
+        ids = np.asarray(base_terms, np.int64)
+        assert ids.ndim == 1 and (ids.size == 0 or (ids.min() >= 0 and ids.max() < half))
+        base_shift = base_shift[ids].reshape(-1, 2)
+        shifts = np.concatenate([base_shift, -base_shift], axis=0)
+        c = c[ids]
+        half = ids.size
     coef = np.concatenate([c, c])
     a_desc, b_desc, a_len, b_len, ta, tb = _build_descriptors(q_left, q_right, d_left, d_right, shifts, pad_even)
     p = Problem(name=name, seed=seed, q_left=q_left, q_right=q_right, d_left=d_left, d_right=d_right,
                 target=target, coef=coef, a_desc=a_desc, b_desc=b_desc, a_len=int(a_len), b_len=int(b_len),
-                shifts=shifts, partner=partner, term_a_range=ta, term_b_range=tb, entry_seed=(seed, 303))
+                shifts=shifts, partner=partner, term_a_range=ta, term_b_range=tb, entry_seed=(seed, 303),
+                base_term_ids=ids)
     if fill:
         p.a_data = np.zeros(max(p.a_len, 1), np.float64)
         p.b_data = np.zeros(max(p.b_len, 1), np.float64)
