@@ -1,5 +1,6 @@
 // C-ABI entry points of include/hpsi.h (plan / bind / apply / query / destroy / debug).
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <vector>
@@ -62,6 +63,7 @@ int upload_schedule(hpsi_plan_t* p) {
   p->dev.n_p1 = (int)sc.p1.size();
   p->dev.n_p2 = (int)sc.p2.size();
   p->dev.max_block_elems = sc.max_block_elems;
+  p->dev.debug = getenv("HPSI_DEBUG") ? atoi(getenv("HPSI_DEBUG")) : 0;
   if (sc.psi_len > 0) {
     HPSI_CUDA(cudaMalloc(&p->d_psi_stage, (size_t)sc.psi_len * sizeof(double)));
     HPSI_CUDA(cudaMalloc(&p->d_out_stage, (size_t)sc.psi_len * sizeof(double)));

@@ -167,6 +167,11 @@ __device__ __forceinline__ void store_tile(double* dst, int ld, int rows_valid, 
   }
 }
 
+// Which tile quadrant consumer warp 0 takes.  Consumer warp w sits on SM sub-partition w, and with odd fragment counts
+// the quadrants carry unequal DMMA counts (e.g. 16/12/12/9), so co-resident CTAs must not all put their heavy
+// quadrant on the same sub-partition.  CTAs are dealt to SMs round-robin (148 = 0 mod 4), hence a hash, not bid & 3.
+__device__ __forceinline__ int quadrant_rotation(unsigned bid) { return (int)((bid * 2654435761u) >> 30); }
+
 // Shared-memory carve-up: NSTAGE stages of [X tile | Y tile], then the barriers and (P1) the row-pointer table.
 struct SmemLayout {
   uint32_t base;                                   // shared-window address of stage 0
@@ -187,13 +192,13 @@ __device__ __forceinline__ void init_barriers(const SmemLayout& sm, int tid) {
 // next staged K-tile, or 0 when the unit is done.  Idle warps (MI == 0) only hand the stages back.
 template <int MI, int NJ, class Seq>
 __device__ __forceinline__ void consume(const double* smem, const SmemLayout& sm, Seq& seq, double (&acc)[4][4][2],
-                                        const WarpTile& w, int lane) {
+                                        const WarpTile& w, int lane, bool skip_mma) {
   int stage = 0;
   uint32_t phase = 0;
   const int xoff = w.wr0 * 4 + lane, yoff = 4 * TILE * 4 + w.wc0 * 4 + lane;
   for (int nk4 = seq.next(); nk4 > 0; nk4 = seq.next()) {
     mbar_wait(sm.full(stage), phase);
-    if (MI > 0) {
+    if (MI > 0 && !skip_mma) {
       const double* st = smem + stage * STAGE_DOUBLES;
       mma_stage<(MI > 0 ? MI : 1), (NJ > 0 ? NJ : 1)>(st + xoff, st + yoff, acc, nk4);
     }
@@ -205,14 +210,14 @@ __device__ __forceinline__ void consume(const double* smem, const SmemLayout& sm
 
 template <class Seq>
 __device__ __forceinline__ void consume_dispatch(const double* smem, const SmemLayout& sm, Seq& seq,
-                                                 double (&acc)[4][4][2], const WarpTile& w, int lane) {
-#define HPSI_CASE(MI, NJ) case MI * 5 + NJ: consume<MI, NJ>(smem, sm, seq, acc, w, lane); break;
+                                                 double (&acc)[4][4][2], const WarpTile& w, int lane, bool skip_mma) {
+#define HPSI_CASE(MI, NJ) case MI * 5 + NJ: consume<MI, NJ>(smem, sm, seq, acc, w, lane, skip_mma); break;
   switch ((w.nj > 0 ? w.mi : 0) * 5 + (w.mi > 0 ? w.nj : 0)) {
     HPSI_CASE(1, 1) HPSI_CASE(1, 2) HPSI_CASE(1, 3) HPSI_CASE(1, 4)
     HPSI_CASE(2, 1) HPSI_CASE(2, 2) HPSI_CASE(2, 3) HPSI_CASE(2, 4)
     HPSI_CASE(3, 1) HPSI_CASE(3, 2) HPSI_CASE(3, 3) HPSI_CASE(3, 4)
     HPSI_CASE(4, 1) HPSI_CASE(4, 2) HPSI_CASE(4, 3) HPSI_CASE(4, 4)
-    default: consume<0, 0>(smem, sm, seq, acc, w, lane); break;
+    default: consume<0, 0>(smem, sm, seq, acc, w, lane, skip_mma); break;
   }
 #undef HPSI_CASE
 }
@@ -254,8 +259,10 @@ __global__ void __launch_bounds__(NTHREADS, 3) p1_kernel(DevSchedule d) {
     for (int t = 0; t < ntiles; ++t) {
       mbar_wait(sm.empty(stage), phase);
       const uint32_t sx = sm.stage(stage), sy = sx + 4 * TILE * 4 * 8;
-      st.load(sx, [&](int p) { return rowtab[st.r0 + p * Stager<CH>::RPP]; }, u.rows_valid, ybase, t * KT, g.K1);
-      st.load(sy, [&](int p) { return yrow0 + p * ystep; }, u.cols_valid, ybase, t * KT, g.K1);
+      if (d.debug != 1) {
+        st.load(sx, [&](int p) { return rowtab[st.r0 + p * Stager<CH>::RPP]; }, u.rows_valid, ybase, t * KT, g.K1);
+        st.load(sy, [&](int p) { return yrow0 + p * ystep; }, u.cols_valid, ybase, t * KT, g.K1);
+      }
       cp_async_mbar_arrive(sm.full(stage));
       if (++stage == NSTAGE) { stage = 0; phase ^= 1; }
     }
@@ -264,7 +271,7 @@ __global__ void __launch_bounds__(NTHREADS, 3) p1_kernel(DevSchedule d) {
   }
 
   // ------------------ consumer warps
-  const int warp = (wid + blockIdx.x) & 3;                  // rotate so light edge warps spread over the 4 SMSPs
+  const int warp = (wid + quadrant_rotation(blockIdx.x)) & 3;
   const WarpTile w(warp, u.rows_valid, u.cols_valid);
   double acc[4][4][2];
 #pragma unroll
@@ -279,7 +286,7 @@ __global__ void __launch_bounds__(NTHREADS, 3) p1_kernel(DevSchedule d) {
       return n > 4 ? 4 : (n < 0 ? 0 : n);
     }
   } seq{g.K1, 0};
-  consume_dispatch(smem, sm, seq, acc, w, lane);
+  consume_dispatch(smem, sm, seq, acc, w, lane, d.debug == 2);
   double* dst = d.ws + g.ws_off + (int64_t)u.R0 * g.ldw + u.j0;
   store_tile(dst, g.ldw, u.rows_valid, u.cols_valid, acc, w, lane, [&](int row) {
     const int ti = (u.R0 + row) / g.rows;
@@ -355,8 +362,10 @@ __global__ void __launch_bounds__(NTHREADS, 3) p2_kernel(DevSchedule d) {
     while (it.valid) {
       mbar_wait(sm.empty(stage), phase);
       const uint32_t sx = sm.stage(stage), sy = sx + 4 * TILE * 4 * 8;
-      st.load(sx, [&](int p) { return xrow0 + p * xstep; }, u.rows_valid, xsafe, it.kappa, it.K);
-      st.load(sy, [&](int p) { return yrow0 + p * ystep; }, u.cols_valid, ysafe, it.kappa, it.K);
+      if (d.debug != 1) {
+        st.load(sx, [&](int p) { return xrow0 + p * xstep; }, u.rows_valid, xsafe, it.kappa, it.K);
+        st.load(sy, [&](int p) { return yrow0 + p * ystep; }, u.cols_valid, ysafe, it.kappa, it.K);
+      }
       cp_async_mbar_arrive(sm.full(stage));
       if (it.advance()) open_seg();
       if (++stage == NSTAGE) { stage = 0; phase ^= 1; }
@@ -366,7 +375,7 @@ __global__ void __launch_bounds__(NTHREADS, 3) p2_kernel(DevSchedule d) {
   }
 
   // ------------------ consumer warps
-  const int warp = (wid + blockIdx.x) & 3;
+  const int warp = (wid + quadrant_rotation(blockIdx.x)) & 3;
   const WarpTile w(warp, u.rows_valid, u.cols_valid);
   double acc[4][4][2];
 #pragma unroll
@@ -382,7 +391,7 @@ __global__ void __launch_bounds__(NTHREADS, 3) p2_kernel(DevSchedule d) {
       return n;
     }
   } seq{it};
-  consume_dispatch(smem, sm, seq, acc, w, lane);
+  consume_dispatch(smem, sm, seq, acc, w, lane, d.debug == 2);
   store_tile(d.ws + u.out_off, u.ldo, u.rows_valid, u.cols_valid, acc, w, lane, [](int) { return 1.0; });
 }
 // ------------------------------------------------------------------------------- prep / reduce / diag kernels

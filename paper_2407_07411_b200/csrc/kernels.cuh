@@ -29,6 +29,7 @@ struct DevSchedule {           // device pointers to the uploaded tables
   const double* b;
   int n_blocks, n_p1, n_p2;
   int max_block_elems;
+  int debug;                   // HPSI_DEBUG env (timing experiments only): 1 = producer skips loads, 2 = consumers skip MMAs
 };
 
 void launch_prep(const DevSchedule& d, const double* psi, cudaStream_t st);
