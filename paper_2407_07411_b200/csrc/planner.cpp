@@ -98,8 +98,8 @@ int build_schedule(const hpsi_sectors_t* s, const hpsi_terms_t* t, uint32_t flag
     b.rows = s->d_left[i];
     b.cols = s->d_right[it->second];
     b.off = off;
-    b.ldp = even_up(b.cols);
-    b.ldt = even_up(b.rows);
+    b.ldp = sector_up(b.cols);
+    b.ldt = sector_up(b.rows);
     off += (int64_t)b.rows * b.cols;
     blk_of_left[i] = (int)sc->blocks.size();
     partner[i] = it->second;
@@ -191,7 +191,7 @@ int build_schedule(const hpsi_sectors_t* s, const hpsi_terms_t* t, uint32_t flag
     g.dst = raw[i].dst;
     if (order == 1) { g.rows = (int32_t)m; g.K1 = (int32_t)k; g.N1 = (int32_t)np; g.ldy1 = S.ldt; g.y1_off = S.t_off; }
     else            { g.rows = (int32_t)n; g.K1 = (int32_t)np; g.N1 = (int32_t)k; g.ldy1 = S.ldp; g.y1_off = S.p_off; }
-    g.ldw = even_up(g.N1);
+    g.ldw = sector_up(g.N1);
     g.ws_off = ws;
     const int64_t per_task = (int64_t)g.rows * g.ldw;
     for (size_t q = i; q < j; ++q) {
@@ -265,7 +265,7 @@ int build_schedule(const hpsi_sectors_t* s, const hpsi_terms_t* t, uint32_t flag
   int64_t issued_p2 = 0;
   for (int d = 0; d < nB; ++d) {
     PsiBlk& D = sc->blocks[d];
-    D.ldo = even_up(D.cols);
+    D.ldo = sector_up(D.cols);
     D.part_off = ws;
     D.nsplit = 0;
     if (dsts[d].nseg == 0) continue;

@@ -209,14 +209,15 @@ def _label_index(q: np.ndarray) -> Dict[Tuple[int, int], int]:
     return {(int(a), int(b)): i for i, (a, b) in enumerate(q)}
 
 
-def _even(x: int) -> int:
-    return x + (x & 1)
+def _round_up(x: int, a: int) -> int:
+    return (x + a - 1) // a * a
 
 
 # -------------------------------------------------------------------------------------------- builder
-def _build_descriptors(q_left, q_right, d_left, d_right, shifts, pad_even: bool):
+def _build_descriptors(q_left, q_right, d_left, d_right, shifts, row_align: int):
     """Descriptor tables for all terms.  Arena layout: term-major, within a term blocks by ascending source
-    (column) sector; ld = #cols (rounded up to even when pad_even, so every row start is 16-byte aligned)."""
+    (column) sector; ld = #cols and block offsets rounded up to a multiple of ``row_align`` doubles (4: every row
+    starts on a 32-byte L2 sector, the library's preferred layout; 2: 16-byte rows; 1: dense, 8-byte rows)."""
     n_terms = shifts.shape[0]
     li, ri = _label_index(q_left), _label_index(q_right)
     a_rows, b_rows = [], []
@@ -230,22 +231,18 @@ def _build_descriptors(q_left, q_right, d_left, d_right, shifts, pad_even: bool)
             r = li.get((int(q_left[c, 0]) + dn, int(q_left[c, 1]) + ds))
             if r is None:
                 continue
-            ld = _even(int(d_left[c])) if pad_even else int(d_left[c])
+            ld = _round_up(int(d_left[c]), row_align)
             a_rows.append((t, r, c, ld, a_off))
-            a_off += int(d_left[r]) * ld
-            if pad_even:
-                a_off = _even(a_off)
+            a_off = _round_up(a_off + int(d_left[r]) * ld, row_align)
         ta[t, 1] = len(a_rows)
         tb[t, 0] = len(b_rows)
         for c in range(q_right.shape[0]):
             r = ri.get((int(q_right[c, 0]) - dn, int(q_right[c, 1]) - ds))
             if r is None:
                 continue
-            ld = _even(int(d_right[c])) if pad_even else int(d_right[c])
+            ld = _round_up(int(d_right[c]), row_align)
             b_rows.append((t, r, c, ld, b_off))
-            b_off += int(d_right[r]) * ld
-            if pad_even:
-                b_off = _even(b_off)
+            b_off = _round_up(b_off + int(d_right[r]) * ld, row_align)
         tb[t, 1] = len(b_rows)
     a_desc = np.array(a_rows, dtype=OPBLOCK_DTYPE) if a_rows else np.zeros(0, OPBLOCK_DTYPE)
     b_desc = np.array(b_rows, dtype=OPBLOCK_DTYPE) if b_rows else np.zeros(0, OPBLOCK_DTYPE)
@@ -288,7 +285,7 @@ def fill_term(p: Problem, t: int, a_data: np.ndarray, b_data: np.ndarray,
 
 
 def make_problem(name: str, seed: Optional[int] = None, fill: bool = True, pad_even: bool = True,
-                 n_terms: Optional[int] = None, base_terms=None) -> Problem:
+                 n_terms: Optional[int] = None, base_terms=None, row_align: Optional[int] = None) -> Problem:
     """Build config ``name`` (seed defaults to the config index).  ``fill=False`` returns descriptors only
     (arenas can then be streamed with ``fill_term``).  ``n_terms`` overrides the term count (tests).
     ``base_terms`` (indices into the T/2 base terms) keeps only those terms and their adjoints, with the same
@@ -314,7 +311,9 @@ def make_problem(name: str, seed: Optional[int] = None, fill: bool = True, pad_e
         c = c[ids]
         half = ids.size
     coef = np.concatenate([c, c])
-    a_desc, b_desc, a_len, b_len, ta, tb = _build_descriptors(q_left, q_right, d_left, d_right, shifts, pad_even)
+    if row_align is None:
+        row_align = 4 if pad_even else 1
+    a_desc, b_desc, a_len, b_len, ta, tb = _build_descriptors(q_left, q_right, d_left, d_right, shifts, row_align)
     p = Problem(name=name, seed=seed, q_left=q_left, q_right=q_right, d_left=d_left, d_right=d_right,
                 target=target, coef=coef, a_desc=a_desc, b_desc=b_desc, a_len=int(a_len), b_len=int(b_len),
                 shifts=shifts, partner=partner, term_a_range=ta, term_b_range=tb, entry_seed=(seed, 303),
@@ -352,7 +351,7 @@ def custom_problem(q_left, d_left, q_right, d_right, target, terms, pad_even: bo
         for (r, cc), arr in ab.items():
             arr = np.asarray(arr, np.float64)
             assert arr.shape == (d_left[r], d_left[cc]), (arr.shape, r, cc)
-            ld = _even(arr.shape[1]) if pad_even else arr.shape[1]
+            ld = _round_up(arr.shape[1], 2) if pad_even else arr.shape[1]
             buf = np.zeros((arr.shape[0], ld))
             buf[:, :arr.shape[1]] = arr
             a_rows.append((t, r, cc, ld, a_off))
@@ -363,7 +362,7 @@ def custom_problem(q_left, d_left, q_right, d_right, target, terms, pad_even: bo
         for (r, cc), arr in bb.items():
             arr = np.asarray(arr, np.float64)
             assert arr.shape == (d_right[r], d_right[cc]), (arr.shape, r, cc)
-            ld = _even(arr.shape[1]) if pad_even else arr.shape[1]
+            ld = _round_up(arr.shape[1], 2) if pad_even else arr.shape[1]
             buf = np.zeros((arr.shape[0], ld))
             buf[:, :arr.shape[1]] = arr
             b_rows.append((t, r, cc, ld, b_off))
