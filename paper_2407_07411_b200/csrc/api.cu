@@ -5,6 +5,8 @@
 #include <new>
 #include <vector>
 
+#include <cuda.h>
+
 #include "plan_dev.h"
 
 namespace hpsi {
@@ -48,6 +50,8 @@ int upload_schedule(hpsi_plan_t* p) {
     return HPSI_ENOMEM;
   }
   HPSI_CUDA(cudaMemset(p->d_ws, 0, (size_t)sc.ws_len * sizeof(double)));
+  HPSI_CUDA(cudaMalloc(&p->d_maps, std::max<size_t>(sc.maps.size(), 1) * TMAP_BYTES));
+  p->dev.maps = static_cast<const unsigned char*>(p->d_maps);
   char* base = static_cast<char*>(p->d_tables);
   size_t cur = 0;
   int rc;
@@ -76,12 +80,50 @@ void free_plan(hpsi_plan_t* p) {
   if (!p->host_only) {
     cudaFree(p->d_tables);
     cudaFree(p->d_ws);
+    cudaFree(p->d_maps);
     cudaFree(p->d_psi_stage);
     cudaFree(p->d_out_stage);
     cudaFree(p->d_dav);
     cudaGetLastError();
   }
   delete p;
+}
+
+// Tensor maps of every operand matrix (plan.h MapSpec): 2-D FP64 tensor {cols, rows} with row pitch ld, box
+// {KT, box_rows}, 128-byte swizzle, zero fill outside the matrix.  The encoder is a driver entry point fetched
+// through the runtime, so the library does not link libcuda.
+typedef CUresult (*tmap_encode_fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                   const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                   CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+int encode_maps(hpsi_plan_t* p) {
+  static_assert(sizeof(CUtensorMap) == TMAP_BYTES, "CUtensorMap size");
+  const std::vector<MapSpec>& specs = p->sc.maps;
+  if (specs.empty()) return HPSI_OK;
+  tmap_encode_fn enc = nullptr;
+  cudaDriverEntryPointQueryResult qr;
+  HPSI_CUDA(cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", reinterpret_cast<void**>(&enc), cudaEnableDefault, &qr));
+  if (!enc || qr != cudaDriverEntryPointSuccess) { set_error("cuTensorMapEncodeTiled not available in this driver"); return HPSI_ECUDA; }
+  std::vector<CUtensorMap> host(specs.size());
+  for (size_t i = 0; i < specs.size(); ++i) {
+    const MapSpec& m = specs[i];
+    const double* base = m.base == BASE_A ? p->dev.a : (m.base == BASE_B ? p->dev.b : p->d_ws);
+    const cuuint64_t dims[2] = {(cuuint64_t)m.cols, (cuuint64_t)m.rows};
+    const cuuint64_t strides[1] = {(cuuint64_t)m.ld * 8};
+    const cuuint32_t box[2] = {(cuuint32_t)KT, (cuuint32_t)m.box_rows};
+    const cuuint32_t estr[2] = {1, 1};
+    CUresult r = enc(&host[i], CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, const_cast<double*>(base + m.off), dims, strides, box, estr,
+                     CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                     CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) {
+      char buf[200];
+      snprintf(buf, sizeof buf, "cuTensorMapEncodeTiled failed (%d) for a %d x %d matrix with ld %d", (int)r, m.rows, m.cols, m.ld);
+      set_error(buf);
+      return HPSI_ECUDA;
+    }
+  }
+  HPSI_CUDA(cudaMemcpy(p->d_maps, host.data(), host.size() * sizeof(CUtensorMap), cudaMemcpyHostToDevice));
+  return HPSI_OK;
 }
 
 }  // namespace
@@ -96,6 +138,10 @@ extern "C" int hpsi_bind(hpsi_plan_t* p, const double* a_dev, const double* b_de
   p->dev.b = b_dev;
   p->aligned16 = p->sc.aligned16 && ((reinterpret_cast<uintptr_t>(a_dev) & 15) == 0) &&
                  ((reinterpret_cast<uintptr_t>(b_dev) & 15) == 0);
+  if (p->aligned16) {
+    int rc = encode_maps(p);
+    if (rc != HPSI_OK) return rc;
+  }
   p->bound = true;
   return HPSI_OK;
 }

@@ -19,22 +19,22 @@ void interpret_schedule(const Schedule& sc, const double* a, const double* b, co
         ws[B.p_off + (int64_t)x * B.ldp + y] = v;
         ws[B.t_off + (int64_t)y * B.ldt + x] = v;
       }
-  // P1: C[R, j] = coef(seg of R) * sum_k X[R,k] Y[j,k]
+  // P1: T_t[i, j] = coef_t * sum_k X_t[i,k] Y[j,k] for the unit's tile and terms
   for (const P1Unit& u : sc.p1) {
     const Group& g = sc.groups[u.group];
     const double* xbase = (g.order == 1) ? a : b;
     const double* y = ws + g.y1_off;
-    for (int r = 0; r < u.rows_valid; ++r) {
-      const int R = u.R0 + r;
-      const int ti = R / g.rows, x = R % g.rows;
-      const Seg& sg = sc.segs[g.seg0 + ti];
-      const double* xr = xbase + sg.p1_off + (int64_t)x * sg.p1_ld;
-      for (int c = 0; c < u.cols_valid; ++c) {
-        const int j = u.j0 + c;
-        const double* yr = y + (int64_t)j * g.ldy1;
-        double s = 0.0;
-        for (int k = 0; k < g.K1; ++k) s += xr[k] * yr[k];
-        ws[g.ws_off + (int64_t)R * g.ldw + j] = sg.coef * s;
+    for (int t = u.t0; t < u.t1; ++t) {
+      const Seg& sg = sc.segs[g.seg0 + t];
+      for (int r = 0; r < u.rows_valid; ++r) {
+        const double* xr = xbase + sg.p1_off + (int64_t)(u.i0 + r) * sg.p1_ld;
+        for (int c = 0; c < u.cols_valid; ++c) {
+          const int j = u.j0 + c;
+          const double* yr = y + (int64_t)j * g.ldy1;
+          double s = 0.0;
+          for (int k = 0; k < g.K1; ++k) s += xr[k] * yr[k];
+          ws[g.ws_off + ((int64_t)t * g.rows + u.i0 + r) * g.ldw + j] = sg.coef * s;
+        }
       }
     }
   }
@@ -47,13 +47,14 @@ void interpret_schedule(const Schedule& sc, const double* a, const double* b, co
           const Run& run = sc.runs[ri];
           for (int si = run.seg_begin; si < run.seg_end; ++si) {
             const Seg& sg = sc.segs[si];
+            const int64_t t_off = run.ws_off + (int64_t)(si - run.seg0) * run.rows * run.ldw;
             const double *xr, *yr;
             if (run.order == 1) {
-              xr = ws + sg.ws_off + (int64_t)(u.i0 + r) * run.ldw;
+              xr = ws + t_off + (int64_t)(u.i0 + r) * run.ldw;
               yr = b + sg.p2_off + (int64_t)(u.j0 + c) * sg.p2_ld;
             } else {
               xr = a + sg.p2_off + (int64_t)(u.i0 + r) * sg.p2_ld;
-              yr = ws + sg.ws_off + (int64_t)(u.j0 + c) * run.ldw;
+              yr = ws + t_off + (int64_t)(u.j0 + c) * run.ldw;
             }
             for (int k = 0; k < run.K; ++k) s += xr[k] * yr[k];
           }

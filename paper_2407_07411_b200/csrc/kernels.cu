@@ -1,22 +1,28 @@
-// sm_100a kernels of hpsi_apply: prep (padded psi, psi^T), P1 (stacked first GEMM), P2 (segmented-K second GEMM
-// with split-K partials), reduce (ordered sum of partials), diag.  See kernels.cuh / plan.h for the vocabulary.
+// sm_100a kernels of hpsi_apply: prep (padded psi, psi^T), P1 (first GEMM, per tile position over a range of terms),
+// P2 (segmented-K second GEMM with split-K partials), reduce (ordered sum of partials), diag.
+// See kernels.cuh / plan.h for the vocabulary.
 //
 // GEMM CTA = 1 producer warp + 4 consumer warps (warp-specialised, mbarrier ring of NSTAGE stages):
-//   producer : cp.async (LDGSTS, zero-fill for ragged edges) of a 64 x 16 X tile and a 64 x 16 Y tile per stage,
-//              completion signalled with cp.async.mbarrier.arrive on the stage's "full" barrier;
+//   producer : one elected lane issues two TMA tile loads per stage (cp.async.bulk.tensor.2d: a 64-row x 16-column
+//              box of the X operand and one of the Y operand, 128-byte swizzle, rows / columns past the matrix edge
+//              zero-filled by the hardware) that complete on the stage's "full" mbarrier (complete_tx::bytes).
+//              Measured on B200 for this access pattern: TMA boxes feed 6.1-6.9 TB/s from HBM and 12-13.9 TB/s from L2,
+//              16-byte LDGSTS 4.8 / 6.4 TB/s.  Matrices whose rows are not 16-byte aligned take the LDGSTS variant
+//              (8-byte cp.async with zero fill into the same swizzled layout).
 //   consumers: 2x2 warps, each <= 4x4 fragments of DMMA.8x8x4 with register accumulators; a warp waits only on the
 //              "full" barrier of its next stage and releases the stage on its "empty" barrier - no CTA-wide barrier
-//              in the main loop.  Measured on B200: one warp issues a DMMA.8x8x4 at most every ~29 clk while the
-//              pipe takes one per 16 clk per SM sub-partition, so >= 2 warps per sub-partition must always be in
-//              their DMMA phase; decoupling the warps is what keeps them there.
+//              in the main loop.
+//
+// Shared-memory tile layout (what the TMA unit writes with CU_TENSOR_MAP_SWIZZLE_128B): row r of a tile is 128
+// bytes (16 doubles); its 16-byte chunk c sits at chunk position c ^ (r & 7).  A fragment (8 rows x 4 k) is read
+// conflict-free when the 4 rows of each half-warp have distinct (r & 7) >> 1, so lane group g of a fragment reads row
+// perm(g) = (0,2,4,6,1,3,5,7)[g] of the fragment's 8 rows; the accumulator rows / columns are permuted accordingly
+// when the tile is stored.
 #include "kernels.cuh"
 
 namespace hpsi {
 
 // ----------------------------------------------------------------------------------------------- PTX helpers
-__device__ __forceinline__ void cp_async_chunk16(uint32_t dst, const void* src, int bytes) {
-  asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n" ::"r"(dst), "l"(src), "r"(bytes) : "memory");
-}
 __device__ __forceinline__ void cp_async_chunk8(uint32_t dst, const void* src, int bytes) {
   asm volatile("cp.async.ca.shared.global [%0], [%1], 8, %2;\n" ::"r"(dst), "l"(src), "r"(bytes) : "memory");
 }
@@ -27,6 +33,10 @@ __device__ __forceinline__ void mbar_init(uint32_t bar, int count) {
 }
 __device__ __forceinline__ void mbar_arrive(uint32_t bar) {
   asm volatile("{\n .reg .b64 st;\n mbarrier.arrive.shared::cta.b64 st, [%0];\n}\n" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(uint32_t bar, uint32_t bytes) {
+  asm volatile("{\n .reg .b64 st;\n mbarrier.arrive.expect_tx.shared::cta.b64 st, [%0], %1;\n}\n" ::"r"(bar), "r"(bytes)
+               : "memory");
 }
 // arrive on `bar` once all cp.async issued so far by this thread have landed (does not change the pending count)
 __device__ __forceinline__ void cp_async_mbar_arrive(uint32_t bar) {
@@ -44,6 +54,13 @@ __device__ __forceinline__ bool mbar_try_wait(uint32_t bar, uint32_t parity) {
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
   while (!mbar_try_wait(bar, parity)) {}
 }
+// TMA tile load: box of the tensor map at column c0 (K index), row c1 -> shared memory, completes on `bar`
+__device__ __forceinline__ void tma_load_2d(uint32_t dst, const void* tmap, int c0, int c1, uint32_t bar) {
+  asm volatile(
+      "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];\n" ::"r"(dst),
+      "l"(tmap), "r"(c0), "r"(c1), "r"(bar)
+      : "memory");
+}
 
 // D(8x8) += A(8x4,row) * B(4x8,col): lane L, g=L>>2, q=L&3 holds a=A[g][q], b=B[q][g], c0,c1=C[g][2q],C[g][2q+1].
 __device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double b) {
@@ -52,41 +69,8 @@ __device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double
                : "d"(a), "d"(b));
 }
 
-// ------------------------------------------------------------------------------------------ staging (LDGSTS)
-// Stage layout per operand: [k-slab (4)][row (64)][4 doubles]; element (row, kc) at ((kc>>2)*64 + row)*4 + (kc&3).
-// A warp's fragment read (row = r0+g, kc = 4*ks+q) is then 32 consecutive doubles: conflict-free.
-// CH = doubles per cp.async (2: 16-byte chunks, needs 16-byte aligned rows; 1: 8-byte chunks, any FP64 alignment).
-// The producer warp's lane handles chunk column (lane % CPR) of rows (lane / CPR) + p * RPP.
-template <int CH>
-struct Stager {
-  static constexpr int CPR = KT / CH;            // chunks per row
-  static constexpr int RPP = 32 / CPR;           // rows per pass of the producer warp
-  static constexpr int PASSES = TILE / RPP;
-  int r0, kc;
-  uint32_t dst0;                                 // byte offset inside an operand's stage
-  __device__ __forceinline__ Stager(int lane) {
-    const int c = lane % CPR;
-    r0 = lane / CPR;
-    kc = c * CH;
-    dst0 = (uint32_t)((((kc >> 2) * TILE + r0) * 4 + (kc & 3)) * 8);
-  }
-  // rowptr(p) = pointer to (row r0 + p*RPP, k = 0) in global memory; rows >= rows_valid and k >= K are zero-filled
-  template <class RowPtr>
-  __device__ __forceinline__ void load(uint32_t s_op, RowPtr rowptr, int rows_valid, const double* safe, int kappa,
-                                       int K) const {
-    const int kcol = kappa + kc;
-    int kvalid = K - kcol;
-    kvalid = kvalid < 0 ? 0 : (kvalid > CH ? CH : kvalid);
-#pragma unroll
-    for (int p = 0; p < PASSES; ++p) {
-      const int r = r0 + p * RPP;
-      const int bytes = (r < rows_valid) ? kvalid * 8 : 0;
-      const double* src = bytes ? rowptr(p) + kcol : safe;
-      if (CH == 2) cp_async_chunk16(s_op + dst0 + p * RPP * 32, src, bytes);
-      else cp_async_chunk8(s_op + dst0 + p * RPP * 32, src, bytes);
-    }
-  }
-};
+// row (or column) of a fragment that lane group / accumulator index x in 0..7 maps to
+__device__ __forceinline__ int frag_perm(int x) { return ((x & 3) << 1) | (x >> 2); }
 
 // ------------------------------------------------------------------------------------------------- MMA core
 struct WarpTile {
@@ -103,8 +87,17 @@ struct WarpTile {
   }
 };
 
-// One staged K-tile for a warp owning MI x NJ fragments (compile-time, so no predicated DMMA and no WARPSYNC):
-// nk4 k-steps of MI*NJ DMMA.8x8x4; the fragments of step ks+1 are fetched while step ks issues.
+// Per-lane element offsets (in doubles, inside an operand tile) of the k-steps 0..3 of a fragment whose first row is
+// row 0: row perm(g), column 4*ks + q, swizzled.  Fragment i of a warp adds (w0 + 8 i) * 16.
+struct LaneOffsets {
+  int k[4];
+  __device__ __forceinline__ LaneOffsets(int lane) {
+    const int g = lane >> 2, q = lane & 3, pg = frag_perm(g);
+#pragma unroll
+    for (int ks = 0; ks < 4; ++ks) k[ks] = pg * 16 + (((2 * ks + (q >> 1)) ^ pg) << 1) + (q & 1);
+  }
+};
+
 template <int MI, int NJ>
 __device__ __forceinline__ void mma_step(const double (&a)[MI], const double (&b)[NJ], double (&acc)[4][4][2]) {
 #pragma unroll
@@ -113,56 +106,58 @@ __device__ __forceinline__ void mma_step(const double (&a)[MI], const double (&b
     for (int j = 0; j < NJ; ++j) dmma884(acc[i][j][0], acc[i][j][1], a[i], b[j]);
 }
 template <int MI, int NJ>
-__device__ __forceinline__ void load_frags(const double* px, const double* py, int ks, double (&a)[MI], double (&b)[NJ]) {
+__device__ __forceinline__ void load_frags(const double* px, const double* py, int off, double (&a)[MI], double (&b)[NJ]) {
 #pragma unroll
-  for (int i = 0; i < MI; ++i) a[i] = px[ks * TILE * 4 + i * 32];
+  for (int i = 0; i < MI; ++i) a[i] = px[off + i * 128];
 #pragma unroll
-  for (int j = 0; j < NJ; ++j) b[j] = py[ks * TILE * 4 + j * 32];
+  for (int j = 0; j < NJ; ++j) b[j] = py[off + j * 128];
 }
+// One staged K-tile for a warp owning MI x NJ fragments (compile-time, so no predicated DMMA and no WARPSYNC):
+// nk4 k-steps of MI*NJ DMMA.8x8x4; the fragments of step ks+1 are fetched while step ks issues.
+// px / py = the warp's first row of the X / Y tile of the stage.
 template <int MI, int NJ>
-__device__ __forceinline__ void mma_stage(const double* px, const double* py, double (&acc)[4][4][2], int nk4) {
+__device__ __forceinline__ void mma_stage(const double* px, const double* py, const LaneOffsets& lo,
+                                          double (&acc)[4][4][2], int nk4) {
   double a0[MI], b0[NJ], a1[MI], b1[NJ];
-  load_frags<MI, NJ>(px, py, 0, a0, b0);
+  load_frags<MI, NJ>(px, py, lo.k[0], a0, b0);
   if (nk4 == 4) {                       // the common case: straight-line, no predication, no WARPSYNC
-    load_frags<MI, NJ>(px, py, 1, a1, b1);
+    load_frags<MI, NJ>(px, py, lo.k[1], a1, b1);
     mma_step<MI, NJ>(a0, b0, acc);
-    load_frags<MI, NJ>(px, py, 2, a0, b0);
+    load_frags<MI, NJ>(px, py, lo.k[2], a0, b0);
     mma_step<MI, NJ>(a1, b1, acc);
-    load_frags<MI, NJ>(px, py, 3, a1, b1);
+    load_frags<MI, NJ>(px, py, lo.k[3], a1, b1);
     mma_step<MI, NJ>(a0, b0, acc);
     mma_step<MI, NJ>(a1, b1, acc);
   } else {                              // ragged K tail of a segment (1..3 k-steps)
     mma_step<MI, NJ>(a0, b0, acc);
-    for (int ks = 1; ks < nk4; ++ks) {
-      load_frags<MI, NJ>(px, py, ks, a0, b0);
-      mma_step<MI, NJ>(a0, b0, acc);
-    }
+    if (nk4 > 1) { load_frags<MI, NJ>(px, py, lo.k[1], a0, b0); mma_step<MI, NJ>(a0, b0, acc); }
+    if (nk4 > 2) { load_frags<MI, NJ>(px, py, lo.k[2], a0, b0); mma_step<MI, NJ>(a0, b0, acc); }
   }
 }
 
-// Store the warp's accumulators: element (row, col) of the CTA tile goes to dst[row*ld + col]; rowscale(row) multiplies.
-template <class RowScale>
-__device__ __forceinline__ void store_tile(double* dst, int ld, int rows_valid, int cols_valid,
-                                           const double (&acc)[4][4][2], const WarpTile& w, int lane, RowScale rowscale) {
-  const int g = lane >> 2, q = lane & 3;
+__device__ __forceinline__ void zero_acc(double (&acc)[4][4][2]) {
 #pragma unroll
-  for (int i = 0; i < 4; ++i) {
-    const int row = w.wr0 + 8 * i + g;
-    if (i >= w.mi || row >= rows_valid) continue;
-    const double sc = rowscale(row);
+  for (int i = 0; i < 4; ++i)
+#pragma unroll
+    for (int j = 0; j < 4; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
+}
+
+// Store the warp's accumulators: element (row, col) of the CTA tile goes to dst[row*ld + col], scaled by sc.
+// acc[i][j][e] holds tile row wr0 + 8i + perm(g) and tile column wc0 + 8j + perm(2q + e)  (perm(2q+1) = perm(2q) + 2).
+template <int MI, int NJ>
+__device__ __forceinline__ void store_tile(double* dst, int ld, int rows_valid, int cols_valid,
+                                           const double (&acc)[4][4][2], const WarpTile& w, int lane, double sc) {
+  const int pg = frag_perm(lane >> 2), pc = frag_perm(2 * (lane & 3));
+#pragma unroll
+  for (int i = 0; i < MI; ++i) {
+    const int row = w.wr0 + 8 * i + pg;
+    if (row >= rows_valid) continue;
     double* drow = dst + (int64_t)row * ld;
 #pragma unroll
-    for (int j = 0; j < 4; ++j) {
-      const int col = w.wc0 + 8 * j + 2 * q;
-      if (j >= w.nj || col >= cols_valid) continue;
-      const double v0 = acc[i][j][0] * sc, v1 = acc[i][j][1] * sc;
-      double* p = drow + col;
-      if (col + 1 < cols_valid) {
-        if ((reinterpret_cast<uintptr_t>(p) & 15) == 0) *reinterpret_cast<double2*>(p) = make_double2(v0, v1);
-        else { p[0] = v0; p[1] = v1; }
-      } else {
-        p[0] = v0;
-      }
+    for (int j = 0; j < NJ; ++j) {
+      const int col = w.wc0 + 8 * j + pc;
+      if (col < cols_valid) drow[col] = acc[i][j][0] * sc;
+      if (col + 2 < cols_valid) drow[col + 2] = acc[i][j][1] * sc;
     }
   }
 }
@@ -172,126 +167,148 @@ __device__ __forceinline__ void store_tile(double* dst, int ld, int rows_valid, 
 // quadrant on the same sub-partition.  CTAs are dealt to SMs round-robin (148 = 0 mod 4), hence a hash, not bid & 3.
 __device__ __forceinline__ int quadrant_rotation(unsigned bid) { return (int)((bid * 2654435761u) >> 30); }
 
-// Shared-memory carve-up: NSTAGE stages of [X tile | Y tile], then the barriers and (P1) the row-pointer table.
+// Shared-memory carve-up: NSTAGE stages of [X tile | Y tile] (1024-byte aligned), then the barriers.
 struct SmemLayout {
-  uint32_t base;                                   // shared-window address of stage 0
-  __device__ __forceinline__ uint32_t stage(int s) const { return base + s * STAGE_DOUBLES * 8; }
-  __device__ __forceinline__ uint32_t full(int s) const { return base + NSTAGE * STAGE_DOUBLES * 8 + s * 8; }
-  __device__ __forceinline__ uint32_t empty(int s) const { return base + NSTAGE * STAGE_DOUBLES * 8 + (NSTAGE + s) * 8; }
+  uint32_t base;                                   // shared-window address of stage 0 (1024-byte aligned)
+  const double* gen;                               // generic pointer to the same byte
+  __device__ __forceinline__ SmemLayout(const void* raw) {
+    const uint32_t r = (uint32_t)__cvta_generic_to_shared(raw);
+    base = (r + 1023u) & ~1023u;
+    gen = reinterpret_cast<const double*>(static_cast<const char*>(raw) + (base - r));
+  }
+  __device__ __forceinline__ uint32_t stage(int s) const { return base + s * STAGE_BYTES; }
+  __device__ __forceinline__ const double* stage_ptr(int s) const { return gen + s * (STAGE_BYTES / 8); }
+  __device__ __forceinline__ uint32_t full(int s) const { return base + NSTAGE * STAGE_BYTES + s * 8; }
+  __device__ __forceinline__ uint32_t empty(int s) const { return base + NSTAGE * STAGE_BYTES + (NSTAGE + s) * 8; }
 };
+// TMA: the full barrier takes the producer's arrive.expect_tx plus the bytes; LDGSTS: one deferred arrive per lane.
+template <bool TMA>
 __device__ __forceinline__ void init_barriers(const SmemLayout& sm, int tid) {
   if (tid == 0) {
-    for (int s = 0; s < NSTAGE; ++s) { mbar_init(sm.full(s), 32); mbar_init(sm.empty(s), NCONS); }
+    for (int s = 0; s < NSTAGE; ++s) { mbar_init(sm.full(s), TMA ? 1 : 32); mbar_init(sm.empty(s), NCONS); }
     asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
   }
   __syncthreads();
 }
 
+// position in the stage ring
+struct Ring {
+  int stage;
+  uint32_t phase;
+  __device__ __forceinline__ void advance() { if (++stage == NSTAGE) { stage = 0; phase ^= 1; } }
+};
 
-// Consumer main loop for a warp owning MI x NJ fragments.  seq.next() returns the number of k-steps (1..4) of the
-// next staged K-tile, or 0 when the unit is done.  Idle warps (MI == 0) only hand the stages back.
-template <int MI, int NJ, class Seq>
-__device__ __forceinline__ void consume(const double* smem, const SmemLayout& sm, Seq& seq, double (&acc)[4][4][2],
-                                        const WarpTile& w, int lane, bool skip_mma) {
-  int stage = 0;
-  uint32_t phase = 0;
-  const int xoff = w.wr0 * 4 + lane, yoff = 4 * TILE * 4 + w.wc0 * 4 + lane;
-  for (int nk4 = seq.next(); nk4 > 0; nk4 = seq.next()) {
-    mbar_wait(sm.full(stage), phase);
-    if (MI > 0 && !skip_mma) {
-      const double* st = smem + stage * STAGE_DOUBLES;
-      mma_stage<(MI > 0 ? MI : 1), (NJ > 0 ? NJ : 1)>(st + xoff, st + yoff, acc, nk4);
-    }
-    __syncwarp();
-    if (lane == 0) mbar_arrive(sm.empty(stage));
-    if (++stage == NSTAGE) { stage = 0; phase ^= 1; }
+// ------------------------------------------------------------------------------------------ LDGSTS staging
+// Fallback for matrices with 8-byte aligned rows: the producer warp copies a rows_valid x (K - kappa, at most 16)
+// piece with 8-byte cp.async into the swizzled layout; everything else of the 64 x 16 tile is zero-filled.
+// Lane handles column (lane & 15) of rows (lane >> 4) + 2 p.
+__device__ __forceinline__ void ldgsts_tile(uint32_t s_op, const double* rows, int64_t ld, int rows_valid, int kappa, int K,
+                                            int lane) {
+  const int kc = lane & 15, r0 = lane >> 4;
+  const bool kvalid = kappa + kc < K;
+#pragma unroll 8
+  for (int p = 0; p < TILE / 2; ++p) {
+    const int r = r0 + 2 * p;
+    const bool ok = kvalid && r < rows_valid;
+    const double* src = ok ? rows + r * ld + kappa + kc : rows;
+    const uint32_t dst = s_op + r * 128 + ((((kc >> 1) ^ (r & 7)) << 4) | ((kc & 1) << 3));
+    cp_async_chunk8(dst, src, ok ? 8 : 0);
   }
-}
-
-template <class Seq>
-__device__ __forceinline__ void consume_dispatch(const double* smem, const SmemLayout& sm, Seq& seq,
-                                                 double (&acc)[4][4][2], const WarpTile& w, int lane, bool skip_mma) {
-#define HPSI_CASE(MI, NJ) case MI * 5 + NJ: consume<MI, NJ>(smem, sm, seq, acc, w, lane, skip_mma); break;
-  switch ((w.nj > 0 ? w.mi : 0) * 5 + (w.mi > 0 ? w.nj : 0)) {
-    HPSI_CASE(1, 1) HPSI_CASE(1, 2) HPSI_CASE(1, 3) HPSI_CASE(1, 4)
-    HPSI_CASE(2, 1) HPSI_CASE(2, 2) HPSI_CASE(2, 3) HPSI_CASE(2, 4)
-    HPSI_CASE(3, 1) HPSI_CASE(3, 2) HPSI_CASE(3, 3) HPSI_CASE(3, 4)
-    HPSI_CASE(4, 1) HPSI_CASE(4, 2) HPSI_CASE(4, 3) HPSI_CASE(4, 4)
-    default: consume<0, 0>(smem, sm, seq, acc, w, lane, skip_mma); break;
-  }
-#undef HPSI_CASE
 }
 
 // ------------------------------------------------------------------------------------------------ P1 kernel
-// One CTA = one P1Unit: C[R0.., j0..] = coef(row) * sum_k X[R,k] Y[j,k], X rows stacked over the group's terms
-// (order 1: A_t rows; order 2: B_t rows), Y = padded psi^T (order 1) or padded psi (order 2) block of the source.
-template <int CH>
+// One CTA = one P1Unit: for each term t of the unit, T_t[i0.., j0..] = coef_t * sum_k X_t[i,k] Y[j,k] with
+// X_t = the term's operator block (order 1: A_t, order 2: B_t) and Y = padded psi^T (order 1) or padded psi
+// (order 2) block of the source.  The stage ring runs across the terms.
+template <int MI, int NJ>
+__device__ __forceinline__ void p1_consume(const DevSchedule& d, const P1Unit& u, const Group& g, const SmemLayout& sm,
+                                           const WarpTile& w, int lane) {
+  double acc[4][4][2];
+  const LaneOffsets lo(lane);
+  const int ntiles = (g.K1 + KT - 1) / KT;
+  const int last_nk4 = ((g.K1 - (ntiles - 1) * KT) + 3) >> 2;
+  Ring ring{0, 0};
+  for (int t = u.t0; t < u.t1; ++t) {
+    zero_acc(acc);
+    for (int kt = 0; kt < ntiles; ++kt) {
+      mbar_wait(sm.full(ring.stage), ring.phase);
+      if (MI > 0 && d.debug != 2) {
+        const double* st = sm.stage_ptr(ring.stage);
+        mma_stage<(MI > 0 ? MI : 1), (NJ > 0 ? NJ : 1)>(st + w.wr0 * 16, st + OP_BYTES / 8 + w.wc0 * 16, lo, acc,
+                                                          kt == ntiles - 1 ? last_nk4 : 4);
+      }
+      __syncwarp();
+      if (lane == 0) mbar_arrive(sm.empty(ring.stage));
+      ring.advance();
+    }
+    if (MI > 0) {
+      double* dst = d.ws + g.ws_off + ((int64_t)t * g.rows + u.i0) * g.ldw + u.j0;
+      store_tile<(MI > 0 ? MI : 1), (NJ > 0 ? NJ : 1)>(dst, g.ldw, u.rows_valid, u.cols_valid, acc, w, lane,
+                                                        d.segs[g.seg0 + t].coef);
+    }
+  }
+}
+
+template <bool TMA>
 __global__ void __launch_bounds__(NTHREADS, 3) p1_kernel(DevSchedule d) {
-  extern __shared__ __align__(16) double smem[];
+  extern __shared__ __align__(16) unsigned char smem_raw[];
   const P1Unit u = d.p1[blockIdx.x];
   const Group g = d.groups[u.group];
   const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
-  SmemLayout sm{(uint32_t)__cvta_generic_to_shared(smem)};
-  const double** rowtab = reinterpret_cast<const double**>(smem + NSTAGE * STAGE_DOUBLES + 2 * NSTAGE);
-  init_barriers(sm, tid);
+  const SmemLayout sm(smem_raw);
+  init_barriers<TMA>(sm, tid);
   const int ntiles = (g.K1 + KT - 1) / KT;
 
   if (wid == NCONS) {
     // ---------------- producer warp
-    const double* xbase = (g.order == 1) ? d.a : d.b;
+    Ring ring{0, 1};
+    const unsigned char* ymap = d.maps + (int64_t)g.y1_map * TMAP_BYTES;
     const double* ybase = d.ws + g.y1_off + (int64_t)u.j0 * g.ldy1;
-    for (int r = lane; r < TILE; r += 32) {                 // row-pointer table of the stacked X rows
-      const double* ptr = ybase;
-      if (r < u.rows_valid) {
-        const int R = u.R0 + r;
-        const int ti = R / g.rows, x = R - ti * g.rows;
-        const Seg* sg = d.segs + g.seg0 + ti;
-        ptr = xbase + sg->p1_off + (int64_t)x * sg->p1_ld;
+    const double* xarena = (g.order == 1) ? d.a : d.b;
+    for (int t = u.t0; t < u.t1; ++t) {
+      const Seg* sg = d.segs + g.seg0 + t;
+      const unsigned char* xmap = nullptr;
+      const double* xbase = nullptr;
+      int64_t xld = 0;
+      if (TMA) xmap = d.maps + (int64_t)sg->p1_map * TMAP_BYTES;
+      else { xld = sg->p1_ld; xbase = xarena + sg->p1_off + (int64_t)u.i0 * xld; }
+      for (int kt = 0; kt < ntiles; ++kt) {
+        mbar_wait(sm.empty(ring.stage), ring.phase);
+        const uint32_t sx = sm.stage(ring.stage), sy = sx + OP_BYTES, full = sm.full(ring.stage);
+        if (TMA) {
+          if (lane == 0) {
+            mbar_arrive_expect_tx(full, d.debug == 1 ? 0 : STAGE_BYTES);
+            if (d.debug != 1) {
+              tma_load_2d(sx, xmap, kt * KT, u.i0, full);
+              tma_load_2d(sy, ymap, kt * KT, u.j0, full);
+            }
+          }
+        } else {
+          if (d.debug != 1) {
+            ldgsts_tile(sx, xbase, xld, u.rows_valid, kt * KT, g.K1, lane);
+            ldgsts_tile(sy, ybase, g.ldy1, u.cols_valid, kt * KT, g.K1, lane);
+          }
+          cp_async_mbar_arrive(full);
+        }
+        ring.advance();
       }
-      rowtab[r] = ptr;
     }
-    __syncwarp();
-    const Stager<CH> st(lane);
-    const double* yrow0 = ybase + (int64_t)st.r0 * g.ldy1;
-    const int64_t ystep = (int64_t)Stager<CH>::RPP * g.ldy1;
-    int stage = 0;
-    uint32_t phase = 1;
-    for (int t = 0; t < ntiles; ++t) {
-      mbar_wait(sm.empty(stage), phase);
-      const uint32_t sx = sm.stage(stage), sy = sx + 4 * TILE * 4 * 8;
-      if (d.debug != 1) {
-        st.load(sx, [&](int p) { return rowtab[st.r0 + p * Stager<CH>::RPP]; }, u.rows_valid, ybase, t * KT, g.K1);
-        st.load(sy, [&](int p) { return yrow0 + p * ystep; }, u.cols_valid, ybase, t * KT, g.K1);
-      }
-      cp_async_mbar_arrive(sm.full(stage));
-      if (++stage == NSTAGE) { stage = 0; phase ^= 1; }
-    }
-    cp_async_wait_all();
+    if (!TMA) cp_async_wait_all();
     return;
   }
 
   // ------------------ consumer warps
   const int warp = (wid + quadrant_rotation(blockIdx.x)) & 3;
   const WarpTile w(warp, u.rows_valid, u.cols_valid);
-  double acc[4][4][2];
-#pragma unroll
-  for (int i = 0; i < 4; ++i)
-#pragma unroll
-    for (int j = 0; j < 4; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
-  struct Seq1 {
-    int K, t;
-    __device__ __forceinline__ int next() {
-      int n = (K - t * KT + 3) >> 2;
-      ++t;
-      return n > 4 ? 4 : (n < 0 ? 0 : n);
-    }
-  } seq{g.K1, 0};
-  consume_dispatch(smem, sm, seq, acc, w, lane, d.debug == 2);
-  double* dst = d.ws + g.ws_off + (int64_t)u.R0 * g.ldw + u.j0;
-  store_tile(dst, g.ldw, u.rows_valid, u.cols_valid, acc, w, lane, [&](int row) {
-    const int ti = (u.R0 + row) / g.rows;
-    return d.segs[g.seg0 + ti].coef;
-  });
+#define HPSI_CASE(MI, NJ) case MI * 5 + NJ: p1_consume<MI, NJ>(d, u, g, sm, w, lane); break;
+  switch ((w.nj > 0 ? w.mi : 0) * 5 + (w.mi > 0 ? w.nj : 0)) {
+    HPSI_CASE(1, 1) HPSI_CASE(1, 2) HPSI_CASE(1, 3) HPSI_CASE(1, 4)
+    HPSI_CASE(2, 1) HPSI_CASE(2, 2) HPSI_CASE(2, 3) HPSI_CASE(2, 4)
+    HPSI_CASE(3, 1) HPSI_CASE(3, 2) HPSI_CASE(3, 3) HPSI_CASE(3, 4)
+    HPSI_CASE(4, 1) HPSI_CASE(4, 2) HPSI_CASE(4, 3) HPSI_CASE(4, 4)
+    default: p1_consume<0, 0>(d, u, g, sm, w, lane); break;
+  }
+#undef HPSI_CASE
 }
 
 // ------------------------------------------------------------------------------------------------ P2 kernel
@@ -299,11 +316,10 @@ __global__ void __launch_bounds__(NTHREADS, 3) p1_kernel(DevSchedule d) {
 // (order 1: X = T_t from the workspace, Y = B_t; order 2: X = A_t, Y = U_t^T from the workspace).
 struct KIter {                 // walks (run, seg, kappa) in K-tile steps
   const Run* runs;
-  int run, run_end, seg, seg_end, K, kappa, ldw, order;
+  int run, run_end, seg, seg_end, K, kappa;
   bool valid;
   __device__ __forceinline__ void open_run() {
-    const Run r = runs[run];
-    seg = r.seg_begin; seg_end = r.seg_end; K = r.K; ldw = r.ldw; order = r.order; kappa = 0;
+    seg = runs[run].seg_begin; seg_end = runs[run].seg_end; K = runs[run].K; kappa = 0;
   }
   __device__ __forceinline__ KIter(const Run* runs_, int rb, int re) : runs(runs_), run(rb), run_end(re) {
     valid = rb < re;
@@ -322,78 +338,103 @@ struct KIter {                 // walks (run, seg, kappa) in K-tile steps
   __device__ __forceinline__ int nk4() const { int n = (K - kappa + 3) >> 2; return n > 4 ? 4 : n; }
 };
 
-template <int CH>
+template <int MI, int NJ>
+__device__ __forceinline__ void p2_consume(const DevSchedule& d, const P2Unit& u, const SmemLayout& sm,
+                                           const WarpTile& w, int lane) {
+  double acc[4][4][2];
+  zero_acc(acc);
+  const LaneOffsets lo(lane);
+  Ring ring{0, 0};
+  for (KIter it(d.runs, u.run_begin, u.run_end); it.valid; it.advance()) {
+    mbar_wait(sm.full(ring.stage), ring.phase);
+    if (MI > 0 && d.debug != 2) {
+      const double* st = sm.stage_ptr(ring.stage);
+      mma_stage<(MI > 0 ? MI : 1), (NJ > 0 ? NJ : 1)>(st + w.wr0 * 16, st + OP_BYTES / 8 + w.wc0 * 16, lo, acc, it.nk4());
+    }
+    __syncwarp();
+    if (lane == 0) mbar_arrive(sm.empty(ring.stage));
+    ring.advance();
+  }
+  if (MI > 0)
+    store_tile<(MI > 0 ? MI : 1), (NJ > 0 ? NJ : 1)>(d.ws + u.out_off, u.ldo, u.rows_valid, u.cols_valid, acc, w, lane, 1.0);
+}
+
+template <bool TMA>
 __global__ void __launch_bounds__(NTHREADS, 3) p2_kernel(DevSchedule d) {
-  extern __shared__ __align__(16) double smem[];
+  extern __shared__ __align__(16) unsigned char smem_raw[];
   const P2Unit u = d.p2[blockIdx.x];
   const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
-  SmemLayout sm{(uint32_t)__cvta_generic_to_shared(smem)};
-  init_barriers(sm, tid);
-  KIter it(d.runs, u.run_begin, u.run_end);
+  const SmemLayout sm(smem_raw);
+  init_barriers<TMA>(sm, tid);
 
   if (wid == NCONS) {
     // ---------------- producer warp
-    const Stager<CH> st(lane);
-    const double *xrow0 = nullptr, *yrow0 = nullptr, *xsafe = nullptr, *ysafe = nullptr;
-    int64_t xstep = 0, ystep = 0;
+    KIter it(d.runs, u.run_begin, u.run_end);
+    Ring ring{0, 1};
+    const unsigned char *xmap = nullptr, *ymap = nullptr;      // TMA: tensor maps and first rows of the segment
+    int xrow = 0, yrow = 0;
+    const double *xbase = nullptr, *ybase = nullptr;           // LDGSTS: first rows and leading dimensions
+    int64_t xld = 0, yld = 0;
     auto open_seg = [&]() {
+      const Run r = d.runs[it.run];
       const Seg* sg = d.segs + it.seg;
-      const int64_t p2_off = sg->p2_off, ws_off = sg->ws_off;
-      const int p2_ld = sg->p2_ld;
-      if (it.order == 1) {
-        xsafe = d.ws + ws_off + (int64_t)u.i0 * it.ldw;
-        xrow0 = xsafe + (int64_t)st.r0 * it.ldw;
-        xstep = (int64_t)Stager<CH>::RPP * it.ldw;
-        ysafe = d.b + p2_off + (int64_t)u.j0 * p2_ld;
-        yrow0 = ysafe + (int64_t)st.r0 * p2_ld;
-        ystep = (int64_t)Stager<CH>::RPP * p2_ld;
+      const int trow = (it.seg - r.seg0) * r.rows;             // first row of the task inside the stacked intermediate
+      if (TMA) {
+        const unsigned char* opmap = d.maps + (int64_t)sg->p2_map * TMAP_BYTES;
+        const unsigned char* wsmap = d.maps + (int64_t)r.ws_map * TMAP_BYTES;
+        if (r.order == 1) { xmap = wsmap; xrow = trow + u.i0; ymap = opmap; yrow = u.j0; }
+        else              { xmap = opmap; xrow = u.i0; ymap = wsmap; yrow = trow + u.j0; }
       } else {
-        xsafe = d.a + p2_off + (int64_t)u.i0 * p2_ld;
-        xrow0 = xsafe + (int64_t)st.r0 * p2_ld;
-        xstep = (int64_t)Stager<CH>::RPP * p2_ld;
-        ysafe = d.ws + ws_off + (int64_t)u.j0 * it.ldw;
-        yrow0 = ysafe + (int64_t)st.r0 * it.ldw;
-        ystep = (int64_t)Stager<CH>::RPP * it.ldw;
+        const double* wsrows = d.ws + r.ws_off + (int64_t)trow * r.ldw;
+        if (r.order == 1) {
+          xld = r.ldw; xbase = wsrows + (int64_t)u.i0 * xld;
+          yld = sg->p2_ld; ybase = d.b + sg->p2_off + (int64_t)u.j0 * yld;
+        } else {
+          xld = sg->p2_ld; xbase = d.a + sg->p2_off + (int64_t)u.i0 * xld;
+          yld = r.ldw; ybase = wsrows + (int64_t)u.j0 * yld;
+        }
       }
     };
     if (it.valid) open_seg();
-    int stage = 0;
-    uint32_t phase = 1;
     while (it.valid) {
-      mbar_wait(sm.empty(stage), phase);
-      const uint32_t sx = sm.stage(stage), sy = sx + 4 * TILE * 4 * 8;
-      if (d.debug != 1) {
-        st.load(sx, [&](int p) { return xrow0 + p * xstep; }, u.rows_valid, xsafe, it.kappa, it.K);
-        st.load(sy, [&](int p) { return yrow0 + p * ystep; }, u.cols_valid, ysafe, it.kappa, it.K);
+      mbar_wait(sm.empty(ring.stage), ring.phase);
+      const uint32_t sx = sm.stage(ring.stage), sy = sx + OP_BYTES, full = sm.full(ring.stage);
+      if (TMA) {
+        if (lane == 0) {
+          mbar_arrive_expect_tx(full, d.debug == 1 ? 0 : STAGE_BYTES);
+          if (d.debug != 1) {
+            tma_load_2d(sx, xmap, it.kappa, xrow, full);
+            tma_load_2d(sy, ymap, it.kappa, yrow, full);
+          }
+        }
+      } else {
+        if (d.debug != 1) {
+          ldgsts_tile(sx, xbase, xld, u.rows_valid, it.kappa, it.K, lane);
+          ldgsts_tile(sy, ybase, yld, u.cols_valid, it.kappa, it.K, lane);
+        }
+        cp_async_mbar_arrive(full);
       }
-      cp_async_mbar_arrive(sm.full(stage));
       if (it.advance()) open_seg();
-      if (++stage == NSTAGE) { stage = 0; phase ^= 1; }
+      ring.advance();
     }
-    cp_async_wait_all();
+    if (!TMA) cp_async_wait_all();
     return;
   }
 
   // ------------------ consumer warps
   const int warp = (wid + quadrant_rotation(blockIdx.x)) & 3;
   const WarpTile w(warp, u.rows_valid, u.cols_valid);
-  double acc[4][4][2];
-#pragma unroll
-  for (int i = 0; i < 4; ++i)
-#pragma unroll
-    for (int j = 0; j < 4; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
-  struct Seq2 {
-    KIter& it;
-    __device__ __forceinline__ int next() {
-      if (!it.valid) return 0;
-      const int n = it.nk4();
-      it.advance();
-      return n;
-    }
-  } seq{it};
-  consume_dispatch(smem, sm, seq, acc, w, lane, d.debug == 2);
-  store_tile(d.ws + u.out_off, u.ldo, u.rows_valid, u.cols_valid, acc, w, lane, [](int) { return 1.0; });
+#define HPSI_CASE(MI, NJ) case MI * 5 + NJ: p2_consume<MI, NJ>(d, u, sm, w, lane); break;
+  switch ((w.nj > 0 ? w.mi : 0) * 5 + (w.mi > 0 ? w.nj : 0)) {
+    HPSI_CASE(1, 1) HPSI_CASE(1, 2) HPSI_CASE(1, 3) HPSI_CASE(1, 4)
+    HPSI_CASE(2, 1) HPSI_CASE(2, 2) HPSI_CASE(2, 3) HPSI_CASE(2, 4)
+    HPSI_CASE(3, 1) HPSI_CASE(3, 2) HPSI_CASE(3, 3) HPSI_CASE(3, 4)
+    HPSI_CASE(4, 1) HPSI_CASE(4, 2) HPSI_CASE(4, 3) HPSI_CASE(4, 4)
+    default: p2_consume<0, 0>(d, u, sm, w, lane); break;
+  }
+#undef HPSI_CASE
 }
+
 // ------------------------------------------------------------------------------- prep / reduce / diag kernels
 // prep: psi block (rows x cols, dense) -> padded copy (rows x ldp) and padded transpose (cols x ldt) in the workspace.
 __global__ void prep_kernel(DevSchedule d, const double* __restrict__ psi) {
@@ -440,10 +481,10 @@ __global__ void diag_kernel(DevSchedule d, double* __restrict__ diag) {
 // -------------------------------------------------------------------------------------------------- launchers
 cudaError_t kernels_init() {
   cudaError_t e;
-  if ((e = cudaFuncSetAttribute(p1_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES))) return e;
-  if ((e = cudaFuncSetAttribute(p1_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES))) return e;
-  if ((e = cudaFuncSetAttribute(p2_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES))) return e;
-  if ((e = cudaFuncSetAttribute(p2_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES))) return e;
+  if ((e = cudaFuncSetAttribute(p1_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES))) return e;
+  if ((e = cudaFuncSetAttribute(p1_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES))) return e;
+  if ((e = cudaFuncSetAttribute(p2_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES))) return e;
+  if ((e = cudaFuncSetAttribute(p2_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES))) return e;
   return cudaSuccess;
 }
 
@@ -457,15 +498,15 @@ static dim3 elem_grid(const DevSchedule& d) {
 void launch_prep(const DevSchedule& d, const double* psi, cudaStream_t st) {
   if (d.n_blocks > 0) prep_kernel<<<elem_grid(d), 256, 0, st>>>(d, psi);
 }
-void launch_p1(const DevSchedule& d, bool aligned16, cudaStream_t st) {
+void launch_p1(const DevSchedule& d, bool tma, cudaStream_t st) {
   if (d.n_p1 == 0) return;
-  if (aligned16) p1_kernel<2><<<d.n_p1, NTHREADS, SMEM_BYTES, st>>>(d);
-  else p1_kernel<1><<<d.n_p1, NTHREADS, SMEM_BYTES, st>>>(d);
+  if (tma) p1_kernel<true><<<d.n_p1, NTHREADS, SMEM_BYTES, st>>>(d);
+  else p1_kernel<false><<<d.n_p1, NTHREADS, SMEM_BYTES, st>>>(d);
 }
-void launch_p2(const DevSchedule& d, bool aligned16, cudaStream_t st) {
+void launch_p2(const DevSchedule& d, bool tma, cudaStream_t st) {
   if (d.n_p2 == 0) return;
-  if (aligned16) p2_kernel<2><<<d.n_p2, NTHREADS, SMEM_BYTES, st>>>(d);
-  else p2_kernel<1><<<d.n_p2, NTHREADS, SMEM_BYTES, st>>>(d);
+  if (tma) p2_kernel<true><<<d.n_p2, NTHREADS, SMEM_BYTES, st>>>(d);
+  else p2_kernel<false><<<d.n_p2, NTHREADS, SMEM_BYTES, st>>>(d);
 }
 void launch_reduce(const DevSchedule& d, double* out, cudaStream_t st) {
   if (d.n_blocks > 0) reduce_kernel<<<elem_grid(d), 256, 0, st>>>(d, out);

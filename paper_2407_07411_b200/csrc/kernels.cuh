@@ -1,6 +1,8 @@
 // sm_100a kernels of hpsi_apply.  FP64 tensor path = mma.sync.m8n8k4.f64 (SASS DMMA.8x8x4), the only FP64 MMA
-// sm_100a has (tcgen05 has no f64 kind); operands staged HBM/L2 -> shared memory with cp.async (LDGSTS),
-// accumulators in registers.  One CTA = 1 producer warp + 2x2 consumer warps on a <=64x64 tile (<=4x4 fragments each).
+// sm_100a has (tcgen05 has no f64 kind), accumulators in registers.  Operands are staged into shared memory by the
+// TMA unit (cp.async.bulk.tensor.2d with one tensor map per operand matrix, 128-byte swizzle, zero fill out of
+// bounds) when every block has 16-byte aligned rows; otherwise by 8-byte cp.async (LDGSTS) into the same layout.
+// One CTA = 1 producer warp + 2x2 consumer warps on a <=64x64 tile (<=4x4 fragments each).
 #pragma once
 #include <cuda_runtime.h>
 
@@ -9,12 +11,13 @@
 namespace hpsi {
 
 constexpr int NCONS = 4;                       // consumer (DMMA) warps per CTA, 2 x 2 over the tile
-constexpr int NTHREADS = (NCONS + 1) * 32;     // + 1 producer (cp.async) warp
+constexpr int NTHREADS = (NCONS + 1) * 32;     // + 1 producer warp
 constexpr int NSTAGE = 4;
-// one stage: X[4 k-slabs][64 rows][4] and Y[4][64][4] doubles = 2 * 8 KB
-constexpr int STAGE_DOUBLES = 2 * 4 * TILE * 4;
-// stages | full[NSTAGE], empty[NSTAGE] mbarriers | 64 row pointers (P1)
-constexpr int SMEM_BYTES = NSTAGE * STAGE_DOUBLES * 8 + 2 * NSTAGE * 8 + TILE * 8;
+constexpr int OP_BYTES = TILE * KT * 8;        // one operand tile of a stage: 64 rows x 128 bytes, 128-byte swizzled
+constexpr int STAGE_BYTES = 2 * OP_BYTES;      // X tile | Y tile
+// 1024 bytes of slack to align the stages (the swizzle pattern is a function of address bits 4-9) | stages | barriers
+constexpr int SMEM_BYTES = 1024 + NSTAGE * STAGE_BYTES + 2 * NSTAGE * 8;
+constexpr int TMAP_BYTES = 128;                // sizeof(CUtensorMap)
 
 struct DevSchedule {           // device pointers to the uploaded tables
   const PsiBlk* blocks;
@@ -24,6 +27,7 @@ struct DevSchedule {           // device pointers to the uploaded tables
   const Run* runs;
   const P2Unit* p2;
   const DiagTask* diag;
+  const unsigned char* maps;   // CUtensorMap[sc.maps.size()], 128 bytes each (TMA staging only)
   double* ws;
   const double* a;
   const double* b;
@@ -33,8 +37,8 @@ struct DevSchedule {           // device pointers to the uploaded tables
 };
 
 void launch_prep(const DevSchedule& d, const double* psi, cudaStream_t st);
-void launch_p1(const DevSchedule& d, bool aligned16, cudaStream_t st);
-void launch_p2(const DevSchedule& d, bool aligned16, cudaStream_t st);
+void launch_p1(const DevSchedule& d, bool tma, cudaStream_t st);
+void launch_p2(const DevSchedule& d, bool tma, cudaStream_t st);
 void launch_reduce(const DevSchedule& d, double* out, cudaStream_t st);
 void launch_diag(const DevSchedule& d, double* diag, cudaStream_t st);
 cudaError_t kernels_init();    // opt-in to >48 KB dynamic shared memory

@@ -27,8 +27,8 @@ enum BaseSel : int32_t { BASE_A = 0, BASE_B = 1, BASE_WS = 2 };
 struct Seg {                  // one task, in schedule order (by destination, source, term)
   int64_t p1_off;             // operator block used by P1 (order 1: A_t, order 2: B_t), doubles into its arena
   int64_t p2_off;             // operator block used by P2 (order 1: B_t, order 2: A_t)
-  int64_t ws_off;             // start of this task's intermediate (rows x ldw) in the workspace
   int32_t p1_ld, p2_ld;       // leading dimensions of those blocks
+  int32_t p1_map, p2_map;     // tensor-map ids of those blocks (TMA staging)
   double coef;                // per-task coefficient (initialised to c_t; reading A4)
 };
 
@@ -42,13 +42,16 @@ struct Group {
   int32_t ldw;                // leading dimension of the intermediate (N1 rounded up to a multiple of 4)
   int32_t ldy1;               // leading dimension of the P1 Y operand (padded psi^T or psi block)
   int64_t y1_off;             // its offset in the workspace
-  int64_t ws_off;             // start of the stacked intermediate  [(tcount*rows) x ldw]
+  int64_t ws_off;             // start of the stacked intermediate  [(tcount*rows) x ldw]; task t starts at row t*rows
+  int32_t y1_map;             // tensor map of the P1 Y operand
+  int32_t ws_map;             // tensor map of the stacked intermediate
   int32_t src, dst;           // psi block indices
 };
 
-struct P1Unit {               // one CTA of the first-GEMM kernel
+struct P1Unit {               // one CTA of the first-GEMM kernel: one tile position, a range of the group's terms
   int32_t group;
-  int32_t R0, rows_valid;     // stacked-row tile
+  int32_t t0, t1;             // terms [t0, t1) of the group, processed one after the other (pipeline never drains)
+  int32_t i0, rows_valid;     // row tile inside one task's intermediate
   int32_t j0, cols_valid;     // column tile
   int32_t pad;
 };
@@ -58,7 +61,10 @@ struct Run {                  // consecutive segs of one group inside one P2 uni
   int32_t K;                  // segment length (group.N1)
   int32_t ldw;                // ld of the intermediate operand
   int32_t order;
-  int32_t pad;
+  int32_t rows;               // rows of one task's intermediate (group.rows)
+  int32_t seg0;               // group.seg0 (seg - seg0 = task index inside the stacked intermediate)
+  int32_t ws_map;             // group.ws_map
+  int64_t ws_off;             // group.ws_off
 };
 
 struct P2Unit {               // one CTA of the second-GEMM kernel
@@ -66,6 +72,16 @@ struct P2Unit {               // one CTA of the second-GEMM kernel
   int32_t i0, rows_valid, j0, cols_valid;
   int64_t out_off;            // partial buffer offset of element (i0, j0) of this split's m x ldp tile
   int32_t ldo;
+  int32_t pad;
+};
+
+// A 2-D row-major matrix the TMA unit reads: rows x cols doubles, leading dimension ld, `off` doubles into `base`.
+// Encoded (api.cu) as a CUtensorMap with box {KT columns, box_rows rows}, 128-byte swizzle, zero fill out of bounds.
+struct MapSpec {
+  int64_t off;
+  int32_t base;               // BaseSel
+  int32_t rows, cols, ld;
+  int32_t box_rows;
   int32_t pad;
 };
 
@@ -78,6 +94,7 @@ struct PsiBlk {               // one psi block and its padded copies
   int32_t nsplit, ldo;
   int32_t left, right;
   int32_t diag0, diag1;       // range in the diagonal-task table
+  int32_t p_map, t_map;       // tensor maps of the padded copy / padded transpose
 };
 
 struct DiagTask {             // sector-diagonal task (for diag(H))
@@ -94,6 +111,7 @@ struct Schedule {
   std::vector<Run> runs;
   std::vector<P2Unit> p2;
   std::vector<DiagTask> diag;
+  std::vector<MapSpec> maps;          // tensor maps the TMA kernels use (only filled / valid when aligned16)
   std::vector<hpsi_task_t> tasks;     // schedule order, for hpsi_query
   int64_t psi_len = 0;
   int64_t ws_len = 0;                 // doubles

@@ -11,11 +11,12 @@ struct hpsi_plan {
   hpsi::Schedule sc;
   bool host_only = false;
   bool bound = false;
-  bool aligned16 = true;          // descriptors AND arena bases allow 16-byte staging
+  bool aligned16 = true;          // descriptors AND arena bases have 16-byte aligned rows: TMA staging is used
   int n_sm = 148;
   hpsi::DevSchedule dev{};
   void* d_tables = nullptr;       // one allocation holding every uploaded table
   double* d_ws = nullptr;
+  void* d_maps = nullptr;         // CUtensorMap[sc.maps.size()], encoded by hpsi_bind
   // apply_host staging
   double* d_psi_stage = nullptr;
   double* d_out_stage = nullptr;

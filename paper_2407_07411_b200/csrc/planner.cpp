@@ -167,6 +167,15 @@ int build_schedule(const hpsi_sectors_t* s, const hpsi_terms_t* t, uint32_t flag
     ws = align_up(ws + (int64_t)b.cols * b.ldt, 16);
     sc->max_block_elems = std::max<int32_t>(sc->max_block_elems, b.rows * b.cols);
   }
+  sc->maps.clear();
+  auto add_map = [&](int base, int64_t moff, int rows, int cols, int ld) -> int32_t {
+    sc->maps.push_back({moff, base, rows, cols, ld, TILE, 0});
+    return (int32_t)sc->maps.size() - 1;
+  };
+  for (auto& b : sc->blocks) {
+    b.p_map = add_map(BASE_WS, b.p_off, b.rows, b.cols, b.ldp);
+    b.t_map = add_map(BASE_WS, b.t_off, b.cols, b.rows, b.ldt);
+  }
 
   // ---- steps 3+4a: order choice, groups, segs
   sc->segs.clear(); sc->groups.clear(); sc->tasks.clear(); sc->diag.clear();
@@ -189,18 +198,26 @@ int build_schedule(const hpsi_sectors_t* s, const hpsi_terms_t* t, uint32_t flag
     g.seg0 = (int32_t)sc->segs.size();
     g.src = raw[i].src;
     g.dst = raw[i].dst;
-    if (order == 1) { g.rows = (int32_t)m; g.K1 = (int32_t)k; g.N1 = (int32_t)np; g.ldy1 = S.ldt; g.y1_off = S.t_off; }
-    else            { g.rows = (int32_t)n; g.K1 = (int32_t)np; g.N1 = (int32_t)k; g.ldy1 = S.ldp; g.y1_off = S.p_off; }
+    if (order == 1) { g.rows = (int32_t)m; g.K1 = (int32_t)k; g.N1 = (int32_t)np; g.ldy1 = S.ldt; g.y1_off = S.t_off; g.y1_map = S.t_map; }
+    else            { g.rows = (int32_t)n; g.K1 = (int32_t)np; g.N1 = (int32_t)k; g.ldy1 = S.ldp; g.y1_off = S.p_off; g.y1_map = S.p_map; }
     g.ldw = sector_up(g.N1);
     g.ws_off = ws;
     const int64_t per_task = (int64_t)g.rows * g.ldw;
+    g.ws_map = add_map(BASE_WS, ws, (int)((int64_t)g.rows * (j - i)), g.N1, g.ldw);
     for (size_t q = i; q < j; ++q) {
       const hpsi_opblock_t& a = t->a_blocks[raw[q].ia];
       const hpsi_opblock_t& b = t->b_blocks[raw[q].ib];
       Seg sg{};
-      if (order == 1) { sg.p1_off = a.offset; sg.p1_ld = a.ld; sg.p2_off = b.offset; sg.p2_ld = b.ld; }
-      else            { sg.p1_off = b.offset; sg.p1_ld = b.ld; sg.p2_off = a.offset; sg.p2_ld = a.ld; }
-      sg.ws_off = ws + (int64_t)(q - i) * per_task;
+      // operator blocks as NT operands: A_t is (m x k), B_t is (n x n'); each block belongs to exactly one task
+      if (order == 1) {
+        sg.p1_off = a.offset; sg.p1_ld = a.ld; sg.p2_off = b.offset; sg.p2_ld = b.ld;
+        sg.p1_map = add_map(BASE_A, a.offset, (int)m, (int)k, a.ld);
+        sg.p2_map = add_map(BASE_B, b.offset, (int)n, (int)np, b.ld);
+      } else {
+        sg.p1_off = b.offset; sg.p1_ld = b.ld; sg.p2_off = a.offset; sg.p2_ld = a.ld;
+        sg.p1_map = add_map(BASE_B, b.offset, (int)n, (int)np, b.ld);
+        sg.p2_map = add_map(BASE_A, a.offset, (int)m, (int)k, a.ld);
+      }
       sg.coef = t->coef[raw[q].term];
       sc->segs.push_back(sg);
       if ((a.offset & 1) || (a.ld & 1) || (b.offset & 1) || (b.ld & 1)) sc->aligned16 = false;
@@ -223,19 +240,43 @@ int build_schedule(const hpsi_sectors_t* s, const hpsi_terms_t* t, uint32_t flag
     sc->blocks[b].diag1 = (int32_t)sc->diag.size();
   }
 
-  // ---- step 4b: P1 units (group-major, row tile, column tile fastest so that tiles sharing operator rows co-run)
+  // ---- step 4b: P1 units.  One unit = one tile position of the (rows x N1) intermediate and a range of the group's
+  // terms, processed back to back by one CTA (the staging pipeline runs across terms, so the CTA prologue and the
+  // load latency are paid once per ~P1_STAGES_PER_UNIT K-tiles instead of once per task).  Column tile fastest, so
+  // the tiles that read the same operator rows are adjacent in launch order; groups go heaviest unit first.
   sc->p1.clear();
   sc->issued_flops_p1 = 0;
-  for (size_t gi = 0; gi < sc->groups.size(); ++gi) {
-    const Group& g = sc->groups[gi];
-    auto rt = split_dim((int64_t)g.tcount * g.rows);
-    auto ct = split_dim(g.N1);
-    const int64_t ks = (g.K1 + 3) / 4;
-    for (auto& r : rt)
-      for (auto& c : ct) {
-        sc->p1.push_back({(int32_t)gi, r.start, r.len, c.start, c.len, 0});
-        sc->issued_flops_p1 += (int64_t)frags(r.len) * frags(c.len) * ks * 512;
+  {
+    constexpr int P1_STAGES_PER_UNIT = 96;
+    struct GOrder { int64_t cost; int gi; };
+    std::vector<GOrder> gorder;
+    std::vector<int> g_nt(sc->groups.size());
+    for (size_t gi = 0; gi < sc->groups.size(); ++gi) {
+      const Group& g = sc->groups[gi];
+      const int stages = (g.K1 + KT - 1) / KT;
+      int nt = std::max(1, std::min(g.tcount, (P1_STAGES_PER_UNIT + stages - 1) / stages));
+      const int nchunk = (g.tcount + nt - 1) / nt;
+      nt = (g.tcount + nchunk - 1) / nchunk;                    // even chunks
+      g_nt[gi] = nt;
+      const int fr = std::min(frags(g.rows), TILE / 8), fc = std::min(frags(g.N1), TILE / 8);
+      gorder.push_back({(int64_t)fr * fc * ((g.K1 + 3) / 4) * nt, (int)gi});
+    }
+    std::stable_sort(gorder.begin(), gorder.end(), [](const GOrder& x, const GOrder& y) { return x.cost > y.cost; });
+    for (const GOrder& go : gorder) {
+      const Group& g = sc->groups[go.gi];
+      auto rt = split_dim(g.rows);
+      auto ct = split_dim(g.N1);
+      const int64_t ks = (g.K1 + 3) / 4;
+      const int nt = g_nt[go.gi];
+      for (int t0 = 0; t0 < g.tcount; t0 += nt) {
+        const int t1 = std::min(g.tcount, t0 + nt);
+        for (auto& r : rt)
+          for (auto& c : ct) {
+            sc->p1.push_back({go.gi, t0, t1, r.start, r.len, c.start, c.len, 0});
+            sc->issued_flops_p1 += (int64_t)frags(r.len) * frags(c.len) * ks * 512 * (t1 - t0);
+          }
       }
+    }
   }
 
   // ---- step 4c: P2 units.  K-space of destination d = all segs of all groups with dst == d, in seg order.
@@ -292,7 +333,7 @@ int build_schedule(const hpsi_sectors_t* s, const hpsi_terms_t* t, uint32_t flag
         if (sp == nsplit - 1) take = g.tcount - ti;
         else take = (int)std::min<int64_t>(g.tcount - ti, std::max<int64_t>(1, (want - cum + per - 1) / per));
         if (take > 0) {
-          sc->runs.push_back({g.seg0 + ti, g.seg0 + ti + take, g.N1, g.ldw, g.order, 0});
+          sc->runs.push_back({g.seg0 + ti, g.seg0 + ti + take, g.N1, g.ldw, g.order, g.rows, g.seg0, g.ws_map, g.ws_off});
           cum += per * take;
           chunk_ksteps += per * take;
           ti += take;
