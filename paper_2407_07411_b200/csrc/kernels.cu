@@ -20,6 +20,8 @@
 // when the tile is stored.
 #include "kernels.cuh"
 
+#define HPSI_BIG_WARP_TILE 1     // 1 when MAXMI > 2 (dispatch cases for 3 and 4 row fragments)
+
 namespace hpsi {
 
 // ----------------------------------------------------------------------------------------------- PTX helpers
@@ -73,17 +75,21 @@ __device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double
 __device__ __forceinline__ int frag_perm(int x) { return ((x & 3) << 1) | (x >> 2); }
 
 // ------------------------------------------------------------------------------------------------- MMA core
+// Balanced split of f fragments over `parts` warps: part p gets ceil or floor of f / parts, heavier parts first.
+__device__ __forceinline__ void split_frags(int f, int parts, int p, int& first, int& count) {
+  const int base = f / parts, rem = f - base * parts;
+  count = base + (p < rem ? 1 : 0);
+  first = p * base + (p < rem ? p : rem);
+}
 struct WarpTile {
   int wr0, wc0;    // first row / col of the warp inside the CTA tile (multiples of 8)
-  int mi, nj;      // fragments owned (0..4 each)
+  int mi, nj;      // fragments owned (0..MAXMI, 0..MAXNJ)
   __device__ __forceinline__ WarpTile(int warp, int rows_valid, int cols_valid) {
-    const int fm = (rows_valid + 7) >> 3, fn = (cols_valid + 7) >> 3;
-    const int hm = (fm + 1) >> 1, hn = (fn + 1) >> 1;
-    const int wr = warp >> 1, wc = warp & 1;
-    wr0 = wr ? hm * 8 : 0;
-    mi = wr ? fm - hm : hm;
-    wc0 = wc ? hn * 8 : 0;
-    nj = wc ? fn - hn : hn;
+    int f0;
+    split_frags((rows_valid + 7) >> 3, WGM, warp / WGN, f0, mi);
+    wr0 = f0 * 8;
+    split_frags((cols_valid + 7) >> 3, WGN, warp % WGN, f0, nj);
+    wc0 = f0 * 8;
   }
 };
 
@@ -99,7 +105,7 @@ struct LaneOffsets {
 };
 
 template <int MI, int NJ>
-__device__ __forceinline__ void mma_step(const double (&a)[MI], const double (&b)[NJ], double (&acc)[4][4][2]) {
+__device__ __forceinline__ void mma_step(const double (&a)[MI], const double (&b)[NJ], double (&acc)[MAXMI][MAXNJ][2]) {
 #pragma unroll
   for (int i = 0; i < MI; ++i)
 #pragma unroll
@@ -117,7 +123,7 @@ __device__ __forceinline__ void load_frags(const double* px, const double* py, i
 // px / py = the warp's first row of the X / Y tile of the stage.
 template <int MI, int NJ>
 __device__ __forceinline__ void mma_stage(const double* px, const double* py, const LaneOffsets& lo,
-                                          double (&acc)[4][4][2], int nk4) {
+                                          double (&acc)[MAXMI][MAXNJ][2], int nk4) {
   double a0[MI], b0[NJ], a1[MI], b1[NJ];
   load_frags<MI, NJ>(px, py, lo.k[0], a0, b0);
   if (nk4 == 4) {                       // the common case: straight-line, no predication, no WARPSYNC
@@ -135,18 +141,18 @@ __device__ __forceinline__ void mma_stage(const double* px, const double* py, co
   }
 }
 
-__device__ __forceinline__ void zero_acc(double (&acc)[4][4][2]) {
+__device__ __forceinline__ void zero_acc(double (&acc)[MAXMI][MAXNJ][2]) {
 #pragma unroll
-  for (int i = 0; i < 4; ++i)
+  for (int i = 0; i < MAXMI; ++i)
 #pragma unroll
-    for (int j = 0; j < 4; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
+    for (int j = 0; j < MAXNJ; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
 }
 
 // Store the warp's accumulators: element (row, col) of the CTA tile goes to dst[row*ld + col], scaled by sc.
 // acc[i][j][e] holds tile row wr0 + 8i + perm(g) and tile column wc0 + 8j + perm(2q + e)  (perm(2q+1) = perm(2q) + 2).
 template <int MI, int NJ>
 __device__ __forceinline__ void store_tile(double* dst, int ld, int rows_valid, int cols_valid,
-                                           const double (&acc)[4][4][2], const WarpTile& w, int lane, double sc) {
+                                           const double (&acc)[MAXMI][MAXNJ][2], const WarpTile& w, int lane, double sc) {
   const int pg = frag_perm(lane >> 2), pc = frag_perm(2 * (lane & 3));
 #pragma unroll
   for (int i = 0; i < MI; ++i) {
@@ -165,7 +171,7 @@ __device__ __forceinline__ void store_tile(double* dst, int ld, int rows_valid, 
 // Which tile quadrant consumer warp 0 takes.  Consumer warp w sits on SM sub-partition w, and with odd fragment counts
 // the quadrants carry unequal DMMA counts (e.g. 16/12/12/9), so co-resident CTAs must not all put their heavy
 // quadrant on the same sub-partition.  CTAs are dealt to SMs round-robin (148 = 0 mod 4), hence a hash, not bid & 3.
-__device__ __forceinline__ int quadrant_rotation(unsigned bid) { return (int)((bid * 2654435761u) >> 30); }
+__device__ __forceinline__ int quadrant_rotation(unsigned bid) { return (int)((bid * 2654435761u) >> 29); }
 
 // Shared-memory carve-up: NSTAGE stages of [X tile | Y tile] (1024-byte aligned), then the barriers.
 struct SmemLayout {
@@ -223,7 +229,7 @@ __device__ __forceinline__ void ldgsts_tile(uint32_t s_op, const double* rows, i
 template <int MI, int NJ>
 __device__ __forceinline__ void p1_consume(const DevSchedule& d, const P1Unit& u, const Group& g, const SmemLayout& sm,
                                            const WarpTile& w, int lane) {
-  double acc[4][4][2];
+  double acc[MAXMI][MAXNJ][2];
   const LaneOffsets lo(lane);
   const int ntiles = (g.K1 + KT - 1) / KT;
   const int last_nk4 = ((g.K1 - (ntiles - 1) * KT) + 3) >> 2;
@@ -250,7 +256,7 @@ __device__ __forceinline__ void p1_consume(const DevSchedule& d, const P1Unit& u
 }
 
 template <bool TMA>
-__global__ void __launch_bounds__(NTHREADS, 3) p1_kernel(DevSchedule d) {
+__global__ void __launch_bounds__(NTHREADS, CTAS_PER_SM) p1_kernel(DevSchedule d) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const P1Unit u = d.p1[blockIdx.x];
   const Group g = d.groups[u.group];
@@ -298,14 +304,16 @@ __global__ void __launch_bounds__(NTHREADS, 3) p1_kernel(DevSchedule d) {
   }
 
   // ------------------ consumer warps
-  const int warp = (wid + quadrant_rotation(blockIdx.x)) & 3;
+  const int warp = (wid + quadrant_rotation(blockIdx.x)) % NCONS;
   const WarpTile w(warp, u.rows_valid, u.cols_valid);
 #define HPSI_CASE(MI, NJ) case MI * 5 + NJ: p1_consume<MI, NJ>(d, u, g, sm, w, lane); break;
   switch ((w.nj > 0 ? w.mi : 0) * 5 + (w.mi > 0 ? w.nj : 0)) {
     HPSI_CASE(1, 1) HPSI_CASE(1, 2) HPSI_CASE(1, 3) HPSI_CASE(1, 4)
     HPSI_CASE(2, 1) HPSI_CASE(2, 2) HPSI_CASE(2, 3) HPSI_CASE(2, 4)
+#if HPSI_BIG_WARP_TILE
     HPSI_CASE(3, 1) HPSI_CASE(3, 2) HPSI_CASE(3, 3) HPSI_CASE(3, 4)
     HPSI_CASE(4, 1) HPSI_CASE(4, 2) HPSI_CASE(4, 3) HPSI_CASE(4, 4)
+#endif
     default: p1_consume<0, 0>(d, u, g, sm, w, lane); break;
   }
 #undef HPSI_CASE
@@ -341,7 +349,7 @@ struct KIter {                 // walks (run, seg, kappa) in K-tile steps
 template <int MI, int NJ>
 __device__ __forceinline__ void p2_consume(const DevSchedule& d, const P2Unit& u, const SmemLayout& sm,
                                            const WarpTile& w, int lane) {
-  double acc[4][4][2];
+  double acc[MAXMI][MAXNJ][2];
   zero_acc(acc);
   const LaneOffsets lo(lane);
   Ring ring{0, 0};
@@ -360,7 +368,7 @@ __device__ __forceinline__ void p2_consume(const DevSchedule& d, const P2Unit& u
 }
 
 template <bool TMA>
-__global__ void __launch_bounds__(NTHREADS, 3) p2_kernel(DevSchedule d) {
+__global__ void __launch_bounds__(NTHREADS, CTAS_PER_SM) p2_kernel(DevSchedule d) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const P2Unit u = d.p2[blockIdx.x];
   const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
@@ -422,14 +430,16 @@ __global__ void __launch_bounds__(NTHREADS, 3) p2_kernel(DevSchedule d) {
   }
 
   // ------------------ consumer warps
-  const int warp = (wid + quadrant_rotation(blockIdx.x)) & 3;
+  const int warp = (wid + quadrant_rotation(blockIdx.x)) % NCONS;
   const WarpTile w(warp, u.rows_valid, u.cols_valid);
 #define HPSI_CASE(MI, NJ) case MI * 5 + NJ: p2_consume<MI, NJ>(d, u, sm, w, lane); break;
   switch ((w.nj > 0 ? w.mi : 0) * 5 + (w.mi > 0 ? w.nj : 0)) {
     HPSI_CASE(1, 1) HPSI_CASE(1, 2) HPSI_CASE(1, 3) HPSI_CASE(1, 4)
     HPSI_CASE(2, 1) HPSI_CASE(2, 2) HPSI_CASE(2, 3) HPSI_CASE(2, 4)
+#if HPSI_BIG_WARP_TILE
     HPSI_CASE(3, 1) HPSI_CASE(3, 2) HPSI_CASE(3, 3) HPSI_CASE(3, 4)
     HPSI_CASE(4, 1) HPSI_CASE(4, 2) HPSI_CASE(4, 3) HPSI_CASE(4, 4)
+#endif
     default: p2_consume<0, 0>(d, u, sm, w, lane); break;
   }
 #undef HPSI_CASE

@@ -10,8 +10,12 @@
 
 namespace hpsi {
 
-constexpr int NCONS = 4;                       // consumer (DMMA) warps per CTA, 2 x 2 over the tile
+constexpr int WGM = 2, WGN = 2;                // consumer (DMMA) warps per CTA: WGM x WGN over the tile
+constexpr int MAXMI = TILE / 8 / WGM;          // fragments per warp, rows
+constexpr int MAXNJ = TILE / 8 / WGN;          // fragments per warp, columns
+constexpr int NCONS = WGM * WGN;
 constexpr int NTHREADS = (NCONS + 1) * 32;     // + 1 producer warp
+constexpr int CTAS_PER_SM = 3;
 constexpr int NSTAGE = 4;
 constexpr int OP_BYTES = TILE * KT * 8;        // one operand tile of a stage: 64 rows x 128 bytes, 128-byte swizzled
 constexpr int STAGE_BYTES = 2 * OP_BYTES;      // X tile | Y tile
