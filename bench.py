@@ -296,8 +296,14 @@ def run_ours(args, rank, world, local_rank):
     fl = [0, fl_p1, q(H.HPSI_Q_USEFUL_FLOPS) - fl_p1, 0]
     dom = int(np.argmax(prof))
     achieved = fl[dom] / (prof[dom] * 1e-3) / 1e12 if prof[dom] > 0 else 0.0
+    traffic = None                       # DRAM bytes per launch of that kernel from the committed ncu --set full capture
+    try:
+        with open(os.path.join(ROOT, "profiles", "ncu_traffic.json.txt")) as fh:
+            traffic = json.load(fh).get(cfg, {}).get(names[dom].split()[0])
+    except (OSError, ValueError):
+        pass
     roofline = {"bound": "tensor", "kernel": names[dom], "achieved": achieved, "peak": dgemm_peak, "unit": "TFLOP/s",
-                "frac": achieved / dgemm_peak, "traffic": None,
+                "frac": achieved / dgemm_peak, "traffic": traffic,
                 "peak_source": "same-run cuBLAS DGEMM calibration (north_star); DMMA.8x8x4 pipe probe "
                                f"{calib['dmma_pipe_probe']} TFLOP/s",
                 "kernel_ms": {k: round(float(v), 4) for k, v in zip(names, prof)},

@@ -20,8 +20,6 @@
 // when the tile is stored.
 #include "kernels.cuh"
 
-#define HPSI_BIG_WARP_TILE 1     // 1 when MAXMI > 2 (dispatch cases for 3 and 4 row fragments)
-
 namespace hpsi {
 
 // ----------------------------------------------------------------------------------------------- PTX helpers
@@ -81,14 +79,17 @@ __device__ __forceinline__ void split_frags(int f, int parts, int p, int& first,
   count = base + (p < rem ? 1 : 0);
   first = p * base + (p < rem ? p : rem);
 }
+// The 4 consumer warps cover the tile as a 2x2, 1x4 or 4x1 grid (plan.h WarpGrid; chosen per unit by the planner so
+// that the heaviest warp is as light as possible); a warp owns at most 16 fragments: <=4x4, <=8x2 or <=2x8.
 struct WarpTile {
   int wr0, wc0;    // first row / col of the warp inside the CTA tile (multiples of 8)
-  int mi, nj;      // fragments owned (0..MAXMI, 0..MAXNJ)
-  __device__ __forceinline__ WarpTile(int warp, int rows_valid, int cols_valid) {
+  int mi, nj;      // fragments owned
+  __device__ __forceinline__ WarpTile(int grid, int warp, int rows_valid, int cols_valid) {
+    const int gn = grid == GRID_2x2 ? 2 : (grid == GRID_1x4 ? 4 : 1), gm = NCONS / gn;
     int f0;
-    split_frags((rows_valid + 7) >> 3, WGM, warp / WGN, f0, mi);
+    split_frags((rows_valid + 7) >> 3, gm, warp / gn, f0, mi);
     wr0 = f0 * 8;
-    split_frags((cols_valid + 7) >> 3, WGN, warp % WGN, f0, nj);
+    split_frags((cols_valid + 7) >> 3, gn, warp % gn, f0, nj);
     wc0 = f0 * 8;
   }
 };
@@ -105,7 +106,7 @@ struct LaneOffsets {
 };
 
 template <int MI, int NJ>
-__device__ __forceinline__ void mma_step(const double (&a)[MI], const double (&b)[NJ], double (&acc)[MAXMI][MAXNJ][2]) {
+__device__ __forceinline__ void mma_step(const double (&a)[MI], const double (&b)[NJ], double (&acc)[MI][NJ][2]) {
 #pragma unroll
   for (int i = 0; i < MI; ++i)
 #pragma unroll
@@ -123,7 +124,7 @@ __device__ __forceinline__ void load_frags(const double* px, const double* py, i
 // px / py = the warp's first row of the X / Y tile of the stage.
 template <int MI, int NJ>
 __device__ __forceinline__ void mma_stage(const double* px, const double* py, const LaneOffsets& lo,
-                                          double (&acc)[MAXMI][MAXNJ][2], int nk4) {
+                                          double (&acc)[MI][NJ][2], int nk4) {
   double a0[MI], b0[NJ], a1[MI], b1[NJ];
   load_frags<MI, NJ>(px, py, lo.k[0], a0, b0);
   if (nk4 == 4) {                       // the common case: straight-line, no predication, no WARPSYNC
@@ -141,18 +142,19 @@ __device__ __forceinline__ void mma_stage(const double* px, const double* py, co
   }
 }
 
-__device__ __forceinline__ void zero_acc(double (&acc)[MAXMI][MAXNJ][2]) {
+template <int MI, int NJ>
+__device__ __forceinline__ void zero_acc(double (&acc)[MI][NJ][2]) {
 #pragma unroll
-  for (int i = 0; i < MAXMI; ++i)
+  for (int i = 0; i < MI; ++i)
 #pragma unroll
-    for (int j = 0; j < MAXNJ; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
+    for (int j = 0; j < NJ; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
 }
 
 // Store the warp's accumulators: element (row, col) of the CTA tile goes to dst[row*ld + col], scaled by sc.
 // acc[i][j][e] holds tile row wr0 + 8i + perm(g) and tile column wc0 + 8j + perm(2q + e)  (perm(2q+1) = perm(2q) + 2).
 template <int MI, int NJ>
 __device__ __forceinline__ void store_tile(double* dst, int ld, int rows_valid, int cols_valid,
-                                           const double (&acc)[MAXMI][MAXNJ][2], const WarpTile& w, int lane, double sc) {
+                                           const double (&acc)[MI][NJ][2], const WarpTile& w, int lane, double sc) {
   const int pg = frag_perm(lane >> 2), pc = frag_perm(2 * (lane & 3));
 #pragma unroll
   for (int i = 0; i < MI; ++i) {
@@ -229,31 +231,47 @@ __device__ __forceinline__ void ldgsts_tile(uint32_t s_op, const double* rows, i
 template <int MI, int NJ>
 __device__ __forceinline__ void p1_consume(const DevSchedule& d, const P1Unit& u, const Group& g, const SmemLayout& sm,
                                            const WarpTile& w, int lane) {
-  double acc[MAXMI][MAXNJ][2];
+  double acc[MI][NJ][2];
   const LaneOffsets lo(lane);
   const int ntiles = (g.K1 + KT - 1) / KT;
   const int last_nk4 = ((g.K1 - (ntiles - 1) * KT) + 3) >> 2;
   Ring ring{0, 0};
   for (int t = u.t0; t < u.t1; ++t) {
-    zero_acc(acc);
+    const double coef = d.segs[g.seg0 + t].coef;            // issued before the K loop, needed after it
+    zero_acc<MI, NJ>(acc);
     for (int kt = 0; kt < ntiles; ++kt) {
       mbar_wait(sm.full(ring.stage), ring.phase);
-      if (MI > 0 && d.debug != 2) {
+      if (d.debug != 2) {
         const double* st = sm.stage_ptr(ring.stage);
-        mma_stage<(MI > 0 ? MI : 1), (NJ > 0 ? NJ : 1)>(st + w.wr0 * 16, st + OP_BYTES / 8 + w.wc0 * 16, lo, acc,
-                                                          kt == ntiles - 1 ? last_nk4 : 4);
+        mma_stage<MI, NJ>(st + w.wr0 * 16, st + OP_BYTES / 8 + w.wc0 * 16, lo, acc, kt == ntiles - 1 ? last_nk4 : 4);
       }
       __syncwarp();
       if (lane == 0) mbar_arrive(sm.empty(ring.stage));
       ring.advance();
     }
-    if (MI > 0) {
-      double* dst = d.ws + g.ws_off + ((int64_t)t * g.rows + u.i0) * g.ldw + u.j0;
-      store_tile<(MI > 0 ? MI : 1), (NJ > 0 ? NJ : 1)>(dst, g.ldw, u.rows_valid, u.cols_valid, acc, w, lane,
-                                                        d.segs[g.seg0 + t].coef);
-    }
+    double* dst = d.ws + g.ws_off + ((int64_t)t * g.rows + u.i0) * g.ldw + u.j0;
+    store_tile<MI, NJ>(dst, g.ldw, u.rows_valid, u.cols_valid, acc, w, lane, coef);
   }
 }
+// a consumer warp without fragments (tile narrower than the warp grid) only hands the stages back
+__device__ __forceinline__ void idle_consume(const SmemLayout& sm, int nstages, int lane) {
+  Ring ring{0, 0};
+  for (int i = 0; i < nstages; ++i) {
+    mbar_wait(sm.full(ring.stage), ring.phase);
+    if (lane == 0) mbar_arrive(sm.empty(ring.stage));
+    ring.advance();
+  }
+}
+
+// Dispatch to the instantiation for the warp's (mi, nj): <=4x4 (2x2 grid), <=8x2 (1x4 grid), <=2x8 (4x1 grid).
+#define HPSI_DISPATCH_FRAGS(CALL)                                                                               \
+  switch (w.mi * 9 + w.nj) {                                                                                    \
+    CALL(1, 1) CALL(1, 2) CALL(1, 3) CALL(1, 4) CALL(2, 1) CALL(2, 2) CALL(2, 3) CALL(2, 4)                     \
+    CALL(3, 1) CALL(3, 2) CALL(3, 3) CALL(3, 4) CALL(4, 1) CALL(4, 2) CALL(4, 3) CALL(4, 4)                     \
+    CALL(5, 1) CALL(5, 2) CALL(6, 1) CALL(6, 2) CALL(7, 1) CALL(7, 2) CALL(8, 1) CALL(8, 2)                     \
+    CALL(1, 5) CALL(2, 5) CALL(1, 6) CALL(2, 6) CALL(1, 7) CALL(2, 7) CALL(1, 8) CALL(2, 8)                     \
+    default: __trap();                                                                                          \
+  }
 
 template <bool TMA>
 __global__ void __launch_bounds__(NTHREADS, CTAS_PER_SM) p1_kernel(DevSchedule d) {
@@ -305,17 +323,10 @@ __global__ void __launch_bounds__(NTHREADS, CTAS_PER_SM) p1_kernel(DevSchedule d
 
   // ------------------ consumer warps
   const int warp = (wid + quadrant_rotation(blockIdx.x)) % NCONS;
-  const WarpTile w(warp, u.rows_valid, u.cols_valid);
-#define HPSI_CASE(MI, NJ) case MI * 5 + NJ: p1_consume<MI, NJ>(d, u, g, sm, w, lane); break;
-  switch ((w.nj > 0 ? w.mi : 0) * 5 + (w.mi > 0 ? w.nj : 0)) {
-    HPSI_CASE(1, 1) HPSI_CASE(1, 2) HPSI_CASE(1, 3) HPSI_CASE(1, 4)
-    HPSI_CASE(2, 1) HPSI_CASE(2, 2) HPSI_CASE(2, 3) HPSI_CASE(2, 4)
-#if HPSI_BIG_WARP_TILE
-    HPSI_CASE(3, 1) HPSI_CASE(3, 2) HPSI_CASE(3, 3) HPSI_CASE(3, 4)
-    HPSI_CASE(4, 1) HPSI_CASE(4, 2) HPSI_CASE(4, 3) HPSI_CASE(4, 4)
-#endif
-    default: p1_consume<0, 0>(d, u, g, sm, w, lane); break;
-  }
+  const WarpTile w(u.grid, warp, u.rows_valid, u.cols_valid);
+  if (w.mi == 0 || w.nj == 0) { idle_consume(sm, ntiles * (u.t1 - u.t0), lane); return; }
+#define HPSI_CASE(MI, NJ) case MI * 9 + NJ: p1_consume<MI, NJ>(d, u, g, sm, w, lane); break;
+  HPSI_DISPATCH_FRAGS(HPSI_CASE)
 #undef HPSI_CASE
 }
 
@@ -349,22 +360,21 @@ struct KIter {                 // walks (run, seg, kappa) in K-tile steps
 template <int MI, int NJ>
 __device__ __forceinline__ void p2_consume(const DevSchedule& d, const P2Unit& u, const SmemLayout& sm,
                                            const WarpTile& w, int lane) {
-  double acc[MAXMI][MAXNJ][2];
-  zero_acc(acc);
+  double acc[MI][NJ][2];
+  zero_acc<MI, NJ>(acc);
   const LaneOffsets lo(lane);
   Ring ring{0, 0};
   for (KIter it(d.runs, u.run_begin, u.run_end); it.valid; it.advance()) {
     mbar_wait(sm.full(ring.stage), ring.phase);
-    if (MI > 0 && d.debug != 2) {
+    if (d.debug != 2) {
       const double* st = sm.stage_ptr(ring.stage);
-      mma_stage<(MI > 0 ? MI : 1), (NJ > 0 ? NJ : 1)>(st + w.wr0 * 16, st + OP_BYTES / 8 + w.wc0 * 16, lo, acc, it.nk4());
+      mma_stage<MI, NJ>(st + w.wr0 * 16, st + OP_BYTES / 8 + w.wc0 * 16, lo, acc, it.nk4());
     }
     __syncwarp();
     if (lane == 0) mbar_arrive(sm.empty(ring.stage));
     ring.advance();
   }
-  if (MI > 0)
-    store_tile<(MI > 0 ? MI : 1), (NJ > 0 ? NJ : 1)>(d.ws + u.out_off, u.ldo, u.rows_valid, u.cols_valid, acc, w, lane, 1.0);
+  store_tile<MI, NJ>(d.ws + u.out_off, u.ldo, u.rows_valid, u.cols_valid, acc, w, lane, 1.0);
 }
 
 template <bool TMA>
@@ -431,17 +441,15 @@ __global__ void __launch_bounds__(NTHREADS, CTAS_PER_SM) p2_kernel(DevSchedule d
 
   // ------------------ consumer warps
   const int warp = (wid + quadrant_rotation(blockIdx.x)) % NCONS;
-  const WarpTile w(warp, u.rows_valid, u.cols_valid);
-#define HPSI_CASE(MI, NJ) case MI * 5 + NJ: p2_consume<MI, NJ>(d, u, sm, w, lane); break;
-  switch ((w.nj > 0 ? w.mi : 0) * 5 + (w.mi > 0 ? w.nj : 0)) {
-    HPSI_CASE(1, 1) HPSI_CASE(1, 2) HPSI_CASE(1, 3) HPSI_CASE(1, 4)
-    HPSI_CASE(2, 1) HPSI_CASE(2, 2) HPSI_CASE(2, 3) HPSI_CASE(2, 4)
-#if HPSI_BIG_WARP_TILE
-    HPSI_CASE(3, 1) HPSI_CASE(3, 2) HPSI_CASE(3, 3) HPSI_CASE(3, 4)
-    HPSI_CASE(4, 1) HPSI_CASE(4, 2) HPSI_CASE(4, 3) HPSI_CASE(4, 4)
-#endif
-    default: p2_consume<0, 0>(d, u, sm, w, lane); break;
+  const WarpTile w(u.grid, warp, u.rows_valid, u.cols_valid);
+  if (w.mi == 0 || w.nj == 0) {
+    int nstages = 0;
+    for (KIter it(d.runs, u.run_begin, u.run_end); it.valid; it.advance()) ++nstages;
+    idle_consume(sm, nstages, lane);
+    return;
   }
+#define HPSI_CASE(MI, NJ) case MI * 9 + NJ: p2_consume<MI, NJ>(d, u, sm, w, lane); break;
+  HPSI_DISPATCH_FRAGS(HPSI_CASE)
 #undef HPSI_CASE
 }
 

@@ -2,7 +2,7 @@
 // sm_100a has (tcgen05 has no f64 kind), accumulators in registers.  Operands are staged into shared memory by the
 // TMA unit (cp.async.bulk.tensor.2d with one tensor map per operand matrix, 128-byte swizzle, zero fill out of
 // bounds) when every block has 16-byte aligned rows; otherwise by 8-byte cp.async (LDGSTS) into the same layout.
-// One CTA = 1 producer warp + 2x2 consumer warps on a <=64x64 tile (<=4x4 fragments each).
+// One CTA = 1 producer warp + 4 consumer warps on a <=64x64 tile (<=16 fragments each).
 #pragma once
 #include <cuda_runtime.h>
 
@@ -10,10 +10,7 @@
 
 namespace hpsi {
 
-constexpr int WGM = 2, WGN = 2;                // consumer (DMMA) warps per CTA: WGM x WGN over the tile
-constexpr int MAXMI = TILE / 8 / WGM;          // fragments per warp, rows
-constexpr int MAXNJ = TILE / 8 / WGN;          // fragments per warp, columns
-constexpr int NCONS = WGM * WGN;
+constexpr int NCONS = 4;                       // consumer (DMMA) warps per CTA, as a 2x2, 1x4 or 4x1 grid over the tile
 constexpr int NTHREADS = (NCONS + 1) * 32;     // + 1 producer warp
 constexpr int CTAS_PER_SM = 3;
 constexpr int NSTAGE = 4;

@@ -23,6 +23,8 @@ constexpr int TILE = 64;      // CTA tile edge (rows and cols), 8 fragments of 8
 constexpr int KT = 16;        // K extent of one staged tile (4 DMMA k-steps)
 
 enum BaseSel : int32_t { BASE_A = 0, BASE_B = 1, BASE_WS = 2 };
+// how the 4 consumer warps of a CTA cover its tile (rows x columns of warps)
+enum WarpGrid : int32_t { GRID_2x2 = 0, GRID_1x4 = 1, GRID_4x1 = 2 };
 
 struct Seg {                  // one task, in schedule order (by destination, source, term)
   int64_t p1_off;             // operator block used by P1 (order 1: A_t, order 2: B_t), doubles into its arena
@@ -53,7 +55,7 @@ struct P1Unit {               // one CTA of the first-GEMM kernel: one tile posi
   int32_t t0, t1;             // terms [t0, t1) of the group, processed one after the other (pipeline never drains)
   int32_t i0, rows_valid;     // row tile inside one task's intermediate
   int32_t j0, cols_valid;     // column tile
-  int32_t pad;
+  int32_t grid;               // WarpGrid
 };
 
 struct Run {                  // consecutive segs of one group inside one P2 unit's K range
@@ -72,7 +74,7 @@ struct P2Unit {               // one CTA of the second-GEMM kernel
   int32_t i0, rows_valid, j0, cols_valid;
   int64_t out_off;            // partial buffer offset of element (i0, j0) of this split's m x ldp tile
   int32_t ldo;
-  int32_t pad;
+  int32_t grid;               // WarpGrid
 };
 
 // A 2-D row-major matrix the TMA unit reads: rows x cols doubles, leading dimension ld, `off` doubles into `base`.
@@ -133,5 +135,16 @@ inline int even_up(int x) { return x + (x & 1); }
 // 128-byte row segment is exactly four sectors (measured: 16-byte-aligned rows cost 1.4x the sectors).
 inline int sector_up(int x) { return (x + 3) & ~3; }
 inline int frags(int x) { return (x + 7) / 8; }
+// Heaviest warp (in fragments) when a tile of fm x fn fragments is covered by 4 warps as a gm x gn grid, and the grid
+// that minimises it (ties: 2x2, which needs the fewest shared-memory reads per DMMA).
+inline int heaviest_warp(int fm, int fn, int gm, int gn) { return ((fm + gm - 1) / gm) * ((fn + gn - 1) / gn); }
+inline int32_t best_grid(int fm, int fn, int* heaviest = nullptr) {
+  int best = heaviest_warp(fm, fn, 2, 2);
+  int32_t g = GRID_2x2;
+  if (heaviest_warp(fm, fn, 1, 4) < best) { best = heaviest_warp(fm, fn, 1, 4); g = GRID_1x4; }
+  if (heaviest_warp(fm, fn, 4, 1) < best) { best = heaviest_warp(fm, fn, 4, 1); g = GRID_4x1; }
+  if (heaviest) *heaviest = best;
+  return g;
+}
 
 }  // namespace hpsi

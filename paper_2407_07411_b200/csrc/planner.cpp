@@ -279,7 +279,7 @@ int build_schedule(const hpsi_sectors_t* s, const hpsi_terms_t* t, uint32_t flag
         const int t1 = std::min(g.tcount, t0 + nt);
         for (auto& r : rt)
           for (auto& c : ct) {
-            sc->p1.push_back({go.gi, t0, t1, r.start, r.len, c.start, c.len, 0});
+            sc->p1.push_back({go.gi, t0, t1, r.start, r.len, c.start, c.len, best_grid(frags(r.len), frags(c.len))});
             sc->issued_flops_p1 += (int64_t)frags(r.len) * frags(c.len) * ks * 512 * (t1 - t0);
           }
       }
@@ -357,6 +357,7 @@ int build_schedule(const hpsi_sectors_t* s, const hpsi_terms_t* t, uint32_t flag
           u.run_begin = run0; u.run_end = run1;
           u.i0 = r.start; u.rows_valid = r.len; u.j0 = c.start; u.cols_valid = c.len;
           u.ldo = D.ldo;
+          u.grid = best_grid(frags(r.len), frags(c.len));
           u.out_off = ws + (int64_t)realised * D.rows * D.ldo + (int64_t)r.start * D.ldo + c.start;
           sc->p2.push_back(u);
           int64_t cost = (int64_t)frags(r.len) * frags(c.len) * chunk_ksteps;
