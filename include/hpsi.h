@@ -62,8 +62,10 @@ typedef struct {
 /* "Term list" (north_star).  Descriptors and coef are HOST (copied).  a_data / b_data are DEVICE arenas,
  * caller-owned and BORROWED: they must outlive the plan (no copy is made - at D=8192 they are ~80 GB).
  * They may be NULL at plan time and bound later with hpsi_bind.  a_len / b_len = arena lengths in doubles
- * (used to validate descriptors).  Fast path: every block has even `offset` and even `ld` and the arenas
- * are 16-byte aligned (16-byte cp.async); otherwise a slower 8-byte staging variant of the kernels runs. */
+ * (used to validate descriptors).  Fast path (TMA staging): every block has even `offset` and even `ld` and the
+ * arenas are 16-byte aligned; preferred: `ld` and `offset` multiples of 4 (rows start on a 32-byte L2 sector).
+ * Anything else runs an 8-byte cp.async variant of the kernels (correct, slower).  Padding elements are never
+ * read into a result (out-of-range rows / columns are zero-filled on the way into shared memory). */
 typedef struct {
   int32_t n_terms;
   const double* coef;              /* [n_terms] c_t                                             */
@@ -81,7 +83,8 @@ typedef struct {
  * CTA work units; uploads the flat schedule and allocates the workspace.  One-off, synchronous. */
 int hpsi_plan(const hpsi_sectors_t* sectors, const hpsi_terms_t* terms, uint32_t flags, hpsi_plan_t** plan_out);
 
-/* (Re)bind the DEVICE operator arenas (same descriptors).  */
+/* (Re)bind the DEVICE operator arenas (same descriptors).  Re-encodes the tensor maps of the operand matrices
+ * (host work proportional to the number of blocks; synchronous). */
 int hpsi_bind(hpsi_plan_t* plan, const double* a_data_dev, const double* b_data_dev);
 
 /* Steps 5-7: out = H psi (overwrite).  psi_dev / out_dev: DEVICE, psi_length doubles each, must not alias.
@@ -138,7 +141,7 @@ enum {
   HPSI_Q_N_P2_UNITS = 10,    /* int64: CTA work units of the second-GEMM kernel                               */
   HPSI_Q_N_ORDER1_TASKS = 11,/* int64: tasks scheduled as (A psi) B^T                                         */
   HPSI_Q_LAUNCHES_PER_APPLY = 12, /* int64: kernels hpsi_apply enqueues                                       */
-  HPSI_Q_ALIGNED16 = 13,     /* int64: 1 if the 16-byte staging path is used                                  */
+  HPSI_Q_ALIGNED16 = 13,     /* int64: 1 if the TMA staging path is used (16-byte aligned rows)              */
   HPSI_Q_INTERMEDIATE_BYTES = 14, /* int64: bytes of first-GEMM results written (and read back) per apply     */
   HPSI_Q_ISSUED_FLOPS_P1 = 15,    /* int64: first-GEMM share of HPSI_Q_ISSUED_FLOPS                           */
   HPSI_Q_TASKS = 16,         /* hpsi_task_t[n_tasks], in schedule order                                      */

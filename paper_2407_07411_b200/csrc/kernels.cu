@@ -9,7 +9,7 @@
 //              Measured on B200 for this access pattern: TMA boxes feed 6.1-6.9 TB/s from HBM and 12-13.9 TB/s from L2,
 //              16-byte LDGSTS 4.8 / 6.4 TB/s.  Matrices whose rows are not 16-byte aligned take the LDGSTS variant
 //              (8-byte cp.async with zero fill into the same swizzled layout).
-//   consumers: 2x2 warps, each <= 4x4 fragments of DMMA.8x8x4 with register accumulators; a warp waits only on the
+//   consumers: 4 warps as a 2x2, 1x4 or 4x1 grid, each <= 16 fragments of DMMA.8x8x4 with register accumulators; a warp waits only on the
 //              "full" barrier of its next stage and releases the stage on its "empty" barrier - no CTA-wide barrier
 //              in the main loop.
 //
