@@ -145,7 +145,8 @@ enum {
   HPSI_Q_INTERMEDIATE_BYTES = 14, /* int64: bytes of first-GEMM results written (and read back) per apply     */
   HPSI_Q_ISSUED_FLOPS_P1 = 15,    /* int64: first-GEMM share of HPSI_Q_ISSUED_FLOPS                           */
   HPSI_Q_TASKS = 16,         /* hpsi_task_t[n_tasks], in schedule order                                      */
-  HPSI_Q_USEFUL_FLOPS_P1 = 17 /* int64: first-GEMM share of HPSI_Q_USEFUL_FLOPS                                */
+  HPSI_Q_USEFUL_FLOPS_P1 = 17,/* int64: first-GEMM share of HPSI_Q_USEFUL_FLOPS                                */
+  HPSI_Q_CRITICAL_FLOPS = 18  /* int64: like ISSUED_FLOPS, but every CTA counted as 4 x its heaviest warp (what warp imbalance costs) */
 };
 
 typedef struct {

@@ -20,7 +20,7 @@ HPSI_PLAN_FIXED_ORDER2 = 1 << 2
 (HPSI_Q_PSI_LENGTH, HPSI_Q_N_PSI_BLOCKS, HPSI_Q_PSI_BLOCKS, HPSI_Q_N_TASKS, HPSI_Q_USEFUL_FLOPS, HPSI_Q_ISSUED_FLOPS,
  HPSI_Q_OPERATOR_BYTES, HPSI_Q_WORKSPACE_BYTES, HPSI_Q_N_GROUPS, HPSI_Q_N_P1_UNITS, HPSI_Q_N_P2_UNITS,
  HPSI_Q_N_ORDER1_TASKS, HPSI_Q_LAUNCHES_PER_APPLY, HPSI_Q_ALIGNED16, HPSI_Q_INTERMEDIATE_BYTES,
- HPSI_Q_ISSUED_FLOPS_P1, HPSI_Q_TASKS, HPSI_Q_USEFUL_FLOPS_P1) = range(18)
+ HPSI_Q_ISSUED_FLOPS_P1, HPSI_Q_TASKS, HPSI_Q_USEFUL_FLOPS_P1, HPSI_Q_CRITICAL_FLOPS) = range(19)
 
 PSI_BLOCK_DTYPE = np.dtype([("left", "<i4"), ("right", "<i4"), ("rows", "<i4"), ("cols", "<i4"), ("offset", "<i8")],
                            align=True)

@@ -280,6 +280,7 @@ extern "C" int hpsi_query(const hpsi_plan_t* p, int what, void* out, size_t byte
     case HPSI_Q_USEFUL_FLOPS_P1: return put_i64(sc.useful_flops_p1);
     case HPSI_Q_ISSUED_FLOPS: return put_i64(sc.issued_flops);
     case HPSI_Q_ISSUED_FLOPS_P1: return put_i64(sc.issued_flops_p1);
+    case HPSI_Q_CRITICAL_FLOPS: return put_i64(sc.critical_flops);
     case HPSI_Q_OPERATOR_BYTES: return put_i64(sc.operator_bytes);
     case HPSI_Q_WORKSPACE_BYTES: return put_i64(sc.ws_len * 8);
     case HPSI_Q_N_GROUPS: return put_i64((int64_t)sc.groups.size());

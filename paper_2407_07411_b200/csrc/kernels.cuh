@@ -10,7 +10,7 @@
 
 namespace hpsi {
 
-constexpr int NCONS = 4;                       // consumer (DMMA) warps per CTA, as a 2x2, 1x4 or 4x1 grid over the tile
+constexpr int NCONS = NCONS_WARPS;                     // consumer (DMMA) warps per CTA, as a 2x2, 1x4 or 4x1 grid over the tile
 constexpr int NTHREADS = (NCONS + 1) * 32;     // + 1 producer warp
 constexpr int CTAS_PER_SM = 3;
 constexpr int NSTAGE = 4;

@@ -21,6 +21,7 @@ namespace hpsi {
 
 constexpr int TILE = 64;      // CTA tile edge (rows and cols), 8 fragments of 8
 constexpr int KT = 16;        // K extent of one staged tile (4 DMMA k-steps)
+constexpr int NCONS_WARPS = 4; // consumer (DMMA) warps per CTA
 
 enum BaseSel : int32_t { BASE_A = 0, BASE_B = 1, BASE_WS = 2 };
 // how the 4 consumer warps of a CTA cover its tile (rows x columns of warps)
@@ -118,6 +119,7 @@ struct Schedule {
   int64_t psi_len = 0;
   int64_t ws_len = 0;                 // doubles
   int64_t useful_flops = 0, useful_flops_p1 = 0, issued_flops = 0, issued_flops_p1 = 0, operator_bytes = 0, intermediate_bytes = 0;
+  int64_t critical_flops = 0;         // 4 warps x the heaviest warp's DMMA flops, summed over units (imbalance included)
   int64_t n_order1 = 0;
   int32_t max_block_elems = 0;
   bool aligned16 = true;              // descriptors allow the 16-byte staging path (arena base checked at bind)

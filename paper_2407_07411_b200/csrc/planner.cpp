@@ -253,6 +253,7 @@ int build_schedule(const hpsi_sectors_t* s, const hpsi_terms_t* t, uint32_t flag
   // the tiles that read the same operator rows are adjacent in launch order; groups go heaviest unit first.
   sc->p1.clear();
   sc->issued_flops_p1 = 0;
+  sc->critical_flops = 0;
   {
     constexpr int P1_STAGES_PER_UNIT = 96;
     struct GOrder { int64_t cost; int gi; };
@@ -281,6 +282,9 @@ int build_schedule(const hpsi_sectors_t* s, const hpsi_terms_t* t, uint32_t flag
           for (auto& c : ct) {
             sc->p1.push_back({go.gi, t0, t1, r.start, r.len, c.start, c.len, best_grid(frags(r.len), frags(c.len))});
             sc->issued_flops_p1 += (int64_t)frags(r.len) * frags(c.len) * ks * 512 * (t1 - t0);
+            int heavy = 0;
+            best_grid(frags(r.len), frags(c.len), &heavy);
+            sc->critical_flops += (int64_t)NCONS_WARPS * heavy * ks * 512 * (t1 - t0);
           }
       }
     }
@@ -361,6 +365,9 @@ int build_schedule(const hpsi_sectors_t* s, const hpsi_terms_t* t, uint32_t flag
           u.out_off = ws + (int64_t)realised * D.rows * D.ldo + (int64_t)r.start * D.ldo + c.start;
           sc->p2.push_back(u);
           int64_t cost = (int64_t)frags(r.len) * frags(c.len) * chunk_ksteps;
+          int heavy = 0;
+          best_grid(frags(r.len), frags(c.len), &heavy);
+          sc->critical_flops += (int64_t)NCONS_WARPS * heavy * chunk_ksteps * 512;
           unit_bundle.push_back((int)bundle_cost.size());
           bundle_max = std::max(bundle_max, cost);
           issued_p2 += cost * 512;

@@ -193,3 +193,81 @@ def test_davidson_small(H, small):
     theta, x, info = _davidson(H, g, workloads.make_psi(small), tol=1e-7, max_iter=300)
     assert info["converged"]
     assert np.linalg.norm(oracle.apply(small, x) - theta * x) <= 1e-6
+
+
+def _nan_padded(p):
+    """Copy of the arenas with every element that is not inside a block (ld padding, gaps) set to NaN."""
+    a, b = np.full_like(p.a_data, np.nan), np.full_like(p.b_data, np.nan)
+    for desc, src, dst, dims in ((p.a_desc, p.a_data, a, p.d_left), (p.b_desc, p.b_data, b, p.d_right)):
+        for e in desc:
+            r, c, ld, off = int(dims[e["row"]]), int(dims[e["col"]]), int(e["ld"]), int(e["offset"])
+            for x in range(r):
+                dst[off + x * ld: off + x * ld + c] = src[off + x * ld: off + x * ld + c]
+    return a, b
+
+
+@pytest.mark.parametrize("misalign", [False, True])
+def test_padding_is_never_read_and_rebind(H, misalign):
+    """TMA boxes (and the LDGSTS fallback) clip at the matrix edge: NaN in the ld padding must not reach the result.
+    hpsi_bind to arenas at a new address re-encodes the tensor maps."""
+    import torch
+    p = workloads.make_problem("small", n_terms=40)
+    g = GpuProblem(p, misalign=misalign)
+    assert g.q(H.HPSI_Q_ALIGNED16) == (0 if misalign else 1)
+    psi = workloads.make_psi(p)
+    ref = oracle.apply(p, psi)
+    assert rel_l2(g.apply(psi), ref) <= TOL
+    a_nan, b_nan = _nan_padded(p)
+    assert np.isnan(a_nan).any() and np.isnan(b_nan).any()
+    a2 = torch.from_numpy(a_nan).cuda()
+    b2 = torch.from_numpy(b_nan).cuda()
+    H.hpsi_bind(g.plan, a2, b2)
+    g.a.fill_(float("nan"))                      # the old arenas must not be read any more
+    g.b.fill_(float("nan"))
+    assert g.q(H.HPSI_Q_ALIGNED16) == 1
+    out = g.apply(psi)
+    assert np.isfinite(out).all() and rel_l2(out, ref) <= TOL
+
+
+def test_warp_grid_shapes(H):
+    """Blocks whose tiles make the planner pick each warp grid: 56x64 (7x8 fragments -> 1x4), 64x56 (-> 4x1),
+    40x40 (5x5 -> 2x2), 8x64 and 64x8 (one fragment row / column), plus ragged 61x59."""
+    rng = np.random.default_rng(21)
+    dL, dR = [56, 64, 40, 8, 64, 61], [64, 56, 40, 64, 8, 59]
+    n = len(dL)
+    terms = []
+    for _ in range(6):
+        ab = {(r, c): rng.standard_normal((dL[r], dL[c])) for r in range(n) for c in range(n) if (r + c) % 2 == 0 or r == c}
+        bb = {(r, c): rng.standard_normal((dR[r], dR[c])) for r in range(n) for c in range(n) if (r + c) % 2 == 0 or r == c}
+        terms.append((float(rng.standard_normal()), ab, bb))
+    qL = [(i, 0) for i in range(n)]
+    qR = [(n - i, 0) for i in range(n)]
+    p = workloads.custom_problem(qL, dL, qR, dR, (n, 0), terms, pad_even=True)
+    psi = rng.standard_normal(p.psi_len)
+    ref = oracle.apply(p, psi)
+    for flags in (0, H.HPSI_PLAN_FIXED_ORDER1, H.HPSI_PLAN_FIXED_ORDER2):
+        assert rel_l2(GpuProblem(p, flags).apply(psi), ref) <= TOL
+
+
+@pytest.mark.parametrize("cfg", ["cyp", "stress"])
+def test_full_size_sampled_parity(H, cfg):
+    """BASELINE.json configs[2] / configs[4] at full size, in the launch configuration bench.py times: 64 sampled
+    outputs that the oracle computes one by one, plus Hermiticity <x,Hy> = <Hx,y> on the full vectors."""
+    p = workloads.make_problem(cfg)
+    g = GpuProblem(p)
+    assert g.q(H.HPSI_Q_ALIGNED16) == 1
+    psi = workloads.make_psi(p)
+    out = g.apply(psi)
+    rng = np.random.default_rng(7)
+    blocks = p.psi_blocks()
+    bi = rng.integers(0, len(blocks), 64)
+    sl = np.array([blocks[b][0] for b in bi], np.int32)
+    sx = np.array([rng.integers(0, blocks[b][2]) for b in bi], np.int32)
+    sy = np.array([rng.integers(0, blocks[b][3]) for b in bi], np.int32)
+    idx = np.array([blocks[b][4] + x * blocks[b][3] + y for b, x, y in zip(bi, sx, sy)], np.int64)
+    ref = oracle.apply_samples(p, psi, sl, sx, sy)
+    assert np.linalg.norm(out[idx] - ref) <= TOL * np.linalg.norm(ref)
+    y = workloads.make_psi(p, 1)
+    Hy = g.apply(y)
+    assert abs(psi @ Hy - out @ y) <= 1e-12 * np.linalg.norm(psi) * np.linalg.norm(Hy)
+    assert np.array_equal(out, g.apply(psi))                       # bitwise reproducible at full size

@@ -190,3 +190,40 @@ def test_struct_sizes():
     assert ctypes.sizeof(H.binding.hpsi_sectors_t) == 48
     assert ctypes.sizeof(H.binding.hpsi_terms_t) == 80
     assert H.binding.PSI_BLOCK_DTYPE.itemsize == 24 and H.binding.TASK_DTYPE.itemsize == 24
+
+
+# --------------------------------------------------------------------------------- tile / warp-grid policy
+def test_schedule_balance_on_cyp_shapes():
+    """The planner's tile split (even fragment counts, at most one odd tile per dimension) and per-unit warp grid keep
+    the heaviest warp of a CTA close to the mean: issued / critical-path DMMA flops >= 0.97 on the cyp-shaped config
+    (it was 0.865 with an even split and a fixed 2x2 grid), and padding to 8x8x4 fragments costs < 7 %."""
+    p = workloads.make_problem("cyp", fill=False)
+    plan = host_plan(p)
+    useful, issued = H.hpsi_query(plan, H.HPSI_Q_USEFUL_FLOPS), H.hpsi_query(plan, H.HPSI_Q_ISSUED_FLOPS)
+    critical = H.hpsi_query(plan, H.HPSI_Q_CRITICAL_FLOPS)
+    assert useful <= issued <= critical
+    assert issued / critical >= 0.97
+    assert useful / issued >= 0.93
+    # ~32 waves of P2 units on 148 SMs x 4 slots, and P1 units that bundle several terms
+    assert 148 * 4 * 16 <= H.hpsi_query(plan, H.HPSI_Q_N_P2_UNITS) <= 148 * 4 * 64
+    assert H.hpsi_query(plan, H.HPSI_Q_N_P1_UNITS) < H.hpsi_query(plan, H.HPSI_Q_N_TASKS)
+
+
+def test_interpreter_parity_with_uneven_tiles():
+    """Dimensions whose fragment counts exercise every branch of the tile split (9, 10, 13, 15, 17 fragments) and of
+    the warp-grid choice, through the host interpreter of the device schedule."""
+    rng = np.random.default_rng(17)
+    dL, dR = [72, 80, 104, 9], [120, 136, 65, 130]
+    n = len(dL)
+    terms = []
+    for _ in range(3):
+        ab = {(r, c): rng.standard_normal((dL[r], dL[c])) for r in range(n) for c in range(n) if (r + c) % 3 != 1}
+        bb = {(r, c): rng.standard_normal((dR[r], dR[c])) for r in range(n) for c in range(n) if (r + c) % 3 != 1}
+        terms.append((float(rng.standard_normal()), ab, bb))
+    p = workloads.custom_problem([(i, 0) for i in range(n)], dL, [(n - i, 0) for i in range(n)], dR, (n, 0), terms,
+                                 pad_even=True)
+    psi = rng.standard_normal(p.psi_len)
+    ref = oracle.apply(p, psi)
+    for flags in (0, H.HPSI_PLAN_FIXED_ORDER1, H.HPSI_PLAN_FIXED_ORDER2):
+        plan = host_plan(p, flags)
+        assert rel(H.hpsi_debug_interpret(plan, p.a_data, p.b_data, psi), ref) <= 1e-13
