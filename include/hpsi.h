@@ -87,6 +87,13 @@ int hpsi_plan(const hpsi_sectors_t* sectors, const hpsi_terms_t* terms, uint32_t
  * (host work proportional to the number of blocks; synchronous). */
 int hpsi_bind(hpsi_plan_t* plan, const double* a_data_dev, const double* b_data_dev);
 
+/* Per-task coupling coefficients (reading A4): replaces the coefficient of every task,
+ * which hpsi_plan initialises to c_term - e.g. SU(2) recoupling factors that depend on the sector quadruple
+ * (l, l', r, r') and not only on the term ("spin adapted", "SU(2)-aware").
+ * coef_host: HOST, n doubles with n == HPSI_Q_N_TASKS, in HPSI_Q_TASKS order.  Synchronous; must not be called while
+ * an apply of this plan is in flight.  hpsi_apply, hpsi_diagonal and hpsi_davidson all use the new values. */
+int hpsi_set_task_coefficients(hpsi_plan_t* plan, const double* coef_host, int64_t n);
+
 /* Steps 5-7: out = H psi (overwrite).  psi_dev / out_dev: DEVICE, psi_length doubles each, must not alias.
  * cuda_stream: a cudaStream_t cast to void* (NULL = default stream).  Enqueue only: no host sync, no
  * allocation, CUDA-graph capturable.  A plan owns one workspace: do not run it on two streams at once.

@@ -71,6 +71,7 @@ def lib() -> ctypes.CDLL:
         L.hpsi_plan.argtypes = [ctypes.POINTER(hpsi_sectors_t), ctypes.POINTER(hpsi_terms_t), ctypes.c_uint32,
                                 ctypes.POINTER(vp)]
         L.hpsi_bind.argtypes = [vp, vp, vp]
+        L.hpsi_set_task_coefficients.argtypes = [vp, vp, i64]
         L.hpsi_apply.argtypes = [vp, vp, vp, vp]
         L.hpsi_apply_host.argtypes = [vp, vp, vp, vp]
         L.hpsi_apply_profiled.argtypes = [vp, vp, vp, vp, ctypes.POINTER(ctypes.c_float)]
@@ -84,7 +85,7 @@ def lib() -> ctypes.CDLL:
         L.hpsi_bench_fp64_pipe.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.POINTER(ctypes.c_double),
                                            ctypes.POINTER(ctypes.c_double)]
         L.hpsi_debug_interpret.argtypes = [vp, vp, vp, vp, vp]
-        for name in ("hpsi_plan", "hpsi_bind", "hpsi_apply", "hpsi_apply_host", "hpsi_apply_profiled", "hpsi_diagonal", "hpsi_davidson",
+        for name in ("hpsi_plan", "hpsi_bind", "hpsi_set_task_coefficients", "hpsi_apply", "hpsi_apply_host", "hpsi_apply_profiled", "hpsi_diagonal", "hpsi_davidson",
                      "hpsi_query", "hpsi_bench_fp64_pipe", "hpsi_debug_interpret"):
             getattr(L, name).restype = ctypes.c_int
         del i32, i64
@@ -155,6 +156,12 @@ def hpsi_plan(q_left, q_right, d_left, d_right, target, coef, a_blocks, b_blocks
 def hpsi_bind(plan: Plan, a_data, b_data) -> None:
     _check(lib().hpsi_bind(plan.handle, _ptr(a_data), _ptr(b_data)))
     plan._keep = (a_data, b_data)
+
+
+def hpsi_set_task_coefficients(plan: Plan, coef) -> None:
+    """Per-task coefficients (numpy float64, HPSI_Q_TASKS order) replacing c_term."""
+    coef = np.ascontiguousarray(coef, np.float64)
+    _check(lib().hpsi_set_task_coefficients(plan.handle, coef.ctypes.data, coef.shape[0]))
 
 
 def hpsi_apply(plan: Plan, psi, out, stream=None) -> None:

@@ -84,6 +84,7 @@ void free_plan(hpsi_plan_t* p) {
     cudaFree(p->d_psi_stage);
     cudaFree(p->d_out_stage);
     cudaFree(p->d_dav);
+    cudaFreeHost(p->h_dav);
     cudaGetLastError();
   }
   delete p;
@@ -185,6 +186,22 @@ extern "C" int hpsi_plan(const hpsi_sectors_t* sectors, const hpsi_terms_t* term
     return HPSI_ENOMEM;
   }
   *plan_out = p;
+  return HPSI_OK;
+}
+
+extern "C" int hpsi_set_task_coefficients(hpsi_plan_t* p, const double* coef_host, int64_t n) {
+  if (!p || !coef_host) { set_error("null argument"); return HPSI_EINVAL; }
+  Schedule& sc = p->sc;
+  if (n != (int64_t)sc.segs.size()) { set_error("coefficient count != number of tasks (HPSI_Q_N_TASKS)"); return HPSI_EINVAL; }
+  for (int64_t i = 0; i < n; ++i) sc.segs[i].coef = coef_host[i];
+  for (DiagTask& t : sc.diag) t.coef = coef_host[t.seg];
+  if (!p->host_only) {
+    HPSI_CUDA(cudaDeviceSynchronize());
+    if (!sc.segs.empty())
+      HPSI_CUDA(cudaMemcpy(const_cast<Seg*>(p->dev.segs), sc.segs.data(), sc.segs.size() * sizeof(Seg), cudaMemcpyHostToDevice));
+    if (!sc.diag.empty())
+      HPSI_CUDA(cudaMemcpy(const_cast<DiagTask*>(p->dev.diag), sc.diag.data(), sc.diag.size() * sizeof(DiagTask), cudaMemcpyHostToDevice));
+  }
   return HPSI_OK;
 }
 

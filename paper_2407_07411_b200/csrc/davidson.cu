@@ -164,6 +164,7 @@ extern "C" int hpsi_davidson(hpsi_plan_t* p, double* psi, double* eig_host, cons
     }
     p->dav_doubles = need;
   }
+  if (!p->h_dav) HPSI_CUDA(cudaMallocHost(&p->h_dav, 8 * sizeof(double)));
   double* V = p->d_dav;
   double* W = V + (size_t)prm.m_max * n;
   double* diag = W + (size_t)prm.m_max * n;
@@ -206,7 +207,7 @@ extern "C" int hpsi_davidson(hpsi_plan_t* p, double* psi, double* eig_host, cons
     }
     dots(s, 1, s, nrm + 3, 1, nullptr, 0);                          // nrm[3] = |s|^2
     scale_kernel<<<eg, 256, 0, st>>>(V + (size_t)j * n, s, nullptr, nullptr, nrm + 3, n);
-    double hostbuf[5];
+    double* hostbuf = p->h_dav;
     HPSI_CUDA(cudaMemcpyAsync(hostbuf, theta, 5 * sizeof(double), cudaMemcpyDeviceToHost, st));
     HPSI_CUDA(cudaStreamSynchronize(st));
     th = hostbuf[0];

@@ -104,6 +104,8 @@ struct DiagTask {             // sector-diagonal task (for diag(H))
   int64_t a_off, b_off;
   int32_t a_ld, b_ld;
   double coef;
+  int32_t seg;                // the task (index into segs) this entry belongs to
+  int32_t pad;
 };
 
 struct Schedule {

@@ -24,6 +24,7 @@ struct hpsi_plan {
   double* d_dav = nullptr;
   size_t dav_doubles = 0;
   int dav_mmax = 0;
+  double* h_dav = nullptr;        // pinned host scalars the Davidson loop reads back each iteration
 };
 
 namespace hpsi {

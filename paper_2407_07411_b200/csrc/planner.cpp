@@ -235,7 +235,7 @@ int build_schedule(const hpsi_sectors_t* s, const hpsi_terms_t* t, uint32_t flag
       sc->intermediate_bytes += 8 * (int64_t)g.rows * g.N1;
       if (order == 1) sc->n_order1++;
       if (raw[q].src == raw[q].dst)
-        diag_by_blk[raw[q].dst].push_back({a.offset, b.offset, a.ld, b.ld, t->coef[raw[q].term]});
+        diag_by_blk[raw[q].dst].push_back({a.offset, b.offset, a.ld, b.ld, t->coef[raw[q].term], (int32_t)sc->segs.size() - 1, 0});
     }
     ws = align_up(ws + per_task * g.tcount, 16);
     sc->groups.push_back(g);
@@ -255,7 +255,7 @@ int build_schedule(const hpsi_sectors_t* s, const hpsi_terms_t* t, uint32_t flag
   sc->issued_flops_p1 = 0;
   sc->critical_flops = 0;
   {
-    constexpr int P1_STAGES_PER_UNIT = 96;
+    const int P1_STAGES_PER_UNIT = getenv("HPSI_P1_STAGES") ? std::max(1, atoi(getenv("HPSI_P1_STAGES"))) : 96;   // tuning experiments
     struct GOrder { int64_t cost; int gi; };
     std::vector<GOrder> gorder;
     std::vector<int> g_nt(sc->groups.size());
@@ -310,7 +310,8 @@ int build_schedule(const hpsi_sectors_t* s, const hpsi_terms_t* t, uint32_t flag
     total_p2_dmma += (int64_t)frags(sc->blocks[d].rows) * frags(sc->blocks[d].cols) * dsts[d].ksteps;
   const int waves = getenv("HPSI_P2_WAVES") ? std::max(1, atoi(getenv("HPSI_P2_WAVES"))) : 32;   // tuning experiments
   const int64_t slots = (int64_t)std::max(n_sm, 1) * 4 * waves;  // 4 resident CTAs per SM, ~32 waves (small units keep the tail of the launch short)
-  const int64_t target = std::max<int64_t>(64 * 4 * 24, total_p2_dmma / slots);
+  const int64_t min_target = getenv("HPSI_P2_MIN") ? std::max(1, atoi(getenv("HPSI_P2_MIN"))) : 1536;   // DMMA per unit at least (~10 us of a CTA)
+  const int64_t target = std::max<int64_t>(min_target, total_p2_dmma / slots);
 
   sc->runs.clear(); sc->p2.clear();
   std::vector<int> unit_bundle;            // (block, split) bundle of each unit

@@ -271,3 +271,23 @@ def test_full_size_sampled_parity(H, cfg):
     Hy = g.apply(y)
     assert abs(psi @ Hy - out @ y) <= 1e-12 * np.linalg.norm(psi) * np.linalg.norm(Hy)
     assert np.array_equal(out, g.apply(psi))                       # bitwise reproducible at full size
+
+
+def test_task_coefficients(H, toy):
+    """hpsi_set_task_coefficients: per-(t, l, l', r, r') factors; checked against the oracle on the same operator
+    written with one term per task; hpsi_diagonal follows."""
+    import torch
+    from test_planner_cpu import exploded_problem
+    p = workloads.make_problem("small", n_terms=30)
+    for prob in (toy, p):
+        g = GpuProblem(prob)
+        f = np.random.default_rng(9).standard_normal(g.q(H.HPSI_Q_N_TASKS))
+        H.hpsi_set_task_coefficients(g.plan, f)
+        ex = exploded_problem(prob, g.plan, f)
+        psi = workloads.make_psi(prob)
+        assert rel_l2(g.apply(psi), oracle.apply(ex, psi)) <= TOL
+        d = torch.empty(g.n, dtype=torch.float64, device="cuda")
+        H.hpsi_diagonal(g.plan, d)
+        torch.cuda.synchronize()
+        ref = oracle.diagonal(ex)
+        assert np.linalg.norm(d.cpu().numpy() - ref) <= 1e-12 * max(np.linalg.norm(ref), 1.0)

@@ -227,3 +227,32 @@ def test_interpreter_parity_with_uneven_tiles():
     for flags in (0, H.HPSI_PLAN_FIXED_ORDER1, H.HPSI_PLAN_FIXED_ORDER2):
         plan = host_plan(p, flags)
         assert rel(H.hpsi_debug_interpret(plan, p.a_data, p.b_data, psi), ref) <= 1e-13
+
+
+# ------------------------------------------------------------------------------ per-task coefficients (8(f)-2)
+def exploded_problem(p, plan, task_coef):
+    """The same operator with every task turned into its own one-block term carrying the task's coefficient: what
+    hpsi_set_task_coefficients must compute, expressed in the boundary's plain per-term form for the oracle."""
+    tasks = H.hpsi_query(plan, H.HPSI_Q_TASKS)
+    terms = []
+    for t, f in zip(tasks, task_coef):
+        ea, eb = p.a_desc[int(t["a_block"])], p.b_desc[int(t["b_block"])]
+        terms.append((float(f), {(int(ea["row"]), int(ea["col"])): p.block("a", int(t["a_block"]))},
+                      {(int(eb["row"]), int(eb["col"])): p.block("b", int(t["b_block"]))}))
+    return workloads.custom_problem(p.q_left, p.d_left, p.q_right, p.d_right, p.target, terms)
+
+
+def test_task_coefficients_interpreter(toy):
+    plan = host_plan(toy)
+    n_tasks = H.hpsi_query(plan, H.HPSI_Q_N_TASKS)
+    f = np.random.default_rng(5).standard_normal(n_tasks)
+    with pytest.raises(H.HpsiError):
+        H.hpsi_set_task_coefficients(plan, f[:-1])
+    H.hpsi_set_task_coefficients(plan, f)
+    psi = workloads.make_psi(toy)
+    ref = oracle.apply(exploded_problem(toy, plan, f), psi)
+    assert rel(H.hpsi_debug_interpret(plan, toy.a_data, toy.b_data, psi), ref) <= 1e-13
+    # back to the per-term coefficients
+    tasks = H.hpsi_query(plan, H.HPSI_Q_TASKS)
+    H.hpsi_set_task_coefficients(plan, toy.coef[tasks["term"]])
+    assert rel(H.hpsi_debug_interpret(plan, toy.a_data, toy.b_data, psi), oracle.apply(toy, psi)) <= 1e-13
