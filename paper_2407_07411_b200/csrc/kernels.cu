@@ -2,14 +2,16 @@
 // P2 (segmented-K second GEMM with split-K partials), reduce (ordered sum of partials), diag.
 // See kernels.cuh / plan.h for the vocabulary.
 //
-// GEMM CTA = 1 producer warp + 4 consumer warps (warp-specialised, mbarrier ring of NSTAGE stages):
+// GEMM CTA = 1 producer warp + NCONS consumer warps (warp-specialised, mbarrier ring of NSTAGE stages).  Default:
+// NCONS = 4 on a <=64x64 tile, 3 CTAs per SM; HPSI_BIG_CTA=1 compiles 8 consumer warps on a <=128x64 tile, 2 CTAs per SM
+// (measured slower on B200: 27.7 vs 31.9 TFLOPS on the cyp config).
 //   producer : one elected lane issues two TMA tile loads per stage (cp.async.bulk.tensor.2d: a 64-row x 16-column
 //              box of the X operand and one of the Y operand, 128-byte swizzle, rows / columns past the matrix edge
 //              zero-filled by the hardware) that complete on the stage's "full" mbarrier (complete_tx::bytes).
 //              Measured on B200 for this access pattern: TMA boxes feed 6.1-6.9 TB/s from HBM and 12-13.9 TB/s from L2,
 //              16-byte LDGSTS 4.8 / 6.4 TB/s.  Matrices whose rows are not 16-byte aligned take the LDGSTS variant
 //              (8-byte cp.async with zero fill into the same swizzled layout).
-//   consumers: 4 warps as a 2x2, 1x4 or 4x1 grid, each <= 16 fragments of DMMA.8x8x4 with register accumulators; a warp waits only on the
+//   consumers: a (NCONS / gn) x gn grid of warps, each <= 16 fragments of DMMA.8x8x4 with register accumulators; a warp waits only on the
 //              "full" barrier of its next stage and releases the stage on its "empty" barrier - no CTA-wide barrier
 //              in the main loop.
 //
@@ -79,13 +81,13 @@ __device__ __forceinline__ void split_frags(int f, int parts, int p, int& first,
   count = base + (p < rem ? 1 : 0);
   first = p * base + (p < rem ? p : rem);
 }
-// The 4 consumer warps cover the tile as a 2x2, 1x4 or 4x1 grid (plan.h WarpGrid; chosen per unit by the planner so
-// that the heaviest warp is as light as possible); a warp owns at most 16 fragments: <=4x4, <=8x2 or <=2x8.
+// The consumer warps cover the tile as a (NCONS / gn) x gn grid (gn = the unit's `grid`, chosen by the planner so that
+// the heaviest warp is as light as possible); a warp owns at most 16 fragments: <=4x4, <=8x2 or <=2x8.
 struct WarpTile {
   int wr0, wc0;    // first row / col of the warp inside the CTA tile (multiples of 8)
   int mi, nj;      // fragments owned
-  __device__ __forceinline__ WarpTile(int grid, int warp, int rows_valid, int cols_valid) {
-    const int gn = grid == GRID_2x2 ? 2 : (grid == GRID_1x4 ? 4 : 1), gm = NCONS / gn;
+  __device__ __forceinline__ WarpTile(int gn, int warp, int rows_valid, int cols_valid) {
+    const int gm = NCONS / gn;
     int f0;
     split_frags((rows_valid + 7) >> 3, gm, warp / gn, f0, mi);
     wr0 = f0 * 8;
@@ -173,7 +175,7 @@ __device__ __forceinline__ void store_tile(double* dst, int ld, int rows_valid, 
 // Which tile quadrant consumer warp 0 takes.  Consumer warp w sits on SM sub-partition w, and with odd fragment counts
 // the quadrants carry unequal DMMA counts (e.g. 16/12/12/9), so co-resident CTAs must not all put their heavy
 // quadrant on the same sub-partition.  CTAs are dealt to SMs round-robin (148 = 0 mod 4), hence a hash, not bid & 3.
-__device__ __forceinline__ int quadrant_rotation(unsigned bid) { return (int)((bid * 2654435761u) >> 29); }
+__device__ __forceinline__ int quadrant_rotation(unsigned bid) { return (int)((bid * 2654435761u) >> 28); }
 
 // Shared-memory carve-up: NSTAGE stages of [X tile | Y tile] (1024-byte aligned), then the barriers.
 struct SmemLayout {
@@ -243,7 +245,7 @@ __device__ __forceinline__ void p1_consume(const DevSchedule& d, const P1Unit& u
       mbar_wait(sm.full(ring.stage), ring.phase);
       if (d.debug != 2) {
         const double* st = sm.stage_ptr(ring.stage);
-        mma_stage<MI, NJ>(st + w.wr0 * 16, st + OP_BYTES / 8 + w.wc0 * 16, lo, acc, kt == ntiles - 1 ? last_nk4 : 4);
+        mma_stage<MI, NJ>(st + w.wr0 * 16, st + X_BOXES * OP_BYTES / 8 + w.wc0 * 16, lo, acc, kt == ntiles - 1 ? last_nk4 : 4);
       }
       __syncwarp();
       if (lane == 0) mbar_arrive(sm.empty(ring.stage));
@@ -274,7 +276,7 @@ __device__ __forceinline__ void idle_consume(const SmemLayout& sm, int nstages, 
   }
 
 template <bool TMA>
-__global__ void __launch_bounds__(NTHREADS, CTAS_PER_SM) p1_kernel(DevSchedule d) {
+__global__ void __maxnreg__(HPSI_BIG_CTA ? 112 : 136) p1_kernel(DevSchedule d) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const P1Unit u = d.p1[blockIdx.x];
   const Group g = d.groups[u.group];
@@ -289,6 +291,7 @@ __global__ void __launch_bounds__(NTHREADS, CTAS_PER_SM) p1_kernel(DevSchedule d
     const unsigned char* ymap = d.maps + (int64_t)g.y1_map * TMAP_BYTES;
     const double* ybase = d.ws + g.y1_off + (int64_t)u.j0 * g.ldy1;
     const double* xarena = (g.order == 1) ? d.a : d.b;
+    const int xboxes = (u.rows_valid + TILE - 1) / TILE;          // 64-row boxes of the X tile that hold valid rows
     for (int t = u.t0; t < u.t1; ++t) {
       const Seg* sg = d.segs + g.seg0 + t;
       const unsigned char* xmap = nullptr;
@@ -298,18 +301,19 @@ __global__ void __launch_bounds__(NTHREADS, CTAS_PER_SM) p1_kernel(DevSchedule d
       else { xld = sg->p1_ld; xbase = xarena + sg->p1_off + (int64_t)u.i0 * xld; }
       for (int kt = 0; kt < ntiles; ++kt) {
         mbar_wait(sm.empty(ring.stage), ring.phase);
-        const uint32_t sx = sm.stage(ring.stage), sy = sx + OP_BYTES, full = sm.full(ring.stage);
+        const uint32_t sx = sm.stage(ring.stage), sy = sx + X_BOXES * OP_BYTES, full = sm.full(ring.stage);
         if (TMA) {
           if (lane == 0) {
-            mbar_arrive_expect_tx(full, d.debug == 1 ? 0 : STAGE_BYTES);
+            mbar_arrive_expect_tx(full, d.debug == 1 ? 0 : (xboxes + 1) * OP_BYTES);
             if (d.debug != 1) {
-              tma_load_2d(sx, xmap, kt * KT, u.i0, full);
+              for (int bx = 0; bx < xboxes; ++bx) tma_load_2d(sx + bx * OP_BYTES, xmap, kt * KT, u.i0 + bx * TILE, full);
               tma_load_2d(sy, ymap, kt * KT, u.j0, full);
             }
           }
         } else {
           if (d.debug != 1) {
-            ldgsts_tile(sx, xbase, xld, u.rows_valid, kt * KT, g.K1, lane);
+            for (int bx = 0; bx < xboxes; ++bx)
+              ldgsts_tile(sx + bx * OP_BYTES, xbase + bx * TILE * xld, xld, u.rows_valid - bx * TILE, kt * KT, g.K1, lane);
             ldgsts_tile(sy, ybase, g.ldy1, u.cols_valid, kt * KT, g.K1, lane);
           }
           cp_async_mbar_arrive(full);
@@ -368,7 +372,7 @@ __device__ __forceinline__ void p2_consume(const DevSchedule& d, const P2Unit& u
     mbar_wait(sm.full(ring.stage), ring.phase);
     if (d.debug != 2) {
       const double* st = sm.stage_ptr(ring.stage);
-      mma_stage<MI, NJ>(st + w.wr0 * 16, st + OP_BYTES / 8 + w.wc0 * 16, lo, acc, it.nk4());
+      mma_stage<MI, NJ>(st + w.wr0 * 16, st + X_BOXES * OP_BYTES / 8 + w.wc0 * 16, lo, acc, it.nk4());
     }
     __syncwarp();
     if (lane == 0) mbar_arrive(sm.empty(ring.stage));
@@ -378,7 +382,7 @@ __device__ __forceinline__ void p2_consume(const DevSchedule& d, const P2Unit& u
 }
 
 template <bool TMA>
-__global__ void __launch_bounds__(NTHREADS, CTAS_PER_SM) p2_kernel(DevSchedule d) {
+__global__ void __maxnreg__(HPSI_BIG_CTA ? 112 : 136) p2_kernel(DevSchedule d) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const P2Unit u = d.p2[blockIdx.x];
   const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
@@ -389,6 +393,7 @@ __global__ void __launch_bounds__(NTHREADS, CTAS_PER_SM) p2_kernel(DevSchedule d
     // ---------------- producer warp
     KIter it(d.runs, u.run_begin, u.run_end);
     Ring ring{0, 1};
+    const int xboxes = (u.rows_valid + TILE - 1) / TILE;          // 64-row boxes of the X tile that hold valid rows
     const unsigned char *xmap = nullptr, *ymap = nullptr;      // TMA: tensor maps and first rows of the segment
     int xrow = 0, yrow = 0;
     const double *xbase = nullptr, *ybase = nullptr;           // LDGSTS: first rows and leading dimensions
@@ -416,18 +421,19 @@ __global__ void __launch_bounds__(NTHREADS, CTAS_PER_SM) p2_kernel(DevSchedule d
     if (it.valid) open_seg();
     while (it.valid) {
       mbar_wait(sm.empty(ring.stage), ring.phase);
-      const uint32_t sx = sm.stage(ring.stage), sy = sx + OP_BYTES, full = sm.full(ring.stage);
+      const uint32_t sx = sm.stage(ring.stage), sy = sx + X_BOXES * OP_BYTES, full = sm.full(ring.stage);
       if (TMA) {
         if (lane == 0) {
-          mbar_arrive_expect_tx(full, d.debug == 1 ? 0 : STAGE_BYTES);
+          mbar_arrive_expect_tx(full, d.debug == 1 ? 0 : (xboxes + 1) * OP_BYTES);
           if (d.debug != 1) {
-            tma_load_2d(sx, xmap, it.kappa, xrow, full);
+            for (int bx = 0; bx < xboxes; ++bx) tma_load_2d(sx + bx * OP_BYTES, xmap, it.kappa, xrow + bx * TILE, full);
             tma_load_2d(sy, ymap, it.kappa, yrow, full);
           }
         }
       } else {
         if (d.debug != 1) {
-          ldgsts_tile(sx, xbase, xld, u.rows_valid, it.kappa, it.K, lane);
+          for (int bx = 0; bx < xboxes; ++bx)
+            ldgsts_tile(sx + bx * OP_BYTES, xbase + bx * TILE * xld, xld, u.rows_valid - bx * TILE, it.kappa, it.K, lane);
           ldgsts_tile(sy, ybase, yld, u.cols_valid, it.kappa, it.K, lane);
         }
         cp_async_mbar_arrive(full);

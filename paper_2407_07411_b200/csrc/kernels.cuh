@@ -12,10 +12,11 @@ namespace hpsi {
 
 constexpr int NCONS = NCONS_WARPS;                     // consumer (DMMA) warps per CTA, as a 2x2, 1x4 or 4x1 grid over the tile
 constexpr int NTHREADS = (NCONS + 1) * 32;     // + 1 producer warp
-constexpr int CTAS_PER_SM = 3;
+constexpr int CTAS_PER_SM = HPSI_BIG_CTA ? 2 : 3;
 constexpr int NSTAGE = 4;
-constexpr int OP_BYTES = TILE * KT * 8;        // one operand tile of a stage: 64 rows x 128 bytes, 128-byte swizzled
-constexpr int STAGE_BYTES = 2 * OP_BYTES;      // X tile | Y tile
+constexpr int OP_BYTES = TILE * KT * 8;        // one TMA box: 64 rows x 128 bytes, 128-byte swizzled
+constexpr int X_BOXES = TILE_M / TILE;         // the X tile of a stage is X_BOXES boxes one under the other
+constexpr int STAGE_BYTES = (X_BOXES + 1) * OP_BYTES;   // X tile | Y tile
 // 1024 bytes of slack to align the stages (the swizzle pattern is a function of address bits 4-9) | stages | barriers
 constexpr int SMEM_BYTES = 1024 + NSTAGE * STAGE_BYTES + 2 * NSTAGE * 8;
 constexpr int TMAP_BYTES = 128;                // sizeof(CUtensorMap)

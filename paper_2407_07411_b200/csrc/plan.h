@@ -19,13 +19,17 @@
 
 namespace hpsi {
 
-constexpr int TILE = 64;      // CTA tile edge (rows and cols), 8 fragments of 8
+#ifndef HPSI_BIG_CTA
+#define HPSI_BIG_CTA 0        // 1: CTA tile <= 128 x 64 with 8 consumer warps, 2 CTAs / SM; 0: <= 64 x 64 with 4 warps, 3 CTAs / SM
+#endif
+constexpr int TILE = 64;      // CTA tile columns (max) and rows of one TMA box, 8 fragments of 8
+constexpr int TILE_M = HPSI_BIG_CTA ? 128 : 64;   // CTA tile rows (max)
 constexpr int KT = 16;        // K extent of one staged tile (4 DMMA k-steps)
-constexpr int NCONS_WARPS = 4; // consumer (DMMA) warps per CTA
+constexpr int NCONS_WARPS = HPSI_BIG_CTA ? 8 : 4;   // consumer (DMMA) warps per CTA
 
 enum BaseSel : int32_t { BASE_A = 0, BASE_B = 1, BASE_WS = 2 };
-// how the 4 consumer warps of a CTA cover its tile (rows x columns of warps)
-enum WarpGrid : int32_t { GRID_2x2 = 0, GRID_1x4 = 1, GRID_4x1 = 2 };
+// How the consumer warps of a CTA cover its tile: P1Unit / P2Unit `grid` = number of warp COLUMNS gn (a power of two
+// dividing NCONS_WARPS); the warps form a (NCONS_WARPS / gn) x gn grid.
 
 struct Seg {                  // one task, in schedule order (by destination, source, term)
   int64_t p1_off;             // operator block used by P1 (order 1: A_t, order 2: B_t), doubles into its arena
@@ -139,14 +143,22 @@ inline int even_up(int x) { return x + (x & 1); }
 // 128-byte row segment is exactly four sectors (measured: 16-byte-aligned rows cost 1.4x the sectors).
 inline int sector_up(int x) { return (x + 3) & ~3; }
 inline int frags(int x) { return (x + 7) / 8; }
-// Heaviest warp (in fragments) when a tile of fm x fn fragments is covered by 4 warps as a gm x gn grid, and the grid
-// that minimises it (ties: 2x2, which needs the fewest shared-memory reads per DMMA).
+// Heaviest warp (in fragments) when a tile of fm x fn fragments is covered by a gm x gn grid of warps, and the grid
+// that minimises it among those whose warp tile has a compiled instantiation (<=4x4, <=8x2, <=2x8 fragments);
+// ties go to the squarest grid (fewest shared-memory reads per DMMA).
 inline int heaviest_warp(int fm, int fn, int gm, int gn) { return ((fm + gm - 1) / gm) * ((fn + gn - 1) / gn); }
+inline bool warp_tile_ok(int mi, int nj) { return (mi <= 4 && nj <= 4) || (mi <= 8 && nj <= 2) || (mi <= 2 && nj <= 8); }
 inline int32_t best_grid(int fm, int fn, int* heaviest = nullptr) {
-  int best = heaviest_warp(fm, fn, 2, 2);
-  int32_t g = GRID_2x2;
-  if (heaviest_warp(fm, fn, 1, 4) < best) { best = heaviest_warp(fm, fn, 1, 4); g = GRID_1x4; }
-  if (heaviest_warp(fm, fn, 4, 1) < best) { best = heaviest_warp(fm, fn, 4, 1); g = GRID_4x1; }
+  const int order[4] = {NCONS_WARPS == 8 ? 2 : 2, NCONS_WARPS == 8 ? 4 : 4, 1, NCONS_WARPS};   // squarest first
+  int best = 1 << 30;
+  int32_t g = 2;
+  for (int gn : order) {
+    if (gn > NCONS_WARPS || NCONS_WARPS % gn) continue;
+    const int gm = NCONS_WARPS / gn;
+    if (!warp_tile_ok((fm + gm - 1) / gm, (fn + gn - 1) / gn)) continue;
+    const int h = heaviest_warp(fm, fn, gm, gn);
+    if (h < best) { best = h; g = gn; }
+  }
   if (heaviest) *heaviest = best;
   return g;
 }

@@ -23,19 +23,24 @@ namespace {
 
 struct Tile1D { int start, len; };
 
-// Split of a dimension into tiles of at most 8 fragments (64).  Inside a CTA the tile is cut again in halves between
-// the consumer warps, so a tile with an odd fragment count leaves one warp row (or column) a fragment short; sizes are
-// therefore balanced in units of TWO fragments and at most one tile (the last) is odd.  On the cyp config this raises
-// issued / critical-path DMMA from 0.865 to 0.954.
-std::vector<Tile1D> split_dim(int64_t n) {
+// Split of a dimension into tiles of at most max_frags fragments.  Inside a CTA the tile is cut again between the
+// consumer warps (2 or 4 ways per dimension), so tile sizes are multiples of `unit` fragments wherever possible and
+// only the last tile takes the remainder: a tile with an odd fragment count leaves a warp row (or column) short and
+// the whole CTA waits for its heaviest warp.  (cyp, 64x64 tiles: issued / critical-path DMMA 0.865 with an even
+// split, 0.954 with unit 2.)
+std::vector<Tile1D> split_dim(int64_t n, int max_frags, int unit) {
   std::vector<Tile1D> out;
   if (n <= 0) return out;
   const int64_t F = (n + 7) / 8;
-  const int64_t nt = (F + 7) / 8;
-  const int64_t P = F / 2, base = P / nt, rem = P % nt;
+  const int64_t nt = (F + max_frags - 1) / max_frags;
   std::vector<int64_t> fr(nt);
-  for (int64_t i = 0; i < nt; ++i) fr[i] = 2 * (base + (i < rem ? 1 : 0));
-  if (F & 1) fr[nt - 1] += 1;                      // the last tile is the smallest (or tied): it takes the odd fragment
+  const int64_t P = F / unit, base = P / nt, rem = P % nt;
+  for (int64_t i = 0; i < nt; ++i) fr[i] = unit * (base + (i < rem ? 1 : 0));
+  fr[nt - 1] += F - unit * P;                      // the last tile is the smallest (or tied): it takes the remainder
+  if (*std::max_element(fr.begin(), fr.end()) > max_frags) {      // cannot happen for unit | max_frags; keep it safe
+    const int64_t b2 = F / nt, r2 = F % nt;
+    for (int64_t i = 0; i < nt; ++i) fr[i] = b2 + (i < r2 ? 1 : 0);
+  }
   int64_t start = 0;
   for (int64_t i = 0; i < nt; ++i) {
     if (fr[i] == 0) continue;
@@ -45,6 +50,9 @@ std::vector<Tile1D> split_dim(int64_t n) {
   }
   return out;
 }
+// rows: up to TILE_M; columns: up to TILE.  Units: half of what the warp grid cuts each dimension into.
+std::vector<Tile1D> split_rows(int64_t n) { return split_dim(n, TILE_M / 8, HPSI_BIG_CTA ? 8 : 2); }
+std::vector<Tile1D> split_cols(int64_t n) { return split_dim(n, TILE / 8, HPSI_BIG_CTA ? 4 : 2); }
 
 int64_t align_up(int64_t x, int64_t a) { return (x + a - 1) / a * a; }
 
@@ -266,14 +274,14 @@ int build_schedule(const hpsi_sectors_t* s, const hpsi_terms_t* t, uint32_t flag
       const int nchunk = (g.tcount + nt - 1) / nt;
       nt = (g.tcount + nchunk - 1) / nchunk;                    // even chunks
       g_nt[gi] = nt;
-      const int fr = std::min(frags(g.rows), TILE / 8), fc = std::min(frags(g.N1), TILE / 8);
+      const int fr = std::min(frags(g.rows), TILE_M / 8), fc = std::min(frags(g.N1), TILE / 8);
       gorder.push_back({(int64_t)fr * fc * ((g.K1 + 3) / 4) * nt, (int)gi});
     }
     std::stable_sort(gorder.begin(), gorder.end(), [](const GOrder& x, const GOrder& y) { return x.cost > y.cost; });
     for (const GOrder& go : gorder) {
       const Group& g = sc->groups[go.gi];
-      auto rt = split_dim(g.rows);
-      auto ct = split_dim(g.N1);
+      auto rt = split_rows(g.rows);
+      auto ct = split_cols(g.N1);
       const int64_t ks = (g.K1 + 3) / 4;
       const int nt = g_nt[go.gi];
       for (int t0 = 0; t0 < g.tcount; t0 += nt) {
@@ -323,8 +331,8 @@ int build_schedule(const hpsi_sectors_t* s, const hpsi_terms_t* t, uint32_t flag
     D.part_off = ws;
     D.nsplit = 0;
     if (dsts[d].nseg == 0) continue;
-    auto rt = split_dim(D.rows);
-    auto ct = split_dim(D.cols);
+    auto rt = split_rows(D.rows);
+    auto ct = split_cols(D.cols);
     int maxf = 0;
     for (auto& r : rt) for (auto& c : ct) maxf = std::max(maxf, frags(r.len) * frags(c.len));
     int64_t nsplit = (maxf * dsts[d].ksteps + target - 1) / target;
