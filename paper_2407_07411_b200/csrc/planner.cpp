@@ -299,27 +299,41 @@ int build_schedule(const hpsi_sectors_t* s, const hpsi_terms_t* t, uint32_t flag
   }
 
   // ---- step 4c: P2 units.  K-space of destination d = all segs of all groups with dst == d, in seg order.
-  struct DstInfo { int g0 = 0, g1 = 0; int64_t ksteps = 0; int64_t nseg = 0; };
+  // Cost model (used to cut K into chunks and to order the units): a staged K-tile costs the CTA its DMMAs, but never
+  // less than STAGE_FLOOR DMMA-equivalents - the barrier round trip and the tile load of a stage take ~500 clk even
+  // when a tiny segment (K <= 4 ... 8) or a tiny tile leaves almost nothing to multiply.  Without the floor, units made
+  // of thousands of tiny segments ran 20x longer than planned (stress config: SMs active 85 % of the P2 launch).
+  constexpr int64_t STAGE_FLOOR = 48;
+  auto seg_cost = [&](const Group& g, int64_t tile_frags) {      // one segment on a tile of tile_frags fragments
+    const int64_t full = g.N1 / KT, rem = g.N1 % KT;
+    int64_t c = full * std::max<int64_t>(4 * tile_frags, STAGE_FLOOR);
+    if (rem) c += std::max<int64_t>(((rem + 3) / 4) * tile_frags, STAGE_FLOOR);
+    return c;
+  };
+  struct DstInfo { int g0 = 0, g1 = 0; int64_t cost = 0; int64_t nseg = 0; int maxf = 0; std::vector<Tile1D> rt, ct; };
   std::vector<DstInfo> dsts(nB);
+  int64_t total_p2_cost = 0;
   {
     size_t gi = 0;
     for (int d = 0; d < nB; ++d) {
-      dsts[d].g0 = (int)gi;
+      DstInfo& di = dsts[d];
+      di.rt = split_rows(sc->blocks[d].rows);
+      di.ct = split_cols(sc->blocks[d].cols);
+      for (auto& r : di.rt) for (auto& c : di.ct) di.maxf = std::max(di.maxf, frags(r.len) * frags(c.len));
+      di.g0 = (int)gi;
       while (gi < sc->groups.size() && sc->groups[gi].dst == d) {
-        dsts[d].ksteps += (int64_t)sc->groups[gi].tcount * ((sc->groups[gi].N1 + 3) / 4);
-        dsts[d].nseg += sc->groups[gi].tcount;
+        di.cost += (int64_t)sc->groups[gi].tcount * seg_cost(sc->groups[gi], di.maxf);   // heaviest tile of the block
+        di.nseg += sc->groups[gi].tcount;
         ++gi;
       }
-      dsts[d].g1 = (int)gi;
+      di.g1 = (int)gi;
+      total_p2_cost += di.cost * (int64_t)(di.rt.size() * di.ct.size());
     }
   }
-  int64_t total_p2_dmma = 0;
-  for (int d = 0; d < nB; ++d)
-    total_p2_dmma += (int64_t)frags(sc->blocks[d].rows) * frags(sc->blocks[d].cols) * dsts[d].ksteps;
   const int waves = getenv("HPSI_P2_WAVES") ? std::max(1, atoi(getenv("HPSI_P2_WAVES"))) : 32;   // tuning experiments
   const int64_t slots = (int64_t)std::max(n_sm, 1) * 4 * waves;  // 4 resident CTAs per SM, ~32 waves (small units keep the tail of the launch short)
   const int64_t min_target = getenv("HPSI_P2_MIN") ? std::max(1, atoi(getenv("HPSI_P2_MIN"))) : 1536;   // DMMA per unit at least (~10 us of a CTA)
-  const int64_t target = std::max<int64_t>(min_target, total_p2_dmma / slots);
+  const int64_t target = std::max<int64_t>(min_target, total_p2_cost / slots);
 
   sc->runs.clear(); sc->p2.clear();
   std::vector<int> unit_bundle;            // (block, split) bundle of each unit
@@ -331,32 +345,31 @@ int build_schedule(const hpsi_sectors_t* s, const hpsi_terms_t* t, uint32_t flag
     D.part_off = ws;
     D.nsplit = 0;
     if (dsts[d].nseg == 0) continue;
-    auto rt = split_rows(D.rows);
-    auto ct = split_cols(D.cols);
-    int maxf = 0;
-    for (auto& r : rt) for (auto& c : ct) maxf = std::max(maxf, frags(r.len) * frags(c.len));
-    int64_t nsplit = (maxf * dsts[d].ksteps + target - 1) / target;
+    const auto& rt = dsts[d].rt;
+    const auto& ct = dsts[d].ct;
+    const int maxf = dsts[d].maxf;
+    int64_t nsplit = (dsts[d].cost + target - 1) / target;
     nsplit = std::max<int64_t>(1, std::min<int64_t>(nsplit, dsts[d].nseg));
-    // cut the seg sequence at cumulative k-step boundaries
+    // cut the seg sequence at cumulative cost boundaries
     std::vector<std::pair<int, int>> split_runs;   // run index range per split
     int64_t cum = 0;
     int gi = dsts[d].g0;
     int ti = 0;                                    // position inside group gi
     int realised = 0;
     for (int64_t sp = 0; sp < nsplit; ++sp) {
-      const int64_t want = dsts[d].ksteps * (sp + 1) / nsplit;
+      const int64_t want = dsts[d].cost * (sp + 1) / nsplit;
       int run0 = (int)sc->runs.size();
       int64_t chunk_ksteps = 0;
       while (gi < dsts[d].g1 && (cum < want || sp == nsplit - 1)) {
         const Group& g = sc->groups[gi];
-        const int64_t per = (g.N1 + 3) / 4;
+        const int64_t per = seg_cost(g, maxf);
         int take;
         if (sp == nsplit - 1) take = g.tcount - ti;
         else take = (int)std::min<int64_t>(g.tcount - ti, std::max<int64_t>(1, (want - cum + per - 1) / per));
         if (take > 0) {
           sc->runs.push_back({g.seg0 + ti, g.seg0 + ti + take, g.N1, g.ldw, g.order, g.rows, g.seg0, g.ws_map, g.ws_off});
           cum += per * take;
-          chunk_ksteps += per * take;
+          chunk_ksteps += (int64_t)((g.N1 + 3) / 4) * take;
           ti += take;
         }
         if (ti >= g.tcount) { ++gi; ti = 0; }
@@ -373,13 +386,20 @@ int build_schedule(const hpsi_sectors_t* s, const hpsi_terms_t* t, uint32_t flag
           u.grid = best_grid(frags(r.len), frags(c.len));
           u.out_off = ws + (int64_t)realised * D.rows * D.ldo + (int64_t)r.start * D.ldo + c.start;
           sc->p2.push_back(u);
-          int64_t cost = (int64_t)frags(r.len) * frags(c.len) * chunk_ksteps;
+          const int64_t dmma = (int64_t)frags(r.len) * frags(c.len) * chunk_ksteps;
+          int64_t cost = 0;                         // this tile's cost over the chunk's runs, stage floor included
+          for (int ri = run0; ri < run1; ++ri) {
+            const Run& rr = sc->runs[ri];
+            Group gg{};
+            gg.N1 = rr.K;
+            cost += (int64_t)(rr.seg_end - rr.seg_begin) * seg_cost(gg, (int64_t)frags(r.len) * frags(c.len));
+          }
           int heavy = 0;
           best_grid(frags(r.len), frags(c.len), &heavy);
           sc->critical_flops += (int64_t)NCONS_WARPS * heavy * chunk_ksteps * 512;
           unit_bundle.push_back((int)bundle_cost.size());
           bundle_max = std::max(bundle_max, cost);
-          issued_p2 += cost * 512;
+          issued_p2 += dmma * 512;
         }
       bundle_cost.push_back(bundle_max);
       ++realised;
