@@ -263,7 +263,12 @@ int build_schedule(const hpsi_sectors_t* s, const hpsi_terms_t* t, uint32_t flag
   sc->issued_flops_p1 = 0;
   sc->critical_flops = 0;
   {
-    const int P1_STAGES_PER_UNIT = getenv("HPSI_P1_STAGES") ? std::max(1, atoi(getenv("HPSI_P1_STAGES"))) : 96;   // tuning experiments
+    // ~96 K-tiles per unit, fewer when the whole launch would otherwise be only a few waves of CTAs (small problems)
+    int64_t total_stages = 0;
+    for (const Group& g : sc->groups)
+      total_stages += (int64_t)split_rows(g.rows).size() * split_cols(g.N1).size() * g.tcount * ((g.K1 + KT - 1) / KT);
+    const int auto_stages = (int)std::max<int64_t>(12, std::min<int64_t>(96, total_stages / ((int64_t)std::max(n_sm, 1) * 3 * 8)));
+    const int P1_STAGES_PER_UNIT = getenv("HPSI_P1_STAGES") ? std::max(1, atoi(getenv("HPSI_P1_STAGES"))) : auto_stages;   // env: tuning experiments
     struct GOrder { int64_t cost; int gi; };
     std::vector<GOrder> gorder;
     std::vector<int> g_nt(sc->groups.size());
