@@ -133,6 +133,14 @@ typedef struct {
 int hpsi_davidson(hpsi_plan_t* plan, double* psi_inout_dev, double* eig_host,
                   const hpsi_davidson_params_t* params, hpsi_davidson_info_t* info, void* cuda_stream);
 
+/* The other eigensolver PAPER.md:62 names ("the Lanczos or Davidson method"): explicitly restarted Lanczos with full
+ * re-orthogonalisation, lowest eigenpair.  Same arguments as hpsi_davidson (params->precondition is ignored, m_max =
+ * Krylov vectors kept before a restart from the Ritz vector).  The loop stops on the Lanczos residual estimate
+ * beta_j |y_j| <= tol; info->residual is the true ||H x - theta x|| computed with one extra mat-vec, and
+ * info->converged says whether it is <= 10 tol.  Synchronises the stream. */
+int hpsi_lanczos(hpsi_plan_t* plan, double* psi_inout_dev, double* eig_host,
+                 const hpsi_davidson_params_t* params, hpsi_davidson_info_t* info, void* cuda_stream);
+
 /* hpsi_query items.  `out` is HOST; `bytes` must be >= the item's size (else EINVAL). */
 enum {
   HPSI_Q_PSI_LENGTH = 0,     /* int64: doubles in psi / out                                                  */

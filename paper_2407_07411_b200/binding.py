@@ -78,6 +78,7 @@ def lib() -> ctypes.CDLL:
         L.hpsi_diagonal.argtypes = [vp, vp, vp]
         L.hpsi_davidson.argtypes = [vp, vp, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(hpsi_davidson_params_t),
                                     ctypes.POINTER(hpsi_davidson_info_t), vp]
+        L.hpsi_lanczos.argtypes = L.hpsi_davidson.argtypes
         L.hpsi_query.argtypes = [vp, ctypes.c_int, vp, ctypes.c_size_t]
         L.hpsi_destroy.argtypes = [vp]
         L.hpsi_destroy.restype = None
@@ -85,7 +86,7 @@ def lib() -> ctypes.CDLL:
         L.hpsi_bench_fp64_pipe.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.POINTER(ctypes.c_double),
                                            ctypes.POINTER(ctypes.c_double)]
         L.hpsi_debug_interpret.argtypes = [vp, vp, vp, vp, vp]
-        for name in ("hpsi_plan", "hpsi_bind", "hpsi_set_task_coefficients", "hpsi_apply", "hpsi_apply_host", "hpsi_apply_profiled", "hpsi_diagonal", "hpsi_davidson",
+        for name in ("hpsi_plan", "hpsi_bind", "hpsi_set_task_coefficients", "hpsi_apply", "hpsi_apply_host", "hpsi_apply_profiled", "hpsi_diagonal", "hpsi_davidson", "hpsi_lanczos",
                      "hpsi_query", "hpsi_bench_fp64_pipe", "hpsi_debug_interpret"):
             getattr(L, name).restype = ctypes.c_int
         del i32, i64
@@ -193,6 +194,16 @@ def hpsi_davidson(plan: Plan, psi_inout, tol: float = 1e-8, max_iter: int = 200,
     eig = ctypes.c_double()
     _check(lib().hpsi_davidson(plan.handle, _ptr(psi_inout), ctypes.byref(eig), ctypes.byref(prm),
                                ctypes.byref(info), _stream(stream)))
+    return eig.value, {"n_matvec": info.n_matvec, "converged": bool(info.converged), "residual": info.residual}
+
+
+def hpsi_lanczos(plan: Plan, psi_inout, tol: float = 1e-8, max_iter: int = 200, m_max: int = 16, stream=None):
+    """Restarted Lanczos; returns (theta, info dict); psi_inout (torch CUDA tensor) is overwritten with the Ritz vector."""
+    prm = hpsi_davidson_params_t(tol, max_iter, m_max, 0)
+    info = hpsi_davidson_info_t()
+    eig = ctypes.c_double()
+    _check(lib().hpsi_lanczos(plan.handle, _ptr(psi_inout), ctypes.byref(eig), ctypes.byref(prm),
+                              ctypes.byref(info), _stream(stream)))
     return eig.value, {"n_matvec": info.n_matvec, "converged": bool(info.converged), "residual": info.residual}
 
 

@@ -228,3 +228,118 @@ extern "C" int hpsi_davidson(hpsi_plan_t* p, double* psi, double* eig_host, cons
   if (info) { info->n_matvec = nmv; info->converged = converged; info->residual = rn; }
   return HPSI_OK;
 }
+
+// ------------------------------------------------------------------------------------------------ Lanczos
+// hpsi_lanczos: explicitly restarted Lanczos with full (CGS2) re-orthogonalisation, lowest eigenpair, single root -
+// the other solver PAPER.md:62 names ("the Lanczos or Davidson method").  Same device buffers and kernels as
+// hpsi_davidson; per iteration the host reads back theta, the last Ritz coefficient and |w|^2 to steer the loop
+// (residual estimate beta_j |y_j|); the true residual |H x - theta x| is computed once at the end.
+namespace {
+
+// x = sum_i y_i V_i
+__global__ void combine_kernel(const double* __restrict__ V, int64_t n, int j, const double* __restrict__ y, double* x) {
+  for (int64_t e = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; e < n; e += (int64_t)gridDim.x * blockDim.x) {
+    double s = 0.0;
+    for (int i = 0; i < j; ++i) s += y[i] * V[i * n + e];
+    x[e] = s;
+  }
+}
+// T[j][j] = alpha_j, T[j][j+1] = T[j+1][j] = beta_j = sqrt(|w|^2)   (T stored with leading dimension MMAX)
+__global__ void lanczos_set_kernel(double* T, int j, const double* alpha, const double* beta2) {
+  T[j * MMAX + j] = *alpha;
+  if (j + 1 < MMAX) { const double b = sqrt(*beta2); T[j * MMAX + j + 1] = b; T[(j + 1) * MMAX + j] = b; }
+}
+
+}  // namespace
+
+extern "C" int hpsi_lanczos(hpsi_plan_t* p, double* psi, double* eig_host, const hpsi_davidson_params_t* params,
+                            hpsi_davidson_info_t* info, void* cuda_stream) {
+  using namespace hpsi;
+  if (!p || !psi || !eig_host) { set_error("null argument"); return HPSI_EINVAL; }
+  if (p->host_only) { set_error("host-only plan: hpsi_lanczos needs a CUDA device (no CPU fallback)"); return HPSI_ESTATE; }
+  if (!p->bound) { set_error("operator arenas not bound (hpsi_bind)"); return HPSI_ESTATE; }
+  hpsi_davidson_params_t prm = {1e-8, 200, 16, 0};
+  if (params) prm = *params;
+  if (prm.m_max < 2 || prm.m_max > MMAX || prm.max_iter < 1 || !(prm.tol >= 0.0)) { set_error("bad Lanczos parameters"); return HPSI_EINVAL; }
+  const int64_t n = p->sc.psi_len;
+  if (n == 0) { set_error("empty target sector"); return HPSI_EINVAL; }
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+
+  // buffers: V[m][n] x w | T[MMAX*MMAX] y[MMAX] c[MMAX] c2[MMAX] theta nrm[7] partial[MMAX*NB]
+  const size_t small = MMAX * MMAX + 3 * MMAX + 8 + MMAX * NB;
+  const size_t need = (size_t)(prm.m_max + 2) * n + small;
+  if (p->dav_doubles < need) {
+    cudaFree(p->d_dav);
+    p->d_dav = nullptr;
+    p->dav_doubles = 0;
+    if (cudaMalloc(&p->d_dav, need * sizeof(double)) != cudaSuccess) {
+      cudaGetLastError();
+      set_error("device allocation for the Lanczos basis failed");
+      return HPSI_ENOMEM;
+    }
+    p->dav_doubles = need;
+  }
+  if (!p->h_dav) HPSI_CUDA(cudaMallocHost(&p->h_dav, 8 * sizeof(double)));
+  double* V = p->d_dav;
+  double* x = V + (size_t)prm.m_max * n;
+  double* w = x + n;
+  double* T = w + n;
+  double *y = T + MMAX * MMAX, *c = y + MMAX, *c2 = c + MMAX, *theta = c2 + MMAX, *nrm = theta + 1, *partial = nrm + 7;
+  HPSI_CUDA(cudaMemsetAsync(T, 0, small * sizeof(double), st));
+  const int eg = (int)std::min<int64_t>((n + 255) / 256, 2048);
+  auto dots = [&](const double* X, int nvec, const double* yv, double* out) {
+    dot_partial_kernel<<<dim3(NB, nvec), 256, 0, st>>>(X, n, yv, n, partial);
+    dot_final_kernel<<<1, MMAX, 0, st>>>(partial, nvec, out, 1, nullptr, 0);
+  };
+  int rc;
+  dots(psi, 1, psi, nrm);
+  scale_kernel<<<eg, 256, 0, st>>>(V, psi, nullptr, nullptr, nrm, n);
+  int j = 0, nmv = 0, converged = 0;
+  double th = 0.0;
+  double* host = p->h_dav;
+  for (;;) {
+    if ((rc = hpsi_apply(p, V + (size_t)j * n, w, cuda_stream)) != HPSI_OK) return rc;
+    ++nmv;
+    dots(V, j + 1, w, c);                                            // c[j] = alpha_j
+    project_kernel<<<eg, 256, 0, st>>>(w, V, n, j + 1, c);           // three-term recurrence + re-orthogonalisation
+    dots(V, j + 1, w, c2);
+    project_kernel<<<eg, 256, 0, st>>>(w, V, n, j + 1, c2);          // second Gram-Schmidt pass
+    dots(w, 1, w, nrm + 3);                                          // beta_j^2
+    lanczos_set_kernel<<<1, 1, 0, st>>>(T, j, c + j, nrm + 3);
+    small_eig_kernel<<<1, 32, 0, st>>>(T, j + 1, theta, y);
+    HPSI_CUDA(cudaMemcpyAsync(host, theta, sizeof(double), cudaMemcpyDeviceToHost, st));
+    HPSI_CUDA(cudaMemcpyAsync(host + 1, y + j, sizeof(double), cudaMemcpyDeviceToHost, st));
+    HPSI_CUDA(cudaMemcpyAsync(host + 2, nrm + 3, sizeof(double), cudaMemcpyDeviceToHost, st));
+    HPSI_CUDA(cudaStreamSynchronize(st));
+    th = host[0];
+    const double beta = std::sqrt(host[2]);
+    const double est = beta * std::fabs(host[1]);
+    const bool done = est <= prm.tol || !(beta >= 1e-14) || nmv >= prm.max_iter;
+    if (done || j + 1 >= prm.m_max) {
+      combine_kernel<<<eg, 256, 0, st>>>(V, n, j + 1, y, x);         // Ritz vector
+      dots(x, 1, x, nrm + 2);
+      if (done) break;
+      scale_kernel<<<eg, 256, 0, st>>>(V, x, nullptr, nullptr, nrm + 2, n);   // restart from the Ritz vector
+      HPSI_CUDA(cudaMemsetAsync(T, 0, MMAX * MMAX * sizeof(double), st));
+      j = 0;
+      continue;
+    }
+    scale_kernel<<<eg, 256, 0, st>>>(V + (size_t)(j + 1) * n, w, nullptr, nullptr, nrm + 3, n);
+    ++j;
+  }
+  // psi = x/|x| ; true residual |H psi - theta psi|
+  scale_kernel<<<eg, 256, 0, st>>>(psi, x, nullptr, nullptr, nrm + 2, n);
+  if ((rc = hpsi_apply(p, psi, w, cuda_stream)) != HPSI_OK) return rc;
+  ++nmv;
+  set_scalar_kernel<<<1, 1, 0, st>>>(c, theta);
+  project_kernel<<<eg, 256, 0, st>>>(w, psi, n, 1, c);
+  dots(w, 1, w, nrm + 1);
+  HPSI_CUDA(cudaMemcpyAsync(host, nrm + 1, sizeof(double), cudaMemcpyDeviceToHost, st));
+  HPSI_CUDA(cudaGetLastError());
+  HPSI_CUDA(cudaStreamSynchronize(st));
+  const double rn = std::sqrt(host[0]);
+  converged = rn <= prm.tol * 10.0 || rn <= prm.tol;      // the estimate steered the loop; the true residual is reported
+  *eig_host = th;
+  if (info) { info->n_matvec = nmv; info->converged = converged; info->residual = rn; }
+  return HPSI_OK;
+}

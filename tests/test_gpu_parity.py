@@ -291,3 +291,39 @@ def test_task_coefficients(H, toy):
         torch.cuda.synchronize()
         ref = oracle.diagonal(ex)
         assert np.linalg.norm(d.cpu().numpy() - ref) <= 1e-12 * max(np.linalg.norm(ref), 1.0)
+
+
+def _lanczos(H, g, v0, **kw):
+    import torch
+    x = torch.from_numpy(np.ascontiguousarray(v0)).cuda()
+    theta, info = H.hpsi_lanczos(g.plan, x, **kw)
+    return theta, x.cpu().numpy(), info
+
+
+def test_lanczos_toy_vs_dense_and_hubbard(H, toy):
+    """hpsi_lanczos ("the Lanczos or Davidson method"): lowest eigenvalue against a dense eigensolver on
+    the toy config, against the textbook Hubbard closed forms, and against hpsi_davidson."""
+    g = GpuProblem(toy)
+    ev = np.linalg.eigvalsh(oracle.dense_hamiltonian(toy))
+    theta, x, info = _lanczos(H, g, workloads.make_psi(toy), tol=1e-9, max_iter=2000, m_max=32)
+    assert info["converged"] and abs(theta - ev[0]) <= 1e-10, (theta, ev[0], info)
+    assert abs(np.linalg.norm(x) - 1.0) <= 1e-12
+    assert np.linalg.norm(oracle.apply(toy, x) - theta * x) <= 1e-7
+    th_d, _, _ = _davidson(H, g, workloads.make_psi(toy), tol=1e-9, max_iter=400)
+    assert abs(theta - th_d) <= 1e-9
+    dimer = hubbard_two_block_problem(1, 1, 1.0, 3.7, 2, 0)
+    theta, _, info = _lanczos(H, GpuProblem(dimer), np.ones(dimer.psi_len), tol=1e-10)
+    assert info["converged"] and abs(theta - (3.7 - np.sqrt(3.7 ** 2 + 16.0)) / 2) <= 1e-10
+    chain = hubbard_two_block_problem(2, 2, 1.0, 0.0, 4, 0)
+    v0 = np.random.default_rng(0).standard_normal(chain.psi_len)
+    theta, _, info = _lanczos(H, GpuProblem(chain), v0, tol=1e-10, max_iter=500, m_max=24)
+    assert info["converged"] and abs(theta + 2 * np.sqrt(5.0)) <= 1e-9
+
+
+def test_lanczos_small(H, small):
+    g = GpuProblem(small)
+    theta, x, info = _lanczos(H, g, workloads.make_psi(small), tol=1e-6, max_iter=600, m_max=32)
+    assert info["residual"] <= 1e-4
+    assert np.linalg.norm(oracle.apply(small, x) - theta * x) <= 2e-4
+    th_d, _, info_d = _davidson(H, g, workloads.make_psi(small), tol=1e-7, max_iter=300)
+    assert info_d["converged"] and abs(theta - th_d) <= 1e-6 * max(1.0, abs(th_d))
