@@ -76,6 +76,13 @@ typedef struct {
   const double* a_data;            /* DEVICE (or NULL)                                           */
   const double* b_data;            /* DEVICE (or NULL)                                           */
   int64_t a_len, b_len;
+  /* Adjoint-pair storage sharing: HOST, [n_a] / [n_b], may be NULL (= all zero).  A non-zero entry
+   * says the arena holds the TRANSPOSE of that block: element (x, x') of the block is arena[offset + x' * ld + x] with
+   * ld >= d[row].  A Hermitian H pairs every term with its adjoint (same c, A^T, B^T): the adjoint term's descriptors
+   * can then point at the base term's storage and the operator arenas halve (80 -> 40 GB at D=8192).  Such blocks are
+   * staged K-major (16 x 16 TMA boxes) and their tiles are padded to 16 instead of 8 rows. */
+  const uint8_t* a_transposed;
+  const uint8_t* b_transposed;
 } hpsi_terms_t;
 
 /* Steps 1-4 of SURVEY.md 8(a): psi block table, task enumeration, per-task order choice

@@ -40,7 +40,8 @@ class hpsi_terms_t(ctypes.Structure):
                 ("n_a", ctypes.c_int64), ("a_blocks", ctypes.c_void_p),
                 ("n_b", ctypes.c_int64), ("b_blocks", ctypes.c_void_p),
                 ("a_data", ctypes.c_void_p), ("b_data", ctypes.c_void_p),
-                ("a_len", ctypes.c_int64), ("b_len", ctypes.c_int64)]
+                ("a_len", ctypes.c_int64), ("b_len", ctypes.c_int64),
+                ("a_transposed", ctypes.c_void_p), ("b_transposed", ctypes.c_void_p)]
 
 
 class hpsi_davidson_params_t(ctypes.Structure):
@@ -134,7 +135,7 @@ class Plan:
 
 
 def hpsi_plan(q_left, q_right, d_left, d_right, target, coef, a_blocks, b_blocks, a_data=None, b_data=None,
-              a_len: int = 0, b_len: int = 0, flags: int = 0) -> Plan:
+              a_len: int = 0, b_len: int = 0, flags: int = 0, a_transposed=None, b_transposed=None) -> Plan:
     """hpsi_plan(sector table, term list).  Host arrays: numpy; a_blocks/b_blocks: numpy arrays with the 24-byte
     hpsi_opblock_t layout; a_data/b_data: torch CUDA float64 tensors (or None, to hpsi_bind later)."""
     q_left = np.ascontiguousarray(q_left, np.int32).reshape(-1, 2)
@@ -147,8 +148,15 @@ def hpsi_plan(q_left, q_right, d_left, d_right, target, coef, a_blocks, b_blocks
     assert a_blocks.dtype.itemsize == 24 and b_blocks.dtype.itemsize == 24
     sec = hpsi_sectors_t(q_left.shape[0], q_right.shape[0], q_left.ctypes.data, q_right.ctypes.data,
                          d_left.ctypes.data, d_right.ctypes.data, (ctypes.c_int32 * 2)(int(target[0]), int(target[1])))
+    if a_transposed is not None:
+        a_transposed = np.ascontiguousarray(a_transposed, np.uint8)
+        assert a_transposed.shape[0] == a_blocks.shape[0]
+    if b_transposed is not None:
+        b_transposed = np.ascontiguousarray(b_transposed, np.uint8)
+        assert b_transposed.shape[0] == b_blocks.shape[0]
     trm = hpsi_terms_t(coef.shape[0], coef.ctypes.data, a_blocks.shape[0], a_blocks.ctypes.data,
-                       b_blocks.shape[0], b_blocks.ctypes.data, _ptr(a_data), _ptr(b_data), int(a_len), int(b_len))
+                       b_blocks.shape[0], b_blocks.ctypes.data, _ptr(a_data), _ptr(b_data), int(a_len), int(b_len),
+                       _ptr(a_transposed), _ptr(b_transposed))
     out = ctypes.c_void_p()
     _check(lib().hpsi_plan(ctypes.byref(sec), ctypes.byref(trm), flags, ctypes.byref(out)))
     return Plan(out.value, (a_data, b_data))
@@ -238,4 +246,4 @@ def hpsi_debug_interpret(plan: Plan, a_host: np.ndarray, b_host: np.ndarray, psi
 def plan_problem(p, a_data=None, b_data=None, flags: int = 0) -> Plan:
     """Marshal a ``workloads.Problem`` (any object with the boundary's fields) into hpsi_plan."""
     return hpsi_plan(p.q_left, p.q_right, p.d_left, p.d_right, p.target, p.coef, p.a_desc, p.b_desc,
-                     a_data, b_data, p.a_len, p.b_len, flags)
+                     a_data, b_data, p.a_len, p.b_len, flags, getattr(p, "a_trans", None), getattr(p, "b_trans", None))

@@ -10,8 +10,8 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libhpsi.so")
-SOURCES = ["planner.cpp", "interp.cpp", "kernels.cu", "api.cu", "davidson.cu", "microbench.cu"]
-HEADERS = ["plan.h", "plan_dev.h", "kernels.cuh", os.path.join("..", "..", "include", "hpsi.h")]
+SOURCES = ["planner.cpp", "interp.cpp", "kernels.cu", "kernels_paired.cu", "api.cu", "davidson.cu", "microbench.cu"]
+HEADERS = ["plan.h", "plan_dev.h", "kernels.cuh", "kernels_common.cuh", os.path.join("..", "..", "include", "hpsi.h")]
 
 
 def _nvcc() -> str:

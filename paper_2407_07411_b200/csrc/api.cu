@@ -67,6 +67,7 @@ int upload_schedule(hpsi_plan_t* p) {
   p->dev.n_p1 = (int)sc.p1.size();
   p->dev.n_p2 = (int)sc.p2.size();
   p->dev.max_block_elems = sc.max_block_elems;
+  p->dev.paired = sc.paired ? 1 : 0;
   p->dev.debug = getenv("HPSI_DEBUG") ? atoi(getenv("HPSI_DEBUG")) : 0;
   if (sc.psi_len > 0) {
     HPSI_CUDA(cudaMalloc(&p->d_psi_stage, (size_t)sc.psi_len * sizeof(double)));
@@ -111,7 +112,7 @@ int encode_maps(hpsi_plan_t* p) {
     const double* base = m.base == BASE_A ? p->dev.a : (m.base == BASE_B ? p->dev.b : p->d_ws);
     const cuuint64_t dims[2] = {(cuuint64_t)m.cols, (cuuint64_t)m.rows};
     const cuuint64_t strides[1] = {(cuuint64_t)m.ld * 8};
-    const cuuint32_t box[2] = {(cuuint32_t)KT, (cuuint32_t)m.box_rows};
+    const cuuint32_t box[2] = {(cuuint32_t)m.box_cols, (cuuint32_t)m.box_rows};
     const cuuint32_t estr[2] = {1, 1};
     CUresult r = enc(&host[i], CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, const_cast<double*>(base + m.off), dims, strides, box, estr,
                      CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,

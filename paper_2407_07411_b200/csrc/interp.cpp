@@ -26,13 +26,15 @@ void interpret_schedule(const Schedule& sc, const double* a, const double* b, co
     const double* y = ws + g.y1_off;
     for (int t = u.t0; t < u.t1; ++t) {
       const Seg& sg = sc.segs[g.seg0 + t];
+      // element (i, k) of the operator block: plain storage [i][k], transposed storage [k][i]
+      const int64_t xsi = sg.p1_trans ? 1 : sg.p1_ld, xsk = sg.p1_trans ? sg.p1_ld : 1;
       for (int r = 0; r < u.rows_valid; ++r) {
-        const double* xr = xbase + sg.p1_off + (int64_t)(u.i0 + r) * sg.p1_ld;
+        const double* xr = xbase + sg.p1_off + (int64_t)(u.i0 + r) * xsi;
         for (int c = 0; c < u.cols_valid; ++c) {
           const int j = u.j0 + c;
           const double* yr = y + (int64_t)j * g.ldy1;
           double s = 0.0;
-          for (int k = 0; k < g.K1; ++k) s += xr[k] * yr[k];
+          for (int k = 0; k < g.K1; ++k) s += xr[k * xsk] * yr[k];
           ws[g.ws_off + ((int64_t)t * g.rows + u.i0 + r) * g.ldw + j] = sg.coef * s;
         }
       }
@@ -48,15 +50,19 @@ void interpret_schedule(const Schedule& sc, const double* a, const double* b, co
           for (int si = run.seg_begin; si < run.seg_end; ++si) {
             const Seg& sg = sc.segs[si];
             const int64_t t_off = run.ws_off + (int64_t)(si - run.seg0) * run.rows * run.ldw;
+            const int64_t osi = sg.p2_trans ? 1 : sg.p2_ld, osk = sg.p2_trans ? sg.p2_ld : 1;   // operator block strides
             const double *xr, *yr;
+            int64_t xsk = 1, ysk = 1;
             if (run.order == 1) {
               xr = ws + t_off + (int64_t)(u.i0 + r) * run.ldw;
-              yr = b + sg.p2_off + (int64_t)(u.j0 + c) * sg.p2_ld;
+              yr = b + sg.p2_off + (int64_t)(u.j0 + c) * osi;
+              ysk = osk;
             } else {
-              xr = a + sg.p2_off + (int64_t)(u.i0 + r) * sg.p2_ld;
+              xr = a + sg.p2_off + (int64_t)(u.i0 + r) * osi;
+              xsk = osk;
               yr = ws + t_off + (int64_t)(u.j0 + c) * run.ldw;
             }
-            for (int k = 0; k < run.K; ++k) s += xr[k] * yr[k];
+            for (int k = 0; k < run.K; ++k) s += xr[k * xsk] * yr[k * ysk];
           }
         }
         ws[u.out_off + (int64_t)r * u.ldo + c] = s;

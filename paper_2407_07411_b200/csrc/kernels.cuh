@@ -35,6 +35,7 @@ struct DevSchedule {           // device pointers to the uploaded tables
   const double* b;
   int n_blocks, n_p1, n_p2;
   int max_block_elems;
+  int paired;                  // the plan has blocks stored transposed: kernels_paired.cu runs the GEMMs
   int debug;                   // HPSI_DEBUG env (timing experiments only): 1 = producer skips loads, 2 = consumers skip MMAs
 };
 
@@ -43,6 +44,9 @@ void launch_p1(const DevSchedule& d, bool tma, cudaStream_t st);
 void launch_p2(const DevSchedule& d, bool tma, cudaStream_t st);
 void launch_reduce(const DevSchedule& d, double* out, cudaStream_t st);
 void launch_diag(const DevSchedule& d, double* diag, cudaStream_t st);
+void launch_p1_paired(const DevSchedule& d, bool tma, cudaStream_t st);   // kernels_paired.cu
+void launch_p2_paired(const DevSchedule& d, bool tma, cudaStream_t st);
+cudaError_t kernels_paired_init();
 cudaError_t kernels_init();    // opt-in to >48 KB dynamic shared memory
 
 }  // namespace hpsi

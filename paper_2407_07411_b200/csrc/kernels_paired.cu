@@ -1,0 +1,338 @@
+// GEMM kernels for plans in which some operator block is stored transposed (hpsi_terms_t a_transposed / b_transposed:
+// adjoint-pair storage sharing).  Same CTA design as kernels.cu (1 TMA producer warp + 4 DMMA consumer
+// warps, mbarrier ring); what differs is how fragments map to tile rows.
+//
+// A block stored transposed is an M-contiguous ("T") operand: the TMA unit stages a 64-row x 16-k piece of it as four
+// 16(k) x 16(rows) boxes (128 bytes per k, 128-byte swizzle), i.e. sub-tile b = rows 16b..16b+15 holds element
+// (k, ii) at  k*128 + (((ii >> 1) ^ (k & 7)) << 4) + (ii & 1)*8  bytes.  A DMMA fragment (8 rows x 4 k, lane (g, q) ->
+// row g, k = 4 ks + q) reads such a tile without bank conflicts iff the 4 rows of each half-warp differ in
+// (bit 3, bit 0) of ii; a K-contiguous ("N") tile (kernels.cu) needs them to differ in bits (2, 1).  Both hold for
+//     fragment sibling 0: rows {0,3,12,15 | 1,2,13,14} of a 16-row group,   sibling 1: the same ^ 4,
+// so in these kernels fragments come in pairs that interleave 16 rows, whatever the layout of the operand: one
+// accumulator <-> tile-element mapping serves a unit whose K range mixes plainly stored and transposed blocks.
+// Tiles are therefore padded to 16 rows / columns (plan.h tile_frags(.., paired = true)), and a warp owns whole pairs.
+#include "kernels_common.cuh"
+
+namespace hpsi {
+
+// row (0..15) of its 16-row group that sibling s of a fragment pair gives to lane group / accumulator index x (0..7)
+__device__ __forceinline__ int row16(int s, int x) { return (int)((0xED21FC30u >> (4 * x)) & 15u) ^ (s << 2); }
+
+// Per-lane element offsets (doubles, relative to the warp's first pair of the operand tile) of k-steps 0..3 for the two
+// siblings; pair p of the warp adds 256 p.  `t` = the operand is an M-contiguous ("T") tile.
+struct PairOffsets {
+  int x[2][4], y[2][4];
+  __device__ __forceinline__ static int off(int r, int q, int ks, bool t) {
+    if (t) { const int k = 4 * ks + q; return k * 16 + ((((r >> 1) ^ (k & 7))) << 1) + (r & 1); }
+    return r * 16 + (((2 * ks + (q >> 1)) ^ (r & 7)) << 1) + (q & 1);
+  }
+  __device__ __forceinline__ void set(int lane, bool xt, bool yt) {
+    const int g = lane >> 2, q = lane & 3;
+#pragma unroll
+    for (int s = 0; s < 2; ++s)
+#pragma unroll
+      for (int ks = 0; ks < 4; ++ks) {
+        x[s][ks] = off(row16(s, g), q, ks, xt);
+        y[s][ks] = off(row16(s, g), q, ks, yt);
+      }
+  }
+};
+
+struct WarpTileP {
+  int wr0, wc0;    // first row / col of the warp inside the CTA tile (multiples of 16)
+  int mi, nj;      // fragments owned (even)
+  __device__ __forceinline__ WarpTileP(int gn, int warp, int rows_valid, int cols_valid) {
+    const int gm = NCONS / gn;
+    int f0, cnt;
+    split_frags((rows_valid + 15) >> 4, gm, warp / gn, f0, cnt);
+    wr0 = f0 * 16; mi = 2 * cnt;
+    split_frags((cols_valid + 15) >> 4, gn, warp % gn, f0, cnt);
+    wc0 = f0 * 16; nj = 2 * cnt;
+  }
+};
+
+template <int MI, int NJ>
+__device__ __forceinline__ void mma_stage_p(const double* px, const double* py, const PairOffsets& po,
+                                            double (&acc)[MI][NJ][2], int nk4) {
+  double a[MI], b[NJ];
+#pragma unroll
+  for (int ks = 0; ks < 4; ++ks) {
+    if (ks < nk4) {
+#pragma unroll
+      for (int i = 0; i < MI; ++i) a[i] = px[po.x[i & 1][ks] + (i >> 1) * 256];
+#pragma unroll
+      for (int j = 0; j < NJ; ++j) b[j] = py[po.y[j & 1][ks] + (j >> 1) * 256];
+      mma_step<MI, NJ>(a, b, acc);
+    }
+  }
+}
+
+// acc[i][j][e] holds tile row wr0 + 16 (i/2) + row16(i&1, g) and tile column wc0 + 16 (j/2) + row16(j&1, 2q + e)
+template <int MI, int NJ>
+__device__ __forceinline__ void store_tile_p(double* dst, int ld, int rows_valid, int cols_valid,
+                                             const double (&acc)[MI][NJ][2], const WarpTileP& w, int lane, double sc) {
+  const int g = lane >> 2, q = lane & 3;
+#pragma unroll
+  for (int i = 0; i < MI; ++i) {
+    const int row = w.wr0 + 16 * (i >> 1) + row16(i & 1, g);
+    if (row >= rows_valid) continue;
+    double* drow = dst + (int64_t)row * ld;
+#pragma unroll
+    for (int j = 0; j < NJ; ++j) {
+#pragma unroll
+      for (int e = 0; e < 2; ++e) {
+        const int col = w.wc0 + 16 * (j >> 1) + row16(j & 1, 2 * q + e);
+        if (col < cols_valid) drow[col] = acc[i][j][e] * sc;
+      }
+    }
+  }
+}
+
+// ---------------------------------------------------------------------------------------------- staging
+// LDGSTS fallback for an M-contiguous operand: rows_valid operand rows starting at `first` (= element (row 0, k 0) of
+// the window), k-major with leading dimension ld.  Lane handles k = lane & 15 of rows (lane >> 4) + 2 p.
+__device__ __forceinline__ void ldgsts_tile_t(uint32_t s_op, const double* first, int64_t ld, int rows_valid, int kappa,
+                                              int K, int lane) {
+  const int k = lane & 15, r0 = lane >> 4;
+  const bool kvalid = kappa + k < K;
+#pragma unroll 8
+  for (int p = 0; p < TILE / 2; ++p) {
+    const int r = r0 + 2 * p, ii = r & 15;
+    const bool ok = kvalid && r < rows_valid;
+    const double* src = ok ? first + (int64_t)(kappa + k) * ld + r : first;
+    const uint32_t dst = s_op + (r >> 4) * 2048 + k * 128 + ((((ii >> 1) ^ (k & 7)) << 4) | ((ii & 1) << 3));
+    cp_async_chunk8(dst, src, ok ? 8 : 0);
+  }
+}
+
+// One operand of a stage.  N: one 64-row x 16-k box (or the 8-byte LDGSTS copy); T: ceil(rows_valid / 16) boxes of
+// 16 k x 16 rows.  `row0` = first operand row of the tile inside the matrix; for LDGSTS `ptr` = element (row0, 0).
+struct OperandSrc {
+  const unsigned char* map;   // TMA
+  const double* ptr;          // LDGSTS
+  int64_t ld;
+  int row0;
+  int trans;
+};
+__device__ __forceinline__ uint32_t operand_bytes(const OperandSrc& o, int rows_valid) {
+  return o.trans ? (uint32_t)((rows_valid + 15) >> 4) * 2048u : (uint32_t)OP_BYTES;
+}
+template <bool TMA>
+__device__ __forceinline__ void stage_operand(const OperandSrc& o, uint32_t s_op, int rows_valid, int kappa, int K,
+                                              uint32_t full, int lane) {
+  if (TMA) {
+    if (lane != 0) return;
+    if (!o.trans) { tma_load_2d(s_op, o.map, kappa, o.row0, full); return; }
+    const int nsub = (rows_valid + 15) >> 4;
+    for (int b = 0; b < nsub; ++b) tma_load_2d(s_op + b * 2048, o.map, o.row0 + 16 * b, kappa, full);
+  } else {
+    if (!o.trans) ldgsts_tile(s_op, o.ptr, o.ld, rows_valid, kappa, K, lane);
+    else ldgsts_tile_t(s_op, o.ptr, o.ld, rows_valid, kappa, K, lane);
+  }
+}
+template <bool TMA>
+__device__ __forceinline__ void stage_both(const OperandSrc& x, const OperandSrc& y, const SmemLayout& sm, const Ring& ring,
+                                           int rows_valid, int cols_valid, int kappa, int K, int lane, int debug) {
+  const uint32_t sx = sm.stage(ring.stage), sy = sx + X_BOXES * OP_BYTES, full = sm.full(ring.stage);
+  if (TMA) {
+    if (lane == 0)
+      mbar_arrive_expect_tx(full, debug == 1 ? 0 : operand_bytes(x, rows_valid) + operand_bytes(y, cols_valid));
+    if (debug != 1) {
+      stage_operand<true>(x, sx, rows_valid, kappa, K, full, lane);
+      stage_operand<true>(y, sy, cols_valid, kappa, K, full, lane);
+    }
+  } else {
+    if (debug != 1) {
+      stage_operand<false>(x, sx, rows_valid, kappa, K, full, lane);
+      stage_operand<false>(y, sy, cols_valid, kappa, K, full, lane);
+    }
+    cp_async_mbar_arrive(full);
+  }
+}
+
+// Dispatch to the instantiation for the warp's (mi, nj) in fragments: whole pairs, at most 16 fragments per warp.
+#define HPSI_DISPATCH_PAIRS(CALL)                                                          \
+  switch (w.mi * 9 + w.nj) {                                                               \
+    CALL(2, 2) CALL(2, 4) CALL(4, 2) CALL(4, 4) CALL(2, 6) CALL(6, 2) CALL(2, 8) CALL(8, 2) \
+    default: __trap();                                                                     \
+  }
+
+__device__ __forceinline__ void idle_consume_p(const SmemLayout& sm, int nstages, int lane) {
+  Ring ring{0, 0};
+  for (int i = 0; i < nstages; ++i) {
+    mbar_wait(sm.full(ring.stage), ring.phase);
+    if (lane == 0) mbar_arrive(sm.empty(ring.stage));
+    ring.advance();
+  }
+}
+
+// ------------------------------------------------------------------------------------------------ P1 kernel
+template <int MI, int NJ>
+__device__ __forceinline__ void p1p_consume(const DevSchedule& d, const P1Unit& u, const Group& g, const SmemLayout& sm,
+                                            const WarpTileP& w, int lane) {
+  double acc[MI][NJ][2];
+  PairOffsets po;
+  po.set(lane, u.xtrans != 0, false);
+  const int ntiles = (g.K1 + KT - 1) / KT;
+  const int last_nk4 = ((g.K1 - (ntiles - 1) * KT) + 3) >> 2;
+  Ring ring{0, 0};
+  for (int t = u.t0; t < u.t1; ++t) {
+    const double coef = d.segs[g.seg0 + t].coef;
+    zero_acc<MI, NJ>(acc);
+    for (int kt = 0; kt < ntiles; ++kt) {
+      mbar_wait(sm.full(ring.stage), ring.phase);
+      if (d.debug != 2) {
+        const double* st = sm.stage_ptr(ring.stage);
+        mma_stage_p<MI, NJ>(st + w.wr0 * 16, st + X_BOXES * OP_BYTES / 8 + w.wc0 * 16, po, acc,
+                            kt == ntiles - 1 ? last_nk4 : 4);
+      }
+      __syncwarp();
+      if (lane == 0) mbar_arrive(sm.empty(ring.stage));
+      ring.advance();
+    }
+    double* dst = d.ws + g.ws_off + ((int64_t)t * g.rows + u.i0) * g.ldw + u.j0;
+    store_tile_p<MI, NJ>(dst, g.ldw, u.rows_valid, u.cols_valid, acc, w, lane, coef);
+  }
+}
+
+template <bool TMA>
+__global__ void __maxnreg__(136) p1p_kernel(DevSchedule d) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  const P1Unit u = d.p1[blockIdx.x];
+  const Group g = d.groups[u.group];
+  const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+  const SmemLayout sm(smem_raw);
+  init_barriers<TMA>(sm, tid);
+  const int ntiles = (g.K1 + KT - 1) / KT;
+
+  if (wid == NCONS) {
+    // ---------------- producer warp
+    Ring ring{0, 1};
+    const OperandSrc y{d.maps + (int64_t)g.y1_map * TMAP_BYTES, d.ws + g.y1_off + (int64_t)u.j0 * g.ldy1, g.ldy1, u.j0, 0};
+    const double* xarena = (g.order == 1) ? d.a : d.b;
+    for (int t = u.t0; t < u.t1; ++t) {
+      const Seg* sg = d.segs + g.seg0 + t;
+      OperandSrc x{d.maps + (int64_t)sg->p1_map * TMAP_BYTES, nullptr, sg->p1_ld, u.i0, u.xtrans};
+      if (!TMA) x.ptr = xarena + sg->p1_off + (u.xtrans ? (int64_t)u.i0 : (int64_t)u.i0 * sg->p1_ld);
+      for (int kt = 0; kt < ntiles; ++kt) {
+        mbar_wait(sm.empty(ring.stage), ring.phase);
+        stage_both<TMA>(x, y, sm, ring, u.rows_valid, u.cols_valid, kt * KT, g.K1, lane, d.debug);
+        ring.advance();
+      }
+    }
+    if (!TMA) cp_async_wait_all();
+    return;
+  }
+
+  // ------------------ consumer warps
+  const int warp = (wid + quadrant_rotation(blockIdx.x)) % NCONS;
+  const WarpTileP w(u.grid, warp, u.rows_valid, u.cols_valid);
+  if (w.mi == 0 || w.nj == 0) { idle_consume_p(sm, ntiles * (u.t1 - u.t0), lane); return; }
+#define HPSI_CASE(MI, NJ) case MI * 9 + NJ: p1p_consume<MI, NJ>(d, u, g, sm, w, lane); break;
+  HPSI_DISPATCH_PAIRS(HPSI_CASE)
+#undef HPSI_CASE
+}
+
+// ------------------------------------------------------------------------------------------------ P2 kernel
+template <int MI, int NJ>
+__device__ __forceinline__ void p2p_consume(const DevSchedule& d, const P2Unit& u, const SmemLayout& sm,
+                                            const WarpTileP& w, int lane) {
+  double acc[MI][NJ][2];
+  zero_acc<MI, NJ>(acc);
+  PairOffsets po;
+  Ring ring{0, 0};
+  for (int r = u.run_begin; r < u.run_end; ++r) {            // same (run, seg, k-tile) order as the producer
+    const Run run = d.runs[r];
+    po.set(lane, run.order == 2 && run.trans, run.order == 1 && run.trans);   // the operator operand may be transposed
+    const int K = run.K, nseg = run.seg_end - run.seg_begin;
+    const int ntiles = (K + KT - 1) / KT, last_nk4 = ((K - (ntiles - 1) * KT) + 3) >> 2;
+    for (int sgi = 0; sgi < nseg; ++sgi)
+      for (int kt = 0; kt < ntiles; ++kt) {
+        mbar_wait(sm.full(ring.stage), ring.phase);
+        if (d.debug != 2) {
+          const double* st = sm.stage_ptr(ring.stage);
+          mma_stage_p<MI, NJ>(st + w.wr0 * 16, st + X_BOXES * OP_BYTES / 8 + w.wc0 * 16, po, acc,
+                              kt == ntiles - 1 ? last_nk4 : 4);
+        }
+        __syncwarp();
+        if (lane == 0) mbar_arrive(sm.empty(ring.stage));
+        ring.advance();
+      }
+  }
+  store_tile_p<MI, NJ>(d.ws + u.out_off, u.ldo, u.rows_valid, u.cols_valid, acc, w, lane, 1.0);
+}
+
+template <bool TMA>
+__global__ void __maxnreg__(136) p2p_kernel(DevSchedule d) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  const P2Unit u = d.p2[blockIdx.x];
+  const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+  const SmemLayout sm(smem_raw);
+  init_barriers<TMA>(sm, tid);
+
+  if (wid == NCONS) {
+    // ---------------- producer warp
+    Ring ring{0, 1};
+    for (int r = u.run_begin; r < u.run_end; ++r) {
+      const Run run = d.runs[r];
+      const unsigned char* wsmap = d.maps + (int64_t)run.ws_map * TMAP_BYTES;
+      const int ntiles = (run.K + KT - 1) / KT;
+      for (int seg = run.seg_begin; seg < run.seg_end; ++seg) {
+        const Seg* sg = d.segs + seg;
+        const int trow = (seg - run.seg0) * run.rows;          // first row of the task inside the stacked intermediate
+        const double* wsrows = d.ws + run.ws_off + (int64_t)trow * run.ldw;
+        OperandSrc x, y;
+        if (run.order == 1) {                                  // X = T_t (workspace), Y = B_t
+          x = OperandSrc{wsmap, wsrows + (int64_t)u.i0 * run.ldw, run.ldw, trow + u.i0, 0};
+          y = OperandSrc{d.maps + (int64_t)sg->p2_map * TMAP_BYTES,
+                         d.b + sg->p2_off + (run.trans ? (int64_t)u.j0 : (int64_t)u.j0 * sg->p2_ld), sg->p2_ld, u.j0, run.trans};
+        } else {                                               // X = A_t, Y = U_t^T (workspace)
+          x = OperandSrc{d.maps + (int64_t)sg->p2_map * TMAP_BYTES,
+                         d.a + sg->p2_off + (run.trans ? (int64_t)u.i0 : (int64_t)u.i0 * sg->p2_ld), sg->p2_ld, u.i0, run.trans};
+          y = OperandSrc{wsmap, wsrows + (int64_t)u.j0 * run.ldw, run.ldw, trow + u.j0, 0};
+        }
+        for (int kt = 0; kt < ntiles; ++kt) {
+          mbar_wait(sm.empty(ring.stage), ring.phase);
+          stage_both<TMA>(x, y, sm, ring, u.rows_valid, u.cols_valid, kt * KT, run.K, lane, d.debug);
+          ring.advance();
+        }
+      }
+    }
+    if (!TMA) cp_async_wait_all();
+    return;
+  }
+
+  // ------------------ consumer warps
+  const int warp = (wid + quadrant_rotation(blockIdx.x)) % NCONS;
+  const WarpTileP w(u.grid, warp, u.rows_valid, u.cols_valid);
+  if (w.mi == 0 || w.nj == 0) {
+    int nstages = 0;
+    for (int r = u.run_begin; r < u.run_end; ++r)
+      nstages += (d.runs[r].seg_end - d.runs[r].seg_begin) * ((d.runs[r].K + KT - 1) / KT);
+    idle_consume_p(sm, nstages, lane);
+    return;
+  }
+#define HPSI_CASE(MI, NJ) case MI * 9 + NJ: p2p_consume<MI, NJ>(d, u, sm, w, lane); break;
+  HPSI_DISPATCH_PAIRS(HPSI_CASE)
+#undef HPSI_CASE
+}
+
+// -------------------------------------------------------------------------------------------------- launchers
+cudaError_t kernels_paired_init() {
+  cudaError_t e;
+  if ((e = cudaFuncSetAttribute(p1p_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES))) return e;
+  if ((e = cudaFuncSetAttribute(p1p_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES))) return e;
+  if ((e = cudaFuncSetAttribute(p2p_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES))) return e;
+  if ((e = cudaFuncSetAttribute(p2p_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES))) return e;
+  return cudaSuccess;
+}
+void launch_p1_paired(const DevSchedule& d, bool tma, cudaStream_t st) {
+  if (tma) p1p_kernel<true><<<d.n_p1, NTHREADS, SMEM_BYTES, st>>>(d);
+  else p1p_kernel<false><<<d.n_p1, NTHREADS, SMEM_BYTES, st>>>(d);
+}
+void launch_p2_paired(const DevSchedule& d, bool tma, cudaStream_t st) {
+  if (tma) p2p_kernel<true><<<d.n_p2, NTHREADS, SMEM_BYTES, st>>>(d);
+  else p2p_kernel<false><<<d.n_p2, NTHREADS, SMEM_BYTES, st>>>(d);
+}
+
+}  // namespace hpsi

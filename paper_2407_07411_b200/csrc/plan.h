@@ -37,6 +37,7 @@ struct Seg {                  // one task, in schedule order (by destination, so
   int32_t p1_ld, p2_ld;       // leading dimensions of those blocks
   int32_t p1_map, p2_map;     // tensor-map ids of those blocks (TMA staging)
   double coef;                // per-task coefficient (initialised to c_t; reading A4)
+  int32_t p1_trans, p2_trans; // 1: that block is stored transposed (hpsi_terms_t a_transposed / b_transposed)
 };
 
 struct Group {
@@ -60,7 +61,9 @@ struct P1Unit {               // one CTA of the first-GEMM kernel: one tile posi
   int32_t t0, t1;             // terms [t0, t1) of the group, processed one after the other (pipeline never drains)
   int32_t i0, rows_valid;     // row tile inside one task's intermediate
   int32_t j0, cols_valid;     // column tile
-  int32_t grid;               // WarpGrid
+  int32_t grid;               // warp columns gn
+  int32_t xtrans;             // 1: the operator blocks of these terms are stored transposed (K-major X operand)
+  int32_t pad;
 };
 
 struct Run {                  // consecutive segs of one group inside one P2 unit's K range
@@ -72,6 +75,8 @@ struct Run {                  // consecutive segs of one group inside one P2 uni
   int32_t seg0;               // group.seg0 (seg - seg0 = task index inside the stacked intermediate)
   int32_t ws_map;             // group.ws_map
   int64_t ws_off;             // group.ws_off
+  int32_t trans;              // 1: the operator blocks of these segs are stored transposed (K-major operand)
+  int32_t pad;
 };
 
 struct P2Unit {               // one CTA of the second-GEMM kernel
@@ -79,17 +84,18 @@ struct P2Unit {               // one CTA of the second-GEMM kernel
   int32_t i0, rows_valid, j0, cols_valid;
   int64_t out_off;            // partial buffer offset of element (i0, j0) of this split's m x ldp tile
   int32_t ldo;
-  int32_t grid;               // WarpGrid
+  int32_t grid;               // warp columns gn
 };
 
-// A 2-D row-major matrix the TMA unit reads: rows x cols doubles, leading dimension ld, `off` doubles into `base`.
-// Encoded (api.cu) as a CUtensorMap with box {KT columns, box_rows rows}, 128-byte swizzle, zero fill out of bounds.
+// A 2-D row-major matrix the TMA unit reads: rows x cols doubles as STORED, leading dimension ld, `off` doubles into
+// `base`.  Encoded (api.cu) as a CUtensorMap with box {box_cols columns, box_rows rows}, 128-byte swizzle, zero fill
+// out of bounds.  K-contiguous operand ("N" layout): rows = the operand's rows, cols = K, box {KT, TILE}.
+// Block stored transposed ("T" layout): rows = K, cols = the operand's rows, box {16, KT}.
 struct MapSpec {
   int64_t off;
   int32_t base;               // BaseSel
   int32_t rows, cols, ld;
-  int32_t box_rows;
-  int32_t pad;
+  int32_t box_rows, box_cols;
 };
 
 struct PsiBlk {               // one psi block and its padded copies
@@ -129,6 +135,7 @@ struct Schedule {
   int64_t n_order1 = 0;
   int32_t max_block_elems = 0;
   bool aligned16 = true;              // descriptors allow the 16-byte staging path (arena base checked at bind)
+  bool paired = false;                // some block is stored transposed: fragments are taken from 16-row groups (kernels.cu)
 };
 
 // Host planner.  Returns HPSI_OK or an error code with `err` filled.
@@ -143,12 +150,28 @@ inline int even_up(int x) { return x + (x & 1); }
 // 128-byte row segment is exactly four sectors (measured: 16-byte-aligned rows cost 1.4x the sectors).
 inline int sector_up(int x) { return (x + 3) & ~3; }
 inline int frags(int x) { return (x + 7) / 8; }
+// fragments a tile dimension of x rows occupies: in paired mode fragments come in pairs that interleave 16 rows
+inline int tile_frags(int x, bool paired) { return paired ? 2 * ((x + 15) / 16) : (x + 7) / 8; }
 // Heaviest warp (in fragments) when a tile of fm x fn fragments is covered by a gm x gn grid of warps, and the grid
 // that minimises it among those whose warp tile has a compiled instantiation (<=4x4, <=8x2, <=2x8 fragments);
 // ties go to the squarest grid (fewest shared-memory reads per DMMA).
 inline int heaviest_warp(int fm, int fn, int gm, int gn) { return ((fm + gm - 1) / gm) * ((fn + gn - 1) / gn); }
 inline bool warp_tile_ok(int mi, int nj) { return (mi <= 4 && nj <= 4) || (mi <= 8 && nj <= 2) || (mi <= 2 && nj <= 8); }
-inline int32_t best_grid(int fm, int fn, int* heaviest = nullptr) {
+inline int32_t best_grid(int fm, int fn, int* heaviest = nullptr, bool paired = false) {
+  if (paired) {                        // warps own whole pairs (2 fragments): <=2x2, <=4x1 or <=1x4 pairs per warp
+    const int pm = fm / 2, pn = fn / 2;
+    const int order[4] = {2, 4, 1, NCONS_WARPS};
+    int best = 1 << 30;
+    int32_t g = 2;
+    for (int gn : order) {
+      if (gn > NCONS_WARPS || NCONS_WARPS % gn) continue;
+      const int gm = NCONS_WARPS / gn, mp = (pm + gm - 1) / gm, np = (pn + gn - 1) / gn;
+      if (!((mp <= 2 && np <= 2) || (mp <= 4 && np <= 1) || (mp <= 1 && np <= 4))) continue;
+      if (mp * np < best) { best = mp * np; g = gn; }
+    }
+    if (heaviest) *heaviest = 4 * best;
+    return g;
+  }
   const int order[4] = {NCONS_WARPS == 8 ? 2 : 2, NCONS_WARPS == 8 ? 4 : 4, 1, NCONS_WARPS};   // squarest first
   int best = 1 << 30;
   int32_t g = 2;

@@ -66,6 +66,7 @@ int64_t align_up(int64_t x, int64_t a) { return (x + a - 1) / a * a; }
 
 struct RawTask {
   int32_t term, ia, ib, src, dst;   // src/dst = psi block indices
+  int32_t ta, tb;                   // A / B block stored transposed
 };
 
 }  // namespace
@@ -125,8 +126,8 @@ int build_schedule(const hpsi_sectors_t* s, const hpsi_terms_t* t, uint32_t flag
 
   // ---- validation of block descriptors
   sc->aligned16 = true;
-  auto check_blocks = [&](int64_t n, const hpsi_opblock_t* blk, const int32_t* d, int nsec, int64_t arena_len,
-                          const char* side) -> int {
+  auto check_blocks = [&](int64_t n, const hpsi_opblock_t* blk, const uint8_t* tr, const int32_t* d, int nsec,
+                          int64_t arena_len, const char* side) -> int {
     std::unordered_map<uint64_t, int64_t> seen;
     seen.reserve((size_t)n * 2);
     for (int64_t i = 0; i < n; ++i) {
@@ -134,9 +135,11 @@ int build_schedule(const hpsi_sectors_t* s, const hpsi_terms_t* t, uint32_t flag
       if (e.term < 0 || e.term >= t->n_terms) FAIL(HPSI_EINVAL, "%s block %lld: term %d out of range", side, (long long)i, e.term);
       if (e.row < 0 || e.row >= nsec || e.col < 0 || e.col >= nsec)
         FAIL(HPSI_EINVAL, "%s block %lld: sector index out of range", side, (long long)i);
-      if (e.ld < d[e.col]) FAIL(HPSI_EINVAL, "%s block %lld: ld %d < cols %d", side, (long long)i, e.ld, d[e.col]);
+      const bool tflag = tr && tr[i];                       // stored as the d[col] x d[row] transpose
+      const int srows = tflag ? d[e.col] : d[e.row], scols = tflag ? d[e.row] : d[e.col];
+      if (e.ld < scols) FAIL(HPSI_EINVAL, "%s block %lld: ld %d < stored cols %d", side, (long long)i, e.ld, scols);
       if (e.offset < 0) FAIL(HPSI_EINVAL, "%s block %lld: negative offset", side, (long long)i);
-      int64_t last = e.offset + (int64_t)(d[e.row] - 1) * e.ld + d[e.col];
+      int64_t last = e.offset + (int64_t)(srows - 1) * e.ld + scols;
       if (arena_len > 0 && last > arena_len)
         FAIL(HPSI_EINVAL, "%s block %lld: extends past the arena (%lld > %lld)", side, (long long)i, (long long)last, (long long)arena_len);
       uint64_t key = ((uint64_t)e.term * (uint64_t)nsec + (uint64_t)e.row) * (uint64_t)nsec + (uint64_t)e.col;
@@ -145,8 +148,13 @@ int build_schedule(const hpsi_sectors_t* s, const hpsi_terms_t* t, uint32_t flag
     }
     return HPSI_OK;
   };
-  if (int rc = check_blocks(t->n_a, t->a_blocks, s->d_left, nL, t->a_len, "A")) return rc;
-  if (int rc = check_blocks(t->n_b, t->b_blocks, s->d_right, nR, t->b_len, "B")) return rc;
+  if (int rc = check_blocks(t->n_a, t->a_blocks, t->a_transposed, s->d_left, nL, t->a_len, "A")) return rc;
+  if (int rc = check_blocks(t->n_b, t->b_blocks, t->b_transposed, s->d_right, nR, t->b_len, "B")) return rc;
+
+  sc->paired = false;
+  if (t->a_transposed) for (int64_t i = 0; i < t->n_a; ++i) if (t->a_transposed[i]) sc->paired = true;
+  if (t->b_transposed) for (int64_t i = 0; i < t->n_b; ++i) if (t->b_transposed[i]) sc->paired = true;
+  const bool paired = sc->paired;
 
   // ---- step 2: task enumeration
   std::unordered_map<uint64_t, int64_t> b_index;
@@ -163,11 +171,16 @@ int build_schedule(const hpsi_sectors_t* s, const hpsi_terms_t* t, uint32_t flag
     uint64_t key = ((uint64_t)a.term * (uint64_t)nR + (uint64_t)partner[a.row]) * (uint64_t)nR + (uint64_t)partner[a.col];
     auto it = b_index.find(key);
     if (it == b_index.end()) continue;
-    raw.push_back({a.term, (int32_t)ia, (int32_t)it->second, src, dst});
+    raw.push_back({a.term, (int32_t)ia, (int32_t)it->second, src, dst,
+                   (t->a_transposed && t->a_transposed[ia]) ? 1 : 0,
+                   (t->b_transposed && t->b_transposed[it->second]) ? 1 : 0});
   }
+  // inside a (source, destination) group: tasks with the same storage layout together, then by term
   std::stable_sort(raw.begin(), raw.end(), [](const RawTask& x, const RawTask& y) {
     if (x.dst != y.dst) return x.dst < y.dst;
     if (x.src != y.src) return x.src < y.src;
+    if (x.ta != y.ta) return x.ta < y.ta;
+    if (x.tb != y.tb) return x.tb < y.tb;
     return x.term < y.term;
   });
 
@@ -184,7 +197,13 @@ int build_schedule(const hpsi_sectors_t* s, const hpsi_terms_t* t, uint32_t flag
   }
   sc->maps.clear();
   auto add_map = [&](int base, int64_t moff, int rows, int cols, int ld) -> int32_t {
-    sc->maps.push_back({moff, base, rows, cols, ld, TILE, 0});
+    sc->maps.push_back({moff, base, rows, cols, ld, TILE, KT});
+    return (int32_t)sc->maps.size() - 1;
+  };
+  // operator block that is an NT operand with op_rows rows and K = op_k columns; stored transposed if tr
+  auto add_op_map = [&](int base, int64_t moff, int op_rows, int op_k, int ld, int tr) -> int32_t {
+    if (!tr) return add_map(base, moff, op_rows, op_k, ld);
+    sc->maps.push_back({moff, base, op_k, op_rows, ld, KT, 16});
     return (int32_t)sc->maps.size() - 1;
   };
   for (auto& b : sc->blocks) {
@@ -226,12 +245,14 @@ int build_schedule(const hpsi_sectors_t* s, const hpsi_terms_t* t, uint32_t flag
       // operator blocks as NT operands: A_t is (m x k), B_t is (n x n'); each block belongs to exactly one task
       if (order == 1) {
         sg.p1_off = a.offset; sg.p1_ld = a.ld; sg.p2_off = b.offset; sg.p2_ld = b.ld;
-        sg.p1_map = add_map(BASE_A, a.offset, (int)m, (int)k, a.ld);
-        sg.p2_map = add_map(BASE_B, b.offset, (int)n, (int)np, b.ld);
+        sg.p1_trans = raw[q].ta; sg.p2_trans = raw[q].tb;
+        sg.p1_map = add_op_map(BASE_A, a.offset, (int)m, (int)k, a.ld, raw[q].ta);
+        sg.p2_map = add_op_map(BASE_B, b.offset, (int)n, (int)np, b.ld, raw[q].tb);
       } else {
         sg.p1_off = b.offset; sg.p1_ld = b.ld; sg.p2_off = a.offset; sg.p2_ld = a.ld;
-        sg.p1_map = add_map(BASE_B, b.offset, (int)n, (int)np, b.ld);
-        sg.p2_map = add_map(BASE_A, a.offset, (int)m, (int)k, a.ld);
+        sg.p1_trans = raw[q].tb; sg.p2_trans = raw[q].ta;
+        sg.p1_map = add_op_map(BASE_B, b.offset, (int)n, (int)np, b.ld, raw[q].tb);
+        sg.p2_map = add_op_map(BASE_A, a.offset, (int)m, (int)k, a.ld, raw[q].ta);
       }
       sg.coef = t->coef[raw[q].term];
       sc->segs.push_back(sg);
@@ -289,16 +310,22 @@ int build_schedule(const hpsi_sectors_t* s, const hpsi_terms_t* t, uint32_t flag
       auto ct = split_cols(g.N1);
       const int64_t ks = (g.K1 + 3) / 4;
       const int nt = g_nt[go.gi];
-      for (int t0 = 0; t0 < g.tcount; t0 += nt) {
-        const int t1 = std::min(g.tcount, t0 + nt);
-        for (auto& r : rt)
-          for (auto& c : ct) {
-            sc->p1.push_back({go.gi, t0, t1, r.start, r.len, c.start, c.len, best_grid(frags(r.len), frags(c.len))});
-            sc->issued_flops_p1 += (int64_t)frags(r.len) * frags(c.len) * ks * 512 * (t1 - t0);
-            int heavy = 0;
-            best_grid(frags(r.len), frags(c.len), &heavy);
-            sc->critical_flops += (int64_t)NCONS_WARPS * heavy * ks * 512 * (t1 - t0);
-          }
+      int tb = 0;                                   // segs [0, tb) have a plainly stored P1 operator block, [tb, tcount) a transposed one
+      while (tb < g.tcount && !sc->segs[g.seg0 + tb].p1_trans) ++tb;
+      for (int part = 0; part < 2; ++part) {
+        const int lo = part ? tb : 0, hi = part ? g.tcount : tb;
+        for (int t0 = lo; t0 < hi; t0 += nt) {
+          const int t1 = std::min(hi, t0 + nt);
+          for (auto& r : rt)
+            for (auto& c : ct) {
+              const int fm = tile_frags(r.len, paired), fn = tile_frags(c.len, paired);
+              int heavy = 0;
+              const int32_t grid = best_grid(fm, fn, &heavy, paired);
+              sc->p1.push_back({go.gi, t0, t1, r.start, r.len, c.start, c.len, grid, part, 0});
+              sc->issued_flops_p1 += (int64_t)fm * fn * ks * 512 * (t1 - t0);
+              sc->critical_flops += (int64_t)NCONS_WARPS * heavy * ks * 512 * (t1 - t0);
+            }
+        }
       }
     }
   }
@@ -324,7 +351,7 @@ int build_schedule(const hpsi_sectors_t* s, const hpsi_terms_t* t, uint32_t flag
       DstInfo& di = dsts[d];
       di.rt = split_rows(sc->blocks[d].rows);
       di.ct = split_cols(sc->blocks[d].cols);
-      for (auto& r : di.rt) for (auto& c : di.ct) di.maxf = std::max(di.maxf, frags(r.len) * frags(c.len));
+      for (auto& r : di.rt) for (auto& c : di.ct) di.maxf = std::max(di.maxf, tile_frags(r.len, paired) * tile_frags(c.len, paired));
       di.g0 = (int)gi;
       while (gi < sc->groups.size() && sc->groups[gi].dst == d) {
         di.cost += (int64_t)sc->groups[gi].tcount * seg_cost(sc->groups[gi], di.maxf);   // heaviest tile of the block
@@ -372,7 +399,13 @@ int build_schedule(const hpsi_sectors_t* s, const hpsi_terms_t* t, uint32_t flag
         if (sp == nsplit - 1) take = g.tcount - ti;
         else take = (int)std::min<int64_t>(g.tcount - ti, std::max<int64_t>(1, (want - cum + per - 1) / per));
         if (take > 0) {
-          sc->runs.push_back({g.seg0 + ti, g.seg0 + ti + take, g.N1, g.ldw, g.order, g.rows, g.seg0, g.ws_map, g.ws_off});
+          // a run has one storage layout of its operator blocks: split [ti, ti + take) at the group's layout boundary
+          int tbnd = ti;
+          while (tbnd < ti + take && !sc->segs[g.seg0 + tbnd].p2_trans) ++tbnd;
+          if (tbnd > ti)
+            sc->runs.push_back({g.seg0 + ti, g.seg0 + tbnd, g.N1, g.ldw, g.order, g.rows, g.seg0, g.ws_map, g.ws_off, 0, 0});
+          if (tbnd < ti + take)
+            sc->runs.push_back({g.seg0 + tbnd, g.seg0 + ti + take, g.N1, g.ldw, g.order, g.rows, g.seg0, g.ws_map, g.ws_off, 1, 0});
           cum += per * take;
           chunk_ksteps += (int64_t)((g.N1 + 3) / 4) * take;
           ti += take;
@@ -388,19 +421,20 @@ int build_schedule(const hpsi_sectors_t* s, const hpsi_terms_t* t, uint32_t flag
           u.run_begin = run0; u.run_end = run1;
           u.i0 = r.start; u.rows_valid = r.len; u.j0 = c.start; u.cols_valid = c.len;
           u.ldo = D.ldo;
-          u.grid = best_grid(frags(r.len), frags(c.len));
+          const int fm = tile_frags(r.len, paired), fn = tile_frags(c.len, paired);
+          u.grid = best_grid(fm, fn, nullptr, paired);
           u.out_off = ws + (int64_t)realised * D.rows * D.ldo + (int64_t)r.start * D.ldo + c.start;
           sc->p2.push_back(u);
-          const int64_t dmma = (int64_t)frags(r.len) * frags(c.len) * chunk_ksteps;
+          const int64_t dmma = (int64_t)fm * fn * chunk_ksteps;
           int64_t cost = 0;                         // this tile's cost over the chunk's runs, stage floor included
           for (int ri = run0; ri < run1; ++ri) {
             const Run& rr = sc->runs[ri];
             Group gg{};
             gg.N1 = rr.K;
-            cost += (int64_t)(rr.seg_end - rr.seg_begin) * seg_cost(gg, (int64_t)frags(r.len) * frags(c.len));
+            cost += (int64_t)(rr.seg_end - rr.seg_begin) * seg_cost(gg, (int64_t)fm * fn);
           }
           int heavy = 0;
-          best_grid(frags(r.len), frags(c.len), &heavy);
+          best_grid(fm, fn, &heavy, paired);
           sc->critical_flops += (int64_t)NCONS_WARPS * heavy * chunk_ksteps * 512;
           unit_bundle.push_back((int)bundle_cost.size());
           bundle_max = std::max(bundle_max, cost);

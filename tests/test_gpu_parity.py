@@ -327,3 +327,62 @@ def test_lanczos_small(H, small):
     assert np.linalg.norm(oracle.apply(small, x) - theta * x) <= 2e-4
     th_d, _, info_d = _davidson(H, g, workloads.make_psi(small), tol=1e-7, max_iter=300)
     assert info_d["converged"] and abs(theta - th_d) <= 1e-6 * max(1.0, abs(th_d))
+
+
+@pytest.mark.parametrize("misalign", [False, True])
+def test_shared_adjoint_storage(H, toy, misalign):
+    """hpsi_terms_t a_transposed / b_transposed: adjoint terms read their partner's blocks transposed (TMA 16x16 boxes,
+    or the 8-byte LDGSTS variant when misaligned); the oracle sees the fully materialised problem."""
+    import torch
+    for name, kw in (("toy", {}), ("small", {"n_terms": 60})):
+        full = workloads.make_problem(name, **kw)
+        shared = workloads.make_problem(name, share_adjoint=True, **kw)
+        psi = workloads.make_psi(full, 1)
+        ref = oracle.apply(full, psi)
+        for flags in (0, H.HPSI_PLAN_FIXED_ORDER1, H.HPSI_PLAN_FIXED_ORDER2):
+            g = GpuProblem(shared, flags, misalign=misalign)
+            assert g.q(H.HPSI_Q_ALIGNED16) == (0 if misalign else 1)
+            out = g.apply(psi)
+            assert rel_l2(out, ref) <= TOL, (name, flags, rel_l2(out, ref))
+            assert np.array_equal(out, g.apply(psi))
+        d = torch.empty(g.n, dtype=torch.float64, device="cuda")
+        H.hpsi_diagonal(g.plan, d)
+        torch.cuda.synchronize()
+        dref = oracle.diagonal(full)
+        assert np.linalg.norm(d.cpu().numpy() - dref) <= 1e-12 * max(np.linalg.norm(dref), 1.0)
+
+
+def test_shared_adjoint_ragged_multi_tile(H):
+    """Transposed blocks spanning several tiles with ragged tails, even-but-not-multiple-of-4 leading dimensions."""
+    rng = np.random.default_rng(31)
+    dL, dR = [150, 70, 9], [131, 9, 77]
+    n = len(dL)
+    terms_full, half = [], []
+    for _ in range(5):
+        ab = {(r, c): rng.standard_normal((dL[r], dL[c])) for r in range(n) for c in range(n) if (r + 2 * c) % 3 != 1}
+        bb = {(r, c): rng.standard_normal((dR[r], dR[c])) for r in range(n) for c in range(n) if (r + 2 * c) % 3 != 1}
+        half.append((float(rng.standard_normal()), ab, bb))
+    adj = [(c, {(cc, r): a.T.copy() for (r, cc), a in ab.items()}, {(cc, r): b.T.copy() for (r, cc), b in bb.items()})
+           for c, ab, bb in half]
+    qL, qR = [(i, 0) for i in range(n)], [(n - i, 0) for i in range(n)]
+    full = workloads.custom_problem(qL, dL, qR, dR, (n, 0), half + adj, pad_even=True)
+    base = workloads.custom_problem(qL, dL, qR, dR, (n, 0), half, pad_even=True)
+    # shared problem: the adjoint terms' descriptors point at the base blocks, flagged transposed
+    import copy
+    shared = copy.copy(full)
+    def share(desc_full, desc_base, nterm):
+        out = desc_full.copy()
+        tr = np.zeros(out.shape[0], np.uint8)
+        key = {(int(e["term"]), int(e["row"]), int(e["col"])): e for e in desc_base}
+        for i, e in enumerate(out):
+            if e["term"] >= nterm:
+                b = key[(int(e["term"]) - nterm, int(e["col"]), int(e["row"]))]
+                out[i]["offset"], out[i]["ld"], tr[i] = b["offset"], b["ld"], 1
+        return out, tr
+    shared.a_desc, shared.a_trans = share(full.a_desc, base.a_desc, len(half))
+    shared.b_desc, shared.b_trans = share(full.b_desc, base.b_desc, len(half))
+    shared.a_data, shared.b_data, shared.a_len, shared.b_len = base.a_data, base.b_data, base.a_len, base.b_len
+    psi = rng.standard_normal(full.psi_len)
+    ref = oracle.apply(full, psi)
+    for misalign in (False, True):
+        assert rel_l2(GpuProblem(shared, misalign=misalign).apply(psi), ref) <= TOL

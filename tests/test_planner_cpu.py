@@ -188,7 +188,7 @@ def test_empty_problems():
 
 def test_struct_sizes():
     assert ctypes.sizeof(H.binding.hpsi_sectors_t) == 48
-    assert ctypes.sizeof(H.binding.hpsi_terms_t) == 80
+    assert ctypes.sizeof(H.binding.hpsi_terms_t) == 96      # + a_transposed, b_transposed
     assert H.binding.PSI_BLOCK_DTYPE.itemsize == 24 and H.binding.TASK_DTYPE.itemsize == 24
 
 
@@ -256,3 +256,31 @@ def test_task_coefficients_interpreter(toy):
     tasks = H.hpsi_query(plan, H.HPSI_Q_TASKS)
     H.hpsi_set_task_coefficients(plan, toy.coef[tasks["term"]])
     assert rel(H.hpsi_debug_interpret(plan, toy.a_data, toy.b_data, psi), oracle.apply(toy, psi)) <= 1e-13
+
+
+# ------------------------------------------------------------------- adjoint-pair storage sharing (8(f)-2)
+@pytest.mark.parametrize("name,kw", [("toy", {}), ("small", {"n_terms": 40})])
+def test_shared_adjoint_storage_interpreter(name, kw):
+    """Adjoint terms that point at their partner's storage (blocks flagged transposed) give the same operator as the
+    fully materialised problem the oracle sees; the arenas are half as long."""
+    full = workloads.make_problem(name, **kw)
+    shared = workloads.make_problem(name, share_adjoint=True, **kw)
+    assert shared.a_len <= 0.51 * full.a_len and shared.b_len <= 0.51 * full.b_len
+    assert int(shared.a_trans.sum()) == full.a_desc.shape[0] // 2
+    psi = workloads.make_psi(full)
+    ref = oracle.apply(full, psi)
+    for flags in (0, H.HPSI_PLAN_FIXED_ORDER1, H.HPSI_PLAN_FIXED_ORDER2):
+        plan = host_plan(shared, flags)
+        assert H.hpsi_query(plan, H.HPSI_Q_N_TASKS) == H.hpsi_query(host_plan(full, flags), H.HPSI_Q_N_TASKS)
+        assert rel(H.hpsi_debug_interpret(plan, shared.a_data, shared.b_data, psi), ref) <= 1e-13
+
+
+def test_transposed_block_validation(toy):
+    shared = workloads.make_problem("toy", share_adjoint=True)
+    bad = shared.a_desc.copy()
+    j = int(np.flatnonzero(shared.a_trans)[0])
+    bad[j]["ld"] = 0                                            # ld < stored columns
+    with pytest.raises(H.HpsiError) as e:
+        H.hpsi_plan(shared.q_left, shared.q_right, shared.d_left, shared.d_right, shared.target, shared.coef, bad,
+                    shared.b_desc, None, None, shared.a_len, shared.b_len, H.HPSI_PLAN_HOST_ONLY, shared.a_trans, shared.b_trans)
+    assert e.value.code == H.HPSI_EINVAL

@@ -60,6 +60,8 @@ class Problem:
     b_len: int
     a_data: Optional[np.ndarray] = None   # float64 arenas (None until filled)
     b_data: Optional[np.ndarray] = None
+    a_trans: Optional[np.ndarray] = None  # [n_a] uint8: 1 = the arena holds this block transposed (adjoint-pair sharing)
+    b_trans: Optional[np.ndarray] = None
     # generator-side bookkeeping (not part of the boundary)
     shifts: Optional[np.ndarray] = None   # [n_terms, 2]
     partner: Optional[np.ndarray] = None  # [n_left] right index paired with left i by construction, -1 if none
@@ -278,14 +280,34 @@ def fill_term(p: Problem, t: int, a_data: np.ndarray, b_data: np.ndarray,
             off = int(e["offset"]) - base
             ld = int(e["ld"])
             np.lib.stride_tricks.as_strided(data[off:], shape=(r, c), strides=(ld * 8, 8))[...] = blk
+            if p.a_trans is not None:          # adjoint terms share the base term's storage (read transposed)
+                continue
             j = adj[(int(e["col"]), int(e["row"]))]
             ea = desc[j]
             offa, lda = int(ea["offset"]) - base, int(ea["ld"])
             np.lib.stride_tricks.as_strided(data[offa:], shape=(c, r), strides=(lda * 8, 8))[...] = blk.T
 
 
+def _share_adjoint(desc: np.ndarray, ranges: np.ndarray, half: int):
+    """Point every block of adjoint term t+half at the storage of its partner block of base term t (same offset and
+    ld, flagged transposed).  Returns (new descriptors, transposed flags, arena length that is still needed)."""
+    desc = desc.copy()
+    trans = np.zeros(desc.shape[0], np.uint8)
+    for t in range(half):
+        lo, hi = ranges[t]
+        alo, ahi = ranges[t + half]
+        base = {(int(desc[i]["row"]), int(desc[i]["col"])): i for i in range(lo, hi)}
+        for j in range(alo, ahi):
+            i = base[(int(desc[j]["col"]), int(desc[j]["row"]))]
+            desc[j]["offset"] = desc[i]["offset"]
+            desc[j]["ld"] = desc[i]["ld"]
+            trans[j] = 1
+    return desc, trans
+
+
 def make_problem(name: str, seed: Optional[int] = None, fill: bool = True, pad_even: bool = True,
-                 n_terms: Optional[int] = None, base_terms=None, row_align: Optional[int] = None) -> Problem:
+                 n_terms: Optional[int] = None, base_terms=None, row_align: Optional[int] = None,
+                 share_adjoint: bool = False) -> Problem:
     """Build config ``name`` (seed defaults to the config index).  ``fill=False`` returns descriptors only
     (arenas can then be streamed with ``fill_term``).  ``n_terms`` overrides the term count (tests).
     ``base_terms`` (indices into the T/2 base terms) keeps only those terms and their adjoints, with the same
@@ -314,10 +336,19 @@ def make_problem(name: str, seed: Optional[int] = None, fill: bool = True, pad_e
     if row_align is None:
         row_align = 4 if pad_even else 1
     a_desc, b_desc, a_len, b_len, ta, tb = _build_descriptors(q_left, q_right, d_left, d_right, shifts, row_align)
+    a_trans = b_trans = None
+    if share_adjoint:
+        # the arenas are term-major with the base terms first: keep that prefix, drop the materialised adjoint copies
+        if half > 0 and ta[half, 0] < a_desc.shape[0]:
+            a_len = int(a_desc["offset"][ta[half, 0]])
+        if half > 0 and tb[half, 0] < b_desc.shape[0]:
+            b_len = int(b_desc["offset"][tb[half, 0]])
+        a_desc, a_trans = _share_adjoint(a_desc, ta, half)
+        b_desc, b_trans = _share_adjoint(b_desc, tb, half)
     p = Problem(name=name, seed=seed, q_left=q_left, q_right=q_right, d_left=d_left, d_right=d_right,
                 target=target, coef=coef, a_desc=a_desc, b_desc=b_desc, a_len=int(a_len), b_len=int(b_len),
                 shifts=shifts, partner=partner, term_a_range=ta, term_b_range=tb, entry_seed=(seed, 303),
-                base_term_ids=ids)
+                base_term_ids=ids, a_trans=a_trans, b_trans=b_trans)
     if fill:
         p.a_data = np.zeros(max(p.a_len, 1), np.float64)
         p.b_data = np.zeros(max(p.b_len, 1), np.float64)
