@@ -52,18 +52,31 @@ struct WarpTileP {
 };
 
 template <int MI, int NJ>
+__device__ __forceinline__ void load_frags_p(const double* px, const double* py, const PairOffsets& po, int ks,
+                                             double (&a)[MI], double (&b)[NJ]) {
+#pragma unroll
+  for (int i = 0; i < MI; ++i) a[i] = px[po.x[i & 1][ks] + (i >> 1) * 256];
+#pragma unroll
+  for (int j = 0; j < NJ; ++j) b[j] = py[po.y[j & 1][ks] + (j >> 1) * 256];
+}
+// as mma_stage (kernels.cu): the fragments of k-step ks+1 are fetched while step ks issues
+template <int MI, int NJ>
 __device__ __forceinline__ void mma_stage_p(const double* px, const double* py, const PairOffsets& po,
                                             double (&acc)[MI][NJ][2], int nk4) {
-  double a[MI], b[NJ];
-#pragma unroll
-  for (int ks = 0; ks < 4; ++ks) {
-    if (ks < nk4) {
-#pragma unroll
-      for (int i = 0; i < MI; ++i) a[i] = px[po.x[i & 1][ks] + (i >> 1) * 256];
-#pragma unroll
-      for (int j = 0; j < NJ; ++j) b[j] = py[po.y[j & 1][ks] + (j >> 1) * 256];
-      mma_step<MI, NJ>(a, b, acc);
-    }
+  double a0[MI], b0[NJ], a1[MI], b1[NJ];
+  load_frags_p<MI, NJ>(px, py, po, 0, a0, b0);
+  if (nk4 == 4) {
+    load_frags_p<MI, NJ>(px, py, po, 1, a1, b1);
+    mma_step<MI, NJ>(a0, b0, acc);
+    load_frags_p<MI, NJ>(px, py, po, 2, a0, b0);
+    mma_step<MI, NJ>(a1, b1, acc);
+    load_frags_p<MI, NJ>(px, py, po, 3, a1, b1);
+    mma_step<MI, NJ>(a0, b0, acc);
+    mma_step<MI, NJ>(a1, b1, acc);
+  } else {
+    mma_step<MI, NJ>(a0, b0, acc);
+    if (nk4 > 1) { load_frags_p<MI, NJ>(px, py, po, 1, a0, b0); mma_step<MI, NJ>(a0, b0, acc); }
+    if (nk4 > 2) { load_frags_p<MI, NJ>(px, py, po, 2, a0, b0); mma_step<MI, NJ>(a0, b0, acc); }
   }
 }
 
