@@ -59,10 +59,12 @@ __global__ void small_eig_kernel(const double* __restrict__ G, int j, double* th
     if (t < j) { A[t][c] = 0.5 * (G[t * MMAX + c] + G[c * MMAX + t]); Q[t][c] = (t == c) ? 1.0 : 0.0; }
   __syncwarp();
   for (int sweep = 0; sweep < 30; ++sweep) {
-    double off = 0.0;
-    for (int p = 0; p < j; ++p)
+    double off = 0.0, dg = 0.0;
+    for (int p = 0; p < j; ++p) {
+      dg += A[p][p] * A[p][p];
       for (int q = p + 1; q < j; ++q) off += A[p][q] * A[p][q];
-    if (off < 1e-300) break;
+    }
+    if (off <= 1e-34 * (dg + 2.0 * off) || off < 1e-300) break;   // off-diagonal norm below 1e-17 of the matrix norm
     for (int p = 0; p < j - 1; ++p)
       for (int q = p + 1; q < j; ++q) {
         const double apq = A[p][q];

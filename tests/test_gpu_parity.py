@@ -386,3 +386,15 @@ def test_shared_adjoint_ragged_multi_tile(H):
     ref = oracle.apply(full, psi)
     for misalign in (False, True):
         assert rel_l2(GpuProblem(shared, misalign=misalign).apply(psi), ref) <= TOL
+
+
+def test_davidson_trajectory_matches_oracle(H, small):
+    """Step-by-step parity of the driver: without the (ill-conditioned) diagonal preconditioner the Ritz value and
+    the residual after k mat-vecs agree with the oracle's textbook Davidson (A21) to rounding."""
+    g = GpuProblem(small)
+    v0 = workloads.make_psi(small)
+    for it in (3, 7, 18):                       # 18 > m_max = 16: goes through a restart
+        theta, _, info = _davidson(H, g, v0, tol=1e-12, max_iter=it, precondition=False)
+        th_o, _, _, rn_o = oracle.davidson(small, v0, tol=1e-12, max_iter=it, precondition=False)
+        assert abs(theta - th_o) <= 1e-9 * abs(th_o), (it, theta, th_o)
+        assert abs(info["residual"] - rn_o) <= 1e-7 * rn_o, (it, info, rn_o)
