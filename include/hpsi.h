@@ -148,6 +148,23 @@ int hpsi_davidson(hpsi_plan_t* plan, double* psi_inout_dev, double* eig_host,
 int hpsi_lanczos(hpsi_plan_t* plan, double* psi_inout_dev, double* eig_host,
                  const hpsi_davidson_params_t* params, hpsi_davidson_info_t* info, void* cuda_stream);
 
+/* Operator streaming from HOST memory ("host-device datacommunication ... due to memory
+ * limitations"): for operators that do not fit HBM.  terms->a_data / b_data are pinned HOST arenas here
+ * (BORROWED, must outlive the object).  The term list is cut into windows of consecutive terms whose arena ranges fit
+ * `window_doubles` (A + B together); the object owns two device staging slots of that size and one plan per window.
+ * hpsi_stream_apply copies window w+1 on an internal copy stream while window w computes on `cuda_stream`; the windows'
+ * results add up in window order (deterministic).  out = H psi (overwrite); psi_dev / out_dev: DEVICE.  Enqueue only,
+ * but uses a second stream and events, so it is not CUDA-graph capturable.  Transposed blocks are not supported. */
+typedef struct hpsi_stream hpsi_stream_t;
+int hpsi_stream_create(const hpsi_sectors_t* sectors, const hpsi_terms_t* terms_with_host_arenas, int64_t window_doubles,
+                       uint32_t flags, hpsi_stream_t** out);
+int hpsi_stream_apply(hpsi_stream_t* s, const double* psi_dev, double* out_dev, void* cuda_stream);
+/* what: HPSI_Q_PSI_LENGTH, HPSI_Q_USEFUL_FLOPS, HPSI_Q_OPERATOR_BYTES (= bytes copied host->device per apply),
+ * HPSI_SQ_N_WINDOWS, HPSI_SQ_STAGING_BYTES; out: HOST int64. */
+enum { HPSI_SQ_N_WINDOWS = 100, HPSI_SQ_STAGING_BYTES = 101 };
+int hpsi_stream_query(const hpsi_stream_t* s, int what, void* out, size_t bytes);
+void hpsi_stream_destroy(hpsi_stream_t* s);
+
 /* hpsi_query items.  `out` is HOST; `bytes` must be >= the item's size (else EINVAL). */
 enum {
   HPSI_Q_PSI_LENGTH = 0,     /* int64: doubles in psi / out                                                  */

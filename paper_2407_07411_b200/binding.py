@@ -81,6 +81,14 @@ def lib() -> ctypes.CDLL:
                                     ctypes.POINTER(hpsi_davidson_info_t), vp]
         L.hpsi_lanczos.argtypes = L.hpsi_davidson.argtypes
         L.hpsi_query.argtypes = [vp, ctypes.c_int, vp, ctypes.c_size_t]
+        L.hpsi_stream_create.argtypes = [ctypes.POINTER(hpsi_sectors_t), ctypes.POINTER(hpsi_terms_t), i64, ctypes.c_uint32,
+                                         ctypes.POINTER(vp)]
+        L.hpsi_stream_apply.argtypes = [vp, vp, vp, vp]
+        L.hpsi_stream_query.argtypes = [vp, ctypes.c_int, vp, ctypes.c_size_t]
+        L.hpsi_stream_destroy.argtypes = [vp]
+        L.hpsi_stream_destroy.restype = None
+        for name in ("hpsi_stream_create", "hpsi_stream_apply", "hpsi_stream_query"):
+            getattr(L, name).restype = ctypes.c_int
         L.hpsi_destroy.argtypes = [vp]
         L.hpsi_destroy.restype = None
         L.hpsi_last_error.restype = ctypes.c_char_p
@@ -213,6 +221,50 @@ def hpsi_lanczos(plan: Plan, psi_inout, tol: float = 1e-8, max_iter: int = 200, 
     _check(lib().hpsi_lanczos(plan.handle, _ptr(psi_inout), ctypes.byref(eig), ctypes.byref(prm),
                               ctypes.byref(info), _stream(stream)))
     return eig.value, {"n_matvec": info.n_matvec, "converged": bool(info.converged), "residual": info.residual}
+
+
+HPSI_SQ_N_WINDOWS, HPSI_SQ_STAGING_BYTES = 100, 101
+
+
+class StreamPlan:
+    """Opaque hpsi_stream_t* (operators streamed from pinned host arenas) plus the host arrays it borrows."""
+
+    def __init__(self, handle: int, keep):
+        self.handle = handle
+        self._keep = keep
+
+    def __del__(self):
+        if getattr(self, "handle", None):
+            lib().hpsi_stream_destroy(self.handle)
+            self.handle = None
+
+
+def hpsi_stream_create(p, a_host, b_host, window_doubles: int, flags: int = 0) -> StreamPlan:
+    """p: a ``workloads.Problem``-like object; a_host / b_host: pinned torch CPU float64 tensors holding the arenas."""
+    q_left = np.ascontiguousarray(p.q_left, np.int32).reshape(-1, 2)
+    q_right = np.ascontiguousarray(p.q_right, np.int32).reshape(-1, 2)
+    d_left = np.ascontiguousarray(p.d_left, np.int32)
+    d_right = np.ascontiguousarray(p.d_right, np.int32)
+    coef = np.ascontiguousarray(p.coef, np.float64)
+    a_blocks, b_blocks = np.ascontiguousarray(p.a_desc), np.ascontiguousarray(p.b_desc)
+    sec = hpsi_sectors_t(q_left.shape[0], q_right.shape[0], q_left.ctypes.data, q_right.ctypes.data,
+                         d_left.ctypes.data, d_right.ctypes.data, (ctypes.c_int32 * 2)(int(p.target[0]), int(p.target[1])))
+    trm = hpsi_terms_t(coef.shape[0], coef.ctypes.data, a_blocks.shape[0], a_blocks.ctypes.data,
+                       b_blocks.shape[0], b_blocks.ctypes.data, _ptr(a_host), _ptr(b_host), int(p.a_len), int(p.b_len),
+                       None, None)
+    out = ctypes.c_void_p()
+    _check(lib().hpsi_stream_create(ctypes.byref(sec), ctypes.byref(trm), int(window_doubles), flags, ctypes.byref(out)))
+    return StreamPlan(out.value, (a_host, b_host))
+
+
+def hpsi_stream_apply(sp: StreamPlan, psi, out, stream=None) -> None:
+    _check(lib().hpsi_stream_apply(sp.handle, _ptr(psi), _ptr(out), _stream(stream)))
+
+
+def hpsi_stream_query(sp: StreamPlan, what: int) -> int:
+    v = ctypes.c_int64()
+    _check(lib().hpsi_stream_query(sp.handle, what, ctypes.addressof(v), 8))
+    return v.value
 
 
 def hpsi_query(plan: Plan, what: int):

@@ -209,6 +209,9 @@ extern "C" int hpsi_set_task_coefficients(hpsi_plan_t* p, const double* coef_hos
 extern "C" void hpsi_destroy(hpsi_plan_t* p) { free_plan(p); }
 
 extern "C" int hpsi_apply(hpsi_plan_t* p, const double* psi_dev, double* out_dev, void* cuda_stream) {
+  return hpsi::apply_impl(p, psi_dev, out_dev, false, cuda_stream);
+}
+int hpsi::apply_impl(hpsi_plan_t* p, const double* psi_dev, double* out_dev, bool accumulate, void* cuda_stream) {
   if (!p) { set_error("null plan"); return HPSI_EINVAL; }
   if (p->host_only) { set_error("host-only plan: hpsi_apply needs a CUDA device (no CPU fallback)"); return HPSI_ESTATE; }
   if (!p->bound) { set_error("operator arenas not bound (hpsi_bind)"); return HPSI_ESTATE; }
@@ -219,7 +222,7 @@ extern "C" int hpsi_apply(hpsi_plan_t* p, const double* psi_dev, double* out_dev
   launch_prep(p->dev, psi_dev, st);
   launch_p1(p->dev, p->aligned16, st);
   launch_p2(p->dev, p->aligned16, st);
-  launch_reduce(p->dev, out_dev, st);
+  launch_reduce(p->dev, out_dev, accumulate, st);
   HPSI_CUDA(cudaGetLastError());
   return HPSI_OK;
 }
@@ -240,7 +243,7 @@ extern "C" int hpsi_apply_profiled(hpsi_plan_t* p, const double* psi_dev, double
   HPSI_CUDA(cudaEventRecord(ev[2], st));
   launch_p2(p->dev, p->aligned16, st);
   HPSI_CUDA(cudaEventRecord(ev[3], st));
-  launch_reduce(p->dev, out_dev, st);
+  launch_reduce(p->dev, out_dev, false, st);
   HPSI_CUDA(cudaEventRecord(ev[4], st));
   HPSI_CUDA(cudaEventSynchronize(ev[4]));
   for (int i = 0; i < 4; ++i) HPSI_CUDA(cudaEventElapsedTime(&ms_host[i], ev[i], ev[i + 1]));

@@ -272,14 +272,14 @@ __global__ void prep_kernel(DevSchedule d, const double* __restrict__ psi) {
 
 // reduce: out block = sum of its split-K partials in split order (fixed order -> bitwise reproducible);
 // a block nobody writes (nsplit == 0) becomes zeros (step 5: overwrite semantics).
-__global__ void reduce_kernel(DevSchedule d, double* __restrict__ out) {
+__global__ void reduce_kernel(DevSchedule d, double* __restrict__ out, int accumulate) {
   const PsiBlk B = d.blocks[blockIdx.y];
   const int n = B.rows * B.cols;
   const int64_t stride = (int64_t)B.rows * B.ldo;
   for (int e = blockIdx.x * blockDim.x + threadIdx.x; e < n; e += gridDim.x * blockDim.x) {
     const int x = e / B.cols, y = e - x * B.cols;
     const double* p = d.ws + B.part_off + (int64_t)x * B.ldo + y;
-    double s = 0.0;
+    double s = accumulate ? out[B.off + e] : 0.0;           // hpsi_stream_apply: windows of terms add up in a fixed order
     for (int sp = 0; sp < B.nsplit; ++sp) s += p[sp * stride];
     out[B.off + e] = s;
   }
@@ -332,8 +332,8 @@ void launch_p2(const DevSchedule& d, bool tma, cudaStream_t st) {
   if (tma) p2_kernel<true><<<d.n_p2, NTHREADS, SMEM_BYTES, st>>>(d);
   else p2_kernel<false><<<d.n_p2, NTHREADS, SMEM_BYTES, st>>>(d);
 }
-void launch_reduce(const DevSchedule& d, double* out, cudaStream_t st) {
-  if (d.n_blocks > 0) reduce_kernel<<<elem_grid(d), 256, 0, st>>>(d, out);
+void launch_reduce(const DevSchedule& d, double* out, bool accumulate, cudaStream_t st) {
+  if (d.n_blocks > 0) reduce_kernel<<<elem_grid(d), 256, 0, st>>>(d, out, accumulate ? 1 : 0);
 }
 void launch_diag(const DevSchedule& d, double* diag, cudaStream_t st) {
   if (d.n_blocks > 0) diag_kernel<<<elem_grid(d), 256, 0, st>>>(d, diag);

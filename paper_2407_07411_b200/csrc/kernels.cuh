@@ -42,7 +42,7 @@ struct DevSchedule {           // device pointers to the uploaded tables
 void launch_prep(const DevSchedule& d, const double* psi, cudaStream_t st);
 void launch_p1(const DevSchedule& d, bool tma, cudaStream_t st);
 void launch_p2(const DevSchedule& d, bool tma, cudaStream_t st);
-void launch_reduce(const DevSchedule& d, double* out, cudaStream_t st);
+void launch_reduce(const DevSchedule& d, double* out, bool accumulate, cudaStream_t st);
 void launch_diag(const DevSchedule& d, double* diag, cudaStream_t st);
 void launch_p1_paired(const DevSchedule& d, bool tma, cudaStream_t st);   // kernels_paired.cu
 void launch_p2_paired(const DevSchedule& d, bool tma, cudaStream_t st);

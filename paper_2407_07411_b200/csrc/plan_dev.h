@@ -30,6 +30,7 @@ struct hpsi_plan {
 namespace hpsi {
 void set_error(const std::string& s);
 int cuda_fail(cudaError_t e, const char* what);   // records the message, returns HPSI_ECUDA
+int apply_impl(hpsi_plan_t* p, const double* psi_dev, double* out_dev, bool accumulate, void* cuda_stream);
 }  // namespace hpsi
 
 #define HPSI_CUDA(call)                                             \

@@ -398,3 +398,36 @@ def test_davidson_trajectory_matches_oracle(H, small):
         th_o, _, _, rn_o = oracle.davidson(small, v0, tol=1e-12, max_iter=it, precondition=False)
         assert abs(theta - th_o) <= 1e-9 * abs(th_o), (it, theta, th_o)
         assert abs(info["residual"] - rn_o) <= 1e-7 * rn_o, (it, info, rn_o)
+
+
+def test_streamed_operators(H, small):
+    """hpsi_stream_*: operator arenas in pinned host memory, streamed through two staging windows; several window
+    sizes (1 window ... one term per window) all reproduce the oracle, and repeated applies are bitwise equal."""
+    import torch
+    a_host = torch.from_numpy(small.a_data).pin_memory()
+    b_host = torch.from_numpy(small.b_data).pin_memory()
+    psi = workloads.make_psi(small, 3)
+    ref = oracle.apply(small, psi)
+    x = torch.from_numpy(psi).cuda()
+    per_term = (small.a_len + small.b_len) // small.n_terms
+    seen = set()
+    for window in (small.a_len + small.b_len, 40 * per_term, 3 * per_term):
+        sp = H.hpsi_stream_create(small, a_host, b_host, window)
+        nwin = H.hpsi_stream_query(sp, H.HPSI_SQ_N_WINDOWS)
+        seen.add(nwin)
+        assert H.hpsi_stream_query(sp, H.HPSI_Q_PSI_LENGTH) == small.psi_len
+        assert H.hpsi_stream_query(sp, H.HPSI_Q_USEFUL_FLOPS) == oracle.useful_flops(small)[0]
+        assert H.hpsi_stream_query(sp, H.HPSI_SQ_STAGING_BYTES) <= 2 * 8 * window + 64
+        y = torch.full_like(x, float("nan"))
+        H.hpsi_stream_apply(sp, x, y, torch.cuda.current_stream())
+        torch.cuda.synchronize()
+        out = y.cpu().numpy()
+        assert rel_l2(out, ref) <= TOL, (window, nwin)
+        y2 = torch.full_like(x, float("nan"))
+        for _ in range(2):                                  # back-to-back applies reuse the slots correctly
+            H.hpsi_stream_apply(sp, x, y2, torch.cuda.current_stream())
+        torch.cuda.synchronize()
+        assert np.array_equal(y2.cpu().numpy(), out)
+    assert min(seen) == 1 and max(seen) > 50
+    with pytest.raises(H.HpsiError):
+        H.hpsi_stream_create(small, a_host, b_host, 16)     # a term does not fit the window
