@@ -10,6 +10,7 @@ real-molecule workloads (F2 / N2 / FeMoco / P450), whose integral f
 from .configs import (CONFIG_NAMES, OPBLOCK_DTYPE, Problem, make_problem, make_psi, config_params,
                       custom_problem)
 from .hubbard import hubbard_two_block_problem
+from .site import make_isometries, pack_isometries, proportional_chi
 
 __all__ = ["CONFIG_NAMES", "OPBLOCK_DTYPE", "Problem", "make_problem", "make_psi", "config_params",
-           "custom_problem", "hubbard_two_block_problem"]
+           "custom_problem", "hubbard_two_block_problem", "make_isometries", "pack_isometries", "proportional_chi"]
