@@ -165,6 +165,74 @@ enum { HPSI_SQ_N_WINDOWS = 100, HPSI_SQ_STAGING_BYTES = 101 };
 int hpsi_stream_query(const hpsi_stream_t* s, int what, void* out, size_t bytes);
 void hpsi_stream_destroy(hpsi_stream_t* s);
 
+/* ------------------------------------------------------------------------------------------------------------------
+ * Site update after the eigen-solve.  PAPER.md:45 names "tensor contraction and matrix
+ * factorization" as the two core operations of tensor-network algorithms and PAPER.md:62 the sweep as a "sequence of
+ * updates of all tensors", but writes out neither step; DESIGN.md section 9 lists the readings R1-R5.
+ *
+ *   hpsi_truncate :  the matrix factorisation.  psi is block diagonal over (left sector l, partner r), so its SVD is
+ *                    the SVD of every block, psi_l = U_l S_l V_l^T.  The chi_max largest singular values over all
+ *                    blocks are kept (ties: lower left sector first; values <=
+ *                    1e-13 * sigma_max are never kept) and  O_l = the kept columns of U_l  is the new left basis.
+ *   hpsi_rotate_* :  the renormalised-operator update  A'_t[l,l'] = O_l^T A_t[l,l'] O_l'  for every block of every
+ *                    left operator, on the same grouped DMMA GEMM engine as hpsi_apply.
+ *
+ * Isometry layout ("ot", used by both): for l = 0..n_sectors-1 ascending, O_l^T as a dense chi_l x d_l row-major
+ * matrix (row a = the a-th kept left singular vector), concatenated; sum_l chi_l d_l doubles.
+ * ------------------------------------------------------------------------------------------------------------------ */
+
+/* One-sided Jacobi SVD (Hestenes) of every psi block of `plan`, on the device, then the global selection on the host.
+ *   psi_dev        DEVICE, psi_length doubles (not modified)
+ *   chi_max        number of singular values to keep over all blocks (>= 0)
+ *   ot_dev         DEVICE, receives the isometries in the layout above; capacity >= HPSI_Q_ISO_CAPACITY doubles
+ *   chi_host       HOST, int32[n_left]: kept states per left sector (0 for a sector without a psi block)
+ *   sigma_host     HOST or NULL, psi-rows doubles (HPSI_Q_PSI_ROWS = sum of d_left over the psi blocks): for every psi
+ *                  block in table order its d_left values, descending; entries past min(d_left, d_right) are 0
+ *   discarded_host HOST or NULL: sum of sigma^2 over everything not kept
+ * Synchronises the stream (chi is needed on the host).  Deterministic (fixed rotation order; the only atomic is the
+ * sweep's "anything rotated" flag).  Errors: EINVAL (null / negative arguments), ESTATE (host-only plan), ENOMEM, ECUDA. */
+int hpsi_truncate(hpsi_plan_t* plan, const double* psi_dev, int32_t chi_max, double* ot_dev, int32_t* chi_host,
+                  double* sigma_host, double* discarded_host, void* cuda_stream);
+
+typedef struct hpsi_rotate hpsi_rotate_t;   /* opaque; owns the schedule, the workspace (padded isometries, T^T) */
+
+/* Plan the update of `n_blocks` operator blocks of one side.  d / chi: HOST int32[n_sectors], enlarged and kept
+ * dimensions (0 <= chi <= d; chi = 0 removes the sector: blocks touching it produce nothing).  blocks: HOST
+ * descriptors as in hpsi_terms_t (copied); a_data_dev: DEVICE arena, BORROWED (must outlive the object; not modified);
+ * a_len: arena length in doubles (validation; 0 = unknown).  flags: HPSI_PLAN_HOST_ONLY (schedule only, for
+ * hpsi_rotate_query / hpsi_rotate_debug_interpret).  The TMA path needs even ld / offset and a 16-byte aligned arena,
+ * otherwise the 8-byte cp.async variant of the kernels runs. */
+int hpsi_rotate_plan(int32_t n_sectors, const int32_t* d, const int32_t* chi, int64_t n_blocks,
+                     const hpsi_opblock_t* blocks, const double* a_data_dev, int64_t a_len, uint32_t flags,
+                     hpsi_rotate_t** out);
+
+/* out_dev (DEVICE, HPSI_RQ_OUT_LENGTH doubles) receives every A' block in the plan-dictated layout that
+ * HPSI_RQ_OUT_BLOCKS describes (ld = chi[col] rounded up to 4, offsets multiples of 4: directly usable as the operator
+ * arena of the next hpsi_plan).  ot_dev: DEVICE isometries (layout above, HPSI_RQ_ISO_LENGTH doubles).  Padding
+ * elements of out_dev are not written.  Enqueue only, CUDA-graph capturable, bitwise reproducible. */
+int hpsi_rotate_apply(hpsi_rotate_t* r, const double* ot_dev, double* out_dev, void* cuda_stream);
+/* same with CUDA events between the kernels: ms_host (HOST, 3 floats) = [isometry copy, first GEMM, second GEMM] */
+int hpsi_rotate_apply_profiled(hpsi_rotate_t* r, const double* ot_dev, double* out_dev, void* cuda_stream, float* ms_host);
+
+enum {
+  HPSI_RQ_OUT_LENGTH = 0,    /* int64: doubles in the output arena                                               */
+  HPSI_RQ_OUT_BLOCKS = 1,    /* hpsi_opblock_t[n_blocks]: descriptor of A'_i for input block i (same term/row/col);
+                                a block that vanished (chi[row] == 0 or chi[col] == 0) has ld = 0, offset = -1     */
+  HPSI_RQ_ISO_LENGTH = 2,    /* int64: sum_l chi_l d_l                                                            */
+  HPSI_RQ_USEFUL_FLOPS = 3,  /* int64: sum over surviving blocks of 2 d_l d_l' chi_l' + 2 chi_l d_l chi_l'        */
+  HPSI_RQ_ALGO_BYTES = 4,    /* int64: 8 * (d_l d_l' read + chi_l chi_l' written) over surviving blocks           */
+  HPSI_RQ_WORKSPACE_BYTES = 5,
+  HPSI_RQ_N_UNITS_1 = 6,     /* int64: CTA work units of the first / second GEMM launch                           */
+  HPSI_RQ_N_UNITS_2 = 7,
+  HPSI_RQ_ALIGNED16 = 8,     /* int64: 1 if the TMA staging path is used                                          */
+  HPSI_RQ_INTERMEDIATE_BYTES = 9 /* int64: bytes of T^T written by the first GEMM (and read by the second)        */
+};
+int hpsi_rotate_query(const hpsi_rotate_t* r, int what, void* out, size_t bytes);
+void hpsi_rotate_destroy(hpsi_rotate_t* r);
+/* test entry point: walks the device schedule of the update with naive loops on the HOST (a_host: the arena,
+ * ot_host: isometries, out_host: HPSI_RQ_OUT_LENGTH doubles) */
+int hpsi_rotate_debug_interpret(const hpsi_rotate_t* r, const double* a_host, const double* ot_host, double* out_host);
+
 /* hpsi_query items.  `out` is HOST; `bytes` must be >= the item's size (else EINVAL). */
 enum {
   HPSI_Q_PSI_LENGTH = 0,     /* int64: doubles in psi / out                                                  */
@@ -185,7 +253,11 @@ enum {
   HPSI_Q_ISSUED_FLOPS_P1 = 15,    /* int64: first-GEMM share of HPSI_Q_ISSUED_FLOPS                           */
   HPSI_Q_TASKS = 16,         /* hpsi_task_t[n_tasks], in schedule order                                      */
   HPSI_Q_USEFUL_FLOPS_P1 = 17,/* int64: first-GEMM share of HPSI_Q_USEFUL_FLOPS                                */
-  HPSI_Q_CRITICAL_FLOPS = 18  /* int64: like ISSUED_FLOPS, but every CTA counted as 4 x its heaviest warp (what warp imbalance costs) */
+  HPSI_Q_CRITICAL_FLOPS = 18, /* int64: like ISSUED_FLOPS, but every CTA counted as 4 x its heaviest warp (what warp imbalance costs) */
+  HPSI_Q_PSI_ROWS = 19,      /* int64: sum of d_left over the psi blocks (length of hpsi_truncate's sigma_host)  */
+  HPSI_Q_ISO_CAPACITY = 20,  /* int64: sum of min(d_left, d_right) * d_left over the psi blocks (ot_dev capacity) */
+  HPSI_Q_SVD_SWEEPS = 21,    /* int64: Jacobi sweeps of the last hpsi_truncate on this plan                      */
+  HPSI_Q_SVD_LAUNCHES = 22   /* int64: kernels it launched                                                       */
 };
 
 typedef struct {

@@ -104,9 +104,12 @@ def rotate(d, chi, blocks, a_data, ot) -> List[np.ndarray]:
 
 def rotate_flops(d, chi, blocks) -> int:
     """Useful flops of the update in the order the product takes (right index first, reading R5):
-    2 d_l d_l' chi_l' + 2 chi_l d_l chi_l' per block."""
+    2 d_l d_l' chi_l' + 2 chi_l d_l chi_l' per block; a block whose row or column sector keeps nothing has no result
+    and counts nothing."""
     f = 0
     for e in blocks:
         l, lp = int(e["row"]), int(e["col"])
+        if int(chi[l]) == 0 or int(chi[lp]) == 0:
+            continue
         f += 2 * int(d[l]) * int(d[lp]) * int(chi[lp]) + 2 * int(chi[l]) * int(d[l]) * int(chi[lp])
     return f

@@ -20,7 +20,11 @@ HPSI_PLAN_FIXED_ORDER2 = 1 << 2
 (HPSI_Q_PSI_LENGTH, HPSI_Q_N_PSI_BLOCKS, HPSI_Q_PSI_BLOCKS, HPSI_Q_N_TASKS, HPSI_Q_USEFUL_FLOPS, HPSI_Q_ISSUED_FLOPS,
  HPSI_Q_OPERATOR_BYTES, HPSI_Q_WORKSPACE_BYTES, HPSI_Q_N_GROUPS, HPSI_Q_N_P1_UNITS, HPSI_Q_N_P2_UNITS,
  HPSI_Q_N_ORDER1_TASKS, HPSI_Q_LAUNCHES_PER_APPLY, HPSI_Q_ALIGNED16, HPSI_Q_INTERMEDIATE_BYTES,
- HPSI_Q_ISSUED_FLOPS_P1, HPSI_Q_TASKS, HPSI_Q_USEFUL_FLOPS_P1, HPSI_Q_CRITICAL_FLOPS) = range(19)
+ HPSI_Q_ISSUED_FLOPS_P1, HPSI_Q_TASKS, HPSI_Q_USEFUL_FLOPS_P1, HPSI_Q_CRITICAL_FLOPS, HPSI_Q_PSI_ROWS,
+ HPSI_Q_ISO_CAPACITY, HPSI_Q_SVD_SWEEPS, HPSI_Q_SVD_LAUNCHES) = range(23)
+(HPSI_RQ_OUT_LENGTH, HPSI_RQ_OUT_BLOCKS, HPSI_RQ_ISO_LENGTH, HPSI_RQ_USEFUL_FLOPS, HPSI_RQ_ALGO_BYTES,
+ HPSI_RQ_WORKSPACE_BYTES, HPSI_RQ_N_UNITS_1, HPSI_RQ_N_UNITS_2, HPSI_RQ_ALIGNED16, HPSI_RQ_INTERMEDIATE_BYTES) = range(10)
+OPBLOCK_DTYPE = np.dtype([("term", "<i4"), ("row", "<i4"), ("col", "<i4"), ("ld", "<i4"), ("offset", "<i8")], align=True)
 
 PSI_BLOCK_DTYPE = np.dtype([("left", "<i4"), ("right", "<i4"), ("rows", "<i4"), ("cols", "<i4"), ("offset", "<i8")],
                            align=True)
@@ -95,6 +99,17 @@ def lib() -> ctypes.CDLL:
         L.hpsi_bench_fp64_pipe.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.POINTER(ctypes.c_double),
                                            ctypes.POINTER(ctypes.c_double)]
         L.hpsi_debug_interpret.argtypes = [vp, vp, vp, vp, vp]
+        L.hpsi_truncate.argtypes = [vp, vp, ctypes.c_int32, vp, vp, vp, vp, vp]
+        L.hpsi_rotate_plan.argtypes = [ctypes.c_int32, vp, vp, i64, vp, vp, i64, ctypes.c_uint32, ctypes.POINTER(vp)]
+        L.hpsi_rotate_apply.argtypes = [vp, vp, vp, vp]
+        L.hpsi_rotate_apply_profiled.argtypes = [vp, vp, vp, vp, ctypes.POINTER(ctypes.c_float)]
+        L.hpsi_rotate_query.argtypes = [vp, ctypes.c_int, vp, ctypes.c_size_t]
+        L.hpsi_rotate_debug_interpret.argtypes = [vp, vp, vp, vp]
+        L.hpsi_rotate_destroy.argtypes = [vp]
+        L.hpsi_rotate_destroy.restype = None
+        for name in ("hpsi_truncate", "hpsi_rotate_plan", "hpsi_rotate_apply", "hpsi_rotate_apply_profiled",
+                     "hpsi_rotate_query", "hpsi_rotate_debug_interpret"):
+            getattr(L, name).restype = ctypes.c_int
         for name in ("hpsi_plan", "hpsi_bind", "hpsi_set_task_coefficients", "hpsi_apply", "hpsi_apply_host", "hpsi_apply_profiled", "hpsi_diagonal", "hpsi_davidson", "hpsi_lanczos",
                      "hpsi_query", "hpsi_bench_fp64_pipe", "hpsi_debug_interpret"):
             getattr(L, name).restype = ctypes.c_int
@@ -167,7 +182,9 @@ def hpsi_plan(q_left, q_right, d_left, d_right, target, coef, a_blocks, b_blocks
                        _ptr(a_transposed), _ptr(b_transposed))
     out = ctypes.c_void_p()
     _check(lib().hpsi_plan(ctypes.byref(sec), ctypes.byref(trm), flags, ctypes.byref(out)))
-    return Plan(out.value, (a_data, b_data))
+    pl = Plan(out.value, (a_data, b_data))
+    pl.n_left = q_left.shape[0]
+    return pl
 
 
 def hpsi_bind(plan: Plan, a_data, b_data) -> None:
@@ -292,6 +309,73 @@ def hpsi_debug_interpret(plan: Plan, a_host: np.ndarray, b_host: np.ndarray, psi
     out = np.empty_like(psi_host)
     _check(lib().hpsi_debug_interpret(plan.handle, _ptr(np.ascontiguousarray(a_host, np.float64)),
                                       _ptr(np.ascontiguousarray(b_host, np.float64)), _ptr(psi_host), _ptr(out)))
+    return out
+
+
+# ------------------------------------------------------------------------ site update
+def hpsi_truncate(plan: Plan, psi, chi_max: int, ot, stream=None):
+    """SVD truncation of psi (torch CUDA tensor).  ot: torch CUDA float64 tensor of >= HPSI_Q_ISO_CAPACITY doubles that
+    receives the isometries.  Returns (chi int32[n_left], sigma float64[HPSI_Q_PSI_ROWS], discarded_weight)."""
+    n_left = int(plan.n_left)
+    chi = np.zeros(n_left, np.int32)
+    sigma = np.zeros(max(hpsi_query(plan, HPSI_Q_PSI_ROWS), 1), np.float64)
+    disc = ctypes.c_double()
+    _check(lib().hpsi_truncate(plan.handle, _ptr(psi), int(chi_max), _ptr(ot), chi.ctypes.data, sigma.ctypes.data,
+                               ctypes.addressof(disc), _stream(stream)))
+    return chi, sigma[:hpsi_query(plan, HPSI_Q_PSI_ROWS)], disc.value
+
+
+class RotatePlan:
+    """Opaque hpsi_rotate_t* plus the arena it borrows."""
+
+    def __init__(self, handle: int, keep, n_blocks: int):
+        self.handle = handle
+        self._keep = keep
+        self.n_blocks = n_blocks
+
+    def __del__(self):
+        if getattr(self, "handle", None):
+            lib().hpsi_rotate_destroy(self.handle)
+            self.handle = None
+
+
+def hpsi_rotate_plan(d, chi, blocks, a_data=None, a_len: int = 0, flags: int = 0) -> RotatePlan:
+    """d / chi: int32 arrays per sector; blocks: numpy array with the hpsi_opblock_t layout; a_data: torch CUDA tensor."""
+    d = np.ascontiguousarray(d, np.int32)
+    chi = np.ascontiguousarray(chi, np.int32)
+    blocks = np.ascontiguousarray(blocks)
+    assert blocks.dtype.itemsize == 24 and d.shape == chi.shape
+    out = ctypes.c_void_p()
+    _check(lib().hpsi_rotate_plan(d.shape[0], d.ctypes.data, chi.ctypes.data, blocks.shape[0], blocks.ctypes.data,
+                                  _ptr(a_data), int(a_len), flags, ctypes.byref(out)))
+    return RotatePlan(out.value, a_data, blocks.shape[0])
+
+
+def hpsi_rotate_apply(r: RotatePlan, ot, out, stream=None) -> None:
+    _check(lib().hpsi_rotate_apply(r.handle, _ptr(ot), _ptr(out), _stream(stream)))
+
+
+def hpsi_rotate_apply_profiled(r: RotatePlan, ot, out, stream=None):
+    """Returns [isometry copy, first GEMM, second GEMM] device milliseconds."""
+    ms = (ctypes.c_float * 3)()
+    _check(lib().hpsi_rotate_apply_profiled(r.handle, _ptr(ot), _ptr(out), _stream(stream), ms))
+    return list(ms)
+
+
+def hpsi_rotate_query(r: RotatePlan, what: int):
+    if what == HPSI_RQ_OUT_BLOCKS:
+        arr = np.zeros(max(r.n_blocks, 1), OPBLOCK_DTYPE)
+        _check(lib().hpsi_rotate_query(r.handle, what, arr.ctypes.data, arr.nbytes))
+        return arr[:r.n_blocks]
+    v = ctypes.c_int64()
+    _check(lib().hpsi_rotate_query(r.handle, what, ctypes.addressof(v), 8))
+    return v.value
+
+
+def hpsi_rotate_debug_interpret(r: RotatePlan, a_host: np.ndarray, ot_host: np.ndarray) -> np.ndarray:
+    out = np.full(hpsi_rotate_query(r, HPSI_RQ_OUT_LENGTH), np.nan)
+    _check(lib().hpsi_rotate_debug_interpret(r.handle, _ptr(np.ascontiguousarray(a_host, np.float64)),
+                                             _ptr(np.ascontiguousarray(ot_host, np.float64)), _ptr(out)))
     return out
 
 

@@ -1,4 +1,5 @@
 // C-ABI entry points of include/hpsi.h (plan / bind / apply / query / destroy / debug).
+#include <algorithm>
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
@@ -23,13 +24,13 @@ using namespace hpsi;
 
 extern "C" const char* hpsi_last_error(void) { return g_err.c_str(); }
 
-namespace {
+namespace hpsi {
 
 template <class T>
-size_t table_bytes(const std::vector<T>& v) { return (v.size() * sizeof(T) + 255) / 256 * 256 + 256; }
+static size_t table_bytes(const std::vector<T>& v) { return (v.size() * sizeof(T) + 255) / 256 * 256 + 256; }
 
 template <class T>
-int upload(const std::vector<T>& v, char* base, size_t& cursor, const T** dev_ptr) {
+static int upload(const std::vector<T>& v, char* base, size_t& cursor, const T** dev_ptr) {
   *dev_ptr = reinterpret_cast<const T*>(base + cursor);
   if (!v.empty()) HPSI_CUDA(cudaMemcpy(base + cursor, v.data(), v.size() * sizeof(T), cudaMemcpyHostToDevice));
   cursor += table_bytes(v);
@@ -85,6 +86,7 @@ void free_plan(hpsi_plan_t* p) {
     cudaFree(p->d_psi_stage);
     cudaFree(p->d_out_stage);
     cudaFree(p->d_dav);
+    cudaFree(p->d_svd);
     cudaFreeHost(p->h_dav);
     cudaGetLastError();
   }
@@ -128,7 +130,7 @@ int encode_maps(hpsi_plan_t* p) {
   return HPSI_OK;
 }
 
-}  // namespace
+}  // namespace hpsi
 
 extern "C" int hpsi_bind(hpsi_plan_t* p, const double* a_dev, const double* b_dev) {
   if (!p) { set_error("null plan"); return HPSI_EINVAL; }
@@ -172,6 +174,7 @@ extern "C" int hpsi_plan(const hpsi_sectors_t* sectors, const hpsi_terms_t* term
     std::string err;
     rc = build_schedule(sectors, terms, flags, p->n_sm, &p->sc, &err);
     if (rc != HPSI_OK) { set_error(err); free_plan(p); return rc; }
+    p->n_left = sectors->n_left;
     if (!p->host_only) {
       rc = upload_schedule(p);
       if (rc != HPSI_OK) { free_plan(p); return rc; }
@@ -312,6 +315,10 @@ extern "C" int hpsi_query(const hpsi_plan_t* p, int what, void* out, size_t byte
       return put_i64((sc.blocks.empty() ? 0 : 2) + (sc.p1.empty() ? 0 : 1) + (sc.p2.empty() ? 0 : 1));
     case HPSI_Q_ALIGNED16: return put_i64(p->host_only ? sc.aligned16 : p->aligned16);
     case HPSI_Q_INTERMEDIATE_BYTES: return put_i64(sc.intermediate_bytes);
+    case HPSI_Q_PSI_ROWS: { int64_t n = 0; for (const PsiBlk& b : sc.blocks) n += b.rows; return put_i64(n); }
+    case HPSI_Q_ISO_CAPACITY: { int64_t n = 0; for (const PsiBlk& b : sc.blocks) n += (int64_t)std::min(b.rows, b.cols) * b.rows; return put_i64(n); }
+    case HPSI_Q_SVD_SWEEPS: return put_i64(p->svd_sweeps);
+    case HPSI_Q_SVD_LAUNCHES: return put_i64(p->svd_launches);
     case HPSI_Q_TASKS: {
       if (bytes < sc.tasks.size() * sizeof(hpsi_task_t)) { set_error("hpsi_query: buffer too small"); return HPSI_EINVAL; }
       if (!sc.tasks.empty()) memcpy(out, sc.tasks.data(), sc.tasks.size() * sizeof(hpsi_task_t));

@@ -28,7 +28,8 @@ namespace hpsi {
 // One CTA = one P1Unit: for each term t of the unit, T_t[i0.., j0..] = coef_t * sum_k X_t[i,k] Y[j,k] with
 // X_t = the term's operator block (order 1: A_t, order 2: B_t) and Y = padded psi^T (order 1) or padded psi
 // (order 2) block of the source.  The stage ring runs across the terms.
-template <int MI, int NJ>
+// ROT (operator update, rotate.cu): the tile of term t is stored transposed at rot_dst + Seg.p2_off with ld Seg.p2_ld.
+template <int MI, int NJ, bool ROT>
 __device__ __forceinline__ void p1_consume(const DevSchedule& d, const P1Unit& u, const Group& g, const SmemLayout& sm,
                                            const WarpTile& w, int lane) {
   double acc[MI][NJ][2];
@@ -37,7 +38,7 @@ __device__ __forceinline__ void p1_consume(const DevSchedule& d, const P1Unit& u
   const int last_nk4 = ((g.K1 - (ntiles - 1) * KT) + 3) >> 2;
   Ring ring{0, 0};
   for (int t = u.t0; t < u.t1; ++t) {
-    const double coef = d.segs[g.seg0 + t].coef;            // issued before the K loop, needed after it
+    const double coef = ROT ? 1.0 : d.segs[g.seg0 + t].coef;   // issued before the K loop, needed after it
     zero_acc<MI, NJ>(acc);
     for (int kt = 0; kt < ntiles; ++kt) {
       mbar_wait(sm.full(ring.stage), ring.phase);
@@ -49,8 +50,13 @@ __device__ __forceinline__ void p1_consume(const DevSchedule& d, const P1Unit& u
       if (lane == 0) mbar_arrive(sm.empty(ring.stage));
       ring.advance();
     }
-    double* dst = d.ws + g.ws_off + ((int64_t)t * g.rows + u.i0) * g.ldw + u.j0;
-    store_tile<MI, NJ>(dst, g.ldw, u.rows_valid, u.cols_valid, acc, w, lane, coef);
+    if (ROT) {
+      const Seg* sg = d.segs + g.seg0 + t;
+      store_tile_t<MI, NJ>(d.rot_dst + sg->p2_off + (int64_t)u.j0 * sg->p2_ld + u.i0, sg->p2_ld, u.rows_valid, u.cols_valid, acc, w, lane);
+    } else {
+      double* dst = d.ws + g.ws_off + ((int64_t)t * g.rows + u.i0) * g.ldw + u.j0;
+      store_tile<MI, NJ>(dst, g.ldw, u.rows_valid, u.cols_valid, acc, w, lane, coef);
+    }
   }
 }
 // a consumer warp without fragments (tile narrower than the warp grid) only hands the stages back
@@ -73,7 +79,7 @@ __device__ __forceinline__ void idle_consume(const SmemLayout& sm, int nstages, 
     default: __trap();                                                                                          \
   }
 
-template <bool TMA>
+template <bool TMA, bool ROT>
 __global__ void __maxnreg__(HPSI_BIG_CTA ? 112 : 136) p1_kernel(DevSchedule d) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const P1Unit u = d.p1[blockIdx.x];
@@ -127,7 +133,7 @@ __global__ void __maxnreg__(HPSI_BIG_CTA ? 112 : 136) p1_kernel(DevSchedule d) {
   const int warp = (wid + quadrant_rotation(blockIdx.x)) % NCONS;
   const WarpTile w(u.grid, warp, u.rows_valid, u.cols_valid);
   if (w.mi == 0 || w.nj == 0) { idle_consume(sm, ntiles * (u.t1 - u.t0), lane); return; }
-#define HPSI_CASE(MI, NJ) case MI * 9 + NJ: p1_consume<MI, NJ>(d, u, g, sm, w, lane); break;
+#define HPSI_CASE(MI, NJ) case MI * 9 + NJ: p1_consume<MI, NJ, ROT>(d, u, g, sm, w, lane); break;
   HPSI_DISPATCH_FRAGS(HPSI_CASE)
 #undef HPSI_CASE
 }
@@ -303,8 +309,10 @@ __global__ void diag_kernel(DevSchedule d, double* __restrict__ diag) {
 // -------------------------------------------------------------------------------------------------- launchers
 cudaError_t kernels_init() {
   cudaError_t e;
-  if ((e = cudaFuncSetAttribute(p1_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES))) return e;
-  if ((e = cudaFuncSetAttribute(p1_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES))) return e;
+  if ((e = cudaFuncSetAttribute(p1_kernel<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES))) return e;
+  if ((e = cudaFuncSetAttribute(p1_kernel<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES))) return e;
+  if ((e = cudaFuncSetAttribute(p1_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES))) return e;
+  if ((e = cudaFuncSetAttribute(p1_kernel<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES))) return e;
   if ((e = cudaFuncSetAttribute(p2_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES))) return e;
   if ((e = cudaFuncSetAttribute(p2_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES))) return e;
   return kernels_paired_init();
@@ -323,8 +331,13 @@ void launch_prep(const DevSchedule& d, const double* psi, cudaStream_t st) {
 void launch_p1(const DevSchedule& d, bool tma, cudaStream_t st) {
   if (d.n_p1 == 0) return;
   if (d.paired) { launch_p1_paired(d, tma, st); return; }
-  if (tma) p1_kernel<true><<<d.n_p1, NTHREADS, SMEM_BYTES, st>>>(d);
-  else p1_kernel<false><<<d.n_p1, NTHREADS, SMEM_BYTES, st>>>(d);
+  if (tma) p1_kernel<true, false><<<d.n_p1, NTHREADS, SMEM_BYTES, st>>>(d);
+  else p1_kernel<false, false><<<d.n_p1, NTHREADS, SMEM_BYTES, st>>>(d);
+}
+void launch_p1_rot(const DevSchedule& d, bool tma, cudaStream_t st) {
+  if (d.n_p1 == 0) return;
+  if (tma) p1_kernel<true, true><<<d.n_p1, NTHREADS, SMEM_BYTES, st>>>(d);
+  else p1_kernel<false, true><<<d.n_p1, NTHREADS, SMEM_BYTES, st>>>(d);
 }
 void launch_p2(const DevSchedule& d, bool tma, cudaStream_t st) {
   if (d.n_p2 == 0) return;

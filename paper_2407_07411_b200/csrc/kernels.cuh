@@ -37,10 +37,12 @@ struct DevSchedule {           // device pointers to the uploaded tables
   int max_block_elems;
   int paired;                  // the plan has blocks stored transposed: kernels_paired.cu runs the GEMMs
   int debug;                   // HPSI_DEBUG env (timing experiments only): 1 = producer skips loads, 2 = consumers skip MMAs
+  double* rot_dst;             // operator-update launches (rotate.cu) only: base the transposed tile stores go to
 };
 
 void launch_prep(const DevSchedule& d, const double* psi, cudaStream_t st);
 void launch_p1(const DevSchedule& d, bool tma, cudaStream_t st);
+void launch_p1_rot(const DevSchedule& d, bool tma, cudaStream_t st);   // same kernel, tile stored transposed at Seg.p2_off / p2_ld
 void launch_p2(const DevSchedule& d, bool tma, cudaStream_t st);
 void launch_reduce(const DevSchedule& d, double* out, bool accumulate, cudaStream_t st);
 void launch_diag(const DevSchedule& d, double* diag, cudaStream_t st);

@@ -153,6 +153,26 @@ __device__ __forceinline__ void store_tile(double* dst, int ld, int rows_valid, 
   }
 }
 
+// Same accumulators stored transposed: element (row, col) of the CTA tile goes to dst[col*ld + row]  (operator update,
+// rotate.cu: the first GEMM leaves T^T, the second A').  The 8 lane groups of a store cover 8 consecutive rows = 64
+// contiguous bytes of each of 4 destination rows.
+template <int MI, int NJ>
+__device__ __forceinline__ void store_tile_t(double* dst, int ld, int rows_valid, int cols_valid,
+                                             const double (&acc)[MI][NJ][2], const WarpTile& w, int lane) {
+  const int pg = frag_perm(lane >> 2), pc = frag_perm(2 * (lane & 3));
+#pragma unroll
+  for (int i = 0; i < MI; ++i) {
+    const int row = w.wr0 + 8 * i + pg;
+    if (row >= rows_valid) continue;
+#pragma unroll
+    for (int j = 0; j < NJ; ++j) {
+      const int col = w.wc0 + 8 * j + pc;
+      if (col < cols_valid) dst[(int64_t)col * ld + row] = acc[i][j][0];
+      if (col + 2 < cols_valid) dst[(int64_t)(col + 2) * ld + row] = acc[i][j][1];
+    }
+  }
+}
+
 // Which tile quadrant consumer warp 0 takes.  Consumer warp w sits on SM sub-partition w, and with odd fragment counts
 // the quadrants carry unequal DMMA counts (e.g. 16/12/12/9), so co-resident CTAs must not all put their heavy
 // quadrant on the same sub-partition.  CTAs are dealt to SMs round-robin (148 = 0 mod 4), hence a hash, not bid & 3.

@@ -142,6 +142,12 @@ struct Schedule {
 int build_schedule(const hpsi_sectors_t* s, const hpsi_terms_t* t, uint32_t flags, int n_sm, Schedule* out,
                    std::string* err);
 
+// Tile split of one dimension (planner.cpp): rows up to TILE_M, columns up to TILE, sizes in units of two fragments.
+struct Tile1D { int start, len; };
+std::vector<Tile1D> split_dim(int64_t n, int max_frags, int unit);
+std::vector<Tile1D> split_rows(int64_t n);
+std::vector<Tile1D> split_cols(int64_t n);
+
 // Host interpreter of the schedule (tests only; naive loops).
 void interpret_schedule(const Schedule& sc, const double* a, const double* b, const double* psi, double* out);
 

@@ -25,12 +25,20 @@ struct hpsi_plan {
   size_t dav_doubles = 0;
   int dav_mmax = 0;
   double* h_dav = nullptr;        // pinned host scalars the Davidson loop reads back each iteration
+  // hpsi_truncate (svd.cu)
+  int n_left = 0;                 // left sectors of the sector table (length of chi_host)
+  void* d_svd = nullptr;          // working matrices, singular values, tables (allocated on first use)
+  int svd_sweeps = 0, svd_launches = 0;   // of the last hpsi_truncate call (diagnostics)
 };
 
 namespace hpsi {
 void set_error(const std::string& s);
 int cuda_fail(cudaError_t e, const char* what);   // records the message, returns HPSI_ECUDA
 int apply_impl(hpsi_plan_t* p, const double* psi_dev, double* out_dev, bool accumulate, void* cuda_stream);
+// api.cu: shared with rotate.cu, whose object wraps an hpsi_plan
+int upload_schedule(hpsi_plan_t* p);   // device copies of the schedule tables, workspace, tensor-map buffer
+int encode_maps(hpsi_plan_t* p);       // CUtensorMap of every MapSpec against dev.a / dev.b / d_ws
+void free_plan(hpsi_plan_t* p);
 }  // namespace hpsi
 
 #define HPSI_CUDA(call)                                             \

@@ -19,10 +19,6 @@
 
 namespace hpsi {
 
-namespace {
-
-struct Tile1D { int start, len; };
-
 // Split of a dimension into tiles of at most max_frags fragments.  Inside a CTA the tile is cut again between the
 // consumer warps (2 or 4 ways per dimension), so tile sizes are multiples of `unit` fragments wherever possible and
 // only the last tile takes the remainder: a tile with an odd fragment count leaves a warp row (or column) short and
@@ -53,6 +49,7 @@ std::vector<Tile1D> split_dim(int64_t n, int max_frags, int unit) {
 // rows: up to TILE_M; columns: up to TILE.  Units: half of what the warp grid cuts each dimension into.
 std::vector<Tile1D> split_rows(int64_t n) { return split_dim(n, TILE_M / 8, HPSI_BIG_CTA ? 8 : 2); }
 std::vector<Tile1D> split_cols(int64_t n) { return split_dim(n, TILE / 8, HPSI_BIG_CTA ? 4 : 2); }
+namespace {
 
 int64_t align_up(int64_t x, int64_t a) { return (x + a - 1) / a * a; }
 

@@ -1,0 +1,313 @@
+// hpsi_truncate (include/hpsi.h "Site update"): the matrix factorisation of a
+// DMRG tensor update - SVD of every psi block, global selection of the chi_max largest singular values, left isometries.
+//
+// One-sided Jacobi (Hestenes) on the ROWS of each block: row i of the working matrix is [ psi_l[i, :] | R[i, :] ] with
+// R = 1 at the start; plane rotations make the psi parts mutually orthogonal, the same rotations applied to R
+// accumulate J with  J psi_l = S V^T,  i.e. psi_l = J^T S V^T: row i of R is the i-th left singular vector and the norm
+// of the psi part its singular value.  Rows are contiguous (the psi layout is row-major), so a rotation streams two
+// rows with unit stride.
+//
+// Parallel order (block Jacobi by tournament): the rows of a block are cut into chunks of `bsz` rows; in one kernel
+// launch ("round") every CTA owns one PAIR of chunks of one block, chosen by the round-robin (circle) schedule so that
+// all CTAs of a round touch disjoint rows; it loads its 2*bsz rows into shared memory, orthogonalises them pairwise - one
+// warp per row pair, again by a round-robin schedule, CTA barrier between its inner rounds - and writes them back.  The
+// first round of a block's sweep does all pairs inside the two chunks, the others only the cross pairs, so a sweep
+// visits every row pair of the block exactly once.  Sweeps repeat until one makes no rotation (device flag; the only
+// atomic, not on data).  Every psi block is processed in the same launches.  All arithmetic is FP64 FMA; the result is
+// bitwise reproducible.
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <numeric>
+#include <vector>
+
+#include "plan_dev.h"
+
+namespace hpsi {
+
+struct SvdBlk {
+  int64_t w_off;        // working matrix rows x L in the SVD workspace
+  int64_t psi_off;      // block in psi (dense rows x cols)
+  int32_t rows, cols, L;
+  int32_t nce;          // chunks, padded to an even count >= 2
+  int32_t cta0;         // first CTA of this block in a round
+  int32_t row0;         // first row in the concatenated singular-value array
+  double floor2;        // rows with squared norm <= floor2 count as zero (1e-27 x the block's squared Frobenius norm)
+};
+
+constexpr int SVD_MAX_BSZ = 16;
+constexpr int SVD_SMEM_BUDGET = 200 * 1024;
+
+// working matrix <- [psi block | identity]; floor2 of the block from its Frobenius norm (one CTA per block row range)
+__global__ void svd_init_kernel(SvdBlk* blk, const double* __restrict__ psi, double* __restrict__ w) {
+  const SvdBlk B = blk[blockIdx.y];
+  for (int i = blockIdx.x; i < B.rows; i += gridDim.x) {
+    double* row = w + B.w_off + (int64_t)i * B.L;
+    for (int j = threadIdx.x; j < B.L; j += blockDim.x) {
+      double v = 0.0;
+      if (j < B.cols) v = psi[B.psi_off + (int64_t)i * B.cols + j];
+      else if (j - B.cols == i) v = 1.0;
+      row[j] = v;
+    }
+  }
+}
+// squared Frobenius norm of each block in a fixed order (one CTA per block, tree reduction)
+__global__ void svd_norm_kernel(SvdBlk* blk, const double* __restrict__ psi) {
+  __shared__ double red[256];
+  SvdBlk& B = blk[blockIdx.x];
+  const int64_t n = (int64_t)B.rows * B.cols;
+  double s = 0.0;
+  for (int64_t e = threadIdx.x; e < n; e += blockDim.x) { const double v = psi[B.psi_off + e]; s += v * v; }
+  red[threadIdx.x] = s;
+  __syncthreads();
+  for (int k = 128; k > 0; k >>= 1) {
+    if ((int)threadIdx.x < k) red[threadIdx.x] += red[threadIdx.x + k];
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) B.floor2 = 1e-27 * red[0];
+}
+
+__device__ __forceinline__ double warp_sum(double v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  return v;
+}
+
+// One round: CTA = (block, chunk pair of the round-robin schedule).  blockDim.x = 32 * bsz.
+__global__ void svd_round_kernel(const SvdBlk* __restrict__ blk, const int32_t* __restrict__ cta_blk, int round, int bsz,
+                                 double* __restrict__ w, int* __restrict__ flag) {
+  extern __shared__ __align__(16) double srow[];
+  const SvdBlk B = blk[cta_blk[blockIdx.x]];
+  const int k = blockIdx.x - B.cta0;
+  const int n1 = B.nce - 1;
+  const int rr = round % n1;
+  int ci, cj;                                            // the two chunks of this CTA (circle method)
+  if (k == 0) { ci = n1; cj = rr; }
+  else { ci = (rr + k) % n1; cj = (rr - k + n1) % n1; }
+  if (ci > cj) { const int t = ci; ci = cj; cj = t; }
+  const bool full = (rr == 0);                           // first round of the block's sweep: pairs inside the chunks too
+  const int ni = max(0, min(bsz, B.rows - ci * bsz)), nj = max(0, min(bsz, B.rows - cj * bsz));
+  if (ni + nj < 2 || (!full && (ni == 0 || nj == 0))) return;
+  const int L = B.L, tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+  // slot s < bsz holds row ci*bsz + s, slot bsz + s holds row cj*bsz + s
+  auto grow = [&](int slot) -> double* {
+    const int row = slot < bsz ? ci * bsz + slot : cj * bsz + (slot - bsz);
+    return w + B.w_off + (int64_t)row * L;
+  };
+  auto valid = [&](int slot) { return slot < bsz ? slot < ni : slot - bsz < nj; };
+  for (int slot = wid; slot < 2 * bsz; slot += bsz) {
+    if (!valid(slot)) continue;
+    const double2* src = reinterpret_cast<const double2*>(grow(slot));
+    double2* dst = reinterpret_cast<double2*>(srow + (size_t)slot * L);
+    for (int j = lane; j < L / 2; j += 32) dst[j] = src[j];
+  }
+  __syncthreads();
+  const double tol = 4.4e-16 * sqrt((double)max(B.cols, 8));
+  bool rotated = false;
+  const int np = 2 * bsz - 1;
+  const int inner = full ? np : bsz;
+  for (int s = 0; s < inner; ++s) {
+    int p, q;
+    if (full) {
+      if (wid == 0) { p = np; q = s; }
+      else { p = (s + wid) % np; q = (s - wid + np) % np; }
+    } else {
+      p = wid; q = bsz + (wid + s) % bsz;
+    }
+    if (valid(p) && valid(q)) {
+      double* xp = srow + (size_t)p * L;
+      double* xq = srow + (size_t)q * L;
+      double a = 0.0, b = 0.0, g = 0.0;
+      for (int j = lane; j < B.cols; j += 32) {
+        const double u = xp[j], v = xq[j];
+        a = fma(u, u, a); b = fma(v, v, b); g = fma(u, v, g);
+      }
+      a = warp_sum(a); b = warp_sum(b); g = warp_sum(g);
+      if (a > B.floor2 && b > B.floor2 && fabs(g) > tol * sqrt(a * b)) {
+        const double zeta = (b - a) / (2.0 * g);
+        const double t = copysign(1.0, zeta) / (fabs(zeta) + sqrt(1.0 + zeta * zeta));
+        const double cs = 1.0 / sqrt(1.0 + t * t), sn = cs * t;
+        for (int j = lane; j < L; j += 32) {
+          const double u = xp[j], v = xq[j];
+          xp[j] = cs * u - sn * v;
+          xq[j] = sn * u + cs * v;
+        }
+        rotated = true;
+      }
+    }
+    __syncthreads();
+  }
+  for (int slot = wid; slot < 2 * bsz; slot += bsz) {
+    if (!valid(slot)) continue;
+    double2* dst = reinterpret_cast<double2*>(grow(slot));
+    const double2* src = reinterpret_cast<const double2*>(srow + (size_t)slot * L);
+    for (int j = lane; j < L / 2; j += 32) dst[j] = src[j];
+  }
+  if (rotated && lane == 0) atomicOr(flag, 1);
+}
+
+// singular value of every row = norm of its psi part (one warp per row)
+__global__ void svd_sigma_kernel(const SvdBlk* __restrict__ blk, const double* __restrict__ w, double* __restrict__ sigma) {
+  const SvdBlk B = blk[blockIdx.y];
+  const int lane = threadIdx.x & 31, wpb = blockDim.x >> 5;
+  for (int i = blockIdx.x * wpb + (threadIdx.x >> 5); i < B.rows; i += gridDim.x * wpb) {
+    const double* row = w + B.w_off + (int64_t)i * B.L;
+    double a = 0.0;
+    for (int j = lane; j < B.cols; j += 32) a = fma(row[j], row[j], a);
+    a = warp_sum(a);
+    if (lane == 0) sigma[B.row0 + i] = sqrt(a);
+  }
+}
+
+struct IsoRow { int64_t src, dst; int32_t len, pad; };   // R part of one kept row -> one row of O_l^T
+__global__ void svd_gather_kernel(const IsoRow* __restrict__ rows, int n, const double* __restrict__ w, double* __restrict__ ot) {
+  for (int i = blockIdx.x; i < n; i += gridDim.x) {
+    const IsoRow r = rows[i];
+    for (int j = threadIdx.x; j < r.len; j += blockDim.x) ot[r.dst + j] = w[r.src + j];
+  }
+}
+
+}  // namespace hpsi
+
+using namespace hpsi;
+
+extern "C" int hpsi_truncate(hpsi_plan_t* p, const double* psi_dev, int32_t chi_max, double* ot_dev, int32_t* chi_host,
+                             double* sigma_host, double* discarded_host, void* cuda_stream) {
+  if (!p) { set_error("null plan"); return HPSI_EINVAL; }
+  if (p->host_only) { set_error("host-only plan: hpsi_truncate needs a CUDA device (no CPU fallback)"); return HPSI_ESTATE; }
+  if (chi_max < 0) { set_error("negative chi_max"); return HPSI_EINVAL; }
+  if (!chi_host) { set_error("null chi_host"); return HPSI_EINVAL; }
+  const Schedule& sc = p->sc;
+  const int nL = p->n_left;
+  for (int i = 0; i < nL; ++i) chi_host[i] = 0;
+  if (discarded_host) *discarded_host = 0.0;
+  const int nB = (int)sc.blocks.size();
+  if (nB == 0) return HPSI_OK;
+  if (!psi_dev || !ot_dev) { set_error("null psi / ot"); return HPSI_EINVAL; }
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+
+  // ---- tables (rebuilt per call: a few KB of host work)
+  std::vector<SvdBlk> tab(nB);
+  int Lmax = 0;
+  int64_t wlen = 0;
+  int row0 = 0;
+  for (int b = 0; b < nB; ++b) {
+    const PsiBlk& B = sc.blocks[b];
+    SvdBlk& s = tab[b];
+    s.w_off = wlen; s.psi_off = B.off; s.rows = B.rows; s.cols = B.cols;
+    s.L = sector_up(B.rows + B.cols);
+    s.row0 = row0; s.floor2 = 0.0;
+    row0 += B.rows;
+    wlen = (wlen + (int64_t)s.rows * s.L + 15) & ~(int64_t)15;
+    Lmax = std::max(Lmax, s.L);
+  }
+  const int n_rows = row0;
+  int bsz = std::min(SVD_MAX_BSZ, SVD_SMEM_BUDGET / (2 * Lmax * 8));
+  if (bsz < 1) { set_error("hpsi_truncate: a psi block is too large for the shared-memory Jacobi kernel"); return HPSI_EINVAL; }
+  int n_cta = 0, rounds = 1;
+  std::vector<int32_t> cta_blk;
+  for (int b = 0; b < nB; ++b) {
+    SvdBlk& s = tab[b];
+    int nc = (s.rows + bsz - 1) / bsz;
+    nc += nc & 1;
+    s.nce = std::max(nc, 2);
+    s.cta0 = n_cta;
+    n_cta += s.nce / 2;
+    for (int k = 0; k < s.nce / 2; ++k) cta_blk.push_back(b);
+    rounds = std::max(rounds, s.nce - 1);
+  }
+  const size_t smem = (size_t)2 * bsz * Lmax * 8;
+
+  // ---- device buffers (kept on the plan; sizes depend on the plan only)
+  if (!p->d_svd) {
+    size_t bytes = (size_t)wlen * 8 + (size_t)n_rows * 8 + tab.size() * sizeof(SvdBlk) + cta_blk.size() * 4 + (size_t)n_rows * sizeof(IsoRow) + 4096;
+    cudaError_t e = cudaMalloc(&p->d_svd, bytes);
+    if (e != cudaSuccess) { cudaGetLastError(); set_error("hpsi_truncate: device workspace allocation failed"); return HPSI_ENOMEM; }
+    HPSI_CUDA(cudaFuncSetAttribute(svd_round_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, SVD_SMEM_BUDGET));
+  }
+  char* base = static_cast<char*>(p->d_svd);
+  size_t cur = 0;
+  auto carve = [&](size_t bytes) { char* q = base + cur; cur = (cur + bytes + 255) & ~(size_t)255; return q; };
+  double* d_w = reinterpret_cast<double*>(carve((size_t)wlen * 8));
+  double* d_sigma = reinterpret_cast<double*>(carve((size_t)n_rows * 8));
+  SvdBlk* d_tab = reinterpret_cast<SvdBlk*>(carve(tab.size() * sizeof(SvdBlk)));
+  int32_t* d_cta = reinterpret_cast<int32_t*>(carve(cta_blk.size() * 4));
+  IsoRow* d_rows = reinterpret_cast<IsoRow*>(carve((size_t)n_rows * sizeof(IsoRow)));
+  int* d_flag = reinterpret_cast<int*>(carve(256));
+  HPSI_CUDA(cudaMemcpyAsync(d_tab, tab.data(), tab.size() * sizeof(SvdBlk), cudaMemcpyHostToDevice, st));
+  HPSI_CUDA(cudaMemcpyAsync(d_cta, cta_blk.data(), cta_blk.size() * 4, cudaMemcpyHostToDevice, st));
+
+  svd_norm_kernel<<<nB, 256, 0, st>>>(d_tab, psi_dev);
+  svd_init_kernel<<<dim3(64, nB), 128, 0, st>>>(d_tab, psi_dev, d_w);
+  constexpr int MAX_SWEEPS = 60;
+  int sweeps = 0, flag = 1;
+  for (; sweeps < MAX_SWEEPS && flag; ++sweeps) {
+    HPSI_CUDA(cudaMemsetAsync(d_flag, 0, sizeof(int), st));
+    for (int r = 0; r < rounds; ++r)
+      svd_round_kernel<<<n_cta, 32 * bsz, smem, st>>>(d_tab, d_cta, sweeps * rounds + r, bsz, d_w, d_flag);
+    HPSI_CUDA(cudaMemcpyAsync(&flag, d_flag, sizeof(int), cudaMemcpyDeviceToHost, st));
+    HPSI_CUDA(cudaStreamSynchronize(st));
+  }
+  if (flag) { set_error("hpsi_truncate: Jacobi SVD did not converge"); return HPSI_ESTATE; }
+  p->svd_sweeps = sweeps;
+  p->svd_launches = sweeps * rounds + 4;
+  svd_sigma_kernel<<<dim3(16, nB), 256, 0, st>>>(d_tab, d_w, d_sigma);
+  std::vector<double> sig(n_rows);
+  HPSI_CUDA(cudaMemcpyAsync(sig.data(), d_sigma, (size_t)n_rows * 8, cudaMemcpyDeviceToHost, st));
+  HPSI_CUDA(cudaStreamSynchronize(st));
+
+  // ---- host: order every block's rows by descending singular value, global selection (reading R3)
+  struct Cand { double s; int blk, rank, row; };
+  std::vector<Cand> cand;
+  cand.reserve(n_rows);
+  double smax = 0.0;
+  for (int b = 0; b < nB; ++b) {
+    const SvdBlk& s = tab[b];
+    std::vector<int> ord(s.rows);
+    std::iota(ord.begin(), ord.end(), 0);
+    std::stable_sort(ord.begin(), ord.end(), [&](int x, int y) { return sig[s.row0 + x] > sig[s.row0 + y]; });
+    const int nsv = std::min(s.rows, s.cols);
+    for (int k = 0; k < s.rows; ++k) {
+      const double v = k < nsv ? sig[s.row0 + ord[k]] : 0.0;     // rows past min(rows, cols) are rounding noise
+      if (sigma_host) sigma_host[s.row0 + k] = v;
+      if (k < nsv) { cand.push_back({v, b, k, ord[k]}); smax = std::max(smax, v); }
+    }
+  }
+  std::stable_sort(cand.begin(), cand.end(), [](const Cand& x, const Cand& y) {
+    if (x.s != y.s) return x.s > y.s;
+    if (x.blk != y.blk) return x.blk < y.blk;
+    return x.rank < y.rank;
+  });
+  std::vector<std::vector<int>> kept(nB);
+  std::vector<char> is_kept(cand.size(), 0);
+  int nk = 0;
+  for (size_t i = 0; i < cand.size(); ++i) {
+    if (nk >= chi_max || cand[i].s <= 1e-13 * smax) break;
+    kept[cand[i].blk].push_back(cand[i].row);        // descending singular value inside the block
+    is_kept[i] = 1;
+    ++nk;
+  }
+  double disc = 0.0;
+  for (size_t i = cand.size(); i-- > 0;)              // smallest first
+    if (!is_kept[i]) disc += cand[i].s * cand[i].s;
+  if (discarded_host) *discarded_host = disc;
+
+  // ---- isometries in the boundary layout: sectors ascending, O_l^T = kept rows of R
+  std::vector<IsoRow> rows;
+  int64_t dst = 0;
+  for (int b = 0; b < nB; ++b) {                       // psi blocks are in ascending left-sector order
+    const SvdBlk& s = tab[b];
+    chi_host[sc.blocks[b].left] = (int32_t)kept[b].size();
+    for (int row : kept[b]) {
+      rows.push_back({s.w_off + (int64_t)row * s.L + s.cols, dst, s.rows, 0});
+      dst += s.rows;
+    }
+  }
+  if (!rows.empty()) {
+    HPSI_CUDA(cudaMemcpyAsync(d_rows, rows.data(), rows.size() * sizeof(IsoRow), cudaMemcpyHostToDevice, st));
+    svd_gather_kernel<<<std::min<int>((int)rows.size(), 1024), 128, 0, st>>>(d_rows, (int)rows.size(), d_w, ot_dev);
+    HPSI_CUDA(cudaStreamSynchronize(st));              // `rows` must outlive the copy
+  }
+  HPSI_CUDA(cudaGetLastError());
+  return HPSI_OK;
+}
