@@ -155,7 +155,7 @@ def test_truncate_cyp_sized_blocks_and_reproducible():
 
 def test_truncate_rank_deficient_wide_tall_and_single_row():
     # block 0: 5 x 2 (tall: three zero singular directions), block 1: 1 x 4 (single row), block 2: 3 x 6 of rank 1
-    p = workloads.custom_problem([(0, 0), (1, 0), (2, 0), (9, 9)], [5, 1, 3, 2], [(2, 0), (1, 0), (0, 0)], [6, 4, 2], (2, 0), [])
+    p = workloads.custom_problem([(0, 0), (1, 0), (2, 0), (9, 9)], [5, 1, 3, 2], [(2, 0), (1, 0), (0, 0)], [2, 4, 6], (2, 0), [])
     assert [(r, c) for (_, _, r, c, _) in p.psi_blocks()] == [(5, 2), (1, 4), (3, 6)]
     rng = np.random.default_rng(41)
     parts = [rng.standard_normal((5, 2)), rng.standard_normal((1, 4)), np.outer(rng.standard_normal(3), rng.standard_normal(6))]
