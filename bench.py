@@ -238,6 +238,136 @@ def run_streamed(args):
     }), flush=True)
 
 
+# -------------------------------------------------------------------------- site update
+def run_site_update(args):
+    """bench.py --site-update: the two steps after the eigen-solve on the named config - hpsi_truncate (block Jacobi
+    SVD of psi, chi_max = D/4: the enlarged basis carries the site dimension 4) and hpsi_rotate_apply
+    (A' = O^T A O for every left operator block).  A step = one truncation + one operator update.  The update's
+    roofline is the FP64 tensor pipe when its flops per operator byte exceed the ridge (same-run DGEMM / HBM copy
+    bandwidth), HBM otherwise; reported beside the H_eff*psi line, not the headline."""
+    import torch
+    import paper_2407_07411_b200 as H
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the product has no CPU fallback)")
+    torch.cuda.set_device(0)
+    cfg = args.config
+    p = workloads.make_problem(cfg)
+    a = torch.from_numpy(p.a_data).cuda()
+    b = torch.zeros(8, dtype=torch.float64, device="cuda")       # the right operators play no part here
+    p_plan = workloads.make_problem(cfg, n_terms=2)               # psi block table only (sector table is the config's)
+    pa, pb = torch.from_numpy(p_plan.a_data).cuda(), torch.from_numpy(p_plan.b_data).cuda()
+    plan = H.plan_problem(p_plan, pa, pb)
+    D = int(p.d_left.sum())
+    chi_max = max(1, D // 4)
+    psi_h = workloads.make_psi(p)
+    psi = torch.from_numpy(psi_h).cuda()
+    ot = torch.zeros(H.hpsi_query(plan, H.HPSI_Q_ISO_CAPACITY), dtype=torch.float64, device="cuda")
+    stream = torch.cuda.current_stream()
+    chi, sigma, disc = H.hpsi_truncate(plan, psi, chi_max, ot, stream)
+    rot = H.hpsi_rotate_plan(p.d_left, chi, p.a_desc, a, p.a_len)
+    rq = lambda w: H.hpsi_rotate_query(rot, w)  # noqa: E731
+    out = torch.empty(rq(H.HPSI_RQ_OUT_LENGTH), dtype=torch.float64, device="cuda")
+    log(f"{cfg}: D {D} -> chi {int(chi.sum())} (discarded weight {disc:.3e}), {len(p.a_desc)} A blocks, "
+        f"{rq(H.HPSI_RQ_ALGO_BYTES) / 1e9:.2f} GB read+written, {rq(H.HPSI_RQ_USEFUL_FLOPS) / 1e9:.1f} GF, "
+        f"T^T {rq(H.HPSI_RQ_INTERMEDIATE_BYTES) / 1e9:.2f} GB, units {rq(H.HPSI_RQ_N_UNITS_1)} + {rq(H.HPSI_RQ_N_UNITS_2)}")
+
+    def step():
+        H.hpsi_truncate(plan, psi, chi_max, ot, stream)
+        H.hpsi_rotate_apply(rot, ot, out, stream)
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    with ClockSampler(0) as clk:
+        e0.record(stream)
+        for _ in range(args.steps):
+            step()
+        e1.record(stream)
+        torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1) / args.steps
+    # the two parts separately
+    e0.record(stream)
+    for _ in range(args.steps):
+        H.hpsi_truncate(plan, psi, chi_max, ot, stream)
+    e1.record(stream)
+    torch.cuda.synchronize()
+    ms_trunc = e0.elapsed_time(e1) / args.steps
+    e0.record(stream)
+    for _ in range(args.steps):
+        H.hpsi_rotate_apply(rot, ot, out, stream)
+    e1.record(stream)
+    torch.cuda.synchronize()
+    ms_rot = e0.elapsed_time(e1) / args.steps
+    prof = np.zeros(3)
+    for _ in range(3):
+        prof += np.array(H.hpsi_rotate_apply_profiled(rot, ot, out, stream))
+    prof /= 3
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as fh:
+            hbm_peak, peak_src = float(json.load(fh)["hbm_gbs"]), "MEASURED_PEAKS.json hbm_gbs (burst copy)"
+    except (OSError, ValueError, KeyError):
+        hbm_peak, peak_src = 6550.0, "fallback of B200_PROFILING.md"
+    algo = rq(H.HPSI_RQ_ALGO_BYTES)
+    dgemm_peak, calib = dgemm_calibration(torch)
+    rot_tf = rq(H.HPSI_RQ_USEFUL_FLOPS) / (ms_rot * 1e-3) / 1e12
+    rot_gbs = algo / (ms_rot * 1e-3) / 1e9
+    ridge = dgemm_peak * 1e12 / (hbm_peak * 1e9)
+    tensor_bound = rq(H.HPSI_RQ_USEFUL_FLOPS) / max(algo, 1) > ridge
+    # parity on a sample of blocks the oracle rotates one by one, with the device's own isometries
+    from oracle import site_update as su
+    oth = ot.cpu().numpy()
+    ots, o = [], 0
+    for l in range(len(chi)):
+        n = int(chi[l]) * int(p.d_left[l])
+        ots.append(oth[o:o + n].reshape(int(chi[l]), int(p.d_left[l])))
+        o += n
+    rng = np.random.default_rng(7)
+    pick = np.sort(rng.choice(len(p.a_desc), size=min(64, len(p.a_desc)), replace=False))
+    desc = H.hpsi_rotate_query(rot, H.HPSI_RQ_OUT_BLOCKS)[pick]
+    t0 = time.time()
+    ref = su.rotate(p.d_left, chi, p.a_desc[pick], p.a_data, ots)
+    outh = out.cpu().numpy()
+    num = den = 0.0
+    for e, x in zip(desc, ref):
+        if e["offset"] < 0:
+            continue
+        g = np.lib.stride_tricks.as_strided(outh[int(e["offset"]):], shape=x.shape, strides=(int(e["ld"]) * 8, 8))
+        num += float(np.sum((g - x) ** 2)); den += float(np.sum(x ** 2))
+    # CPU baseline: the oracle (numpy SVD per block + BLAS rotation) on a bounded sample of blocks
+    t0 = time.time()
+    su.truncate(p, psi_h, chi_max)
+    t_trunc_cpu = time.time() - t0
+    nb = min(len(p.a_desc), 4000)
+    t0 = time.time()
+    su.rotate(p.d_left, chi, p.a_desc[:nb], p.a_data, ots)
+    t_rot_cpu = (time.time() - t0) * len(p.a_desc) / nb
+    print(json.dumps({
+        "metric": "site update (SVD truncation + operator update O^T A O) per second, FP64", "value": 1e3 / ms,
+        "unit": "updates/s", "n_gpus": 1, "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms,
+        "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": CONFIG_DESC[cfg] + " - site update", "D": D, "chi_max": chi_max, "kept": int(chi.sum()),
+                   "a_blocks": int(len(p.a_desc)), "algorithmic_bytes": algo, "useful_flops": rq(H.HPSI_RQ_USEFUL_FLOPS),
+                   "intermediate_bytes": rq(H.HPSI_RQ_INTERMEDIATE_BYTES), "l2": "inputs larger than L2 (operators read once)"},
+        "parts_ms": {"hpsi_truncate": ms_trunc, "hpsi_rotate_apply": ms_rot, "rot_prep": float(prof[0]),
+                     "rotate launch 1 (A O)": float(prof[1]), "rotate launch 2 (O^T T)": float(prof[2]),
+                     "svd_sweeps": H.hpsi_query(plan, H.HPSI_Q_SVD_SWEEPS), "svd_launches": H.hpsi_query(plan, H.HPSI_Q_SVD_LAUNCHES)},
+        "roofline": {"bound": "tensor" if tensor_bound else "hbm", "kernel": "p1_kernel<TMA, ROT> x2 (hpsi_rotate_apply)",
+                     "achieved": rot_tf if tensor_bound else rot_gbs, "peak": dgemm_peak if tensor_bound else hbm_peak,
+                     "unit": "TFLOP/s" if tensor_bound else "GB/s",
+                     "frac": rot_tf / dgemm_peak if tensor_bound else rot_gbs / hbm_peak, "traffic": None,
+                     "peak_source": "same-run cuBLAS DGEMM calibration" if tensor_bound else peak_src,
+                     "flops_per_algorithmic_byte": rq(H.HPSI_RQ_USEFUL_FLOPS) / max(algo, 1), "ridge": ridge,
+                     "tflops": rot_tf, "algorithmic_gbs": rot_gbs},
+        "calibration": {"fp64_tc_peak_tflops": dgemm_peak, **calib},
+        "clocks": clk.summary(), "parity_sample_rel_err": float(np.sqrt(num / max(den, 1e-300))),
+        "gpu_launches": (H.hpsi_query(plan, H.HPSI_Q_SVD_LAUNCHES) + 3) * args.steps,
+        "cpu_baseline": {"value": 1.0 / (t_trunc_cpu + t_rot_cpu), "unit": "updates/s", "cores": os.cpu_count(), "kind": "oracle",
+                         "sample": f"oracle truncate in full ({t_trunc_cpu:.2f} s) + oracle rotate on the first {nb} of "
+                                   f"{len(p.a_desc)} blocks, scaled ({t_rot_cpu:.2f} s)"},
+    }), flush=True)
+
+
 # ------------------------------------------------------------------------------------------------- our arm
 def run_ours(args, rank, world, local_rank):
     import torch
@@ -410,6 +540,8 @@ def main():
                     help="stream the operators from pinned host memory through two windows of this fraction of the arenas")
     ap.add_argument("--share-adjoint", action="store_true",
                     help="adjoint terms read their partner's blocks transposed (half the operator bytes; hpsi_terms_t a_transposed)")
+    ap.add_argument("--site-update", action="store_true",
+                    help="time the steps after the eigen-solve instead: hpsi_truncate + hpsi_rotate_apply (SURVEY 8(f)-4)")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -419,6 +551,9 @@ def main():
     elif args.stream > 0:
         if rank == 0:
             run_streamed(args)
+    elif args.site_update:
+        if rank == 0:
+            run_site_update(args)
     else:
         run_ours(args, rank, world, local_rank)
 

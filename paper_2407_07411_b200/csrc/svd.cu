@@ -5,19 +5,22 @@
 // R = 1 at the start; plane rotations make the psi parts mutually orthogonal, the same rotations applied to R
 // accumulate J with  J psi_l = S V^T,  i.e. psi_l = J^T S V^T: row i of R is the i-th left singular vector and the norm
 // of the psi part its singular value.  Rows are contiguous (the psi layout is row-major), so a rotation streams two
-// rows with unit stride.
+// rows with unit stride.  A block with more rows than columns has linearly dependent rows (the surplus rows would only
+// decay linearly, sweep after sweep: measured 22 sweeps instead of 12 on the cyp blocks), so there the vectors are the COLUMNS: the working
+// matrix is psi_l^T alone, its converged rows are sigma_j u_j^T and the isometry rows are those rows divided by sigma_j.
 //
 // Parallel order (block Jacobi by tournament): the rows of a block are cut into chunks of `bsz` rows; in one kernel
 // launch ("round") every CTA owns one PAIR of chunks of one block, chosen by the round-robin (circle) schedule so that
 // all CTAs of a round touch disjoint rows; it loads its 2*bsz rows into shared memory, orthogonalises them pairwise - one
 // warp per row pair, again by a round-robin schedule, CTA barrier between its inner rounds - and writes them back.  The
 // first round of a block's sweep does all pairs inside the two chunks, the others only the cross pairs, so a sweep
-// visits every row pair of the block exactly once.  Sweeps repeat until one makes no rotation (device flag; the only
-// atomic, not on data).  Every psi block is processed in the same launches.  All arithmetic is FP64 FMA; the result is
+// visits every row pair of the block exactly once.  Sweeps repeat until one makes no rotation (device counter of rotations; the
+// only atomic, not on data).  Every psi block is processed in the same launches.  All arithmetic is FP64 FMA; the result is
 // bitwise reproducible.
 #include <algorithm>
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <numeric>
 #include <vector>
 
@@ -26,9 +29,12 @@
 namespace hpsi {
 
 struct SvdBlk {
-  int64_t w_off;        // working matrix rows x L in the SVD workspace
+  int64_t w_off;        // working matrix nv x L in the SVD workspace
   int64_t psi_off;      // block in psi (dense rows x cols)
-  int32_t rows, cols, L;
+  int32_t rows, cols;   // of the psi block
+  int32_t nv, vlen;     // vectors orthogonalised and their length: (rows, cols) if rows <= cols, else (cols, rows)
+  int32_t tall;         // 1: rows > cols, the working matrix is the transposed block without the R part
+  int32_t L;            // leading dimension: vlen (+ rows for the R part) rounded up to 4
   int32_t nce;          // chunks, padded to an even count >= 2
   int32_t cta0;         // first CTA of this block in a round
   int32_t row0;         // first row in the concatenated singular-value array
@@ -41,12 +47,12 @@ constexpr int SVD_SMEM_BUDGET = 200 * 1024;
 // working matrix <- [psi block | identity]; floor2 of the block from its Frobenius norm (one CTA per block row range)
 __global__ void svd_init_kernel(SvdBlk* blk, const double* __restrict__ psi, double* __restrict__ w) {
   const SvdBlk B = blk[blockIdx.y];
-  for (int i = blockIdx.x; i < B.rows; i += gridDim.x) {
+  for (int i = blockIdx.x; i < B.nv; i += gridDim.x) {
     double* row = w + B.w_off + (int64_t)i * B.L;
     for (int j = threadIdx.x; j < B.L; j += blockDim.x) {
       double v = 0.0;
-      if (j < B.cols) v = psi[B.psi_off + (int64_t)i * B.cols + j];
-      else if (j - B.cols == i) v = 1.0;
+      if (j < B.vlen) v = B.tall ? psi[B.psi_off + (int64_t)j * B.cols + i] : psi[B.psi_off + (int64_t)i * B.cols + j];
+      else if (!B.tall && j - B.vlen == i) v = 1.0;
       row[j] = v;
     }
   }
@@ -86,7 +92,7 @@ __global__ void svd_round_kernel(const SvdBlk* __restrict__ blk, const int32_t* 
   else { ci = (rr + k) % n1; cj = (rr - k + n1) % n1; }
   if (ci > cj) { const int t = ci; ci = cj; cj = t; }
   const bool full = (rr == 0);                           // first round of the block's sweep: pairs inside the chunks too
-  const int ni = max(0, min(bsz, B.rows - ci * bsz)), nj = max(0, min(bsz, B.rows - cj * bsz));
+  const int ni = max(0, min(bsz, B.nv - ci * bsz)), nj = max(0, min(bsz, B.nv - cj * bsz));
   if (ni + nj < 2 || (!full && (ni == 0 || nj == 0))) return;
   const int L = B.L, tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
   // slot s < bsz holds row ci*bsz + s, slot bsz + s holds row cj*bsz + s
@@ -102,10 +108,14 @@ __global__ void svd_round_kernel(const SvdBlk* __restrict__ blk, const int32_t* 
     for (int j = lane; j < L / 2; j += 32) dst[j] = src[j];
   }
   __syncthreads();
-  const double tol = 4.4e-16 * sqrt((double)max(B.cols, 8));
-  bool rotated = false;
+  // rotate when |<x_p,x_q>| > tol |x_p||x_q| with tol = cols * 2^-53, the threshold LAPACK's Jacobi SVD (dgesvj) uses:
+  // a dot product of `cols` terms cannot resolve angles below ~sqrt(cols) * 2^-53, and a tighter test only makes
+  // rounding noise trigger further sweeps
+  const double tol = 1.1102230246251565e-16 * (double)max(B.vlen, 8);
+  int rotated = 0;
   const int np = 2 * bsz - 1;
   const int inner = full ? np : bsz;
+  const int c2 = B.vlen >> 1, L2 = L >> 1;               // rows as double2 (L is a multiple of 4, rows 16-byte aligned)
   for (int s = 0; s < inner; ++s) {
     int p, q;
     if (full) {
@@ -115,11 +125,20 @@ __global__ void svd_round_kernel(const SvdBlk* __restrict__ blk, const int32_t* 
       p = wid; q = bsz + (wid + s) % bsz;
     }
     if (valid(p) && valid(q)) {
+      // (de Rijk's ordering - exchanging the two vectors so that the lower index keeps the larger norm - was tried and
+      // needed two MORE sweeps on these spectra, 14 vs 12 on cyp, so the plain small-angle rotation stays)
       double* xp = srow + (size_t)p * L;
       double* xq = srow + (size_t)q * L;
+      double2* xp2 = reinterpret_cast<double2*>(xp);
+      double2* xq2 = reinterpret_cast<double2*>(xq);
       double a = 0.0, b = 0.0, g = 0.0;
-      for (int j = lane; j < B.cols; j += 32) {
-        const double u = xp[j], v = xq[j];
+      for (int j = lane; j < c2; j += 32) {
+        const double2 u = xp2[j], v = xq2[j];
+        a = fma(u.x, u.x, a); b = fma(v.x, v.x, b); g = fma(u.x, v.x, g);
+        a = fma(u.y, u.y, a); b = fma(v.y, v.y, b); g = fma(u.y, v.y, g);
+      }
+      if ((B.vlen & 1) && lane == 0) {
+        const double u = xp[B.vlen - 1], v = xq[B.vlen - 1];
         a = fma(u, u, a); b = fma(v, v, b); g = fma(u, v, g);
       }
       a = warp_sum(a); b = warp_sum(b); g = warp_sum(g);
@@ -127,12 +146,12 @@ __global__ void svd_round_kernel(const SvdBlk* __restrict__ blk, const int32_t* 
         const double zeta = (b - a) / (2.0 * g);
         const double t = copysign(1.0, zeta) / (fabs(zeta) + sqrt(1.0 + zeta * zeta));
         const double cs = 1.0 / sqrt(1.0 + t * t), sn = cs * t;
-        for (int j = lane; j < L; j += 32) {
-          const double u = xp[j], v = xq[j];
-          xp[j] = cs * u - sn * v;
-          xq[j] = sn * u + cs * v;
+        for (int j = lane; j < L2; j += 32) {
+          const double2 u = xp2[j], v = xq2[j];
+          xp2[j] = make_double2(cs * u.x - sn * v.x, cs * u.y - sn * v.y);
+          xq2[j] = make_double2(sn * u.x + cs * v.x, sn * u.y + cs * v.y);
         }
-        rotated = true;
+        ++rotated;
       }
     }
     __syncthreads();
@@ -143,27 +162,27 @@ __global__ void svd_round_kernel(const SvdBlk* __restrict__ blk, const int32_t* 
     const double2* src = reinterpret_cast<const double2*>(srow + (size_t)slot * L);
     for (int j = lane; j < L / 2; j += 32) dst[j] = src[j];
   }
-  if (rotated && lane == 0) atomicOr(flag, 1);
+  if (rotated && lane == 0) atomicAdd(flag, rotated);    // rotations of the sweep (control only, not data)
 }
 
 // singular value of every row = norm of its psi part (one warp per row)
 __global__ void svd_sigma_kernel(const SvdBlk* __restrict__ blk, const double* __restrict__ w, double* __restrict__ sigma) {
   const SvdBlk B = blk[blockIdx.y];
   const int lane = threadIdx.x & 31, wpb = blockDim.x >> 5;
-  for (int i = blockIdx.x * wpb + (threadIdx.x >> 5); i < B.rows; i += gridDim.x * wpb) {
+  for (int i = blockIdx.x * wpb + (threadIdx.x >> 5); i < B.nv; i += gridDim.x * wpb) {
     const double* row = w + B.w_off + (int64_t)i * B.L;
     double a = 0.0;
-    for (int j = lane; j < B.cols; j += 32) a = fma(row[j], row[j], a);
+    for (int j = lane; j < B.vlen; j += 32) a = fma(row[j], row[j], a);
     a = warp_sum(a);
     if (lane == 0) sigma[B.row0 + i] = sqrt(a);
   }
 }
 
-struct IsoRow { int64_t src, dst; int32_t len, pad; };   // R part of one kept row -> one row of O_l^T
+struct IsoRow { int64_t src, dst; double scale; int32_t len, pad; };   // kept vector (R part, or row / sigma) -> one row of O_l^T
 __global__ void svd_gather_kernel(const IsoRow* __restrict__ rows, int n, const double* __restrict__ w, double* __restrict__ ot) {
   for (int i = blockIdx.x; i < n; i += gridDim.x) {
     const IsoRow r = rows[i];
-    for (int j = threadIdx.x; j < r.len; j += blockDim.x) ot[r.dst + j] = w[r.src + j];
+    for (int j = threadIdx.x; j < r.len; j += blockDim.x) ot[r.dst + j] = w[r.src + j] * r.scale;
   }
 }
 
@@ -195,10 +214,12 @@ extern "C" int hpsi_truncate(hpsi_plan_t* p, const double* psi_dev, int32_t chi_
     const PsiBlk& B = sc.blocks[b];
     SvdBlk& s = tab[b];
     s.w_off = wlen; s.psi_off = B.off; s.rows = B.rows; s.cols = B.cols;
-    s.L = sector_up(B.rows + B.cols);
+    s.tall = B.rows > B.cols ? 1 : 0;
+    s.nv = std::min(B.rows, B.cols); s.vlen = std::max(B.rows, B.cols);
+    s.L = s.tall ? sector_up(s.vlen) : sector_up(B.rows + B.cols);
     s.row0 = row0; s.floor2 = 0.0;
-    row0 += B.rows;
-    wlen = (wlen + (int64_t)s.rows * s.L + 15) & ~(int64_t)15;
+    row0 += s.nv;
+    wlen = (wlen + (int64_t)s.nv * s.L + 15) & ~(int64_t)15;
     Lmax = std::max(Lmax, s.L);
   }
   const int n_rows = row0;
@@ -208,7 +229,7 @@ extern "C" int hpsi_truncate(hpsi_plan_t* p, const double* psi_dev, int32_t chi_
   std::vector<int32_t> cta_blk;
   for (int b = 0; b < nB; ++b) {
     SvdBlk& s = tab[b];
-    int nc = (s.rows + bsz - 1) / bsz;
+    int nc = (s.nv + bsz - 1) / bsz;
     nc += nc & 1;
     s.nce = std::max(nc, 2);
     s.cta0 = n_cta;
@@ -247,6 +268,7 @@ extern "C" int hpsi_truncate(hpsi_plan_t* p, const double* psi_dev, int32_t chi_
       svd_round_kernel<<<n_cta, 32 * bsz, smem, st>>>(d_tab, d_cta, sweeps * rounds + r, bsz, d_w, d_flag);
     HPSI_CUDA(cudaMemcpyAsync(&flag, d_flag, sizeof(int), cudaMemcpyDeviceToHost, st));
     HPSI_CUDA(cudaStreamSynchronize(st));
+    if (getenv("HPSI_SVD_DEBUG")) fprintf(stderr, "hpsi_truncate: sweep %d: %d rotations\n", sweeps, flag);
   }
   if (flag) { set_error("hpsi_truncate: Jacobi SVD did not converge"); return HPSI_ESTATE; }
   p->svd_sweeps = sweeps;
@@ -261,17 +283,18 @@ extern "C" int hpsi_truncate(hpsi_plan_t* p, const double* psi_dev, int32_t chi_
   std::vector<Cand> cand;
   cand.reserve(n_rows);
   double smax = 0.0;
+  int64_t out_row0 = 0;                                // sigma_host holds d_left entries per block
   for (int b = 0; b < nB; ++b) {
     const SvdBlk& s = tab[b];
-    std::vector<int> ord(s.rows);
+    std::vector<int> ord(s.nv);
     std::iota(ord.begin(), ord.end(), 0);
     std::stable_sort(ord.begin(), ord.end(), [&](int x, int y) { return sig[s.row0 + x] > sig[s.row0 + y]; });
-    const int nsv = std::min(s.rows, s.cols);
     for (int k = 0; k < s.rows; ++k) {
-      const double v = k < nsv ? sig[s.row0 + ord[k]] : 0.0;     // rows past min(rows, cols) are rounding noise
-      if (sigma_host) sigma_host[s.row0 + k] = v;
-      if (k < nsv) { cand.push_back({v, b, k, ord[k]}); smax = std::max(smax, v); }
+      const double v = k < s.nv ? sig[s.row0 + ord[k]] : 0.0;
+      if (sigma_host) sigma_host[out_row0 + k] = v;
+      if (k < s.nv) { cand.push_back({v, b, k, ord[k]}); smax = std::max(smax, v); }
     }
+    out_row0 += s.rows;
   }
   std::stable_sort(cand.begin(), cand.end(), [](const Cand& x, const Cand& y) {
     if (x.s != y.s) return x.s > y.s;
@@ -299,7 +322,8 @@ extern "C" int hpsi_truncate(hpsi_plan_t* p, const double* psi_dev, int32_t chi_
     const SvdBlk& s = tab[b];
     chi_host[sc.blocks[b].left] = (int32_t)kept[b].size();
     for (int row : kept[b]) {
-      rows.push_back({s.w_off + (int64_t)row * s.L + s.cols, dst, s.rows, 0});
+      if (s.tall) rows.push_back({s.w_off + (int64_t)row * s.L, dst, 1.0 / sig[s.row0 + row], s.rows, 0});
+      else rows.push_back({s.w_off + (int64_t)row * s.L + s.cols, dst, 1.0, s.rows, 0});
       dst += s.rows;
     }
   }
