@@ -314,6 +314,12 @@ def run_site_update(args):
     rot_gbs = algo / (ms_rot * 1e-3) / 1e9
     ridge = dgemm_peak * 1e12 / (hbm_peak * 1e9)
     tensor_bound = rq(H.HPSI_RQ_USEFUL_FLOPS) / max(algo, 1) > ridge
+    traffic = None                       # DRAM bytes of the two launches from the committed ncu --set full capture
+    try:
+        with open(os.path.join(ROOT, "profiles", "ncu_traffic.json.txt")) as fh:
+            traffic = json.load(fh).get(cfg + "_site_update", {}).get("p1_kernel_rot")
+    except (OSError, ValueError):
+        pass
     # parity on a sample of blocks the oracle rotates one by one, with the device's own isometries
     from oracle import site_update as su
     oth = ot.cpu().numpy()
@@ -355,7 +361,7 @@ def run_site_update(args):
         "roofline": {"bound": "tensor" if tensor_bound else "hbm", "kernel": "p1_kernel<TMA, ROT> x2 (hpsi_rotate_apply)",
                      "achieved": rot_tf if tensor_bound else rot_gbs, "peak": dgemm_peak if tensor_bound else hbm_peak,
                      "unit": "TFLOP/s" if tensor_bound else "GB/s",
-                     "frac": rot_tf / dgemm_peak if tensor_bound else rot_gbs / hbm_peak, "traffic": None,
+                     "frac": rot_tf / dgemm_peak if tensor_bound else rot_gbs / hbm_peak, "traffic": traffic,
                      "peak_source": "same-run cuBLAS DGEMM calibration" if tensor_bound else peak_src,
                      "flops_per_algorithmic_byte": rq(H.HPSI_RQ_USEFUL_FLOPS) / max(algo, 1), "ridge": ridge,
                      "tflops": rot_tf, "algorithmic_gbs": rot_gbs},
