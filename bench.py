@@ -391,7 +391,7 @@ def run_ours(args, rank, world, local_rank):
     half = workloads.config_params(cfg)["n_terms"] // 2
     t0 = time.time()
     shard = None if world == 1 else np.arange(rank, half, world)
-    p = workloads.make_problem(cfg, base_terms=shard, share_adjoint=args.share_adjoint)
+    p = workloads.make_problem(cfg, base_terms=shard, share_adjoint=args.share_adjoint, D=args.D)
     gen_s = time.time() - t0
     a = torch.from_numpy(p.a_data).to(dev)
     b = torch.from_numpy(p.b_data).to(dev)
@@ -523,12 +523,15 @@ def run_ours(args, rank, world, local_rank):
         got = out.cpu().numpy()[idx]
         if args.share_adjoint:                   # the oracle only knows fully materialised operators
             del a, b
-            p = workloads.make_problem(cfg)
+            p = workloads.make_problem(cfg, D=args.D)
         ref = oracle.apply_samples(p, psi0, sl, sx, sy)
         res["parity_sample_rel_err"] = float(np.linalg.norm(got - ref) / np.linalg.norm(ref))
         if not args.share_adjoint:
             del a, b
-        res["cpu_baseline"], _, _ = cpu_baseline(cfg)
+        if args.D is None:
+            res["cpu_baseline"], _, _ = cpu_baseline(cfg)
+        else:
+            res["config"]["workload"] += f" with D overridden to {args.D} (bond-dimension sweep, not a BASELINE config)"
     if rank == 0:
         print(json.dumps(res), flush=True)
     if world > 1:
@@ -546,6 +549,8 @@ def main():
                     help="stream the operators from pinned host memory through two windows of this fraction of the arenas")
     ap.add_argument("--share-adjoint", action="store_true",
                     help="adjoint terms read their partner's blocks transposed (half the operator bytes; hpsi_terms_t a_transposed)")
+    ap.add_argument("--D", type=int, default=None,
+                    help="override the config's bond dimension per side (sweep over D as in the paper's Fig. 1-2; 1 GPU)")
     ap.add_argument("--site-update", action="store_true",
                     help="time the steps after the eigen-solve instead: hpsi_truncate + hpsi_rotate_apply (SURVEY 8(f)-4)")
     args = ap.parse_args()

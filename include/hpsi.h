@@ -184,6 +184,8 @@ void hpsi_stream_destroy(hpsi_stream_t* s);
 /* One-sided Jacobi SVD (Hestenes) of every psi block of `plan`, on the device, then the global selection on the host.
  *   psi_dev        DEVICE, psi_length doubles (not modified)
  *   chi_max        number of singular values to keep over all blocks (>= 0)
+ *   eps_discard    if >= 0: keep only as many of them as it takes for the discarded weight to be <= eps_discard
+ *                  (the paper quotes its results by "truncation error"); < 0: keep chi_max
  *   ot_dev         DEVICE, receives the isometries in the layout above; capacity >= HPSI_Q_ISO_CAPACITY doubles
  *   chi_host       HOST, int32[n_left]: kept states per left sector (0 for a sector without a psi block)
  *   sigma_host     HOST or NULL, psi-rows doubles (HPSI_Q_PSI_ROWS = sum of d_left over the psi blocks): for every psi
@@ -191,8 +193,8 @@ void hpsi_stream_destroy(hpsi_stream_t* s);
  *   discarded_host HOST or NULL: sum of sigma^2 over everything not kept
  * Synchronises the stream (chi is needed on the host).  Deterministic (fixed rotation order; the only atomic is the
  * sweep's "anything rotated" flag).  Errors: EINVAL (null / negative arguments), ESTATE (host-only plan), ENOMEM, ECUDA. */
-int hpsi_truncate(hpsi_plan_t* plan, const double* psi_dev, int32_t chi_max, double* ot_dev, int32_t* chi_host,
-                  double* sigma_host, double* discarded_host, void* cuda_stream);
+int hpsi_truncate(hpsi_plan_t* plan, const double* psi_dev, int32_t chi_max, double eps_discard, double* ot_dev,
+                  int32_t* chi_host, double* sigma_host, double* discarded_host, void* cuda_stream);
 
 typedef struct hpsi_rotate hpsi_rotate_t;   /* opaque; owns the schedule, the workspace (padded isometries, T^T) */
 

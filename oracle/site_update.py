@@ -41,10 +41,12 @@ def psi_block_list(p) -> List[Tuple[int, int, int, int, int]]:
     return out
 
 
-def truncate(p, psi: np.ndarray, chi_max: int):
+def truncate(p, psi: np.ndarray, chi_max: int, eps_discard: float = -1.0):
     """Reading R1-R3: psi is block diagonal over (left sector, partner), so its SVD is the SVD of every block
     psi_l = U_l S_l V_l^T.  Keep the ``chi_max`` largest singular values over all blocks (ties: lower left sector, then
     lower index first; values <= SIGMA_FLOOR * sigma_max never kept).  O_l = the kept columns of U_l.
+    Reading R6 (the paper quotes results by their "truncation error"): with ``eps_discard`` >= 0 only as
+    many of those values are kept as it takes for the discarded weight to be <= eps_discard (never more than chi_max).
 
     Returns (chi[n_left], ot, sigma, discarded_weight):
       chi    int32 kept states per left sector (0 for a sector without a psi block);
@@ -61,9 +63,14 @@ def truncate(p, psi: np.ndarray, chi_max: int):
     cand.sort()
     smax = -cand[0][0] if cand else 0.0
     kept = {i: [] for i in S}
+    limit = chi_max
+    if eps_discard >= 0.0:
+        # tail[n] = weight discarded when the n largest are kept, summed smallest first
+        tail = np.concatenate([np.cumsum(np.array([c[0] for c in cand[::-1]]) ** 2)[::-1], [0.0]])
+        limit = min(chi_max, int(np.argmax(tail <= eps_discard)))
     n = 0
     for (ms, i, k) in cand:
-        if n >= chi_max or -ms <= SIGMA_FLOOR * smax:
+        if n >= limit or -ms <= SIGMA_FLOOR * smax:
             break
         kept[i].append(k)
         n += 1

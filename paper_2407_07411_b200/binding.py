@@ -99,7 +99,7 @@ def lib() -> ctypes.CDLL:
         L.hpsi_bench_fp64_pipe.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.POINTER(ctypes.c_double),
                                            ctypes.POINTER(ctypes.c_double)]
         L.hpsi_debug_interpret.argtypes = [vp, vp, vp, vp, vp]
-        L.hpsi_truncate.argtypes = [vp, vp, ctypes.c_int32, vp, vp, vp, vp, vp]
+        L.hpsi_truncate.argtypes = [vp, vp, ctypes.c_int32, ctypes.c_double, vp, vp, vp, vp, vp]
         L.hpsi_rotate_plan.argtypes = [ctypes.c_int32, vp, vp, i64, vp, vp, i64, ctypes.c_uint32, ctypes.POINTER(vp)]
         L.hpsi_rotate_apply.argtypes = [vp, vp, vp, vp]
         L.hpsi_rotate_apply_profiled.argtypes = [vp, vp, vp, vp, ctypes.POINTER(ctypes.c_float)]
@@ -313,14 +313,15 @@ def hpsi_debug_interpret(plan: Plan, a_host: np.ndarray, b_host: np.ndarray, psi
 
 
 # ------------------------------------------------------------------------ site update
-def hpsi_truncate(plan: Plan, psi, chi_max: int, ot, stream=None):
+def hpsi_truncate(plan: Plan, psi, chi_max: int, ot, stream=None, eps_discard: float = -1.0):
     """SVD truncation of psi (torch CUDA tensor).  ot: torch CUDA float64 tensor of >= HPSI_Q_ISO_CAPACITY doubles that
-    receives the isometries.  Returns (chi int32[n_left], sigma float64[HPSI_Q_PSI_ROWS], discarded_weight)."""
+    receives the isometries; eps_discard >= 0 keeps only as many states as the discarded weight <= eps_discard needs.
+    Returns (chi int32[n_left], sigma float64[HPSI_Q_PSI_ROWS], discarded_weight)."""
     n_left = int(plan.n_left)
     chi = np.zeros(n_left, np.int32)
     sigma = np.zeros(max(hpsi_query(plan, HPSI_Q_PSI_ROWS), 1), np.float64)
     disc = ctypes.c_double()
-    _check(lib().hpsi_truncate(plan.handle, _ptr(psi), int(chi_max), _ptr(ot), chi.ctypes.data, sigma.ctypes.data,
+    _check(lib().hpsi_truncate(plan.handle, _ptr(psi), int(chi_max), float(eps_discard), _ptr(ot), chi.ctypes.data, sigma.ctypes.data,
                                ctypes.addressof(disc), _stream(stream)))
     return chi, sigma[:hpsi_query(plan, HPSI_Q_PSI_ROWS)], disc.value
 

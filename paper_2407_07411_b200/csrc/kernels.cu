@@ -286,7 +286,17 @@ __global__ void reduce_kernel(DevSchedule d, double* __restrict__ out, int accum
     const int x = e / B.cols, y = e - x * B.cols;
     const double* p = d.ws + B.part_off + (int64_t)x * B.ldo + y;
     double s = accumulate ? out[B.off + e] : 0.0;           // hpsi_stream_apply: windows of terms add up in a fixed order
-    for (int sp = 0; sp < B.nsplit; ++sp) s += p[sp * stride];
+    // eight partials in flight, added in split order: a thread's chain of dependent L2 round trips was the whole
+    // kernel at small D (tens to hundreds of splits of a few-KB block)
+    int sp = 0;
+    for (; sp + 8 <= B.nsplit; sp += 8) {
+      double v[8];
+#pragma unroll
+      for (int i = 0; i < 8; ++i) v[i] = __ldg(p + (sp + i) * stride);
+#pragma unroll
+      for (int i = 0; i < 8; ++i) s += v[i];
+    }
+    for (; sp < B.nsplit; ++sp) s += __ldg(p + sp * stride);
     out[B.off + e] = s;
   }
 }

@@ -190,8 +190,8 @@ __global__ void svd_gather_kernel(const IsoRow* __restrict__ rows, int n, const 
 
 using namespace hpsi;
 
-extern "C" int hpsi_truncate(hpsi_plan_t* p, const double* psi_dev, int32_t chi_max, double* ot_dev, int32_t* chi_host,
-                             double* sigma_host, double* discarded_host, void* cuda_stream) {
+extern "C" int hpsi_truncate(hpsi_plan_t* p, const double* psi_dev, int32_t chi_max, double eps_discard, double* ot_dev,
+                             int32_t* chi_host, double* sigma_host, double* discarded_host, void* cuda_stream) {
   if (!p) { set_error("null plan"); return HPSI_EINVAL; }
   if (p->host_only) { set_error("host-only plan: hpsi_truncate needs a CUDA device (no CPU fallback)"); return HPSI_ESTATE; }
   if (chi_max < 0) { set_error("negative chi_max"); return HPSI_EINVAL; }
@@ -303,9 +303,16 @@ extern "C" int hpsi_truncate(hpsi_plan_t* p, const double* psi_dev, int32_t chi_
   });
   std::vector<std::vector<int>> kept(nB);
   std::vector<char> is_kept(cand.size(), 0);
+  int limit = chi_max;
+  if (eps_discard >= 0.0) {                            // reading R6: smallest count whose discarded weight is <= eps_discard
+    double tail = 0.0;                                 // weight discarded when the first i are kept, summed smallest first
+    size_t i = cand.size();
+    while (i > 0 && tail + cand[i - 1].s * cand[i - 1].s <= eps_discard) { tail += cand[i - 1].s * cand[i - 1].s; --i; }
+    limit = std::min<int64_t>(chi_max, (int64_t)i);
+  }
   int nk = 0;
   for (size_t i = 0; i < cand.size(); ++i) {
-    if (nk >= chi_max || cand[i].s <= 1e-13 * smax) break;
+    if (nk >= limit || cand[i].s <= 1e-13 * smax) break;
     kept[cand[i].blk].push_back(cand[i].row);        // descending singular value inside the block
     is_kept[i] = 1;
     ++nk;

@@ -98,21 +98,21 @@ def test_rotate_nothing_survives():
 
 
 # ------------------------------------------------------------------------------------------ truncate
-def run_truncate(p, psi, chi_max):
+def run_truncate(p, psi, chi_max, eps=-1.0):
     torch, H = _gpu()
     a = torch.from_numpy(p.a_data).cuda()
     b = torch.from_numpy(p.b_data).cuda()
     plan = H.plan_problem(p, a, b)
     x = torch.from_numpy(np.ascontiguousarray(psi)).cuda()
     ot = torch.full((max(H.hpsi_query(plan, H.HPSI_Q_ISO_CAPACITY), 1),), float("nan"), dtype=torch.float64, device="cuda:0")
-    chi, sigma, disc = H.hpsi_truncate(plan, x, chi_max, ot, torch.cuda.current_stream())
+    chi, sigma, disc = H.hpsi_truncate(plan, x, chi_max, ot, torch.cuda.current_stream(), eps)
     assert np.array_equal(x.cpu().numpy(), psi)                          # psi is not modified
     return plan, chi, sigma, disc, ot.cpu().numpy(), H
 
 
-def check_truncation(p, psi, chi_max, proj_tol=1e-9):
-    plan, chi, sigma, disc, ot, H = run_truncate(p, psi, chi_max)
-    chi_ref, ot_ref, sigma_ref, disc_ref = su.truncate(p, psi, chi_max)
+def check_truncation(p, psi, chi_max, proj_tol=1e-9, eps=-1.0):
+    plan, chi, sigma, disc, ot, H = run_truncate(p, psi, chi_max, eps)
+    chi_ref, ot_ref, sigma_ref, disc_ref = su.truncate(p, psi, chi_max, eps)
     assert np.array_equal(chi, chi_ref)
     smax = max(float(s[0]) for s in sigma_ref if s.size)
     row0 = iso0 = 0
@@ -139,6 +139,12 @@ def check_truncation(p, psi, chi_max, proj_tol=1e-9):
 def test_truncate_matches_oracle(name, chi_max):
     p = workloads.make_problem(name, n_terms=8)
     check_truncation(p, workloads.make_psi(p), chi_max)
+
+
+@pytest.mark.parametrize("eps,chi_max", [(1e-1, 10 ** 6), (1e-3, 10 ** 6), (1e-3, 300), (0.0, 10 ** 6)])
+def test_truncate_by_discarded_weight_matches_oracle(eps, chi_max):
+    p = workloads.make_problem("small", n_terms=8)
+    check_truncation(p, workloads.make_psi(p), chi_max, eps=eps)
 
 
 def test_truncate_cyp_sized_blocks_and_reproducible():

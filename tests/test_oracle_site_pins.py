@@ -44,6 +44,25 @@ def test_truncate_closed_form_diagonal():
     np.testing.assert_allclose(np.abs(ot[0]), np.eye(3)[:2], atol=1e-15)
 
 
+def test_truncate_by_discarded_weight_closed_form():
+    g = golden()["diag321_eps"]
+    psi = np.diag([3.0, 2.0, 1.0]) / np.sqrt(14.0)
+    for eps, kept in zip(g[0::2], g[1::2]):
+        chi, ot, sigma, dw = su.truncate(one_block_problem(psi), psi.ravel(), 3, float(eps))
+        assert chi.tolist() == [int(kept)] and dw <= float(eps)
+    chi, _, _, _ = su.truncate(one_block_problem(psi), psi.ravel(), 1, 0.08)      # chi_max still caps it
+    assert chi.tolist() == [1]
+
+
+def test_truncate_by_discarded_weight_is_minimal(small):
+    psi = workloads.make_psi(small)
+    for eps in (1e-1, 1e-2, 1e-4):
+        chi, ot, sigma, dw = su.truncate(small, psi, 10 ** 6, eps)
+        allsig2 = np.sort(np.concatenate(sigma) ** 2)            # ascending
+        n_drop = int(np.searchsorted(np.cumsum(allsig2), eps, side="right"))
+        assert int(chi.sum()) == allsig2.size - n_drop and dw <= eps
+
+
 def test_truncate_closed_form_rank_one():
     g = golden()["rank1"]
     u = np.array([float(x) for x in g[5:8]])

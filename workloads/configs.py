@@ -167,8 +167,11 @@ def _pareto_mix_dims(rng: np.random.Generator, n: int, D: int) -> np.ndarray:
 
 
 # ------------------------------------------------------------------------------------- sector tables
-def _sector_tables(name: str, seed: int):
-    p = _PARAMS[name]
+def _sector_tables(name: str, seed: int, D: Optional[int] = None):
+    p = dict(_PARAMS[name])
+    if D is not None:                       # bond-dimension sweep (Fig. 1 / Fig. 2 plot against D): same grid,
+        assert p["D"] is not None           # same profile and jitter, dims rounded to the new total
+        p["D"] = int(D)
     gN, gS = p["grid"]
     rng = np.random.default_rng([seed, 101])
     n = gN * gS
@@ -307,15 +310,16 @@ def _share_adjoint(desc: np.ndarray, ranges: np.ndarray, half: int):
 
 def make_problem(name: str, seed: Optional[int] = None, fill: bool = True, pad_even: bool = True,
                  n_terms: Optional[int] = None, base_terms=None, row_align: Optional[int] = None,
-                 share_adjoint: bool = False) -> Problem:
+                 share_adjoint: bool = False, D: Optional[int] = None) -> Problem:
     """Build config ``name`` (seed defaults to the config index).  ``fill=False`` returns descriptors only
     (arenas can then be streamed with ``fill_term``).  ``n_terms`` overrides the term count (tests).
     ``base_terms`` (indices into the T/2 base terms) keeps only those terms and their adjoints, with the same
     coefficients, shifts and entries they have in the full config (term shards for multi-GPU runs, bounded
-    samples for the timed CPU baseline); arenas are compacted to the kept terms."""
+    samples for the timed CPU baseline); arenas are compacted to the kept terms.  ``D`` overrides the total bond
+    dimension per side of a Gaussian / Pareto config (sweeps over D as in PAPER.md Fig. 1-2; not one of the five configs)."""
     par = _PARAMS[name]
     seed = par["index"] if seed is None else seed
-    q_left, q_right, d_left, d_right, target, partner = _sector_tables(name, seed)
+    q_left, q_right, d_left, d_right, target, partner = _sector_tables(name, seed, D)
     T = par["n_terms"] if n_terms is None else n_terms
     assert T % 2 == 0
     rng = np.random.default_rng([seed, 202])
