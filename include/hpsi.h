@@ -172,7 +172,7 @@ void hpsi_stream_destroy(hpsi_stream_t* s);
  *
  *   hpsi_truncate :  the matrix factorisation.  psi is block diagonal over (left sector l, partner r), so its SVD is
  *                    the SVD of every block, psi_l = U_l S_l V_l^T.  The chi_max largest singular values over all
- *                    blocks are kept (ties: lower left sector first; values <=
+ *                    blocks are kept (ties: the block that comes first in the psi table; values <=
  *                    1e-13 * sigma_max are never kept) and  O_l = the kept columns of U_l  is the new left basis.
  *   hpsi_rotate_* :  the renormalised-operator update  A'_t[l,l'] = O_l^T A_t[l,l'] O_l'  for every block of every
  *                    left operator, on the same grouped DMMA GEMM engine as hpsi_apply.
@@ -183,18 +183,23 @@ void hpsi_stream_destroy(hpsi_stream_t* s);
 
 /* One-sided Jacobi SVD (Hestenes) of every psi block of `plan`, on the device, then the global selection on the host.
  *   psi_dev        DEVICE, psi_length doubles (not modified)
+ *   side           HPSI_SIDE_LEFT: new LEFT basis, O_l = kept left singular vectors (a right-moving sweep);
+ *                  HPSI_SIDE_RIGHT: new RIGHT basis, O_r = kept right singular vectors of the block whose right
+ *                  sector is r (a left-moving sweep) - "left" below then reads "right", d_left reads d_right
  *   chi_max        number of singular values to keep over all blocks (>= 0)
  *   eps_discard    if >= 0: keep only as many of them as it takes for the discarded weight to be <= eps_discard
  *                  (the paper quotes its results by "truncation error"); < 0: keep chi_max
  *   ot_dev         DEVICE, receives the isometries in the layout above; capacity >= HPSI_Q_ISO_CAPACITY doubles
- *   chi_host       HOST, int32[n_left]: kept states per left sector (0 for a sector without a psi block)
+ *   chi_host       HOST, int32[n_left] (n_right for the right side): kept states per sector (0 without a psi block)
  *   sigma_host     HOST or NULL, psi-rows doubles (HPSI_Q_PSI_ROWS = sum of d_left over the psi blocks): for every psi
  *                  block in table order its d_left values, descending; entries past min(d_left, d_right) are 0
  *   discarded_host HOST or NULL: sum of sigma^2 over everything not kept
  * Synchronises the stream (chi is needed on the host).  Deterministic (fixed rotation order; the only atomic is the
  * sweep's "anything rotated" flag).  Errors: EINVAL (null / negative arguments), ESTATE (host-only plan), ENOMEM, ECUDA. */
-int hpsi_truncate(hpsi_plan_t* plan, const double* psi_dev, int32_t chi_max, double eps_discard, double* ot_dev,
-                  int32_t* chi_host, double* sigma_host, double* discarded_host, void* cuda_stream);
+#define HPSI_SIDE_LEFT  0
+#define HPSI_SIDE_RIGHT 1
+int hpsi_truncate(hpsi_plan_t* plan, const double* psi_dev, int32_t side, int32_t chi_max, double eps_discard,
+                  double* ot_dev, int32_t* chi_host, double* sigma_host, double* discarded_host, void* cuda_stream);
 
 typedef struct hpsi_rotate hpsi_rotate_t;   /* opaque; owns the schedule, the workspace (padded isometries, T^T) */
 
@@ -259,7 +264,9 @@ enum {
   HPSI_Q_PSI_ROWS = 19,      /* int64: sum of d_left over the psi blocks (length of hpsi_truncate's sigma_host)  */
   HPSI_Q_ISO_CAPACITY = 20,  /* int64: sum of min(d_left, d_right) * d_left over the psi blocks (ot_dev capacity) */
   HPSI_Q_SVD_SWEEPS = 21,    /* int64: Jacobi sweeps of the last hpsi_truncate on this plan                      */
-  HPSI_Q_SVD_LAUNCHES = 22   /* int64: kernels it launched                                                       */
+  HPSI_Q_SVD_LAUNCHES = 22,  /* int64: kernels it launched                                                       */
+  HPSI_Q_PSI_COLS = 23,      /* int64: sum of d_right over the psi blocks (sigma_host length for HPSI_SIDE_RIGHT)  */
+  HPSI_Q_ISO_CAPACITY_RIGHT = 24 /* int64: sum of min(d_left, d_right) * d_right over the psi blocks              */
 };
 
 typedef struct {

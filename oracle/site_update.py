@@ -41,12 +41,14 @@ def psi_block_list(p) -> List[Tuple[int, int, int, int, int]]:
     return out
 
 
-def truncate(p, psi: np.ndarray, chi_max: int, eps_discard: float = -1.0):
+def truncate(p, psi: np.ndarray, chi_max: int, eps_discard: float = -1.0, side: str = "left"):
     """Reading R1-R3: psi is block diagonal over (left sector, partner), so its SVD is the SVD of every block
     psi_l = U_l S_l V_l^T.  Keep the ``chi_max`` largest singular values over all blocks (ties: lower left sector, then
     lower index first; values <= SIGMA_FLOOR * sigma_max never kept).  O_l = the kept columns of U_l.
     Reading R6 (the paper quotes results by their "truncation error"): with ``eps_discard`` >= 0 only as
     many of those values are kept as it takes for the discarded weight to be <= eps_discard (never more than chi_max).
+    ``side="right"``: the new RIGHT basis instead - every block is transposed first, sectors / dims are the right ones
+    (O_r = kept right singular vectors of the block whose right sector is r); ties still go by psi-table order.
 
     Returns (chi[n_left], ot, sigma, discarded_weight):
       chi    int32 kept states per left sector (0 for a sector without a psi block);
@@ -54,13 +56,18 @@ def truncate(p, psi: np.ndarray, chi_max: int, eps_discard: float = -1.0):
       sigma  list over left sectors of ALL min(d_l, d_r) singular values, descending (empty without a block);
       discarded_weight = sum of sigma^2 over everything not kept."""
     psi = np.asarray(psi, np.float64)
-    nL = int(np.asarray(p.q_left).shape[0])
-    U, S = {}, {}
-    for (i, j, r, c, off) in psi_block_list(p):
-        u, s, _ = np.linalg.svd(psi[off:off + r * c].reshape(r, c), full_matrices=False)
-        U[i], S[i] = u, s
-    cand = [(-float(s), i, k) for i in S for k, s in enumerate(S[i])]
+    right = side == "right"
+    nL = int(np.asarray(p.q_right if right else p.q_left).shape[0])
+    dims = p.d_right if right else p.d_left
+    U, S, pos = {}, {}, {}
+    for n_blk, (i, j, r, c, off) in enumerate(psi_block_list(p)):
+        blk = psi[off:off + r * c].reshape(r, c)
+        u, s, _ = np.linalg.svd(blk.T if right else blk, full_matrices=False)
+        sec = j if right else i
+        U[sec], S[sec], pos[sec] = u, s, n_blk
+    cand = [(-float(s), pos[i], k, i) for i in S for k, s in enumerate(S[i])]
     cand.sort()
+    cand = [(ms, i, k) for (ms, _, k, i) in cand]
     smax = -cand[0][0] if cand else 0.0
     kept = {i: [] for i in S}
     limit = chi_max
@@ -79,7 +86,7 @@ def truncate(p, psi: np.ndarray, chi_max: int, eps_discard: float = -1.0):
     disc = 0.0
     for i in range(nL):
         if i not in S:
-            ot.append(np.zeros((0, int(p.d_left[i]))))
+            ot.append(np.zeros((0, int(dims[i]))))
             sigma.append(np.zeros(0))
             continue
         ks = kept[i]

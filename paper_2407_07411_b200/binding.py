@@ -21,7 +21,8 @@ HPSI_PLAN_FIXED_ORDER2 = 1 << 2
  HPSI_Q_OPERATOR_BYTES, HPSI_Q_WORKSPACE_BYTES, HPSI_Q_N_GROUPS, HPSI_Q_N_P1_UNITS, HPSI_Q_N_P2_UNITS,
  HPSI_Q_N_ORDER1_TASKS, HPSI_Q_LAUNCHES_PER_APPLY, HPSI_Q_ALIGNED16, HPSI_Q_INTERMEDIATE_BYTES,
  HPSI_Q_ISSUED_FLOPS_P1, HPSI_Q_TASKS, HPSI_Q_USEFUL_FLOPS_P1, HPSI_Q_CRITICAL_FLOPS, HPSI_Q_PSI_ROWS,
- HPSI_Q_ISO_CAPACITY, HPSI_Q_SVD_SWEEPS, HPSI_Q_SVD_LAUNCHES) = range(23)
+ HPSI_Q_ISO_CAPACITY, HPSI_Q_SVD_SWEEPS, HPSI_Q_SVD_LAUNCHES, HPSI_Q_PSI_COLS, HPSI_Q_ISO_CAPACITY_RIGHT) = range(25)
+HPSI_SIDE_LEFT, HPSI_SIDE_RIGHT = 0, 1
 (HPSI_RQ_OUT_LENGTH, HPSI_RQ_OUT_BLOCKS, HPSI_RQ_ISO_LENGTH, HPSI_RQ_USEFUL_FLOPS, HPSI_RQ_ALGO_BYTES,
  HPSI_RQ_WORKSPACE_BYTES, HPSI_RQ_N_UNITS_1, HPSI_RQ_N_UNITS_2, HPSI_RQ_ALIGNED16, HPSI_RQ_INTERMEDIATE_BYTES) = range(10)
 OPBLOCK_DTYPE = np.dtype([("term", "<i4"), ("row", "<i4"), ("col", "<i4"), ("ld", "<i4"), ("offset", "<i8")], align=True)
@@ -99,7 +100,7 @@ def lib() -> ctypes.CDLL:
         L.hpsi_bench_fp64_pipe.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.POINTER(ctypes.c_double),
                                            ctypes.POINTER(ctypes.c_double)]
         L.hpsi_debug_interpret.argtypes = [vp, vp, vp, vp, vp]
-        L.hpsi_truncate.argtypes = [vp, vp, ctypes.c_int32, ctypes.c_double, vp, vp, vp, vp, vp]
+        L.hpsi_truncate.argtypes = [vp, vp, ctypes.c_int32, ctypes.c_int32, ctypes.c_double, vp, vp, vp, vp, vp]
         L.hpsi_rotate_plan.argtypes = [ctypes.c_int32, vp, vp, i64, vp, vp, i64, ctypes.c_uint32, ctypes.POINTER(vp)]
         L.hpsi_rotate_apply.argtypes = [vp, vp, vp, vp]
         L.hpsi_rotate_apply_profiled.argtypes = [vp, vp, vp, vp, ctypes.POINTER(ctypes.c_float)]
@@ -183,7 +184,7 @@ def hpsi_plan(q_left, q_right, d_left, d_right, target, coef, a_blocks, b_blocks
     out = ctypes.c_void_p()
     _check(lib().hpsi_plan(ctypes.byref(sec), ctypes.byref(trm), flags, ctypes.byref(out)))
     pl = Plan(out.value, (a_data, b_data))
-    pl.n_left = q_left.shape[0]
+    pl.n_left, pl.n_right = q_left.shape[0], q_right.shape[0]
     return pl
 
 
@@ -313,17 +314,17 @@ def hpsi_debug_interpret(plan: Plan, a_host: np.ndarray, b_host: np.ndarray, psi
 
 
 # ------------------------------------------------------------------------ site update
-def hpsi_truncate(plan: Plan, psi, chi_max: int, ot, stream=None, eps_discard: float = -1.0):
+def hpsi_truncate(plan: Plan, psi, chi_max: int, ot, stream=None, eps_discard: float = -1.0, side: int = 0):
     """SVD truncation of psi (torch CUDA tensor).  ot: torch CUDA float64 tensor of >= HPSI_Q_ISO_CAPACITY doubles that
     receives the isometries; eps_discard >= 0 keeps only as many states as the discarded weight <= eps_discard needs.
     Returns (chi int32[n_left], sigma float64[HPSI_Q_PSI_ROWS], discarded_weight)."""
-    n_left = int(plan.n_left)
-    chi = np.zeros(n_left, np.int32)
-    sigma = np.zeros(max(hpsi_query(plan, HPSI_Q_PSI_ROWS), 1), np.float64)
+    chi = np.zeros(int(plan.n_right if side == HPSI_SIDE_RIGHT else plan.n_left), np.int32)
+    n_sig = hpsi_query(plan, HPSI_Q_PSI_COLS if side == HPSI_SIDE_RIGHT else HPSI_Q_PSI_ROWS)
+    sigma = np.zeros(max(n_sig, 1), np.float64)
     disc = ctypes.c_double()
-    _check(lib().hpsi_truncate(plan.handle, _ptr(psi), int(chi_max), float(eps_discard), _ptr(ot), chi.ctypes.data, sigma.ctypes.data,
+    _check(lib().hpsi_truncate(plan.handle, _ptr(psi), int(side), int(chi_max), float(eps_discard), _ptr(ot), chi.ctypes.data, sigma.ctypes.data,
                                ctypes.addressof(disc), _stream(stream)))
-    return chi, sigma[:hpsi_query(plan, HPSI_Q_PSI_ROWS)], disc.value
+    return chi, sigma[:n_sig], disc.value
 
 
 class RotatePlan:

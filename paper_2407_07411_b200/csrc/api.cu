@@ -175,6 +175,7 @@ extern "C" int hpsi_plan(const hpsi_sectors_t* sectors, const hpsi_terms_t* term
     rc = build_schedule(sectors, terms, flags, p->n_sm, &p->sc, &err);
     if (rc != HPSI_OK) { set_error(err); free_plan(p); return rc; }
     p->n_left = sectors->n_left;
+    p->n_right = sectors->n_right;
     if (!p->host_only) {
       rc = upload_schedule(p);
       if (rc != HPSI_OK) { free_plan(p); return rc; }
@@ -317,6 +318,8 @@ extern "C" int hpsi_query(const hpsi_plan_t* p, int what, void* out, size_t byte
     case HPSI_Q_INTERMEDIATE_BYTES: return put_i64(sc.intermediate_bytes);
     case HPSI_Q_PSI_ROWS: { int64_t n = 0; for (const PsiBlk& b : sc.blocks) n += b.rows; return put_i64(n); }
     case HPSI_Q_ISO_CAPACITY: { int64_t n = 0; for (const PsiBlk& b : sc.blocks) n += (int64_t)std::min(b.rows, b.cols) * b.rows; return put_i64(n); }
+    case HPSI_Q_PSI_COLS: { int64_t n = 0; for (const PsiBlk& b : sc.blocks) n += b.cols; return put_i64(n); }
+    case HPSI_Q_ISO_CAPACITY_RIGHT: { int64_t n = 0; for (const PsiBlk& b : sc.blocks) n += (int64_t)std::min(b.rows, b.cols) * b.cols; return put_i64(n); }
     case HPSI_Q_SVD_SWEEPS: return put_i64(p->svd_sweeps);
     case HPSI_Q_SVD_LAUNCHES: return put_i64(p->svd_launches);
     case HPSI_Q_TASKS: {

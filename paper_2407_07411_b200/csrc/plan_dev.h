@@ -26,7 +26,7 @@ struct hpsi_plan {
   int dav_mmax = 0;
   double* h_dav = nullptr;        // pinned host scalars the Davidson loop reads back each iteration
   // hpsi_truncate (svd.cu)
-  int n_left = 0;                 // left sectors of the sector table (length of chi_host)
+  int n_left = 0, n_right = 0;    // sectors of the sector table (length of chi_host for either side)
   void* d_svd = nullptr;          // working matrices, singular values, tables (allocated on first use)
   int svd_sweeps = 0, svd_launches = 0;   // of the last hpsi_truncate call (diagnostics)
 };

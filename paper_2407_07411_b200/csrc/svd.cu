@@ -31,9 +31,10 @@ namespace hpsi {
 struct SvdBlk {
   int64_t w_off;        // working matrix nv x L in the SVD workspace
   int64_t psi_off;      // block in psi (dense rows x cols)
-  int32_t rows, cols;   // of the psi block
+  int32_t rows, cols;   // of the block whose ROW space is truncated: the psi block (left side) or its transpose (right side)
   int32_t nv, vlen;     // vectors orthogonalised and their length: (rows, cols) if rows <= cols, else (cols, rows)
   int32_t tall;         // 1: rows > cols, the working matrix is the transposed block without the R part
+  int32_t pcols, rt;    // leading dimension of the block in psi; rt = 1: working vector i, element j is psi[j][i]
   int32_t L;            // leading dimension: vlen (+ rows for the R part) rounded up to 4
   int32_t nce;          // chunks, padded to an even count >= 2
   int32_t cta0;         // first CTA of this block in a round
@@ -51,7 +52,7 @@ __global__ void svd_init_kernel(SvdBlk* blk, const double* __restrict__ psi, dou
     double* row = w + B.w_off + (int64_t)i * B.L;
     for (int j = threadIdx.x; j < B.L; j += blockDim.x) {
       double v = 0.0;
-      if (j < B.vlen) v = B.tall ? psi[B.psi_off + (int64_t)j * B.cols + i] : psi[B.psi_off + (int64_t)i * B.cols + j];
+      if (j < B.vlen) v = B.rt ? psi[B.psi_off + (int64_t)j * B.pcols + i] : psi[B.psi_off + (int64_t)i * B.pcols + j];
       else if (!B.tall && j - B.vlen == i) v = 1.0;
       row[j] = v;
     }
@@ -190,15 +191,16 @@ __global__ void svd_gather_kernel(const IsoRow* __restrict__ rows, int n, const 
 
 using namespace hpsi;
 
-extern "C" int hpsi_truncate(hpsi_plan_t* p, const double* psi_dev, int32_t chi_max, double eps_discard, double* ot_dev,
-                             int32_t* chi_host, double* sigma_host, double* discarded_host, void* cuda_stream) {
+extern "C" int hpsi_truncate(hpsi_plan_t* p, const double* psi_dev, int32_t side, int32_t chi_max, double eps_discard,
+                             double* ot_dev, int32_t* chi_host, double* sigma_host, double* discarded_host, void* cuda_stream) {
   if (!p) { set_error("null plan"); return HPSI_EINVAL; }
   if (p->host_only) { set_error("host-only plan: hpsi_truncate needs a CUDA device (no CPU fallback)"); return HPSI_ESTATE; }
   if (chi_max < 0) { set_error("negative chi_max"); return HPSI_EINVAL; }
+  if (side != HPSI_SIDE_LEFT && side != HPSI_SIDE_RIGHT) { set_error("side must be HPSI_SIDE_LEFT or HPSI_SIDE_RIGHT"); return HPSI_EINVAL; }
   if (!chi_host) { set_error("null chi_host"); return HPSI_EINVAL; }
   const Schedule& sc = p->sc;
-  const int nL = p->n_left;
-  for (int i = 0; i < nL; ++i) chi_host[i] = 0;
+  const int n_sec = side == HPSI_SIDE_LEFT ? p->n_left : p->n_right;
+  for (int i = 0; i < n_sec; ++i) chi_host[i] = 0;
   if (discarded_host) *discarded_host = 0.0;
   const int nB = (int)sc.blocks.size();
   if (nB == 0) return HPSI_OK;
@@ -213,8 +215,11 @@ extern "C" int hpsi_truncate(hpsi_plan_t* p, const double* psi_dev, int32_t chi_
   for (int b = 0; b < nB; ++b) {
     const PsiBlk& B = sc.blocks[b];
     SvdBlk& s = tab[b];
-    s.w_off = wlen; s.psi_off = B.off; s.rows = B.rows; s.cols = B.cols;
-    s.tall = B.rows > B.cols ? 1 : 0;
+    s.w_off = wlen; s.psi_off = B.off; s.pcols = B.cols;
+    s.rows = side == HPSI_SIDE_LEFT ? B.rows : B.cols;       // the right side truncates the row space of psi_l^T
+    s.cols = side == HPSI_SIDE_LEFT ? B.cols : B.rows;
+    s.tall = s.rows > s.cols ? 1 : 0;
+    s.rt = s.tall ^ (side == HPSI_SIDE_LEFT ? 0 : 1);
     s.nv = std::min(B.rows, B.cols); s.vlen = std::max(B.rows, B.cols);
     s.L = s.tall ? sector_up(s.vlen) : sector_up(B.rows + B.cols);
     s.row0 = row0; s.floor2 = 0.0;
@@ -322,12 +327,16 @@ extern "C" int hpsi_truncate(hpsi_plan_t* p, const double* psi_dev, int32_t chi_
     if (!is_kept[i]) disc += cand[i].s * cand[i].s;
   if (discarded_host) *discarded_host = disc;
 
-  // ---- isometries in the boundary layout: sectors ascending, O_l^T = kept rows of R
+  // ---- isometries in the boundary layout: sectors of the chosen side ascending, O^T = kept vectors
+  std::vector<int> by_sector(nB);
+  std::iota(by_sector.begin(), by_sector.end(), 0);
+  if (side == HPSI_SIDE_RIGHT)                         // psi blocks are stored by ascending LEFT sector
+    std::sort(by_sector.begin(), by_sector.end(), [&](int x, int y) { return sc.blocks[x].right < sc.blocks[y].right; });
   std::vector<IsoRow> rows;
   int64_t dst = 0;
-  for (int b = 0; b < nB; ++b) {                       // psi blocks are in ascending left-sector order
+  for (int b : by_sector) {
     const SvdBlk& s = tab[b];
-    chi_host[sc.blocks[b].left] = (int32_t)kept[b].size();
+    chi_host[side == HPSI_SIDE_LEFT ? sc.blocks[b].left : sc.blocks[b].right] = (int32_t)kept[b].size();
     for (int row : kept[b]) {
       if (s.tall) rows.push_back({s.w_off + (int64_t)row * s.L, dst, 1.0 / sig[s.row0 + row], s.rows, 0});
       else rows.push_back({s.w_off + (int64_t)row * s.L + s.cols, dst, 1.0, s.rows, 0});

@@ -87,6 +87,30 @@ def test_rotate_stress_shapes_sampled():
     assert np.sqrt(num / den) <= 1e-12
 
 
+def test_rotate_right_operators_with_right_isometries():
+    """A left-moving sweep: right isometries from hpsi_truncate(HPSI_SIDE_RIGHT) rotate the B blocks (the update is
+    side-agnostic: sector dims, kept dims, descriptors, arena)."""
+    torch, H = _gpu()
+    p = workloads.make_problem("small", n_terms=40)
+    psi = workloads.make_psi(p)
+    a, b = torch.from_numpy(p.a_data).cuda(), torch.from_numpy(p.b_data).cuda()
+    plan = H.plan_problem(p, a, b)
+    ot = torch.zeros(H.hpsi_query(plan, H.HPSI_Q_ISO_CAPACITY_RIGHT), dtype=torch.float64, device="cuda:0")
+    chi, sigma, disc = H.hpsi_truncate(plan, torch.from_numpy(psi).cuda(), 300, ot, torch.cuda.current_stream(), -1.0, H.HPSI_SIDE_RIGHT)
+    assert chi.shape[0] == p.q_right.shape[0] and int(chi.sum()) == 300
+    r = H.hpsi_rotate_plan(p.d_right, chi, p.b_desc, b, p.b_len)
+    out = torch.full((H.hpsi_rotate_query(r, H.HPSI_RQ_OUT_LENGTH),), float("nan"), dtype=torch.float64, device="cuda:0")
+    H.hpsi_rotate_apply(r, ot, out, torch.cuda.current_stream())
+    torch.cuda.synchronize()
+    oth, ots, o = ot.cpu().numpy(), [], 0
+    for l in range(len(chi)):
+        n = int(chi[l]) * int(p.d_right[l])
+        ots.append(oth[o:o + n].reshape(int(chi[l]), int(p.d_right[l])))
+        o += n
+    err = compare_blocks(H, r, out.cpu().numpy(), chi, su.rotate(p.d_right, chi, p.b_desc, p.b_data, ots))
+    assert err <= 1e-12, err
+
+
 def test_rotate_nothing_survives():
     torch, H = _gpu()
     p = workloads.make_problem("toy")
@@ -98,33 +122,42 @@ def test_rotate_nothing_survives():
 
 
 # ------------------------------------------------------------------------------------------ truncate
-def run_truncate(p, psi, chi_max, eps=-1.0):
+def run_truncate(p, psi, chi_max, eps=-1.0, side="left"):
     torch, H = _gpu()
     a = torch.from_numpy(p.a_data).cuda()
     b = torch.from_numpy(p.b_data).cuda()
     plan = H.plan_problem(p, a, b)
     x = torch.from_numpy(np.ascontiguousarray(psi)).cuda()
-    ot = torch.full((max(H.hpsi_query(plan, H.HPSI_Q_ISO_CAPACITY), 1),), float("nan"), dtype=torch.float64, device="cuda:0")
-    chi, sigma, disc = H.hpsi_truncate(plan, x, chi_max, ot, torch.cuda.current_stream(), eps)
+    cap = H.hpsi_query(plan, H.HPSI_Q_ISO_CAPACITY_RIGHT if side == "right" else H.HPSI_Q_ISO_CAPACITY)
+    ot = torch.full((max(cap, 1),), float("nan"), dtype=torch.float64, device="cuda:0")
+    chi, sigma, disc = H.hpsi_truncate(plan, x, chi_max, ot, torch.cuda.current_stream(), eps,
+                                       H.HPSI_SIDE_RIGHT if side == "right" else H.HPSI_SIDE_LEFT)
     assert np.array_equal(x.cpu().numpy(), psi)                          # psi is not modified
     return plan, chi, sigma, disc, ot.cpu().numpy(), H
 
 
-def check_truncation(p, psi, chi_max, proj_tol=1e-9, eps=-1.0):
-    plan, chi, sigma, disc, ot, H = run_truncate(p, psi, chi_max, eps)
-    chi_ref, ot_ref, sigma_ref, disc_ref = su.truncate(p, psi, chi_max, eps)
+def check_truncation(p, psi, chi_max, proj_tol=1e-9, eps=-1.0, side="left"):
+    plan, chi, sigma, disc, ot, H = run_truncate(p, psi, chi_max, eps, side)
+    chi_ref, ot_ref, sigma_ref, disc_ref = su.truncate(p, psi, chi_max, eps, side)
     assert np.array_equal(chi, chi_ref)
     smax = max(float(s[0]) for s in sigma_ref if s.size)
-    row0 = iso0 = 0
-    for (i, j, r, c, off) in p.psi_blocks():
+    row0 = 0
+    blocks = p.psi_blocks()
+    if side == "right":      # effective blocks psi_l^T, sector = the right one; isometries are laid out by ascending sector
+        blocks = [(j, i, c, r, off) for (i, j, r, c, off) in blocks]
+    iso_off, o = {}, 0
+    for sec in sorted(b[0] for b in blocks):
+        iso_off[sec] = o
+        o += int(chi[sec]) * int((p.d_right if side == "right" else p.d_left)[sec])
+    for (i, j, r, c, off) in blocks:
+        iso0 = iso_off[i]
         s_gpu = sigma[row0:row0 + r]
         row0 += r
         k = min(r, c)
         np.testing.assert_allclose(s_gpu[:k], sigma_ref[i], rtol=0, atol=1e-12 * smax)
         assert np.all(s_gpu[k:] == 0.0)
         O = ot[iso0:iso0 + int(chi[i]) * r].reshape(int(chi[i]), r)
-        iso0 += int(chi[i]) * r
-        blk = psi[off:off + r * c].reshape(r, c)
+        blk = psi[off:off + r * c].reshape(c, r).T if side == "right" else psi[off:off + r * c].reshape(r, c)
         np.testing.assert_allclose(O @ O.T, np.eye(O.shape[0]), atol=1e-12)            # orthonormal rows
         # row a is a left singular vector with singular value sigma_a:  || O psi ||_row = sigma,  O psi psi^T = sigma^2 O
         np.testing.assert_allclose(np.linalg.norm(O @ blk, axis=1), sigma_ref[i][:O.shape[0]], atol=1e-12 * smax)
@@ -145,6 +178,12 @@ def test_truncate_matches_oracle(name, chi_max):
 def test_truncate_by_discarded_weight_matches_oracle(eps, chi_max):
     p = workloads.make_problem("small", n_terms=8)
     check_truncation(p, workloads.make_psi(p), chi_max, eps=eps)
+
+
+@pytest.mark.parametrize("name,chi_max,eps", [("toy", 12, -1.0), ("small", 256, -1.0), ("small", 10 ** 6, 1e-2)])
+def test_truncate_right_side_matches_oracle(name, chi_max, eps):
+    p = workloads.make_problem(name, n_terms=8)
+    check_truncation(p, workloads.make_psi(p), chi_max, eps=eps, side="right")
 
 
 def test_truncate_cyp_sized_blocks_and_reproducible():

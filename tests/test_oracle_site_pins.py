@@ -116,6 +116,25 @@ def test_truncate_against_density_matrix_and_eckart_young(name, chi_max):
     assert abs(dw - np.sum(np.sort(allsig ** 2)[::-1][chi_max:])) <= 1e-13
 
 
+def test_truncate_right_side(small):
+    """Right basis: rows of O_r^T are eigenvectors of psi_l^T psi_l; the singular values - hence the kept total and the
+    discarded weight - are those of the left-side truncation."""
+    p = small
+    psi = workloads.make_psi(p)
+    chiL, _, sigL, dwL = su.truncate(p, psi, 200)
+    chiR, otR, sigR, dwR = su.truncate(p, psi, 200, side="right")
+    assert chiR.shape[0] == p.q_right.shape[0] and int(chiR.sum()) == int(chiL.sum()) == 200
+    assert abs(dwL - dwR) <= 1e-14
+    for (i, j, r, c, off) in p.psi_blocks():
+        blk = psi[off:off + r * c].reshape(r, c)
+        assert chiR[j] == chiL[i]
+        np.testing.assert_allclose(sigR[j], sigL[i], atol=1e-14)
+        O = otR[j]
+        assert O.shape == (chiR[j], c)
+        np.testing.assert_allclose(O @ O.T, np.eye(O.shape[0]), atol=1e-13)
+        np.testing.assert_allclose(O @ (blk.T @ blk), (sigR[j][:O.shape[0]] ** 2)[:, None] * O, atol=1e-13)
+
+
 def test_truncate_sector_without_block_and_wide_block():
     # left sector 1 has no partner; block of sector 0 is 2 x 5 (more columns than rows), of sector 2 is 4 x 2
     p = workloads.custom_problem([(0, 0), (7, 0), (1, 0)], [2, 3, 4], [(2, 0), (1, 0)], [5, 2], (2, 0), [])
