@@ -240,3 +240,55 @@ def test_site_update_pipeline_truncate_then_rotate():
         o += n
     err = compare_blocks(H, r, out.cpu().numpy(), chi, su.rotate(p.d_left, chi, p.a_desc, p.a_data, ots))
     assert err <= 1e-12, err
+
+
+def test_rotated_arena_feeds_the_next_plan():
+    """The output arena + HPSI_RQ_OUT_BLOCKS of hpsi_rotate_apply are used, unchanged, as the A arena of a new hpsi_plan
+    over the truncated left basis; applying it to phi must equal projecting the full apply:
+    H' phi = (O^T (x) 1) H (O (x) 1) phi   (all three applies and the update on the device, isometries from hpsi_truncate)."""
+    torch, H = _gpu()
+    p = workloads.make_problem("small", n_terms=60)
+    psi = workloads.make_psi(p)
+    a, b = torch.from_numpy(p.a_data).cuda(), torch.from_numpy(p.b_data).cuda()
+    plan = H.plan_problem(p, a, b)
+    st = torch.cuda.current_stream()
+    ot = torch.zeros(H.hpsi_query(plan, H.HPSI_Q_ISO_CAPACITY), dtype=torch.float64, device="cuda:0")
+    chi, _, _ = H.hpsi_truncate(plan, torch.from_numpy(psi).cuda(), 200, ot, st)
+    rot = H.hpsi_rotate_plan(p.d_left, chi, p.a_desc, a, p.a_len)
+    arena2 = torch.zeros(H.hpsi_rotate_query(rot, H.HPSI_RQ_OUT_LENGTH), dtype=torch.float64, device="cuda:0")
+    H.hpsi_rotate_apply(rot, ot, arena2, st)
+    desc2 = H.hpsi_rotate_query(rot, H.HPSI_RQ_OUT_BLOCKS)
+    # new sector table: the left sectors that kept something, renumbered; right side unchanged
+    keep = np.flatnonzero(chi > 0)
+    renum = -np.ones(len(chi), np.int64); renum[keep] = np.arange(len(keep))
+    d2 = desc2[desc2["offset"] >= 0].copy()
+    d2["row"] = renum[d2["row"]]; d2["col"] = renum[d2["col"]]
+    plan2 = H.hpsi_plan(p.q_left[keep], p.q_right, chi[keep], p.d_right, p.target, p.coef, d2, p.b_desc, arena2, b,
+                        arena2.numel(), p.b_len)
+    assert H.hpsi_query(plan2, H.HPSI_Q_ALIGNED16) == 1                       # the dictated layout takes the TMA path
+    blocks2 = H.hpsi_query(plan2, H.HPSI_Q_PSI_BLOCKS)
+    rng = np.random.default_rng(77)
+    phi = rng.standard_normal(H.hpsi_query(plan2, H.HPSI_Q_PSI_LENGTH))
+    oth, ots, o = ot.cpu().numpy(), {}, 0
+    for l in range(len(chi)):
+        n = int(chi[l]) * int(p.d_left[l])
+        ots[l] = oth[o:o + n].reshape(int(chi[l]), int(p.d_left[l]))
+        o += n
+    full_blocks = {i: (r, c, off) for (i, j, r, c, off) in p.psi_blocks()}
+    lifted = np.zeros(p.psi_len)
+    for e in blocks2:
+        l = int(keep[e["left"]])
+        r, c, off = full_blocks[l]
+        lifted[off:off + r * c] = (ots[l].T @ phi[int(e["offset"]):int(e["offset"]) + int(e["rows"]) * c].reshape(int(e["rows"]), c)).ravel()
+    x = torch.from_numpy(lifted).cuda(); y = torch.empty_like(x)
+    H.hpsi_apply(plan, x, y, st)
+    x2 = torch.from_numpy(phi).cuda(); y2 = torch.empty_like(x2)
+    H.hpsi_apply(plan2, x2, y2, st)
+    torch.cuda.synchronize()
+    hl, got = y.cpu().numpy(), y2.cpu().numpy()
+    proj = np.zeros_like(phi)
+    for e in blocks2:
+        l = int(keep[e["left"]])
+        r, c, off = full_blocks[l]
+        proj[int(e["offset"]):int(e["offset"]) + int(e["rows"]) * c] = (ots[l] @ hl[off:off + r * c].reshape(r, c)).ravel()
+    assert np.linalg.norm(got - proj) <= 1e-12 * np.linalg.norm(proj)
