@@ -168,7 +168,7 @@ void hpsi_stream_destroy(hpsi_stream_t* s);
 /* ------------------------------------------------------------------------------------------------------------------
  * Site update after the eigen-solve.  PAPER.md:45 names "tensor contraction and matrix
  * factorization" as the two core operations of tensor-network algorithms and PAPER.md:62 the sweep as a "sequence of
- * updates of all tensors", but writes out neither step; DESIGN.md section 9 lists the readings R1-R5.
+ * updates of all tensors", but writes out neither step; DESIGN.md section 9 lists the readings R1-R6.
  *
  *   hpsi_truncate :  the matrix factorisation.  psi is block diagonal over (left sector l, partner r), so its SVD is
  *                    the SVD of every block, psi_l = U_l S_l V_l^T.  The chi_max largest singular values over all
@@ -190,12 +190,14 @@ void hpsi_stream_destroy(hpsi_stream_t* s);
  *   eps_discard    if >= 0: keep only as many of them as it takes for the discarded weight to be <= eps_discard
  *                  (the paper quotes its results by "truncation error"); < 0: keep chi_max
  *   ot_dev         DEVICE, receives the isometries in the layout above; capacity >= HPSI_Q_ISO_CAPACITY doubles
+ *                  (HPSI_Q_ISO_CAPACITY_RIGHT for the right side)
  *   chi_host       HOST, int32[n_left] (n_right for the right side): kept states per sector (0 without a psi block)
  *   sigma_host     HOST or NULL, psi-rows doubles (HPSI_Q_PSI_ROWS = sum of d_left over the psi blocks): for every psi
  *                  block in table order its d_left values, descending; entries past min(d_left, d_right) are 0
  *   discarded_host HOST or NULL: sum of sigma^2 over everything not kept
  * Synchronises the stream (chi is needed on the host).  Deterministic (fixed rotation order; the only atomic is the
- * sweep's "anything rotated" flag).  Errors: EINVAL (null / negative arguments), ESTATE (host-only plan), ENOMEM, ECUDA. */
+ * sweep's rotation counter, which steers nothing but the stop test).  A psi block whose rows + columns exceed ~12 000
+ * does not fit the shared-memory kernel (EINVAL).  Errors: EINVAL (null / negative arguments), ESTATE (host-only plan), ENOMEM, ECUDA. */
 #define HPSI_SIDE_LEFT  0
 #define HPSI_SIDE_RIGHT 1
 int hpsi_truncate(hpsi_plan_t* plan, const double* psi_dev, int32_t side, int32_t chi_max, double eps_discard,
