@@ -28,6 +28,7 @@ struct hpsi_plan {
   // hpsi_truncate (svd.cu)
   int n_left = 0, n_right = 0;    // sectors of the sector table (length of chi_host for either side)
   void* d_svd = nullptr;          // working matrices, singular values, tables (allocated on first use)
+  size_t svd_bytes = 0;
   int svd_sweeps = 0, svd_launches = 0;   // of the last hpsi_truncate call (diagnostics)
 };
 

@@ -244,12 +244,19 @@ extern "C" int hpsi_truncate(hpsi_plan_t* p, const double* psi_dev, int32_t side
   }
   const size_t smem = (size_t)2 * bsz * Lmax * 8;
 
-  // ---- device buffers (kept on the plan; sizes depend on the plan only)
-  if (!p->d_svd) {
-    size_t bytes = (size_t)wlen * 8 + (size_t)n_rows * 8 + tab.size() * sizeof(SvdBlk) + cta_blk.size() * 4 + (size_t)n_rows * sizeof(IsoRow) + 4096;
-    cudaError_t e = cudaMalloc(&p->d_svd, bytes);
-    if (e != cudaSuccess) { cudaGetLastError(); set_error("hpsi_truncate: device workspace allocation failed"); return HPSI_ENOMEM; }
-    HPSI_CUDA(cudaFuncSetAttribute(svd_round_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, SVD_SMEM_BUDGET));
+  // ---- device buffers (kept on the plan; regrown if a call needs more, e.g. the other side)
+  {
+    const size_t bytes = (size_t)wlen * 8 + (size_t)n_rows * 8 + tab.size() * sizeof(SvdBlk) + cta_blk.size() * 4 + (size_t)n_rows * sizeof(IsoRow) + 4096;
+    if (bytes > p->svd_bytes) {
+      HPSI_CUDA(cudaStreamSynchronize(st));
+      cudaFree(p->d_svd);
+      p->d_svd = nullptr;
+      p->svd_bytes = 0;
+      cudaError_t e = cudaMalloc(&p->d_svd, bytes);
+      if (e != cudaSuccess) { cudaGetLastError(); set_error("hpsi_truncate: device workspace allocation failed"); return HPSI_ENOMEM; }
+      p->svd_bytes = bytes;
+      HPSI_CUDA(cudaFuncSetAttribute(svd_round_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, SVD_SMEM_BUDGET));
+    }
   }
   char* base = static_cast<char*>(p->d_svd);
   size_t cur = 0;

@@ -186,6 +186,26 @@ def test_truncate_right_side_matches_oracle(name, chi_max, eps):
     check_truncation(p, workloads.make_psi(p), chi_max, eps=eps, side="right")
 
 
+def test_truncate_both_sides_on_one_plan():
+    """The plan's SVD workspace is regrown when the other side needs more; results do not depend on call history."""
+    torch, H = _gpu()
+    p = workloads.make_problem("small", n_terms=8)
+    psi = workloads.make_psi(p)
+    plan = H.plan_problem(p, torch.from_numpy(p.a_data).cuda(), torch.from_numpy(p.b_data).cuda())
+    x = torch.from_numpy(psi).cuda()
+    otl = torch.zeros(H.hpsi_query(plan, H.HPSI_Q_ISO_CAPACITY), dtype=torch.float64, device="cuda:0")
+    otr = torch.zeros(H.hpsi_query(plan, H.HPSI_Q_ISO_CAPACITY_RIGHT), dtype=torch.float64, device="cuda:0")
+    st = torch.cuda.current_stream()
+    c1, s1, d1 = H.hpsi_truncate(plan, x, 128, otl, st)
+    first = otl.clone()
+    cr, sr, dr = H.hpsi_truncate(plan, x, 128, otr, st, -1.0, H.HPSI_SIDE_RIGHT)
+    c2, s2, d2 = H.hpsi_truncate(plan, x, 128, otl, st)
+    assert np.array_equal(c1, c2) and np.array_equal(s1, s2) and d1 == d2 and torch.equal(first, otl)
+    assert int(cr.sum()) == int(c1.sum()) == 128 and abs(dr - d1) <= 1e-13
+    for (i, j, r, c, off) in p.psi_blocks():
+        assert cr[j] == c1[i]
+
+
 def test_truncate_cyp_sized_blocks_and_reproducible():
     """Full-size sector dims of the metric's config (blocks up to ~350 x 350: several chunk pairs, many rounds)."""
     p = workloads.make_problem("cyp", n_terms=2)
