@@ -12,11 +12,17 @@ namespace {
 constexpr int NB = 256;       // partial blocks per dot product
 constexpr int MMAX = 32;
 
-// partial[v*NB + b] = sum over block b's slice of X_v[e] * y[e]
-__global__ void dot_partial_kernel(const double* __restrict__ X, int64_t ldx, const double* __restrict__ y, int64_t n,
-                                   double* __restrict__ partial) {
+// out[v*stride] (and mirror[v*mstride] if given) = X_v . y for the nvec vectors X_v = X + v*ldx.
+// Two stages in one launch: block (b, v) reduces its slice into partial[v][b]; the block that finishes last for vector v
+// (ticket from an atomic counter - control only) adds the NB partials in a fixed order, so the result does not depend
+// on which block that is and a run is bitwise reproducible.  The counter is left at zero for the next call.
+__global__ void dot_kernel(const double* __restrict__ X, int64_t ldx, const double* __restrict__ y, int64_t n,
+                           double* __restrict__ partial, unsigned int* __restrict__ counters, double* out, int stride,
+                           double* mirror, int mstride) {
   __shared__ double red[256];
-  const double* x = X + (int64_t)blockIdx.y * ldx;
+  __shared__ bool last;
+  const int v = blockIdx.y;
+  const double* x = X + (int64_t)v * ldx;
   const int64_t per = (n + NB - 1) / NB;
   const int64_t lo = (int64_t)blockIdx.x * per, hi = (lo + per < n) ? lo + per : n;
   double s = 0.0;
@@ -27,17 +33,24 @@ __global__ void dot_partial_kernel(const double* __restrict__ X, int64_t ldx, co
     if ((int)threadIdx.x < w) red[threadIdx.x] += red[threadIdx.x + w];
     __syncthreads();
   }
-  if (threadIdx.x == 0) partial[blockIdx.y * NB + blockIdx.x] = red[0];
-}
-// out[v*stride] (and mirror[v*mstride] if given) = sum_b partial[v][b], b ascending
-__global__ void dot_final_kernel(const double* __restrict__ partial, int nvec, double* out, int stride, double* mirror,
-                                 int mstride) {
-  const int v = threadIdx.x;
-  if (v >= nvec) return;
-  double s = 0.0;
-  for (int b = 0; b < NB; ++b) s += partial[v * NB + b];
-  out[(int64_t)v * stride] = s;
-  if (mirror) mirror[(int64_t)v * mstride] = s;
+  if (threadIdx.x == 0) {
+    partial[v * NB + blockIdx.x] = red[0];
+    __threadfence();
+    last = atomicAdd(counters + v, 1u) == NB - 1;
+  }
+  __syncthreads();
+  if (!last || threadIdx.x >= 32) return;
+  __threadfence();
+  double t = 0.0;                                        // lane l: partials 8l .. 8l+7 in order, then a fixed shuffle tree
+  const volatile double* pv = partial + v * NB + threadIdx.x * (NB / 32);
+  for (int i = 0; i < NB / 32; ++i) t += pv[i];
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) t += __shfl_xor_sync(0xffffffffu, t, o);
+  if (threadIdx.x == 0) {
+    out[(int64_t)v * stride] = t;
+    if (mirror) mirror[(int64_t)v * mstride] = t;
+    counters[v] = 0;
+  }
 }
 
 // dst = src / sqrt(*nrm2)   (dst2 = src2 / sqrt(*nrm2) if given)
@@ -50,53 +63,76 @@ __global__ void scale_kernel(double* dst, const double* src, double* dst2, const
   }
 }
 
-// Smallest eigenpair of the symmetric j x j matrix G (leading dimension MMAX) by cyclic Jacobi, one warp.
-// Writes theta[0] and y[0..j).  G itself is left untouched (work copy in shared memory).
+// Smallest eigenpair of the symmetric j x j matrix G (leading dimension MMAX) by parallel two-sided Jacobi: the j/2
+// disjoint rotations of a round-robin round are applied together, warp k = pair k, lane t = row t (blockDim.x =
+// 32 * ceil(j/2)); first all column updates A J, then all row updates J^T (A J).  (A one-warp cyclic version took 86 us per
+// call at j ~ 10 - a quarter of a Davidson iteration's fixed cost.)  Writes theta[0] and y[0..j); G is left untouched.
 __global__ void small_eig_kernel(const double* __restrict__ G, int j, double* theta, double* y) {
   __shared__ double A[MMAX][MMAX + 1], Q[MMAX][MMAX + 1];
-  const int t = threadIdx.x;
-  for (int c = 0; c < j; ++c)
+  __shared__ double norms[2];
+  const int t = threadIdx.x & 31, k = threadIdx.x >> 5;
+  const int m = (j + 1) & ~1;                            // players of the round-robin (a dummy one if j is odd)
+  const int np = m > 1 ? m / 2 : 1;                      // = warps in the block
+  for (int c = k; c < j; c += np)
     if (t < j) { A[t][c] = 0.5 * (G[t * MMAX + c] + G[c * MMAX + t]); Q[t][c] = (t == c) ? 1.0 : 0.0; }
-  __syncwarp();
-  for (int sweep = 0; sweep < 30; ++sweep) {
-    double off = 0.0, dg = 0.0;
-    for (int p = 0; p < j; ++p) {
-      dg += A[p][p] * A[p][p];
-      for (int q = p + 1; q < j; ++q) off += A[p][q] * A[p][q];
-    }
-    if (off <= 1e-34 * (dg + 2.0 * off) || off < 1e-300) break;   // off-diagonal norm below 1e-17 of the matrix norm
-    for (int p = 0; p < j - 1; ++p)
-      for (int q = p + 1; q < j; ++q) {
-        const double apq = A[p][q];
-        if (fabs(apq) < 1e-300) continue;                 // uniform: every lane reads the same value
-        const double app = A[p][p], aqq = A[q][q];
-        const double tau = (aqq - app) / (2.0 * apq);
-        const double tt = (tau >= 0 ? 1.0 : -1.0) / (fabs(tau) + sqrt(1.0 + tau * tau));
-        const double c = 1.0 / sqrt(1.0 + tt * tt), s = tt * c;
-        __syncwarp();
-        if (t < j) {                                      // columns p,q
-          const double akp = A[t][p], akq = A[t][q];
-          A[t][p] = c * akp - s * akq;
-          A[t][q] = s * akp + c * akq;
-          const double qkp = Q[t][p], qkq = Q[t][q];
-          Q[t][p] = c * qkp - s * qkq;
-          Q[t][q] = s * qkp + c * qkq;
-        }
-        __syncwarp();
-        if (t < j) {                                      // rows p,q
-          const double apk = A[p][t], aqk = A[q][t];
-          A[p][t] = c * apk - s * aqk;
-          A[q][t] = s * apk + c * aqk;
-        }
-        __syncwarp();
+  __syncthreads();
+  for (int sweep = 0; sweep < 30 && j > 1; ++sweep) {
+    if (k == 0) {                                        // squared norms of the off-diagonal part and of the diagonal
+      double off = 0.0, dg = 0.0;
+      if (t < j) {
+        dg = A[t][t] * A[t][t];
+        for (int q = t + 1; q < j; ++q) off += A[t][q] * A[t][q];
       }
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) { off += __shfl_xor_sync(0xffffffffu, off, o); dg += __shfl_xor_sync(0xffffffffu, dg, o); }
+      if (t == 0) { norms[0] = off; norms[1] = dg; }
+    }
+    __syncthreads();
+    const double off = norms[0], dg = norms[1];
+    if (off <= 1e-34 * (dg + 2.0 * off) || off < 1e-300) break;   // off-diagonal norm below 1e-17 of the matrix norm
+    for (int r = 0; r < m - 1; ++r) {
+      int p, q;
+      if (k == 0) { p = m - 1; q = r; }
+      else { p = (r + k) % (m - 1); q = (r - k + m - 1) % (m - 1); }
+      if (p > q) { const int tmp = p; p = q; q = tmp; }
+      double c = 1.0, sn = 0.0;
+      if (q < j) {                                       // not the dummy player
+        const double apq = A[p][q];
+        if (fabs(apq) >= 1e-300) {
+          const double app = A[p][p], aqq = A[q][q];
+          const double tau = (aqq - app) / (2.0 * apq);
+          const double tt = (tau >= 0 ? 1.0 : -1.0) / (fabs(tau) + sqrt(1.0 + tau * tau));
+          c = 1.0 / sqrt(1.0 + tt * tt);
+          sn = tt * c;
+        }
+      }
+      __syncwarp();
+      const bool act = sn != 0.0 && t < j;
+      if (act) {                                         // columns p, q (this warp's alone)
+        const double akp = A[t][p], akq = A[t][q];
+        A[t][p] = c * akp - sn * akq;
+        A[t][q] = sn * akp + c * akq;
+        const double qkp = Q[t][p], qkq = Q[t][q];
+        Q[t][p] = c * qkp - sn * qkq;
+        Q[t][q] = sn * qkp + c * qkq;
+      }
+      __syncthreads();
+      if (act) {                                         // rows p, q
+        const double apk = A[p][t], aqk = A[q][t];
+        A[p][t] = c * apk - sn * aqk;
+        A[q][t] = sn * apk + c * aqk;
+      }
+      __syncthreads();
+    }
   }
-  __syncwarp();
-  int best = 0;
-  for (int i = 1; i < j; ++i)
-    if (A[i][i] < A[best][best]) best = i;
-  if (t == 0) theta[0] = A[best][best];
-  if (t < j) y[t] = Q[t][best];
+  __syncthreads();
+  if (k == 0) {
+    int best = 0;
+    for (int i = 1; i < j; ++i)
+      if (A[i][i] < A[best][best]) best = i;
+    if (t == 0) theta[0] = A[best][best];
+    if (t < j) y[t] = Q[t][best];
+  }
 }
 
 // x = sum_i y_i V_i ; wy = sum_i y_i W_i ; r = wy - theta x
@@ -152,8 +188,8 @@ extern "C" int hpsi_davidson(hpsi_plan_t* p, double* psi, double* eig_host, cons
   if (n == 0) { set_error("empty target sector"); return HPSI_EINVAL; }
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
 
-  // buffers: V[m][n] W[m][n] diag x wy r s | G[MMAX*MMAX] y[MMAX] c[MMAX] theta nrm[4] partial[MMAX*NB]
-  const size_t small = MMAX * MMAX + 2 * MMAX + 8 + MMAX * NB;
+  // buffers: V[m][n] W[m][n] diag x wy r s | G[MMAX*MMAX] y[MMAX] c[MMAX] theta nrm[4] partial[MMAX*NB] counters[MMAX]
+  const size_t small = MMAX * MMAX + 2 * MMAX + 8 + MMAX * NB + MMAX;
   const size_t need = (size_t)(2 * prm.m_max + 5) * n + small;
   if (p->dav_doubles < need) {
     cudaFree(p->d_dav);
@@ -173,12 +209,12 @@ extern "C" int hpsi_davidson(hpsi_plan_t* p, double* psi, double* eig_host, cons
   double *x = diag + n, *wy = x + n, *r = wy + n, *s = r + n;
   double* G = s + n;
   double *y = G + MMAX * MMAX, *c = y + MMAX, *theta = c + MMAX, *nrm = theta + 1, *partial = nrm + 7;
+  unsigned int* counters = reinterpret_cast<unsigned int*>(partial + MMAX * NB);
   HPSI_CUDA(cudaMemsetAsync(G, 0, small * sizeof(double), st));
 
   const int eg = (int)std::min<int64_t>((n + 255) / 256, 2048);
   auto dots = [&](const double* X, int nvec, const double* yv, double* out, int stride, double* mirror, int mstride) {
-    dot_partial_kernel<<<dim3(NB, nvec), 256, 0, st>>>(X, n, yv, n, partial);
-    dot_final_kernel<<<1, MMAX, 0, st>>>(partial, nvec, out, stride, mirror, mstride);
+    dot_kernel<<<dim3(NB, nvec), 256, 0, st>>>(X, n, yv, n, partial, counters, out, stride, mirror, mstride);
   };
   int rc;
   if (prm.precondition && (rc = hpsi_diagonal(p, diag, cuda_stream)) != HPSI_OK) return rc;
@@ -192,7 +228,7 @@ extern "C" int hpsi_davidson(hpsi_plan_t* p, double* psi, double* eig_host, cons
   for (int it = 0; it < prm.max_iter; ++it) {
     // new column of G = V^T W:  G[i][j-1] = G[j-1][i] = V_i . W_{j-1}
     dots(V, j, W + (size_t)(j - 1) * n, G + (j - 1), MMAX, G + (size_t)(j - 1) * MMAX, 1);
-    small_eig_kernel<<<1, 32, 0, st>>>(G, j, theta, y);
+    small_eig_kernel<<<1, 32 * std::max(1, (j + 1) / 2), 0, st>>>(G, j, theta, y);
     ritz_kernel<<<eg, 256, 0, st>>>(V, W, n, j, y, theta, x, wy, r);
     dots(r, 1, r, nrm + 1, 1, nullptr, 0);                          // nrm[1] = |r|^2
     precond_kernel<<<eg, 256, 0, st>>>(r, diag, theta, prm.precondition, s, n);
@@ -267,8 +303,8 @@ extern "C" int hpsi_lanczos(hpsi_plan_t* p, double* psi, double* eig_host, const
   if (n == 0) { set_error("empty target sector"); return HPSI_EINVAL; }
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
 
-  // buffers: V[m][n] x w | T[MMAX*MMAX] y[MMAX] c[MMAX] c2[MMAX] theta nrm[7] partial[MMAX*NB]
-  const size_t small = MMAX * MMAX + 3 * MMAX + 8 + MMAX * NB;
+  // buffers: V[m][n] x w | T[MMAX*MMAX] y[MMAX] c[MMAX] c2[MMAX] theta nrm[7] partial[MMAX*NB] counters[MMAX]
+  const size_t small = MMAX * MMAX + 3 * MMAX + 8 + MMAX * NB + MMAX;
   const size_t need = (size_t)(prm.m_max + 2) * n + small;
   if (p->dav_doubles < need) {
     cudaFree(p->d_dav);
@@ -287,11 +323,11 @@ extern "C" int hpsi_lanczos(hpsi_plan_t* p, double* psi, double* eig_host, const
   double* w = x + n;
   double* T = w + n;
   double *y = T + MMAX * MMAX, *c = y + MMAX, *c2 = c + MMAX, *theta = c2 + MMAX, *nrm = theta + 1, *partial = nrm + 7;
+  unsigned int* counters = reinterpret_cast<unsigned int*>(partial + MMAX * NB);
   HPSI_CUDA(cudaMemsetAsync(T, 0, small * sizeof(double), st));
   const int eg = (int)std::min<int64_t>((n + 255) / 256, 2048);
   auto dots = [&](const double* X, int nvec, const double* yv, double* out) {
-    dot_partial_kernel<<<dim3(NB, nvec), 256, 0, st>>>(X, n, yv, n, partial);
-    dot_final_kernel<<<1, MMAX, 0, st>>>(partial, nvec, out, 1, nullptr, 0);
+    dot_kernel<<<dim3(NB, nvec), 256, 0, st>>>(X, n, yv, n, partial, counters, out, 1, nullptr, 0);
   };
   int rc;
   dots(psi, 1, psi, nrm);
@@ -308,7 +344,7 @@ extern "C" int hpsi_lanczos(hpsi_plan_t* p, double* psi, double* eig_host, const
     project_kernel<<<eg, 256, 0, st>>>(w, V, n, j + 1, c2);          // second Gram-Schmidt pass
     dots(w, 1, w, nrm + 3);                                          // beta_j^2
     lanczos_set_kernel<<<1, 1, 0, st>>>(T, j, c + j, nrm + 3);
-    small_eig_kernel<<<1, 32, 0, st>>>(T, j + 1, theta, y);
+    small_eig_kernel<<<1, 32 * std::max(1, (j + 2) / 2), 0, st>>>(T, j + 1, theta, y);
     HPSI_CUDA(cudaMemcpyAsync(host, theta, sizeof(double), cudaMemcpyDeviceToHost, st));
     HPSI_CUDA(cudaMemcpyAsync(host + 1, y + j, sizeof(double), cudaMemcpyDeviceToHost, st));
     HPSI_CUDA(cudaMemcpyAsync(host + 2, nrm + 3, sizeof(double), cudaMemcpyDeviceToHost, st));
