@@ -88,7 +88,7 @@ class ClockSampler:
 def dgemm_calibration(torch, secs=1.0):
     """Same-run FP64 tensor-core peak: cuBLAS DGEMM (torch.matmul on float64), best sustained 2N^3/t (north_star)."""
     best, detail = 0.0, {}
-    for N in (4096, 8192):
+    for N in (4096, 8192, 16384):
         a = torch.randn(N, N, dtype=torch.float64, device="cuda")
         b = torch.randn(N, N, dtype=torch.float64, device="cuda")
         c = torch.empty_like(a)
@@ -412,6 +412,8 @@ def run_ours(args, rank, world, local_rank):
     dgemm_peak, calib = dgemm_calibration(torch)
     ms_pipe, fl_pipe = H.hpsi_bench_fp64_pipe(0, 20000)
     calib["dmma_pipe_probe"] = round(fl_pipe / ms_pipe / 1e9, 3)
+    ms_pipe, fl_pipe = H.hpsi_bench_fp64_pipe(1, 20000)
+    calib["dfma_pipe_probe"] = round(fl_pipe / ms_pipe / 1e9, 3)
 
     stream = torch.cuda.current_stream()
     n_psi = 10 if cfg == "femoco" else 1                      # A17: 10 different psi's for the FeMoco config
@@ -500,6 +502,7 @@ def run_ours(args, rank, world, local_rank):
         "warmup": args.warmup, "ms_per_step": ms_total / args.steps, "higher_is_better": True, "scaling": "strong",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "pct_of_fp64_tc_peak": 100.0 * value / (dgemm_peak * world),
+        "operator_gbs": operator_bytes * args.steps / (ms_total * 1e-3) / 1e9,   # operator bytes streamed once per apply
         "config": {"workload": CONFIG_DESC[cfg], "sectors_per_side": int(p.q_left.shape[0]),
                    "D": int(p.d_left.sum()), "terms": int(workloads.config_params(cfg)["n_terms"]), "tasks": n_tasks,
                    "useful_flops_per_step": useful_flops, "operator_bytes": operator_bytes, "psi_length": n,
