@@ -133,6 +133,7 @@ __global__ void svd_round_kernel(const SvdBlk* __restrict__ blk, const int32_t* 
       double2* xp2 = reinterpret_cast<double2*>(xp);
       double2* xq2 = reinterpret_cast<double2*>(xq);
       double a = 0.0, b = 0.0, g = 0.0;
+#pragma unroll 4
       for (int j = lane; j < c2; j += 32) {
         const double2 u = xp2[j], v = xq2[j];
         a = fma(u.x, u.x, a); b = fma(v.x, v.x, b); g = fma(u.x, v.x, g);
@@ -143,10 +144,14 @@ __global__ void svd_round_kernel(const SvdBlk* __restrict__ blk, const int32_t* 
         a = fma(u, u, a); b = fma(v, v, b); g = fma(u, v, g);
       }
       a = warp_sum(a); b = warp_sum(b); g = warp_sum(g);
-      if (a > B.floor2 && b > B.floor2 && fabs(g) > tol * sqrt(a * b)) {
-        const double zeta = (b - a) / (2.0 * g);
-        const double t = copysign(1.0, zeta) / (fabs(zeta) + sqrt(1.0 + zeta * zeta));
-        const double cs = 1.0 / sqrt(1.0 + t * t), sn = cs * t;
+      if (a > B.floor2 && b > B.floor2 && g * g > tol * tol * a * b) {
+        // tan of the smaller rotation angle: t = sign(zeta) / (|zeta| + sqrt(1 + zeta^2)) with zeta = (b - a) / 2g, written
+        // with one square root, one division and one reciprocal square root (the chain of three divisions and three
+        // square roots was a third of a pair's latency)
+        const double d = b - a;
+        const double t = 2.0 * g / (d + copysign(sqrt(d * d + 4.0 * g * g), d));
+        const double cs = rsqrt(1.0 + t * t), sn = cs * t;
+#pragma unroll 4
         for (int j = lane; j < L2; j += 32) {
           const double2 u = xp2[j], v = xq2[j];
           xp2[j] = make_double2(cs * u.x - sn * v.x, cs * u.y - sn * v.y);
