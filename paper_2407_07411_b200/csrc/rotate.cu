@@ -145,13 +145,15 @@ int build_rotate(hpsi_rotate* r, int32_t nsec, const int32_t* d, const int32_t* 
   });
 
   // ---- groups and segs of launch 1, then of launch 2 (same (l,l') groups, same order of blocks)
-  const size_t ng = [&] { size_t n = 0; for (size_t i = 0; i < alive.size(); ++n) { size_t j = i; while (j < alive.size() && blk[alive[j]].row == blk[alive[i]].row && blk[alive[j]].col == blk[alive[i]].col) ++j; i = j; } return n; }();
-  sc.groups.reserve(2 * ng);
+  auto group_end = [&](size_t i) {                     // one past the last block of the (row, col) group starting at i
+    size_t j = i;
+    while (j < alive.size() && blk[alive[j]].row == blk[alive[i]].row && blk[alive[j]].col == blk[alive[i]].col) ++j;
+    return j;
+  };
   sc.segs.reserve(2 * alive.size());
   std::vector<int64_t> tt_off(alive.size());          // workspace offset of T_t^T, in `alive` order
   for (size_t i = 0; i < alive.size();) {
-    size_t j = i;
-    while (j < alive.size() && blk[alive[j]].row == blk[alive[i]].row && blk[alive[j]].col == blk[alive[i]].col) ++j;
+    const size_t j = group_end(i);
     const int l = blk[alive[i]].row, lp = blk[alive[i]].col;
     Group g{};
     g.order = 1;                          // X operands come from the A arena (DevSchedule.a)
@@ -180,8 +182,7 @@ int build_rotate(hpsi_rotate* r, int32_t nsec, const int32_t* d, const int32_t* 
   }
   const int ng1 = (int)sc.groups.size();
   for (size_t i = 0; i < alive.size();) {
-    size_t j = i;
-    while (j < alive.size() && blk[alive[j]].row == blk[alive[i]].row && blk[alive[j]].col == blk[alive[i]].col) ++j;
+    const size_t j = group_end(i);
     const int l = blk[alive[i]].row, lp = blk[alive[i]].col;
     Group g{};
     g.order = 2;                          // X operands come from DevSchedule.b, which the update points at the workspace
