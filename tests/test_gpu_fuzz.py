@@ -1,0 +1,106 @@
+"""Randomised structures through the C ABI against the oracle: irregular label sets, partner-less sectors, sector dims
+from 1 to 200 mixed in one problem, sparse and dense block patterns, odd leading dimensions, misaligned arenas, forced
+contraction orders; every case runs hpsi_apply, hpsi_rotate_apply (random kept dims, some zero) and hpsi_truncate
+(either side, by count or by discarded weight).  (4000 seeds of this generator were run once on a B200 with no failure;
+the committed test keeps 60.)"""
+import numpy as np
+import pytest
+
+import oracle
+import workloads
+from oracle import site_update as su
+from gpu_util import GpuProblem
+
+pytestmark = pytest.mark.gpu
+
+
+def rand_dims(rng, n):
+    kind = rng.integers(0, 4, n)
+    d = np.where(kind == 0, rng.integers(1, 9, n), np.where(kind == 1, rng.integers(8, 70, n),
+                 np.where(kind == 2, rng.integers(60, 200, n), rng.integers(1, 3, n))))
+    return d.astype(np.int64)
+
+
+def rand_problem(seed):
+    rng = np.random.default_rng(seed)
+    nL = int(rng.integers(2, 8))
+    nR = int(rng.integers(nL, nL + 3))
+    qL = rng.permutation(np.array([(a, b) for a in range(-3, 4) for b in range(-2, 3)], np.int32))[:nL]
+    target = np.array([5, 1], np.int32)
+    npart = int(rng.integers(max(1, nL - 2), nL + 1))
+    qR = [tuple(target - q) for q in qL[rng.permutation(nL)[:npart]]]
+    qR += [(99, 99 + i) for i in range(nR - len(qR))]
+    qR = np.array(qR, np.int32)[rng.permutation(nR)]
+    dL, dR = rand_dims(rng, nL), rand_dims(rng, nR)
+    terms = []
+    dense = rng.random() < 0.5
+    for _ in range(int(rng.integers(1, 40))):
+        ab, bb = {}, {}
+        for _k in range(int(rng.integers(1, nL * nL + 1)) if dense else int(rng.integers(1, 6))):
+            r, c = int(rng.integers(nL)), int(rng.integers(nL))
+            ab[(r, c)] = rng.standard_normal((dL[r], dL[c]))
+        for _k in range(int(rng.integers(1, nR * nR + 1)) if dense else int(rng.integers(1, 7))):
+            r, c = int(rng.integers(nR)), int(rng.integers(nR))
+            bb[(r, c)] = rng.standard_normal((dR[r], dR[c]))
+        terms.append((float(rng.standard_normal()), ab, bb))
+    return workloads.custom_problem(qL, dL, qR, dR, target, terms, pad_even=bool(rng.integers(2))), rng
+
+
+@pytest.mark.parametrize("seed", range(1000, 1060))
+def test_random_structure(seed):
+    import torch
+    import paper_2407_07411_b200 as H
+    p, rng = rand_problem(seed)
+    if p.psi_len == 0:
+        pytest.skip("no psi block in this draw")
+    flags = [0, H.HPSI_PLAN_FIXED_ORDER1, H.HPSI_PLAN_FIXED_ORDER2][int(rng.integers(3))]
+    g = GpuProblem(p, flags, misalign=bool(rng.integers(2)))
+    st = torch.cuda.current_stream()
+    psi = rng.standard_normal(p.psi_len)
+    ref = oracle.apply(p, psi)
+    assert np.linalg.norm(g.apply(psi) - ref) <= 1e-12 * max(np.linalg.norm(ref), 1.0)
+
+    # operator update with random kept dimensions (zeros included)
+    chi = np.minimum(p.d_left, np.maximum(0, np.rint(rng.random() * p.d_left * rng.random(len(p.d_left)) * 2))).astype(np.int32)
+    ot = workloads.make_isometries(p.d_left, chi, seed)
+    r = H.hpsi_rotate_plan(p.d_left, chi, p.a_desc, g.a, p.a_len)
+    otd = torch.from_numpy(np.concatenate([workloads.pack_isometries(ot), np.zeros(1)])).cuda()
+    out = torch.full((H.hpsi_rotate_query(r, H.HPSI_RQ_OUT_LENGTH),), float("nan"), dtype=torch.float64, device="cuda")
+    H.hpsi_rotate_apply(r, otd, out, st)
+    torch.cuda.synchronize()
+    outh = out.cpu().numpy()
+    num = den = 0.0
+    for e, x in zip(H.hpsi_rotate_query(r, H.HPSI_RQ_OUT_BLOCKS), su.rotate(p.d_left, chi, p.a_desc, p.a_data, ot)):
+        if e["offset"] < 0:
+            assert x.size == 0
+            continue
+        got = np.lib.stride_tricks.as_strided(outh[int(e["offset"]):], shape=x.shape, strides=(int(e["ld"]) * 8, 8))
+        num += np.sum((got - x) ** 2)
+        den += np.sum(x ** 2)
+    assert num <= (1e-12 ** 2) * max(den, 1e-300) or den == 0.0
+
+    # truncation: unique quantities directly, isometries for validity
+    side = int(rng.integers(2))
+    chi_max = int(rng.integers(0, 2 * int(p.d_left.sum())))
+    eps = [-1.0, 1e-3, 1e-1][int(rng.integers(3))]
+    cap = H.hpsi_query(g.plan, H.HPSI_Q_ISO_CAPACITY_RIGHT if side else H.HPSI_Q_ISO_CAPACITY)
+    otb = torch.zeros(max(cap, 1), dtype=torch.float64, device="cuda")
+    psin = psi / np.linalg.norm(psi)
+    chi_g, sig_g, disc_g = H.hpsi_truncate(g.plan, torch.from_numpy(psin).cuda(), chi_max, otb, st, eps, side)
+    chi_o, _, sig_o, disc_o = su.truncate(p, psin, chi_max, eps, "right" if side else "left")
+    assert np.array_equal(chi_g, chi_o) and abs(disc_g - disc_o) <= 1e-12
+    smax = max([float(s[0]) for s in sig_o if s.size] + [1e-300])
+    row0 = 0
+    for (i, j, rr, cc, off) in p.psi_blocks():
+        nrow = cc if side else rr
+        so = sig_o[j if side else i]
+        np.testing.assert_allclose(sig_g[row0:row0 + so.size], so, rtol=0, atol=1e-12 * smax)
+        row0 += nrow
+    oth, o = otb.cpu().numpy(), 0
+    dims = p.d_right if side else p.d_left
+    for l in range(len(chi_g)):
+        n = int(chi_g[l]) * int(dims[l])
+        O = oth[o:o + n].reshape(int(chi_g[l]), int(dims[l]))
+        o += n
+        if O.size:
+            np.testing.assert_allclose(O @ O.T, np.eye(O.shape[0]), atol=1e-11)
