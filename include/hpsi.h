@@ -39,6 +39,8 @@ extern "C" {
                                            Such a plan serves hpsi_query and hpsi_debug_* ; hpsi_apply -> ESTATE. */
 #define HPSI_PLAN_FIXED_ORDER1 (1u << 1) /* diagnostic: force (A psi) B^T for every task                  */
 #define HPSI_PLAN_FIXED_ORDER2 (1u << 2) /* diagnostic: force A (psi B^T) for every task                  */
+#define HPSI_PLAN_NO_FUSION    (1u << 3) /* diagnostic: every task goes through the two-launch path with the workspace */
+#define HPSI_PLAN_FUSE_ALL     (1u << 4) /* diagnostic: fuse every task that fits one CTA tile, whatever the cost model says */
 
 typedef struct hpsi_plan hpsi_plan_t;   /* opaque; owns the device schedule and the workspace */
 
@@ -268,7 +270,9 @@ enum {
   HPSI_Q_SVD_SWEEPS = 21,    /* int64: Jacobi sweeps of the last hpsi_truncate on this plan                      */
   HPSI_Q_SVD_LAUNCHES = 22,  /* int64: kernels it launched                                                       */
   HPSI_Q_PSI_COLS = 23,      /* int64: sum of d_right over the psi blocks (sigma_host length for HPSI_SIDE_RIGHT)  */
-  HPSI_Q_ISO_CAPACITY_RIGHT = 24 /* int64: sum of min(d_left, d_right) * d_right over the psi blocks              */
+  HPSI_Q_ISO_CAPACITY_RIGHT = 24, /* int64: sum of min(d_left, d_right) * d_right over the psi blocks             */
+  HPSI_Q_N_FUSED_UNITS = 25, /* int64: CTA work units of the fused kernel (both GEMMs of a task in one CTA)       */
+  HPSI_Q_N_FUSED_TASKS = 26  /* int64: tasks whose intermediate never leaves the chip                             */
 };
 
 typedef struct {

@@ -16,12 +16,15 @@ HPSI_OK, HPSI_EINVAL, HPSI_ENOMEM, HPSI_ECUDA, HPSI_ESTATE = 0, -1, -2, -3, -4
 HPSI_PLAN_HOST_ONLY = 1 << 0
 HPSI_PLAN_FIXED_ORDER1 = 1 << 1
 HPSI_PLAN_FIXED_ORDER2 = 1 << 2
+HPSI_PLAN_NO_FUSION = 1 << 3
+HPSI_PLAN_FUSE_ALL = 1 << 4
 
 (HPSI_Q_PSI_LENGTH, HPSI_Q_N_PSI_BLOCKS, HPSI_Q_PSI_BLOCKS, HPSI_Q_N_TASKS, HPSI_Q_USEFUL_FLOPS, HPSI_Q_ISSUED_FLOPS,
  HPSI_Q_OPERATOR_BYTES, HPSI_Q_WORKSPACE_BYTES, HPSI_Q_N_GROUPS, HPSI_Q_N_P1_UNITS, HPSI_Q_N_P2_UNITS,
  HPSI_Q_N_ORDER1_TASKS, HPSI_Q_LAUNCHES_PER_APPLY, HPSI_Q_ALIGNED16, HPSI_Q_INTERMEDIATE_BYTES,
  HPSI_Q_ISSUED_FLOPS_P1, HPSI_Q_TASKS, HPSI_Q_USEFUL_FLOPS_P1, HPSI_Q_CRITICAL_FLOPS, HPSI_Q_PSI_ROWS,
- HPSI_Q_ISO_CAPACITY, HPSI_Q_SVD_SWEEPS, HPSI_Q_SVD_LAUNCHES, HPSI_Q_PSI_COLS, HPSI_Q_ISO_CAPACITY_RIGHT) = range(25)
+ HPSI_Q_ISO_CAPACITY, HPSI_Q_SVD_SWEEPS, HPSI_Q_SVD_LAUNCHES, HPSI_Q_PSI_COLS, HPSI_Q_ISO_CAPACITY_RIGHT,
+ HPSI_Q_N_FUSED_UNITS, HPSI_Q_N_FUSED_TASKS) = range(27)
 HPSI_SIDE_LEFT, HPSI_SIDE_RIGHT = 0, 1
 (HPSI_RQ_OUT_LENGTH, HPSI_RQ_OUT_BLOCKS, HPSI_RQ_ISO_LENGTH, HPSI_RQ_USEFUL_FLOPS, HPSI_RQ_ALGO_BYTES,
  HPSI_RQ_WORKSPACE_BYTES, HPSI_RQ_N_UNITS_1, HPSI_RQ_N_UNITS_2, HPSI_RQ_ALIGNED16, HPSI_RQ_INTERMEDIATE_BYTES) = range(10)

@@ -10,7 +10,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libhpsi.so")
-SOURCES = ["planner.cpp", "interp.cpp", "kernels.cu", "kernels_paired.cu", "api.cu", "stream.cu", "davidson.cu", "microbench.cu", "rotate.cu", "svd.cu"]
+SOURCES = ["planner.cpp", "interp.cpp", "kernels.cu", "kernels_paired.cu", "kernels_fused.cu", "api.cu", "stream.cu", "davidson.cu", "microbench.cu", "rotate.cu", "svd.cu"]
 HEADERS = ["plan.h", "plan_dev.h", "kernels.cuh", "kernels_common.cuh", os.path.join("..", "..", "include", "hpsi.h")]
 
 

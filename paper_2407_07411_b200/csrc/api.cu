@@ -40,7 +40,7 @@ static int upload(const std::vector<T>& v, char* base, size_t& cursor, const T**
 int upload_schedule(hpsi_plan_t* p) {
   const Schedule& sc = p->sc;
   size_t total = table_bytes(sc.blocks) + table_bytes(sc.segs) + table_bytes(sc.groups) + table_bytes(sc.p1) +
-                 table_bytes(sc.runs) + table_bytes(sc.p2) + table_bytes(sc.diag);
+                 table_bytes(sc.runs) + table_bytes(sc.p2) + table_bytes(sc.pf) + table_bytes(sc.diag);
   HPSI_CUDA(cudaMalloc(&p->d_tables, total));
   cudaError_t e = cudaMalloc(&p->d_ws, (size_t)sc.ws_len * sizeof(double));
   if (e != cudaSuccess) {
@@ -62,11 +62,13 @@ int upload_schedule(hpsi_plan_t* p) {
   if ((rc = upload(sc.p1, base, cur, &p->dev.p1))) return rc;
   if ((rc = upload(sc.runs, base, cur, &p->dev.runs))) return rc;
   if ((rc = upload(sc.p2, base, cur, &p->dev.p2))) return rc;
+  if ((rc = upload(sc.pf, base, cur, &p->dev.pf))) return rc;
   if ((rc = upload(sc.diag, base, cur, &p->dev.diag))) return rc;
   p->dev.ws = p->d_ws;
   p->dev.n_blocks = (int)sc.blocks.size();
   p->dev.n_p1 = (int)sc.p1.size();
   p->dev.n_p2 = (int)sc.p2.size();
+  p->dev.n_pf = (int)sc.pf.size();
   p->dev.max_block_elems = sc.max_block_elems;
   p->dev.paired = sc.paired ? 1 : 0;
   p->dev.debug = getenv("HPSI_DEBUG") ? atoi(getenv("HPSI_DEBUG")) : 0;
@@ -226,6 +228,7 @@ int hpsi::apply_impl(hpsi_plan_t* p, const double* psi_dev, double* out_dev, boo
   launch_prep(p->dev, psi_dev, st);
   launch_p1(p->dev, p->aligned16, st);
   launch_p2(p->dev, p->aligned16, st);
+  launch_pf(p->dev, p->aligned16, st);
   launch_reduce(p->dev, out_dev, accumulate, st);
   HPSI_CUDA(cudaGetLastError());
   return HPSI_OK;
@@ -246,6 +249,7 @@ extern "C" int hpsi_apply_profiled(hpsi_plan_t* p, const double* psi_dev, double
   launch_p1(p->dev, p->aligned16, st);
   HPSI_CUDA(cudaEventRecord(ev[2], st));
   launch_p2(p->dev, p->aligned16, st);
+  launch_pf(p->dev, p->aligned16, st);                 // fused units are timed with the second GEMM
   HPSI_CUDA(cudaEventRecord(ev[3], st));
   launch_reduce(p->dev, out_dev, false, st);
   HPSI_CUDA(cudaEventRecord(ev[4], st));
@@ -313,7 +317,9 @@ extern "C" int hpsi_query(const hpsi_plan_t* p, int what, void* out, size_t byte
     case HPSI_Q_N_P2_UNITS: return put_i64((int64_t)sc.p2.size());
     case HPSI_Q_N_ORDER1_TASKS: return put_i64(sc.n_order1);
     case HPSI_Q_LAUNCHES_PER_APPLY:
-      return put_i64((sc.blocks.empty() ? 0 : 2) + (sc.p1.empty() ? 0 : 1) + (sc.p2.empty() ? 0 : 1));
+      return put_i64((sc.blocks.empty() ? 0 : 2) + (sc.p1.empty() ? 0 : 1) + (sc.p2.empty() ? 0 : 1) + (sc.pf.empty() ? 0 : 1));
+    case HPSI_Q_N_FUSED_UNITS: return put_i64((int64_t)sc.pf.size());
+    case HPSI_Q_N_FUSED_TASKS: { int64_t n = 0; for (const Group& g : sc.groups) if (g.fused) n += g.tcount; return put_i64(n); }
     case HPSI_Q_ALIGNED16: return put_i64(p->host_only ? sc.aligned16 : p->aligned16);
     case HPSI_Q_INTERMEDIATE_BYTES: return put_i64(sc.intermediate_bytes);
     case HPSI_Q_PSI_ROWS: { int64_t n = 0; for (const PsiBlk& b : sc.blocks) n += b.rows; return put_i64(n); }

@@ -68,6 +68,42 @@ void interpret_schedule(const Schedule& sc, const double* a, const double* b, co
         ws[u.out_off + (int64_t)r * u.ldo + c] = s;
       }
   }
+  // fused units: per segment the first GEMM into a local buffer (the kernel's shared-memory operand tile), then the second
+  for (const P2Unit& u : sc.pf) {
+    std::vector<double> acc((size_t)u.rows_valid * u.cols_valid, 0.0);
+    for (int ri = u.run_begin; ri < u.run_end; ++ri) {
+      const Run& run = sc.runs[ri];
+      const int rows_a = (run.order == 1) ? u.rows_valid : u.cols_valid, row_a0 = (run.order == 1) ? u.i0 : u.j0;
+      const double* arena_a = (run.order == 1) ? a : b;
+      const double* arena_b = (run.order == 1) ? b : a;
+      std::vector<double> c1((size_t)rows_a * run.K);
+      for (int si = run.seg_begin; si < run.seg_end; ++si) {
+        const Seg& sg = sc.segs[si];
+        for (int i = 0; i < rows_a; ++i)
+          for (int j = 0; j < run.K; ++j) {
+            const double* xr = arena_a + sg.p1_off + (int64_t)(row_a0 + i) * sg.p1_ld;
+            const double* yr = ws + run.y1_off + (int64_t)j * run.ldy1;
+            double s = 0.0;
+            for (int k = 0; k < run.K1; ++k) s += xr[k] * yr[k];
+            c1[(size_t)i * run.K + j] = sg.coef * s;
+          }
+        for (int r = 0; r < u.rows_valid; ++r)
+          for (int c = 0; c < u.cols_valid; ++c) {
+            double s = 0.0;
+            if (run.order == 1) {
+              const double* yr = arena_b + sg.p2_off + (int64_t)(u.j0 + c) * sg.p2_ld;
+              for (int k = 0; k < run.K; ++k) s += c1[(size_t)r * run.K + k] * yr[k];
+            } else {
+              const double* xr = arena_b + sg.p2_off + (int64_t)(u.i0 + r) * sg.p2_ld;
+              for (int k = 0; k < run.K; ++k) s += xr[k] * c1[(size_t)c * run.K + k];
+            }
+            acc[(size_t)r * u.cols_valid + c] += s;
+          }
+      }
+    }
+    for (int r = 0; r < u.rows_valid; ++r)
+      for (int c = 0; c < u.cols_valid; ++c) ws[u.out_off + (int64_t)r * u.ldo + c] = acc[(size_t)r * u.cols_valid + c];
+  }
   // ordered reduce
   for (const PsiBlk& B : sc.blocks)
     for (int x = 0; x < B.rows; ++x)

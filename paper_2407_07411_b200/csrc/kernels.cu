@@ -325,6 +325,7 @@ cudaError_t kernels_init() {
   if ((e = cudaFuncSetAttribute(p1_kernel<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES))) return e;
   if ((e = cudaFuncSetAttribute(p2_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES))) return e;
   if ((e = cudaFuncSetAttribute(p2_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES))) return e;
+  if ((e = kernels_fused_init())) return e;
   return kernels_paired_init();
 }
 

@@ -28,12 +28,13 @@ struct DevSchedule {           // device pointers to the uploaded tables
   const P1Unit* p1;
   const Run* runs;
   const P2Unit* p2;
+  const P2Unit* pf;            // fused units (kernels_fused.cu)
   const DiagTask* diag;
   const unsigned char* maps;   // CUtensorMap[sc.maps.size()], 128 bytes each (TMA staging only)
   double* ws;
   const double* a;
   const double* b;
-  int n_blocks, n_p1, n_p2;
+  int n_blocks, n_p1, n_p2, n_pf;
   int max_block_elems;
   int paired;                  // the plan has blocks stored transposed: kernels_paired.cu runs the GEMMs
   int debug;                   // HPSI_DEBUG env (timing experiments only): 1 = producer skips loads, 2 = consumers skip MMAs
@@ -44,6 +45,8 @@ void launch_prep(const DevSchedule& d, const double* psi, cudaStream_t st);
 void launch_p1(const DevSchedule& d, bool tma, cudaStream_t st);
 void launch_p1_rot(const DevSchedule& d, bool tma, cudaStream_t st);   // same kernel, tile stored transposed at Seg.p2_off / p2_ld
 void launch_p2(const DevSchedule& d, bool tma, cudaStream_t st);
+void launch_pf(const DevSchedule& d, bool tma, cudaStream_t st);            // kernels_fused.cu
+cudaError_t kernels_fused_init();
 void launch_reduce(const DevSchedule& d, double* out, bool accumulate, cudaStream_t st);
 void launch_diag(const DevSchedule& d, double* diag, cudaStream_t st);
 void launch_p1_paired(const DevSchedule& d, bool tma, cudaStream_t st);   // kernels_paired.cu

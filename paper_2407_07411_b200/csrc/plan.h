@@ -54,6 +54,8 @@ struct Group {
   int32_t y1_map;             // tensor map of the P1 Y operand
   int32_t ws_map;             // tensor map of the stacked intermediate
   int32_t src, dst;           // psi block indices
+  int32_t fused;              // 1: narrow group, both GEMMs run in one CTA (kernels_fused.cu): no P1 unit, no workspace intermediate
+  int32_t pad;
 };
 
 struct P1Unit {               // one CTA of the first-GEMM kernel: one tile position, a range of the group's terms
@@ -76,7 +78,10 @@ struct Run {                  // consecutive segs of one group inside one P2 uni
   int32_t ws_map;             // group.ws_map
   int64_t ws_off;             // group.ws_off
   int32_t trans;              // 1: the operator blocks of these segs are stored transposed (K-major operand)
+  int32_t K1;                 // fused runs only: contraction length of the first GEMM (group.K1)
+  int32_t y1_map, ldy1;       // fused runs only: the first GEMM's shared operand (padded psi^T / psi block), group.y1_map / ldy1
   int32_t pad;
+  int64_t y1_off;             // fused runs only: group.y1_off
 };
 
 struct P2Unit {               // one CTA of the second-GEMM kernel
@@ -125,6 +130,7 @@ struct Schedule {
   std::vector<P1Unit> p1;
   std::vector<Run> runs;
   std::vector<P2Unit> p2;
+  std::vector<P2Unit> pf;             // units of the fused kernel (same descriptor; their runs are fused runs)
   std::vector<DiagTask> diag;
   std::vector<MapSpec> maps;          // tensor maps the TMA kernels use (only filled / valid when aligned16)
   std::vector<hpsi_task_t> tasks;     // schedule order, for hpsi_query

@@ -208,6 +208,12 @@ int build_schedule(const hpsi_sectors_t* s, const hpsi_terms_t* t, uint32_t flag
     b.t_map = add_map(BASE_WS, b.t_off, b.cols, b.rows, b.ldt);
   }
 
+  // The fused kernel is OFF by default: measured on B200 it loses to the two launches even where every task fits it
+  // (cyp-shaped config at D = 1024: 1.83 ms per apply fused, 0.63 ms through the workspace - per segment the first GEMM,
+  // a CTA barrier, the shared-memory write, a barrier and the second GEMM run back to back, where the two-launch kernels
+  // stream stages without ever draining).  HPSI_PLAN_FUSE_ALL or env HPSI_FUSE=1 select it (tests, experiments).
+  const bool fuse_default = getenv("HPSI_FUSE") && atoi(getenv("HPSI_FUSE")) == 1;
+
   // ---- steps 3+4a: order choice, groups, segs
   sc->segs.clear(); sc->groups.clear(); sc->tasks.clear(); sc->diag.clear();
   sc->useful_flops = sc->useful_flops_p1 = sc->operator_bytes = sc->intermediate_bytes = 0;
@@ -232,9 +238,17 @@ int build_schedule(const hpsi_sectors_t* s, const hpsi_terms_t* t, uint32_t flag
     if (order == 1) { g.rows = (int32_t)m; g.K1 = (int32_t)k; g.N1 = (int32_t)np; g.ldy1 = S.ldt; g.y1_off = S.t_off; g.y1_map = S.t_map; }
     else            { g.rows = (int32_t)n; g.K1 = (int32_t)np; g.N1 = (int32_t)k; g.ldy1 = S.ldp; g.y1_off = S.p_off; g.y1_map = S.p_map; }
     g.ldw = sector_up(g.N1);
+    // Narrow groups run both GEMMs in one CTA (kernels_fused.cu; north_star: "the intermediate block kept in shared
+    // memory or registers between the two GEMMs"): the whole intermediate of a tile fits one operand buffer (N1 <= 64)
+    // and the output dimension that would otherwise recompute it is a single tile (order 1: n <= 64, order 2: m <= 64).
+    {
+      const int64_t other = (order == 1) ? n : m;
+      const bool fits = g.N1 <= TILE && other <= TILE && !paired && !HPSI_BIG_CTA;
+      g.fused = (fits && !(flags & HPSI_PLAN_NO_FUSION) && (fuse_default || (flags & HPSI_PLAN_FUSE_ALL))) ? 1 : 0;
+    }
     g.ws_off = ws;
-    const int64_t per_task = (int64_t)g.rows * g.ldw;
-    g.ws_map = add_map(BASE_WS, ws, (int)((int64_t)g.rows * (j - i)), g.N1, g.ldw);
+    const int64_t per_task = g.fused ? 0 : (int64_t)g.rows * g.ldw;
+    g.ws_map = g.fused ? -1 : add_map(BASE_WS, ws, (int)((int64_t)g.rows * (j - i)), g.N1, g.ldw);
     for (size_t q = i; q < j; ++q) {
       const hpsi_opblock_t& a = t->a_blocks[raw[q].ia];
       const hpsi_opblock_t& b = t->b_blocks[raw[q].ib];
@@ -258,7 +272,7 @@ int build_schedule(const hpsi_sectors_t* s, const hpsi_terms_t* t, uint32_t flag
       sc->useful_flops += std::min(f1, f2);
       sc->useful_flops_p1 += (f2 < f1) ? 2 * k * np * n : 2 * m * k * np;   // first GEMM of the min-flop order
       sc->operator_bytes += 8 * (m * k + n * np);
-      sc->intermediate_bytes += 8 * (int64_t)g.rows * g.N1;
+      if (!g.fused) sc->intermediate_bytes += 8 * (int64_t)g.rows * g.N1;
       if (order == 1) sc->n_order1++;
       if (raw[q].src == raw[q].dst)
         diag_by_blk[raw[q].dst].push_back({a.offset, b.offset, a.ld, b.ld, t->coef[raw[q].term], (int32_t)sc->segs.size() - 1, 0});
@@ -284,7 +298,7 @@ int build_schedule(const hpsi_sectors_t* s, const hpsi_terms_t* t, uint32_t flag
     // ~96 K-tiles per unit, fewer when the whole launch would otherwise be only a few waves of CTAs (small problems)
     int64_t total_stages = 0;
     for (const Group& g : sc->groups)
-      total_stages += (int64_t)split_rows(g.rows).size() * split_cols(g.N1).size() * g.tcount * ((g.K1 + KT - 1) / KT);
+      if (!g.fused) total_stages += (int64_t)split_rows(g.rows).size() * split_cols(g.N1).size() * g.tcount * ((g.K1 + KT - 1) / KT);
     const int auto_stages = (int)std::max<int64_t>(12, std::min<int64_t>(96, total_stages / ((int64_t)std::max(n_sm, 1) * 3 * 8)));
     const int P1_STAGES_PER_UNIT = getenv("HPSI_P1_STAGES") ? std::max(1, atoi(getenv("HPSI_P1_STAGES"))) : auto_stages;   // env: tuning experiments
     struct GOrder { int64_t cost; int gi; };
@@ -292,6 +306,7 @@ int build_schedule(const hpsi_sectors_t* s, const hpsi_terms_t* t, uint32_t flag
     std::vector<int> g_nt(sc->groups.size());
     for (size_t gi = 0; gi < sc->groups.size(); ++gi) {
       const Group& g = sc->groups[gi];
+      if (g.fused) continue;
       const int stages = (g.K1 + KT - 1) / KT;
       int nt = std::max(1, std::min(g.tcount, (P1_STAGES_PER_UNIT + stages - 1) / stages));
       const int nchunk = (g.tcount + nt - 1) / nt;
@@ -339,9 +354,22 @@ int build_schedule(const hpsi_sectors_t* s, const hpsi_terms_t* t, uint32_t flag
     if (rem) c += std::max<int64_t>(((rem + 3) / 4) * tile_frags, STAGE_FLOOR);
     return c;
   };
-  struct DstInfo { int g0 = 0, g1 = 0; int64_t cost = 0; int64_t nseg = 0; int maxf = 0; std::vector<Tile1D> rt, ct; };
+  // A fused segment (kernels_fused.cu) runs its first GEMM in the same CTA: ceil(K1/16) more stages on the intermediate's tile.
+  auto fused_extra = [&](const Group& g, int64_t tile_frags_a) {
+    const int64_t full = g.K1 / KT, rem = g.K1 % KT;
+    int64_t c = full * std::max<int64_t>(4 * tile_frags_a, STAGE_FLOOR);
+    if (rem) c += std::max<int64_t>(((rem + 3) / 4) * tile_frags_a, STAGE_FLOOR);
+    return c;
+  };
+  // pass 0: groups whose intermediate is in the workspace (p2 units); pass 1: fused groups (pf units)
+  struct DstInfo { int g0 = 0, g1 = 0; int64_t cost[2] = {0, 0}; int64_t nseg[2] = {0, 0}; int maxf = 0; std::vector<Tile1D> rt, ct; };
   std::vector<DstInfo> dsts(nB);
-  int64_t total_p2_cost = 0;
+  int64_t total_cost[2] = {0, 0};
+  auto group_seg_cost = [&](const Group& g, int64_t tile_frags_b) {
+    int64_t c = seg_cost(g, tile_frags_b);
+    if (g.fused) c += fused_extra(g, (int64_t)std::min(frags(g.rows), TILE_M / 8) * frags(g.N1));
+    return c;
+  };
   {
     size_t gi = 0;
     for (int d = 0; d < nB; ++d) {
@@ -351,12 +379,13 @@ int build_schedule(const hpsi_sectors_t* s, const hpsi_terms_t* t, uint32_t flag
       for (auto& r : di.rt) for (auto& c : di.ct) di.maxf = std::max(di.maxf, tile_frags(r.len, paired) * tile_frags(c.len, paired));
       di.g0 = (int)gi;
       while (gi < sc->groups.size() && sc->groups[gi].dst == d) {
-        di.cost += (int64_t)sc->groups[gi].tcount * seg_cost(sc->groups[gi], di.maxf);   // heaviest tile of the block
-        di.nseg += sc->groups[gi].tcount;
+        const Group& g = sc->groups[gi];
+        di.cost[g.fused] += (int64_t)g.tcount * group_seg_cost(g, di.maxf);   // heaviest tile of the block
+        di.nseg[g.fused] += g.tcount;
         ++gi;
       }
       di.g1 = (int)gi;
-      total_p2_cost += di.cost * (int64_t)(di.rt.size() * di.ct.size());
+      for (int pass = 0; pass < 2; ++pass) total_cost[pass] += di.cost[pass] * (int64_t)(di.rt.size() * di.ct.size());
     }
   }
   const int waves = getenv("HPSI_P2_WAVES") ? std::max(1, atoi(getenv("HPSI_P2_WAVES"))) : 48;   // env: tuning experiments
@@ -366,99 +395,118 @@ int build_schedule(const hpsi_sectors_t* s, const hpsi_terms_t* t, uint32_t flag
   // 64 waves gain nothing more (the ordered reduce grows as fast as p2 shrinks).
   const int64_t slots = (int64_t)std::max(n_sm, 1) * 4 * waves;
   const int64_t min_target = getenv("HPSI_P2_MIN") ? std::max(1, atoi(getenv("HPSI_P2_MIN"))) : 1536;   // DMMA per unit at least (~10 us of a CTA)
-  const int64_t target = std::max<int64_t>(min_target, total_p2_cost / slots);
+  const int64_t target_of[2] = {std::max<int64_t>(min_target, total_cost[0] / slots),
+                                std::max<int64_t>(min_target, total_cost[1] / slots)};
 
-  sc->runs.clear(); sc->p2.clear();
-  std::vector<int> unit_bundle;            // (block, split) bundle of each unit
-  std::vector<int64_t> bundle_cost;        // heaviest tile of the bundle, in DMMA count
+  sc->runs.clear(); sc->p2.clear(); sc->pf.clear();
+  std::vector<int> unit_bundle[2];         // (block, split) bundle of each unit, per pass
+  std::vector<int64_t> bundle_cost[2];     // heaviest tile of the bundle, in DMMA count
   int64_t issued_p2 = 0;
   for (int d = 0; d < nB; ++d) {
     PsiBlk& D = sc->blocks[d];
     D.ldo = sector_up(D.cols);
     D.part_off = ws;
     D.nsplit = 0;
-    if (dsts[d].nseg == 0) continue;
     const auto& rt = dsts[d].rt;
     const auto& ct = dsts[d].ct;
     const int maxf = dsts[d].maxf;
-    int64_t nsplit = (dsts[d].cost + target - 1) / target;
-    nsplit = std::max<int64_t>(1, std::min<int64_t>(nsplit, dsts[d].nseg));
-    // cut the seg sequence at cumulative cost boundaries
-    std::vector<std::pair<int, int>> split_runs;   // run index range per split
-    int64_t cum = 0;
-    int gi = dsts[d].g0;
-    int ti = 0;                                    // position inside group gi
     int realised = 0;
-    for (int64_t sp = 0; sp < nsplit; ++sp) {
-      const int64_t want = dsts[d].cost * (sp + 1) / nsplit;
-      int run0 = (int)sc->runs.size();
-      int64_t chunk_ksteps = 0;
-      while (gi < dsts[d].g1 && (cum < want || sp == nsplit - 1)) {
-        const Group& g = sc->groups[gi];
-        const int64_t per = seg_cost(g, maxf);
-        int take;
-        if (sp == nsplit - 1) take = g.tcount - ti;
-        else take = (int)std::min<int64_t>(g.tcount - ti, std::max<int64_t>(1, (want - cum + per - 1) / per));
-        if (take > 0) {
-          // a run has one storage layout of its operator blocks: split [ti, ti + take) at the group's layout boundary
-          int tbnd = ti;
-          while (tbnd < ti + take && !sc->segs[g.seg0 + tbnd].p2_trans) ++tbnd;
-          if (tbnd > ti)
-            sc->runs.push_back({g.seg0 + ti, g.seg0 + tbnd, g.N1, g.ldw, g.order, g.rows, g.seg0, g.ws_map, g.ws_off, 0, 0});
-          if (tbnd < ti + take)
-            sc->runs.push_back({g.seg0 + tbnd, g.seg0 + ti + take, g.N1, g.ldw, g.order, g.rows, g.seg0, g.ws_map, g.ws_off, 1, 0});
-          cum += per * take;
-          chunk_ksteps += (int64_t)((g.N1 + 3) / 4) * take;
-          ti += take;
-        }
-        if (ti >= g.tcount) { ++gi; ti = 0; }
-      }
-      int run1 = (int)sc->runs.size();
-      if (run1 == run0) continue;                  // empty chunk (rounding): skip
-      int64_t bundle_max = 0;
-      for (auto& r : rt)
-        for (auto& c : ct) {
-          P2Unit u{};
-          u.run_begin = run0; u.run_end = run1;
-          u.i0 = r.start; u.rows_valid = r.len; u.j0 = c.start; u.cols_valid = c.len;
-          u.ldo = D.ldo;
-          const int fm = tile_frags(r.len, paired), fn = tile_frags(c.len, paired);
-          u.grid = best_grid(fm, fn, nullptr, paired);
-          u.out_off = ws + (int64_t)realised * D.rows * D.ldo + (int64_t)r.start * D.ldo + c.start;
-          sc->p2.push_back(u);
-          const int64_t dmma = (int64_t)fm * fn * chunk_ksteps;
-          int64_t cost = 0;                         // this tile's cost over the chunk's runs, stage floor included
-          for (int ri = run0; ri < run1; ++ri) {
-            const Run& rr = sc->runs[ri];
-            Group gg{};
-            gg.N1 = rr.K;
-            cost += (int64_t)(rr.seg_end - rr.seg_begin) * seg_cost(gg, (int64_t)fm * fn);
+    for (int pass = 0; pass < 2; ++pass) {
+      if (dsts[d].nseg[pass] == 0) continue;
+      std::vector<P2Unit>& units = pass ? sc->pf : sc->p2;
+      const int64_t target = target_of[pass];
+      int64_t nsplit = (dsts[d].cost[pass] + target - 1) / target;
+      nsplit = std::max<int64_t>(1, std::min<int64_t>(nsplit, dsts[d].nseg[pass]));
+      // cut the seg sequence of this pass at cumulative cost boundaries
+      int64_t cum = 0;
+      int gi = dsts[d].g0;
+      int ti = 0;                                    // position inside group gi
+      auto skip_other = [&]() { while (gi < dsts[d].g1 && sc->groups[gi].fused != pass) { ++gi; ti = 0; } };
+      skip_other();
+      for (int64_t sp = 0; sp < nsplit; ++sp) {
+        const int64_t want = dsts[d].cost[pass] * (sp + 1) / nsplit;
+        int run0 = (int)sc->runs.size();
+        int64_t chunk_ksteps = 0;
+        while (gi < dsts[d].g1 && (cum < want || sp == nsplit - 1)) {
+          const Group& g = sc->groups[gi];
+          const int64_t per = group_seg_cost(g, maxf);
+          int take;
+          if (sp == nsplit - 1) take = g.tcount - ti;
+          else take = (int)std::min<int64_t>(g.tcount - ti, std::max<int64_t>(1, (want - cum + per - 1) / per));
+          if (take > 0) {
+            // a run has one storage layout of its operator blocks: split [ti, ti + take) at the group's layout boundary
+            int tbnd = ti;
+            while (tbnd < ti + take && !sc->segs[g.seg0 + tbnd].p2_trans) ++tbnd;
+            Run r{g.seg0 + ti, g.seg0 + tbnd, g.N1, g.ldw, g.order, g.rows, g.seg0, g.ws_map, g.ws_off, 0, 0, 0, 0, 0, 0};
+            if (g.fused) { r.K1 = g.K1; r.y1_map = g.y1_map; r.ldy1 = g.ldy1; r.y1_off = g.y1_off; }
+            if (tbnd > ti) sc->runs.push_back(r);
+            if (tbnd < ti + take) {
+              r.seg_begin = g.seg0 + tbnd; r.seg_end = g.seg0 + ti + take; r.trans = 1;
+              sc->runs.push_back(r);
+            }
+            cum += per * take;
+            chunk_ksteps += (int64_t)((g.N1 + 3) / 4) * take;
+            ti += take;
           }
-          int heavy = 0;
-          best_grid(fm, fn, &heavy, paired);
-          sc->critical_flops += (int64_t)NCONS_WARPS * heavy * chunk_ksteps * 512;
-          unit_bundle.push_back((int)bundle_cost.size());
-          bundle_max = std::max(bundle_max, cost);
-          issued_p2 += dmma * 512;
+          if (ti >= g.tcount) { ++gi; ti = 0; skip_other(); }
         }
-      bundle_cost.push_back(bundle_max);
-      ++realised;
+        int run1 = (int)sc->runs.size();
+        if (run1 == run0) continue;                  // empty chunk (rounding): skip
+        int64_t bundle_max = 0;
+        for (auto& r : rt)
+          for (auto& c : ct) {
+            P2Unit u{};
+            u.run_begin = run0; u.run_end = run1;
+            u.i0 = r.start; u.rows_valid = r.len; u.j0 = c.start; u.cols_valid = c.len;
+            u.ldo = D.ldo;
+            const int fm = tile_frags(r.len, paired), fn = tile_frags(c.len, paired);
+            u.grid = pass ? 2 : best_grid(fm, fn, nullptr, paired);       // fused CTAs: 2x2 warps, <= 4x4 fragments each
+            u.out_off = ws + (int64_t)realised * D.rows * D.ldo + (int64_t)r.start * D.ldo + c.start;
+            units.push_back(u);
+            int64_t dmma = (int64_t)fm * fn * chunk_ksteps;
+            int64_t cost = 0;                         // this tile's cost over the chunk's runs, stage floor included
+            for (int ri = run0; ri < run1; ++ri) {
+              const Run& rr = sc->runs[ri];
+              Group gg{};
+              gg.N1 = rr.K;
+              int64_t per = seg_cost(gg, (int64_t)fm * fn);
+              if (pass) {                             // first GEMM of the fused segment on its own tile
+                const int64_t fa = (int64_t)(rr.order == 1 ? fm : fn) * frags(rr.K);
+                gg.K1 = rr.K1;
+                per += fused_extra(gg, fa);
+                dmma += fa * ((rr.K1 + 3) / 4) * (rr.seg_end - rr.seg_begin);
+              }
+              cost += (int64_t)(rr.seg_end - rr.seg_begin) * per;
+            }
+            int heavy = 0;
+            best_grid(fm, fn, &heavy, paired);
+            sc->critical_flops += (int64_t)NCONS_WARPS * heavy * chunk_ksteps * 512;
+            unit_bundle[pass].push_back((int)bundle_cost[pass].size());
+            bundle_max = std::max(bundle_max, cost);
+            issued_p2 += dmma * 512;
+          }
+        bundle_cost[pass].push_back(bundle_max);
+        ++realised;
+      }
     }
     D.nsplit = realised;
     ws = align_up(ws + (int64_t)realised * D.rows * D.ldo, 16);
   }
   // LPT order over (block, split) bundles: the tiles of one bundle read the same operand segments, so they stay
   // adjacent in launch order (co-resident CTAs -> the second reader hits L2); bundles go heaviest tile first.
-  {
-    std::vector<int> idx(sc->p2.size());
+  for (int pass = 0; pass < 2; ++pass) {
+    std::vector<P2Unit>& units = pass ? sc->pf : sc->p2;
+    std::vector<int> idx(units.size());
     std::iota(idx.begin(), idx.end(), 0);
+    const auto& ub = unit_bundle[pass];
+    const auto& bc = bundle_cost[pass];
     std::stable_sort(idx.begin(), idx.end(), [&](int a, int b) {
-      if (bundle_cost[unit_bundle[a]] != bundle_cost[unit_bundle[b]]) return bundle_cost[unit_bundle[a]] > bundle_cost[unit_bundle[b]];
-      return unit_bundle[a] < unit_bundle[b];
+      if (bc[ub[a]] != bc[ub[b]]) return bc[ub[a]] > bc[ub[b]];
+      return ub[a] < ub[b];
     });
-    std::vector<P2Unit> sorted(sc->p2.size());
-    for (size_t i = 0; i < idx.size(); ++i) sorted[i] = sc->p2[idx[i]];
-    sc->p2.swap(sorted);
+    std::vector<P2Unit> sorted(units.size());
+    for (size_t i = 0; i < idx.size(); ++i) sorted[i] = units[idx[i]];
+    units.swap(sorted);
   }
   sc->issued_flops = sc->issued_flops_p1 + issued_p2;
   sc->ws_len = std::max<int64_t>(ws, 16);

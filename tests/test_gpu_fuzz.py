@@ -54,6 +54,8 @@ def test_random_structure(seed):
     if p.psi_len == 0:
         pytest.skip("no psi block in this draw")
     flags = [0, H.HPSI_PLAN_FIXED_ORDER1, H.HPSI_PLAN_FIXED_ORDER2][int(rng.integers(3))]
+    if seed % 2:
+        flags |= H.HPSI_PLAN_FUSE_ALL            # narrow groups through the fused kernel (aligned and misaligned staging)
     g = GpuProblem(p, flags, misalign=bool(rng.integers(2)))
     st = torch.cuda.current_stream()
     psi = rng.standard_normal(p.psi_len)

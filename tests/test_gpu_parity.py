@@ -21,19 +21,36 @@ def H():
     return H
 
 
-@pytest.mark.parametrize("flags_name", ["min_flops", "order1", "order2"])
+FLAG_NAMES = ["min_flops", "order1", "order2", "fused", "fused_order1", "fused_order2"]
+
+
+def plan_flags(H, name):
+    """Contraction-order and fusion variants of the planner (fused = every narrow group runs both GEMMs in one CTA)."""
+    return {"min_flops": 0, "order1": H.HPSI_PLAN_FIXED_ORDER1, "order2": H.HPSI_PLAN_FIXED_ORDER2,
+            "fused": H.HPSI_PLAN_FUSE_ALL, "fused_order1": H.HPSI_PLAN_FUSE_ALL | H.HPSI_PLAN_FIXED_ORDER1,
+            "fused_order2": H.HPSI_PLAN_FUSE_ALL | H.HPSI_PLAN_FIXED_ORDER2}[name]
+
+
+@pytest.mark.parametrize("flags_name", FLAG_NAMES)
 def test_toy_parity(H, toy, flags_name):
-    flags = {"min_flops": 0, "order1": H.HPSI_PLAN_FIXED_ORDER1, "order2": H.HPSI_PLAN_FIXED_ORDER2}[flags_name]
+    flags = plan_flags(H, flags_name)
     g = GpuProblem(toy, flags)
+    if flags_name.startswith("fused"):          # every toy dim is <= 6: all tasks fused, nothing through the workspace
+        assert g.q(H.HPSI_Q_N_FUSED_TASKS) == g.q(H.HPSI_Q_N_TASKS) and g.q(H.HPSI_Q_N_P1_UNITS) == 0
+        assert g.q(H.HPSI_Q_INTERMEDIATE_BYTES) == 0
+    else:
+        assert g.q(H.HPSI_Q_N_FUSED_TASKS) == 0
     for k in range(3):
         psi = workloads.make_psi(toy, k)
         assert rel_l2(g.apply(psi), oracle.apply(toy, psi)) <= TOL
 
 
-@pytest.mark.parametrize("flags_name", ["min_flops", "order1", "order2"])
+@pytest.mark.parametrize("flags_name", FLAG_NAMES)
 def test_small_parity(H, small, flags_name):
-    flags = {"min_flops": 0, "order1": H.HPSI_PLAN_FIXED_ORDER1, "order2": H.HPSI_PLAN_FIXED_ORDER2}[flags_name]
+    flags = plan_flags(H, flags_name)
     g = GpuProblem(small, flags)
+    if flags_name.startswith("fused"):          # dims 7..136: a mix of fused groups and groups through the workspace
+        assert 0 < g.q(H.HPSI_Q_N_FUSED_TASKS) < g.q(H.HPSI_Q_N_TASKS)
     psi = workloads.make_psi(small)
     ref = oracle.apply(small, psi)
     got = g.apply(psi)
@@ -58,7 +75,7 @@ def test_small_unaligned_staging(H):
 @pytest.mark.parametrize("seed", range(8))
 def test_irregular_parity(H, seed):
     p = random_custom(seed, grid=(seed < 4))
-    g = GpuProblem(p)
+    g = GpuProblem(p, H.HPSI_PLAN_FUSE_ALL if seed % 2 else 0)
     psi = np.random.default_rng(seed).standard_normal(p.psi_len)
     ref = oracle.apply(p, psi)
     assert np.linalg.norm(g.apply(psi) - ref) <= TOL * max(np.linalg.norm(ref), 1.0)

@@ -66,7 +66,8 @@ def test_psi_blocks_match_oracle_table(toy, small):
 
 
 # ------------------------------------------------------------------------- schedule == oracle (CPU)
-@pytest.mark.parametrize("flags", [0, H.HPSI_PLAN_FIXED_ORDER1, H.HPSI_PLAN_FIXED_ORDER2])
+@pytest.mark.parametrize("flags", [0, H.HPSI_PLAN_FIXED_ORDER1, H.HPSI_PLAN_FIXED_ORDER2, H.HPSI_PLAN_FUSE_ALL,
+                                   H.HPSI_PLAN_FUSE_ALL | H.HPSI_PLAN_FIXED_ORDER1, H.HPSI_PLAN_FUSE_ALL | H.HPSI_PLAN_FIXED_ORDER2])
 def test_schedule_interpreter_toy(toy, flags):
     plan = host_plan(toy, flags)
     for k in range(2):
@@ -74,10 +75,19 @@ def test_schedule_interpreter_toy(toy, flags):
         assert rel(H.hpsi_debug_interpret(plan, toy.a_data, toy.b_data, psi), oracle.apply(toy, psi)) <= 1e-13
 
 
-def test_schedule_interpreter_small(small):
-    plan = host_plan(small)
+@pytest.mark.parametrize("flags", [0, H.HPSI_PLAN_FUSE_ALL])
+def test_schedule_interpreter_small(small, flags):
+    plan = host_plan(small, flags)
     psi = workloads.make_psi(small)
     assert rel(H.hpsi_debug_interpret(plan, small.a_data, small.b_data, psi), oracle.apply(small, psi)) <= 1e-13
+    fused = H.hpsi_query(plan, H.HPSI_Q_N_FUSED_TASKS)
+    if flags:      # the narrow groups go to fused units and write no intermediate; the others keep the two-launch path
+        assert 0 < fused < H.hpsi_query(plan, H.HPSI_Q_N_TASKS) and H.hpsi_query(plan, H.HPSI_Q_N_FUSED_UNITS) > 0
+        assert H.hpsi_query(plan, H.HPSI_Q_INTERMEDIATE_BYTES) < H.hpsi_query(host_plan(small), H.HPSI_Q_INTERMEDIATE_BYTES)
+        assert H.hpsi_query(plan, H.HPSI_Q_LAUNCHES_PER_APPLY) == 5
+        assert H.hpsi_query(host_plan(small, flags | H.HPSI_PLAN_NO_FUSION), H.HPSI_Q_N_FUSED_TASKS) == 0
+    else:
+        assert fused == 0 and H.hpsi_query(plan, H.HPSI_Q_LAUNCHES_PER_APPLY) == 4
 
 
 @pytest.mark.parametrize("seed", range(8))
