@@ -101,8 +101,10 @@ __global__ void __maxnreg__(HPSI_BIG_CTA ? 112 : 136) p1_kernel(DevSchedule d) {
       const unsigned char* xmap = nullptr;
       const double* xbase = nullptr;
       int64_t xld = 0;
-      if (TMA) xmap = d.maps + (int64_t)sg->p1_map * TMAP_BYTES;
-      else { xld = sg->p1_ld; xbase = xarena + sg->p1_off + (int64_t)u.i0 * xld; }
+      if (TMA) {
+        xmap = d.maps + (int64_t)sg->p1_map * TMAP_BYTES;
+        if (lane == 0 && t + 2 < u.t1) tma_prefetch_desc(d.maps + (int64_t)sg[2].p1_map * TMAP_BYTES);   // descriptor of the term after next
+      } else { xld = sg->p1_ld; xbase = xarena + sg->p1_off + (int64_t)u.i0 * xld; }
       for (int kt = 0; kt < ntiles; ++kt) {
         mbar_wait(sm.empty(ring.stage), ring.phase);
         const uint32_t sx = sm.stage(ring.stage), sy = sx + X_BOXES * OP_BYTES, full = sm.full(ring.stage);
@@ -209,6 +211,7 @@ __global__ void __maxnreg__(HPSI_BIG_CTA ? 112 : 136) p2_kernel(DevSchedule d) {
       if (TMA) {
         const unsigned char* opmap = d.maps + (int64_t)sg->p2_map * TMAP_BYTES;
         const unsigned char* wsmap = d.maps + (int64_t)r.ws_map * TMAP_BYTES;
+        if (lane == 0 && it.seg + 2 < r.seg_end) tma_prefetch_desc(d.maps + (int64_t)sg[2].p2_map * TMAP_BYTES);   // descriptor of the segment after next
         if (r.order == 1) { xmap = wsmap; xrow = trow + u.i0; ymap = opmap; yrow = u.j0; }
         else              { xmap = opmap; xrow = u.i0; ymap = wsmap; yrow = trow + u.j0; }
       } else {

@@ -45,6 +45,11 @@ __device__ __forceinline__ void tma_load_2d(uint32_t dst, const void* tmap, int 
       : "memory");
 }
 
+// fetch a tensor map into the TMA unit's descriptor cache ahead of its first use (short segments change maps every 2-4 stages)
+__device__ __forceinline__ void tma_prefetch_desc(const void* tmap) {
+  asm volatile("prefetch.tensormap [%0];\n" ::"l"(tmap) : "memory");
+}
+
 // D(8x8) += A(8x4,row) * B(4x8,col): lane L, g=L>>2, q=L&3 holds a=A[g][q], b=B[q][g], c0,c1=C[g][2q],C[g][2q+1].
 __device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double b) {
   asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"

@@ -72,6 +72,10 @@ __global__ void __launch_bounds__(NTHREADS, 2) pf_kernel(DevSchedule d) {
       const double* arenaB = (r.order == 1) ? d.b : d.a;
       for (int si = r.seg_begin; si < r.seg_end; ++si) {
         const Seg* sg = d.segs + si;
+        if (TMA && lane == 0 && si + 2 < r.seg_end) {              // descriptors of the segment after next
+          tma_prefetch_desc(d.maps + (int64_t)sg[2].p1_map * TMAP_BYTES);
+          tma_prefetch_desc(d.maps + (int64_t)sg[2].p2_map * TMAP_BYTES);
+        }
         for (int kt = 0; kt < nta + ntb; ++kt) {
           mbar_wait(empty_bar(ring.stage), ring.phase);
           const uint32_t sx = sm.stage(ring.stage), sy = sx + X_BOXES * OP_BYTES, full = full_bar(ring.stage);
