@@ -226,6 +226,7 @@ __global__ void __maxnreg__(136) p1p_kernel(DevSchedule d) {
     for (int t = u.t0; t < u.t1; ++t) {
       const Seg* sg = d.segs + g.seg0 + t;
       OperandSrc x{d.maps + (int64_t)sg->p1_map * TMAP_BYTES, nullptr, sg->p1_ld, u.i0, u.xtrans};
+      if (TMA && lane == 0 && t + 2 < u.t1) tma_prefetch_desc(d.maps + (int64_t)sg[2].p1_map * TMAP_BYTES);   // descriptor of the term after next
       if (!TMA) x.ptr = xarena + sg->p1_off + (u.xtrans ? (int64_t)u.i0 : (int64_t)u.i0 * sg->p1_ld);
       for (int kt = 0; kt < ntiles; ++kt) {
         mbar_wait(sm.empty(ring.stage), ring.phase);
@@ -292,6 +293,7 @@ __global__ void __maxnreg__(136) p2p_kernel(DevSchedule d) {
       const int ntiles = (run.K + KT - 1) / KT;
       for (int seg = run.seg_begin; seg < run.seg_end; ++seg) {
         const Seg* sg = d.segs + seg;
+        if (TMA && lane == 0 && seg + 2 < run.seg_end) tma_prefetch_desc(d.maps + (int64_t)sg[2].p2_map * TMAP_BYTES);
         const int trow = (seg - run.seg0) * run.rows;          // first row of the task inside the stacked intermediate
         const double* wsrows = d.ws + run.ws_off + (int64_t)trow * run.ldw;
         OperandSrc x, y;
