@@ -111,6 +111,32 @@ def test_rotate_right_operators_with_right_isometries():
     assert err <= 1e-12, err
 
 
+def test_rotate_apply_is_graph_capturable():
+    """hpsi_rotate_apply only enqueues (no sync, no allocation): captured into a CUDA graph and replayed."""
+    torch, H = _gpu()
+    p = workloads.make_problem("small", n_terms=20)
+    chi = workloads.proportional_chi(p.d_left, 0.3)
+    ot = workloads.make_isometries(p.d_left, chi, seed=61)
+    a = torch.from_numpy(p.a_data).cuda()
+    r = H.hpsi_rotate_plan(p.d_left, chi, p.a_desc, a, p.a_len)
+    otd = torch.from_numpy(workloads.pack_isometries(ot)).cuda()
+    out = torch.zeros(H.hpsi_rotate_query(r, H.HPSI_RQ_OUT_LENGTH), dtype=torch.float64, device="cuda:0")
+    s = torch.cuda.Stream()
+    s.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(s):
+        H.hpsi_rotate_apply(r, otd, out, s)                 # warm-up outside the capture
+        s.synchronize()
+        expect = out.clone()
+        out.zero_()
+        graph = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(graph, stream=s):
+            H.hpsi_rotate_apply(r, otd, out, s)
+        assert float(out.abs().sum()) == 0.0                # capture enqueued nothing yet
+        graph.replay()
+        s.synchronize()
+    assert torch.equal(out, expect)
+
+
 def test_rotate_nothing_survives():
     torch, H = _gpu()
     p = workloads.make_problem("toy")
