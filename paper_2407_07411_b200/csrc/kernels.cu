@@ -20,6 +20,8 @@
 // conflict-free when the 4 rows of each half-warp have distinct (r & 7) >> 1, so lane group g of a fragment reads row
 // perm(g) = (0,2,4,6,1,3,5,7)[g] of the fragment's 8 rows; the accumulator rows / columns are permuted accordingly
 // when the tile is stored.
+#include <algorithm>
+
 #include "kernels_common.cuh"
 
 namespace hpsi {
@@ -279,9 +281,47 @@ __global__ void prep_kernel(DevSchedule d, const double* __restrict__ psi) {
   }
 }
 
-// reduce: out block = sum of its split-K partials in split order (fixed order -> bitwise reproducible);
-// a block nobody writes (nsplit == 0) becomes zeros (step 5: overwrite semantics).
+// reduce: out block = sum of its split-K partials in a fixed order -> bitwise reproducible; a block nobody writes
+// (nsplit == 0) becomes zeros (step 5: overwrite semantics).  Eight lanes share one element: lane q adds the partials of
+// splits [q * per, (q + 1) * per) in order (eight loads in flight), then the eight sums are added in lane order.  (One
+// thread per element walked up to ~80 dependent L2 round trips: 0.079 -> 0.040 ms of a 0.59 ms apply at D = 1024.)
+// Large vectors are bandwidth-bound and lose with eight rows in flight per warp (cyp 0.115 -> 0.207 ms): they take
+// reduce_plain_kernel below; the launcher picks by size.
+constexpr int RED_LANES = 8;
 __global__ void reduce_kernel(DevSchedule d, double* __restrict__ out, int accumulate) {
+  const PsiBlk B = d.blocks[blockIdx.y];
+  const int n = B.rows * B.cols;
+  const int64_t stride = (int64_t)B.rows * B.ldo;
+  const int q = threadIdx.x & (RED_LANES - 1);
+  const int per = (B.nsplit + RED_LANES - 1) / RED_LANES;
+  const int sp0 = min(q * per, B.nsplit), sp1 = min(sp0 + per, B.nsplit);
+  const int epb = blockDim.x / RED_LANES;                      // elements per block and pass
+  const int n_pad = (n + epb - 1) / epb * epb;                 // whole warps stay in the loop for the shuffles
+  for (int e = blockIdx.x * epb + (threadIdx.x / RED_LANES); e < n_pad; e += gridDim.x * epb) {
+    double s = 0.0;
+    if (e < n) {
+      const int x = e / B.cols, y = e - x * B.cols;
+      const double* p = d.ws + B.part_off + (int64_t)x * B.ldo + y;
+      int sp = sp0;
+      for (; sp + 8 <= sp1; sp += 8) {
+        double v[8];
+#pragma unroll
+        for (int i = 0; i < 8; ++i) v[i] = __ldg(p + (sp + i) * stride);
+#pragma unroll
+        for (int i = 0; i < 8; ++i) s += v[i];
+      }
+      for (; sp < sp1; ++sp) s += __ldg(p + sp * stride);
+    }
+    // lane 0 of the group collects the eight sums in lane order
+    double tot = s;
+#pragma unroll
+    for (int i = 1; i < RED_LANES; ++i) tot += __shfl_sync(0xffffffffu, s, (threadIdx.x & 31 & ~(RED_LANES - 1)) + i);
+    if (q == 0 && e < n) out[B.off + e] = accumulate ? out[B.off + e] + tot : tot;   // hpsi_stream_apply: windows add up in a fixed order
+  }
+}
+
+// the plain form: one thread per element, rows fully coalesced (large vectors; bandwidth-bound)
+__global__ void reduce_plain_kernel(DevSchedule d, double* __restrict__ out, int accumulate) {
   const PsiBlk B = d.blocks[blockIdx.y];
   const int n = B.rows * B.cols;
   const int64_t stride = (int64_t)B.rows * B.ldo;
@@ -289,10 +329,8 @@ __global__ void reduce_kernel(DevSchedule d, double* __restrict__ out, int accum
     const int x = e / B.cols, y = e - x * B.cols;
     const double* p = d.ws + B.part_off + (int64_t)x * B.ldo + y;
     double s = accumulate ? out[B.off + e] : 0.0;           // hpsi_stream_apply: windows of terms add up in a fixed order
-    // eight partials in flight, added in split order: a thread's chain of dependent L2 round trips was the whole
-    // kernel at small D (tens to hundreds of splits of a few-KB block)
     int sp = 0;
-    for (; sp + 8 <= B.nsplit; sp += 8) {
+    for (; sp + 8 <= B.nsplit; sp += 8) {                   // eight partials in flight, added in split order
       double v[8];
 #pragma unroll
       for (int i = 0; i < 8; ++i) v[i] = __ldg(p + (sp + i) * stride);
@@ -360,7 +398,13 @@ void launch_p2(const DevSchedule& d, bool tma, cudaStream_t st) {
   else p2_kernel<false><<<d.n_p2, NTHREADS, SMEM_BYTES, st>>>(d);
 }
 void launch_reduce(const DevSchedule& d, double* out, bool accumulate, cudaStream_t st) {
-  if (d.n_blocks > 0) reduce_kernel<<<elem_grid(d), 256, 0, st>>>(d, out, accumulate ? 1 : 0);
+  if (d.n_blocks == 0) return;
+  const bool small_vec = (int64_t)d.max_block_elems * d.n_blocks <= 400000;     // latency-bound sizes (D <~ 1500)
+  const int lanes = small_vec ? 8 : 1;
+  int gx = (d.max_block_elems + 256 / lanes - 1) / (256 / lanes);
+  gx = std::max(1, std::min(gx, 1024));
+  if (small_vec) reduce_kernel<<<dim3(gx, d.n_blocks), 256, 0, st>>>(d, out, accumulate ? 1 : 0);
+  else reduce_plain_kernel<<<dim3(gx, d.n_blocks), 256, 0, st>>>(d, out, accumulate ? 1 : 0);
 }
 void launch_diag(const DevSchedule& d, double* diag, cudaStream_t st) {
   if (d.n_blocks > 0) diag_kernel<<<elem_grid(d), 256, 0, st>>>(d, diag);
