@@ -2,14 +2,17 @@
 """bench.py - H_eff*psi sustained FP64 TFLOPS on B200 (BASELINE.json metric), one JSON line on stdout.
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--config cyp] [--impl ours|reference]
+                    [--davidson | --site-update | --stream FRAC] [--share-adjoint] [--D D]
 
 A *step* is one pass of the whole hot path (hpsi_apply: prep, first GEMM, second GEMM, reduce) over one seeded
 synthetic psi of the named config (default ``cyp`` = BASELINE.json configs[2], the D=4096 config the metric is
 quoted on).  ``value`` = useful flops (A18: sum over tasks of min(f1, f2)) x steps / device time, inputs
 resident in HBM; ``e2e`` = the same through hpsi_apply_host with pinned HOST psi/out buffers (H2D + D2H inside the
-timed region).  N > 1 (torchrun): the term list is sharded over ranks (operators are the big object), psi is
-replicated and one NCCL all-reduce of psi' per step is inside the timed region; total work is fixed -> "strong".
-``--impl reference`` times the CPU oracle (oracle/, as it stands) on a bounded sample of the same config.
+timed region).  N > 1: one rank per GPU (started by torchrun, or by this script itself when WORLD_SIZE is not set);
+the term list is sharded over the ranks by hpsi_shard_terms (balanced by useful flops; operators are the big object),
+every rank plans its shard with hpsi_plan_ex, psi is replicated, and the exchange step inside the timed region is one
+NCCL all-gather of the partial psi' plus hpsi_sum_shards (rank-ordered sum: same bits on every rank); total work is
+fixed -> "strong".  ``--impl reference`` times the CPU oracle (oracle/, as it stands) on a bounded sample.
 """
 import argparse
 import json
@@ -85,33 +88,92 @@ class ClockSampler:
 
 
 # ------------------------------------------------------------------------------------------------ calibration
-def dgemm_calibration(torch, secs=1.0):
-    """Same-run FP64 tensor-core peak: cuBLAS DGEMM (torch.matmul on float64), best sustained 2N^3/t (north_star)."""
+def dgemm_calibration(torch, secs=2.0, sizes=(4096, 8192, 16384), device_index=0):
+    """Same-run FP64 tensor-core peak: cuBLAS DGEMM (torch.matmul on float64), sustained 2N^3/t over >= ``secs`` of
+    back-to-back launches per N between two CUDA events (no host synchronisation inside the window), SM clocks sampled
+    meanwhile.  Returns (best TFLOP/s, {per-N figures, clocks})."""
     best, detail = 0.0, {}
-    for N in (4096, 8192, 16384):
-        a = torch.randn(N, N, dtype=torch.float64, device="cuda")
-        b = torch.randn(N, N, dtype=torch.float64, device="cuda")
-        c = torch.empty_like(a)
-        for _ in range(2):
-            torch.matmul(a, b, out=c)
-        torch.cuda.synchronize()
-        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        reps, t0 = 0, time.time()
-        e0.record()
-        while True:
-            for _ in range(3):
+    stream = torch.cuda.current_stream()
+    with ClockSampler(device_index) as clk:
+        for N in sizes:
+            a = torch.randn(N, N, dtype=torch.float64, device="cuda")
+            b = torch.randn(N, N, dtype=torch.float64, device="cuda")
+            c = torch.empty_like(a)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            for _ in range(2):
                 torch.matmul(a, b, out=c)
-            reps += 3
+            e0.record(stream)
+            torch.matmul(a, b, out=c)
+            e1.record(stream)
             torch.cuda.synchronize()
-            if time.time() - t0 > secs:
-                break
-        e1.record()
-        torch.cuda.synchronize()
-        tf = 2.0 * N ** 3 * reps / (e0.elapsed_time(e1) * 1e-3) / 1e12
-        detail[f"dgemm_{N}"] = round(tf, 3)
-        best = max(best, tf)
-        del a, b, c
+            reps = max(3, int(np.ceil(secs * 1e3 / max(e0.elapsed_time(e1), 1e-3))))
+            e0.record(stream)
+            for _ in range(reps):
+                torch.matmul(a, b, out=c)
+            e1.record(stream)
+            torch.cuda.synchronize()
+            sec = e0.elapsed_time(e1) * 1e-3
+            tf = 2.0 * N ** 3 * reps / sec / 1e12
+            detail[f"dgemm_{N}"] = round(tf, 3)
+            detail[f"dgemm_{N}_seconds"] = round(sec, 2)
+            best = max(best, tf)
+            del a, b, c
+    detail["clocks"] = clk.summary()
     return best, detail
+
+
+def pipe_probes(H, calib):
+    """Register-resident DMMA / DFMA issue-rate probes (libhpsi_bench.so) next to the DGEMM figure."""
+    for kind, name in ((0, "dmma_pipe_probe"), (1, "dfma_pipe_probe")):
+        ms_pipe, fl_pipe = H.hpsi_bench_fp64_pipe(kind, 20000)
+        calib[name] = round(fl_pipe / ms_pipe / 1e9, 3)
+
+
+def git_head():
+    try:
+        return subprocess.check_output(["git", "-C", ROOT, "rev-parse", "--short", "HEAD"], stderr=subprocess.DEVNULL,
+                                       text=True).strip()
+    except (OSError, subprocess.CalledProcessError):
+        return None
+
+
+def ncu_traffic(key, kernel):
+    """DRAM bytes per launch of ``kernel`` from the committed ncu --set full capture (profiles/ncu_traffic.json.txt),
+    with the commit the capture was taken at, so that a reader can tell whether it describes the kernels being timed."""
+    try:
+        with open(os.path.join(ROOT, "profiles", "ncu_traffic.json.txt")) as fh:
+            tab = json.load(fh)
+    except (OSError, ValueError):
+        return None, None
+    val = tab.get(key, {}).get(kernel)
+    src = {"file": "profiles/ncu_traffic.json.txt", "capture": tab.get("_capture"), "capture_commit": tab.get("_commit"),
+           "bench_commit": git_head()}
+    return val, src
+
+
+def host_cores():
+    """What the CPU baseline ran on: logical CPUs the process may use, and physical cores if /proc/cpuinfo tells."""
+    try:
+        usable = len(os.sched_getaffinity(0))
+    except AttributeError:
+        usable = os.cpu_count()
+    phys = None
+    try:
+        pairs = set()
+        pid = cid = None
+        for line in open("/proc/cpuinfo"):
+            if line.startswith("physical id"):
+                pid = line.split(":")[1].strip()
+            elif line.startswith("core id"):
+                cid = line.split(":")[1].strip()
+            elif not line.strip():
+                if pid is not None and cid is not None:
+                    pairs.add((pid, cid))
+                pid = cid = None
+        phys = len(pairs) or None
+    except OSError:
+        pass
+    return {"logical_cpus_usable": usable, "physical_cores_on_box": phys}
 
 
 def sample_points(p, n, seed=1):
@@ -147,6 +209,7 @@ def cpu_baseline(cfg, budget_s=15.0):
         n = int(max(n + 1, min(half, n * budget_s / max(dt, 1e-3))))
         fl, dt, _ = run(n)
     return {"value": fl / dt / 1e12, "unit": "TFLOPS", "cores": oracle.num_threads(), "kind": "oracle",
+            "cores_detail": {"openmp_threads": oracle.num_threads(), **host_cores()},
             "sample": f"one oracle.apply on the first {n} of {half} base terms + adjoints of {cfg} "
                       f"({fl / 1e9:.2f} useful GF in {dt:.2f} s)"}, fl, dt
 
@@ -314,12 +377,7 @@ def run_site_update(args):
     rot_gbs = algo / (ms_rot * 1e-3) / 1e9
     ridge = dgemm_peak * 1e12 / (hbm_peak * 1e9)
     tensor_bound = rq(H.HPSI_RQ_USEFUL_FLOPS) / max(algo, 1) > ridge
-    traffic = None                       # DRAM bytes of the two launches from the committed ncu --set full capture
-    try:
-        with open(os.path.join(ROOT, "profiles", "ncu_traffic.json.txt")) as fh:
-            traffic = json.load(fh).get(cfg + "_site_update", {}).get("p1_kernel_rot")
-    except (OSError, ValueError):
-        pass
+    traffic, traffic_src = ncu_traffic(cfg + "_site_update", "p1_kernel_rot")   # DRAM bytes of the two launches (ncu --set full)
     # parity on a sample of blocks the oracle rotates one by one, with the device's own isometries
     from oracle import site_update as su
     oth = ot.cpu().numpy()
@@ -362,7 +420,7 @@ def run_site_update(args):
                      "achieved": rot_tf if tensor_bound else rot_gbs, "peak": dgemm_peak if tensor_bound else hbm_peak,
                      "unit": "TFLOP/s" if tensor_bound else "GB/s",
                      "frac": rot_tf / dgemm_peak if tensor_bound else rot_gbs / hbm_peak, "traffic": traffic,
-                     "peak_source": "same-run cuBLAS DGEMM calibration" if tensor_bound else peak_src,
+                     "traffic_source": traffic_src, "peak_source": "same-run cuBLAS DGEMM calibration" if tensor_bound else peak_src,
                      "flops_per_algorithmic_byte": rq(H.HPSI_RQ_USEFUL_FLOPS) / max(algo, 1), "ridge": ridge,
                      "tflops": rot_tf, "algorithmic_gbs": rot_gbs},
         "calibration": {"fp64_tc_peak_tflops": dgemm_peak, **calib},
@@ -375,6 +433,33 @@ def run_site_update(args):
 
 
 # ------------------------------------------------------------------------------------------------- our arm
+def shard_for_rank(cfg, rank, world, share_adjoint=False, D=None):
+    """What rank ``rank`` of ``world`` holds and plans: the library partitions the term list
+    (hpsi_shard_terms, balanced by useful flops, adjoint pairs kept together), the generator fills the arenas of the
+    rank's own terms only, and the returned keyword arguments make hpsi_plan_ex plan exactly that shard.
+    Returns (problem, plan kwargs, useful flops per shard or None)."""
+    if world == 1:
+        return workloads.make_problem(cfg, share_adjoint=share_adjoint, D=D), {}, None
+    import paper_2407_07411_b200 as H
+    desc = workloads.make_problem(cfg, fill=False, share_adjoint=share_adjoint, D=D)
+    half = desc.n_terms // 2
+    shard_of, shard_flops = H.hpsi_shard_terms(desc, world, np.arange(desc.n_terms) % half)
+    p = workloads.make_shard(cfg, shard_of, rank, share_adjoint=share_adjoint, D=D)
+    return p, {"shard_of_term": shard_of, "shard_index": rank}, shard_flops
+
+
+def oracle_samples(cfg, psi, sl, sx, sy, D=None, chunk_terms=64):
+    """Sampled outputs of the UNSHARDED, fully materialised config, the oracle computing them one by one; the terms are
+    streamed through it in chunks so that the host never holds more than ``chunk_terms`` base terms of operators."""
+    import oracle
+    half = workloads.config_params(cfg)["n_terms"] // 2
+    vals = np.zeros(len(sl))
+    for lo in range(0, half, chunk_terms):
+        sp = workloads.make_problem(cfg, base_terms=np.arange(lo, min(half, lo + chunk_terms)), D=D)
+        oracle.apply_samples(sp, psi, sl, sx, sy, vals=vals)
+    return vals
+
+
 def run_ours(args, rank, world, local_rank):
     import torch
     import torch.distributed as dist
@@ -388,63 +473,87 @@ def run_ours(args, rank, world, local_rank):
     H.lib()
 
     cfg = args.config
-    half = workloads.config_params(cfg)["n_terms"] // 2
     t0 = time.time()
-    shard = None if world == 1 else np.arange(rank, half, world)
-    p = workloads.make_problem(cfg, base_terms=shard, share_adjoint=args.share_adjoint, D=args.D)
+    p, plan_kw, shard_flops = shard_for_rank(cfg, rank, world, args.share_adjoint, args.D)
     gen_s = time.time() - t0
     a = torch.from_numpy(p.a_data).to(dev)
     b = torch.from_numpy(p.b_data).to(dev)
+    arena_bytes = int(8 * (p.a_len + p.b_len))
+    keep_host = world == 1 and not args.share_adjoint         # the parity leg's oracle reads the very same host arrays
+    if not keep_host:
+        p.a_data = p.b_data = None
     t0 = time.time()
-    plan = H.plan_problem(p, a, b)
+    plan = H.plan_problem(p, a, b, **plan_kw)
     plan_s = time.time() - t0
     q = lambda w: H.hpsi_query(plan, w)  # noqa: E731
     n = q(H.HPSI_Q_PSI_LENGTH)
-    useful = torch.tensor([q(H.HPSI_Q_USEFUL_FLOPS), q(H.HPSI_Q_OPERATOR_BYTES), q(H.HPSI_Q_N_TASKS)],
-                          dtype=torch.int64, device=dev)
+    sums = torch.tensor([q(H.HPSI_Q_USEFUL_FLOPS), q(H.HPSI_Q_OPERATOR_BYTES), q(H.HPSI_Q_N_TASKS), arena_bytes],
+                        dtype=torch.int64, device=dev)
     if world > 1:
-        dist.all_reduce(useful)
-    useful_flops, operator_bytes, n_tasks = (int(v) for v in useful.tolist())
+        dist.all_reduce(sums)
+    useful_flops, operator_bytes, n_tasks, arena_total = (int(v) for v in sums.tolist())
     log(f"[rank {rank}] {cfg}: gen {gen_s:.1f}s plan {plan_s:.2f}s tasks {q(H.HPSI_Q_N_TASKS)} "
         f"useful {q(H.HPSI_Q_USEFUL_FLOPS) / 1e9:.1f} GF issued {q(H.HPSI_Q_ISSUED_FLOPS) / 1e9:.1f} GF "
         f"operators {q(H.HPSI_Q_OPERATOR_BYTES) / 1e9:.2f} GB workspace {q(H.HPSI_Q_WORKSPACE_BYTES) / 1e9:.2f} GB")
 
-    dgemm_peak, calib = dgemm_calibration(torch)
-    ms_pipe, fl_pipe = H.hpsi_bench_fp64_pipe(0, 20000)
-    calib["dmma_pipe_probe"] = round(fl_pipe / ms_pipe / 1e9, 3)
-    ms_pipe, fl_pipe = H.hpsi_bench_fp64_pipe(1, 20000)
-    calib["dfma_pipe_probe"] = round(fl_pipe / ms_pipe / 1e9, 3)
+    # DGEMM calibration before the timed region (and again after it: same process, interleaved - SURVEY.md 8(d), H6)
+    dgemm_before, calib = dgemm_calibration(torch, device_index=local_rank)
+    pipe_probes(H, calib)
 
     stream = torch.cuda.current_stream()
     n_psi = 10 if cfg == "femoco" else 1                      # A17: 10 different psi's for the FeMoco config
     psis = [torch.from_numpy(workloads.make_psi(p, k)).to(dev) for k in range(n_psi)]
     out = torch.empty(n, dtype=torch.float64, device=dev)
+    parts = torch.empty(world * n, dtype=torch.float64, device=dev) if world > 1 else None
+    mine = parts[rank * n:(rank + 1) * n] if world > 1 else out
 
     def step(i):
-        H.hpsi_apply(plan, psis[i % n_psi], out, stream)
-        if world > 1:
-            dist.all_reduce(out)
+        H.hpsi_apply(plan, psis[i % n_psi], mine, stream)
+        if world > 1:                                         # exchange step: all-gather + rank-ordered sum
+            dist.all_gather_into_tensor(parts, mine)
+            H.hpsi_sum_shards(parts, world, out, stream)
 
     def sync_all():
         if world > 1:
             dist.barrier()
         torch.cuda.synchronize()
 
-    for i in range(args.warmup):
-        step(i)
-    sync_all()
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    with ClockSampler(local_rank) as clk:
+    def timed(fn, steps, sampler=None):
+        """device milliseconds of ``steps`` calls: barrier + synchronize on both sides, events on the launching stream,
+        max over ranks (plus every rank's own figure)"""
+        sync_all()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         e0.record(stream)
-        for i in range(args.steps):
-            step(i)
+        for i in range(steps):
+            fn(i)
         e1.record(stream)
         sync_all()
-    ms = torch.tensor([e0.elapsed_time(e1)], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(ms, op=dist.ReduceOp.MAX)
-    ms_total = float(ms.item())
+        ms = torch.tensor([e0.elapsed_time(e1)], dtype=torch.float64, device=dev)
+        allms = [ms.clone() for _ in range(world)]
+        if world > 1:
+            dist.all_gather(allms, ms)
+        per_rank = [float(x.item()) for x in allms]
+        return max(per_rank), per_rank
+
+    for i in range(args.warmup):
+        step(i)
+    with ClockSampler(local_rank) as clk:
+        ms_total, per_rank_ms = timed(step, args.steps)
     value = useful_flops * args.steps / (ms_total * 1e-3) / 1e12
+
+    # ---- the same, sustained: >= 2 s of back-to-back steps (SURVEY.md 8(d) protocol; the K-step figure above is a burst
+    # when K steps last a fraction of a second)
+    n_sus = max(args.steps, int(np.ceil(2000.0 / max(ms_total / args.steps, 1e-3))))
+    with ClockSampler(local_rank) as clk_sus:
+        ms_sus, _ = timed(step, n_sus)
+    sustained = {"value": useful_flops * n_sus / (ms_sus * 1e-3) / 1e12, "unit": "TFLOPS", "steps": n_sus,
+                 "seconds": ms_sus * 1e-3, "clocks": clk_sus.summary()}
+
+    # ---- compute only (no exchange step): shows the imbalance of the term shards
+    apply_ms = None
+    if world > 1:
+        _, per_rank_apply = timed(lambda i: H.hpsi_apply(plan, psis[i % n_psi], mine, stream), args.steps)
+        apply_ms = [x / args.steps for x in per_rank_apply]
 
     # ---- end to end: pinned HOST psi / out, H2D + D2H inside the timed region
     hpsi_in = [torch.from_numpy(workloads.make_psi(p, k)).pin_memory() for k in range(n_psi)]
@@ -456,44 +565,38 @@ def run_ours(args, rank, world, local_rank):
             H.hpsi_apply_host(plan, hpsi_in[i % n_psi], hout, stream)       # the C-ABI call with HOST buffers
         else:
             xdev.copy_(hpsi_in[i % n_psi], non_blocking=True)
-            H.hpsi_apply(plan, xdev, out, stream)
-            dist.all_reduce(out)
+            H.hpsi_apply(plan, xdev, mine, stream)
+            dist.all_gather_into_tensor(parts, mine)
+            H.hpsi_sum_shards(parts, world, out, stream)
             hout.copy_(out, non_blocking=True)
             torch.cuda.synchronize()
 
     for i in range(min(args.warmup, 3)):
         e2e_step(i)
-    sync_all()
-    e0.record(stream)
-    for i in range(args.steps):
-        e2e_step(i)
-    e1.record(stream)
-    sync_all()
-    ms2 = torch.tensor([e0.elapsed_time(e1)], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(ms2, op=dist.ReduceOp.MAX)
-    e2e_value = useful_flops * args.steps / (float(ms2.item()) * 1e-3) / 1e12
+    ms2, _ = timed(e2e_step, args.steps)
+    e2e_value = useful_flops * args.steps / (ms2 * 1e-3) / 1e12
 
     # ---- roofline of the dominant kernel (live CUDA events between the kernels of an apply)
     prof = np.zeros(4)
     for i in range(3):
-        prof += np.array(H.hpsi_apply_profiled(plan, psis[0], out, stream))
+        prof += np.array(H.hpsi_apply_profiled(plan, psis[0], mine, stream))
     prof /= 3
     names = ["prep_kernel", "p1_kernel (first GEMM)", "p2_kernel (second GEMM)", "reduce_kernel"]
     fl_p1 = q(H.HPSI_Q_USEFUL_FLOPS_P1)
     fl = [0, fl_p1, q(H.HPSI_Q_USEFUL_FLOPS) - fl_p1, 0]
     dom = int(np.argmax(prof))
     achieved = fl[dom] / (prof[dom] * 1e-3) / 1e12 if prof[dom] > 0 else 0.0
-    traffic = None                       # DRAM bytes per launch of that kernel from the committed ncu --set full capture
-    try:
-        with open(os.path.join(ROOT, "profiles", "ncu_traffic.json.txt")) as fh:
-            traffic = json.load(fh).get(cfg, {}).get(names[dom].split()[0])
-    except (OSError, ValueError):
-        pass
+
+    dgemm_after, calib_after = dgemm_calibration(torch, device_index=local_rank)
+    calib["after_timed_region"] = calib_after
+    dgemm_peak = max(dgemm_before, dgemm_after)               # the larger denominator (the smaller fraction)
+    traffic, traffic_src = (None, None)
+    if world == 1 and args.D is None:
+        traffic, traffic_src = ncu_traffic(cfg + ("_share_adjoint" if args.share_adjoint else ""), names[dom].split()[0])
     roofline = {"bound": "tensor", "kernel": names[dom], "achieved": achieved, "peak": dgemm_peak, "unit": "TFLOP/s",
-                "frac": achieved / dgemm_peak, "traffic": traffic,
-                "peak_source": "same-run cuBLAS DGEMM calibration (north_star); DMMA.8x8x4 pipe probe "
-                               f"{calib['dmma_pipe_probe']} TFLOP/s",
+                "frac": achieved / dgemm_peak, "traffic": traffic, "traffic_source": traffic_src,
+                "peak_source": "same-run cuBLAS DGEMM calibration (north_star), best of N = 4096 / 8192 / 16384 sustained "
+                               f">= 2 s each, before and after the timed region; DMMA.8x8x4 pipe probe {calib['dmma_pipe_probe']} TFLOP/s",
                 "kernel_ms": {k: round(float(v), 4) for k, v in zip(names, prof)},
                 "useful_flops_per_launch": int(fl[dom])}
 
@@ -502,43 +605,137 @@ def run_ours(args, rank, world, local_rank):
         "warmup": args.warmup, "ms_per_step": ms_total / args.steps, "higher_is_better": True, "scaling": "strong",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "pct_of_fp64_tc_peak": 100.0 * value / (dgemm_peak * world),
+        "sustained": sustained,
         "operator_gbs": operator_bytes * args.steps / (ms_total * 1e-3) / 1e9,   # operator bytes streamed once per apply
         "config": {"workload": CONFIG_DESC[cfg], "sectors_per_side": int(p.q_left.shape[0]),
                    "D": int(p.d_left.sum()), "terms": int(workloads.config_params(cfg)["n_terms"]), "tasks": n_tasks,
                    "useful_flops_per_step": useful_flops, "operator_bytes": operator_bytes, "psi_length": n,
-                   "parallelism": "1 GPU" if world == 1 else f"term-sharded x{world} + NCCL all-reduce of psi'",
+                   "parallelism": "1 GPU" if world == 1 else
+                   f"terms sharded x{world} (hpsi_shard_terms + hpsi_plan_ex), psi replicated, NCCL all-gather of psi' + "
+                   "hpsi_sum_shards (rank-ordered sum)",
                    "l2": "inputs larger than L2 (operators streamed once per step)",
                    "operator_storage": "adjoint terms share their partner's blocks (read transposed)" if args.share_adjoint
-                   else "every block materialised", "operator_arena_bytes": int(8 * (p.a_len + p.b_len))},
+                   else "every block materialised", "operator_arena_bytes": arena_total,
+                   "schedule": dict(zip(("p1_stages_per_unit", "p2_waves", "p2_min_unit_dmma"), q(H.HPSI_Q_TUNING)))},
         "calibration": {"fp64_tc_peak_tflops": dgemm_peak, **calib},
         "clocks": clk.summary(),
-        "e2e": {"value": e2e_value, "unit": "TFLOPS", "h2d_bytes_per_step": 8 * n, "d2h_bytes_per_step": 8 * n},
-        "gpu_launches": int(q(H.HPSI_Q_LAUNCHES_PER_APPLY)) * args.steps,
+        "e2e": {"value": e2e_value, "unit": "TFLOPS", "h2d_bytes_per_step": 8 * n * world, "d2h_bytes_per_step": 8 * n * world},
+        "gpu_launches": (int(q(H.HPSI_Q_LAUNCHES_PER_APPLY)) + (1 if world > 1 else 0)) * args.steps * world,
         "roofline": roofline,
     }
-    if rank == 0 and world == 1:
-        import oracle
-        # parity spot check on sampled outputs the oracle computes one by one
+    if world > 1:
+        res["ranks"] = {"step_ms": [x / args.steps for x in per_rank_ms], "apply_only_ms": apply_ms,
+                        "apply_only_ms_min_max": [min(apply_ms), max(apply_ms)],
+                        "shard_useful_flops": [int(x) for x in shard_flops],
+                        "exchange_bytes_per_rank_per_step": 8 * n * (world - 1)}
+    # ---- parity spot check on sampled outputs the oracle computes one by one, on the UNSHARDED problem (all ranks ran the
+    # step; rank 0 checks the summed result)
+    step(0)
+    torch.cuda.synchronize()
+    if rank == 0:
         sl, sx, sy, idx = sample_points(p, 32)
         psi0 = workloads.make_psi(p, 0)
-        H.hpsi_apply(plan, psis[0], out, stream)
-        torch.cuda.synchronize()
         got = out.cpu().numpy()[idx]
-        if args.share_adjoint:                   # the oracle only knows fully materialised operators
-            del a, b
-            p = workloads.make_problem(cfg, D=args.D)
-        ref = oracle.apply_samples(p, psi0, sl, sx, sy)
+        del a, b
+        if keep_host:
+            import oracle
+            ref = oracle.apply_samples(p, psi0, sl, sx, sy)
+        else:                                   # the oracle only knows fully materialised, unsharded operators
+            ref = oracle_samples(cfg, psi0, sl, sx, sy, D=args.D)
         res["parity_sample_rel_err"] = float(np.linalg.norm(got - ref) / np.linalg.norm(ref))
-        if not args.share_adjoint:
-            del a, b
         if args.D is None:
             res["cpu_baseline"], _, _ = cpu_baseline(cfg)
         else:
             res["config"]["workload"] += f" with D overridden to {args.D} (bond-dimension sweep, not a BASELINE config)"
-    if rank == 0:
         print(json.dumps(res), flush=True)
     if world > 1:
+        dist.barrier()
         dist.destroy_process_group()
+
+
+# ----------------------------------------------------------------- eigensolver drivers (reading A17)
+def run_davidson(args):
+    """bench.py --davidson: the on-device drivers themselves ("total wall time spent in the Davidson
+    diagonalization").  hpsi_davidson / hpsi_lanczos run a fixed number of mat-vecs (tol = 0 never stops them); reported:
+    time per iteration, time of a bare hpsi_apply, and the driver's overhead = iteration time / apply time - 1."""
+    import torch
+    import paper_2407_07411_b200 as H
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the product has no CPU fallback)")
+    torch.cuda.set_device(0)
+    cfg = args.config
+    p = workloads.make_problem(cfg, D=args.D)
+    a, b = torch.from_numpy(p.a_data).cuda(), torch.from_numpy(p.b_data).cuda()
+    p.a_data = p.b_data = None
+    plan = H.plan_problem(p, a, b)
+    n = H.hpsi_query(plan, H.HPSI_Q_PSI_LENGTH)
+    flops = H.hpsi_query(plan, H.HPSI_Q_USEFUL_FLOPS)
+    stream = torch.cuda.current_stream()
+    psi0 = torch.from_numpy(workloads.make_psi(p)).cuda()
+    out = torch.empty_like(psi0)
+    iters = max(args.steps, 8)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+
+    def time_apply(k):
+        for _ in range(3):
+            H.hpsi_apply(plan, psi0, out, stream)
+        torch.cuda.synchronize()
+        e0.record(stream)
+        for _ in range(k):
+            H.hpsi_apply(plan, psi0, out, stream)
+        e1.record(stream)
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) / k
+
+    res_solvers = {}
+    with ClockSampler(0) as clk:
+        apply_ms = time_apply(iters)
+        for name, fn in (("davidson", H.hpsi_davidson), ("davidson_unpreconditioned", H.hpsi_davidson), ("lanczos", H.hpsi_lanczos)):
+            kw = dict(tol=0.0, max_iter=iters, m_max=16)
+            if name == "davidson_unpreconditioned":
+                kw["precondition"] = False
+            x = psi0.clone()
+            fn(plan, x, stream=stream, **dict(kw, max_iter=4))                  # warm-up (allocates the subspace buffers)
+            best = None
+            for _ in range(3):
+                x.copy_(psi0)
+                torch.cuda.synchronize()
+                t0 = time.perf_counter()
+                e0.record(stream)
+                theta, info = fn(plan, x, stream=stream, **kw)
+                e1.record(stream)
+                torch.cuda.synchronize()
+                wall = (time.perf_counter() - t0) * 1e3
+                ms = e0.elapsed_time(e1)
+                if best is None or ms < best[0]:
+                    best = (ms, wall, theta, info)
+            ms, wall, theta, info = best
+            per_it = ms / info["n_matvec"]
+            res_solvers[name] = {"total_ms": ms, "host_wall_ms": wall, "n_matvec": info["n_matvec"], "ms_per_matvec": per_it,
+                                 "overhead_vs_bare_apply": per_it / apply_ms - 1.0, "theta": theta, "residual": info["residual"],
+                                 "tflops": flops * info["n_matvec"] / (ms * 1e-3) / 1e12}
+        apply_ms_after = time_apply(iters)
+    d = res_solvers["davidson"]
+    print(json.dumps({
+        "metric": "hpsi_davidson sustained FP64 TFLOPS (useful flops of its mat-vecs / total solver time)", "value": d["tflops"],
+        "unit": "TFLOPS", "n_gpus": 1, "steps": d["n_matvec"], "warmup": 4, "ms_per_step": d["ms_per_matvec"],
+        "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": CONFIG_DESC[cfg] + " - eigensolver drivers, fixed mat-vec count (tol = 0)", "psi_length": n,
+                   "m_max": 16, "useful_flops_per_matvec": flops, "D": int(p.d_left.sum()),
+                   "l2": "inputs larger than L2 (operators streamed once per mat-vec)" if cfg not in ("toy", "small") else
+                   "operators fit L2 at this size; the regime is latency-bound (PAPER.md:82 pre-plateau)"},
+        "bare_apply_ms": apply_ms, "bare_apply_ms_after": apply_ms_after, "solvers": res_solvers, "clocks": clk.summary(),
+        "gpu_launches": int(d["n_matvec"] * (H.hpsi_query(plan, H.HPSI_Q_LAUNCHES_PER_APPLY) + 8)),
+    }), flush=True)
+
+
+def free_port():
+    import socket
+    sock = socket.socket()
+    sock.bind(("127.0.0.1", 0))
+    port = sock.getsockname()[1]
+    sock.close()
+    return port
 
 
 def main():
@@ -556,10 +753,25 @@ def main():
                     help="override the config's bond dimension per side (sweep over D as in the paper's Fig. 1-2; 1 GPU)")
     ap.add_argument("--site-update", action="store_true",
                     help="time the steps after the eigen-solve instead: hpsi_truncate + hpsi_rotate_apply (SURVEY 8(f)-4)")
+    ap.add_argument("--davidson", action="store_true",
+                    help="time the eigensolver drivers (hpsi_davidson, hpsi_lanczos) and their overhead over a bare hpsi_apply")
     args = ap.parse_args()
+    if args.gpus < 1:
+        raise SystemExit("bench.py: --gpus must be >= 1")
+    if "WORLD_SIZE" not in os.environ and args.gpus > 1 and args.impl == "ours":
+        # started as plain `python bench.py --gpus N`: become N ranks, one per GPU (same launch the driver uses)
+        import torch
+        have = torch.cuda.device_count()
+        if have < args.gpus:
+            raise SystemExit(f"bench.py: --gpus {args.gpus} but only {have} CUDA device(s) are visible")
+        cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+               "--master-addr", "127.0.0.1", "--master-port", str(free_port()), os.path.abspath(__file__)] + sys.argv[1:]
+        os.execv(sys.executable, cmd)
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if world != args.gpus and args.impl == "ours":
+        raise SystemExit(f"bench.py: --gpus {args.gpus} but WORLD_SIZE is {world}")
     if args.impl == "reference":
         run_reference(args, rank)
     elif args.stream > 0:
@@ -568,6 +780,9 @@ def main():
     elif args.site_update:
         if rank == 0:
             run_site_update(args)
+    elif args.davidson:
+        if rank == 0:
+            run_davidson(args)
     else:
         run_ours(args, rank, world, local_rank)
 

@@ -39,8 +39,9 @@ extern "C" {
                                            Such a plan serves hpsi_query and hpsi_debug_* ; hpsi_apply -> ESTATE. */
 #define HPSI_PLAN_FIXED_ORDER1 (1u << 1) /* diagnostic: force (A psi) B^T for every task                  */
 #define HPSI_PLAN_FIXED_ORDER2 (1u << 2) /* diagnostic: force A (psi B^T) for every task                  */
-#define HPSI_PLAN_NO_FUSION    (1u << 3) /* diagnostic: every task goes through the two-launch path with the workspace */
-#define HPSI_PLAN_FUSE_ALL     (1u << 4) /* diagnostic: fuse every task that fits one CTA tile, whatever the cost model says */
+#define HPSI_PLAN_NO_FUSION    (1u << 3) /* every task goes through the two-launch path with the workspace (the default)  */
+#define HPSI_PLAN_FUSE_ALL     (1u << 4) /* run every task that fits one CTA tile through the fused kernel: both GEMMs in
+                                            one CTA, the intermediate kept in shared memory        */
 
 typedef struct hpsi_plan hpsi_plan_t;   /* opaque; owns the device schedule and the workspace */
 
@@ -92,6 +93,51 @@ typedef struct {
  * CTA work units; uploads the flat schedule and allocates the workspace.  One-off, synchronous. */
 int hpsi_plan(const hpsi_sectors_t* sectors, const hpsi_terms_t* terms, uint32_t flags, hpsi_plan_t** plan_out);
 
+/* hpsi_plan with options.  options == NULL is hpsi_plan.
+ *   struct_bytes        sizeof(hpsi_plan_options_t) as the caller compiled it (lets the struct grow)
+ *   shard_of_term       HOST int32[n_terms] or NULL.  Term sharding for the multi-GPU apply (PAPER.md:27
+ *                       "hybrid CPU-multi GPU", "eight GPU accelerated diagonalization procedure"): only the
+ *                       terms with shard_of_term[t] == shard_index are planned.  The blocks of every other term are
+ *                       ignored and not validated, so the arenas need hold the shard's blocks only (operators are the
+ *                       13-80 GB object; psi is replicated).  The sum over shard_index of the shards' H psi is H psi.
+ *                       hpsi_shard_terms below produces a balanced assignment.
+ *   p1_stages_per_unit  schedule knobs, 0 = automatic: staged K-tiles per CTA of the first-GEMM kernel; waves of CTAs the
+ *   p2_waves            second GEMM's split-K aims at; least DMMA count per second-GEMM CTA.  They change the schedule
+ *   p2_min_unit_dmma    (and so the rounding order of the sums), never the result beyond that; HPSI_Q_TUNING reports
+ *                       the values a plan was built with. */
+typedef struct {
+  uint32_t struct_bytes;
+  int32_t shard_index;
+  const int32_t* shard_of_term;
+  int32_t p1_stages_per_unit;
+  int32_t p2_waves;
+  int32_t p2_min_unit_dmma;
+  int32_t reserved;
+} hpsi_plan_options_t;
+int hpsi_plan_ex(const hpsi_sectors_t* sectors, const hpsi_terms_t* terms, uint32_t flags,
+                 const hpsi_plan_options_t* options, hpsi_plan_t** plan_out);
+
+/* Balanced partition of the term list over `shard_count` ranks ("Partition the terms (balanced by
+ * useful_flops ...)").  HOST only, deterministic (every rank computes the same answer): bundles of terms are sorted by
+ * useful flops (descending, ties by lowest term) and dealt greedily to the lightest shard so far (ties: lowest index).
+ *   terms              descriptors only (coef, arenas, ld and offset are not read)
+ *   bundle_of_term     HOST int32[n_terms] or NULL: terms with the same value stay on one rank - e.g. a term and its
+ *                      adjoint when the adjoint reads its partner's storage (a_transposed); NULL = every term alone
+ *   shard_of_term      HOST out, int32[n_terms], values 0..shard_count-1
+ *   shard_flops        HOST out or NULL, int64[shard_count]: useful flops of every shard */
+int hpsi_shard_terms(const hpsi_sectors_t* sectors, const hpsi_terms_t* terms, const int32_t* bundle_of_term,
+                     int32_t shard_count, int32_t* shard_of_term, int64_t* shard_flops);
+
+/* The operator-arena layout the kernels like best, written into the descriptors (SURVEY.md 8(b) "preferred ld / arena
+ * layout"; HPSI_Q_PREFERRED_LAYOUT gives the rule as numbers).  For every descriptor, in the order given: ld = stored
+ * columns rounded up to 4 doubles, offset = running total rounded up to 4 doubles (every row starts on a 32-byte L2
+ * sector and is a legal TMA row).  A block flagged transposed stores d[col] x d[row].  Blocks with ld == -1 on input
+ * share storage with another descriptor and are skipped (the caller copies offset / ld from its partner).
+ * blocks: HOST, in/out; d: HOST sector dims of that side; transposed: HOST or NULL; arena_len: HOST out, doubles.
+ * Use: describe -> hpsi_layout_blocks (both sides) -> fill the arenas -> hpsi_plan (arenas may be NULL) -> hpsi_bind. */
+int hpsi_layout_blocks(int32_t n_sectors, const int32_t* d, int64_t n_blocks, hpsi_opblock_t* blocks,
+                       const uint8_t* transposed, int64_t* arena_len);
+
 /* (Re)bind the DEVICE operator arenas (same descriptors).  Re-encodes the tensor maps of the operand matrices
  * (host work proportional to the number of blocks; synchronous). */
 int hpsi_bind(hpsi_plan_t* plan, const double* a_data_dev, const double* b_data_dev);
@@ -99,15 +145,24 @@ int hpsi_bind(hpsi_plan_t* plan, const double* a_data_dev, const double* b_data_
 /* Per-task coupling coefficients (reading A4): replaces the coefficient of every task,
  * which hpsi_plan initialises to c_term - e.g. SU(2) recoupling factors that depend on the sector quadruple
  * (l, l', r, r') and not only on the term ("spin adapted", "SU(2)-aware").
- * coef_host: HOST, n doubles with n == HPSI_Q_N_TASKS, in HPSI_Q_TASKS order.  Synchronous; must not be called while
- * an apply of this plan is in flight.  hpsi_apply, hpsi_diagonal and hpsi_davidson all use the new values. */
-int hpsi_set_task_coefficients(hpsi_plan_t* plan, const double* coef_host, int64_t n);
+ * coef_host: HOST, n doubles with n == HPSI_Q_N_TASKS, in HPSI_Q_TASKS order (copied before the call returns).
+ * Stream-ordered: the device tables are updated by copies enqueued on cuda_stream, so applies enqueued on that stream
+ * before the call see the old values and applies enqueued after it the new ones; no device-wide synchronisation.
+ * hpsi_apply, hpsi_diagonal, hpsi_davidson and hpsi_lanczos all use the new values. */
+int hpsi_set_task_coefficients(hpsi_plan_t* plan, const double* coef_host, int64_t n, void* cuda_stream);
 
 /* Steps 5-7: out = H psi (overwrite).  psi_dev / out_dev: DEVICE, psi_length doubles each, must not alias.
  * cuda_stream: a cudaStream_t cast to void* (NULL = default stream).  Enqueue only: no host sync, no
  * allocation, CUDA-graph capturable.  A plan owns one workspace: do not run it on two streams at once.
  * Repeated applies on the same inputs are bitwise identical (no atomics on data). */
 int hpsi_apply(hpsi_plan_t* plan, const double* psi_dev, double* out_dev, void* cuda_stream);
+
+/* Exchange step of the term-sharded apply: out[i] = parts[0*n + i] + parts[1*n + i] + ... added in
+ * that order.  Each rank hpsi_apply's its shard, the partial results are all-gathered (NCCL; psi' is 5-17 MB) into
+ * parts_dev in rank order, and this sum gives every rank the same bits on every run - a library all-reduce does not
+ * promise its summation order.  parts_dev: DEVICE, n_parts * n doubles; out_dev: DEVICE, n doubles, may equal
+ * parts_dev (in place over shard 0) but must not overlap it otherwise.  Enqueue only. */
+int hpsi_sum_shards(const double* parts_dev, int32_t n_parts, int64_t n, double* out_dev, void* cuda_stream);
 
 /* hpsi_apply with a CUDA event between its kernels: ms_host (HOST, 4 floats) receives the device time of
  * [prep, first-GEMM kernel, second-GEMM kernel, reduce].  Synchronises the stream.  For bench.py's roofline object. */
@@ -272,8 +327,23 @@ enum {
   HPSI_Q_PSI_COLS = 23,      /* int64: sum of d_right over the psi blocks (sigma_host length for HPSI_SIDE_RIGHT)  */
   HPSI_Q_ISO_CAPACITY_RIGHT = 24, /* int64: sum of min(d_left, d_right) * d_right over the psi blocks             */
   HPSI_Q_N_FUSED_UNITS = 25, /* int64: CTA work units of the fused kernel (both GEMMs of a task in one CTA)       */
-  HPSI_Q_N_FUSED_TASKS = 26  /* int64: tasks whose intermediate never leaves the chip                             */
+  HPSI_Q_N_FUSED_TASKS = 26, /* int64: tasks whose intermediate never leaves the chip                             */
+  HPSI_Q_TUNING = 27,        /* int64[3]: schedule knobs the plan was built with (hpsi_plan_options_t): first-GEMM K-tiles
+                                per CTA, second-GEMM waves, least DMMA count per second-GEMM CTA                    */
+  HPSI_Q_PREFERRED_LAYOUT = 28, /* hpsi_layout_t: the operator-arena layout rule (what hpsi_layout_blocks applies)    */
+  HPSI_Q_N_TERMS_PLANNED = 29   /* int64: terms of this plan's shard (= n_terms without hpsi_plan_options_t.shard_of_term) */
 };
+
+/* Layout rule of the operator arenas.  A block's rows are `stored columns` doubles long (d[col], or
+ * d[row] when the block is flagged transposed) with leading dimension ld. */
+typedef struct {
+  int32_t ld_multiple;           /* preferred: ld a multiple of this many doubles (4: rows start on 32-byte L2 sectors) */
+  int32_t offset_multiple;       /* preferred: block offsets a multiple of this many doubles (4)                       */
+  int32_t tma_ld_multiple;       /* required for the TMA staging path: ld and offset multiples of this (2 = 16 bytes);  */
+  int32_t tma_offset_multiple;   /*   anything else runs the 8-byte cp.async kernels (correct, slower)                  */
+  int32_t arena_align_bytes;     /* required for the TMA path: arena base address alignment (16)                        */
+  int32_t transposed_pad_rows;   /* tiles of a plan with transposed blocks are padded to this many rows (16; plain: 8)  */
+} hpsi_layout_t;
 
 typedef struct {
   int32_t left, right;   /* sector indices                     */
@@ -292,12 +362,6 @@ int hpsi_query(const hpsi_plan_t* plan, int what, void* out, size_t bytes);
 void hpsi_destroy(hpsi_plan_t* plan);
 
 const char* hpsi_last_error(void);
-
-/* FP64 tensor-pipe microbenchmarks used by bench.py's calibration: run `iters`
- * dependent-chain rounds of register-resident DMMA.8x8x4 (kind 0), DFMA (kind 1) or both interleaved (kind 2)
- * on every SM (4 CTAs of 8 warps per SM) and return the elapsed milliseconds and the flops executed; kind 100+w runs
- * the DMMA probe with w one-warp CTAs (1..32) per SM (occupancy sensitivity of the pipe).  HOST outputs. */
-int hpsi_bench_fp64_pipe(int kind, int iters, double* ms_out, double* flops_out);
 
 /* ---- debug / test entry points (HOST memory only; run the *device schedule* with naive loops on the CPU) ----
  * hpsi_debug_interpret executes exactly the work-unit tables the kernels consume (prep, first GEMM units,

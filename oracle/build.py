@@ -10,7 +10,7 @@ LIB = os.path.join(HERE, "liboracle.so")
 def build(force: bool = False) -> str:
     if (not force and os.path.exists(LIB) and os.path.getmtime(LIB) >= os.path.getmtime(SRC)):
         return LIB
-    # no -ffast-math: the summation order written in the source is the one executed
+    # no -ffast-math: nothing is re-associated except the one dot product the source marks `omp simd reduction`
     cmd = ["gcc", "-O3", "-march=native", "-fopenmp", "-fPIC", "-shared", "-Wall", "-Wextra", "-o", LIB, SRC]
     subprocess.check_call(cmd)
     return LIB

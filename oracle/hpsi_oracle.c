@@ -13,7 +13,10 @@
  *
  * Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may use this
  * file.  It shares no code, header, table or ordering with paper_2407_07411_b200/ (the CUDA path):
- * always the (A psi) B^T order, naive loops, one writer per output element, fixed summation order.
+ * always the (A psi) B^T order, naive loops, one writer per output element, loop order = order of the additions into
+ * an output element.  One exception, stated here because it is not "as written": the inner dot product over y' of the
+ * second product carries `omp simd reduction(+)`, so the compiler may add it up as a few lane-wise partial sums (still
+ * deterministic for a given build; the difference is at rounding level, far below the 1e-12 bar).
  *
  * Pins (tests/test_oracle_pins.py): brute-force Kronecker expansion, Hermiticity, single-block = A@psi@B.T,
  * closed forms (identity, rank-1, linearity, power-of-two scaling), Hubbard dimer / 4-site chain energies.
@@ -91,8 +94,9 @@ static int term_index(int32_t n_terms, int64_t n, const oracle_opblock_t* blk, i
  *        T[x,y']   = sum_{x'} a[x,x'] psi_{l'}[x',y']
  *        out_l[x,y] += c_t * sum_{y'} T[x,y'] b[y,y']
  * Blocks of one term are looked up by scanning the descriptor arrays in the order given.
- * OpenMP is over the rows x of one task only, so every output element has one writer and the
- * order of additions into it is the loop order above. Returns 0, or -1 on allocation failure. */
+ * OpenMP is over the rows x of one task only, so every output element has one writer and the order of the
+ * task contributions added into it is the loop order above (inside one contribution the y' dot product is a simd
+ * reduction, see the file header).  Returns 0, or -1 on allocation failure. */
 int oracle_apply(int32_t n_left, int32_t n_right, const int32_t* q_left, const int32_t* q_right,
                  const int32_t* d_left, const int32_t* d_right, const int32_t* target,
                  int32_t n_terms, const double* coef,

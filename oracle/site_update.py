@@ -14,7 +14,8 @@ from ``paper_2407_07411_b200`` and shares no code with it.
 
 Pins: tests/test_oracle_site_pins.py (eigenvalues of psi psi^T, Eckart-Young discarded weight, rank-1 and diagonal
 closed forms from tests/golden/site_update_closed_forms.txt, dense embedding O^T A O with einsum, identity and
-orthogonal-invariance special cases, and  (O^T (x) 1) H (O (x) 1)  against the pinned ``oracle.apply``).
+orthogonal-invariance special cases,  (O^T (x) 1) H (O (x) 1)  against the pinned ``oracle.apply``, and ``rotate_flops``
+against flops counted by hand block by block, golden item 6, plus the x8 doubling law).
 """
 from __future__ import annotations
 

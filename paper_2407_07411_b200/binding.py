@@ -10,7 +10,7 @@ from typing import Optional
 
 import numpy as np
 
-from .build import LIB, build
+from .build import BENCH_LIB, LIB, build, build_bench
 
 HPSI_OK, HPSI_EINVAL, HPSI_ENOMEM, HPSI_ECUDA, HPSI_ESTATE = 0, -1, -2, -3, -4
 HPSI_PLAN_HOST_ONLY = 1 << 0
@@ -24,7 +24,7 @@ HPSI_PLAN_FUSE_ALL = 1 << 4
  HPSI_Q_N_ORDER1_TASKS, HPSI_Q_LAUNCHES_PER_APPLY, HPSI_Q_ALIGNED16, HPSI_Q_INTERMEDIATE_BYTES,
  HPSI_Q_ISSUED_FLOPS_P1, HPSI_Q_TASKS, HPSI_Q_USEFUL_FLOPS_P1, HPSI_Q_CRITICAL_FLOPS, HPSI_Q_PSI_ROWS,
  HPSI_Q_ISO_CAPACITY, HPSI_Q_SVD_SWEEPS, HPSI_Q_SVD_LAUNCHES, HPSI_Q_PSI_COLS, HPSI_Q_ISO_CAPACITY_RIGHT,
- HPSI_Q_N_FUSED_UNITS, HPSI_Q_N_FUSED_TASKS) = range(27)
+ HPSI_Q_N_FUSED_UNITS, HPSI_Q_N_FUSED_TASKS, HPSI_Q_TUNING, HPSI_Q_PREFERRED_LAYOUT, HPSI_Q_N_TERMS_PLANNED) = range(30)
 HPSI_SIDE_LEFT, HPSI_SIDE_RIGHT = 0, 1
 (HPSI_RQ_OUT_LENGTH, HPSI_RQ_OUT_BLOCKS, HPSI_RQ_ISO_LENGTH, HPSI_RQ_USEFUL_FLOPS, HPSI_RQ_ALGO_BYTES,
  HPSI_RQ_WORKSPACE_BYTES, HPSI_RQ_N_UNITS_1, HPSI_RQ_N_UNITS_2, HPSI_RQ_ALIGNED16, HPSI_RQ_INTERMEDIATE_BYTES) = range(10)
@@ -50,6 +50,17 @@ class hpsi_terms_t(ctypes.Structure):
                 ("a_data", ctypes.c_void_p), ("b_data", ctypes.c_void_p),
                 ("a_len", ctypes.c_int64), ("b_len", ctypes.c_int64),
                 ("a_transposed", ctypes.c_void_p), ("b_transposed", ctypes.c_void_p)]
+
+
+class hpsi_plan_options_t(ctypes.Structure):
+    _fields_ = [("struct_bytes", ctypes.c_uint32), ("shard_index", ctypes.c_int32), ("shard_of_term", ctypes.c_void_p),
+                ("p1_stages_per_unit", ctypes.c_int32), ("p2_waves", ctypes.c_int32),
+                ("p2_min_unit_dmma", ctypes.c_int32), ("reserved", ctypes.c_int32)]
+
+
+class hpsi_layout_t(ctypes.Structure):
+    _fields_ = [(n, ctypes.c_int32) for n in ("ld_multiple", "offset_multiple", "tma_ld_multiple", "tma_offset_multiple",
+                                              "arena_align_bytes", "transposed_pad_rows")]
 
 
 class hpsi_davidson_params_t(ctypes.Structure):
@@ -79,10 +90,16 @@ def lib() -> ctypes.CDLL:
         vp, i32, i64 = ctypes.c_void_p, ctypes.c_int32, ctypes.c_int64
         L.hpsi_plan.argtypes = [ctypes.POINTER(hpsi_sectors_t), ctypes.POINTER(hpsi_terms_t), ctypes.c_uint32,
                                 ctypes.POINTER(vp)]
+        L.hpsi_plan_ex.argtypes = [ctypes.POINTER(hpsi_sectors_t), ctypes.POINTER(hpsi_terms_t), ctypes.c_uint32,
+                                   ctypes.POINTER(hpsi_plan_options_t), ctypes.POINTER(vp)]
+        L.hpsi_shard_terms.argtypes = [ctypes.POINTER(hpsi_sectors_t), ctypes.POINTER(hpsi_terms_t), vp, i32, vp, vp]
+        L.hpsi_layout_blocks.argtypes = [i32, vp, i64, vp, vp, ctypes.POINTER(i64)]
         L.hpsi_bind.argtypes = [vp, vp, vp]
-        L.hpsi_set_task_coefficients.argtypes = [vp, vp, i64]
+        L.hpsi_set_task_coefficients.argtypes = [vp, vp, i64, vp]
         L.hpsi_apply.argtypes = [vp, vp, vp, vp]
         L.hpsi_apply_host.argtypes = [vp, vp, vp, vp]
+        L.hpsi_sum_shards.argtypes = [vp, i32, i64, vp, vp]
+        L.hpsi_sum_shards.restype = ctypes.c_int
         L.hpsi_apply_profiled.argtypes = [vp, vp, vp, vp, ctypes.POINTER(ctypes.c_float)]
         L.hpsi_diagonal.argtypes = [vp, vp, vp]
         L.hpsi_davidson.argtypes = [vp, vp, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(hpsi_davidson_params_t),
@@ -100,8 +117,6 @@ def lib() -> ctypes.CDLL:
         L.hpsi_destroy.argtypes = [vp]
         L.hpsi_destroy.restype = None
         L.hpsi_last_error.restype = ctypes.c_char_p
-        L.hpsi_bench_fp64_pipe.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.POINTER(ctypes.c_double),
-                                           ctypes.POINTER(ctypes.c_double)]
         L.hpsi_debug_interpret.argtypes = [vp, vp, vp, vp, vp]
         L.hpsi_truncate.argtypes = [vp, vp, ctypes.c_int32, ctypes.c_int32, ctypes.c_double, vp, vp, vp, vp, vp]
         L.hpsi_rotate_plan.argtypes = [ctypes.c_int32, vp, vp, i64, vp, vp, i64, ctypes.c_uint32, ctypes.POINTER(vp)]
@@ -114,8 +129,9 @@ def lib() -> ctypes.CDLL:
         for name in ("hpsi_truncate", "hpsi_rotate_plan", "hpsi_rotate_apply", "hpsi_rotate_apply_profiled",
                      "hpsi_rotate_query", "hpsi_rotate_debug_interpret"):
             getattr(L, name).restype = ctypes.c_int
-        for name in ("hpsi_plan", "hpsi_bind", "hpsi_set_task_coefficients", "hpsi_apply", "hpsi_apply_host", "hpsi_apply_profiled", "hpsi_diagonal", "hpsi_davidson", "hpsi_lanczos",
-                     "hpsi_query", "hpsi_bench_fp64_pipe", "hpsi_debug_interpret"):
+        for name in ("hpsi_plan", "hpsi_plan_ex", "hpsi_shard_terms", "hpsi_layout_blocks", "hpsi_bind",
+                     "hpsi_set_task_coefficients", "hpsi_apply", "hpsi_apply_host", "hpsi_apply_profiled", "hpsi_diagonal",
+                     "hpsi_davidson", "hpsi_lanczos", "hpsi_query", "hpsi_debug_interpret"):
             getattr(L, name).restype = ctypes.c_int
         del i32, i64
         _lib = L
@@ -161,10 +177,9 @@ class Plan:
             self.handle = None
 
 
-def hpsi_plan(q_left, q_right, d_left, d_right, target, coef, a_blocks, b_blocks, a_data=None, b_data=None,
-              a_len: int = 0, b_len: int = 0, flags: int = 0, a_transposed=None, b_transposed=None) -> Plan:
-    """hpsi_plan(sector table, term list).  Host arrays: numpy; a_blocks/b_blocks: numpy arrays with the 24-byte
-    hpsi_opblock_t layout; a_data/b_data: torch CUDA float64 tensors (or None, to hpsi_bind later)."""
+def _marshal(q_left, q_right, d_left, d_right, target, coef, a_blocks, b_blocks, a_data, b_data, a_len, b_len,
+             a_transposed, b_transposed):
+    """(hpsi_sectors_t, hpsi_terms_t, arrays to keep alive) from numpy / torch arguments."""
     q_left = np.ascontiguousarray(q_left, np.int32).reshape(-1, 2)
     q_right = np.ascontiguousarray(q_right, np.int32).reshape(-1, 2)
     d_left = np.ascontiguousarray(d_left, np.int32)
@@ -184,11 +199,56 @@ def hpsi_plan(q_left, q_right, d_left, d_right, target, coef, a_blocks, b_blocks
     trm = hpsi_terms_t(coef.shape[0], coef.ctypes.data, a_blocks.shape[0], a_blocks.ctypes.data,
                        b_blocks.shape[0], b_blocks.ctypes.data, _ptr(a_data), _ptr(b_data), int(a_len), int(b_len),
                        _ptr(a_transposed), _ptr(b_transposed))
+    return sec, trm, (q_left, q_right, d_left, d_right, coef, a_blocks, b_blocks, a_transposed, b_transposed)
+
+
+def hpsi_plan(q_left, q_right, d_left, d_right, target, coef, a_blocks, b_blocks, a_data=None, b_data=None,
+              a_len: int = 0, b_len: int = 0, flags: int = 0, a_transposed=None, b_transposed=None,
+              shard_of_term=None, shard_index: int = 0, p1_stages_per_unit: int = 0, p2_waves: int = 0,
+              p2_min_unit_dmma: int = 0) -> Plan:
+    """hpsi_plan / hpsi_plan_ex(sector table, term list).  Host arrays: numpy; a_blocks/b_blocks: numpy arrays with the
+    24-byte hpsi_opblock_t layout; a_data/b_data: torch CUDA float64 tensors (or None, to hpsi_bind later).  Any of the
+    keyword options of hpsi_plan_options_t (term shard, schedule knobs) routes the call through hpsi_plan_ex."""
+    sec, trm, keep = _marshal(q_left, q_right, d_left, d_right, target, coef, a_blocks, b_blocks, a_data, b_data,
+                              a_len, b_len, a_transposed, b_transposed)
     out = ctypes.c_void_p()
-    _check(lib().hpsi_plan(ctypes.byref(sec), ctypes.byref(trm), flags, ctypes.byref(out)))
+    if shard_of_term is not None or p1_stages_per_unit or p2_waves or p2_min_unit_dmma:
+        sot = None
+        if shard_of_term is not None:
+            sot = np.ascontiguousarray(shard_of_term, np.int32)
+            assert sot.shape[0] == trm.n_terms
+        opt = hpsi_plan_options_t(ctypes.sizeof(hpsi_plan_options_t), int(shard_index), _ptr(sot),
+                                  int(p1_stages_per_unit), int(p2_waves), int(p2_min_unit_dmma), 0)
+        _check(lib().hpsi_plan_ex(ctypes.byref(sec), ctypes.byref(trm), flags, ctypes.byref(opt), ctypes.byref(out)))
+    else:
+        _check(lib().hpsi_plan(ctypes.byref(sec), ctypes.byref(trm), flags, ctypes.byref(out)))
     pl = Plan(out.value, (a_data, b_data))
-    pl.n_left, pl.n_right = q_left.shape[0], q_right.shape[0]
+    pl.n_left, pl.n_right = sec.n_left, sec.n_right
     return pl
+
+
+def hpsi_shard_terms(p, shard_count: int, bundle_of_term=None):
+    """Balanced term partition of a ``workloads.Problem``-like object: (shard_of_term int32[n_terms], shard_flops
+    int64[shard_count])."""
+    sec, trm, keep = _marshal(p.q_left, p.q_right, p.d_left, p.d_right, p.target, p.coef, p.a_desc, p.b_desc, None, None,
+                              0, 0, None, None)
+    bundle = None if bundle_of_term is None else np.ascontiguousarray(bundle_of_term, np.int32)
+    shard = np.zeros(max(trm.n_terms, 1), np.int32)
+    fl = np.zeros(int(shard_count), np.int64)
+    _check(lib().hpsi_shard_terms(ctypes.byref(sec), ctypes.byref(trm), _ptr(bundle), int(shard_count), shard.ctypes.data,
+                                  fl.ctypes.data))
+    return shard[:trm.n_terms], fl
+
+
+def hpsi_layout_blocks(d, blocks, transposed=None):
+    """Write the preferred ld / offset into a copy of the descriptors; returns (blocks, arena_len)."""
+    d = np.ascontiguousarray(d, np.int32)
+    blocks = np.array(blocks, copy=True)
+    assert blocks.dtype.itemsize == 24
+    tr = None if transposed is None else np.ascontiguousarray(transposed, np.uint8)
+    n = ctypes.c_int64()
+    _check(lib().hpsi_layout_blocks(d.shape[0], d.ctypes.data, blocks.shape[0], blocks.ctypes.data, _ptr(tr), ctypes.byref(n)))
+    return blocks, n.value
 
 
 def hpsi_bind(plan: Plan, a_data, b_data) -> None:
@@ -196,15 +256,20 @@ def hpsi_bind(plan: Plan, a_data, b_data) -> None:
     plan._keep = (a_data, b_data)
 
 
-def hpsi_set_task_coefficients(plan: Plan, coef) -> None:
-    """Per-task coefficients (numpy float64, HPSI_Q_TASKS order) replacing c_term."""
+def hpsi_set_task_coefficients(plan: Plan, coef, stream=None) -> None:
+    """Per-task coefficients (numpy float64, HPSI_Q_TASKS order) replacing c_term; ordered on ``stream``."""
     coef = np.ascontiguousarray(coef, np.float64)
-    _check(lib().hpsi_set_task_coefficients(plan.handle, coef.ctypes.data, coef.shape[0]))
+    _check(lib().hpsi_set_task_coefficients(plan.handle, coef.ctypes.data, coef.shape[0], _stream(stream)))
 
 
 def hpsi_apply(plan: Plan, psi, out, stream=None) -> None:
     """out = H psi; psi/out: torch CUDA float64 tensors of psi_length; stream: torch.cuda.Stream or None."""
     _check(lib().hpsi_apply(plan.handle, _ptr(psi), _ptr(out), _stream(stream)))
+
+
+def hpsi_sum_shards(parts, n_parts: int, out, stream=None) -> None:
+    """out = sum over r of parts[r*n:(r+1)*n] in rank order (parts: torch CUDA tensor of n_parts * n doubles)."""
+    _check(lib().hpsi_sum_shards(_ptr(parts), int(n_parts), int(out.numel()), _ptr(out), _stream(stream)))
 
 
 def hpsi_apply_profiled(plan: Plan, psi, out, stream=None):
@@ -290,6 +355,14 @@ def hpsi_stream_query(sp: StreamPlan, what: int) -> int:
 
 def hpsi_query(plan: Plan, what: int):
     """Scalar items return int; HPSI_Q_PSI_BLOCKS / HPSI_Q_TASKS return structured numpy arrays."""
+    if what == HPSI_Q_TUNING:
+        arr = np.zeros(3, np.int64)
+        _check(lib().hpsi_query(plan.handle, what, arr.ctypes.data, arr.nbytes))
+        return [int(v) for v in arr]
+    if what == HPSI_Q_PREFERRED_LAYOUT:
+        lay = hpsi_layout_t()
+        _check(lib().hpsi_query(plan.handle, what, ctypes.addressof(lay), ctypes.sizeof(lay)))
+        return {n: getattr(lay, n) for n, _ in hpsi_layout_t._fields_}
     if what in (HPSI_Q_PSI_BLOCKS, HPSI_Q_TASKS):
         n = hpsi_query(plan, HPSI_Q_N_PSI_BLOCKS if what == HPSI_Q_PSI_BLOCKS else HPSI_Q_N_TASKS)
         arr = np.zeros(max(n, 1), PSI_BLOCK_DTYPE if what == HPSI_Q_PSI_BLOCKS else TASK_DTYPE)
@@ -300,10 +373,28 @@ def hpsi_query(plan: Plan, what: int):
     return v.value
 
 
+_bench_lib = None
+
+
+def bench_lib() -> ctypes.CDLL:
+    """libhpsi_bench.so (include/hpsi_bench.h): calibration probes, loaded by bench.py only."""
+    global _bench_lib
+    if _bench_lib is None:
+        L = ctypes.CDLL(build_bench() if not os.environ.get("HPSI_NO_BUILD") else BENCH_LIB)
+        L.hpsi_bench_fp64_pipe.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.POINTER(ctypes.c_double),
+                                           ctypes.POINTER(ctypes.c_double)]
+        L.hpsi_bench_fp64_pipe.restype = ctypes.c_int
+        L.hpsi_bench_last_error.restype = ctypes.c_char_p
+        _bench_lib = L
+    return _bench_lib
+
+
 def hpsi_bench_fp64_pipe(kind: int, iters: int):
     """(milliseconds, flops) of the register-resident FP64 pipe probe (0 DMMA, 1 DFMA, 2 both)."""
     ms, fl = ctypes.c_double(), ctypes.c_double()
-    _check(lib().hpsi_bench_fp64_pipe(kind, iters, ctypes.byref(ms), ctypes.byref(fl)))
+    rc = bench_lib().hpsi_bench_fp64_pipe(kind, iters, ctypes.byref(ms), ctypes.byref(fl))
+    if rc != 0:
+        raise HpsiError(rc, bench_lib().hpsi_bench_last_error().decode())
     return ms.value, fl.value
 
 
@@ -384,7 +475,8 @@ def hpsi_rotate_debug_interpret(r: RotatePlan, a_host: np.ndarray, ot_host: np.n
     return out
 
 
-def plan_problem(p, a_data=None, b_data=None, flags: int = 0) -> Plan:
-    """Marshal a ``workloads.Problem`` (any object with the boundary's fields) into hpsi_plan."""
+def plan_problem(p, a_data=None, b_data=None, flags: int = 0, **options) -> Plan:
+    """Marshal a ``workloads.Problem`` (any object with the boundary's fields) into hpsi_plan / hpsi_plan_ex."""
     return hpsi_plan(p.q_left, p.q_right, p.d_left, p.d_right, p.target, p.coef, p.a_desc, p.b_desc,
-                     a_data, b_data, p.a_len, p.b_len, flags, getattr(p, "a_trans", None), getattr(p, "b_trans", None))
+                     a_data, b_data, p.a_len, p.b_len, flags, getattr(p, "a_trans", None), getattr(p, "b_trans", None),
+                     **options)

@@ -71,7 +71,6 @@ int upload_schedule(hpsi_plan_t* p) {
   p->dev.n_pf = (int)sc.pf.size();
   p->dev.max_block_elems = sc.max_block_elems;
   p->dev.paired = sc.paired ? 1 : 0;
-  p->dev.debug = getenv("HPSI_DEBUG") ? atoi(getenv("HPSI_DEBUG")) : 0;
   if (sc.psi_len > 0) {
     HPSI_CUDA(cudaMalloc(&p->d_psi_stage, (size_t)sc.psi_len * sizeof(double)));
     HPSI_CUDA(cudaMalloc(&p->d_out_stage, (size_t)sc.psi_len * sizeof(double)));
@@ -81,7 +80,7 @@ int upload_schedule(hpsi_plan_t* p) {
 
 void free_plan(hpsi_plan_t* p) {
   if (!p) return;
-  if (!p->host_only) {
+  if (p->device_ok) {              // whatever upload_schedule / hpsi_davidson / hpsi_truncate got as far as allocating
     cudaFree(p->d_tables);
     cudaFree(p->d_ws);
     cudaFree(p->d_maps);
@@ -154,8 +153,22 @@ extern "C" int hpsi_bind(hpsi_plan_t* p, const double* a_dev, const double* b_de
 
 extern "C" int hpsi_plan(const hpsi_sectors_t* sectors, const hpsi_terms_t* terms, uint32_t flags,
                          hpsi_plan_t** plan_out) {
+  return hpsi_plan_ex(sectors, terms, flags, nullptr, plan_out);
+}
+
+extern "C" int hpsi_plan_ex(const hpsi_sectors_t* sectors, const hpsi_terms_t* terms, uint32_t flags,
+                            const hpsi_plan_options_t* options, hpsi_plan_t** plan_out) {
   if (!plan_out) { set_error("null plan_out"); return HPSI_EINVAL; }
   *plan_out = nullptr;
+  PlanOptions opt;
+  if (options) {
+    if (options->struct_bytes < sizeof(hpsi_plan_options_t)) { set_error("hpsi_plan_options_t.struct_bytes too small"); return HPSI_EINVAL; }
+    opt.shard_of_term = options->shard_of_term;
+    opt.shard_index = options->shard_index;
+    opt.p1_stages_per_unit = options->p1_stages_per_unit;
+    opt.p2_waves = options->p2_waves;
+    opt.p2_min_unit_dmma = options->p2_min_unit_dmma;
+  }
   hpsi_plan_t* p = new (std::nothrow) hpsi_plan_t();
   if (!p) { set_error("out of host memory"); return HPSI_ENOMEM; }
   p->host_only = (flags & HPSI_PLAN_HOST_ONLY) != 0;
@@ -168,13 +181,13 @@ extern "C" int hpsi_plan(const hpsi_sectors_t* sectors, const hpsi_terms_t* term
       if (e == cudaSuccess) e = kernels_init();
       if (e != cudaSuccess) {
         rc = cuda_fail(e, "device initialisation (no CPU fallback exists)");
-        p->host_only = true;   // nothing to free on the device
-        free_plan(p);
+        free_plan(p);          // device_ok is still false: nothing to free on the device
         return rc;
       }
+      p->device_ok = true;
     }
     std::string err;
-    rc = build_schedule(sectors, terms, flags, p->n_sm, &p->sc, &err);
+    rc = build_schedule(sectors, terms, flags, p->n_sm, opt, &p->sc, &err);
     if (rc != HPSI_OK) { set_error(err); free_plan(p); return rc; }
     p->n_left = sectors->n_left;
     p->n_right = sectors->n_right;
@@ -188,26 +201,91 @@ extern "C" int hpsi_plan(const hpsi_sectors_t* sectors, const hpsi_terms_t* term
     }
   } catch (const std::bad_alloc&) {
     set_error("out of host memory while planning");
-    p->host_only = true;
-    free_plan(p);
+    free_plan(p);              // frees whatever device buffers were already allocated
     return HPSI_ENOMEM;
   }
   *plan_out = p;
   return HPSI_OK;
 }
 
-extern "C" int hpsi_set_task_coefficients(hpsi_plan_t* p, const double* coef_host, int64_t n) {
+extern "C" int hpsi_shard_terms(const hpsi_sectors_t* sectors, const hpsi_terms_t* terms, const int32_t* bundle_of_term,
+                                int32_t shard_count, int32_t* shard_of_term, int64_t* shard_flops) {
+  if (!sectors || !terms || !shard_of_term) { set_error("null argument"); return HPSI_EINVAL; }
+  if (shard_count < 1) { set_error("shard_count < 1"); return HPSI_EINVAL; }
+  try {
+    std::vector<int64_t> flops;
+    std::string err;
+    int rc = term_useful_flops(sectors, terms, &flops, &err);
+    if (rc != HPSI_OK) { set_error(err); return rc; }
+    const int T = terms->n_terms;
+    // bundles: first term of the bundle is its representative
+    struct Bundle { int64_t flops; int32_t first; std::vector<int32_t> terms; };
+    std::vector<Bundle> bundles;
+    if (bundle_of_term) {
+      std::vector<std::pair<int32_t, int32_t>> key(T);
+      for (int t = 0; t < T; ++t) key[t] = {bundle_of_term[t], t};
+      std::sort(key.begin(), key.end());
+      for (int i = 0; i < T; ++i) {
+        if (i == 0 || key[i].first != key[i - 1].first) bundles.push_back({0, key[i].second, {}});
+        bundles.back().flops += flops[key[i].second];
+        bundles.back().terms.push_back(key[i].second);
+      }
+    } else {
+      for (int t = 0; t < T; ++t) bundles.push_back({flops[t], t, {t}});
+    }
+    std::stable_sort(bundles.begin(), bundles.end(), [](const Bundle& x, const Bundle& y) {
+      if (x.flops != y.flops) return x.flops > y.flops;
+      return x.first < y.first;
+    });
+    std::vector<int64_t> load(shard_count, 0);
+    for (const Bundle& b : bundles) {
+      int best = 0;
+      for (int s = 1; s < shard_count; ++s) if (load[s] < load[best]) best = s;
+      load[best] += b.flops;
+      for (int32_t t : b.terms) shard_of_term[t] = best;
+    }
+    if (shard_flops) for (int s = 0; s < shard_count; ++s) shard_flops[s] = load[s];
+  } catch (const std::bad_alloc&) {
+    set_error("out of host memory in hpsi_shard_terms");
+    return HPSI_ENOMEM;
+  }
+  return HPSI_OK;
+}
+
+extern "C" int hpsi_layout_blocks(int32_t n_sectors, const int32_t* d, int64_t n_blocks, hpsi_opblock_t* blocks,
+                                  const uint8_t* transposed, int64_t* arena_len) {
+  if (n_sectors < 0 || n_blocks < 0 || (n_sectors > 0 && !d) || (n_blocks > 0 && !blocks) || !arena_len) {
+    set_error("bad argument"); return HPSI_EINVAL;
+  }
+  int64_t off = 0;
+  for (int64_t i = 0; i < n_blocks; ++i) {
+    hpsi_opblock_t& e = blocks[i];
+    if (e.row < 0 || e.row >= n_sectors || e.col < 0 || e.col >= n_sectors) { set_error("block sector index out of range"); return HPSI_EINVAL; }
+    if (e.ld == -1) continue;                             // shares another descriptor's storage
+    const bool tr = transposed && transposed[i];
+    const int64_t srows = tr ? d[e.col] : d[e.row], scols = tr ? d[e.row] : d[e.col];
+    e.ld = sector_up((int)scols);
+    e.offset = off;
+    off = (off + srows * e.ld + 3) & ~(int64_t)3;
+  }
+  *arena_len = off;
+  return HPSI_OK;
+}
+
+extern "C" int hpsi_set_task_coefficients(hpsi_plan_t* p, const double* coef_host, int64_t n, void* cuda_stream) {
   if (!p || !coef_host) { set_error("null argument"); return HPSI_EINVAL; }
   Schedule& sc = p->sc;
   if (n != (int64_t)sc.segs.size()) { set_error("coefficient count != number of tasks (HPSI_Q_N_TASKS)"); return HPSI_EINVAL; }
   for (int64_t i = 0; i < n; ++i) sc.segs[i].coef = coef_host[i];
   for (DiagTask& t : sc.diag) t.coef = coef_host[t.seg];
   if (!p->host_only) {
-    HPSI_CUDA(cudaDeviceSynchronize());
+    // Stream-ordered update of the device tables.  The sources are pageable plan-owned vectors: cudaMemcpyAsync stages
+    // them before it returns, and the copies run on `cuda_stream` after whatever was enqueued there before.
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
     if (!sc.segs.empty())
-      HPSI_CUDA(cudaMemcpy(const_cast<Seg*>(p->dev.segs), sc.segs.data(), sc.segs.size() * sizeof(Seg), cudaMemcpyHostToDevice));
+      HPSI_CUDA(cudaMemcpyAsync(const_cast<Seg*>(p->dev.segs), sc.segs.data(), sc.segs.size() * sizeof(Seg), cudaMemcpyHostToDevice, st));
     if (!sc.diag.empty())
-      HPSI_CUDA(cudaMemcpy(const_cast<DiagTask*>(p->dev.diag), sc.diag.data(), sc.diag.size() * sizeof(DiagTask), cudaMemcpyHostToDevice));
+      HPSI_CUDA(cudaMemcpyAsync(const_cast<DiagTask*>(p->dev.diag), sc.diag.data(), sc.diag.size() * sizeof(DiagTask), cudaMemcpyHostToDevice, st));
   }
   return HPSI_OK;
 }
@@ -241,8 +319,8 @@ extern "C" int hpsi_apply_profiled(hpsi_plan_t* p, const double* psi_dev, double
   if (!p->bound) { set_error("operator arenas not bound (hpsi_bind)"); return HPSI_ESTATE; }
   if (!psi_dev || !out_dev || psi_dev == out_dev) { set_error("bad psi/out"); return HPSI_EINVAL; }
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
-  cudaEvent_t ev[5];
-  for (auto& e : ev) HPSI_CUDA(cudaEventCreate(&e));
+  EventSet<5> ev;
+  HPSI_CUDA(ev.create());
   HPSI_CUDA(cudaEventRecord(ev[0], st));
   launch_prep(p->dev, psi_dev, st);
   HPSI_CUDA(cudaEventRecord(ev[1], st));
@@ -255,7 +333,6 @@ extern "C" int hpsi_apply_profiled(hpsi_plan_t* p, const double* psi_dev, double
   HPSI_CUDA(cudaEventRecord(ev[4], st));
   HPSI_CUDA(cudaEventSynchronize(ev[4]));
   for (int i = 0; i < 4; ++i) HPSI_CUDA(cudaEventElapsedTime(&ms_host[i], ev[i], ev[i + 1]));
-  for (auto& e : ev) cudaEventDestroy(e);
   HPSI_CUDA(cudaGetLastError());
   return HPSI_OK;
 }
@@ -272,6 +349,18 @@ extern "C" int hpsi_apply_host(hpsi_plan_t* p, const double* psi_host, double* o
   if (rc != HPSI_OK) return rc;
   HPSI_CUDA(cudaMemcpyAsync(out_host, p->d_out_stage, bytes, cudaMemcpyDeviceToHost, st));
   HPSI_CUDA(cudaStreamSynchronize(st));
+  return HPSI_OK;
+}
+
+extern "C" int hpsi_sum_shards(const double* parts_dev, int32_t n_parts, int64_t n, double* out_dev, void* cuda_stream) {
+  if (n_parts < 1 || n < 0) { set_error("bad shard count / length"); return HPSI_EINVAL; }
+  if (n == 0) return HPSI_OK;
+  if (!parts_dev || !out_dev) { set_error("null argument"); return HPSI_EINVAL; }
+  if (out_dev > parts_dev - n && out_dev < parts_dev + (int64_t)n_parts * n && out_dev != parts_dev) {
+    set_error("out overlaps parts (only out == parts, i.e. in place over shard 0, is allowed)"); return HPSI_EINVAL;
+  }
+  launch_sum_shards(parts_dev, n_parts, n, out_dev, static_cast<cudaStream_t>(cuda_stream));
+  HPSI_CUDA(cudaGetLastError());
   return HPSI_OK;
 }
 
@@ -328,6 +417,18 @@ extern "C" int hpsi_query(const hpsi_plan_t* p, int what, void* out, size_t byte
     case HPSI_Q_ISO_CAPACITY_RIGHT: { int64_t n = 0; for (const PsiBlk& b : sc.blocks) n += (int64_t)std::min(b.rows, b.cols) * b.cols; return put_i64(n); }
     case HPSI_Q_SVD_SWEEPS: return put_i64(p->svd_sweeps);
     case HPSI_Q_SVD_LAUNCHES: return put_i64(p->svd_launches);
+    case HPSI_Q_N_TERMS_PLANNED: return put_i64(sc.n_terms_planned);
+    case HPSI_Q_TUNING: {
+      if (bytes < sizeof sc.tuning) { set_error("hpsi_query: buffer too small"); return HPSI_EINVAL; }
+      memcpy(out, sc.tuning, sizeof sc.tuning);
+      return HPSI_OK;
+    }
+    case HPSI_Q_PREFERRED_LAYOUT: {
+      if (bytes < sizeof(hpsi_layout_t)) { set_error("hpsi_query: buffer too small"); return HPSI_EINVAL; }
+      const hpsi_layout_t lay = {4, 4, 2, 2, 16, 16};
+      memcpy(out, &lay, sizeof lay);
+      return HPSI_OK;
+    }
     case HPSI_Q_TASKS: {
       if (bytes < sc.tasks.size() * sizeof(hpsi_task_t)) { set_error("hpsi_query: buffer too small"); return HPSI_EINVAL; }
       if (!sc.tasks.empty()) memcpy(out, sc.tasks.data(), sc.tasks.size() * sizeof(hpsi_task_t));

@@ -2,9 +2,8 @@
 // P2 (segmented-K second GEMM with split-K partials), reduce (ordered sum of partials), diag.
 // See kernels.cuh / plan.h for the vocabulary.
 //
-// GEMM CTA = 1 producer warp + NCONS consumer warps (warp-specialised, mbarrier ring of NSTAGE stages).  Default:
-// NCONS = 4 on a <=64x64 tile, 3 CTAs per SM; HPSI_BIG_CTA=1 compiles 8 consumer warps on a <=128x64 tile, 2 CTAs per SM
-// (measured slower on B200: 27.7 vs 31.9 TFLOPS on the cyp config).
+// GEMM CTA = 1 producer warp + NCONS = 4 consumer warps on a <=64x64 tile (warp-specialised, mbarrier ring of NSTAGE
+// stages), 3 CTAs per SM.  (8 consumer warps on a <=128x64 tile at 2 CTAs per SM measured slower: 27.7 vs 31.9 TFLOPS.)
 //   producer : one elected lane issues two TMA tile loads per stage (cp.async.bulk.tensor.2d: a 64-row x 16-column
 //              box of the X operand and one of the Y operand, 128-byte swizzle, rows / columns past the matrix edge
 //              zero-filled by the hardware) that complete on the stage's "full" mbarrier (complete_tx::bytes).
@@ -44,10 +43,8 @@ __device__ __forceinline__ void p1_consume(const DevSchedule& d, const P1Unit& u
     zero_acc<MI, NJ>(acc);
     for (int kt = 0; kt < ntiles; ++kt) {
       mbar_wait(sm.full(ring.stage), ring.phase);
-      if (d.debug != 2) {
-        const double* st = sm.stage_ptr(ring.stage);
-        mma_stage<MI, NJ>(st + w.wr0 * 16, st + X_BOXES * OP_BYTES / 8 + w.wc0 * 16, lo, acc, kt == ntiles - 1 ? last_nk4 : 4);
-      }
+      const double* st = sm.stage_ptr(ring.stage);
+      mma_stage<MI, NJ>(st + w.wr0 * 16, st + X_BOXES * OP_BYTES / 8 + w.wc0 * 16, lo, acc, kt == ntiles - 1 ? last_nk4 : 4);
       __syncwarp();
       if (lane == 0) mbar_arrive(sm.empty(ring.stage));
       ring.advance();
@@ -82,7 +79,7 @@ __device__ __forceinline__ void idle_consume(const SmemLayout& sm, int nstages, 
   }
 
 template <bool TMA, bool ROT>
-__global__ void __maxnreg__(HPSI_BIG_CTA ? 112 : 136) p1_kernel(DevSchedule d) {
+__global__ void __maxnreg__(136) p1_kernel(DevSchedule d) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const P1Unit u = d.p1[blockIdx.x];
   const Group g = d.groups[u.group];
@@ -112,18 +109,14 @@ __global__ void __maxnreg__(HPSI_BIG_CTA ? 112 : 136) p1_kernel(DevSchedule d) {
         const uint32_t sx = sm.stage(ring.stage), sy = sx + X_BOXES * OP_BYTES, full = sm.full(ring.stage);
         if (TMA) {
           if (lane == 0) {
-            mbar_arrive_expect_tx(full, d.debug == 1 ? 0 : (xboxes + 1) * OP_BYTES);
-            if (d.debug != 1) {
-              for (int bx = 0; bx < xboxes; ++bx) tma_load_2d(sx + bx * OP_BYTES, xmap, kt * KT, u.i0 + bx * TILE, full);
-              tma_load_2d(sy, ymap, kt * KT, u.j0, full);
-            }
+            mbar_arrive_expect_tx(full, (xboxes + 1) * OP_BYTES);
+            for (int bx = 0; bx < xboxes; ++bx) tma_load_2d(sx + bx * OP_BYTES, xmap, kt * KT, u.i0 + bx * TILE, full);
+            tma_load_2d(sy, ymap, kt * KT, u.j0, full);
           }
         } else {
-          if (d.debug != 1) {
-            for (int bx = 0; bx < xboxes; ++bx)
-              ldgsts_tile(sx + bx * OP_BYTES, xbase + bx * TILE * xld, xld, u.rows_valid - bx * TILE, kt * KT, g.K1, lane);
-            ldgsts_tile(sy, ybase, g.ldy1, u.cols_valid, kt * KT, g.K1, lane);
-          }
+          for (int bx = 0; bx < xboxes; ++bx)
+            ldgsts_tile(sx + bx * OP_BYTES, xbase + bx * TILE * xld, xld, u.rows_valid - bx * TILE, kt * KT, g.K1, lane);
+          ldgsts_tile(sy, ybase, g.ldy1, u.cols_valid, kt * KT, g.K1, lane);
           cp_async_mbar_arrive(full);
         }
         ring.advance();
@@ -178,10 +171,8 @@ __device__ __forceinline__ void p2_consume(const DevSchedule& d, const P2Unit& u
   Ring ring{0, 0};
   for (KIter it(d.runs, u.run_begin, u.run_end); it.valid; it.advance()) {
     mbar_wait(sm.full(ring.stage), ring.phase);
-    if (d.debug != 2) {
-      const double* st = sm.stage_ptr(ring.stage);
-      mma_stage<MI, NJ>(st + w.wr0 * 16, st + X_BOXES * OP_BYTES / 8 + w.wc0 * 16, lo, acc, it.nk4());
-    }
+    const double* st = sm.stage_ptr(ring.stage);
+    mma_stage<MI, NJ>(st + w.wr0 * 16, st + X_BOXES * OP_BYTES / 8 + w.wc0 * 16, lo, acc, it.nk4());
     __syncwarp();
     if (lane == 0) mbar_arrive(sm.empty(ring.stage));
     ring.advance();
@@ -190,7 +181,7 @@ __device__ __forceinline__ void p2_consume(const DevSchedule& d, const P2Unit& u
 }
 
 template <bool TMA>
-__global__ void __maxnreg__(HPSI_BIG_CTA ? 112 : 136) p2_kernel(DevSchedule d) {
+__global__ void __maxnreg__(136) p2_kernel(DevSchedule d) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const P2Unit u = d.p2[blockIdx.x];
   const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
@@ -233,18 +224,14 @@ __global__ void __maxnreg__(HPSI_BIG_CTA ? 112 : 136) p2_kernel(DevSchedule d) {
       const uint32_t sx = sm.stage(ring.stage), sy = sx + X_BOXES * OP_BYTES, full = sm.full(ring.stage);
       if (TMA) {
         if (lane == 0) {
-          mbar_arrive_expect_tx(full, d.debug == 1 ? 0 : (xboxes + 1) * OP_BYTES);
-          if (d.debug != 1) {
-            for (int bx = 0; bx < xboxes; ++bx) tma_load_2d(sx + bx * OP_BYTES, xmap, it.kappa, xrow + bx * TILE, full);
-            tma_load_2d(sy, ymap, it.kappa, yrow, full);
-          }
+          mbar_arrive_expect_tx(full, (xboxes + 1) * OP_BYTES);
+          for (int bx = 0; bx < xboxes; ++bx) tma_load_2d(sx + bx * OP_BYTES, xmap, it.kappa, xrow + bx * TILE, full);
+          tma_load_2d(sy, ymap, it.kappa, yrow, full);
         }
       } else {
-        if (d.debug != 1) {
-          for (int bx = 0; bx < xboxes; ++bx)
-            ldgsts_tile(sx + bx * OP_BYTES, xbase + bx * TILE * xld, xld, u.rows_valid - bx * TILE, it.kappa, it.K, lane);
-          ldgsts_tile(sy, ybase, yld, u.cols_valid, it.kappa, it.K, lane);
-        }
+        for (int bx = 0; bx < xboxes; ++bx)
+          ldgsts_tile(sx + bx * OP_BYTES, xbase + bx * TILE * xld, xld, u.rows_valid - bx * TILE, it.kappa, it.K, lane);
+        ldgsts_tile(sy, ybase, yld, u.cols_valid, it.kappa, it.K, lane);
         cp_async_mbar_arrive(full);
       }
       if (it.advance()) open_seg();
@@ -355,6 +342,21 @@ __global__ void diag_kernel(DevSchedule d, double* __restrict__ diag) {
     }
     diag[B.off + e] = s;
   }
+}
+
+// out[e] = parts[0][e] + parts[1][e] + ... in that order (term-sharded apply: the ranks' partial H psi, gathered, are added
+// in rank order - bitwise the same on every rank and every run, whatever the transport did)
+__global__ void sum_shards_kernel(const double* __restrict__ parts, int n_parts, int64_t n, double* __restrict__ out) {
+  for (int64_t e = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; e < n; e += (int64_t)gridDim.x * blockDim.x) {
+    double s = parts[e];
+    for (int r = 1; r < n_parts; ++r) s += parts[(int64_t)r * n + e];
+    out[e] = s;
+  }
+}
+void launch_sum_shards(const double* parts, int n_parts, int64_t n, double* out, cudaStream_t st) {
+  if (n <= 0) return;
+  const int grid = (int)std::min<int64_t>((n + 255) / 256, 148 * 8);
+  sum_shards_kernel<<<grid, 256, 0, st>>>(parts, n_parts, n, out);
 }
 
 // -------------------------------------------------------------------------------------------------- launchers

@@ -12,7 +12,7 @@ namespace hpsi {
 
 constexpr int NCONS = NCONS_WARPS;                     // consumer (DMMA) warps per CTA, as a 2x2, 1x4 or 4x1 grid over the tile
 constexpr int NTHREADS = (NCONS + 1) * 32;     // + 1 producer warp
-constexpr int CTAS_PER_SM = HPSI_BIG_CTA ? 2 : 3;
+constexpr int CTAS_PER_SM = 3;
 constexpr int NSTAGE = 4;
 constexpr int OP_BYTES = TILE * KT * 8;        // one TMA box: 64 rows x 128 bytes, 128-byte swizzled
 constexpr int X_BOXES = TILE_M / TILE;         // the X tile of a stage is X_BOXES boxes one under the other
@@ -37,7 +37,6 @@ struct DevSchedule {           // device pointers to the uploaded tables
   int n_blocks, n_p1, n_p2, n_pf;
   int max_block_elems;
   int paired;                  // the plan has blocks stored transposed: kernels_paired.cu runs the GEMMs
-  int debug;                   // HPSI_DEBUG env (timing experiments only): 1 = producer skips loads, 2 = consumers skip MMAs
   double* rot_dst;             // operator-update launches (rotate.cu) only: base the transposed tile stores go to
 };
 
@@ -49,6 +48,7 @@ void launch_pf(const DevSchedule& d, bool tma, cudaStream_t st);            // k
 cudaError_t kernels_fused_init();
 void launch_reduce(const DevSchedule& d, double* out, bool accumulate, cudaStream_t st);
 void launch_diag(const DevSchedule& d, double* diag, cudaStream_t st);
+void launch_sum_shards(const double* parts, int n_parts, int64_t n, double* out, cudaStream_t st);
 void launch_p1_paired(const DevSchedule& d, bool tma, cudaStream_t st);   // kernels_paired.cu
 void launch_p2_paired(const DevSchedule& d, bool tma, cudaStream_t st);
 cudaError_t kernels_paired_init();

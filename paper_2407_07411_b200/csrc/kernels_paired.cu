@@ -145,20 +145,16 @@ __device__ __forceinline__ void stage_operand(const OperandSrc& o, uint32_t s_op
 }
 template <bool TMA>
 __device__ __forceinline__ void stage_both(const OperandSrc& x, const OperandSrc& y, const SmemLayout& sm, const Ring& ring,
-                                           int rows_valid, int cols_valid, int kappa, int K, int lane, int debug) {
+                                           int rows_valid, int cols_valid, int kappa, int K, int lane) {
   const uint32_t sx = sm.stage(ring.stage), sy = sx + X_BOXES * OP_BYTES, full = sm.full(ring.stage);
   if (TMA) {
     if (lane == 0)
-      mbar_arrive_expect_tx(full, debug == 1 ? 0 : operand_bytes(x, rows_valid) + operand_bytes(y, cols_valid));
-    if (debug != 1) {
-      stage_operand<true>(x, sx, rows_valid, kappa, K, full, lane);
-      stage_operand<true>(y, sy, cols_valid, kappa, K, full, lane);
-    }
+      mbar_arrive_expect_tx(full, operand_bytes(x, rows_valid) + operand_bytes(y, cols_valid));
+    stage_operand<true>(x, sx, rows_valid, kappa, K, full, lane);
+    stage_operand<true>(y, sy, cols_valid, kappa, K, full, lane);
   } else {
-    if (debug != 1) {
-      stage_operand<false>(x, sx, rows_valid, kappa, K, full, lane);
-      stage_operand<false>(y, sy, cols_valid, kappa, K, full, lane);
-    }
+    stage_operand<false>(x, sx, rows_valid, kappa, K, full, lane);
+    stage_operand<false>(y, sy, cols_valid, kappa, K, full, lane);
     cp_async_mbar_arrive(full);
   }
 }
@@ -194,11 +190,8 @@ __device__ __forceinline__ void p1p_consume(const DevSchedule& d, const P1Unit& 
     zero_acc<MI, NJ>(acc);
     for (int kt = 0; kt < ntiles; ++kt) {
       mbar_wait(sm.full(ring.stage), ring.phase);
-      if (d.debug != 2) {
-        const double* st = sm.stage_ptr(ring.stage);
-        mma_stage_p<MI, NJ>(st + w.wr0 * 16, st + X_BOXES * OP_BYTES / 8 + w.wc0 * 16, po, acc,
-                            kt == ntiles - 1 ? last_nk4 : 4);
-      }
+      const double* st = sm.stage_ptr(ring.stage);
+      mma_stage_p<MI, NJ>(st + w.wr0 * 16, st + X_BOXES * OP_BYTES / 8 + w.wc0 * 16, po, acc, kt == ntiles - 1 ? last_nk4 : 4);
       __syncwarp();
       if (lane == 0) mbar_arrive(sm.empty(ring.stage));
       ring.advance();
@@ -230,7 +223,7 @@ __global__ void __maxnreg__(136) p1p_kernel(DevSchedule d) {
       if (!TMA) x.ptr = xarena + sg->p1_off + (u.xtrans ? (int64_t)u.i0 : (int64_t)u.i0 * sg->p1_ld);
       for (int kt = 0; kt < ntiles; ++kt) {
         mbar_wait(sm.empty(ring.stage), ring.phase);
-        stage_both<TMA>(x, y, sm, ring, u.rows_valid, u.cols_valid, kt * KT, g.K1, lane, d.debug);
+        stage_both<TMA>(x, y, sm, ring, u.rows_valid, u.cols_valid, kt * KT, g.K1, lane);
         ring.advance();
       }
     }
@@ -263,11 +256,8 @@ __device__ __forceinline__ void p2p_consume(const DevSchedule& d, const P2Unit& 
     for (int sgi = 0; sgi < nseg; ++sgi)
       for (int kt = 0; kt < ntiles; ++kt) {
         mbar_wait(sm.full(ring.stage), ring.phase);
-        if (d.debug != 2) {
-          const double* st = sm.stage_ptr(ring.stage);
-          mma_stage_p<MI, NJ>(st + w.wr0 * 16, st + X_BOXES * OP_BYTES / 8 + w.wc0 * 16, po, acc,
-                              kt == ntiles - 1 ? last_nk4 : 4);
-        }
+        const double* st = sm.stage_ptr(ring.stage);
+        mma_stage_p<MI, NJ>(st + w.wr0 * 16, st + X_BOXES * OP_BYTES / 8 + w.wc0 * 16, po, acc, kt == ntiles - 1 ? last_nk4 : 4);
         __syncwarp();
         if (lane == 0) mbar_arrive(sm.empty(ring.stage));
         ring.advance();
@@ -308,7 +298,7 @@ __global__ void __maxnreg__(136) p2p_kernel(DevSchedule d) {
         }
         for (int kt = 0; kt < ntiles; ++kt) {
           mbar_wait(sm.empty(ring.stage), ring.phase);
-          stage_both<TMA>(x, y, sm, ring, u.rows_valid, u.cols_valid, kt * KT, run.K, lane, d.debug);
+          stage_both<TMA>(x, y, sm, ring, u.rows_valid, u.cols_valid, kt * KT, run.K, lane);
           ring.advance();
         }
       }

@@ -19,13 +19,10 @@
 
 namespace hpsi {
 
-#ifndef HPSI_BIG_CTA
-#define HPSI_BIG_CTA 0        // 1: CTA tile <= 128 x 64 with 8 consumer warps, 2 CTAs / SM; 0: <= 64 x 64 with 4 warps, 3 CTAs / SM
-#endif
 constexpr int TILE = 64;      // CTA tile columns (max) and rows of one TMA box, 8 fragments of 8
-constexpr int TILE_M = HPSI_BIG_CTA ? 128 : 64;   // CTA tile rows (max)
+constexpr int TILE_M = 64;    // CTA tile rows (max)
 constexpr int KT = 16;        // K extent of one staged tile (4 DMMA k-steps)
-constexpr int NCONS_WARPS = HPSI_BIG_CTA ? 8 : 4;   // consumer (DMMA) warps per CTA
+constexpr int NCONS_WARPS = 4;   // consumer (DMMA) warps per CTA (3 CTAs / SM)
 
 enum BaseSel : int32_t { BASE_A = 0, BASE_B = 1, BASE_WS = 2 };
 // How the consumer warps of a CTA cover its tile: P1Unit / P2Unit `grid` = number of warp COLUMNS gn (a power of two
@@ -142,11 +139,24 @@ struct Schedule {
   int32_t max_block_elems = 0;
   bool aligned16 = true;              // descriptors allow the 16-byte staging path (arena base checked at bind)
   bool paired = false;                // some block is stored transposed: fragments are taken from 16-row groups (kernels.cu)
+  int64_t tuning[3] = {0, 0, 0};      // realised schedule knobs: P1 K-tiles per unit, P2 waves, P2 minimum DMMA per unit
+  int32_t n_terms_planned = 0;        // terms of this plan's shard (all terms without a shard)
+};
+
+// What hpsi_plan_ex adds to hpsi_plan (include/hpsi.h hpsi_plan_options_t): a term shard and the schedule knobs.
+struct PlanOptions {
+  const int32_t* shard_of_term = nullptr;   // [n_terms] or null (= every term)
+  int32_t shard_index = 0;
+  int32_t p1_stages_per_unit = 0;           // 0 = automatic
+  int32_t p2_waves = 0;
+  int32_t p2_min_unit_dmma = 0;
 };
 
 // Host planner.  Returns HPSI_OK or an error code with `err` filled.
-int build_schedule(const hpsi_sectors_t* s, const hpsi_terms_t* t, uint32_t flags, int n_sm, Schedule* out,
-                   std::string* err);
+int build_schedule(const hpsi_sectors_t* s, const hpsi_terms_t* t, uint32_t flags, int n_sm, const PlanOptions& opt,
+                   Schedule* out, std::string* err);
+// Useful flops (reading A18) of every term: flops[t] = sum over the term's tasks of min(f1, f2).  Descriptors only.
+int term_useful_flops(const hpsi_sectors_t* s, const hpsi_terms_t* t, std::vector<int64_t>* flops, std::string* err);
 
 // Tile split of one dimension (planner.cpp): rows up to TILE_M, columns up to TILE, sizes in units of two fragments.
 struct Tile1D { int start, len; };
@@ -184,7 +194,7 @@ inline int32_t best_grid(int fm, int fn, int* heaviest = nullptr, bool paired = 
     if (heaviest) *heaviest = 4 * best;
     return g;
   }
-  const int order[4] = {NCONS_WARPS == 8 ? 2 : 2, NCONS_WARPS == 8 ? 4 : 4, 1, NCONS_WARPS};   // squarest first
+  const int order[4] = {2, 4, 1, NCONS_WARPS};   // squarest first
   int best = 1 << 30;
   int32_t g = 2;
   for (int gn : order) {

@@ -10,6 +10,7 @@
 struct hpsi_plan {
   hpsi::Schedule sc;
   bool host_only = false;
+  bool device_ok = false;         // a CUDA device was initialised for this plan: device buffers may exist and must be freed
   bool bound = false;
   bool aligned16 = true;          // descriptors AND arena bases have 16-byte aligned rows: TMA staging is used
   int n_sm = 148;
@@ -41,6 +42,18 @@ int upload_schedule(hpsi_plan_t* p);   // device copies of the schedule tables, 
 int encode_maps(hpsi_plan_t* p);       // CUtensorMap of every MapSpec against dev.a / dev.b / d_ws
 void free_plan(hpsi_plan_t* p);
 }  // namespace hpsi
+
+// CUDA events that are destroyed on every return path
+template <int N>
+struct EventSet {
+  cudaEvent_t ev[N] = {};
+  cudaError_t create() {
+    for (auto& e : ev) { cudaError_t rc = cudaEventCreate(&e); if (rc != cudaSuccess) return rc; }
+    return cudaSuccess;
+  }
+  ~EventSet() { for (auto& e : ev) if (e) cudaEventDestroy(e); }
+  cudaEvent_t& operator[](int i) { return ev[i]; }
+};
 
 #define HPSI_CUDA(call)                                             \
   do {                                                              \

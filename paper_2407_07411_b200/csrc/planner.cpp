@@ -47,8 +47,8 @@ std::vector<Tile1D> split_dim(int64_t n, int max_frags, int unit) {
   return out;
 }
 // rows: up to TILE_M; columns: up to TILE.  Units: half of what the warp grid cuts each dimension into.
-std::vector<Tile1D> split_rows(int64_t n) { return split_dim(n, TILE_M / 8, HPSI_BIG_CTA ? 8 : 2); }
-std::vector<Tile1D> split_cols(int64_t n) { return split_dim(n, TILE / 8, HPSI_BIG_CTA ? 4 : 2); }
+std::vector<Tile1D> split_rows(int64_t n) { return split_dim(n, TILE_M / 8, 2); }
+std::vector<Tile1D> split_cols(int64_t n) { return split_dim(n, TILE / 8, 2); }
 namespace {
 
 int64_t align_up(int64_t x, int64_t a) { return (x + a - 1) / a * a; }
@@ -68,8 +68,55 @@ struct RawTask {
 
 }  // namespace
 
-int build_schedule(const hpsi_sectors_t* s, const hpsi_terms_t* t, uint32_t flags, int n_sm, Schedule* sc,
-                   std::string* err) {
+// psi block table alone (step 1): blk_of_left[i] = psi block of left sector i or -1, partner[i] = its right sector
+static void psi_pairs(const hpsi_sectors_t* s, std::vector<int>* blk_of_left, std::vector<int>* partner) {
+  std::unordered_map<uint64_t, int> right_by_label;
+  for (int j = 0; j < s->n_right; ++j)
+    right_by_label[((uint64_t)(uint32_t)s->q_right[2 * j] << 32) | (uint32_t)s->q_right[2 * j + 1]] = j;
+  blk_of_left->assign(s->n_left, -1);
+  partner->assign(s->n_left, -1);
+  int nb = 0;
+  for (int i = 0; i < s->n_left; ++i) {
+    const int32_t wantN = s->target[0] - s->q_left[2 * i], wantS = s->target[1] - s->q_left[2 * i + 1];
+    auto it = right_by_label.find(((uint64_t)(uint32_t)wantN << 32) | (uint32_t)wantS);
+    if (it == right_by_label.end()) continue;
+    (*blk_of_left)[i] = nb++;
+    (*partner)[i] = it->second;
+  }
+}
+
+int term_useful_flops(const hpsi_sectors_t* s, const hpsi_terms_t* t, std::vector<int64_t>* flops, std::string* err) {
+  if (!s || !t || !flops) FAIL(HPSI_EINVAL, "null argument");
+  const int nL = s->n_left, nR = s->n_right;
+  if (nL < 0 || nR < 0 || t->n_terms < 0 || t->n_a < 0 || t->n_b < 0) FAIL(HPSI_EINVAL, "negative count");
+  if ((nL > 0 && (!s->q_left || !s->d_left)) || (nR > 0 && (!s->q_right || !s->d_right))) FAIL(HPSI_EINVAL, "null sector arrays");
+  if ((t->n_a > 0 && !t->a_blocks) || (t->n_b > 0 && !t->b_blocks)) FAIL(HPSI_EINVAL, "null term arrays");
+  std::vector<int> blk_of_left, partner;
+  psi_pairs(s, &blk_of_left, &partner);
+  flops->assign((size_t)t->n_terms, 0);
+  std::unordered_map<uint64_t, int64_t> b_index;
+  b_index.reserve((size_t)t->n_b * 2);
+  for (int64_t i = 0; i < t->n_b; ++i) {
+    const hpsi_opblock_t& e = t->b_blocks[i];
+    if (e.term < 0 || e.term >= t->n_terms || e.row < 0 || e.row >= nR || e.col < 0 || e.col >= nR)
+      FAIL(HPSI_EINVAL, "B block %lld: term or sector index out of range", (long long)i);
+    b_index[((uint64_t)e.term * (uint64_t)nR + (uint64_t)e.row) * (uint64_t)nR + (uint64_t)e.col] = i;
+  }
+  for (int64_t ia = 0; ia < t->n_a; ++ia) {
+    const hpsi_opblock_t& a = t->a_blocks[ia];
+    if (a.term < 0 || a.term >= t->n_terms || a.row < 0 || a.row >= nL || a.col < 0 || a.col >= nL)
+      FAIL(HPSI_EINVAL, "A block %lld: term or sector index out of range", (long long)ia);
+    if (blk_of_left[a.row] < 0 || blk_of_left[a.col] < 0) continue;
+    const uint64_t key = ((uint64_t)a.term * (uint64_t)nR + (uint64_t)partner[a.row]) * (uint64_t)nR + (uint64_t)partner[a.col];
+    if (b_index.find(key) == b_index.end()) continue;
+    const int64_t m = s->d_left[a.row], k = s->d_left[a.col], n = s->d_right[partner[a.row]], np = s->d_right[partner[a.col]];
+    (*flops)[a.term] += std::min(2 * m * np * (k + n), 2 * k * n * (np + m));
+  }
+  return HPSI_OK;
+}
+
+int build_schedule(const hpsi_sectors_t* s, const hpsi_terms_t* t, uint32_t flags, int n_sm, const PlanOptions& opt,
+                   Schedule* sc, std::string* err) {
   if (!s || !t || !sc) FAIL(HPSI_EINVAL, "null argument");
   const int nL = s->n_left, nR = s->n_right;
   if (nL < 0 || nR < 0) FAIL(HPSI_EINVAL, "negative sector count");
@@ -80,6 +127,12 @@ int build_schedule(const hpsi_sectors_t* s, const hpsi_terms_t* t, uint32_t flag
     FAIL(HPSI_EINVAL, "null term arrays");
   if ((flags & HPSI_PLAN_FIXED_ORDER1) && (flags & HPSI_PLAN_FIXED_ORDER2))
     FAIL(HPSI_EINVAL, "both fixed-order flags set");
+  if (opt.p1_stages_per_unit < 0 || opt.p2_waves < 0 || opt.p2_min_unit_dmma < 0) FAIL(HPSI_EINVAL, "negative schedule knob");
+  // term shard: only the terms with shard_of_term[t] == shard_index are planned; the blocks of every
+  // other term are ignored altogether (their descriptors are not validated: the caller's arenas need not hold them)
+  auto in_shard = [&](int32_t term) { return !opt.shard_of_term || opt.shard_of_term[term] == opt.shard_index; };
+  sc->n_terms_planned = 0;
+  for (int32_t term = 0; term < t->n_terms; ++term) sc->n_terms_planned += in_shard(term) ? 1 : 0;
 
   // ---- validation of the sector table (reading A22: labels unique per side, dims >= 1)
   auto check_side = [&](int n, const int32_t* q, const int32_t* d, const char* side) -> int {
@@ -130,6 +183,7 @@ int build_schedule(const hpsi_sectors_t* s, const hpsi_terms_t* t, uint32_t flag
     for (int64_t i = 0; i < n; ++i) {
       const hpsi_opblock_t& e = blk[i];
       if (e.term < 0 || e.term >= t->n_terms) FAIL(HPSI_EINVAL, "%s block %lld: term %d out of range", side, (long long)i, e.term);
+      if (!in_shard(e.term)) continue;
       if (e.row < 0 || e.row >= nsec || e.col < 0 || e.col >= nsec)
         FAIL(HPSI_EINVAL, "%s block %lld: sector index out of range", side, (long long)i);
       const bool tflag = tr && tr[i];                       // stored as the d[col] x d[row] transpose
@@ -149,8 +203,8 @@ int build_schedule(const hpsi_sectors_t* s, const hpsi_terms_t* t, uint32_t flag
   if (int rc = check_blocks(t->n_b, t->b_blocks, t->b_transposed, s->d_right, nR, t->b_len, "B")) return rc;
 
   sc->paired = false;
-  if (t->a_transposed) for (int64_t i = 0; i < t->n_a; ++i) if (t->a_transposed[i]) sc->paired = true;
-  if (t->b_transposed) for (int64_t i = 0; i < t->n_b; ++i) if (t->b_transposed[i]) sc->paired = true;
+  if (t->a_transposed) for (int64_t i = 0; i < t->n_a; ++i) if (t->a_transposed[i] && in_shard(t->a_blocks[i].term)) sc->paired = true;
+  if (t->b_transposed) for (int64_t i = 0; i < t->n_b; ++i) if (t->b_transposed[i] && in_shard(t->b_blocks[i].term)) sc->paired = true;
   const bool paired = sc->paired;
 
   // ---- step 2: task enumeration
@@ -158,11 +212,13 @@ int build_schedule(const hpsi_sectors_t* s, const hpsi_terms_t* t, uint32_t flag
   b_index.reserve((size_t)t->n_b * 2);
   for (int64_t i = 0; i < t->n_b; ++i) {
     const hpsi_opblock_t& e = t->b_blocks[i];
+    if (!in_shard(e.term)) continue;
     b_index[((uint64_t)e.term * (uint64_t)nR + (uint64_t)e.row) * (uint64_t)nR + (uint64_t)e.col] = i;
   }
   std::vector<RawTask> raw;
   for (int64_t ia = 0; ia < t->n_a; ++ia) {
     const hpsi_opblock_t& a = t->a_blocks[ia];
+    if (!in_shard(a.term)) continue;
     int dst = blk_of_left[a.row], src = blk_of_left[a.col];
     if (dst < 0 || src < 0) continue;
     uint64_t key = ((uint64_t)a.term * (uint64_t)nR + (uint64_t)partner[a.row]) * (uint64_t)nR + (uint64_t)partner[a.col];
@@ -211,8 +267,7 @@ int build_schedule(const hpsi_sectors_t* s, const hpsi_terms_t* t, uint32_t flag
   // The fused kernel is OFF by default: measured on B200 it loses to the two launches even where every task fits it
   // (cyp-shaped config at D = 1024: 1.83 ms per apply fused, 0.63 ms through the workspace - per segment the first GEMM,
   // a CTA barrier, the shared-memory write, a barrier and the second GEMM run back to back, where the two-launch kernels
-  // stream stages without ever draining).  HPSI_PLAN_FUSE_ALL or env HPSI_FUSE=1 select it (tests, experiments).
-  const bool fuse_default = getenv("HPSI_FUSE") && atoi(getenv("HPSI_FUSE")) == 1;
+  // stream stages without ever draining).  HPSI_PLAN_FUSE_ALL selects it.
 
   // ---- steps 3+4a: order choice, groups, segs
   sc->segs.clear(); sc->groups.clear(); sc->tasks.clear(); sc->diag.clear();
@@ -243,8 +298,8 @@ int build_schedule(const hpsi_sectors_t* s, const hpsi_terms_t* t, uint32_t flag
     // and the output dimension that would otherwise recompute it is a single tile (order 1: n <= 64, order 2: m <= 64).
     {
       const int64_t other = (order == 1) ? n : m;
-      const bool fits = g.N1 <= TILE && other <= TILE && !paired && !HPSI_BIG_CTA;
-      g.fused = (fits && !(flags & HPSI_PLAN_NO_FUSION) && (fuse_default || (flags & HPSI_PLAN_FUSE_ALL))) ? 1 : 0;
+      const bool fits = g.N1 <= TILE && other <= TILE && !paired;
+      g.fused = (fits && !(flags & HPSI_PLAN_NO_FUSION) && (flags & HPSI_PLAN_FUSE_ALL)) ? 1 : 0;
     }
     g.ws_off = ws;
     const int64_t per_task = g.fused ? 0 : (int64_t)g.rows * g.ldw;
@@ -300,7 +355,8 @@ int build_schedule(const hpsi_sectors_t* s, const hpsi_terms_t* t, uint32_t flag
     for (const Group& g : sc->groups)
       if (!g.fused) total_stages += (int64_t)split_rows(g.rows).size() * split_cols(g.N1).size() * g.tcount * ((g.K1 + KT - 1) / KT);
     const int auto_stages = (int)std::max<int64_t>(12, std::min<int64_t>(96, total_stages / ((int64_t)std::max(n_sm, 1) * 3 * 8)));
-    const int P1_STAGES_PER_UNIT = getenv("HPSI_P1_STAGES") ? std::max(1, atoi(getenv("HPSI_P1_STAGES"))) : auto_stages;   // env: tuning experiments
+    const int P1_STAGES_PER_UNIT = opt.p1_stages_per_unit > 0 ? opt.p1_stages_per_unit : auto_stages;
+    sc->tuning[0] = P1_STAGES_PER_UNIT;
     struct GOrder { int64_t cost; int gi; };
     std::vector<GOrder> gorder;
     std::vector<int> g_nt(sc->groups.size());
@@ -388,13 +444,15 @@ int build_schedule(const hpsi_sectors_t* s, const hpsi_terms_t* t, uint32_t flag
       for (int pass = 0; pass < 2; ++pass) total_cost[pass] += di.cost[pass] * (int64_t)(di.rt.size() * di.ct.size());
     }
   }
-  const int waves = getenv("HPSI_P2_WAVES") ? std::max(1, atoi(getenv("HPSI_P2_WAVES"))) : 48;   // env: tuning experiments
+  const int waves = opt.p2_waves > 0 ? opt.p2_waves : 48;
   // 4 resident CTAs per SM, ~48 waves: small units keep the tail of the launch short and the operand segments of a
   // (block, K-chunk) bundle L2-resident while its tiles pass over them.  Measured A/B/A/B on B200, 32 -> 48 waves:
   // cyp 31.6 -> 32.0 TFLOPS, stress 32.2 -> 32.5, femoco 31.7 -> 32.0, small unchanged (p2 -2 %, reduce +0.035 ms);
   // 64 waves gain nothing more (the ordered reduce grows as fast as p2 shrinks).
   const int64_t slots = (int64_t)std::max(n_sm, 1) * 4 * waves;
-  const int64_t min_target = getenv("HPSI_P2_MIN") ? std::max(1, atoi(getenv("HPSI_P2_MIN"))) : 1536;   // DMMA per unit at least (~10 us of a CTA)
+  const int64_t min_target = opt.p2_min_unit_dmma > 0 ? opt.p2_min_unit_dmma : 1536;   // DMMA per unit at least (~10 us of a CTA)
+  sc->tuning[1] = waves;
+  sc->tuning[2] = min_target;
   const int64_t target_of[2] = {std::max<int64_t>(min_target, total_cost[0] / slots),
                                 std::max<int64_t>(min_target, total_cost[1] / slots)};
 

@@ -238,7 +238,7 @@ int build_rotate(hpsi_rotate* r, int32_t nsec, const int32_t* d, const int32_t* 
 
 void free_rotate(hpsi_rotate* r) {
   if (!r) return;
-  if (!r->core.host_only) {
+  if (r->core.device_ok) {
     cudaFree(r->d_iso);
     cudaFree(r->core.d_tables);
     cudaFree(r->core.d_ws);
@@ -268,10 +268,10 @@ extern "C" int hpsi_rotate_plan(int32_t n_sectors, const int32_t* d, const int32
       if (e == cudaSuccess) e = kernels_init();
       if (e != cudaSuccess) {
         rc = cuda_fail(e, "device initialisation (no CPU fallback exists)");
-        p.host_only = true;
         free_rotate(r);
         return rc;
       }
+      p.device_ok = true;
     }
     rc = build_rotate(r, n_sectors, d, chi, n_blocks, blocks, a_len, p.n_sm);
     if (rc != HPSI_OK) { free_rotate(r); return rc; }
@@ -297,7 +297,6 @@ extern "C" int hpsi_rotate_plan(int32_t n_sectors, const int32_t* d, const int32
     }
   } catch (const std::bad_alloc&) {
     set_error("out of host memory while planning");
-    p.host_only = true;
     free_rotate(r);
     return HPSI_ENOMEM;
   }
@@ -349,14 +348,13 @@ extern "C" int hpsi_rotate_apply_profiled(hpsi_rotate_t* r, const double* ot_dev
   const int rc = rotate_check(r, ot_dev, out_dev);
   if (rc != HPSI_OK) return rc > 0 ? HPSI_OK : rc;
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
-  cudaEvent_t ev[4];
-  for (auto& e : ev) HPSI_CUDA(cudaEventCreate(&e));
-  int rc2 = rotate_launch(r, ot_dev, out_dev, st, ev);
+  EventSet<4> ev;
+  HPSI_CUDA(ev.create());
+  int rc2 = rotate_launch(r, ot_dev, out_dev, st, ev.ev);
   if (rc2 == HPSI_OK) {
     HPSI_CUDA(cudaEventSynchronize(ev[3]));
     for (int i = 0; i < 3; ++i) HPSI_CUDA(cudaEventElapsedTime(&ms_host[i], ev[i], ev[i + 1]));
   }
-  for (auto& e : ev) cudaEventDestroy(e);
   return rc2;
 }
 

@@ -285,7 +285,6 @@ extern "C" int hpsi_truncate(hpsi_plan_t* p, const double* psi_dev, int32_t side
       svd_round_kernel<<<n_cta, 32 * bsz, smem, st>>>(d_tab, d_cta, sweeps * rounds + r, bsz, d_w, d_flag);
     HPSI_CUDA(cudaMemcpyAsync(&flag, d_flag, sizeof(int), cudaMemcpyDeviceToHost, st));
     HPSI_CUDA(cudaStreamSynchronize(st));
-    if (getenv("HPSI_SVD_DEBUG")) fprintf(stderr, "hpsi_truncate: sweep %d: %d rotations\n", sweeps, flag);
   }
   if (flag) { set_error("hpsi_truncate: Jacobi SVD did not converge"); return HPSI_ESTATE; }
   p->svd_sweeps = sweeps;

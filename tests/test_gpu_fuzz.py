@@ -51,8 +51,10 @@ def test_random_structure(seed):
     import torch
     import paper_2407_07411_b200 as H
     p, rng = rand_problem(seed)
-    if p.psi_len == 0:
-        pytest.skip("no psi block in this draw")
+    redraw = 0
+    while p.psi_len == 0:                        # a draw without any psi block: draw again (never skip a seed)
+        redraw += 1
+        p, rng = rand_problem(seed + 100000 * redraw)
     flags = [0, H.HPSI_PLAN_FIXED_ORDER1, H.HPSI_PLAN_FIXED_ORDER2][int(rng.integers(3))]
     if seed % 2:
         flags |= H.HPSI_PLAN_FUSE_ALL            # narrow groups through the fused kernel (aligned and misaligned staging)
@@ -106,3 +108,16 @@ def test_random_structure(seed):
         o += n
         if O.size:
             np.testing.assert_allclose(O @ O.T, np.eye(O.shape[0]), atol=1e-11)
+    # the rows are singular vectors: O (psi psi^T) = sigma^2 O  (psi^T psi for the right side), block by block
+    o, row0 = 0, 0
+    offs = np.concatenate([[0], np.cumsum(chi_g.astype(np.int64) * dims)])
+    for (i, j, rr, cc, off) in p.psi_blocks():
+        sec = j if side else i
+        blk = psin[off:off + rr * cc].reshape(rr, cc)
+        M = blk.T @ blk if side else blk @ blk.T
+        k = int(chi_g[sec])
+        O = oth[offs[sec]:offs[sec] + k * int(dims[sec])].reshape(k, int(dims[sec]))
+        sig = sig_g[row0:row0 + k]
+        row0 += cc if side else rr
+        if k:
+            np.testing.assert_allclose(O @ M, (sig ** 2)[:, None] * O, atol=1e-11 * max(smax ** 2, 1e-300))

@@ -6,7 +6,7 @@ import pytest
 import oracle
 import workloads
 from workloads.hubbard import hubbard_two_block_problem
-from gpu_util import GpuProblem, rel_l2
+from gpu_util import GpuProblem, assert_blockwise, fill_device_arenas, rel_l2, shard_sum
 from test_oracle_pins import random_custom
 
 pytestmark = pytest.mark.gpu
@@ -266,28 +266,168 @@ def test_warp_grid_shapes(H):
         assert rel_l2(GpuProblem(p, flags).apply(psi), ref) <= TOL
 
 
+def _samples(p, n, seed=7):
+    rng = np.random.default_rng(seed)
+    blocks = p.psi_blocks()
+    bi = rng.integers(0, len(blocks), n)
+    sl = np.array([blocks[b][0] for b in bi], np.int32)
+    sx = np.array([rng.integers(0, blocks[b][2]) for b in bi], np.int32)
+    sy = np.array([rng.integers(0, blocks[b][3]) for b in bi], np.int32)
+    idx = np.array([blocks[b][4] + x * blocks[b][3] + y for b, x, y in zip(bi, sx, sy)], np.int64)
+    return sl, sx, sy, idx
+
+
 @pytest.mark.parametrize("cfg", ["cyp", "stress"])
-def test_full_size_sampled_parity(H, cfg):
-    """BASELINE.json configs[2] / configs[4] at full size, in the launch configuration bench.py times: 64 sampled
-    outputs that the oracle computes one by one, plus Hermiticity <x,Hy> = <Hx,y> on the full vectors."""
+def test_full_size_full_vector_parity(H, cfg):
+    """BASELINE.json configs[2] / configs[4] at full size, in the launch configuration bench.py times: the WHOLE output
+    vector against one full oracle apply (620 188 / 1 583 102 elements), block by block; Hermiticity of the GPU result
+    against the oracle's; bitwise reproducibility; and the same operators cut into 8 term shards (hpsi_shard_terms +
+    hpsi_plan_ex), every shard through the CUDA kernels, summed in rank order by hpsi_sum_shards."""
+    import torch
     p = workloads.make_problem(cfg)
     g = GpuProblem(p)
     assert g.q(H.HPSI_Q_ALIGNED16) == 1
     psi = workloads.make_psi(p)
     out = g.apply(psi)
-    rng = np.random.default_rng(7)
-    blocks = p.psi_blocks()
-    bi = rng.integers(0, len(blocks), 64)
-    sl = np.array([blocks[b][0] for b in bi], np.int32)
-    sx = np.array([rng.integers(0, blocks[b][2]) for b in bi], np.int32)
-    sy = np.array([rng.integers(0, blocks[b][3]) for b in bi], np.int32)
-    idx = np.array([blocks[b][4] + x * blocks[b][3] + y for b, x, y in zip(bi, sx, sy)], np.int64)
-    ref = oracle.apply_samples(p, psi, sl, sx, sy)
-    assert np.linalg.norm(out[idx] - ref) <= TOL * np.linalg.norm(ref)
+    ref = oracle.apply(p, psi)
+    assert_blockwise(p, out, ref, TOL)
     y = workloads.make_psi(p, 1)
     Hy = g.apply(y)
-    assert abs(psi @ Hy - out @ y) <= 1e-12 * np.linalg.norm(psi) * np.linalg.norm(Hy)
+    assert abs(psi @ Hy - ref @ y) <= 1e-12 * np.linalg.norm(psi) * np.linalg.norm(Hy)     # <x, H_gpu y> = <H_oracle x, y>
     assert np.array_equal(out, g.apply(psi))                       # bitwise reproducible at full size
+    # term shards through the kernels (the multi-GPU path's compute, one shard after the other on this GPU)
+    world, half = 8, p.n_terms // 2
+    shard, fl = H.hpsi_shard_terms(p, world, np.arange(p.n_terms) % half)
+    assert int(fl.sum()) == g.q(H.HPSI_Q_USEFUL_FLOPS) and fl.max() <= 1.02 * fl.mean()
+    x = torch.from_numpy(psi).cuda()
+    parts, ntask = [], 0
+    for r in range(world):
+        gs = GpuProblem(p, arenas=(g.a, g.b), shard_of_term=shard, shard_index=r)
+        assert gs.q(H.HPSI_Q_USEFUL_FLOPS) == fl[r]
+        ntask += gs.q(H.HPSI_Q_N_TASKS)
+        parts.append(gs.apply_dev(x))
+        del gs
+    assert ntask == g.q(H.HPSI_Q_N_TASKS)
+    assert_blockwise(p, shard_sum(H, torch, parts), ref, TOL)
+
+
+def test_femoco_shaped_full_vector_parity(H):
+    """BASELINE.json configs[3] (D = 8192, sector dims up to 653: ~11 tiles per block edge, K-stacks across several
+    groups) with 120 of its 2900 terms, so that the operators are 3.3 GB instead of 80: the whole output vector against
+    the oracle, block by block, for the planner's order choice and both forced orders."""
+    p = workloads.make_problem("femoco", n_terms=120)
+    assert p.d_left.sum() == 8192 and p.d_left.max() > 600
+    psi = workloads.make_psi(p)
+    ref = oracle.apply(p, psi)
+    g = GpuProblem(p)
+    assert g.q(H.HPSI_Q_ALIGNED16) == 1
+    out = g.apply(psi)
+    assert_blockwise(p, out, ref, TOL)
+    assert np.array_equal(out, g.apply(psi))
+    for flags in (H.HPSI_PLAN_FIXED_ORDER1, H.HPSI_PLAN_FIXED_ORDER2):
+        assert_blockwise(p, GpuProblem(p, flags, arenas=(g.a, g.b)).apply(psi), ref, TOL)
+    sh = workloads.make_problem("femoco", n_terms=120, share_adjoint=True)      # the 40 GB storage mode of the full config
+    assert_blockwise(p, GpuProblem(sh).apply(psi), ref, TOL)
+
+
+def test_femoco_full_config_sampled_parity(H):
+    """BASELINE.json configs[3] in full (2900 terms, 80 GB of operators resident, the launch configuration bench.py
+    --config femoco times): device arenas filled chunk by chunk, the same chunks streamed through the oracle, which
+    computes 48 sampled outputs one by one (a full oracle apply would take minutes: 5.7 TFLOP)."""
+    import torch
+    free, total = torch.cuda.mem_get_info()
+    full = workloads.make_problem("femoco", fill=False)
+    need = 8 * (full.a_len + full.b_len)
+    assert total > need + 45e9, "the FeMoco-shaped config is sized for a 180 GB B200 (BASELINE.json configs[3])"
+    psi = workloads.make_psi(full)
+    sl, sx, sy, idx = _samples(full, 48)
+    vals = np.zeros(len(sl))
+    a, b = fill_device_arenas(torch, full, on_chunk=lambda sub: oracle.apply_samples(sub, psi, sl, sx, sy, vals=vals))
+    g = GpuProblem(full, arenas=(a, b))
+    assert g.q(H.HPSI_Q_N_TASKS) > 100000 and g.q(H.HPSI_Q_ALIGNED16) == 1
+    out = g.apply(psi)
+    assert np.linalg.norm(out[idx] - vals) <= TOL * np.linalg.norm(vals)
+    assert np.max(np.abs(out[idx] - vals)) <= 10 * TOL * np.max(np.abs(vals))
+    assert np.isfinite(out).all() and np.array_equal(out, g.apply(psi))
+
+
+@pytest.mark.parametrize("world", [2, 8])
+@pytest.mark.parametrize("share", [False, True])
+def test_term_shards_through_the_kernels(H, small, world, share):
+    """The multi-GPU apply on one GPU, rank after rank: hpsi_shard_terms partitions the terms, every rank's arenas hold
+    its own terms only (workloads.make_shard), hpsi_plan_ex plans the shard, hpsi_apply runs it through the DMMA
+    kernels, hpsi_sum_shards adds the partial results in rank order - against the oracle on the unsharded problem,
+    element by element."""
+    import torch
+    psi = workloads.make_psi(small)
+    ref = oracle.apply(small, psi)
+    desc = workloads.make_problem("small", fill=False, share_adjoint=share)
+    half = desc.n_terms // 2
+    shard, fl = H.hpsi_shard_terms(desc, world, np.arange(desc.n_terms) % half)
+    x = torch.from_numpy(psi).cuda()
+    parts, flops, tasks = [], 0, 0
+    for r in range(world):
+        p = workloads.make_shard("small", shard, r, share_adjoint=share)
+        g = GpuProblem(p, shard_of_term=shard, shard_index=r)
+        assert g.q(H.HPSI_Q_N_TERMS_PLANNED) == int((shard == r).sum())
+        flops += g.q(H.HPSI_Q_USEFUL_FLOPS); tasks += g.q(H.HPSI_Q_N_TASKS)
+        parts.append(g.apply_dev(x))
+    assert (flops, tasks) == oracle.useful_flops(small)
+    got = shard_sum(H, torch, parts)
+    assert_blockwise(small, got, ref, TOL)
+    assert np.array_equal(got, shard_sum(H, torch, parts))
+    # in place over shard 0 is allowed, any other overlap is refused
+    buf = torch.cat(parts)
+    H.hpsi_sum_shards(buf, world, buf[:small.psi_len], torch.cuda.current_stream())
+    torch.cuda.synchronize()
+    assert np.array_equal(buf[:small.psi_len].cpu().numpy(), got)
+    with pytest.raises(H.HpsiError):
+        H.hpsi_sum_shards(buf, world, buf[1:small.psi_len + 1], torch.cuda.current_stream())
+
+
+def test_term_sharded_site_update_on_gpu(H):
+    """Operator update under term sharding (no exchange step): every rank rotates the blocks of its own terms with the
+    replicated isometries through the DMMA kernels; every block against the oracle on the full operator set."""
+    import torch
+    from oracle import site_update as su
+    half, world = 40, 2
+    full = workloads.make_problem("small", n_terms=2 * half)
+    chi = workloads.proportional_chi(full.d_left, 0.25, zero_every=6)
+    ot = workloads.make_isometries(full.d_left, chi, seed=5)
+    otd = torch.from_numpy(np.concatenate([workloads.pack_isometries(ot), np.zeros(1)])).cuda()
+    ref = su.rotate(full.d_left, chi, full.a_desc, full.a_data, ot)
+    where = {(int(e["term"]), int(e["row"]), int(e["col"])): i for i, e in enumerate(full.a_desc)}
+    seen = flops = 0
+    for rank in range(world):
+        p = workloads.make_problem("small", n_terms=2 * half, base_terms=np.arange(rank, half, world))
+        gid = np.concatenate([p.base_term_ids, p.base_term_ids + half])
+        a = torch.from_numpy(p.a_data).cuda()
+        r = H.hpsi_rotate_plan(p.d_left, chi, p.a_desc, a, p.a_len)
+        out = torch.full((H.hpsi_rotate_query(r, H.HPSI_RQ_OUT_LENGTH),), float("nan"), dtype=torch.float64, device="cuda")
+        H.hpsi_rotate_apply(r, otd, out, torch.cuda.current_stream())
+        torch.cuda.synchronize()
+        outh = out.cpu().numpy()
+        flops += H.hpsi_rotate_query(r, H.HPSI_RQ_USEFUL_FLOPS)
+        for e in H.hpsi_rotate_query(r, H.HPSI_RQ_OUT_BLOCKS):
+            x = ref[where[(int(gid[e["term"]]), int(e["row"]), int(e["col"]))]]
+            seen += 1
+            if e["offset"] < 0:
+                assert x.size == 0
+                continue
+            blk = np.lib.stride_tricks.as_strided(outh[int(e["offset"]):], shape=x.shape, strides=(int(e["ld"]) * 8, 8))
+            assert np.max(np.abs(blk - x)) <= 1e-12 * max(np.max(np.abs(x)), 1e-300)
+    assert seen == len(full.a_desc) and flops == su.rotate_flops(full.d_left, chi, full.a_desc)
+
+
+def test_plan_options_on_gpu(H, small):
+    """hpsi_plan_options_t schedule knobs re-cut the work; the result stays within the bar and HPSI_Q_TUNING reports them."""
+    psi = workloads.make_psi(small)
+    ref = oracle.apply(small, psi)
+    base = GpuProblem(small)
+    for kw in (dict(p1_stages_per_unit=5), dict(p2_waves=2), dict(p2_min_unit_dmma=100000, p1_stages_per_unit=400)):
+        g = GpuProblem(small, arenas=(base.a, base.b), **kw)
+        assert g.q(H.HPSI_Q_TUNING) != base.q(H.HPSI_Q_TUNING)
+        assert_blockwise(small, g.apply(psi), ref, TOL)
 
 
 def test_task_coefficients(H, toy):
@@ -299,9 +439,20 @@ def test_task_coefficients(H, toy):
     for prob in (toy, p):
         g = GpuProblem(prob)
         f = np.random.default_rng(9).standard_normal(g.q(H.HPSI_Q_N_TASKS))
-        H.hpsi_set_task_coefficients(g.plan, f)
-        ex = exploded_problem(prob, g.plan, f)
         psi = workloads.make_psi(prob)
+        # stream-ordered: an apply enqueued before the call sees the old coefficients, one enqueued after it the new ones
+        s = torch.cuda.Stream()
+        x = torch.from_numpy(psi).cuda()
+        y0, y1 = torch.full_like(x, float("nan")), torch.full_like(x, float("nan"))
+        torch.cuda.synchronize()
+        with torch.cuda.stream(s):
+            H.hpsi_apply(g.plan, x, y0, s)
+            H.hpsi_set_task_coefficients(g.plan, f, s)
+            H.hpsi_apply(g.plan, x, y1, s)
+        s.synchronize()
+        ex = exploded_problem(prob, g.plan, f)
+        assert rel_l2(y0.cpu().numpy(), oracle.apply(prob, psi)) <= TOL
+        assert rel_l2(y1.cpu().numpy(), oracle.apply(ex, psi)) <= TOL
         assert rel_l2(g.apply(psi), oracle.apply(ex, psi)) <= TOL
         d = torch.empty(g.n, dtype=torch.float64, device="cuda")
         H.hpsi_diagonal(g.plan, d)

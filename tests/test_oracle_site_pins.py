@@ -251,3 +251,19 @@ def test_rotate_flops_doubling_law(toy):
     f1 = su.rotate_flops(d, chi, toy.a_desc)
     f2 = su.rotate_flops(2 * d, 2 * chi, toy.a_desc)
     assert f2 == 8 * f1                                      # the O(D^3) law of PAPER.md:62
+
+
+def test_rotate_flops_hand_count():
+    """tests/golden/site_update_closed_forms.txt item 6: the counter against flops counted by hand, block by block - a
+    wrong coefficient, a dropped GEMM or swapped row / column dims changes one of the five numbers."""
+    line = [l for l in open(os.path.join(os.path.dirname(__file__), "golden", "site_update_closed_forms.txt")) if l.startswith("rotate_flops")][0]
+    first, second = line.split(";")
+    tok = first.split(":")[1].split()
+    want = {tok[i]: int(tok[i + 1]) for i in range(0, len(tok), 2)}
+    d = np.array([3, 2])
+    desc = np.zeros(4, workloads.OPBLOCK_DTYPE)
+    for i, (r, c) in enumerate([(0, 1), (1, 0), (0, 0), (1, 1)]):
+        desc[i] = (i, r, c, d[c], 0)
+        assert su.rotate_flops(d, np.array([2, 1]), desc[i:i + 1]) == want[f"{r}<-{c}"]
+    assert su.rotate_flops(d, np.array([2, 1]), desc) == want["all"] == 24 + 32 + 60 + 12
+    assert su.rotate_flops(d, np.array([2, 0]), desc) == int(second.split()[-1]) == 60

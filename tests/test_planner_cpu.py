@@ -25,15 +25,143 @@ def rel(x, ref):
 
 
 # ------------------------------------------------------------------------------------------------ ABI
-def test_library_exports_every_declared_symbol():
-    hdr = open(os.path.join(ROOT, "include", "hpsi.h")).read()
+def _declared(header):
+    hdr = open(os.path.join(ROOT, "include", header)).read()
     hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
-    names = set(re.findall(r"\b(hpsi_[a-z0-9_]+)\s*\(", hdr))
-    assert {"hpsi_plan", "hpsi_apply", "hpsi_apply_host", "hpsi_bind", "hpsi_davidson", "hpsi_query", "hpsi_destroy",
-            "hpsi_last_error", "hpsi_diagonal", "hpsi_debug_interpret", "hpsi_bench_fp64_pipe", "hpsi_apply_profiled"} <= names
+    return set(re.findall(r"\b(hpsi_[a-z0-9_]+)\s*\(", hdr))
+
+
+def test_library_exports_every_declared_symbol():
+    """Every include/*.h has its library, and each library exports exactly what its header declares."""
+    assert sorted(os.listdir(os.path.join(ROOT, "include"))) == ["hpsi.h", "hpsi_bench.h"]
+    names = _declared("hpsi.h")
+    assert {"hpsi_plan", "hpsi_plan_ex", "hpsi_shard_terms", "hpsi_layout_blocks", "hpsi_apply", "hpsi_apply_host",
+            "hpsi_bind", "hpsi_davidson", "hpsi_query", "hpsi_destroy", "hpsi_last_error", "hpsi_diagonal",
+            "hpsi_debug_interpret", "hpsi_apply_profiled"} <= names
     L = H.lib()
     for n in names:
         assert hasattr(L, n), n
+    bench_names = _declared("hpsi_bench.h")
+    assert bench_names == {"hpsi_bench_fp64_pipe", "hpsi_bench_last_error"}
+    LB = H.binding.bench_lib()
+    for n in bench_names:
+        assert hasattr(LB, n), n
+        assert not hasattr(L, n), f"{n}: calibration probes do not belong in the product library"
+
+
+def test_schedule_ignores_the_environment(small, monkeypatch):
+    """A plan depends on its arguments only: no environment variable changes the schedule (the old tuning hooks)."""
+    base = host_plan(small)
+    want = [H.hpsi_query(base, w) for w in (H.HPSI_Q_N_P1_UNITS, H.HPSI_Q_N_P2_UNITS, H.HPSI_Q_N_FUSED_UNITS)]
+    for k, v in (("HPSI_FUSE", "1"), ("HPSI_P1_STAGES", "7"), ("HPSI_P2_WAVES", "3"), ("HPSI_P2_MIN", "99999"), ("HPSI_DEBUG", "2")):
+        monkeypatch.setenv(k, v)
+    again = host_plan(small)
+    assert [H.hpsi_query(again, w) for w in (H.HPSI_Q_N_P1_UNITS, H.HPSI_Q_N_P2_UNITS, H.HPSI_Q_N_FUSED_UNITS)] == want
+    assert H.hpsi_query(again, H.HPSI_Q_TUNING) == H.hpsi_query(base, H.HPSI_Q_TUNING)
+
+
+def test_plan_options_change_the_schedule_not_the_result(small):
+    """hpsi_plan_options_t knobs are visible through HPSI_Q_TUNING and only re-cut the work."""
+    psi = workloads.make_psi(small)
+    ref = oracle.apply(small, psi)
+    base = host_plan(small)
+    t0 = H.hpsi_query(base, H.HPSI_Q_TUNING)
+    assert t0[1] == 48 and t0[2] == 1536 and 12 <= t0[0] <= 96
+    for kw in (dict(p1_stages_per_unit=7), dict(p2_waves=3), dict(p2_min_unit_dmma=200000), dict(p1_stages_per_unit=500, p2_waves=100)):
+        plan = H.plan_problem(small, flags=H.HPSI_PLAN_HOST_ONLY, **kw)
+        t = H.hpsi_query(plan, H.HPSI_Q_TUNING)
+        assert t != t0
+        for k, v in kw.items():
+            assert t[("p1_stages_per_unit", "p2_waves", "p2_min_unit_dmma").index(k)] == v
+        assert rel(H.hpsi_debug_interpret(plan, small.a_data, small.b_data, psi), ref) <= 1e-13
+    with pytest.raises(H.HpsiError):
+        H.plan_problem(small, flags=H.HPSI_PLAN_HOST_ONLY, p2_waves=-1)
+
+
+def test_preferred_layout_query_and_layout_blocks(small):
+    """SURVEY.md 8(b) "preferred ld / arena layout": the rule as a query, and hpsi_layout_blocks applying it - a caller
+    can describe its blocks, let the library lay them out, fill the arenas and plan (arenas bound later)."""
+    lay = H.hpsi_query(host_plan(small), H.HPSI_Q_PREFERRED_LAYOUT)
+    assert lay == {"ld_multiple": 4, "offset_multiple": 4, "tma_ld_multiple": 2, "tma_offset_multiple": 2,
+                   "arena_align_bytes": 16, "transposed_pad_rows": 16}
+    dense = workloads.make_problem("small", n_terms=20, pad_even=False)           # odd lds, dense offsets
+    a_desc, a_len = H.hpsi_layout_blocks(dense.d_left, dense.a_desc)
+    b_desc, b_len = H.hpsi_layout_blocks(dense.d_right, dense.b_desc)
+    for desc, dims, n in ((a_desc, dense.d_left, a_len), (b_desc, dense.d_right, b_len)):
+        assert np.all(desc["ld"] % lay["ld_multiple"] == 0) and np.all(desc["offset"] % lay["offset_multiple"] == 0)
+        assert np.all(desc["ld"] >= dims[desc["col"]]) and np.all(desc["ld"] < dims[desc["col"]] + 4)
+        ends = desc["offset"] + dims[desc["row"]].astype(np.int64) * desc["ld"]
+        assert np.all(desc["offset"][1:] >= ends[:-1]) and n >= ends[-1]          # no overlap, in the order given
+    # the library's layout is the generator's preferred one (row_align = 4)
+    pref = workloads.make_problem("small", n_terms=20)
+    assert np.array_equal(a_desc, pref.a_desc) and np.array_equal(b_desc, pref.b_desc) and (a_len, b_len) == (pref.a_len, pref.b_len)
+    # move the entries into that layout and plan: same operator
+    import copy
+    moved = copy.copy(dense)
+    moved.a_desc, moved.b_desc, moved.a_len, moved.b_len = a_desc, b_desc, a_len, b_len
+    moved.a_data, moved.b_data = np.full(a_len, np.nan), np.full(b_len, np.nan)
+    for side, old, new, data, dims in (("a", dense.a_desc, a_desc, moved.a_data, dense.d_left), ("b", dense.b_desc, b_desc, moved.b_data, dense.d_right)):
+        for i, e in enumerate(new):
+            r, c = int(dims[e["row"]]), int(dims[e["col"]])
+            np.lib.stride_tricks.as_strided(data[int(e["offset"]):], shape=(r, c), strides=(int(e["ld"]) * 8, 8))[...] = dense.block(side, i)
+    plan = host_plan(moved)
+    assert H.hpsi_query(plan, H.HPSI_Q_ALIGNED16) == 1 and H.hpsi_query(host_plan(dense), H.HPSI_Q_ALIGNED16) == 0
+    psi = workloads.make_psi(dense)
+    assert rel(H.hpsi_debug_interpret(plan, moved.a_data, moved.b_data, psi), oracle.apply(dense, psi)) <= 1e-13
+    # transposed blocks store d[col] x d[row]; ld == -1 marks a descriptor that shares storage and is left alone
+    sh = workloads.make_problem("toy", share_adjoint=True)
+    probe = sh.a_desc.copy()
+    probe["ld"][sh.a_trans == 1] = -1
+    laid, n = H.hpsi_layout_blocks(sh.d_left, probe, sh.a_trans)
+    own = sh.a_trans == 0
+    assert np.array_equal(laid[own], sh.a_desc[own]) and np.all(laid["ld"][~own] == -1) and n == sh.a_len
+
+
+def test_shard_terms_partition(small):
+    """hpsi_shard_terms: deterministic, balanced by useful flops, bundles stay together, every term placed; the shards
+    planned with hpsi_plan_ex partition the tasks and the flops."""
+    T, half = small.n_terms, small.n_terms // 2
+    flops, ntask = oracle.useful_flops(small)
+    for world in (1, 2, 5, 8):
+        shard, fl = H.hpsi_shard_terms(small, world, np.arange(T) % half)
+        assert shard.min() >= 0 and shard.max() < world and np.array_equal(shard[:half], shard[half:])
+        assert int(fl.sum()) == flops and fl.max() <= 1.02 * fl.mean()
+        again, _ = H.hpsi_shard_terms(small, world, np.arange(T) % half)
+        assert np.array_equal(shard, again)
+        tot_tasks = tot_flops = tot_terms = 0
+        for r in range(world):
+            plan = H.plan_problem(small, flags=H.HPSI_PLAN_HOST_ONLY, shard_of_term=shard, shard_index=r)
+            assert H.hpsi_query(plan, H.HPSI_Q_USEFUL_FLOPS) == fl[r]
+            tasks = H.hpsi_query(plan, H.HPSI_Q_TASKS)
+            assert np.all(shard[tasks["term"]] == r)
+            tot_tasks += len(tasks); tot_flops += int(fl[r]); tot_terms += H.hpsi_query(plan, H.HPSI_Q_N_TERMS_PLANNED)
+        assert (tot_tasks, tot_flops, tot_terms) == (ntask, flops, T)
+    alone, fl = H.hpsi_shard_terms(small, 4)                        # no bundles: every term on its own
+    assert int(fl.sum()) == flops and fl.max() <= 1.02 * fl.mean()
+    with pytest.raises(H.HpsiError):
+        H.hpsi_shard_terms(small, 0)
+
+
+def test_shard_plan_never_reads_other_terms(small):
+    """A shard's arenas hold only its own terms (workloads.make_shard gives the other descriptors offset -1): the plan
+    must accept that, and the shards' results must add up to the oracle's H psi element by element."""
+    T, half = small.n_terms, small.n_terms // 2
+    psi = workloads.make_psi(small)
+    ref = oracle.apply(small, psi)
+    for share in (False, True):
+        desc = workloads.make_problem("small", fill=False, share_adjoint=share)
+        shard, fl = H.hpsi_shard_terms(desc, 3, np.arange(T) % half)
+        tot, a_doubles = np.zeros_like(ref), 0
+        for r in range(3):
+            p = workloads.make_shard("small", shard, r, share_adjoint=share)
+            assert np.all(p.a_desc["offset"][shard[p.a_desc["term"]] != r] == -1)
+            a_doubles += p.a_len
+            plan = H.plan_problem(p, flags=H.HPSI_PLAN_HOST_ONLY, shard_of_term=shard, shard_index=r)
+            tot += H.hpsi_debug_interpret(plan, p.a_data, p.b_data, psi)
+            with pytest.raises(H.HpsiError):                      # without the shard map the -1 offsets are rejected
+                H.plan_problem(p, flags=H.HPSI_PLAN_HOST_ONLY)
+        assert a_doubles == desc.a_len                            # the shards partition the operator storage
+        assert rel(tot, ref) <= 1e-13
 
 
 def test_opblock_layout_matches_header():
@@ -199,6 +327,7 @@ def test_empty_problems():
 def test_struct_sizes():
     assert ctypes.sizeof(H.binding.hpsi_sectors_t) == 48
     assert ctypes.sizeof(H.binding.hpsi_terms_t) == 96      # + a_transposed, b_transposed
+    assert ctypes.sizeof(H.binding.hpsi_plan_options_t) == 32 and ctypes.sizeof(H.binding.hpsi_layout_t) == 24
     assert H.binding.PSI_BLOCK_DTYPE.itemsize == 24 and H.binding.TASK_DTYPE.itemsize == 24
 
 

@@ -361,6 +361,83 @@ def make_problem(name: str, seed: Optional[int] = None, fill: bool = True, pad_e
     return p
 
 
+def make_shard(name: str, shard_of_term, shard_index: int, seed: Optional[int] = None, fill: bool = True,
+               share_adjoint: bool = False, D: Optional[int] = None) -> Problem:
+    """One rank's part of config ``name`` under a term partition (``shard_of_term[t] == shard_index`` keeps term t), in
+    the term numbering of the FULL config: the sector table, the coefficients and the descriptor tables are the full
+    config's, but the arenas hold the kept terms only (their blocks moved up, same alignment) and the descriptors of
+    every other term get offset -1 - they must not be read, which is what hpsi_plan_ex with the same ``shard_of_term``
+    promises.  A base term and its adjoint must be kept together (their entries are drawn together)."""
+    p = make_problem(name, seed=seed, fill=False, share_adjoint=share_adjoint, D=D)
+    half = p.n_terms // 2
+    keep = np.asarray(shard_of_term) == shard_index
+    assert keep.shape == (p.n_terms,) and np.array_equal(keep[:half], keep[half:]), "adjoint pairs must stay together"
+    for side in ("a", "b"):
+        desc = (p.a_desc if side == "a" else p.b_desc).copy()
+        rng_tab = p.term_a_range if side == "a" else p.term_b_range
+        total = p.a_len if side == "a" else p.b_len
+        n_own = half if share_adjoint else p.n_terms             # terms that own storage (term-major arena)
+        starts = [int(desc["offset"][rng_tab[t, 0]]) if rng_tab[t, 0] < rng_tab[t, 1] else None for t in range(n_own)]
+        ends, nxt = [0] * n_own, total                            # a term's range ends where the next non-empty one starts
+        for t in range(n_own - 1, -1, -1):
+            ends[t] = nxt
+            if starts[t] is not None:
+                nxt = starts[t]
+        shift, run = np.zeros(p.n_terms, np.int64), 0
+        for t in range(n_own):
+            if keep[t] and starts[t] is not None:
+                shift[t] = starts[t] - run
+                run += ends[t] - starts[t]
+        if share_adjoint:
+            shift[half:] = shift[:half]
+        for t in range(p.n_terms):
+            lo, hi = rng_tab[t]
+            if keep[t]:
+                desc["offset"][lo:hi] -= shift[t]
+            else:
+                desc["offset"][lo:hi] = -1
+        if side == "a":
+            p.a_desc, p.a_len = desc, int(run)
+        else:
+            p.b_desc, p.b_len = desc, int(run)
+    if fill:
+        p.a_data = np.zeros(max(p.a_len, 1), np.float64)
+        p.b_data = np.zeros(max(p.b_len, 1), np.float64)
+        for t in range(half):
+            if keep[t]:
+                fill_term(p, t, p.a_data, p.b_data)
+    return p
+
+
+def term_chunk(full: Problem, lo: int, hi: int, D: Optional[int] = None):
+    """Base terms [lo, hi) of config ``full.name`` and their adjoints as a filled sub-problem, plus where its arenas sit in
+    the arenas of the full config: ``full`` = make_problem(name, fill=False) (descriptors only), the result is
+    (sub, [(side, src_lo, src_hi, dst_lo), ...]) with sub = make_problem(name, base_terms=arange(lo, hi)).  Lets a caller
+    fill device arenas of the D = 8192 config (80 GB) without ever holding them on the host, and lets the oracle stream
+    the same terms (oracle.apply_samples accumulates over disjoint term subsets)."""
+    assert full.a_trans is None, "chunks are cut from the fully materialised layout"
+    half = full.n_terms // 2
+    sub = make_problem(full.name, seed=full.seed, base_terms=np.arange(lo, hi), D=D)
+    n = hi - lo
+    place = []
+    for side, fdesc, frng, ftot, sdesc, srng, stot in (("a", full.a_desc, full.term_a_range, full.a_len, sub.a_desc, sub.term_a_range, sub.a_len),
+                                                       ("b", full.b_desc, full.term_b_range, full.b_len, sub.b_desc, sub.term_b_range, sub.b_len)):
+        def start(desc, rng_tab, total, t):           # arena offset where term t's range starts (term-major arenas)
+            while t < rng_tab.shape[0] and rng_tab[t, 0] == rng_tab[t, 1]:
+                t += 1
+            return int(desc["offset"][rng_tab[t, 0]]) if t < rng_tab.shape[0] else int(total)
+        for part, (f0, f1, s0, s1) in enumerate(((lo, hi, 0, n), (half + lo, half + hi, n, 2 * n))):
+            src_lo, src_hi = start(sdesc, srng, stot, s0), start(sdesc, srng, stot, s1)
+            dst_lo = start(fdesc, frng, ftot, f0)
+            # same blocks, same relative layout
+            a0, a1 = srng[s0, 0], srng[s1 - 1, 1]
+            b0 = frng[f0, 0]
+            assert np.array_equal(sdesc["offset"][a0:a1] - src_lo, fdesc["offset"][b0:b0 + (a1 - a0)] - dst_lo)
+            assert np.array_equal(sdesc["ld"][a0:a1], fdesc["ld"][b0:b0 + (a1 - a0)])
+            place.append((side, src_lo, src_hi, dst_lo))
+    return sub, place
+
+
 def make_psi(p: Problem, k: int = 0) -> np.ndarray:
     """k-th seeded wavefunction for problem p: N(0,1) entries on the psi blocks, global 2-norm 1 (A11, A17)."""
     rng = np.random.default_rng([p.seed, 404, k])
