@@ -104,7 +104,11 @@ int hpsi_plan(const hpsi_sectors_t* sectors, const hpsi_terms_t* terms, uint32_t
  *   p1_stages_per_unit  schedule knobs, 0 = automatic: staged K-tiles per CTA of the first-GEMM kernel; waves of CTAs the
  *   p2_waves            second GEMM's split-K aims at; least DMMA count per second-GEMM CTA.  They change the schedule
  *   p2_min_unit_dmma    (and so the rounding order of the sums), never the result beyond that; HPSI_Q_TUNING reports
- *                       the values a plan was built with. */
+ *                       the values a plan was built with.
+ *   n_vectors           k > 1 plans a BATCHED apply (hpsi_apply_multi): the k vectors widen the first GEMM's N dimension
+ *                       and multiply the second GEMM's tiles, so the operators stream from HBM once for k products - what a
+ *                       block (multi-root) Davidson calls.  Workspace grows k-fold.  Not available for plans
+ *                       with transposed blocks or HPSI_PLAN_FUSE_ALL (EINVAL).  Queries of flops / bytes stay per vector. */
 typedef struct {
   uint32_t struct_bytes;
   int32_t shard_index;
@@ -112,7 +116,7 @@ typedef struct {
   int32_t p1_stages_per_unit;
   int32_t p2_waves;
   int32_t p2_min_unit_dmma;
-  int32_t reserved;
+  int32_t n_vectors;              /* 0 or 1: single-vector plan; k > 1: lay the plan out for hpsi_apply_multi on up to k vectors */
 } hpsi_plan_options_t;
 int hpsi_plan_ex(const hpsi_sectors_t* sectors, const hpsi_terms_t* terms, uint32_t flags,
                  const hpsi_plan_options_t* options, hpsi_plan_t** plan_out);
@@ -157,6 +161,13 @@ int hpsi_set_task_coefficients(hpsi_plan_t* plan, const double* coef_host, int64
  * Repeated applies on the same inputs are bitwise identical (no atomics on data). */
 int hpsi_apply(hpsi_plan_t* plan, const double* psi_dev, double* out_dev, void* cuda_stream);
 
+/* Batched apply: out_v = H psi_v for v = 0 .. n_vectors-1 in one pass over the operators (plan built with
+ * hpsi_plan_options_t.n_vectors >= n_vectors).  Vector v of psi starts at psi_dev + v * ld_psi, of out at out_dev + v * ld_out
+ * (ld_* >= psi_length; the two sets must not overlap).  Same kernels, same launches as hpsi_apply; every vector's result
+ * is bitwise what hpsi_apply_multi gives for it in any batch of the same plan.  Enqueue only, CUDA-graph capturable. */
+int hpsi_apply_multi(hpsi_plan_t* plan, const double* psi_dev, int64_t ld_psi, double* out_dev, int64_t ld_out,
+                     int32_t n_vectors, void* cuda_stream);
+
 /* Exchange step of the term-sharded apply: out[i] = parts[0*n + i] + parts[1*n + i] + ... added in
  * that order.  Each rank hpsi_apply's its shard, the partial results are all-gathered (NCCL; psi' is 5-17 MB) into
  * parts_dev in rank order, and this sum gives every rank the same bits on every run - a library all-reduce does not
@@ -196,6 +207,21 @@ typedef struct {
  * eig_host: HOST, receives theta.  params may be NULL (defaults); info may be NULL.  Synchronises the stream. */
 int hpsi_davidson(hpsi_plan_t* plan, double* psi_inout_dev, double* eig_host,
                   const hpsi_davidson_params_t* params, hpsi_davidson_info_t* info, void* cuda_stream);
+
+/* Multi-root variant (SURVEY.md 8(f)-4 "a multi-root / Lanczos variant"; reading A21b): block Davidson-Liu for
+ * the n_roots lowest eigenpairs.  Per iteration the k lowest Ritz pairs of G = V^T H V are taken, and for every root whose
+ * residual exceeds tol a preconditioned correction vector is orthogonalised (twice) against the basis and appended; the
+ * new vectors are multiplied by H in one batched pass over the operators (hpsi_apply_multi) when the plan was built with
+ * hpsi_plan_options_t.n_vectors > 1, else one hpsi_apply each.  The basis restarts from the k Ritz vectors when it would
+ * outgrow m_max (2 n_roots <= m_max <= 32).  max_iter bounds the mat-vecs.
+ *   psi_inout_dev  DEVICE, n_roots vectors `ld` doubles apart (ld >= psi_length): in = start vectors (linearly
+ *                  independent), out = orthonormal Ritz vectors, ascending eigenvalue
+ *   eig_host       HOST, n_roots doubles;  residual_host: HOST or NULL, n_roots doubles ||H x_i - theta_i x_i||
+ *   info           n_matvec, converged (every root <= tol), residual (the largest)
+ * Synchronises the stream once per iteration. */
+int hpsi_davidson_multi(hpsi_plan_t* plan, double* psi_inout_dev, int64_t ld, int32_t n_roots, double* eig_host,
+                        double* residual_host, const hpsi_davidson_params_t* params, hpsi_davidson_info_t* info,
+                        void* cuda_stream);
 
 /* The other eigensolver PAPER.md:62 names ("the Lanczos or Davidson method"): explicitly restarted Lanczos with full
  * re-orthogonalisation, lowest eigenpair.  Same arguments as hpsi_davidson (params->precondition is ignored, m_max =
@@ -238,7 +264,8 @@ void hpsi_stream_destroy(hpsi_stream_t* s);
  * matrix (row a = the a-th kept left singular vector), concatenated; sum_l chi_l d_l doubles.
  * ------------------------------------------------------------------------------------------------------------------ */
 
-/* One-sided Jacobi SVD (Hestenes) of every psi block of `plan`, on the device, then the global selection on the host.
+/* One-sided block Jacobi SVD (Hestenes rotations, applied 32 rows at a time on the FP64 tensor pipe) of every psi block
+ * of `plan`, on the device, then the global selection on the host.
  *   psi_dev        DEVICE, psi_length doubles (not modified)
  *   side           HPSI_SIDE_LEFT: new LEFT basis, O_l = kept left singular vectors (a right-moving sweep);
  *                  HPSI_SIDE_RIGHT: new RIGHT basis, O_r = kept right singular vectors of the block whose right
@@ -253,8 +280,8 @@ void hpsi_stream_destroy(hpsi_stream_t* s);
  *                  block in table order its d_left values, descending; entries past min(d_left, d_right) are 0
  *   discarded_host HOST or NULL: sum of sigma^2 over everything not kept
  * Synchronises the stream (chi is needed on the host).  Deterministic (fixed rotation order; the only atomic is the
- * sweep's rotation counter, which steers nothing but the stop test).  A psi block whose rows + columns exceed ~12 000
- * does not fit the shared-memory kernel (EINVAL).  Errors: EINVAL (null / negative arguments), ESTATE (host-only plan), ENOMEM, ECUDA. */
+ * sweep's rotation counter, which steers nothing but the stop test).  Any block size is accepted.
+ * Errors: EINVAL (null / negative arguments), ESTATE (host-only plan, or no convergence in 60 sweeps), ENOMEM, ECUDA. */
 #define HPSI_SIDE_LEFT  0
 #define HPSI_SIDE_RIGHT 1
 int hpsi_truncate(hpsi_plan_t* plan, const double* psi_dev, int32_t side, int32_t chi_max, double eps_discard,
@@ -331,7 +358,8 @@ enum {
   HPSI_Q_TUNING = 27,        /* int64[3]: schedule knobs the plan was built with (hpsi_plan_options_t): first-GEMM K-tiles
                                 per CTA, second-GEMM waves, least DMMA count per second-GEMM CTA                    */
   HPSI_Q_PREFERRED_LAYOUT = 28, /* hpsi_layout_t: the operator-arena layout rule (what hpsi_layout_blocks applies)    */
-  HPSI_Q_N_TERMS_PLANNED = 29   /* int64: terms of this plan's shard (= n_terms without hpsi_plan_options_t.shard_of_term) */
+  HPSI_Q_N_TERMS_PLANNED = 29,  /* int64: terms of this plan's shard (= n_terms without hpsi_plan_options_t.shard_of_term) */
+  HPSI_Q_N_VECTORS = 30         /* int64: vectors the plan was laid out for (hpsi_plan_options_t.n_vectors, at least 1)     */
 };
 
 /* Layout rule of the operator arenas.  A block's rows are `stored columns` doubles long (d[col], or
@@ -369,6 +397,9 @@ const char* hpsi_last_error(void);
  * a_host / b_host are HOST copies of the arenas, psi_host / out_host HOST vectors of psi_length doubles. */
 int hpsi_debug_interpret(const hpsi_plan_t* plan, const double* a_host, const double* b_host,
                          const double* psi_host, double* out_host);
+/* the same for n_vectors vectors of a batched plan, psi_length doubles apart in psi_host / out_host */
+int hpsi_debug_interpret_multi(const hpsi_plan_t* plan, const double* a_host, const double* b_host,
+                               const double* psi_host, double* out_host, int32_t n_vectors);
 
 #ifdef __cplusplus
 }

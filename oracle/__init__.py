@@ -11,13 +11,15 @@ Plain, slow, obviously-correct CPU implementation of what the hot path computes 
 * ``dense_hamiltonian``- H restricted to the target sector, column by column through ``apply``.
 * ``diagonal``         - diag(H) from the terms whose A and B blocks are both sector-diagonal (reading A21).
 * ``davidson``         - Davidson-Liu, single root, step by step as reading A21 states it.
+* ``davidson_block``   - the same for the k lowest eigenpairs at once (block / multi-root variant, reading A21b).
 * ``useful_flops``     - the flop convention of reading A18.
 
 Only tests/, ``__graft_entry__.smoke()`` and bench.py's cpu_baseline / ``--impl reference`` legs may import
 this package.  It imports nothing from ``paper_2407_07411_b200`` and shares no code with it.
 
 Pins: tests/test_oracle_pins.py (Kronecker brute force, Hermiticity, A@psi@B.T, closed forms, Hubbard
-dimer and 4-site chain energies, dense eigensolver).  Unpinned: SU(2) recoupling / real-molecule
+dimer and 4-site chain energies, dense eigensolver; ``davidson_block``: the k lowest levels of the dense toy
+Hamiltonian, the dimer's closed-form spectrum, and k = 1 reproducing ``davidson`` step for step).  Unpinned: SU(2) recoupling / real-molecule
 energies (the paper's integrals are not available) - "parity unpinned", out of scope.
 """
 from __future__ import annotations
@@ -238,3 +240,73 @@ def davidson(p, v0: np.ndarray, tol: float = 1e-8, max_iter: int = 200, m_max: i
         Wc.append(mv(s))
         nmv += 1
     return theta, x / np.linalg.norm(x), nmv, rn
+
+
+def davidson_block(p, V0: np.ndarray, tol: float = 1e-8, max_iter: int = 200, m_max: int = 16,
+                   precondition: bool = True, matvec=None):
+    """Block Davidson-Liu for the k lowest eigenpairs (k = number of columns of V0), reading A21b of DESIGN.md - the
+    "multi-root" companion of ``davidson`` (PAPER.md:62 only names "the Lanczos or Davidson method"):
+
+    V = the k start vectors orthonormalised one after the other (classical Gram-Schmidt applied twice); W = H V.  Loop:
+    G = V^T W (symmetrised), its k lowest Ritz pairs (theta_i, y_i), x_i = V y_i, r_i = W y_i - theta_i x_i; stop when
+    every |r_i| <= tol or ``max_iter`` mat-vecs are spent.  For every root with |r_i| > tol, in ascending i:
+    s = r_i / (diag(H) - theta_i) with the small-denominator guard (or s = r_i), orthogonalised twice against the current
+    V (which includes the vectors appended before it in this iteration), dropped if |s| < 1e-14, else normalised and
+    appended.  If appending would exceed m_max columns, V is first replaced by [x_1 .. x_k] (and W by [W y_1 .. W y_k]).
+    One mat-vec per appended vector.  Returns (theta[k], X[n, k], n_matvec, residual_norms[k])."""
+    mv = (lambda x: apply(p, x)) if matvec is None else matvec
+    d = diagonal(p) if precondition else None
+    V0 = np.asarray(V0, np.float64)
+    k = V0.shape[1]
+    assert 1 <= k <= m_max // 2, "m_max must hold the k Ritz vectors and k corrections"
+    V = []
+    for i in range(k):
+        v = V0[:, i].copy()
+        for _pass in range(2):
+            for u in V:
+                v = v - u * (u @ v)
+        V.append(v / np.linalg.norm(v))
+    Wc = [mv(v) for v in V]
+    nmv = k
+    theta, X, rn = np.zeros(k), np.stack(V, axis=1), np.full(k, np.inf)
+    while True:
+        Vm, Wm = np.stack(V, axis=1), np.stack(Wc, axis=1)
+        G = Vm.T @ Wm
+        G = 0.5 * (G + G.T)
+        ev, Y = np.linalg.eigh(G)
+        theta, Yk = ev[:k].copy(), Y[:, :k]
+        X = Vm @ Yk
+        WY = Wm @ Yk
+        Rm = WY - X * theta[None, :]
+        rn = np.linalg.norm(Rm, axis=0)
+        todo = [i for i in range(k) if rn[i] > tol]
+        if not todo or nmv >= max_iter:
+            break
+        if len(V) + len(todo) > m_max:                 # restart from the Ritz vectors
+            V = [X[:, i].copy() for i in range(k)]
+            Wc = [WY[:, i].copy() for i in range(k)]
+        new = []
+        for i in todo:
+            if nmv + len(new) >= max_iter:
+                break
+            r = Rm[:, i]
+            if d is not None:
+                den = d - theta[i]
+                den = np.where(np.abs(den) < 1e-8, np.where(den < 0, -1e-8, 1e-8), den)
+                s = r / den
+            else:
+                s = r.copy()
+            for _pass in range(2):
+                Vm = np.stack(V, axis=1)
+                s = s - Vm @ (Vm.T @ s)
+            ns = np.linalg.norm(s)
+            if ns < 1e-14:
+                continue
+            V.append(s / ns)
+            new.append(V[-1])
+        if not new:
+            break
+        for v in new:
+            Wc.append(mv(v))
+        nmv += len(new)
+    return theta, X, nmv, rn

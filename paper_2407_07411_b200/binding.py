@@ -24,7 +24,8 @@ HPSI_PLAN_FUSE_ALL = 1 << 4
  HPSI_Q_N_ORDER1_TASKS, HPSI_Q_LAUNCHES_PER_APPLY, HPSI_Q_ALIGNED16, HPSI_Q_INTERMEDIATE_BYTES,
  HPSI_Q_ISSUED_FLOPS_P1, HPSI_Q_TASKS, HPSI_Q_USEFUL_FLOPS_P1, HPSI_Q_CRITICAL_FLOPS, HPSI_Q_PSI_ROWS,
  HPSI_Q_ISO_CAPACITY, HPSI_Q_SVD_SWEEPS, HPSI_Q_SVD_LAUNCHES, HPSI_Q_PSI_COLS, HPSI_Q_ISO_CAPACITY_RIGHT,
- HPSI_Q_N_FUSED_UNITS, HPSI_Q_N_FUSED_TASKS, HPSI_Q_TUNING, HPSI_Q_PREFERRED_LAYOUT, HPSI_Q_N_TERMS_PLANNED) = range(30)
+ HPSI_Q_N_FUSED_UNITS, HPSI_Q_N_FUSED_TASKS, HPSI_Q_TUNING, HPSI_Q_PREFERRED_LAYOUT, HPSI_Q_N_TERMS_PLANNED,
+ HPSI_Q_N_VECTORS) = range(31)
 HPSI_SIDE_LEFT, HPSI_SIDE_RIGHT = 0, 1
 (HPSI_RQ_OUT_LENGTH, HPSI_RQ_OUT_BLOCKS, HPSI_RQ_ISO_LENGTH, HPSI_RQ_USEFUL_FLOPS, HPSI_RQ_ALGO_BYTES,
  HPSI_RQ_WORKSPACE_BYTES, HPSI_RQ_N_UNITS_1, HPSI_RQ_N_UNITS_2, HPSI_RQ_ALIGNED16, HPSI_RQ_INTERMEDIATE_BYTES) = range(10)
@@ -55,7 +56,7 @@ class hpsi_terms_t(ctypes.Structure):
 class hpsi_plan_options_t(ctypes.Structure):
     _fields_ = [("struct_bytes", ctypes.c_uint32), ("shard_index", ctypes.c_int32), ("shard_of_term", ctypes.c_void_p),
                 ("p1_stages_per_unit", ctypes.c_int32), ("p2_waves", ctypes.c_int32),
-                ("p2_min_unit_dmma", ctypes.c_int32), ("reserved", ctypes.c_int32)]
+                ("p2_min_unit_dmma", ctypes.c_int32), ("n_vectors", ctypes.c_int32)]
 
 
 class hpsi_layout_t(ctypes.Structure):
@@ -98,6 +99,10 @@ def lib() -> ctypes.CDLL:
         L.hpsi_set_task_coefficients.argtypes = [vp, vp, i64, vp]
         L.hpsi_apply.argtypes = [vp, vp, vp, vp]
         L.hpsi_apply_host.argtypes = [vp, vp, vp, vp]
+        L.hpsi_apply_multi.argtypes = [vp, vp, i64, vp, i64, i32, vp]
+        L.hpsi_apply_multi.restype = ctypes.c_int
+        L.hpsi_debug_interpret_multi.argtypes = [vp, vp, vp, vp, vp, i32]
+        L.hpsi_debug_interpret_multi.restype = ctypes.c_int
         L.hpsi_sum_shards.argtypes = [vp, i32, i64, vp, vp]
         L.hpsi_sum_shards.restype = ctypes.c_int
         L.hpsi_apply_profiled.argtypes = [vp, vp, vp, vp, ctypes.POINTER(ctypes.c_float)]
@@ -105,6 +110,9 @@ def lib() -> ctypes.CDLL:
         L.hpsi_davidson.argtypes = [vp, vp, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(hpsi_davidson_params_t),
                                     ctypes.POINTER(hpsi_davidson_info_t), vp]
         L.hpsi_lanczos.argtypes = L.hpsi_davidson.argtypes
+        L.hpsi_davidson_multi.argtypes = [vp, vp, i64, i32, vp, vp, ctypes.POINTER(hpsi_davidson_params_t),
+                                          ctypes.POINTER(hpsi_davidson_info_t), vp]
+        L.hpsi_davidson_multi.restype = ctypes.c_int
         L.hpsi_query.argtypes = [vp, ctypes.c_int, vp, ctypes.c_size_t]
         L.hpsi_stream_create.argtypes = [ctypes.POINTER(hpsi_sectors_t), ctypes.POINTER(hpsi_terms_t), i64, ctypes.c_uint32,
                                          ctypes.POINTER(vp)]
@@ -205,20 +213,20 @@ def _marshal(q_left, q_right, d_left, d_right, target, coef, a_blocks, b_blocks,
 def hpsi_plan(q_left, q_right, d_left, d_right, target, coef, a_blocks, b_blocks, a_data=None, b_data=None,
               a_len: int = 0, b_len: int = 0, flags: int = 0, a_transposed=None, b_transposed=None,
               shard_of_term=None, shard_index: int = 0, p1_stages_per_unit: int = 0, p2_waves: int = 0,
-              p2_min_unit_dmma: int = 0) -> Plan:
+              p2_min_unit_dmma: int = 0, n_vectors: int = 0) -> Plan:
     """hpsi_plan / hpsi_plan_ex(sector table, term list).  Host arrays: numpy; a_blocks/b_blocks: numpy arrays with the
     24-byte hpsi_opblock_t layout; a_data/b_data: torch CUDA float64 tensors (or None, to hpsi_bind later).  Any of the
     keyword options of hpsi_plan_options_t (term shard, schedule knobs) routes the call through hpsi_plan_ex."""
     sec, trm, keep = _marshal(q_left, q_right, d_left, d_right, target, coef, a_blocks, b_blocks, a_data, b_data,
                               a_len, b_len, a_transposed, b_transposed)
     out = ctypes.c_void_p()
-    if shard_of_term is not None or p1_stages_per_unit or p2_waves or p2_min_unit_dmma:
+    if shard_of_term is not None or p1_stages_per_unit or p2_waves or p2_min_unit_dmma or n_vectors:
         sot = None
         if shard_of_term is not None:
             sot = np.ascontiguousarray(shard_of_term, np.int32)
             assert sot.shape[0] == trm.n_terms
         opt = hpsi_plan_options_t(ctypes.sizeof(hpsi_plan_options_t), int(shard_index), _ptr(sot),
-                                  int(p1_stages_per_unit), int(p2_waves), int(p2_min_unit_dmma), 0)
+                                  int(p1_stages_per_unit), int(p2_waves), int(p2_min_unit_dmma), int(n_vectors))
         _check(lib().hpsi_plan_ex(ctypes.byref(sec), ctypes.byref(trm), flags, ctypes.byref(opt), ctypes.byref(out)))
     else:
         _check(lib().hpsi_plan(ctypes.byref(sec), ctypes.byref(trm), flags, ctypes.byref(out)))
@@ -267,6 +275,14 @@ def hpsi_apply(plan: Plan, psi, out, stream=None) -> None:
     _check(lib().hpsi_apply(plan.handle, _ptr(psi), _ptr(out), _stream(stream)))
 
 
+def hpsi_apply_multi(plan: Plan, psi, out, n_vectors: int, stream=None, ld_psi: int = 0, ld_out: int = 0) -> None:
+    """out_v = H psi_v for v < n_vectors; psi/out: torch CUDA float64 tensors holding the vectors ld_* doubles apart
+    (default: psi_length, i.e. a contiguous [n_vectors, psi_length] array)."""
+    n = hpsi_query(plan, HPSI_Q_PSI_LENGTH)
+    _check(lib().hpsi_apply_multi(plan.handle, _ptr(psi), int(ld_psi or n), _ptr(out), int(ld_out or n), int(n_vectors),
+                                  _stream(stream)))
+
+
 def hpsi_sum_shards(parts, n_parts: int, out, stream=None) -> None:
     """out = sum over r of parts[r*n:(r+1)*n] in rank order (parts: torch CUDA tensor of n_parts * n doubles)."""
     _check(lib().hpsi_sum_shards(_ptr(parts), int(n_parts), int(out.numel()), _ptr(out), _stream(stream)))
@@ -297,6 +313,20 @@ def hpsi_davidson(plan: Plan, psi_inout, tol: float = 1e-8, max_iter: int = 200,
     _check(lib().hpsi_davidson(plan.handle, _ptr(psi_inout), ctypes.byref(eig), ctypes.byref(prm),
                                ctypes.byref(info), _stream(stream)))
     return eig.value, {"n_matvec": info.n_matvec, "converged": bool(info.converged), "residual": info.residual}
+
+
+def hpsi_davidson_multi(plan: Plan, psi_inout, n_roots: int, tol: float = 1e-8, max_iter: int = 200, m_max: int = 16,
+                        precondition: bool = True, stream=None):
+    """Block Davidson for the n_roots lowest eigenpairs.  psi_inout: torch CUDA float64 tensor [n_roots, psi_length]
+    (start vectors in, Ritz vectors out).  Returns (theta[n_roots], info dict with per-root residuals)."""
+    prm = hpsi_davidson_params_t(tol, max_iter, m_max, 1 if precondition else 0)
+    info = hpsi_davidson_info_t()
+    eig = np.zeros(n_roots)
+    res = np.zeros(n_roots)
+    assert psi_inout.dim() == 2 and psi_inout.shape[0] == n_roots and psi_inout.is_contiguous()
+    _check(lib().hpsi_davidson_multi(plan.handle, _ptr(psi_inout), int(psi_inout.shape[1]), int(n_roots), eig.ctypes.data,
+                                     res.ctypes.data, ctypes.byref(prm), ctypes.byref(info), _stream(stream)))
+    return eig, {"n_matvec": info.n_matvec, "converged": bool(info.converged), "residual": info.residual, "residuals": res}
 
 
 def hpsi_lanczos(plan: Plan, psi_inout, tol: float = 1e-8, max_iter: int = 200, m_max: int = 16, stream=None):
@@ -399,11 +429,13 @@ def hpsi_bench_fp64_pipe(kind: int, iters: int):
 
 
 def hpsi_debug_interpret(plan: Plan, a_host: np.ndarray, b_host: np.ndarray, psi_host: np.ndarray) -> np.ndarray:
-    """Run the device schedule with naive loops on the CPU (planner verification; tests only)."""
+    """Run the device schedule with naive loops on the CPU (planner verification; tests only).  psi_host of shape
+    [psi_length] or, for a batched plan, [n_vectors, psi_length]."""
     psi_host = np.ascontiguousarray(psi_host, np.float64)
     out = np.empty_like(psi_host)
-    _check(lib().hpsi_debug_interpret(plan.handle, _ptr(np.ascontiguousarray(a_host, np.float64)),
-                                      _ptr(np.ascontiguousarray(b_host, np.float64)), _ptr(psi_host), _ptr(out)))
+    nvec = 1 if psi_host.ndim == 1 else psi_host.shape[0]
+    _check(lib().hpsi_debug_interpret_multi(plan.handle, _ptr(np.ascontiguousarray(a_host, np.float64)),
+                                            _ptr(np.ascontiguousarray(b_host, np.float64)), _ptr(psi_host), _ptr(out), nvec))
     return out
 
 

@@ -40,7 +40,7 @@ static int upload(const std::vector<T>& v, char* base, size_t& cursor, const T**
 int upload_schedule(hpsi_plan_t* p) {
   const Schedule& sc = p->sc;
   size_t total = table_bytes(sc.blocks) + table_bytes(sc.segs) + table_bytes(sc.groups) + table_bytes(sc.p1) +
-                 table_bytes(sc.runs) + table_bytes(sc.p2) + table_bytes(sc.pf) + table_bytes(sc.diag);
+                 table_bytes(sc.runs) + table_bytes(sc.p2) + table_bytes(sc.pf) + table_bytes(sc.diag) + table_bytes(sc.elem);
   HPSI_CUDA(cudaMalloc(&p->d_tables, total));
   cudaError_t e = cudaMalloc(&p->d_ws, (size_t)sc.ws_len * sizeof(double));
   if (e != cudaSuccess) {
@@ -64,6 +64,8 @@ int upload_schedule(hpsi_plan_t* p) {
   if ((rc = upload(sc.p2, base, cur, &p->dev.p2))) return rc;
   if ((rc = upload(sc.pf, base, cur, &p->dev.pf))) return rc;
   if ((rc = upload(sc.diag, base, cur, &p->dev.diag))) return rc;
+  if ((rc = upload(sc.elem, base, cur, &p->dev.elem))) return rc;
+  p->dev.n_elem = (int)sc.elem.size();
   p->dev.ws = p->d_ws;
   p->dev.n_blocks = (int)sc.blocks.size();
   p->dev.n_p1 = (int)sc.p1.size();
@@ -71,6 +73,9 @@ int upload_schedule(hpsi_plan_t* p) {
   p->dev.n_pf = (int)sc.pf.size();
   p->dev.max_block_elems = sc.max_block_elems;
   p->dev.paired = sc.paired ? 1 : 0;
+  p->dev.nvec = sc.nvec;
+  p->dev.nvec_active = 1;
+  p->dev.ld_psi = p->dev.ld_out = sc.psi_len;
   if (sc.psi_len > 0) {
     HPSI_CUDA(cudaMalloc(&p->d_psi_stage, (size_t)sc.psi_len * sizeof(double)));
     HPSI_CUDA(cudaMalloc(&p->d_out_stage, (size_t)sc.psi_len * sizeof(double)));
@@ -89,6 +94,8 @@ void free_plan(hpsi_plan_t* p) {
     cudaFree(p->d_dav);
     cudaFree(p->d_svd);
     cudaFreeHost(p->h_dav);
+    if (p->dav_side) cudaStreamDestroy(p->dav_side);
+    for (auto& e : p->dav_ev) if (e) cudaEventDestroy(e);
     cudaGetLastError();
   }
   delete p;
@@ -168,6 +175,7 @@ extern "C" int hpsi_plan_ex(const hpsi_sectors_t* sectors, const hpsi_terms_t* t
     opt.p1_stages_per_unit = options->p1_stages_per_unit;
     opt.p2_waves = options->p2_waves;
     opt.p2_min_unit_dmma = options->p2_min_unit_dmma;
+    opt.n_vectors = options->n_vectors;
   }
   hpsi_plan_t* p = new (std::nothrow) hpsi_plan_t();
   if (!p) { set_error("out of host memory"); return HPSI_ENOMEM; }
@@ -295,7 +303,21 @@ extern "C" void hpsi_destroy(hpsi_plan_t* p) { free_plan(p); }
 extern "C" int hpsi_apply(hpsi_plan_t* p, const double* psi_dev, double* out_dev, void* cuda_stream) {
   return hpsi::apply_impl(p, psi_dev, out_dev, false, cuda_stream);
 }
-int hpsi::apply_impl(hpsi_plan_t* p, const double* psi_dev, double* out_dev, bool accumulate, void* cuda_stream) {
+
+extern "C" int hpsi_apply_multi(hpsi_plan_t* p, const double* psi_dev, int64_t ld_psi, double* out_dev, int64_t ld_out,
+                                int32_t n_vectors, void* cuda_stream) {
+  if (!p) { set_error("null plan"); return HPSI_EINVAL; }
+  if (n_vectors < 1 || n_vectors > p->sc.nvec) { set_error("n_vectors outside 1 .. hpsi_plan_options_t.n_vectors of the plan"); return HPSI_EINVAL; }
+  if (ld_psi < p->sc.psi_len || ld_out < p->sc.psi_len) { set_error("vector stride below psi_length"); return HPSI_EINVAL; }
+  if (psi_dev && out_dev) {                      // the two sets of vectors must not overlap
+    const double *a0 = psi_dev, *a1 = psi_dev + (n_vectors - 1) * ld_psi + p->sc.psi_len;
+    const double *b0 = out_dev, *b1 = out_dev + (n_vectors - 1) * ld_out + p->sc.psi_len;
+    if (a0 < b1 && b0 < a1 && p->sc.psi_len > 0) { set_error("psi and out must not overlap"); return HPSI_EINVAL; }
+  }
+  return hpsi::apply_impl(p, psi_dev, out_dev, false, cuda_stream, nullptr, nullptr, n_vectors, ld_psi, ld_out);
+}
+int hpsi::apply_impl(hpsi_plan_t* p, const double* psi_dev, double* out_dev, bool accumulate, void* cuda_stream,
+                     const double* nrm2_dev, double* normalized_dev, int n_vectors, int64_t ld_psi, int64_t ld_out) {
   if (!p) { set_error("null plan"); return HPSI_EINVAL; }
   if (p->host_only) { set_error("host-only plan: hpsi_apply needs a CUDA device (no CPU fallback)"); return HPSI_ESTATE; }
   if (!p->bound) { set_error("operator arenas not bound (hpsi_bind)"); return HPSI_ESTATE; }
@@ -303,11 +325,15 @@ int hpsi::apply_impl(hpsi_plan_t* p, const double* psi_dev, double* out_dev, boo
   if (!psi_dev || !out_dev) { set_error("null psi/out"); return HPSI_EINVAL; }
   if (psi_dev == out_dev) { set_error("psi and out must not alias"); return HPSI_EINVAL; }
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
-  launch_prep(p->dev, psi_dev, st);
-  launch_p1(p->dev, p->aligned16, st);
-  launch_p2(p->dev, p->aligned16, st);
-  launch_pf(p->dev, p->aligned16, st);
-  launch_reduce(p->dev, out_dev, accumulate, st);
+  DevSchedule dv = p->dev;                       // per-call view: how many vectors, how far apart
+  dv.nvec_active = n_vectors;
+  dv.ld_psi = ld_psi > 0 ? ld_psi : p->sc.psi_len;
+  dv.ld_out = ld_out > 0 ? ld_out : p->sc.psi_len;
+  launch_prep(dv, psi_dev, nrm2_dev, normalized_dev, st);
+  launch_p1(dv, p->aligned16, st);
+  launch_p2(dv, p->aligned16, st);
+  launch_pf(dv, p->aligned16, st);
+  launch_reduce(dv, out_dev, accumulate, st);
   HPSI_CUDA(cudaGetLastError());
   return HPSI_OK;
 }
@@ -322,7 +348,7 @@ extern "C" int hpsi_apply_profiled(hpsi_plan_t* p, const double* psi_dev, double
   EventSet<5> ev;
   HPSI_CUDA(ev.create());
   HPSI_CUDA(cudaEventRecord(ev[0], st));
-  launch_prep(p->dev, psi_dev, st);
+  launch_prep(p->dev, psi_dev, nullptr, nullptr, st);
   HPSI_CUDA(cudaEventRecord(ev[1], st));
   launch_p1(p->dev, p->aligned16, st);
   HPSI_CUDA(cudaEventRecord(ev[2], st));
@@ -418,6 +444,7 @@ extern "C" int hpsi_query(const hpsi_plan_t* p, int what, void* out, size_t byte
     case HPSI_Q_SVD_SWEEPS: return put_i64(p->svd_sweeps);
     case HPSI_Q_SVD_LAUNCHES: return put_i64(p->svd_launches);
     case HPSI_Q_N_TERMS_PLANNED: return put_i64(sc.n_terms_planned);
+    case HPSI_Q_N_VECTORS: return put_i64(sc.nvec);
     case HPSI_Q_TUNING: {
       if (bytes < sizeof sc.tuning) { set_error("hpsi_query: buffer too small"); return HPSI_EINVAL; }
       memcpy(out, sc.tuning, sizeof sc.tuning);
@@ -440,11 +467,17 @@ extern "C" int hpsi_query(const hpsi_plan_t* p, int what, void* out, size_t byte
 
 extern "C" int hpsi_debug_interpret(const hpsi_plan_t* p, const double* a_host, const double* b_host,
                                     const double* psi_host, double* out_host) {
+  return hpsi_debug_interpret_multi(p, a_host, b_host, psi_host, out_host, 1);
+}
+
+extern "C" int hpsi_debug_interpret_multi(const hpsi_plan_t* p, const double* a_host, const double* b_host,
+                                          const double* psi_host, double* out_host, int32_t n_vectors) {
   if (!p) { set_error("null plan"); return HPSI_EINVAL; }
+  if (n_vectors < 1 || n_vectors > p->sc.nvec) { set_error("n_vectors outside 1 .. the plan's n_vectors"); return HPSI_EINVAL; }
   if (p->sc.psi_len > 0 && (!psi_host || !out_host)) { set_error("null psi/out"); return HPSI_EINVAL; }
   if (!p->sc.segs.empty() && (!a_host || !b_host)) { set_error("null arena"); return HPSI_EINVAL; }
   try {
-    interpret_schedule(p->sc, a_host, b_host, psi_host, out_host);
+    interpret_schedule(p->sc, a_host, b_host, psi_host, out_host, n_vectors);
   } catch (const std::bad_alloc&) {
     set_error("out of host memory in interpreter");
     return HPSI_ENOMEM;

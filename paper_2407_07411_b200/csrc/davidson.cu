@@ -1,9 +1,11 @@
 // hpsi_davidson: Davidson-Liu, lowest eigenpair, single root (PAPER.md:62 names "Lanczos or Davidson"; the algorithm
-// is DESIGN.md reading A21).  Every O(psi_length) operation and the small subspace eigenproblem (cyclic Jacobi in one
-// warp) run on the device; the host reads back two scalars per iteration (residual norm^2, |s|^2) to steer the loop.
-// All reductions are two-stage with a fixed order, so a run is bitwise reproducible.
+// is DESIGN.md reading A21).  Every O(psi_length) operation and the small subspace eigenproblem (parallel Jacobi in one
+// thread block) run on the device, five fused launches per iteration besides the mat-vec; the host reads back theta and
+// the residual norm on a side stream while the orthogonalisation of the same iteration is still running, so the next
+// mat-vec is enqueued without a bubble.  All reductions are two-stage with a fixed order: bitwise reproducible.
 #include <algorithm>
 #include <cmath>
+#include <vector>
 
 #include "plan_dev.h"
 
@@ -63,103 +65,231 @@ __global__ void scale_kernel(double* dst, const double* src, double* dst2, const
   }
 }
 
-// Smallest eigenpair of the symmetric j x j matrix G (leading dimension MMAX) by parallel two-sided Jacobi: the j/2
-// disjoint rotations of a round-robin round are applied together, warp k = pair k, lane t = row t (blockDim.x =
-// 32 * ceil(j/2)); first all column updates A J, then all row updates J^T (A J).  (A one-warp cyclic version took 86 us per
-// call at j ~ 10 - a quarter of a Davidson iteration's fixed cost.)  Writes theta[0] and y[0..j); G is left untouched.
-__global__ void small_eig_kernel(const double* __restrict__ G, int j, double* theta, double* y) {
-  __shared__ double A[MMAX][MMAX + 1], Q[MMAX][MMAX + 1];
-  __shared__ double norms[2];
-  const int t = threadIdx.x & 31, k = threadIdx.x >> 5;
+// Smallest eigenpair of the symmetric j x j matrix G (leading dimension MMAX) by parallel two-sided Jacobi, run by ONE
+// thread block of nw = blockDim.x / 32 warps: the m/2 disjoint rotations of a round-robin round are applied together,
+// pair k by warp k % nw, lane t = row t; first all column updates A J, then all row updates J^T (A J).  (A one-warp cyclic
+// version took 86 us per call at j ~ 10 - a quarter of a Davidson iteration's fixed cost.)  Writes theta[0] and y[0..j);
+// G is left untouched.  Shared memory is passed in so that the fused Gram kernel can run it in its last block.
+struct EigSmem {
+  double A[MMAX][MMAX + 1], Q[MMAX][MMAX + 1];
+  double cs[MMAX / 2][2];
+  double norms[2];
+};
+__device__ void small_eig_block(const double* __restrict__ G, int j, double* theta, double* y, EigSmem& sm, int k = 1) {
+  const int t = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
   const int m = (j + 1) & ~1;                            // players of the round-robin (a dummy one if j is odd)
-  const int np = m > 1 ? m / 2 : 1;                      // = warps in the block
-  for (int c = k; c < j; c += np)
-    if (t < j) { A[t][c] = 0.5 * (G[t * MMAX + c] + G[c * MMAX + t]); Q[t][c] = (t == c) ? 1.0 : 0.0; }
+  const int np = m > 1 ? m / 2 : 1;                      // pairs per round
+  for (int c = wid; c < j; c += nw)
+    if (t < j) { sm.A[t][c] = 0.5 * (G[t * MMAX + c] + G[c * MMAX + t]); sm.Q[t][c] = (t == c) ? 1.0 : 0.0; }
   __syncthreads();
   for (int sweep = 0; sweep < 30 && j > 1; ++sweep) {
-    if (k == 0) {                                        // squared norms of the off-diagonal part and of the diagonal
+    if (wid == 0) {                                      // squared norms of the off-diagonal part and of the diagonal
       double off = 0.0, dg = 0.0;
       if (t < j) {
-        dg = A[t][t] * A[t][t];
-        for (int q = t + 1; q < j; ++q) off += A[t][q] * A[t][q];
+        dg = sm.A[t][t] * sm.A[t][t];
+        for (int q = t + 1; q < j; ++q) off += sm.A[t][q] * sm.A[t][q];
       }
 #pragma unroll
       for (int o = 16; o > 0; o >>= 1) { off += __shfl_xor_sync(0xffffffffu, off, o); dg += __shfl_xor_sync(0xffffffffu, dg, o); }
-      if (t == 0) { norms[0] = off; norms[1] = dg; }
+      if (t == 0) { sm.norms[0] = off; sm.norms[1] = dg; }
     }
     __syncthreads();
-    const double off = norms[0], dg = norms[1];
+    const double off = sm.norms[0], dg = sm.norms[1];
     if (off <= 1e-34 * (dg + 2.0 * off) || off < 1e-300) break;   // off-diagonal norm below 1e-17 of the matrix norm
     for (int r = 0; r < m - 1; ++r) {
-      int p, q;
-      if (k == 0) { p = m - 1; q = r; }
-      else { p = (r + k) % (m - 1); q = (r - k + m - 1) % (m - 1); }
-      if (p > q) { const int tmp = p; p = q; q = tmp; }
-      double c = 1.0, sn = 0.0;
-      if (q < j) {                                       // not the dummy player
-        const double apq = A[p][q];
-        if (fabs(apq) >= 1e-300) {
-          const double app = A[p][p], aqq = A[q][q];
-          const double tau = (aqq - app) / (2.0 * apq);
-          const double tt = (tau >= 0 ? 1.0 : -1.0) / (fabs(tau) + sqrt(1.0 + tau * tau));
-          c = 1.0 / sqrt(1.0 + tt * tt);
-          sn = tt * c;
+      for (int k = wid; k < np; k += nw) {               // columns p, q of pair k (this pair's alone)
+        int p, q;
+        if (k == 0) { p = m - 1; q = r; }
+        else { p = (r + k) % (m - 1); q = (r - k + m - 1) % (m - 1); }
+        if (p > q) { const int tmp = p; p = q; q = tmp; }
+        double c = 1.0, sn = 0.0;
+        if (q < j) {                                     // not the dummy player
+          const double apq = sm.A[p][q];
+          if (fabs(apq) >= 1e-300) {
+            const double app = sm.A[p][p], aqq = sm.A[q][q];
+            const double tau = (aqq - app) / (2.0 * apq);
+            const double tt = (tau >= 0 ? 1.0 : -1.0) / (fabs(tau) + sqrt(1.0 + tau * tau));
+            c = 1.0 / sqrt(1.0 + tt * tt);
+            sn = tt * c;
+          }
+        }
+        __syncwarp();
+        if (t == 0) { sm.cs[k][0] = c; sm.cs[k][1] = sn; }
+        if (sn != 0.0 && t < j) {
+          const double akp = sm.A[t][p], akq = sm.A[t][q];
+          sm.A[t][p] = c * akp - sn * akq;
+          sm.A[t][q] = sn * akp + c * akq;
+          const double qkp = sm.Q[t][p], qkq = sm.Q[t][q];
+          sm.Q[t][p] = c * qkp - sn * qkq;
+          sm.Q[t][q] = sn * qkp + c * qkq;
         }
       }
-      __syncwarp();
-      const bool act = sn != 0.0 && t < j;
-      if (act) {                                         // columns p, q (this warp's alone)
-        const double akp = A[t][p], akq = A[t][q];
-        A[t][p] = c * akp - sn * akq;
-        A[t][q] = sn * akp + c * akq;
-        const double qkp = Q[t][p], qkq = Q[t][q];
-        Q[t][p] = c * qkp - sn * qkq;
-        Q[t][q] = sn * qkp + c * qkq;
-      }
       __syncthreads();
-      if (act) {                                         // rows p, q
-        const double apk = A[p][t], aqk = A[q][t];
-        A[p][t] = c * apk - sn * aqk;
-        A[q][t] = sn * apk + c * aqk;
+      for (int k = wid; k < np; k += nw) {               // rows p, q
+        int p, q;
+        if (k == 0) { p = m - 1; q = r; }
+        else { p = (r + k) % (m - 1); q = (r - k + m - 1) % (m - 1); }
+        if (p > q) { const int tmp = p; p = q; q = tmp; }
+        const double c = sm.cs[k][0], sn = sm.cs[k][1];
+        if (sn != 0.0 && t < j) {
+          const double apk = sm.A[p][t], aqk = sm.A[q][t];
+          sm.A[p][t] = c * apk - sn * aqk;
+          sm.A[q][t] = sn * apk + c * aqk;
+        }
       }
       __syncthreads();
     }
   }
   __syncthreads();
-  if (k == 0) {
-    int best = 0;
-    for (int i = 1; i < j; ++i)
-      if (A[i][i] < A[best][best]) best = i;
-    if (t == 0) theta[0] = A[best][best];
-    if (t < j) y[t] = Q[t][best];
+  if (wid == 0) {                                        // the k lowest Ritz pairs, ascending: theta[r], y[r * MMAX + t]
+    unsigned taken = 0u;
+    for (int r = 0; r < k && r < j; ++r) {
+      int best = -1;
+      for (int i = 0; i < j; ++i)
+        if (!((taken >> i) & 1u) && (best < 0 || sm.A[i][i] < sm.A[best][best])) best = i;
+      taken |= 1u << best;
+      if (t == 0) theta[r] = sm.A[best][best];
+      if (t < j) y[r * MMAX + t] = sm.Q[t][best];
+    }
   }
 }
+__global__ void small_eig_kernel(const double* __restrict__ G, int j, double* theta, double* y, int k) {
+  __shared__ EigSmem sm;
+  small_eig_block(G, j, theta, y, sm, k);
+}
 
-// x = sum_i y_i V_i ; wy = sum_i y_i W_i ; r = wy - theta x
-__global__ void ritz_kernel(const double* __restrict__ V, const double* __restrict__ W, int64_t n, int j,
-                            const double* __restrict__ y, const double* __restrict__ theta, double* x, double* wy,
-                            double* r) {
+// ---------------------------------------------------------------------------------- fused Davidson iteration kernels
+// One Davidson iteration is five launches besides the mat-vec (it was twelve): every kernel below runs NB blocks, block b
+// owning the slice [b * per, (b + 1) * per) of the vectors; phase A is element-wise on the slice, phase B takes the dot
+// products the NEXT step needs on the same slice (warp w: dot products w, w + 8, ...), and the block that finishes last
+// (ticket from an atomic counter - control only) adds the NB partials of every dot product in a fixed order.  `ctl[5]`
+// != 0 ("dead": the correction vector vanished, |s| < 1e-14) turns the kernels that would overwrite results into no-ops,
+// so the host may learn of it one iteration late.
+__device__ __forceinline__ double warp_sum_d(double v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  return v;
+}
+__device__ __forceinline__ bool dav_last_block(unsigned int* ticket) {
+  __shared__ bool last;
+  __syncthreads();
+  if (threadIdx.x == 0) { __threadfence(); last = atomicAdd(ticket, 1u) == gridDim.x - 1; }
+  __syncthreads();
+  if (last) __threadfence();
+  return last;
+}
+// sum of the NB partials of one dot product, by one warp, in a fixed order
+__device__ __forceinline__ double dav_sum_partials(const double* partial, int lane) {
+  const volatile double* pv = partial + lane * (NB / 32);
+  double t = 0.0;
+  for (int i = 0; i < NB / 32; ++i) t += pv[i];
+  return warp_sum_d(t);
+}
+__device__ __forceinline__ void dav_slice(int64_t n, int64_t& lo, int64_t& hi) {
+  const int64_t per = (n + NB - 1) / NB;
+  lo = (int64_t)blockIdx.x * per;
+  hi = lo + per < n ? lo + per : n;
+  if (lo > hi) lo = hi;
+}
+
+// G[:, j-1] = G[j-1, :] = V^T W_{j-1};  then (last block) the smallest Ritz pair of G -> theta, y
+__global__ void __launch_bounds__(256) dav_gram_eig_kernel(const double* __restrict__ V, const double* __restrict__ wl, int64_t n,
+                                                           int j, double* partial, unsigned int* ticket, double* G,
+                                                           double* theta, double* y, const double* ctl) {
+  __shared__ EigSmem sm;
+  if (ctl[5] != 0.0) return;
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
+  int64_t lo, hi;
+  dav_slice(n, lo, hi);
+  for (int i = wid; i < j; i += nw) {
+    const double* v = V + (int64_t)i * n;
+    double s = 0.0;
+    for (int64_t e = lo + lane; e < hi; e += 32) s += v[e] * wl[e];
+    s = warp_sum_d(s);
+    if (lane == 0) partial[i * NB + blockIdx.x] = s;
+  }
+  if (!dav_last_block(ticket)) return;
+  for (int i = wid; i < j; i += nw) {
+    const double t = dav_sum_partials(partial + i * NB, lane);
+    if (lane == 0) { G[i * MMAX + (j - 1)] = t; G[(j - 1) * MMAX + i] = t; }
+  }
+  if (threadIdx.x == 0) *ticket = 0;
+  __syncthreads();
+  small_eig_block(G, j, theta, y, sm);
+}
+
+// x = V y, wy = W y, r = wy - theta x, s = r / (diag - theta) (or r);  c_i = V_i . s,  nrm_r2 = r . r
+__global__ void __launch_bounds__(256) dav_ritz_kernel(const double* __restrict__ V, const double* __restrict__ W,
+                                                       const double* __restrict__ diag, int64_t n, int j,
+                                                       const double* __restrict__ y, const double* __restrict__ theta,
+                                                       int precondition, double* x, double* wy, double* r, double* s,
+                                                       double* partial, unsigned int* ticket, double* c, double* nrm_r2,
+                                                       const double* ctl) {
+  if (ctl[5] != 0.0) return;
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
   const double th = *theta;
-  for (int64_t e = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; e < n; e += (int64_t)gridDim.x * blockDim.x) {
+  int64_t lo, hi;
+  dav_slice(n, lo, hi);
+  for (int64_t e = lo + threadIdx.x; e < hi; e += blockDim.x) {
     double sx = 0.0, sw = 0.0;
     for (int i = 0; i < j; ++i) { const double yi = y[i]; sx += yi * V[i * n + e]; sw += yi * W[i * n + e]; }
-    x[e] = sx; wy[e] = sw; r[e] = sw - th * sx;
-  }
-}
-
-// s = r / (diag - theta) with |den| clamped to >= 1e-8 keeping its sign; or s = r
-__global__ void precond_kernel(const double* __restrict__ r, const double* __restrict__ diag,
-                               const double* __restrict__ theta, int precondition, double* s, int64_t n) {
-  const double th = *theta;
-  for (int64_t e = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; e < n; e += (int64_t)gridDim.x * blockDim.x) {
-    double v = r[e];
+    const double rr = sw - th * sx;
+    double v = rr;
     if (precondition) {
       double den = diag[e] - th;
       if (fabs(den) < 1e-8) den = (den < 0) ? -1e-8 : 1e-8;
       v /= den;
     }
-    s[e] = v;
+    x[e] = sx; wy[e] = sw; r[e] = rr; s[e] = v;
   }
+  __syncthreads();                                       // this block's slice of r and s is written (and visible to the block)
+  for (int i = wid; i <= j; i += nw) {
+    const double* a = i < j ? V + (int64_t)i * n : r;
+    const double* b = i < j ? s : r;
+    double t = 0.0;
+    for (int64_t e = lo + lane; e < hi; e += 32) t += a[e] * b[e];
+    t = warp_sum_d(t);
+    if (lane == 0) partial[i * NB + blockIdx.x] = t;
+  }
+  if (!dav_last_block(ticket)) return;
+  for (int i = wid; i <= j; i += nw) {
+    const double t = dav_sum_partials(partial + i * NB, lane);
+    if (lane == 0) { if (i < j) c[i] = t; else *nrm_r2 = t; }
+  }
+  if (threadIdx.x == 0) *ticket = 0;
+}
+
+// s -= sum_i c_in[i] V_i;  then either c_out[i] = V_i . s (first Gram-Schmidt pass) or nrm_s2 = s . s (second pass, which
+// also raises the "dead" flag when |s| < 1e-14)
+__global__ void __launch_bounds__(256) dav_project_kernel(double* s, const double* __restrict__ V, int64_t n, int j,
+                                                          const double* __restrict__ c_in, double* partial,
+                                                          unsigned int* ticket, double* c_out, double* nrm_s2, double* ctl) {
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
+  int64_t lo, hi;
+  dav_slice(n, lo, hi);
+  for (int64_t e = lo + threadIdx.x; e < hi; e += blockDim.x) {
+    double acc = s[e];
+    for (int i = 0; i < j; ++i) acc -= c_in[i] * V[i * n + e];
+    s[e] = acc;
+  }
+  __syncthreads();
+  const int ndots = c_out ? j : 1;
+  for (int i = wid; i < ndots; i += nw) {
+    const double* a = c_out ? V + (int64_t)i * n : s;
+    double t = 0.0;
+    for (int64_t e = lo + lane; e < hi; e += 32) t += a[e] * s[e];
+    t = warp_sum_d(t);
+    if (lane == 0) partial[i * NB + blockIdx.x] = t;
+  }
+  if (!dav_last_block(ticket)) return;
+  for (int i = wid; i < ndots; i += nw) {
+    const double t = dav_sum_partials(partial + i * NB, lane);
+    if (lane == 0) {
+      if (c_out) c_out[i] = t;
+      else { *nrm_s2 = t; if (!(t >= 1e-28) && ctl[5] == 0.0) ctl[5] = 1.0; }
+    }
+  }
+  if (threadIdx.x == 0) *ticket = 0;
 }
 
 // s -= sum_i c_i V_i
@@ -188,10 +318,11 @@ extern "C" int hpsi_davidson(hpsi_plan_t* p, double* psi, double* eig_host, cons
   if (n == 0) { set_error("empty target sector"); return HPSI_EINVAL; }
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
 
-  // buffers: V[m][n] W[m][n] diag x wy r s | G[MMAX*MMAX] y[MMAX] c[MMAX] theta nrm[4] partial[MMAX*NB] counters[MMAX]
-  const size_t small = MMAX * MMAX + 2 * MMAX + 8 + MMAX * NB + MMAX;
+  // buffers: V[m][n] W[m][n] diag x wy r s | G[MMAX*MMAX] y[MMAX] c[MMAX] c2[MMAX] theta ctl[7] partial[(MMAX+1)*NB] tickets
+  const size_t small = MMAX * MMAX + 3 * MMAX + 8 + (MMAX + 1) * NB + MMAX;
   const size_t need = (size_t)(2 * prm.m_max + 5) * n + small;
   if (p->dav_doubles < need) {
+    HPSI_CUDA(cudaStreamSynchronize(st));
     cudaFree(p->d_dav);
     p->d_dav = nullptr;
     p->dav_doubles = 0;
@@ -203,67 +334,260 @@ extern "C" int hpsi_davidson(hpsi_plan_t* p, double* psi, double* eig_host, cons
     p->dav_doubles = need;
   }
   if (!p->h_dav) HPSI_CUDA(cudaMallocHost(&p->h_dav, 8 * sizeof(double)));
+  if (!p->dav_side) {
+    HPSI_CUDA(cudaStreamCreateWithFlags(&p->dav_side, cudaStreamNonBlocking));
+    for (auto& e : p->dav_ev) HPSI_CUDA(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+  }
   double* V = p->d_dav;
   double* W = V + (size_t)prm.m_max * n;
   double* diag = W + (size_t)prm.m_max * n;
   double *x = diag + n, *wy = x + n, *r = wy + n, *s = r + n;
   double* G = s + n;
-  double *y = G + MMAX * MMAX, *c = y + MMAX, *theta = c + MMAX, *nrm = theta + 1, *partial = nrm + 7;
-  unsigned int* counters = reinterpret_cast<unsigned int*>(partial + MMAX * NB);
+  double *y = G + MMAX * MMAX, *c = y + MMAX, *c2 = c + MMAX, *theta = c2 + MMAX, *ctl = theta + 1, *partial = ctl + 7;
+  unsigned int* tickets = reinterpret_cast<unsigned int*>(partial + (MMAX + 1) * NB);
+  // ctl: [0] |psi|^2  [1] |r|^2  [2] |x|^2  [3] |s|^2  [5] dead flag   (theta, ctl[0..5] are read back together)
   HPSI_CUDA(cudaMemsetAsync(G, 0, small * sizeof(double), st));
 
   const int eg = (int)std::min<int64_t>((n + 255) / 256, 2048);
   auto dots = [&](const double* X, int nvec, const double* yv, double* out, int stride, double* mirror, int mstride) {
-    dot_kernel<<<dim3(NB, nvec), 256, 0, st>>>(X, n, yv, n, partial, counters, out, stride, mirror, mstride);
+    dot_kernel<<<dim3(NB, nvec), 256, 0, st>>>(X, n, yv, n, partial, tickets + 8, out, stride, mirror, mstride);
   };
   int rc;
   if (prm.precondition && (rc = hpsi_diagonal(p, diag, cuda_stream)) != HPSI_OK) return rc;
 
-  // V0 = psi/|psi| ; W0 = H V0
-  dots(psi, 1, psi, nrm, 1, nullptr, 0);
-  scale_kernel<<<eg, 256, 0, st>>>(V, psi, nullptr, nullptr, nrm, n);
-  if ((rc = hpsi_apply(p, V, W, cuda_stream)) != HPSI_OK) return rc;
+  // V0 = psi/|psi| ; W0 = H V0   (the normalisation rides on the mat-vec's prep kernel)
+  dots(psi, 1, psi, ctl, 1, nullptr, 0);
+  if ((rc = apply_impl(p, psi, W, false, cuda_stream, ctl, V)) != HPSI_OK) return rc;
   int j = 1, nmv = 1, converged = 0;
   double rn = INFINITY, th = 0.0;
+  double* hostbuf = p->h_dav;
   for (int it = 0; it < prm.max_iter; ++it) {
-    // new column of G = V^T W:  G[i][j-1] = G[j-1][i] = V_i . W_{j-1}
-    dots(V, j, W + (size_t)(j - 1) * n, G + (j - 1), MMAX, G + (size_t)(j - 1) * MMAX, 1);
-    small_eig_kernel<<<1, 32 * std::max(1, (j + 1) / 2), 0, st>>>(G, j, theta, y);
-    ritz_kernel<<<eg, 256, 0, st>>>(V, W, n, j, y, theta, x, wy, r);
-    dots(r, 1, r, nrm + 1, 1, nullptr, 0);                          // nrm[1] = |r|^2
-    precond_kernel<<<eg, 256, 0, st>>>(r, diag, theta, prm.precondition, s, n);
+    // new column of G = V^T W and its smallest Ritz pair; Ritz vector, residual, correction vector and its overlaps with V
+    dav_gram_eig_kernel<<<NB, 256, 0, st>>>(V, W + (size_t)(j - 1) * n, n, j, partial, tickets, G, theta, y, ctl);
+    dav_ritz_kernel<<<NB, 256, 0, st>>>(V, W, diag, n, j, y, theta, prm.precondition, x, wy, r, s, partial, tickets + 1, c,
+                                         ctl + 1, ctl);
+    // theta and |r|^2 travel to the host on a side stream while the orthogonalisation below is still running
+    HPSI_CUDA(cudaEventRecord(p->dav_ev[0], st));
+    HPSI_CUDA(cudaStreamWaitEvent(p->dav_side, p->dav_ev[0], 0));
+    HPSI_CUDA(cudaMemcpyAsync(hostbuf, theta, 7 * sizeof(double), cudaMemcpyDeviceToHost, p->dav_side));
+    HPSI_CUDA(cudaEventRecord(p->dav_ev[1], p->dav_side));
     if (j >= prm.m_max) {                                           // restart with V = [x/|x|]
-      dots(x, 1, x, nrm + 2, 1, nullptr, 0);
-      scale_kernel<<<eg, 256, 0, st>>>(V, x, W, wy, nrm + 2, n);
+      dots(x, 1, x, ctl + 2, 1, nullptr, 0);
+      scale_kernel<<<eg, 256, 0, st>>>(V, x, W, wy, ctl + 2, n);
       HPSI_CUDA(cudaMemsetAsync(G, 0, MMAX * MMAX * sizeof(double), st));
       set_scalar_kernel<<<1, 1, 0, st>>>(G, theta);
       j = 1;
+      dots(V, 1, s, c, 1, nullptr, 0);
     }
-    for (int pass = 0; pass < 2; ++pass) {                          // classical Gram-Schmidt, twice
-      dots(V, j, s, c, 1, nullptr, 0);
-      project_kernel<<<eg, 256, 0, st>>>(s, V, n, j, c);
-    }
-    dots(s, 1, s, nrm + 3, 1, nullptr, 0);                          // nrm[3] = |s|^2
-    scale_kernel<<<eg, 256, 0, st>>>(V + (size_t)j * n, s, nullptr, nullptr, nrm + 3, n);
-    double* hostbuf = p->h_dav;
-    HPSI_CUDA(cudaMemcpyAsync(hostbuf, theta, 5 * sizeof(double), cudaMemcpyDeviceToHost, st));
-    HPSI_CUDA(cudaStreamSynchronize(st));
+    // classical Gram-Schmidt, twice; the second pass leaves |s|^2 (and the dead flag)
+    dav_project_kernel<<<NB, 256, 0, st>>>(s, V, n, j, c, partial, tickets + 2, c2, nullptr, ctl);
+    dav_project_kernel<<<NB, 256, 0, st>>>(s, V, n, j, c2, partial, tickets + 3, nullptr, ctl + 3, ctl);
+    HPSI_CUDA(cudaEventSynchronize(p->dav_ev[1]));
     th = hostbuf[0];
     rn = std::sqrt(hostbuf[2]);
-    const double ns = std::sqrt(hostbuf[4]);
+    if (hostbuf[6] != 0.0) break;                                   // the previous correction vector vanished: theta, x are the last good ones
     if (rn <= prm.tol) { converged = 1; break; }
-    if (!(ns >= 1e-14) || nmv >= prm.max_iter) break;
-    if ((rc = hpsi_apply(p, V + (size_t)j * n, W + (size_t)j * n, cuda_stream)) != HPSI_OK) return rc;
+    if (nmv >= prm.max_iter) break;
+    // V_j = s/|s| (written by the prep kernel), W_j = H V_j - enqueued while the orthogonalisation may still be running
+    if ((rc = apply_impl(p, s, W + (size_t)j * n, false, cuda_stream, ctl + 3, V + (size_t)j * n)) != HPSI_OK) return rc;
     ++j;
     ++nmv;
   }
   // psi = x/|x|
-  dots(x, 1, x, nrm + 2, 1, nullptr, 0);
-  scale_kernel<<<eg, 256, 0, st>>>(psi, x, nullptr, nullptr, nrm + 2, n);
+  dots(x, 1, x, ctl + 2, 1, nullptr, 0);
+  scale_kernel<<<eg, 256, 0, st>>>(psi, x, nullptr, nullptr, ctl + 2, n);
   HPSI_CUDA(cudaGetLastError());
   HPSI_CUDA(cudaStreamSynchronize(st));
   *eig_host = th;
   if (info) { info->n_matvec = nmv; info->converged = converged; info->residual = rn; }
+  return HPSI_OK;
+}
+
+// ------------------------------------------------------------------------------------- block (multi-root) Davidson
+// hpsi_davidson_multi: block Davidson-Liu for the k lowest eigenpairs (reading A21b; PAPER.md:62 names the
+// method only).  The new correction vectors of an iteration are multiplied by H in ONE batched apply (hpsi_apply_multi
+// when the plan was laid out for several vectors), so the operators stream from HBM once per iteration, not once per root.
+namespace {
+
+// x_r = V y_r, wy_r = W y_r, res_r = wy_r - theta_r x_r  for root r = blockIdx.y (y_r = Y + r * MMAX)
+__global__ void ritz_multi_kernel(const double* __restrict__ V, const double* __restrict__ W, int64_t n, int j,
+                                  const double* __restrict__ Y, const double* __restrict__ theta, double* X, double* WY,
+                                  double* Rv) {
+  const int r = blockIdx.y;
+  const double* y = Y + r * MMAX;
+  const double th = theta[r];
+  for (int64_t e = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; e < n; e += (int64_t)gridDim.x * blockDim.x) {
+    double sx = 0.0, sw = 0.0;
+    for (int i = 0; i < j; ++i) { const double yi = y[i]; sx += yi * V[i * n + e]; sw += yi * W[i * n + e]; }
+    X[r * n + e] = sx; WY[r * n + e] = sw; Rv[r * n + e] = sw - th * sx;
+  }
+}
+
+// s = r / (diag - theta) with |den| clamped to >= 1e-8 keeping its sign; or s = r
+__global__ void precond_kernel(const double* __restrict__ r, const double* __restrict__ diag,
+                               const double* __restrict__ theta, int precondition, double* s, int64_t n) {
+  const double th = *theta;
+  for (int64_t e = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; e < n; e += (int64_t)gridDim.x * blockDim.x) {
+    double v = r[e];
+    if (precondition) {
+      double den = diag[e] - th;
+      if (fabs(den) < 1e-8) den = (den < 0) ? -1e-8 : 1e-8;
+      v /= den;
+    }
+    s[e] = v;
+  }
+}
+
+__global__ void set_diag_kernel(double* G, const double* theta, int k) {
+  if ((int)threadIdx.x < k) G[threadIdx.x * MMAX + threadIdx.x] = theta[threadIdx.x];
+}
+
+}  // namespace
+
+extern "C" int hpsi_davidson_multi(hpsi_plan_t* p, double* psi, int64_t ld, int32_t n_roots, double* eig_host,
+                                   double* residual_host, const hpsi_davidson_params_t* params, hpsi_davidson_info_t* info,
+                                   void* cuda_stream) {
+  using namespace hpsi;
+  if (!p || !psi || !eig_host) { set_error("null argument"); return HPSI_EINVAL; }
+  if (p->host_only) { set_error("host-only plan: hpsi_davidson_multi needs a CUDA device (no CPU fallback)"); return HPSI_ESTATE; }
+  if (!p->bound) { set_error("operator arenas not bound (hpsi_bind)"); return HPSI_ESTATE; }
+  hpsi_davidson_params_t prm = {1e-8, 200, 16, 1};
+  if (params) prm = *params;
+  const int k = n_roots;
+  if (prm.m_max < 2 || prm.m_max > MMAX || prm.max_iter < 1 || !(prm.tol >= 0.0)) { set_error("bad Davidson parameters"); return HPSI_EINVAL; }
+  if (k < 1 || 2 * k > prm.m_max) { set_error("n_roots must be between 1 and m_max / 2"); return HPSI_EINVAL; }
+  const int64_t n = p->sc.psi_len;
+  if (n == 0) { set_error("empty target sector"); return HPSI_EINVAL; }
+  if (ld < n) { set_error("vector stride below psi_length"); return HPSI_EINVAL; }
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+
+  // buffers: V[m][n] W[m][n] diag X[k][n] WY[k][n] R[k][n] s | G[MMAX^2] Y[MMAX^2] theta[MMAX] c[MMAX] nrm[MMAX] partial[MMAX*NB] counters
+  const size_t small = 2 * MMAX * MMAX + 3 * MMAX + MMAX * NB + MMAX;
+  const size_t need = (size_t)(2 * prm.m_max + 3 * k + 2) * n + small;
+  if (p->dav_doubles < need) {
+    HPSI_CUDA(cudaStreamSynchronize(st));
+    cudaFree(p->d_dav);
+    p->d_dav = nullptr;
+    p->dav_doubles = 0;
+    if (cudaMalloc(&p->d_dav, need * sizeof(double)) != cudaSuccess) {
+      cudaGetLastError();
+      set_error("device allocation for the Davidson subspace failed");
+      return HPSI_ENOMEM;
+    }
+    p->dav_doubles = need;
+  }
+  std::vector<double> host(2 * MMAX + 2);
+  double* V = p->d_dav;
+  double* W = V + (size_t)prm.m_max * n;
+  double* diag = W + (size_t)prm.m_max * n;
+  double* X = diag + n;
+  double* WY = X + (size_t)k * n;
+  double* Rv = WY + (size_t)k * n;
+  double* s = Rv + (size_t)k * n;
+  double* G = s + n;
+  double *Y = G + MMAX * MMAX, *theta = Y + MMAX * MMAX, *c = theta + MMAX, *nrm = c + MMAX, *partial = nrm + MMAX;
+  unsigned int* counters = reinterpret_cast<unsigned int*>(partial + MMAX * NB);
+  HPSI_CUDA(cudaMemsetAsync(G, 0, small * sizeof(double), st));
+  const int eg = (int)std::min<int64_t>((n + 255) / 256, 2048);
+  auto dots = [&](const double* Xv, int nvec, const double* yv, double* out, int stride, double* mirror, int mstride) {
+    dot_kernel<<<dim3(NB, nvec), 256, 0, st>>>(Xv, n, yv, n, partial, counters, out, stride, mirror, mstride);
+  };
+  // W[j0 .. j0 + cnt) = H V[j0 .. j0 + cnt): as few passes over the operators as the plan's batch width allows
+  auto apply_block = [&](int j0, int cnt) -> int {
+    for (int off = 0; off < cnt; off += p->sc.nvec) {
+      const int nb = std::min(p->sc.nvec, cnt - off);
+      int rc = apply_impl(p, V + (size_t)(j0 + off) * n, W + (size_t)(j0 + off) * n, false, cuda_stream, nullptr, nullptr, nb, n, n);
+      if (rc != HPSI_OK) return rc;
+    }
+    return HPSI_OK;
+  };
+  // s orthogonalised twice against V[0 .. j), normalised into V[j]; returns |s|^2 location nrm[slot]
+  auto orth_append = [&](int j, int slot) {
+    for (int pass = 0; pass < 2 && j > 0; ++pass) {
+      dots(V, j, s, c, 1, nullptr, 0);
+      project_kernel<<<eg, 256, 0, st>>>(s, V, n, j, c);
+    }
+    dots(s, 1, s, nrm + slot, 1, nullptr, 0);
+    scale_kernel<<<eg, 256, 0, st>>>(V + (size_t)j * n, s, nullptr, nullptr, nrm + slot, n);
+  };
+  int rc;
+  if (prm.precondition && (rc = hpsi_diagonal(p, diag, cuda_stream)) != HPSI_OK) return rc;
+
+  // start vectors, orthonormalised one after the other
+  for (int i = 0; i < k; ++i) {
+    HPSI_CUDA(cudaMemcpyAsync(s, psi + (size_t)i * ld, n * sizeof(double), cudaMemcpyDeviceToDevice, st));
+    orth_append(i, i);
+  }
+  if ((rc = apply_block(0, k)) != HPSI_OK) return rc;
+  int j = k, g0 = 0, nmv = k, converged = 0;
+  std::vector<double> th(k, 0.0), rn(k, INFINITY);
+  for (;;) {
+    for (int col = g0; col < j; ++col)                                // new columns (and rows) of G = V^T W
+      dots(V, j, W + (size_t)col * n, G + col, MMAX, G + (size_t)col * MMAX, 1);
+    g0 = j;
+    small_eig_kernel<<<1, 32 * std::min(8, std::max(1, (j + 1) / 2)), 0, st>>>(G, j, theta, Y, k);
+    ritz_multi_kernel<<<dim3(eg, k), 256, 0, st>>>(V, W, n, j, Y, theta, X, WY, Rv);
+    for (int r = 0; r < k; ++r) dots(Rv + (size_t)r * n, 1, Rv + (size_t)r * n, nrm + r, 1, nullptr, 0);
+    HPSI_CUDA(cudaMemcpyAsync(host.data(), theta, k * sizeof(double), cudaMemcpyDeviceToHost, st));
+    HPSI_CUDA(cudaMemcpyAsync(host.data() + MMAX, nrm, k * sizeof(double), cudaMemcpyDeviceToHost, st));
+    HPSI_CUDA(cudaStreamSynchronize(st));
+    std::vector<int> todo;
+    for (int r = 0; r < k; ++r) {
+      th[r] = host[r];
+      rn[r] = std::sqrt(host[MMAX + r]);
+      if (rn[r] > prm.tol) todo.push_back(r);
+    }
+    if (todo.empty()) { converged = 1; break; }
+    if (nmv >= prm.max_iter) break;
+    if (j + (int)todo.size() > prm.m_max) {                           // restart from the Ritz vectors
+      HPSI_CUDA(cudaMemcpyAsync(V, X, (size_t)k * n * sizeof(double), cudaMemcpyDeviceToDevice, st));
+      HPSI_CUDA(cudaMemcpyAsync(W, WY, (size_t)k * n * sizeof(double), cudaMemcpyDeviceToDevice, st));
+      HPSI_CUDA(cudaMemsetAsync(G, 0, MMAX * MMAX * sizeof(double), st));
+      set_diag_kernel<<<1, 32, 0, st>>>(G, theta, k);
+      j = g0 = k;
+    }
+    // correction vectors of the unconverged roots, each orthogonalised against V and the ones appended before it.  Fast
+    // path: all of them without a host round trip, their norms read back together; if one vanished (|s| < 1e-14, it
+    // must be dropped and the later ones change) the iteration's appends are redone one by one.
+    auto append_all = [&](bool check_each) -> int {
+      int added = 0;
+      for (int r : todo) {
+        if (nmv + added >= prm.max_iter) break;
+        precond_kernel<<<eg, 256, 0, st>>>(Rv + (size_t)r * n, diag, theta + r, prm.precondition, s, n);
+        orth_append(j + added, added);
+        if (check_each) {
+          cudaMemcpyAsync(host.data(), nrm + added, sizeof(double), cudaMemcpyDeviceToHost, st);
+          cudaStreamSynchronize(st);
+          if (!(host[0] >= 1e-28)) continue;                          // dropped: the slot is reused by the next root
+        }
+        ++added;
+      }
+      return added;
+    };
+    int added = append_all(false);
+    if (added > 0) {
+      HPSI_CUDA(cudaMemcpyAsync(host.data(), nrm, added * sizeof(double), cudaMemcpyDeviceToHost, st));
+      HPSI_CUDA(cudaStreamSynchronize(st));
+      bool ok = true;
+      for (int a = 0; a < added; ++a) ok = ok && host[a] >= 1e-28;
+      if (!ok) added = append_all(true);
+    }
+    if (added == 0) break;
+    if ((rc = apply_block(j, added)) != HPSI_OK) return rc;
+    j += added;
+    nmv += added;
+  }
+  for (int r = 0; r < k; ++r)
+    HPSI_CUDA(cudaMemcpyAsync(psi + (size_t)r * ld, X + (size_t)r * n, n * sizeof(double), cudaMemcpyDeviceToDevice, st));
+  HPSI_CUDA(cudaGetLastError());
+  HPSI_CUDA(cudaStreamSynchronize(st));
+  double worst = 0.0;
+  for (int r = 0; r < k; ++r) {
+    eig_host[r] = th[r];
+    if (residual_host) residual_host[r] = rn[r];
+    worst = std::max(worst, rn[r]);
+  }
+  if (info) { info->n_matvec = nmv; info->converged = converged; info->residual = worst; }
   return HPSI_OK;
 }
 
@@ -344,7 +668,7 @@ extern "C" int hpsi_lanczos(hpsi_plan_t* p, double* psi, double* eig_host, const
     project_kernel<<<eg, 256, 0, st>>>(w, V, n, j + 1, c2);          // second Gram-Schmidt pass
     dots(w, 1, w, nrm + 3);                                          // beta_j^2
     lanczos_set_kernel<<<1, 1, 0, st>>>(T, j, c + j, nrm + 3);
-    small_eig_kernel<<<1, 32 * std::max(1, (j + 2) / 2), 0, st>>>(T, j + 1, theta, y);
+    small_eig_kernel<<<1, 32 * std::max(1, (j + 2) / 2), 0, st>>>(T, j + 1, theta, y, 1);
     HPSI_CUDA(cudaMemcpyAsync(host, theta, sizeof(double), cudaMemcpyDeviceToHost, st));
     HPSI_CUDA(cudaMemcpyAsync(host + 1, y + j, sizeof(double), cudaMemcpyDeviceToHost, st));
     HPSI_CUDA(cudaMemcpyAsync(host + 2, nrm + 3, sizeof(double), cudaMemcpyDeviceToHost, st));

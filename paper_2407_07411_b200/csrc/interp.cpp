@@ -8,22 +8,24 @@
 
 namespace hpsi {
 
-void interpret_schedule(const Schedule& sc, const double* a, const double* b, const double* psi, double* out) {
+void interpret_schedule(const Schedule& sc, const double* a, const double* b, const double* psi, double* out, int nvec) {
   std::vector<double> wsv((size_t)sc.ws_len, 0.0);
   double* ws = wsv.data();
-  // prep
-  for (const PsiBlk& B : sc.blocks)
-    for (int x = 0; x < B.rows; ++x)
-      for (int y = 0; y < B.cols; ++y) {
-        double v = psi[B.off + (int64_t)x * B.cols + y];
-        ws[B.p_off + (int64_t)x * B.ldp + y] = v;
-        ws[B.t_off + (int64_t)y * B.ldt + x] = v;
-      }
+  // prep: the copies of vector v sit p_vstride / t_vstride after those of vector v - 1
+  for (int v = 0; v < nvec; ++v)
+    for (const PsiBlk& B : sc.blocks)
+      for (int x = 0; x < B.rows; ++x)
+        for (int y = 0; y < B.cols; ++y) {
+          double val = psi[(int64_t)v * sc.psi_len + B.off + (int64_t)x * B.cols + y];
+          ws[B.p_off + v * B.p_vstride + (int64_t)x * B.ldp + y] = val;
+          ws[B.t_off + v * B.t_vstride + (int64_t)y * B.ldt + x] = val;
+        }
   // P1: T_t[i, j] = coef_t * sum_k X_t[i,k] Y[j,k] for the unit's tile and terms
   for (const P1Unit& u : sc.p1) {
+    if (u.vec >= nvec) continue;
     const Group& g = sc.groups[u.group];
     const double* xbase = (g.order == 1) ? a : b;
-    const double* y = ws + g.y1_off;
+    const double* y = ws + g.y1_off + (int64_t)u.vec * g.N1 * g.ldy1;     // vector v: rows [v N1, (v + 1) N1) of the stacked operand
     for (int t = u.t0; t < u.t1; ++t) {
       const Seg& sg = sc.segs[g.seg0 + t];
       // element (i, k) of the operator block: plain storage [i][k], transposed storage [k][i]
@@ -35,13 +37,14 @@ void interpret_schedule(const Schedule& sc, const double* a, const double* b, co
           const double* yr = y + (int64_t)j * g.ldy1;
           double s = 0.0;
           for (int k = 0; k < g.K1; ++k) s += xr[k * xsk] * yr[k];
-          ws[g.ws_off + ((int64_t)t * g.rows + u.i0 + r) * g.ldw + j] = sg.coef * s;
+          ws[g.ws_off + ((int64_t)t * g.rows + u.i0 + r) * g.ldw + u.vec * g.N1p + j] = sg.coef * s;
         }
       }
     }
   }
   // P2: partial[i,j] = sum over runs, segs, k of X[i,k] Y[j,k]
   for (const P2Unit& u : sc.p2) {
+    if (u.vec >= nvec) continue;
     for (int r = 0; r < u.rows_valid; ++r)
       for (int c = 0; c < u.cols_valid; ++c) {
         double s = 0.0;
@@ -49,7 +52,7 @@ void interpret_schedule(const Schedule& sc, const double* a, const double* b, co
           const Run& run = sc.runs[ri];
           for (int si = run.seg_begin; si < run.seg_end; ++si) {
             const Seg& sg = sc.segs[si];
-            const int64_t t_off = run.ws_off + (int64_t)(si - run.seg0) * run.rows * run.ldw;
+            const int64_t t_off = run.ws_off + (int64_t)(si - run.seg0) * run.rows * run.ldw + u.vec * run.Kp;
             const int64_t osi = sg.p2_trans ? 1 : sg.p2_ld, osk = sg.p2_trans ? sg.p2_ld : 1;   // operator block strides
             const double *xr, *yr;
             int64_t xsk = 1, ysk = 1;
@@ -104,15 +107,16 @@ void interpret_schedule(const Schedule& sc, const double* a, const double* b, co
     for (int r = 0; r < u.rows_valid; ++r)
       for (int c = 0; c < u.cols_valid; ++c) ws[u.out_off + (int64_t)r * u.ldo + c] = acc[(size_t)r * u.cols_valid + c];
   }
-  // ordered reduce
-  for (const PsiBlk& B : sc.blocks)
-    for (int x = 0; x < B.rows; ++x)
-      for (int y = 0; y < B.cols; ++y) {
-        double s = 0.0;
-        for (int sp = 0; sp < B.nsplit; ++sp)
-          s += ws[B.part_off + (int64_t)sp * B.rows * B.ldo + (int64_t)x * B.ldo + y];
-        out[B.off + (int64_t)x * B.cols + y] = s;
-      }
+  // ordered reduce (partials: split-major, vector-minor)
+  for (int v = 0; v < nvec; ++v)
+    for (const PsiBlk& B : sc.blocks)
+      for (int x = 0; x < B.rows; ++x)
+        for (int y = 0; y < B.cols; ++y) {
+          double s = 0.0;
+          for (int sp = 0; sp < B.nsplit; ++sp)
+            s += ws[B.part_off + ((int64_t)sp * sc.nvec + v) * B.rows * B.ldo + (int64_t)x * B.ldo + y];
+          out[(int64_t)v * sc.psi_len + B.off + (int64_t)x * B.cols + y] = s;
+        }
 }
 
 }  // namespace hpsi

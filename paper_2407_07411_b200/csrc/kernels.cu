@@ -53,7 +53,7 @@ __device__ __forceinline__ void p1_consume(const DevSchedule& d, const P1Unit& u
       const Seg* sg = d.segs + g.seg0 + t;
       store_tile_t<MI, NJ>(d.rot_dst + sg->p2_off + (int64_t)u.j0 * sg->p2_ld + u.i0, sg->p2_ld, u.rows_valid, u.cols_valid, acc, w, lane);
     } else {
-      double* dst = d.ws + g.ws_off + ((int64_t)t * g.rows + u.i0) * g.ldw + u.j0;
+      double* dst = d.ws + g.ws_off + ((int64_t)t * g.rows + u.i0) * g.ldw + u.vec * g.N1p + u.j0;
       store_tile<MI, NJ>(dst, g.ldw, u.rows_valid, u.cols_valid, acc, w, lane, coef);
     }
   }
@@ -82,17 +82,19 @@ template <bool TMA, bool ROT>
 __global__ void __maxnreg__(136) p1_kernel(DevSchedule d) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const P1Unit u = d.p1[blockIdx.x];
+  if (!ROT && u.vec >= d.nvec_active) return;            // batched plan applied to fewer vectors than it was laid out for
   const Group g = d.groups[u.group];
   const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
   const SmemLayout sm(smem_raw);
   init_barriers<TMA>(sm, tid);
   const int ntiles = (g.K1 + KT - 1) / KT;
+  const int yrow0 = u.vec * g.N1 + u.j0;                 // the Y operand of vector v starts at row v * N1 of the stacked copies
 
   if (wid == NCONS) {
     // ---------------- producer warp
     Ring ring{0, 1};
     const unsigned char* ymap = d.maps + (int64_t)g.y1_map * TMAP_BYTES;
-    const double* ybase = d.ws + g.y1_off + (int64_t)u.j0 * g.ldy1;
+    const double* ybase = d.ws + g.y1_off + (int64_t)yrow0 * g.ldy1;
     const double* xarena = (g.order == 1) ? d.a : d.b;
     const int xboxes = (u.rows_valid + TILE - 1) / TILE;          // 64-row boxes of the X tile that hold valid rows
     for (int t = u.t0; t < u.t1; ++t) {
@@ -111,7 +113,7 @@ __global__ void __maxnreg__(136) p1_kernel(DevSchedule d) {
           if (lane == 0) {
             mbar_arrive_expect_tx(full, (xboxes + 1) * OP_BYTES);
             for (int bx = 0; bx < xboxes; ++bx) tma_load_2d(sx + bx * OP_BYTES, xmap, kt * KT, u.i0 + bx * TILE, full);
-            tma_load_2d(sy, ymap, kt * KT, u.j0, full);
+            tma_load_2d(sy, ymap, kt * KT, yrow0, full);
           }
         } else {
           for (int bx = 0; bx < xboxes; ++bx)
@@ -184,6 +186,7 @@ template <bool TMA>
 __global__ void __maxnreg__(136) p2_kernel(DevSchedule d) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const P2Unit u = d.p2[blockIdx.x];
+  if (u.vec >= d.nvec_active) return;                    // batched plan applied to fewer vectors than it was laid out for
   const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
   const SmemLayout sm(smem_raw);
   init_barriers<TMA>(sm, tid);
@@ -195,6 +198,7 @@ __global__ void __maxnreg__(136) p2_kernel(DevSchedule d) {
     const int xboxes = (u.rows_valid + TILE - 1) / TILE;          // 64-row boxes of the X tile that hold valid rows
     const unsigned char *xmap = nullptr, *ymap = nullptr;      // TMA: tensor maps and first rows of the segment
     int xrow = 0, yrow = 0;
+    int xcol = 0, ycol = 0;                                    // batched plans: first column of this unit's vector in the intermediate
     const double *xbase = nullptr, *ybase = nullptr;           // LDGSTS: first rows and leading dimensions
     int64_t xld = 0, yld = 0;
     auto open_seg = [&]() {
@@ -205,10 +209,10 @@ __global__ void __maxnreg__(136) p2_kernel(DevSchedule d) {
         const unsigned char* opmap = d.maps + (int64_t)sg->p2_map * TMAP_BYTES;
         const unsigned char* wsmap = d.maps + (int64_t)r.ws_map * TMAP_BYTES;
         if (lane == 0 && it.seg + 2 < r.seg_end) tma_prefetch_desc(d.maps + (int64_t)sg[2].p2_map * TMAP_BYTES);   // descriptor of the segment after next
-        if (r.order == 1) { xmap = wsmap; xrow = trow + u.i0; ymap = opmap; yrow = u.j0; }
-        else              { xmap = opmap; xrow = u.i0; ymap = wsmap; yrow = trow + u.j0; }
+        if (r.order == 1) { xmap = wsmap; xrow = trow + u.i0; xcol = u.vec * r.Kp; ymap = opmap; yrow = u.j0; ycol = 0; }
+        else              { xmap = opmap; xrow = u.i0; xcol = 0; ymap = wsmap; yrow = trow + u.j0; ycol = u.vec * r.Kp; }
       } else {
-        const double* wsrows = d.ws + r.ws_off + (int64_t)trow * r.ldw;
+        const double* wsrows = d.ws + r.ws_off + (int64_t)trow * r.ldw + u.vec * r.Kp;
         if (r.order == 1) {
           xld = r.ldw; xbase = wsrows + (int64_t)u.i0 * xld;
           yld = sg->p2_ld; ybase = d.b + sg->p2_off + (int64_t)u.j0 * yld;
@@ -225,8 +229,8 @@ __global__ void __maxnreg__(136) p2_kernel(DevSchedule d) {
       if (TMA) {
         if (lane == 0) {
           mbar_arrive_expect_tx(full, (xboxes + 1) * OP_BYTES);
-          for (int bx = 0; bx < xboxes; ++bx) tma_load_2d(sx + bx * OP_BYTES, xmap, it.kappa, xrow + bx * TILE, full);
-          tma_load_2d(sy, ymap, it.kappa, yrow, full);
+          for (int bx = 0; bx < xboxes; ++bx) tma_load_2d(sx + bx * OP_BYTES, xmap, xcol + it.kappa, xrow + bx * TILE, full);
+          tma_load_2d(sy, ymap, ycol + it.kappa, yrow, full);
         }
       } else {
         for (int bx = 0; bx < xboxes; ++bx)
@@ -256,16 +260,25 @@ __global__ void __maxnreg__(136) p2_kernel(DevSchedule d) {
 }
 
 // ------------------------------------------------------------------------------- prep / reduce / diag kernels
+// Element-wise launches run one CTA per ElemCta granule (256 consecutive elements of one psi block): every CTA has work,
+// whatever the spread of block sizes (a (largest block / 256) x n_blocks grid left most CTAs of the small blocks idle:
+// reduce 0.030 -> see DESIGN.md on the D = 1024 config).  blockIdx.y = vector of a batched apply.
+//
 // prep: psi block (rows x cols, dense) -> padded copy (rows x ldp) and padded transpose (cols x ldt) in the workspace.
-__global__ void prep_kernel(DevSchedule d, const double* __restrict__ psi) {
-  const PsiBlk B = d.blocks[blockIdx.y];
-  const int n = B.rows * B.cols;
-  for (int e = blockIdx.x * blockDim.x + threadIdx.x; e < n; e += gridDim.x * blockDim.x) {
-    const int x = e / B.cols, y = e - x * B.cols;
-    const double v = psi[B.off + e];
-    d.ws[B.p_off + (int64_t)x * B.ldp + y] = v;
-    d.ws[B.t_off + (int64_t)y * B.ldt + x] = v;
-  }
+// With nrm2 given, psi is first divided by sqrt(nrm2[v]) and the normalised vector is also written to `normalized` (the
+// eigensolver drivers hand over a new basis vector unnormalised: one launch fewer per iteration).
+__global__ void prep_kernel(DevSchedule d, const double* __restrict__ psi, const double* __restrict__ nrm2,
+                            double* __restrict__ normalized) {
+  const ElemCta c = d.elem[blockIdx.x];
+  const PsiBlk B = d.blocks[c.blk];
+  const int e = c.e0 + threadIdx.x;
+  if (e >= B.rows * B.cols) return;
+  const int v_ = blockIdx.y;
+  const int x = e / B.cols, y = e - x * B.cols;
+  double v = psi[(int64_t)v_ * d.ld_psi + B.off + e];
+  if (nrm2) { v *= 1.0 / sqrt(nrm2[v_]); normalized[(int64_t)v_ * d.ld_psi + B.off + e] = v; }
+  d.ws[B.p_off + v_ * B.p_vstride + (int64_t)x * B.ldp + y] = v;
+  d.ws[B.t_off + v_ * B.t_vstride + (int64_t)y * B.ldt + x] = v;
 }
 
 // reduce: out block = sum of its split-K partials in a fixed order -> bitwise reproducible; a block nobody writes
@@ -273,22 +286,26 @@ __global__ void prep_kernel(DevSchedule d, const double* __restrict__ psi) {
 // splits [q * per, (q + 1) * per) in order (eight loads in flight), then the eight sums are added in lane order.  (One
 // thread per element walked up to ~80 dependent L2 round trips: 0.079 -> 0.040 ms of a 0.59 ms apply at D = 1024.)
 // Large vectors are bandwidth-bound and lose with eight rows in flight per warp (cyp 0.115 -> 0.207 ms): they take
-// reduce_plain_kernel below; the launcher picks by size.
+// reduce_plain_kernel below; the launcher picks by size.  Partials: split-major, vector-minor.
 constexpr int RED_LANES = 8;
 __global__ void reduce_kernel(DevSchedule d, double* __restrict__ out, int accumulate) {
-  const PsiBlk B = d.blocks[blockIdx.y];
+  const ElemCta c = d.elem[blockIdx.x];
+  const PsiBlk B = d.blocks[c.blk];
   const int n = B.rows * B.cols;
-  const int64_t stride = (int64_t)B.rows * B.ldo;
+  const int64_t stride = (int64_t)d.nvec * B.rows * B.ldo;
+  out += (int64_t)blockIdx.y * d.ld_out;
+  const double* part = d.ws + B.part_off + (int64_t)blockIdx.y * B.rows * B.ldo;
   const int q = threadIdx.x & (RED_LANES - 1);
   const int per = (B.nsplit + RED_LANES - 1) / RED_LANES;
   const int sp0 = min(q * per, B.nsplit), sp1 = min(sp0 + per, B.nsplit);
-  const int epb = blockDim.x / RED_LANES;                      // elements per block and pass
-  const int n_pad = (n + epb - 1) / epb * epb;                 // whole warps stay in the loop for the shuffles
-  for (int e = blockIdx.x * epb + (threadIdx.x / RED_LANES); e < n_pad; e += gridDim.x * epb) {
+  constexpr int EPP = 256 / RED_LANES;                         // elements per pass
+#pragma unroll 1
+  for (int pass = 0; pass < RED_LANES; ++pass) {               // whole warps stay in the loop for the shuffles
+    const int e = c.e0 + pass * EPP + (threadIdx.x / RED_LANES);
     double s = 0.0;
     if (e < n) {
       const int x = e / B.cols, y = e - x * B.cols;
-      const double* p = d.ws + B.part_off + (int64_t)x * B.ldo + y;
+      const double* p = part + (int64_t)x * B.ldo + y;
       int sp = sp0;
       for (; sp + 8 <= sp1; sp += 8) {
         double v[8];
@@ -309,39 +326,40 @@ __global__ void reduce_kernel(DevSchedule d, double* __restrict__ out, int accum
 
 // the plain form: one thread per element, rows fully coalesced (large vectors; bandwidth-bound)
 __global__ void reduce_plain_kernel(DevSchedule d, double* __restrict__ out, int accumulate) {
-  const PsiBlk B = d.blocks[blockIdx.y];
-  const int n = B.rows * B.cols;
-  const int64_t stride = (int64_t)B.rows * B.ldo;
-  for (int e = blockIdx.x * blockDim.x + threadIdx.x; e < n; e += gridDim.x * blockDim.x) {
-    const int x = e / B.cols, y = e - x * B.cols;
-    const double* p = d.ws + B.part_off + (int64_t)x * B.ldo + y;
-    double s = accumulate ? out[B.off + e] : 0.0;           // hpsi_stream_apply: windows of terms add up in a fixed order
-    int sp = 0;
-    for (; sp + 8 <= B.nsplit; sp += 8) {                   // eight partials in flight, added in split order
-      double v[8];
+  const ElemCta c = d.elem[blockIdx.x];
+  const PsiBlk B = d.blocks[c.blk];
+  const int e = c.e0 + threadIdx.x;
+  if (e >= B.rows * B.cols) return;
+  const int64_t stride = (int64_t)d.nvec * B.rows * B.ldo;
+  out += (int64_t)blockIdx.y * d.ld_out;
+  const int x = e / B.cols, y = e - x * B.cols;
+  const double* p = d.ws + B.part_off + (int64_t)blockIdx.y * B.rows * B.ldo + (int64_t)x * B.ldo + y;
+  double s = accumulate ? out[B.off + e] : 0.0;             // hpsi_stream_apply: windows of terms add up in a fixed order
+  int sp = 0;
+  for (; sp + 8 <= B.nsplit; sp += 8) {                     // eight partials in flight, added in split order
+    double v[8];
 #pragma unroll
-      for (int i = 0; i < 8; ++i) v[i] = __ldg(p + (sp + i) * stride);
+    for (int i = 0; i < 8; ++i) v[i] = __ldg(p + (sp + i) * stride);
 #pragma unroll
-      for (int i = 0; i < 8; ++i) s += v[i];
-    }
-    for (; sp < B.nsplit; ++sp) s += __ldg(p + sp * stride);
-    out[B.off + e] = s;
+    for (int i = 0; i < 8; ++i) s += v[i];
   }
+  for (; sp < B.nsplit; ++sp) s += __ldg(p + sp * stride);
+  out[B.off + e] = s;
 }
 
 // diag(H): diag[l][x,y] = sum over sector-diagonal tasks of c_t A[x,x] B[y,y]   (reading A21)
 __global__ void diag_kernel(DevSchedule d, double* __restrict__ diag) {
-  const PsiBlk B = d.blocks[blockIdx.y];
-  const int n = B.rows * B.cols;
-  for (int e = blockIdx.x * blockDim.x + threadIdx.x; e < n; e += gridDim.x * blockDim.x) {
-    const int x = e / B.cols, y = e - x * B.cols;
-    double s = 0.0;
-    for (int i = B.diag0; i < B.diag1; ++i) {
-      const DiagTask t = d.diag[i];
-      s += t.coef * d.a[t.a_off + (int64_t)x * t.a_ld + x] * d.b[t.b_off + (int64_t)y * t.b_ld + y];
-    }
-    diag[B.off + e] = s;
+  const ElemCta c = d.elem[blockIdx.x];
+  const PsiBlk B = d.blocks[c.blk];
+  const int e = c.e0 + threadIdx.x;
+  if (e >= B.rows * B.cols) return;
+  const int x = e / B.cols, y = e - x * B.cols;
+  double s = 0.0;
+  for (int i = B.diag0; i < B.diag1; ++i) {
+    const DiagTask t = d.diag[i];
+    s += t.coef * d.a[t.a_off + (int64_t)x * t.a_ld + x] * d.b[t.b_off + (int64_t)y * t.b_ld + y];
   }
+  diag[B.off + e] = s;
 }
 
 // out[e] = parts[0][e] + parts[1][e] + ... in that order (term-sharded apply: the ranks' partial H psi, gathered, are added
@@ -372,15 +390,8 @@ cudaError_t kernels_init() {
   return kernels_paired_init();
 }
 
-static dim3 elem_grid(const DevSchedule& d) {
-  int gx = (d.max_block_elems + 255) / 256;
-  if (gx < 1) gx = 1;
-  if (gx > 1024) gx = 1024;
-  return dim3(gx, d.n_blocks);
-}
-
-void launch_prep(const DevSchedule& d, const double* psi, cudaStream_t st) {
-  if (d.n_blocks > 0) prep_kernel<<<elem_grid(d), 256, 0, st>>>(d, psi);
+void launch_prep(const DevSchedule& d, const double* psi, const double* nrm2, double* normalized, cudaStream_t st) {
+  if (d.n_elem > 0) prep_kernel<<<dim3(d.n_elem, d.nvec_active), 256, 0, st>>>(d, psi, nrm2, normalized);
 }
 void launch_p1(const DevSchedule& d, bool tma, cudaStream_t st) {
   if (d.n_p1 == 0) return;
@@ -400,16 +411,13 @@ void launch_p2(const DevSchedule& d, bool tma, cudaStream_t st) {
   else p2_kernel<false><<<d.n_p2, NTHREADS, SMEM_BYTES, st>>>(d);
 }
 void launch_reduce(const DevSchedule& d, double* out, bool accumulate, cudaStream_t st) {
-  if (d.n_blocks == 0) return;
-  const bool small_vec = (int64_t)d.max_block_elems * d.n_blocks <= 400000;     // latency-bound sizes (D <~ 1500)
-  const int lanes = small_vec ? 8 : 1;
-  int gx = (d.max_block_elems + 256 / lanes - 1) / (256 / lanes);
-  gx = std::max(1, std::min(gx, 1024));
-  if (small_vec) reduce_kernel<<<dim3(gx, d.n_blocks), 256, 0, st>>>(d, out, accumulate ? 1 : 0);
-  else reduce_plain_kernel<<<dim3(gx, d.n_blocks), 256, 0, st>>>(d, out, accumulate ? 1 : 0);
+  if (d.n_elem == 0) return;
+  const bool small_vec = (int64_t)d.n_elem * 256 <= 500000;     // latency-bound sizes (D <~ 1500)
+  if (small_vec) reduce_kernel<<<dim3(d.n_elem, d.nvec_active), 256, 0, st>>>(d, out, accumulate ? 1 : 0);
+  else reduce_plain_kernel<<<dim3(d.n_elem, d.nvec_active), 256, 0, st>>>(d, out, accumulate ? 1 : 0);
 }
 void launch_diag(const DevSchedule& d, double* diag, cudaStream_t st) {
-  if (d.n_blocks > 0) diag_kernel<<<elem_grid(d), 256, 0, st>>>(d, diag);
+  if (d.n_elem > 0) diag_kernel<<<d.n_elem, 256, 0, st>>>(d, diag);
 }
 
 }  // namespace hpsi

@@ -30,6 +30,8 @@ struct DevSchedule {           // device pointers to the uploaded tables
   const P2Unit* p2;
   const P2Unit* pf;            // fused units (kernels_fused.cu)
   const DiagTask* diag;
+  const ElemCta* elem;         // granules of the element-wise kernels
+  int n_elem;
   const unsigned char* maps;   // CUtensorMap[sc.maps.size()], 128 bytes each (TMA staging only)
   double* ws;
   const double* a;
@@ -37,10 +39,13 @@ struct DevSchedule {           // device pointers to the uploaded tables
   int n_blocks, n_p1, n_p2, n_pf;
   int max_block_elems;
   int paired;                  // the plan has blocks stored transposed: kernels_paired.cu runs the GEMMs
+  int nvec;                    // vectors the plan was laid out for (batched plans: hpsi_plan_options_t.n_vectors)
+  int nvec_active;             // vectors of THIS apply (<= nvec): units of the others return at once
+  int64_t ld_psi, ld_out;      // doubles between consecutive vectors of psi / out (hpsi_apply_multi)
   double* rot_dst;             // operator-update launches (rotate.cu) only: base the transposed tile stores go to
 };
 
-void launch_prep(const DevSchedule& d, const double* psi, cudaStream_t st);
+void launch_prep(const DevSchedule& d, const double* psi, const double* nrm2, double* normalized, cudaStream_t st);   // nrm2 != null: psi / sqrt(*nrm2), also written to `normalized`
 void launch_p1(const DevSchedule& d, bool tma, cudaStream_t st);
 void launch_p1_rot(const DevSchedule& d, bool tma, cudaStream_t st);   // same kernel, tile stored transposed at Seg.p2_off / p2_ld
 void launch_p2(const DevSchedule& d, bool tma, cudaStream_t st);

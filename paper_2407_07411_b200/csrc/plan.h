@@ -52,7 +52,8 @@ struct Group {
   int32_t ws_map;             // tensor map of the stacked intermediate
   int32_t src, dst;           // psi block indices
   int32_t fused;              // 1: narrow group, both GEMMs run in one CTA (kernels_fused.cu): no P1 unit, no workspace intermediate
-  int32_t pad;
+  int32_t N1p;                // batched plans (nvec > 1): columns one vector occupies in the intermediate (N1 rounded up to 16,
+                              // pad columns stay zero), vector v at column v * N1p; single-vector plans: N1
 };
 
 struct P1Unit {               // one CTA of the first-GEMM kernel: one tile position, a range of the group's terms
@@ -62,7 +63,7 @@ struct P1Unit {               // one CTA of the first-GEMM kernel: one tile posi
   int32_t j0, cols_valid;     // column tile
   int32_t grid;               // warp columns gn
   int32_t xtrans;             // 1: the operator blocks of these terms are stored transposed (K-major X operand)
-  int32_t pad;
+  int32_t vec;                // batched plans: which of the nvec vectors this unit works on
 };
 
 struct Run {                  // consecutive segs of one group inside one P2 unit's K range
@@ -77,7 +78,7 @@ struct Run {                  // consecutive segs of one group inside one P2 uni
   int32_t trans;              // 1: the operator blocks of these segs are stored transposed (K-major operand)
   int32_t K1;                 // fused runs only: contraction length of the first GEMM (group.K1)
   int32_t y1_map, ldy1;       // fused runs only: the first GEMM's shared operand (padded psi^T / psi block), group.y1_map / ldy1
-  int32_t pad;
+  int32_t Kp;                 // group.N1p: column stride between the vectors of a batched intermediate
   int64_t y1_off;             // fused runs only: group.y1_off
 };
 
@@ -87,6 +88,8 @@ struct P2Unit {               // one CTA of the second-GEMM kernel
   int64_t out_off;            // partial buffer offset of element (i0, j0) of this split's m x ldp tile
   int32_t ldo;
   int32_t grid;               // warp columns gn
+  int32_t vec;                // batched plans: which of the nvec vectors this unit works on
+  int32_t pad;
 };
 
 // A 2-D row-major matrix the TMA unit reads: rows x cols doubles as STORED, leading dimension ld, `off` doubles into
@@ -105,11 +108,16 @@ struct PsiBlk {               // one psi block and its padded copies
   int64_t p_off;              // padded copy   rows x ldp   in workspace
   int64_t t_off;              // padded transpose cols x ldt in workspace
   int32_t rows, cols, ldp, ldt;
-  int64_t part_off;           // split-K partials: nsplit x (rows x ldo)
+  int64_t part_off;           // split-K partials: nsplit x nvec x (rows x ldo), vector fastest
+  int64_t p_vstride, t_vstride;   // batched plans: doubles between the padded copies (transposes) of consecutive vectors
   int32_t nsplit, ldo;
   int32_t left, right;
   int32_t diag0, diag1;       // range in the diagonal-task table
   int32_t p_map, t_map;       // tensor maps of the padded copy / padded transpose
+};
+
+struct ElemCta {              // one CTA of the element-wise kernels (prep, reduce, diag): 256 consecutive elements of one psi block
+  int32_t blk, e0;
 };
 
 struct DiagTask {             // sector-diagonal task (for diag(H))
@@ -129,6 +137,7 @@ struct Schedule {
   std::vector<P2Unit> p2;
   std::vector<P2Unit> pf;             // units of the fused kernel (same descriptor; their runs are fused runs)
   std::vector<DiagTask> diag;
+  std::vector<ElemCta> elem;          // psi elements in granules of 256 per block: no CTA of an element-wise launch is idle
   std::vector<MapSpec> maps;          // tensor maps the TMA kernels use (only filled / valid when aligned16)
   std::vector<hpsi_task_t> tasks;     // schedule order, for hpsi_query
   int64_t psi_len = 0;
@@ -141,6 +150,7 @@ struct Schedule {
   bool paired = false;                // some block is stored transposed: fragments are taken from 16-row groups (kernels.cu)
   int64_t tuning[3] = {0, 0, 0};      // realised schedule knobs: P1 K-tiles per unit, P2 waves, P2 minimum DMMA per unit
   int32_t n_terms_planned = 0;        // terms of this plan's shard (all terms without a shard)
+  int32_t nvec = 1;                   // vectors one hpsi_apply_multi works on (hpsi_plan_options_t.n_vectors)
 };
 
 // What hpsi_plan_ex adds to hpsi_plan (include/hpsi.h hpsi_plan_options_t): a term shard and the schedule knobs.
@@ -150,6 +160,7 @@ struct PlanOptions {
   int32_t p1_stages_per_unit = 0;           // 0 = automatic
   int32_t p2_waves = 0;
   int32_t p2_min_unit_dmma = 0;
+  int32_t n_vectors = 0;                    // 0 / 1: single-vector plan
 };
 
 // Host planner.  Returns HPSI_OK or an error code with `err` filled.
@@ -165,7 +176,7 @@ std::vector<Tile1D> split_rows(int64_t n);
 std::vector<Tile1D> split_cols(int64_t n);
 
 // Host interpreter of the schedule (tests only; naive loops).
-void interpret_schedule(const Schedule& sc, const double* a, const double* b, const double* psi, double* out);
+void interpret_schedule(const Schedule& sc, const double* a, const double* b, const double* psi, double* out, int nvec = 1);   // vectors psi_len apart
 
 inline int even_up(int x) { return x + (x & 1); }
 // Plan-owned matrices (padded psi, intermediates, partials) start every row on a 32-byte L2 sector, so that a staged

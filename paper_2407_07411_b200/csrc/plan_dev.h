@@ -26,6 +26,8 @@ struct hpsi_plan {
   size_t dav_doubles = 0;
   int dav_mmax = 0;
   double* h_dav = nullptr;        // pinned host scalars the Davidson loop reads back each iteration
+  cudaStream_t dav_side = nullptr;   // side stream + events: the read-back of an iteration's residual overlaps its
+  cudaEvent_t dav_ev[2] = {nullptr, nullptr};   // orthogonalisation kernels (davidson.cu)
   // hpsi_truncate (svd.cu)
   int n_left = 0, n_right = 0;    // sectors of the sector table (length of chi_host for either side)
   void* d_svd = nullptr;          // working matrices, singular values, tables (allocated on first use)
@@ -36,7 +38,9 @@ struct hpsi_plan {
 namespace hpsi {
 void set_error(const std::string& s);
 int cuda_fail(cudaError_t e, const char* what);   // records the message, returns HPSI_ECUDA
-int apply_impl(hpsi_plan_t* p, const double* psi_dev, double* out_dev, bool accumulate, void* cuda_stream);
+int apply_impl(hpsi_plan_t* p, const double* psi_dev, double* out_dev, bool accumulate, void* cuda_stream,
+               const double* nrm2_dev = nullptr, double* normalized_dev = nullptr,   // out = H (psi / sqrt(nrm2[v])), see prep_kernel
+               int n_vectors = 1, int64_t ld_psi = 0, int64_t ld_out = 0);             // batched plans: vectors ld_* doubles apart
 // api.cu: shared with rotate.cu, whose object wraps an hpsi_plan
 int upload_schedule(hpsi_plan_t* p);   // device copies of the schedule tables, workspace, tensor-map buffer
 int encode_maps(hpsi_plan_t* p);       // CUtensorMap of every MapSpec against dev.a / dev.b / d_ws

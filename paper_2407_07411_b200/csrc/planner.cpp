@@ -128,6 +128,10 @@ int build_schedule(const hpsi_sectors_t* s, const hpsi_terms_t* t, uint32_t flag
   if ((flags & HPSI_PLAN_FIXED_ORDER1) && (flags & HPSI_PLAN_FIXED_ORDER2))
     FAIL(HPSI_EINVAL, "both fixed-order flags set");
   if (opt.p1_stages_per_unit < 0 || opt.p2_waves < 0 || opt.p2_min_unit_dmma < 0) FAIL(HPSI_EINVAL, "negative schedule knob");
+  if (opt.n_vectors < 0 || opt.n_vectors > 64) FAIL(HPSI_EINVAL, "n_vectors outside 0..64");
+  const int nvec = std::max(1, opt.n_vectors);
+  sc->nvec = nvec;
+  if (nvec > 1 && (flags & HPSI_PLAN_FUSE_ALL)) FAIL(HPSI_EINVAL, "batched plans (n_vectors > 1) do not run the fused kernel");
   // term shard: only the terms with shard_of_term[t] == shard_index are planned; the blocks of every
   // other term are ignored altogether (their descriptors are not validated: the caller's arenas need not hold them)
   auto in_shard = [&](int32_t term) { return !opt.shard_of_term || opt.shard_of_term[term] == opt.shard_index; };
@@ -173,6 +177,9 @@ int build_schedule(const hpsi_sectors_t* s, const hpsi_terms_t* t, uint32_t flag
   }
   sc->psi_len = off;
   const int nB = (int)sc->blocks.size();
+  sc->elem.clear();
+  for (int b = 0; b < nB; ++b)
+    for (int e0 = 0; e0 < sc->blocks[b].rows * sc->blocks[b].cols; e0 += 256) sc->elem.push_back({b, e0});
 
   // ---- validation of block descriptors
   sc->aligned16 = true;
@@ -206,6 +213,7 @@ int build_schedule(const hpsi_sectors_t* s, const hpsi_terms_t* t, uint32_t flag
   if (t->a_transposed) for (int64_t i = 0; i < t->n_a; ++i) if (t->a_transposed[i] && in_shard(t->a_blocks[i].term)) sc->paired = true;
   if (t->b_transposed) for (int64_t i = 0; i < t->n_b; ++i) if (t->b_transposed[i] && in_shard(t->b_blocks[i].term)) sc->paired = true;
   const bool paired = sc->paired;
+  if (nvec > 1 && paired) FAIL(HPSI_EINVAL, "batched plans (n_vectors > 1) do not support blocks stored transposed");
 
   // ---- step 2: task enumeration
   std::unordered_map<uint64_t, int64_t> b_index;
@@ -239,13 +247,15 @@ int build_schedule(const hpsi_sectors_t* s, const hpsi_terms_t* t, uint32_t flag
 
   // ---- workspace layout part 1: padded psi and psi^T
   int64_t ws = 0;
-  for (auto& b : sc->blocks) {
+  for (auto& b : sc->blocks) {                  // batched plans: the nvec copies one under the other, no padding rows
     b.p_off = ws;
-    ws = align_up(ws + (int64_t)b.rows * b.ldp, 16);
+    b.p_vstride = (int64_t)b.rows * b.ldp;
+    ws = align_up(ws + nvec * b.p_vstride, 16);
   }
   for (auto& b : sc->blocks) {
     b.t_off = ws;
-    ws = align_up(ws + (int64_t)b.cols * b.ldt, 16);
+    b.t_vstride = (int64_t)b.cols * b.ldt;
+    ws = align_up(ws + nvec * b.t_vstride, 16);
     sc->max_block_elems = std::max<int32_t>(sc->max_block_elems, b.rows * b.cols);
   }
   sc->maps.clear();
@@ -260,8 +270,8 @@ int build_schedule(const hpsi_sectors_t* s, const hpsi_terms_t* t, uint32_t flag
     return (int32_t)sc->maps.size() - 1;
   };
   for (auto& b : sc->blocks) {
-    b.p_map = add_map(BASE_WS, b.p_off, b.rows, b.cols, b.ldp);
-    b.t_map = add_map(BASE_WS, b.t_off, b.cols, b.rows, b.ldt);
+    b.p_map = add_map(BASE_WS, b.p_off, nvec * b.rows, b.cols, b.ldp);
+    b.t_map = add_map(BASE_WS, b.t_off, nvec * b.cols, b.rows, b.ldt);
   }
 
   // The fused kernel is OFF by default: measured on B200 it loses to the two launches even where every task fits it
@@ -292,7 +302,11 @@ int build_schedule(const hpsi_sectors_t* s, const hpsi_terms_t* t, uint32_t flag
     g.dst = raw[i].dst;
     if (order == 1) { g.rows = (int32_t)m; g.K1 = (int32_t)k; g.N1 = (int32_t)np; g.ldy1 = S.ldt; g.y1_off = S.t_off; g.y1_map = S.t_map; }
     else            { g.rows = (int32_t)n; g.K1 = (int32_t)np; g.N1 = (int32_t)k; g.ldy1 = S.ldp; g.y1_off = S.p_off; g.y1_map = S.p_map; }
-    g.ldw = sector_up(g.N1);
+    // Batched plans: the first GEMM's results of the nvec vectors sit side by side in one row, vector v in columns
+    // [v N1p, v N1p + N1); N1p is a multiple of the K-tile and the pad columns are never written (the workspace is zeroed
+    // at plan time), so a K-tile of the second GEMM never reaches into the next vector.
+    g.N1p = nvec > 1 ? (int32_t)align_up(g.N1, KT) : g.N1;
+    g.ldw = nvec > 1 ? nvec * g.N1p : sector_up(g.N1);
     // Narrow groups run both GEMMs in one CTA (kernels_fused.cu; north_star: "the intermediate block kept in shared
     // memory or registers between the two GEMMs"): the whole intermediate of a tile fits one operand buffer (N1 <= 64)
     // and the output dimension that would otherwise recompute it is a single tile (order 1: n <= 64, order 2: m <= 64).
@@ -303,7 +317,7 @@ int build_schedule(const hpsi_sectors_t* s, const hpsi_terms_t* t, uint32_t flag
     }
     g.ws_off = ws;
     const int64_t per_task = g.fused ? 0 : (int64_t)g.rows * g.ldw;
-    g.ws_map = g.fused ? -1 : add_map(BASE_WS, ws, (int)((int64_t)g.rows * (j - i)), g.N1, g.ldw);
+    g.ws_map = g.fused ? -1 : add_map(BASE_WS, ws, (int)((int64_t)g.rows * (j - i)), nvec > 1 ? g.ldw : g.N1, g.ldw);
     for (size_t q = i; q < j; ++q) {
       const hpsi_opblock_t& a = t->a_blocks[raw[q].ia];
       const hpsi_opblock_t& b = t->b_blocks[raw[q].ib];
@@ -353,7 +367,7 @@ int build_schedule(const hpsi_sectors_t* s, const hpsi_terms_t* t, uint32_t flag
     // ~96 K-tiles per unit, fewer when the whole launch would otherwise be only a few waves of CTAs (small problems)
     int64_t total_stages = 0;
     for (const Group& g : sc->groups)
-      if (!g.fused) total_stages += (int64_t)split_rows(g.rows).size() * split_cols(g.N1).size() * g.tcount * ((g.K1 + KT - 1) / KT);
+      if (!g.fused) total_stages += (int64_t)nvec * split_rows(g.rows).size() * split_cols(g.N1).size() * g.tcount * ((g.K1 + KT - 1) / KT);
     const int auto_stages = (int)std::max<int64_t>(12, std::min<int64_t>(96, total_stages / ((int64_t)std::max(n_sm, 1) * 3 * 8)));
     const int P1_STAGES_PER_UNIT = opt.p1_stages_per_unit > 0 ? opt.p1_stages_per_unit : auto_stages;
     sc->tuning[0] = P1_STAGES_PER_UNIT;
@@ -389,8 +403,9 @@ int build_schedule(const hpsi_sectors_t* s, const hpsi_terms_t* t, uint32_t flag
               const int fm = tile_frags(r.len, paired), fn = tile_frags(c.len, paired);
               int heavy = 0;
               const int32_t grid = best_grid(fm, fn, &heavy, paired);
-              sc->p1.push_back({go.gi, t0, t1, r.start, r.len, c.start, c.len, grid, part, 0});
-              sc->issued_flops_p1 += (int64_t)fm * fn * ks * 512 * (t1 - t0);
+              for (int v = 0; v < nvec; ++v)            // the vectors of a tile are adjacent: they read the same operator rows
+                sc->p1.push_back({go.gi, t0, t1, r.start, r.len, c.start, c.len, grid, part, v});
+              sc->issued_flops_p1 += (int64_t)fm * fn * ks * 512 * (t1 - t0);        // flop counts are per vector
               sc->critical_flops += (int64_t)NCONS_WARPS * heavy * ks * 512 * (t1 - t0);
             }
         }
@@ -449,7 +464,7 @@ int build_schedule(const hpsi_sectors_t* s, const hpsi_terms_t* t, uint32_t flag
   // (block, K-chunk) bundle L2-resident while its tiles pass over them.  Measured A/B/A/B on B200, 32 -> 48 waves:
   // cyp 31.6 -> 32.0 TFLOPS, stress 32.2 -> 32.5, femoco 31.7 -> 32.0, small unchanged (p2 -2 %, reduce +0.035 ms);
   // 64 waves gain nothing more (the ordered reduce grows as fast as p2 shrinks).
-  const int64_t slots = (int64_t)std::max(n_sm, 1) * 4 * waves;
+  const int64_t slots = std::max<int64_t>(1, (int64_t)std::max(n_sm, 1) * 4 * waves / nvec);   // every unit exists once per vector
   const int64_t min_target = opt.p2_min_unit_dmma > 0 ? opt.p2_min_unit_dmma : 1536;   // DMMA per unit at least (~10 us of a CTA)
   sc->tuning[1] = waves;
   sc->tuning[2] = min_target;
@@ -495,7 +510,7 @@ int build_schedule(const hpsi_sectors_t* s, const hpsi_terms_t* t, uint32_t flag
             // a run has one storage layout of its operator blocks: split [ti, ti + take) at the group's layout boundary
             int tbnd = ti;
             while (tbnd < ti + take && !sc->segs[g.seg0 + tbnd].p2_trans) ++tbnd;
-            Run r{g.seg0 + ti, g.seg0 + tbnd, g.N1, g.ldw, g.order, g.rows, g.seg0, g.ws_map, g.ws_off, 0, 0, 0, 0, 0, 0};
+            Run r{g.seg0 + ti, g.seg0 + tbnd, g.N1, g.ldw, g.order, g.rows, g.seg0, g.ws_map, g.ws_off, 0, 0, 0, 0, g.N1p, 0};
             if (g.fused) { r.K1 = g.K1; r.y1_map = g.y1_map; r.ldy1 = g.ldy1; r.y1_off = g.y1_off; }
             if (tbnd > ti) sc->runs.push_back(r);
             if (tbnd < ti + take) {
@@ -519,8 +534,12 @@ int build_schedule(const hpsi_sectors_t* s, const hpsi_terms_t* t, uint32_t flag
             u.ldo = D.ldo;
             const int fm = tile_frags(r.len, paired), fn = tile_frags(c.len, paired);
             u.grid = pass ? 2 : best_grid(fm, fn, nullptr, paired);       // fused CTAs: 2x2 warps, <= 4x4 fragments each
-            u.out_off = ws + (int64_t)realised * D.rows * D.ldo + (int64_t)r.start * D.ldo + c.start;
-            units.push_back(u);
+            for (int v = 0; v < nvec; ++v) {              // the vectors of a tile are adjacent: they read the same operator tile
+              u.vec = v;
+              u.out_off = ws + ((int64_t)realised * nvec + v) * D.rows * D.ldo + (int64_t)r.start * D.ldo + c.start;
+              units.push_back(u);
+              unit_bundle[pass].push_back((int)bundle_cost[pass].size());
+            }
             int64_t dmma = (int64_t)fm * fn * chunk_ksteps;
             int64_t cost = 0;                         // this tile's cost over the chunk's runs, stage floor included
             for (int ri = run0; ri < run1; ++ri) {
@@ -539,7 +558,6 @@ int build_schedule(const hpsi_sectors_t* s, const hpsi_terms_t* t, uint32_t flag
             int heavy = 0;
             best_grid(fm, fn, &heavy, paired);
             sc->critical_flops += (int64_t)NCONS_WARPS * heavy * chunk_ksteps * 512;
-            unit_bundle[pass].push_back((int)bundle_cost[pass].size());
             bundle_max = std::max(bundle_max, cost);
             issued_p2 += dmma * 512;
           }
@@ -548,7 +566,7 @@ int build_schedule(const hpsi_sectors_t* s, const hpsi_terms_t* t, uint32_t flag
       }
     }
     D.nsplit = realised;
-    ws = align_up(ws + (int64_t)realised * D.rows * D.ldo, 16);
+    ws = align_up(ws + (int64_t)realised * nvec * D.rows * D.ldo, 16);
   }
   // LPT order over (block, split) bundles: the tiles of one bundle read the same operand segments, so they stay
   // adjacent in launch order (co-resident CTAs -> the second reader hits L2); bundles go heaviest tile first.

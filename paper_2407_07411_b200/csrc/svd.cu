@@ -9,14 +9,16 @@
 // decay linearly, sweep after sweep: measured 22 sweeps instead of 12 on the cyp blocks), so there the vectors are the COLUMNS: the working
 // matrix is psi_l^T alone, its converged rows are sigma_j u_j^T and the isometry rows are those rows divided by sigma_j.
 //
-// Parallel order (block Jacobi by tournament): the rows of a block are cut into chunks of `bsz` rows; in one kernel
-// launch ("round") every CTA owns one PAIR of chunks of one block, chosen by the round-robin (circle) schedule so that
-// all CTAs of a round touch disjoint rows; it loads its 2*bsz rows into shared memory, orthogonalises them pairwise - one
-// warp per row pair, again by a round-robin schedule, CTA barrier between its inner rounds - and writes them back.  The
-// first round of a block's sweep does all pairs inside the two chunks, the others only the cross pairs, so a sweep
-// visits every row pair of the block exactly once.  Sweeps repeat until one makes no rotation (device counter of rotations; the
-// only atomic, not on data).  Every psi block is processed in the same launches.  All arithmetic is FP64 FMA; the result is
-// bitwise reproducible.
+// Parallel order (block Jacobi by tournament): the rows of a block are cut into chunks of 16 rows; in one kernel launch
+// ("round") every CTA owns one PAIR of chunks of one block, chosen by the round-robin (circle) schedule so that all CTAs
+// of a round touch disjoint rows.  A visit does not rotate the 32 rows themselves pair by pair (that streams two rows
+// through shared memory three times per pair - the first version of this kernel was bound by shared-memory bandwidth):
+// it forms their 32 x 32 Gram matrix G on the tensor pipe, runs the visit's plane rotations on G (both sides) while
+// accumulating their product Q, and applies Q to the rows once, again on the tensor pipe (svd_round_kernel).  The pairs,
+// their order, the rotation formula and the threshold are those of the row-by-row method: the first round of a block's
+// sweep does all pairs inside the two chunks, the others only the cross pairs, so a sweep visits every row pair of the
+// block exactly once.  Sweeps repeat until one makes no rotation (device counter of rotations; the only atomic, not on
+// data).  Every psi block is processed in the same launches.  FP64 throughout; the result is bitwise reproducible.
 #include <algorithm>
 #include <cmath>
 #include <cstdio>
@@ -41,9 +43,6 @@ struct SvdBlk {
   int32_t row0;         // first row in the concatenated singular-value array
   double floor2;        // rows with squared norm <= floor2 count as zero (1e-27 x the block's squared Frobenius norm)
 };
-
-constexpr int SVD_MAX_BSZ = 16;
-constexpr int SVD_SMEM_BUDGET = 200 * 1024;
 
 // working matrix <- [psi block | identity]; floor2 of the block from its Frobenius norm (one CTA per block row range)
 __global__ void svd_init_kernel(SvdBlk* blk, const double* __restrict__ psi, double* __restrict__ w) {
@@ -80,10 +79,35 @@ __device__ __forceinline__ double warp_sum(double v) {
   return v;
 }
 
-// One round: CTA = (block, chunk pair of the round-robin schedule).  blockDim.x = 32 * bsz.
-__global__ void svd_round_kernel(const SvdBlk* __restrict__ blk, const int32_t* __restrict__ cta_blk, int round, int bsz,
-                                 double* __restrict__ w, int* __restrict__ flag) {
-  extern __shared__ __align__(16) double srow[];
+constexpr int SV_B = 16;             // rows per chunk
+constexpr int SV_M = 2 * SV_B;       // rows one CTA orthogonalises per visit (a chunk pair)
+constexpr int SV_KC = 32;            // columns of the psi part staged per Gram step
+constexpr int SV_THREADS = 256;
+
+__device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double b) {
+  asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
+               : "+d"(c0), "+d"(c1)
+               : "d"(a), "d"(b));
+}
+
+struct SvdSmem {
+  double G[SV_M][SV_M + 1];          // Gram matrix of the psi parts of the 32 rows, rotated two-sidedly
+  double Q[SV_M][SV_M + 1];          // product of the visit's rotations: the rows become Q X
+  double stage[2][SV_M][SV_KC + 4];  // psi part, one K-chunk of all 32 rows (double buffered)
+  double cs[SV_B][2];                // rotations of the current step
+};
+
+// One round: CTA = (block, chunk pair of the round-robin schedule).  Block Jacobi on the tensor pipe:
+//   1. G = X_psi X_psi^T for the 32 rows of the chunk pair (DMMA, the rows streamed once through shared memory);
+//   2. one cyclic pass of plane rotations over the row pairs of the visit, applied to G from both sides (32-long vectors
+//      in shared memory instead of the rows themselves) and accumulated in Q - same pairs, same order, same rotation
+//      formula and threshold as rotating the rows one pair at a time;
+//   3. X <- Q X over all L columns (DMMA, every element read and written once).
+// Shared-memory traffic per visit drops from ~93 passes over the 32 rows (31 inner rounds x 3) to 2 passes through
+// global memory / L2; measured on cyp: 9.7 ms -> see DESIGN.md section 9.
+__global__ void __launch_bounds__(SV_THREADS) svd_round_kernel(const SvdBlk* __restrict__ blk, const int32_t* __restrict__ cta_blk,
+                                                               int round, double* __restrict__ w, int* __restrict__ flag) {
+  __shared__ SvdSmem sm;
   const SvdBlk B = blk[cta_blk[blockIdx.x]];
   const int k = blockIdx.x - B.cta0;
   const int n1 = B.nce - 1;
@@ -93,82 +117,150 @@ __global__ void svd_round_kernel(const SvdBlk* __restrict__ blk, const int32_t* 
   else { ci = (rr + k) % n1; cj = (rr - k + n1) % n1; }
   if (ci > cj) { const int t = ci; ci = cj; cj = t; }
   const bool full = (rr == 0);                           // first round of the block's sweep: pairs inside the chunks too
-  const int ni = max(0, min(bsz, B.nv - ci * bsz)), nj = max(0, min(bsz, B.nv - cj * bsz));
+  const int ni = max(0, min(SV_B, B.nv - ci * SV_B)), nj = max(0, min(SV_B, B.nv - cj * SV_B));
   if (ni + nj < 2 || (!full && (ni == 0 || nj == 0))) return;
   const int L = B.L, tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
-  // slot s < bsz holds row ci*bsz + s, slot bsz + s holds row cj*bsz + s
+  const int g = lane >> 2, q = lane & 3;
+  // slot s < 16 holds row ci*16 + s, slot 16 + s holds row cj*16 + s
+  auto valid = [&](int slot) { return slot < SV_B ? slot < ni : slot - SV_B < nj; };
   auto grow = [&](int slot) -> double* {
-    const int row = slot < bsz ? ci * bsz + slot : cj * bsz + (slot - bsz);
+    const int row = slot < SV_B ? ci * SV_B + slot : cj * SV_B + (slot - SV_B);
     return w + B.w_off + (int64_t)row * L;
   };
-  auto valid = [&](int slot) { return slot < bsz ? slot < ni : slot - bsz < nj; };
-  for (int slot = wid; slot < 2 * bsz; slot += bsz) {
-    if (!valid(slot)) continue;
-    const double2* src = reinterpret_cast<const double2*>(grow(slot));
-    double2* dst = reinterpret_cast<double2*>(srow + (size_t)slot * L);
-    for (int j = lane; j < L / 2; j += 32) dst[j] = src[j];
+
+  // ---- 1. Gram matrix: warp wid owns fragments (i, j) = (wid / 2, 2 (wid % 2) + {0, 1}) of the 4 x 4 grid of 8 x 8 fragments
+  {
+    const int fi = wid >> 1, fj = (wid & 1) * 2;
+    double acc[2][2] = {{0.0, 0.0}, {0.0, 0.0}};
+    const int lrow = tid >> 3, lc = (tid & 7) * 4;       // this thread stages 4 consecutive columns of one row
+    const bool lvalid = valid(lrow);
+    const double* lsrc = grow(lrow);
+    double v[4];
+    auto fetch = [&](int kc) {
+#pragma unroll
+      for (int e = 0; e < 4; ++e) { const int c = kc + lc + e; v[e] = (lvalid && c < B.vlen) ? lsrc[c] : 0.0; }
+    };
+    const int nchunk = (B.vlen + SV_KC - 1) / SV_KC;
+    fetch(0);
+    for (int ch = 0; ch < nchunk; ++ch) {
+      double (*st)[SV_KC + 4] = sm.stage[ch & 1];
+#pragma unroll
+      for (int e = 0; e < 4; ++e) st[lrow][lc + e] = v[e];
+      __syncthreads();                                   // chunk ch staged; everybody is past the DMMAs of chunk ch - 2
+      if (ch + 1 < nchunk) fetch((ch + 1) * SV_KC);
+#pragma unroll
+      for (int ks = 0; ks < SV_KC / 4; ++ks) {
+        const double a = st[8 * fi + g][4 * ks + q];
+        const double b0 = st[8 * fj + g][4 * ks + q], b1 = st[8 * fj + 8 + g][4 * ks + q];
+        dmma884(acc[0][0], acc[0][1], a, b0);
+        dmma884(acc[1][0], acc[1][1], a, b1);
+      }
+    }
+#pragma unroll
+    for (int f = 0; f < 2; ++f) {
+      sm.G[8 * fi + g][8 * (fj + f) + 2 * q] = acc[f][0];
+      sm.G[8 * fi + g][8 * (fj + f) + 2 * q + 1] = acc[f][1];
+    }
+    for (int e = tid; e < SV_M * SV_M; e += SV_THREADS) sm.Q[e >> 5][e & 31] = ((e >> 5) == (e & 31)) ? 1.0 : 0.0;
   }
   __syncthreads();
+
+  // ---- 2. one pass over the row pairs of the visit, on G (two-sided) and Q
   // rotate when |<x_p,x_q>| > tol |x_p||x_q| with tol = cols * 2^-53, the threshold LAPACK's Jacobi SVD (dgesvj) uses:
   // a dot product of `cols` terms cannot resolve angles below ~sqrt(cols) * 2^-53, and a tighter test only makes
   // rounding noise trigger further sweeps
   const double tol = 1.1102230246251565e-16 * (double)max(B.vlen, 8);
   int rotated = 0;
-  const int np = 2 * bsz - 1;
-  const int inner = full ? np : bsz;
-  const int c2 = B.vlen >> 1, L2 = L >> 1;               // rows as double2 (L is a multiple of 4, rows 16-byte aligned)
+  const int np = SV_M - 1;
+  const int inner = full ? np : SV_B;
   for (int s = 0; s < inner; ++s) {
-    int p, q;
-    if (full) {
-      if (wid == 0) { p = np; q = s; }
-      else { p = (s + wid) % np; q = (s - wid + np) % np; }
-    } else {
-      p = wid; q = bsz + (wid + s) % bsz;
-    }
-    if (valid(p) && valid(q)) {
-      // (de Rijk's ordering - exchanging the two vectors so that the lower index keeps the larger norm - was tried and
-      // needed two MORE sweeps on these spectra, 14 vs 12 on cyp, so the plain small-angle rotation stays)
-      double* xp = srow + (size_t)p * L;
-      double* xq = srow + (size_t)q * L;
-      double2* xp2 = reinterpret_cast<double2*>(xp);
-      double2* xq2 = reinterpret_cast<double2*>(xq);
-      double a = 0.0, b = 0.0, g = 0.0;
-#pragma unroll 4
-      for (int j = lane; j < c2; j += 32) {
-        const double2 u = xp2[j], v = xq2[j];
-        a = fma(u.x, u.x, a); b = fma(v.x, v.x, b); g = fma(u.x, v.x, g);
-        a = fma(u.y, u.y, a); b = fma(v.y, v.y, b); g = fma(u.y, v.y, g);
+#pragma unroll
+    for (int h = 0; h < 2; ++h) {                        // 16 pairs per step, two per warp
+      const int pp = wid + 8 * h;
+      int p, qq;
+      if (full) {
+        if (pp == 0) { p = np; qq = s; }
+        else { p = (s + pp) % np; qq = (s - pp + np) % np; }
+      } else {
+        p = pp; qq = SV_B + (pp + s) % SV_B;
       }
-      if ((B.vlen & 1) && lane == 0) {
-        const double u = xp[B.vlen - 1], v = xq[B.vlen - 1];
-        a = fma(u, u, a); b = fma(v, v, b); g = fma(u, v, g);
-      }
-      a = warp_sum(a); b = warp_sum(b); g = warp_sum(g);
-      if (a > B.floor2 && b > B.floor2 && g * g > tol * tol * a * b) {
-        // tan of the smaller rotation angle: t = sign(zeta) / (|zeta| + sqrt(1 + zeta^2)) with zeta = (b - a) / 2g, written
-        // with one square root, one division and one reciprocal square root (the chain of three divisions and three
-        // square roots was a third of a pair's latency)
-        const double d = b - a;
-        const double t = 2.0 * g / (d + copysign(sqrt(d * d + 4.0 * g * g), d));
-        const double cs = rsqrt(1.0 + t * t), sn = cs * t;
-#pragma unroll 4
-        for (int j = lane; j < L2; j += 32) {
-          const double2 u = xp2[j], v = xq2[j];
-          xp2[j] = make_double2(cs * u.x - sn * v.x, cs * u.y - sn * v.y);
-          xq2[j] = make_double2(sn * u.x + cs * v.x, sn * u.y + cs * v.y);
+      double cs = 1.0, sn = 0.0;
+      if (valid(p) && valid(qq)) {
+        const double a = sm.G[p][p], b = sm.G[qq][qq], gg = sm.G[p][qq];
+        if (a > B.floor2 && b > B.floor2 && gg * gg > tol * tol * a * b) {
+          // tan of the smaller rotation angle: t = sign(zeta) / (|zeta| + sqrt(1 + zeta^2)) with zeta = (b - a) / 2g
+          const double d = b - a;
+          const double t = 2.0 * gg / (d + copysign(sqrt(d * d + 4.0 * gg * gg), d));
+          cs = rsqrt(1.0 + t * t);
+          sn = cs * t;
+          ++rotated;
         }
-        ++rotated;
+      }
+      __syncwarp();
+      if (lane == 0) { sm.cs[pp][0] = cs; sm.cs[pp][1] = sn; }
+      if (sn != 0.0) {                                   // rows p, q of G and of Q (this pair's alone)
+        const double gp = sm.G[p][lane], gq = sm.G[qq][lane];
+        sm.G[p][lane] = cs * gp - sn * gq;
+        sm.G[qq][lane] = sn * gp + cs * gq;
+        const double qp = sm.Q[p][lane], qv = sm.Q[qq][lane];
+        sm.Q[p][lane] = cs * qp - sn * qv;
+        sm.Q[qq][lane] = sn * qp + cs * qv;
+      }
+    }
+    __syncthreads();
+#pragma unroll
+    for (int h = 0; h < 2; ++h) {                        // columns p, q of G
+      const int pp = wid + 8 * h;
+      int p, qq;
+      if (full) {
+        if (pp == 0) { p = np; qq = s; }
+        else { p = (s + pp) % np; qq = (s - pp + np) % np; }
+      } else {
+        p = pp; qq = SV_B + (pp + s) % SV_B;
+      }
+      const double cs = sm.cs[pp][0], sn = sm.cs[pp][1];
+      if (sn != 0.0) {
+        const double gp = sm.G[lane][p], gq = sm.G[lane][qq];
+        sm.G[lane][p] = cs * gp - sn * gq;
+        sm.G[lane][qq] = sn * gp + cs * gq;
       }
     }
     __syncthreads();
   }
-  for (int slot = wid; slot < 2 * bsz; slot += bsz) {
-    if (!valid(slot)) continue;
-    double2* dst = reinterpret_cast<double2*>(grow(slot));
-    const double2* src = reinterpret_cast<const double2*>(srow + (size_t)slot * L);
-    for (int j = lane; j < L / 2; j += 32) dst[j] = src[j];
+  const int any = __syncthreads_or(rotated);
+  if (!any) return;                                      // nothing rotated: the rows stay as they are
+
+  // ---- 3. X <- Q X over all L columns: warp wid owns the 8-column blocks wid, wid + 8, ...
+  double qa[4][SV_M / 4];                                // A fragments of Q: row block i, k-step ks
+#pragma unroll
+  for (int i = 0; i < 4; ++i)
+#pragma unroll
+    for (int ks = 0; ks < SV_M / 4; ++ks) qa[i][ks] = sm.Q[8 * i + g][4 * ks + q];
+  const double* brow[SV_M / 4];                          // row 4 ks + q of the visit (B fragment: k = q, n = g)
+  bool bval[SV_M / 4];
+#pragma unroll
+  for (int ks = 0; ks < SV_M / 4; ++ks) { bval[ks] = valid(4 * ks + q); brow[ks] = grow(4 * ks + q); }
+  for (int col0 = 8 * wid; col0 < L; col0 += 64) {
+    double bf[SV_M / 4];
+    const bool cok = col0 + g < L;
+#pragma unroll
+    for (int ks = 0; ks < SV_M / 4; ++ks) bf[ks] = (bval[ks] && cok) ? brow[ks][col0 + g] : 0.0;
+    double acc[4][2];
+#pragma unroll
+    for (int i = 0; i < 4; ++i) acc[i][0] = acc[i][1] = 0.0;
+#pragma unroll
+    for (int ks = 0; ks < SV_M / 4; ++ks)
+#pragma unroll
+      for (int i = 0; i < 4; ++i) dmma884(acc[i][0], acc[i][1], qa[i][ks], bf[ks]);
+    __syncwarp();                                        // every lane has read its part of the column block
+    const int c = col0 + 2 * q;
+    if (c < L) {                                         // L is even: the pair (c, c + 1) is inside the row or outside it
+#pragma unroll
+      for (int i = 0; i < 4; ++i)
+        if (valid(8 * i + g)) *reinterpret_cast<double2*>(grow(8 * i + g) + c) = make_double2(acc[i][0], acc[i][1]);
+    }
   }
-  if (rotated && lane == 0) atomicAdd(flag, rotated);    // rotations of the sweep (control only, not data)
+  if (lane == 0 && rotated) atomicAdd(flag, rotated);    // rotations of the sweep (control only, not data)
 }
 
 // singular value of every row = norm of its psi part (one warp per row)
@@ -233,8 +325,7 @@ extern "C" int hpsi_truncate(hpsi_plan_t* p, const double* psi_dev, int32_t side
     Lmax = std::max(Lmax, s.L);
   }
   const int n_rows = row0;
-  int bsz = std::min(SVD_MAX_BSZ, SVD_SMEM_BUDGET / (2 * Lmax * 8));
-  if (bsz < 1) { set_error("hpsi_truncate: a psi block is too large for the shared-memory Jacobi kernel"); return HPSI_EINVAL; }
+  const int bsz = SV_B;
   int n_cta = 0, rounds = 1;
   std::vector<int32_t> cta_blk;
   for (int b = 0; b < nB; ++b) {
@@ -247,8 +338,6 @@ extern "C" int hpsi_truncate(hpsi_plan_t* p, const double* psi_dev, int32_t side
     for (int k = 0; k < s.nce / 2; ++k) cta_blk.push_back(b);
     rounds = std::max(rounds, s.nce - 1);
   }
-  const size_t smem = (size_t)2 * bsz * Lmax * 8;
-
   // ---- device buffers (kept on the plan; regrown if a call needs more, e.g. the other side)
   {
     const size_t bytes = (size_t)wlen * 8 + (size_t)n_rows * 8 + tab.size() * sizeof(SvdBlk) + cta_blk.size() * 4 + (size_t)n_rows * sizeof(IsoRow) + 4096;
@@ -260,7 +349,6 @@ extern "C" int hpsi_truncate(hpsi_plan_t* p, const double* psi_dev, int32_t side
       cudaError_t e = cudaMalloc(&p->d_svd, bytes);
       if (e != cudaSuccess) { cudaGetLastError(); set_error("hpsi_truncate: device workspace allocation failed"); return HPSI_ENOMEM; }
       p->svd_bytes = bytes;
-      HPSI_CUDA(cudaFuncSetAttribute(svd_round_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, SVD_SMEM_BUDGET));
     }
   }
   char* base = static_cast<char*>(p->d_svd);
@@ -282,7 +370,7 @@ extern "C" int hpsi_truncate(hpsi_plan_t* p, const double* psi_dev, int32_t side
   for (; sweeps < MAX_SWEEPS && flag; ++sweeps) {
     HPSI_CUDA(cudaMemsetAsync(d_flag, 0, sizeof(int), st));
     for (int r = 0; r < rounds; ++r)
-      svd_round_kernel<<<n_cta, 32 * bsz, smem, st>>>(d_tab, d_cta, sweeps * rounds + r, bsz, d_w, d_flag);
+      svd_round_kernel<<<n_cta, SV_THREADS, 0, st>>>(d_tab, d_cta, sweeps * rounds + r, d_w, d_flag);
     HPSI_CUDA(cudaMemcpyAsync(&flag, d_flag, sizeof(int), cudaMemcpyDeviceToHost, st));
     HPSI_CUDA(cudaStreamSynchronize(st));
   }

@@ -312,11 +312,11 @@ def test_full_size_full_vector_parity(H, cfg):
 
 
 def test_femoco_shaped_full_vector_parity(H):
-    """BASELINE.json configs[3] (D = 8192, sector dims up to 653: ~11 tiles per block edge, K-stacks across several
+    """BASELINE.json configs[3] (D = 8192, sector dims up to 555: ~9 tiles per block edge, K-stacks across several
     groups) with 120 of its 2900 terms, so that the operators are 3.3 GB instead of 80: the whole output vector against
     the oracle, block by block, for the planner's order choice and both forced orders."""
     p = workloads.make_problem("femoco", n_terms=120)
-    assert p.d_left.sum() == 8192 and p.d_left.max() > 600
+    assert p.d_left.sum() == 8192 and p.d_right.sum() == 8192 and max(p.d_left.max(), p.d_right.max()) > 500
     psi = workloads.make_psi(p)
     ref = oracle.apply(p, psi)
     g = GpuProblem(p)
@@ -599,3 +599,106 @@ def test_streamed_operators(H, small):
     assert min(seen) == 1 and max(seen) > 50
     with pytest.raises(H.HpsiError):
         H.hpsi_stream_create(small, a_host, b_host, 16)     # a term does not fit the window
+
+
+# ------------------------------------------------------------ batched apply and multi-root Davidson
+@pytest.mark.parametrize("flags_name", ["min_flops", "order1", "order2"])
+def test_apply_multi_parity(H, small, flags_name):
+    """hpsi_apply_multi: nv vectors through one pass over the operators; every vector against the oracle, block by block;
+    a partial batch and a strided layout give the same bits; hpsi_apply on a batched plan is the nv = 1 case."""
+    import torch
+    nv = 4
+    g = GpuProblem(small, plan_flags(H, flags_name), n_vectors=nv)
+    assert g.q(H.HPSI_Q_N_VECTORS) == nv
+    psis = np.stack([workloads.make_psi(small, k) for k in range(nv)])
+    refs = [oracle.apply(small, psis[k]) for k in range(nv)]
+    x = torch.from_numpy(psis).cuda()
+    y = torch.full_like(x, float("nan"))
+    H.hpsi_apply_multi(g.plan, x, y, nv, torch.cuda.current_stream())
+    torch.cuda.synchronize()
+    out = y.cpu().numpy()
+    for k in range(nv):
+        assert_blockwise(small, out[k], refs[k], TOL)
+    # two of the four vectors, 7 doubles of slack between them
+    n = small.psi_len
+    xs = torch.zeros(2 * (n + 7), dtype=torch.float64, device="cuda")
+    ys = torch.full_like(xs, float("nan"))
+    xs[:n] = x[0]; xs[n + 7:2 * n + 7] = x[1]
+    H.hpsi_apply_multi(g.plan, xs, ys, 2, torch.cuda.current_stream(), ld_psi=n + 7, ld_out=n + 7)
+    torch.cuda.synchronize()
+    ysh = ys.cpu().numpy()
+    assert np.array_equal(ysh[:n], out[0]) and np.array_equal(ysh[n + 7:2 * n + 7], out[1]) and np.isnan(ysh[n:n + 7]).all()
+    assert np.array_equal(g.apply(psis[2]), out[2])
+    with pytest.raises(H.HpsiError):
+        H.hpsi_apply_multi(g.plan, x, y, nv + 1, torch.cuda.current_stream())
+    with pytest.raises(H.HpsiError):
+        H.hpsi_apply_multi(g.plan, x, x[1:], 2, torch.cuda.current_stream())        # overlapping sets
+
+
+def test_apply_multi_ragged_and_unaligned(H):
+    """Batched plans on irregular structures (dims 1 .. 200, odd leading dimensions, misaligned arenas: the 8-byte staging
+    kernels) and on the multi-tile ragged problem."""
+    import torch
+    for seed in range(4):
+        p = random_custom(seed, grid=(seed < 2))
+        g = GpuProblem(p, misalign=bool(seed % 2), n_vectors=3)
+        rng = np.random.default_rng(seed)
+        psis = rng.standard_normal((3, p.psi_len))
+        x = torch.from_numpy(psis).cuda()
+        y = torch.full_like(x, float("nan"))
+        H.hpsi_apply_multi(g.plan, x, y, 3, torch.cuda.current_stream())
+        torch.cuda.synchronize()
+        for k in range(3):
+            ref = oracle.apply(p, psis[k])
+            assert np.linalg.norm(y[k].cpu().numpy() - ref) <= TOL * max(np.linalg.norm(ref), 1.0)
+
+
+def _davidson_multi(H, g, V0, **kw):
+    import torch
+    x = torch.from_numpy(np.ascontiguousarray(V0.T)).cuda()          # [k, n]
+    theta, info = H.hpsi_davidson_multi(g.plan, x, V0.shape[1], **kw)
+    return theta, x.cpu().numpy().T, info
+
+
+@pytest.mark.parametrize("nvec_plan", [1, 3])
+def test_davidson_multi_vs_dense_and_oracle(H, toy, nvec_plan):
+    """hpsi_davidson_multi: the k lowest eigenvalues against LAPACK on the dense toy Hamiltonian, Ritz vectors orthonormal
+    eigenvectors, and - without the preconditioner - the same trajectory as the oracle's block Davidson (reading A21b).
+    A plan laid out for one vector runs the same method with one mat-vec per new vector."""
+    g = GpuProblem(toy, n_vectors=nvec_plan)
+    Hd = oracle.dense_hamiltonian(toy)
+    ev = np.linalg.eigvalsh(Hd)
+    k = 3
+    V0 = np.random.default_rng(k).standard_normal((toy.psi_len, k))
+    theta, X, info = _davidson_multi(H, g, V0, tol=1e-9, max_iter=800)
+    assert info["converged"] and np.max(np.abs(theta - ev[:k])) <= 1e-10, (theta, ev[:k], info)
+    assert np.max(np.abs(X.T @ X - np.eye(k))) <= 1e-11
+    assert np.max(np.linalg.norm(Hd @ X - X * theta[None, :], axis=0)) <= 1e-8
+    for it in (9, 20, 41):                                             # 41 > m_max: through restarts
+        th_g, _, info_g = _davidson_multi(H, g, V0, tol=1e-12, max_iter=it, precondition=False)
+        th_o, _, nmv_o, rn_o = oracle.davidson_block(toy, V0, tol=1e-12, max_iter=it, precondition=False)
+        assert info_g["n_matvec"] == nmv_o
+        assert np.max(np.abs(th_g - th_o)) <= 1e-9 * np.max(np.abs(th_o)), (it, th_g, th_o)
+        assert np.max(np.abs(info_g["residuals"] - rn_o)) <= 1e-6 * np.max(rn_o)
+
+
+def test_davidson_multi_hubbard_and_small(H, small):
+    """Two lowest levels of the Hubbard dimer sector (closed form, tests/golden/hubbard_closed_forms.txt) and of the
+    four-site chain (dense spectrum); on the D = 1024 config two roots through batched mat-vecs, residuals against the
+    oracle's H."""
+    dimer = hubbard_two_block_problem(1, 1, 1.0, 3.7, 2, 0)
+    theta, _, info = _davidson_multi(H, GpuProblem(dimer, n_vectors=2), np.eye(4)[:, :2] + 0.1, tol=1e-11, m_max=4)
+    assert info["converged"] and np.max(np.abs(theta - [(3.7 - np.sqrt(3.7 ** 2 + 16.0)) / 2, 0.0])) <= 1e-10
+    chain = hubbard_two_block_problem(2, 2, 1.0, 0.0, 4, 0)
+    ev = np.linalg.eigvalsh(oracle.dense_hamiltonian(chain))
+    V0 = np.random.default_rng(4).standard_normal((chain.psi_len, 2))
+    theta, _, info = _davidson_multi(H, GpuProblem(chain, n_vectors=2), V0, tol=1e-10, precondition=False, max_iter=400)
+    assert info["converged"] and np.max(np.abs(theta - ev[:2])) <= 1e-9
+    g = GpuProblem(small, n_vectors=2)
+    V0 = np.stack([workloads.make_psi(small, 0), workloads.make_psi(small, 1)], axis=1)
+    theta, X, info = _davidson_multi(H, g, V0, tol=1e-6, max_iter=400)
+    assert info["converged"] and theta[0] < theta[1]
+    for r in range(2):
+        assert np.linalg.norm(oracle.apply(small, X[:, r]) - theta[r] * X[:, r]) <= 1e-5
+    th1, _, _ = _davidson(H, g, V0[:, 0].copy(), tol=1e-7, max_iter=300)
+    assert abs(th1 - theta[0]) <= 1e-6 * abs(th1)

@@ -325,3 +325,45 @@ def test_davidson_vs_dense_eigensolver(toy, precondition):
     assert abs(theta - e0) <= 1e-10
     assert rn <= 1e-9 and np.linalg.norm(H @ x - theta * x) <= 1e-8
     assert abs(np.linalg.norm(x) - 1.0) <= 1e-12
+
+
+# ----------------------------------------------------------------------------- block (multi-root) Davidson
+@pytest.mark.parametrize("k", [2, 3])
+@pytest.mark.parametrize("precondition", [True, False])
+def test_davidson_block_vs_dense_eigensolver(toy, k, precondition):
+    """Reading A21b: the k lowest Ritz values against LAPACK's eigenvalues of the dense toy Hamiltonian, the Ritz vectors
+    orthonormal and each one an eigenvector to the tolerance."""
+    H = oracle.dense_hamiltonian(toy)
+    ev = np.linalg.eigvalsh(H)
+    V0 = np.random.default_rng(k).standard_normal((toy.psi_len, k))
+    theta, X, nmv, rn = oracle.davidson_block(toy, V0, tol=1e-9, max_iter=800, precondition=precondition)
+    assert np.max(np.abs(theta - ev[:k])) <= 1e-10 and rn.max() <= 1e-9
+    assert np.max(np.abs(X.T @ X - np.eye(k))) <= 1e-12
+    assert np.max(np.linalg.norm(H @ X - X * theta[None, :], axis=0)) <= 1e-8
+    assert k <= nmv <= 800
+
+
+def test_davidson_block_single_root_is_davidson(toy):
+    """k = 1 is the single-root method of reading A21, mat-vec for mat-vec."""
+    v0 = workloads.make_psi(toy)
+    for it in (5, 11, 30):
+        th1, x1, n1, r1 = oracle.davidson(toy, v0, tol=1e-12, max_iter=it, precondition=False)
+        thb, xb, nb, rb = oracle.davidson_block(toy, v0[:, None], tol=1e-12, max_iter=it, precondition=False)
+        # (the single-root routine spends one more mat-vec on a correction vector it then never uses: max_iter bounds its
+        # iterations, while the block routine - like hpsi_davidson - bounds the mat-vecs)
+        assert nb == it and n1 == it + 1
+        assert abs(thb[0] - th1) <= 1e-12 * abs(th1) and abs(rb[0] - r1) <= 1e-6 * r1
+
+
+def test_davidson_block_hubbard_levels():
+    """tests/golden/hubbard_closed_forms.txt: the two lowest levels of the dimer sector, (U - sqrt(U^2 + 16 t^2)) / 2 and
+    0, and the lowest two of the four-site chain against the dense spectrum."""
+    g = sorted(_golden()["dimer"])
+    dimer = hubbard_two_block_problem(1, 1, 1.0, 3.7, 2, 0)
+    theta, X, _, rn = oracle.davidson_block(dimer, np.eye(4)[:, :2] + 0.1, tol=1e-12, m_max=4)
+    assert np.max(np.abs(theta - g[:2])) <= 1e-12 and rn.max() <= 1e-12
+    chain = hubbard_two_block_problem(2, 2, 1.0, 0.0, 4, 0)
+    ev = np.linalg.eigvalsh(oracle.dense_hamiltonian(chain))
+    V0 = np.random.default_rng(4).standard_normal((chain.psi_len, 2))
+    theta, X, _, rn = oracle.davidson_block(chain, V0, tol=1e-10, precondition=False, max_iter=400)
+    assert abs(theta[0] - _golden()["chain4"][0]) <= 1e-10 and abs(theta[1] - ev[1]) <= 1e-9

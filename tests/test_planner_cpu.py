@@ -423,3 +423,32 @@ def test_transposed_block_validation(toy):
         H.hpsi_plan(shared.q_left, shared.q_right, shared.d_left, shared.d_right, shared.target, shared.coef, bad,
                     shared.b_desc, None, None, shared.a_len, shared.b_len, H.HPSI_PLAN_HOST_ONLY, shared.a_trans, shared.b_trans)
     assert e.value.code == H.HPSI_EINVAL
+
+
+# --------------------------------------------------------------------------------- batched plans (n_vectors > 1)
+@pytest.mark.parametrize("flags", [0, H.HPSI_PLAN_FIXED_ORDER1, H.HPSI_PLAN_FIXED_ORDER2])
+def test_batched_schedule_interpreter(toy, flags):
+    """hpsi_plan_options_t.n_vectors: the schedule of a batched apply (vectors side by side in the intermediate, one unit
+    per tile and vector) executed by the host interpreter gives H psi_v for every vector; fewer vectors than planned are
+    a prefix of the same work; flop / byte queries stay per vector; transposed blocks and the fused kernel are refused."""
+    for p in (toy, workloads.make_problem("small", n_terms=40), random_custom(5)):
+        single = host_plan(p, flags)
+        plan = H.plan_problem(p, flags=H.HPSI_PLAN_HOST_ONLY | flags, n_vectors=3)
+        assert H.hpsi_query(plan, H.HPSI_Q_N_VECTORS) == 3 and H.hpsi_query(single, H.HPSI_Q_N_VECTORS) == 1
+        rng = np.random.default_rng(1)
+        psis = rng.standard_normal((3, p.psi_len))
+        out = H.hpsi_debug_interpret(plan, p.a_data, p.b_data, psis)
+        for k in range(3):
+            ref = oracle.apply(p, psis[k])
+            assert np.linalg.norm(out[k] - ref) <= 1e-13 * max(np.linalg.norm(ref), 1.0)
+        assert np.array_equal(H.hpsi_debug_interpret(plan, p.a_data, p.b_data, psis[:2]), out[:2])
+        assert np.array_equal(H.hpsi_debug_interpret(plan, p.a_data, p.b_data, psis[0]), out[0])
+        for w in (H.HPSI_Q_USEFUL_FLOPS, H.HPSI_Q_ISSUED_FLOPS, H.HPSI_Q_OPERATOR_BYTES, H.HPSI_Q_N_TASKS):
+            assert H.hpsi_query(plan, w) == H.hpsi_query(single, w)
+        assert H.hpsi_query(plan, H.HPSI_Q_N_P1_UNITS) == 3 * H.hpsi_query(single, H.HPSI_Q_N_P1_UNITS)
+    with pytest.raises(H.HpsiError):
+        H.plan_problem(workloads.make_problem("toy", share_adjoint=True), flags=H.HPSI_PLAN_HOST_ONLY, n_vectors=2)
+    with pytest.raises(H.HpsiError):
+        H.plan_problem(toy, flags=H.HPSI_PLAN_HOST_ONLY | H.HPSI_PLAN_FUSE_ALL, n_vectors=2)
+    with pytest.raises(H.HpsiError):
+        H.plan_problem(toy, flags=H.HPSI_PLAN_HOST_ONLY, n_vectors=65)
