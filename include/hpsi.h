@@ -83,7 +83,7 @@ typedef struct {
    * says the arena holds the TRANSPOSE of that block: element (x, x') of the block is arena[offset + x' * ld + x] with
    * ld >= d[row].  A Hermitian H pairs every term with its adjoint (same c, A^T, B^T): the adjoint term's descriptors
    * can then point at the base term's storage and the operator arenas halve (80 -> 40 GB at D=8192).  Such blocks are
-   * staged K-major (16 x 16 TMA boxes) and their tiles are padded to 16 instead of 8 rows. */
+   * staged K-major (TMA boxes of 8 rows x 16 k, 64-byte swizzle); tiles stay padded to 8 rows as in plain plans. */
   const uint8_t* a_transposed;
   const uint8_t* b_transposed;
 } hpsi_terms_t;
@@ -370,7 +370,7 @@ typedef struct {
   int32_t tma_ld_multiple;       /* required for the TMA staging path: ld and offset multiples of this (2 = 16 bytes);  */
   int32_t tma_offset_multiple;   /*   anything else runs the 8-byte cp.async kernels (correct, slower)                  */
   int32_t arena_align_bytes;     /* required for the TMA path: arena base address alignment (16)                        */
-  int32_t transposed_pad_rows;   /* tiles of a plan with transposed blocks are padded to this many rows (16; plain: 8)  */
+  int32_t transposed_pad_rows;   /* tiles of a plan with transposed blocks are padded to this many rows (8, as plain plans) */
 } hpsi_layout_t;
 
 typedef struct {

@@ -102,7 +102,7 @@ void free_plan(hpsi_plan_t* p) {
 }
 
 // Tensor maps of every operand matrix (plan.h MapSpec): 2-D FP64 tensor {cols, rows} with row pitch ld, box
-// {KT, box_rows}, 128-byte swizzle, zero fill outside the matrix.  The encoder is a driver entry point fetched
+// {box_cols, box_rows}, 128-byte swizzle (64-byte for the 8-column boxes of transposed blocks), zero fill outside the matrix.  The encoder is a driver entry point fetched
 // through the runtime, so the library does not link libcuda.
 typedef CUresult (*tmap_encode_fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
                                    const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
@@ -125,7 +125,8 @@ int encode_maps(hpsi_plan_t* p) {
     const cuuint32_t box[2] = {(cuuint32_t)m.box_cols, (cuuint32_t)m.box_rows};
     const cuuint32_t estr[2] = {1, 1};
     CUresult r = enc(&host[i], CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, const_cast<double*>(base + m.off), dims, strides, box, estr,
-                     CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                     CU_TENSOR_MAP_INTERLEAVE_NONE, m.box_cols * 8 == 64 ? CU_TENSOR_MAP_SWIZZLE_64B : CU_TENSOR_MAP_SWIZZLE_128B,
+                     CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
                      CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) {
       char buf[200];
@@ -452,7 +453,7 @@ extern "C" int hpsi_query(const hpsi_plan_t* p, int what, void* out, size_t byte
     }
     case HPSI_Q_PREFERRED_LAYOUT: {
       if (bytes < sizeof(hpsi_layout_t)) { set_error("hpsi_query: buffer too small"); return HPSI_EINVAL; }
-      const hpsi_layout_t lay = {4, 4, 2, 2, 16, 16};
+      const hpsi_layout_t lay = {4, 4, 2, 2, 16, 8};
       memcpy(out, &lay, sizeof lay);
       return HPSI_OK;
     }

@@ -289,7 +289,7 @@ __global__ void prep_kernel(DevSchedule d, const double* __restrict__ psi, const
 // reduce_plain_kernel below; the launcher picks by size.  Partials: split-major, vector-minor.
 constexpr int RED_LANES = 8;
 __global__ void reduce_kernel(DevSchedule d, double* __restrict__ out, int accumulate) {
-  const ElemCta c = d.elem[blockIdx.x];
+  const ElemCta c = d.elem[blockIdx.x >> 3];                   // eight CTAs per granule: 32 elements each (lanes x 8 = 256 threads)
   const PsiBlk B = d.blocks[c.blk];
   const int n = B.rows * B.cols;
   const int64_t stride = (int64_t)d.nvec * B.rows * B.ldo;
@@ -298,10 +298,9 @@ __global__ void reduce_kernel(DevSchedule d, double* __restrict__ out, int accum
   const int q = threadIdx.x & (RED_LANES - 1);
   const int per = (B.nsplit + RED_LANES - 1) / RED_LANES;
   const int sp0 = min(q * per, B.nsplit), sp1 = min(sp0 + per, B.nsplit);
-  constexpr int EPP = 256 / RED_LANES;                         // elements per pass
-#pragma unroll 1
-  for (int pass = 0; pass < RED_LANES; ++pass) {               // whole warps stay in the loop for the shuffles
-    const int e = c.e0 + pass * EPP + (threadIdx.x / RED_LANES);
+  constexpr int EPP = 256 / RED_LANES;                         // elements per CTA
+  {                                                            // whole warps stay in for the shuffles
+    const int e = c.e0 + (blockIdx.x & 7) * EPP + (threadIdx.x / RED_LANES);
     double s = 0.0;
     if (e < n) {
       const int x = e / B.cols, y = e - x * B.cols;
@@ -413,7 +412,7 @@ void launch_p2(const DevSchedule& d, bool tma, cudaStream_t st) {
 void launch_reduce(const DevSchedule& d, double* out, bool accumulate, cudaStream_t st) {
   if (d.n_elem == 0) return;
   const bool small_vec = (int64_t)d.n_elem * 256 <= 500000;     // latency-bound sizes (D <~ 1500)
-  if (small_vec) reduce_kernel<<<dim3(d.n_elem, d.nvec_active), 256, 0, st>>>(d, out, accumulate ? 1 : 0);
+  if (small_vec) reduce_kernel<<<dim3(d.n_elem * 8, d.nvec_active), 256, 0, st>>>(d, out, accumulate ? 1 : 0);
   else reduce_plain_kernel<<<dim3(d.n_elem, d.nvec_active), 256, 0, st>>>(d, out, accumulate ? 1 : 0);
 }
 void launch_diag(const DevSchedule& d, double* diag, cudaStream_t st) {

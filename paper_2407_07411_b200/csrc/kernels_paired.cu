@@ -1,67 +1,54 @@
 // GEMM kernels for plans in which some operator block is stored transposed (hpsi_terms_t a_transposed / b_transposed:
 // adjoint-pair storage sharing).  Same CTA design as kernels.cu (1 TMA producer warp + 4 DMMA consumer
-// warps, mbarrier ring); what differs is how fragments map to tile rows.
+// warps, mbarrier ring, 8 x 8 fragments, tiles padded to 8); what differs is how a fragment's rows map to tile rows, so
+// that one mapping reads BOTH operand layouts without bank conflicts:
 //
-// A block stored transposed is an M-contiguous ("T") operand: the TMA unit stages a 64-row x 16-k piece of it as four
-// 16(k) x 16(rows) boxes (128 bytes per k, 128-byte swizzle), i.e. sub-tile b = rows 16b..16b+15 holds element
-// (k, ii) at  k*128 + (((ii >> 1) ^ (k & 7)) << 4) + (ii & 1)*8  bytes.  A DMMA fragment (8 rows x 4 k, lane (g, q) ->
-// row g, k = 4 ks + q) reads such a tile without bank conflicts iff the 4 rows of each half-warp differ in
-// (bit 3, bit 0) of ii; a K-contiguous ("N") tile (kernels.cu) needs them to differ in bits (2, 1).  Both hold for
-//     fragment sibling 0: rows {0,3,12,15 | 1,2,13,14} of a 16-row group,   sibling 1: the same ^ 4,
-// so in these kernels fragments come in pairs that interleave 16 rows, whatever the layout of the operand: one
-// accumulator <-> tile-element mapping serves a unit whose K range mixes plainly stored and transposed blocks.
-// Tiles are therefore padded to 16 rows / columns (plan.h tile_frags(.., paired = true)), and a warp owns whole pairs.
+//   N tile (K-contiguous operand, kernels.cu): one 64-row x 16-k TMA box, 128 bytes per row, 128-byte swizzle: element
+//            (row r, k) at  r*128 + (((k >> 1) ^ (r & 7)) << 4) + (k & 1)*8  bytes.
+//   T tile (block stored transposed = M-contiguous operand): 8 TMA boxes of 8 rows x 16 k from a tensor map whose inner
+//            dimension is the operand's ROW index (64 bytes per k, 64-byte swizzle), box b = rows 8b .. 8b+7 at b*1024:
+//            element (row r, k) at  k*64 + ((((r >> 1) ^ (k >> 1)) & 3) << 4) + (r & 1)*8  bytes.
+//
+// A DMMA fragment is 8 rows x 4 k, lane (g, q) reading (row g, k = 4 ks + q); a 64-bit shared load is served per
+// half-warp (g = 0..3 | 4..7).  The N tile is conflict-free iff the 4 rows of a half-warp differ in bits (2,1) of r; the T
+// tile iff their (r >> 1, r & 1) pairs and those with r >> 1 flipped in bit 0 are all distinct.  Rows {0,3,4,7 | 1,2,5,6}
+// satisfy both, so lane group g reads row perm8(g) = (0,3,4,7,1,2,5,6)[g] of the fragment whatever the layout, and a
+// unit whose K range mixes plainly stored and transposed blocks keeps ONE accumulator <-> tile-element mapping.
+// (Round 1 used 16-row boxes with the 128-byte swizzle for T tiles, which forced fragments to interleave 16 rows and tiles
+// to be padded to 16: issued / useful flops 1.109 instead of 1.059 on cyp, 28.5 vs 31.9 TFLOPS.)
 #include "kernels_common.cuh"
 
 namespace hpsi {
 
-// row (0..15) of its 16-row group that sibling s of a fragment pair gives to lane group / accumulator index x (0..7)
-__device__ __forceinline__ int row16(int s, int x) { return (int)((0xED21FC30u >> (4 * x)) & 15u) ^ (s << 2); }
+// row (0..7) of its fragment that lane group / accumulator index x (0..7) maps to
+__device__ __forceinline__ int perm8(int x) { return (int)((0x65217430u >> (4 * x)) & 15u); }
 
-// Per-lane element offsets (doubles, relative to the warp's first pair of the operand tile) of k-steps 0..3 for the two
-// siblings; pair p of the warp adds 256 p.  `t` = the operand is an M-contiguous ("T") tile.
-struct PairOffsets {
-  int x[2][4], y[2][4];
+// Per-lane element offsets (doubles, relative to the warp's first fragment of the operand tile) of k-steps 0..3; fragment
+// i of the warp adds 128 i in both layouts.  `t` = the operand is an M-contiguous ("T") tile.
+struct MixOffsets {
+  int x[4], y[4];
   __device__ __forceinline__ static int off(int r, int q, int ks, bool t) {
-    if (t) { const int k = 4 * ks + q; return k * 16 + ((((r >> 1) ^ (k & 7))) << 1) + (r & 1); }
+    if (t) { const int k = 4 * ks + q; return k * 8 + ((((r >> 1) ^ (k >> 1)) & 3) << 1) + (r & 1); }
     return r * 16 + (((2 * ks + (q >> 1)) ^ (r & 7)) << 1) + (q & 1);
   }
   __device__ __forceinline__ void set(int lane, bool xt, bool yt) {
-    const int g = lane >> 2, q = lane & 3;
+    const int r = perm8(lane >> 2), q = lane & 3;
 #pragma unroll
-    for (int s = 0; s < 2; ++s)
-#pragma unroll
-      for (int ks = 0; ks < 4; ++ks) {
-        x[s][ks] = off(row16(s, g), q, ks, xt);
-        y[s][ks] = off(row16(s, g), q, ks, yt);
-      }
-  }
-};
-
-struct WarpTileP {
-  int wr0, wc0;    // first row / col of the warp inside the CTA tile (multiples of 16)
-  int mi, nj;      // fragments owned (even)
-  __device__ __forceinline__ WarpTileP(int gn, int warp, int rows_valid, int cols_valid) {
-    const int gm = NCONS / gn;
-    int f0, cnt;
-    split_frags((rows_valid + 15) >> 4, gm, warp / gn, f0, cnt);
-    wr0 = f0 * 16; mi = 2 * cnt;
-    split_frags((cols_valid + 15) >> 4, gn, warp % gn, f0, cnt);
-    wc0 = f0 * 16; nj = 2 * cnt;
+    for (int ks = 0; ks < 4; ++ks) { x[ks] = off(r, q, ks, xt); y[ks] = off(r, q, ks, yt); }
   }
 };
 
 template <int MI, int NJ>
-__device__ __forceinline__ void load_frags_p(const double* px, const double* py, const PairOffsets& po, int ks,
+__device__ __forceinline__ void load_frags_p(const double* px, const double* py, const MixOffsets& po, int ks,
                                              double (&a)[MI], double (&b)[NJ]) {
 #pragma unroll
-  for (int i = 0; i < MI; ++i) a[i] = px[po.x[i & 1][ks] + (i >> 1) * 256];
+  for (int i = 0; i < MI; ++i) a[i] = px[po.x[ks] + i * 128];
 #pragma unroll
-  for (int j = 0; j < NJ; ++j) b[j] = py[po.y[j & 1][ks] + (j >> 1) * 256];
+  for (int j = 0; j < NJ; ++j) b[j] = py[po.y[ks] + j * 128];
 }
 // as mma_stage (kernels.cu): the fragments of k-step ks+1 are fetched while step ks issues
 template <int MI, int NJ>
-__device__ __forceinline__ void mma_stage_p(const double* px, const double* py, const PairOffsets& po,
+__device__ __forceinline__ void mma_stage_p(const double* px, const double* py, const MixOffsets& po,
                                             double (&acc)[MI][NJ][2], int nk4) {
   double a0[MI], b0[NJ], a1[MI], b1[NJ];
   load_frags_p<MI, NJ>(px, py, po, 0, a0, b0);
@@ -80,46 +67,46 @@ __device__ __forceinline__ void mma_stage_p(const double* px, const double* py, 
   }
 }
 
-// acc[i][j][e] holds tile row wr0 + 16 (i/2) + row16(i&1, g) and tile column wc0 + 16 (j/2) + row16(j&1, 2q + e)
+// acc[i][j][e] holds tile row wr0 + 8 i + perm8(g) and tile column wc0 + 8 j + perm8(2 q + e)
 template <int MI, int NJ>
 __device__ __forceinline__ void store_tile_p(double* dst, int ld, int rows_valid, int cols_valid,
-                                             const double (&acc)[MI][NJ][2], const WarpTileP& w, int lane, double sc) {
-  const int g = lane >> 2, q = lane & 3;
+                                             const double (&acc)[MI][NJ][2], const WarpTile& w, int lane, double sc) {
+  const int pg = perm8(lane >> 2), q = lane & 3;
+  const int pc0 = perm8(2 * q), pc1 = perm8(2 * q + 1);
 #pragma unroll
   for (int i = 0; i < MI; ++i) {
-    const int row = w.wr0 + 16 * (i >> 1) + row16(i & 1, g);
+    const int row = w.wr0 + 8 * i + pg;
     if (row >= rows_valid) continue;
     double* drow = dst + (int64_t)row * ld;
 #pragma unroll
     for (int j = 0; j < NJ; ++j) {
-#pragma unroll
-      for (int e = 0; e < 2; ++e) {
-        const int col = w.wc0 + 16 * (j >> 1) + row16(j & 1, 2 * q + e);
-        if (col < cols_valid) drow[col] = acc[i][j][e] * sc;
-      }
+      const int c0 = w.wc0 + 8 * j + pc0, c1 = w.wc0 + 8 * j + pc1;
+      if (c0 < cols_valid) drow[c0] = acc[i][j][0] * sc;
+      if (c1 < cols_valid) drow[c1] = acc[i][j][1] * sc;
     }
   }
 }
 
 // ---------------------------------------------------------------------------------------------- staging
 // LDGSTS fallback for an M-contiguous operand: rows_valid operand rows starting at `first` (= element (row 0, k 0) of
-// the window), k-major with leading dimension ld.  Lane handles k = lane & 15 of rows (lane >> 4) + 2 p.
+// the window), k-major with leading dimension ld, written in the T-tile layout above.  Lane handles k = lane & 15 of rows
+// (lane >> 4) + 2 p.
 __device__ __forceinline__ void ldgsts_tile_t(uint32_t s_op, const double* first, int64_t ld, int rows_valid, int kappa,
                                               int K, int lane) {
   const int k = lane & 15, r0 = lane >> 4;
   const bool kvalid = kappa + k < K;
 #pragma unroll 8
   for (int p = 0; p < TILE / 2; ++p) {
-    const int r = r0 + 2 * p, ii = r & 15;
+    const int r = r0 + 2 * p, rr = r & 7;
     const bool ok = kvalid && r < rows_valid;
     const double* src = ok ? first + (int64_t)(kappa + k) * ld + r : first;
-    const uint32_t dst = s_op + (r >> 4) * 2048 + k * 128 + ((((ii >> 1) ^ (k & 7)) << 4) | ((ii & 1) << 3));
+    const uint32_t dst = s_op + (r >> 3) * 1024 + k * 64 + (((((rr >> 1) ^ (k >> 1)) & 3) << 4) | ((rr & 1) << 3));
     cp_async_chunk8(dst, src, ok ? 8 : 0);
   }
 }
 
-// One operand of a stage.  N: one 64-row x 16-k box (or the 8-byte LDGSTS copy); T: ceil(rows_valid / 16) boxes of
-// 16 k x 16 rows.  `row0` = first operand row of the tile inside the matrix; for LDGSTS `ptr` = element (row0, 0).
+// One operand of a stage.  N: one 64-row x 16-k box (or the 8-byte LDGSTS copy); T: ceil(rows_valid / 8) boxes of
+// 16 k x 8 rows.  `row0` = first operand row of the tile inside the matrix; for LDGSTS `ptr` = element (row0, 0).
 struct OperandSrc {
   const unsigned char* map;   // TMA
   const double* ptr;          // LDGSTS
@@ -128,7 +115,7 @@ struct OperandSrc {
   int trans;
 };
 __device__ __forceinline__ uint32_t operand_bytes(const OperandSrc& o, int rows_valid) {
-  return o.trans ? (uint32_t)((rows_valid + 15) >> 4) * 2048u : (uint32_t)OP_BYTES;
+  return o.trans ? (uint32_t)((rows_valid + 7) >> 3) * 1024u : (uint32_t)OP_BYTES;
 }
 template <bool TMA>
 __device__ __forceinline__ void stage_operand(const OperandSrc& o, uint32_t s_op, int rows_valid, int kappa, int K,
@@ -136,8 +123,8 @@ __device__ __forceinline__ void stage_operand(const OperandSrc& o, uint32_t s_op
   if (TMA) {
     if (lane != 0) return;
     if (!o.trans) { tma_load_2d(s_op, o.map, kappa, o.row0, full); return; }
-    const int nsub = (rows_valid + 15) >> 4;
-    for (int b = 0; b < nsub; ++b) tma_load_2d(s_op + b * 2048, o.map, o.row0 + 16 * b, kappa, full);
+    const int nsub = (rows_valid + 7) >> 3;
+    for (int b = 0; b < nsub; ++b) tma_load_2d(s_op + b * 1024, o.map, o.row0 + 8 * b, kappa, full);
   } else {
     if (!o.trans) ldgsts_tile(s_op, o.ptr, o.ld, rows_valid, kappa, K, lane);
     else ldgsts_tile_t(s_op, o.ptr, o.ld, rows_valid, kappa, K, lane);
@@ -159,11 +146,14 @@ __device__ __forceinline__ void stage_both(const OperandSrc& x, const OperandSrc
   }
 }
 
-// Dispatch to the instantiation for the warp's (mi, nj) in fragments: whole pairs, at most 16 fragments per warp.
-#define HPSI_DISPATCH_PAIRS(CALL)                                                          \
-  switch (w.mi * 9 + w.nj) {                                                               \
-    CALL(2, 2) CALL(2, 4) CALL(4, 2) CALL(4, 4) CALL(2, 6) CALL(6, 2) CALL(2, 8) CALL(8, 2) \
-    default: __trap();                                                                     \
+// Dispatch to the instantiation for the warp's (mi, nj): <=4x4 (2x2 grid), <=8x2 (1x4 grid), <=2x8 (4x1 grid), as kernels.cu.
+#define HPSI_DISPATCH_PAIRS(CALL)                                                                               \
+  switch (w.mi * 9 + w.nj) {                                                                                    \
+    CALL(1, 1) CALL(1, 2) CALL(1, 3) CALL(1, 4) CALL(2, 1) CALL(2, 2) CALL(2, 3) CALL(2, 4)                     \
+    CALL(3, 1) CALL(3, 2) CALL(3, 3) CALL(3, 4) CALL(4, 1) CALL(4, 2) CALL(4, 3) CALL(4, 4)                     \
+    CALL(5, 1) CALL(5, 2) CALL(6, 1) CALL(6, 2) CALL(7, 1) CALL(7, 2) CALL(8, 1) CALL(8, 2)                     \
+    CALL(1, 5) CALL(2, 5) CALL(1, 6) CALL(2, 6) CALL(1, 7) CALL(2, 7) CALL(1, 8) CALL(2, 8)                     \
+    default: __trap();                                                                                          \
   }
 
 __device__ __forceinline__ void idle_consume_p(const SmemLayout& sm, int nstages, int lane) {
@@ -178,9 +168,9 @@ __device__ __forceinline__ void idle_consume_p(const SmemLayout& sm, int nstages
 // ------------------------------------------------------------------------------------------------ P1 kernel
 template <int MI, int NJ>
 __device__ __forceinline__ void p1p_consume(const DevSchedule& d, const P1Unit& u, const Group& g, const SmemLayout& sm,
-                                            const WarpTileP& w, int lane) {
+                                            const WarpTile& w, int lane) {
   double acc[MI][NJ][2];
-  PairOffsets po;
+  MixOffsets po;
   po.set(lane, u.xtrans != 0, false);
   const int ntiles = (g.K1 + KT - 1) / KT;
   const int last_nk4 = ((g.K1 - (ntiles - 1) * KT) + 3) >> 2;
@@ -233,7 +223,7 @@ __global__ void __maxnreg__(136) p1p_kernel(DevSchedule d) {
 
   // ------------------ consumer warps
   const int warp = (wid + quadrant_rotation(blockIdx.x)) % NCONS;
-  const WarpTileP w(u.grid, warp, u.rows_valid, u.cols_valid);
+  const WarpTile w(u.grid, warp, u.rows_valid, u.cols_valid);
   if (w.mi == 0 || w.nj == 0) { idle_consume_p(sm, ntiles * (u.t1 - u.t0), lane); return; }
 #define HPSI_CASE(MI, NJ) case MI * 9 + NJ: p1p_consume<MI, NJ>(d, u, g, sm, w, lane); break;
   HPSI_DISPATCH_PAIRS(HPSI_CASE)
@@ -243,10 +233,10 @@ __global__ void __maxnreg__(136) p1p_kernel(DevSchedule d) {
 // ------------------------------------------------------------------------------------------------ P2 kernel
 template <int MI, int NJ>
 __device__ __forceinline__ void p2p_consume(const DevSchedule& d, const P2Unit& u, const SmemLayout& sm,
-                                            const WarpTileP& w, int lane) {
+                                            const WarpTile& w, int lane) {
   double acc[MI][NJ][2];
   zero_acc<MI, NJ>(acc);
-  PairOffsets po;
+  MixOffsets po;
   Ring ring{0, 0};
   for (int r = u.run_begin; r < u.run_end; ++r) {            // same (run, seg, k-tile) order as the producer
     const Run run = d.runs[r];
@@ -309,7 +299,7 @@ __global__ void __maxnreg__(136) p2p_kernel(DevSchedule d) {
 
   // ------------------ consumer warps
   const int warp = (wid + quadrant_rotation(blockIdx.x)) % NCONS;
-  const WarpTileP w(u.grid, warp, u.rows_valid, u.cols_valid);
+  const WarpTile w(u.grid, warp, u.rows_valid, u.cols_valid);
   if (w.mi == 0 || w.nj == 0) {
     int nstages = 0;
     for (int r = u.run_begin; r < u.run_end; ++r)

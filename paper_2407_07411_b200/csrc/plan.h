@@ -95,7 +95,7 @@ struct P2Unit {               // one CTA of the second-GEMM kernel
 // A 2-D row-major matrix the TMA unit reads: rows x cols doubles as STORED, leading dimension ld, `off` doubles into
 // `base`.  Encoded (api.cu) as a CUtensorMap with box {box_cols columns, box_rows rows}, 128-byte swizzle, zero fill
 // out of bounds.  K-contiguous operand ("N" layout): rows = the operand's rows, cols = K, box {KT, TILE}.
-// Block stored transposed ("T" layout): rows = K, cols = the operand's rows, box {16, KT}.
+// Block stored transposed ("T" layout): rows = K, cols = the operand's rows, box {8, KT}, 64-byte swizzle.
 struct MapSpec {
   int64_t off;
   int32_t base;               // BaseSel
@@ -147,7 +147,7 @@ struct Schedule {
   int64_t n_order1 = 0;
   int32_t max_block_elems = 0;
   bool aligned16 = true;              // descriptors allow the 16-byte staging path (arena base checked at bind)
-  bool paired = false;                // some block is stored transposed: fragments are taken from 16-row groups (kernels.cu)
+  bool paired = false;                // some block is stored transposed: the GEMMs run the mixed-layout kernels (kernels_paired.cu)
   int64_t tuning[3] = {0, 0, 0};      // realised schedule knobs: P1 K-tiles per unit, P2 waves, P2 minimum DMMA per unit
   int32_t n_terms_planned = 0;        // terms of this plan's shard (all terms without a shard)
   int32_t nvec = 1;                   // vectors one hpsi_apply_multi works on (hpsi_plan_options_t.n_vectors)
@@ -183,28 +183,14 @@ inline int even_up(int x) { return x + (x & 1); }
 // 128-byte row segment is exactly four sectors (measured: 16-byte-aligned rows cost 1.4x the sectors).
 inline int sector_up(int x) { return (x + 3) & ~3; }
 inline int frags(int x) { return (x + 7) / 8; }
-// fragments a tile dimension of x rows occupies: in paired mode fragments come in pairs that interleave 16 rows
-inline int tile_frags(int x, bool paired) { return paired ? 2 * ((x + 15) / 16) : (x + 7) / 8; }
+// fragments a tile dimension of x rows occupies (plans with transposed blocks use 8-row fragments too, kernels_paired.cu)
+inline int tile_frags(int x, bool /*paired*/) { return (x + 7) / 8; }
 // Heaviest warp (in fragments) when a tile of fm x fn fragments is covered by a gm x gn grid of warps, and the grid
 // that minimises it among those whose warp tile has a compiled instantiation (<=4x4, <=8x2, <=2x8 fragments);
 // ties go to the squarest grid (fewest shared-memory reads per DMMA).
 inline int heaviest_warp(int fm, int fn, int gm, int gn) { return ((fm + gm - 1) / gm) * ((fn + gn - 1) / gn); }
 inline bool warp_tile_ok(int mi, int nj) { return (mi <= 4 && nj <= 4) || (mi <= 8 && nj <= 2) || (mi <= 2 && nj <= 8); }
-inline int32_t best_grid(int fm, int fn, int* heaviest = nullptr, bool paired = false) {
-  if (paired) {                        // warps own whole pairs (2 fragments): <=2x2, <=4x1 or <=1x4 pairs per warp
-    const int pm = fm / 2, pn = fn / 2;
-    const int order[4] = {2, 4, 1, NCONS_WARPS};
-    int best = 1 << 30;
-    int32_t g = 2;
-    for (int gn : order) {
-      if (gn > NCONS_WARPS || NCONS_WARPS % gn) continue;
-      const int gm = NCONS_WARPS / gn, mp = (pm + gm - 1) / gm, np = (pn + gn - 1) / gn;
-      if (!((mp <= 2 && np <= 2) || (mp <= 4 && np <= 1) || (mp <= 1 && np <= 4))) continue;
-      if (mp * np < best) { best = mp * np; g = gn; }
-    }
-    if (heaviest) *heaviest = 4 * best;
-    return g;
-  }
+inline int32_t best_grid(int fm, int fn, int* heaviest = nullptr, bool /*paired*/ = false) {
   const int order[4] = {2, 4, 1, NCONS_WARPS};   // squarest first
   int best = 1 << 30;
   int32_t g = 2;

@@ -266,7 +266,7 @@ int build_schedule(const hpsi_sectors_t* s, const hpsi_terms_t* t, uint32_t flag
   // operator block that is an NT operand with op_rows rows and K = op_k columns; stored transposed if tr
   auto add_op_map = [&](int base, int64_t moff, int op_rows, int op_k, int ld, int tr) -> int32_t {
     if (!tr) return add_map(base, moff, op_rows, op_k, ld);
-    sc->maps.push_back({moff, base, op_k, op_rows, ld, KT, 16});
+    sc->maps.push_back({moff, base, op_k, op_rows, ld, KT, 8});     // T layout: 8 operand rows (64 bytes) x 16 k per box
     return (int32_t)sc->maps.size() - 1;
   };
   for (auto& b : sc->blocks) {

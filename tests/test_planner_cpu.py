@@ -83,7 +83,7 @@ def test_preferred_layout_query_and_layout_blocks(small):
     can describe its blocks, let the library lay them out, fill the arenas and plan (arenas bound later)."""
     lay = H.hpsi_query(host_plan(small), H.HPSI_Q_PREFERRED_LAYOUT)
     assert lay == {"ld_multiple": 4, "offset_multiple": 4, "tma_ld_multiple": 2, "tma_offset_multiple": 2,
-                   "arena_align_bytes": 16, "transposed_pad_rows": 16}
+                   "arena_align_bytes": 16, "transposed_pad_rows": 8}
     dense = workloads.make_problem("small", n_terms=20, pad_even=False)           # odd lds, dense offsets
     a_desc, a_len = H.hpsi_layout_blocks(dense.d_left, dense.a_desc)
     b_desc, b_len = H.hpsi_layout_blocks(dense.d_right, dense.b_desc)
