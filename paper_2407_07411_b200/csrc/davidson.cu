@@ -104,6 +104,7 @@ __device__ void small_eig_block(const double* __restrict__ G, int j, double* the
       if (t < j) { sm.A[t][c] = 0.5 * (G[t * MMAX + c] + G[c * MMAX + t]); sm.Q[t][c] = (t == c) ? 1.0 : 0.0; }
   }
   __syncthreads();
+  double prev_off = 0.0;
   for (int sweep = 0; sweep < 30 && j > 1; ++sweep) {
     if (wid == 0) {                                      // squared norms of the off-diagonal part and of the diagonal
       double off = 0.0, dg = 0.0;
@@ -116,8 +117,13 @@ __device__ void small_eig_block(const double* __restrict__ G, int j, double* the
       if (t == 0) { sm.norms[0] = off; sm.norms[1] = dg; }
     }
     __syncthreads();
+    // Stop when the off-diagonal Frobenius norm is below 1e-15 of the matrix norm - the floor rounding leaves (every
+    // rotation perturbs the entries by ~2^-53 of the norm) - or when a sweep no longer reduces it by at least 4x: Jacobi
+    // converges quadratically, so stagnation means the floor has been reached.  (The first version asked for 1e-17, which
+    // rounding never reaches: every call ran all 30 sweeps, 50-70 us at j ~ 12 - most of a Davidson iteration's overhead.)
     const double off = sm.norms[0], dg = sm.norms[1];
-    if (off <= 1e-34 * (dg + 2.0 * off) || off < 1e-300) break;   // off-diagonal norm below 1e-17 of the matrix norm
+    if (off <= 1e-30 * (dg + 2.0 * off) || off < 1e-300 || (sweep > 0 && off > 0.0625 * prev_off && off <= 1e-26 * (dg + 2.0 * off))) break;
+    prev_off = off;
     for (int r = 0; r < m - 1; ++r) {
       for (int k = wid; k < np; k += nw) {               // columns p, q of pair k (this pair's alone)
         int p, q;

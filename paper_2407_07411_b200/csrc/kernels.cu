@@ -49,7 +49,27 @@ __device__ __forceinline__ void p1_consume(const DevSchedule& d, const P1Unit& u
       if (lane == 0) mbar_arrive(sm.empty(ring.stage));
       ring.advance();
     }
-    if (ROT) {
+    if (ROT && g.N1p > 0) {
+      // operator update, second launch (rotate.cu): "term" t is the slab of 64 rows [64 t, 64 t + 64) of the group's
+      // STACKED first-GEMM results (N1p rows per block, the first g.ldw of them real); row R of the stack belongs to
+      // block R / N1p and goes, transposed, to that block's A' at Seg.p2_off / p2_ld
+      const int pg = frag_perm(lane >> 2), pc = frag_perm(2 * (lane & 3));
+#pragma unroll
+      for (int i = 0; i < MI; ++i) {
+        const int R = t * TILE + w.wr0 + 8 * i + pg;
+        if (R >= g.rows) continue;
+        const int blk = R / g.N1p, a = R - blk * g.N1p;
+        if (a >= g.ldw) continue;
+        const Seg* sg = d.segs + g.seg0 + blk;
+        double* dst = d.rot_dst + sg->p2_off + a;
+#pragma unroll
+        for (int j = 0; j < NJ; ++j) {
+          const int col = w.wc0 + 8 * j + pc;
+          if (col < u.cols_valid) dst[(int64_t)(u.j0 + col) * sg->p2_ld] = acc[i][j][0];
+          if (col + 2 < u.cols_valid) dst[(int64_t)(u.j0 + col + 2) * sg->p2_ld] = acc[i][j][1];
+        }
+      }
+    } else if (ROT) {
       const Seg* sg = d.segs + g.seg0 + t;
       store_tile_t<MI, NJ>(d.rot_dst + sg->p2_off + (int64_t)u.j0 * sg->p2_ld + u.i0, sg->p2_ld, u.rows_valid, u.cols_valid, acc, w, lane);
     } else {
@@ -97,27 +117,30 @@ __global__ void __maxnreg__(136) p1_kernel(DevSchedule d) {
     const double* ybase = d.ws + g.y1_off + (int64_t)yrow0 * g.ldy1;
     const double* xarena = (g.order == 1) ? d.a : d.b;
     const int xboxes = (u.rows_valid + TILE - 1) / TILE;          // 64-row boxes of the X tile that hold valid rows
+    const bool stacked = ROT && g.N1p > 0;                         // "terms" are 64-row slabs of one stacked matrix (see p1_consume)
     for (int t = u.t0; t < u.t1; ++t) {
-      const Seg* sg = d.segs + g.seg0 + t;
+      const Seg* sg = d.segs + g.seg0 + (stacked ? 0 : t);
       const unsigned char* xmap = nullptr;
       const double* xbase = nullptr;
       int64_t xld = 0;
+      const int xrow0 = stacked ? t * TILE : u.i0;
+      const int xrows = stacked ? min(TILE, g.rows - t * TILE) : u.rows_valid;
       if (TMA) {
         xmap = d.maps + (int64_t)sg->p1_map * TMAP_BYTES;
-        if (lane == 0 && t + 2 < u.t1) tma_prefetch_desc(d.maps + (int64_t)sg[2].p1_map * TMAP_BYTES);   // descriptor of the term after next
-      } else { xld = sg->p1_ld; xbase = xarena + sg->p1_off + (int64_t)u.i0 * xld; }
+        if (!stacked && lane == 0 && t + 2 < u.t1) tma_prefetch_desc(d.maps + (int64_t)sg[2].p1_map * TMAP_BYTES);   // descriptor of the term after next
+      } else { xld = sg->p1_ld; xbase = xarena + sg->p1_off + (int64_t)xrow0 * xld; }
       for (int kt = 0; kt < ntiles; ++kt) {
         mbar_wait(sm.empty(ring.stage), ring.phase);
         const uint32_t sx = sm.stage(ring.stage), sy = sx + X_BOXES * OP_BYTES, full = sm.full(ring.stage);
         if (TMA) {
           if (lane == 0) {
             mbar_arrive_expect_tx(full, (xboxes + 1) * OP_BYTES);
-            for (int bx = 0; bx < xboxes; ++bx) tma_load_2d(sx + bx * OP_BYTES, xmap, kt * KT, u.i0 + bx * TILE, full);
+            for (int bx = 0; bx < xboxes; ++bx) tma_load_2d(sx + bx * OP_BYTES, xmap, kt * KT, xrow0 + bx * TILE, full);
             tma_load_2d(sy, ymap, kt * KT, yrow0, full);
           }
         } else {
           for (int bx = 0; bx < xboxes; ++bx)
-            ldgsts_tile(sx + bx * OP_BYTES, xbase + bx * TILE * xld, xld, u.rows_valid - bx * TILE, kt * KT, g.K1, lane);
+            ldgsts_tile(sx + bx * OP_BYTES, xbase + bx * TILE * xld, xld, xrows - bx * TILE, kt * KT, g.K1, lane);
           ldgsts_tile(sy, ybase, g.ldy1, u.cols_valid, kt * KT, g.K1, lane);
           cp_async_mbar_arrive(full);
         }

@@ -61,6 +61,23 @@ int64_t align4(int64_t x) { return (x + 3) & ~(int64_t)3; }
 void add_units(Schedule& sc, int gi, int stages_per_unit) {
   const Group& g = sc.groups[gi];
   const int stages = (g.K1 + KT - 1) / KT;
+  if (g.N1p > 0) {                                   // stacked second launch: "terms" are 64-row slabs, a unit = a range of slabs
+    const int nslab = (g.rows + TILE - 1) / TILE;
+    int ns = std::max(1, std::min(nslab, (stages_per_unit + stages - 1) / stages));
+    const int nchunk = (nslab + ns - 1) / ns;
+    ns = (nslab + nchunk - 1) / nchunk;
+    auto ct = split_cols(g.N1);
+    const int rows_first = std::min(g.rows, TILE);
+    for (int t0 = 0; t0 < nslab; t0 += ns) {
+      const int t1 = std::min(nslab, t0 + ns);
+      for (auto& c : ct) {
+        const int32_t grid = best_grid(frags(rows_first), frags(c.len));
+        sc.p1.push_back({gi, t0, t1, 0, rows_first, c.start, c.len, grid, 0, 0});
+        sc.issued_flops += (int64_t)frags(rows_first) * frags(c.len) * ((g.K1 + 3) / 4) * 512 * (t1 - t0);
+      }
+    }
+    return;
+  }
   int nt = std::max(1, std::min(g.tcount, (stages_per_unit + stages - 1) / stages));
   const int nchunk = (g.tcount + nt - 1) / nt;
   nt = (g.tcount + nchunk - 1) / nchunk;
@@ -165,6 +182,9 @@ int build_rotate(hpsi_rotate* r, int32_t nsec, const int32_t* d, const int32_t* 
     g.ws_off = ws;
     g.ws_map = -1;
     g.src = lp; g.dst = l;
+    // The T_t^T of a group sit one under the other, sector_up(chi_l') rows each (the pad rows stay zero: the workspace is
+    // zeroed at plan time and never written there), so that the second launch can read them as ONE stacked matrix.
+    const int chip = sector_up(chi[lp]);
     for (size_t q = i; q < j; ++q) {
       const hpsi_opblock_t& e = blk[alive[q]];
       Seg sg{};
@@ -174,9 +194,10 @@ int build_rotate(hpsi_rotate* r, int32_t nsec, const int32_t* d, const int32_t* 
       sg.p2_map = -1;
       sg.coef = 1.0;
       tt_off[q] = ws;
-      ws = (ws + (int64_t)chi[lp] * g.ldw + 15) & ~(int64_t)15;
+      ws += (int64_t)chip * g.ldw;
       sc.segs.push_back(sg);
     }
+    ws = (ws + 15) & ~(int64_t)15;
     sc.groups.push_back(g);
     i = j;
   }
@@ -184,21 +205,28 @@ int build_rotate(hpsi_rotate* r, int32_t nsec, const int32_t* d, const int32_t* 
   for (size_t i = 0; i < alive.size();) {
     const size_t j = group_end(i);
     const int l = blk[alive[i]].row, lp = blk[alive[i]].col;
+    // Second launch, STACKED: the group's T_t^T form one matrix of tcount x chip rows (chip = sector_up(chi_l') per block,
+    // chi_l' of them real); a CTA works on 64-row slabs of it - 2 to 3 blocks at once instead of one chi' x chi tile
+    // (~25 x 25, a quarter of a CTA tile) per block - and scatters every row to its block's A' (kernels.cu p1_consume).
+    const int chip = sector_up(chi[lp]);
     Group g{};
     g.order = 2;                          // X operands come from DevSchedule.b, which the update points at the workspace
     g.tcount = (int32_t)(j - i);
     g.seg0 = (int32_t)sc.segs.size();
-    g.rows = chi[lp]; g.K1 = d[l]; g.N1 = chi[l];
-    g.ldw = sector_up(chi[lp]);           // = ld of the output blocks of this group
+    g.rows = g.tcount * chip;             // rows of the stacked matrix
+    g.K1 = d[l]; g.N1 = chi[l];
+    g.N1p = chip;                         // > 0 marks the stacked mode: rows per block ...
+    g.ldw = chi[lp];                      // ... of which this many are real
     g.ldy1 = iso_ld[l]; g.y1_off = iso_off[l]; g.y1_map = iso_map[l];
     g.ws_off = 0; g.ws_map = -1;
     g.src = lp; g.dst = l;
     const int ldt = sector_up(d[l]);
+    const int32_t stack_map = add_map(BASE_WS, tt_off[i], g.rows, d[l], ldt);
     for (size_t q = i; q < j; ++q) {
       const hpsi_opblock_t& o = r->out_blocks[alive[q]];
       Seg sg{};
-      sg.p1_off = tt_off[q]; sg.p1_ld = ldt;
-      sg.p1_map = add_map(BASE_WS, tt_off[q], chi[lp], d[l], ldt);
+      sg.p1_off = tt_off[i]; sg.p1_ld = ldt;            // the stacked matrix (every seg: the kernel reads seg0's)
+      sg.p1_map = stack_map;
       sg.p2_off = o.offset; sg.p2_ld = o.ld;
       sg.p2_map = -1;
       sg.coef = 1.0;
@@ -215,7 +243,8 @@ int build_rotate(hpsi_rotate* r, int32_t nsec, const int32_t* d, const int32_t* 
     int64_t total = 0;
     for (int gi = g0; gi < g1; ++gi) {
       const Group& g = sc.groups[gi];
-      total += (int64_t)split_rows(g.rows).size() * split_cols(g.N1).size() * g.tcount * ((g.K1 + KT - 1) / KT);
+      total += (g.N1p > 0 ? (int64_t)((g.rows + TILE - 1) / TILE) * split_cols(g.N1).size()
+                          : (int64_t)split_rows(g.rows).size() * split_cols(g.N1).size() * g.tcount) * ((g.K1 + KT - 1) / KT);
     }
     const int spu = (int)std::max<int64_t>(12, std::min<int64_t>(96, total / ((int64_t)std::max(n_sm, 1) * 3 * 8)));
     // heaviest groups first
@@ -404,6 +433,24 @@ extern "C" int hpsi_rotate_debug_interpret(const hpsi_rotate_t* r, const double*
       const double* xbase = (g.order == 1) ? a_host : ws;
       double* dst = second ? out_host : ws;
       for (int t = u.t0; t < u.t1; ++t) {
+        if (g.N1p > 0) {                       // stacked second launch: slab t of the stacked T^T, rows scattered to their blocks
+          const Seg& s0 = sc.segs[g.seg0];
+          for (int i = 0; i < TILE; ++i) {
+            const int R = t * TILE + i;
+            if (R >= g.rows) break;
+            const int b = R / g.N1p, a = R - b * g.N1p;
+            if (a >= g.ldw) continue;
+            const Seg& sg = sc.segs[g.seg0 + b];
+            for (int j = 0; j < u.cols_valid; ++j) {
+              const double* xr = xbase + s0.p1_off + (int64_t)R * s0.p1_ld;
+              const double* yr = ws + g.y1_off + (int64_t)(u.j0 + j) * g.ldy1;
+              double s = 0.0;
+              for (int k = 0; k < g.K1; ++k) s += xr[k] * yr[k];
+              dst[sg.p2_off + (int64_t)(u.j0 + j) * sg.p2_ld + a] = s;
+            }
+          }
+          continue;
+        }
         const Seg& sg = sc.segs[g.seg0 + t];
         for (int i = 0; i < u.rows_valid; ++i)
           for (int j = 0; j < u.cols_valid; ++j) {
