@@ -483,6 +483,9 @@ def run_ours(args, rank, world, local_rank):
     if not keep_host:
         p.a_data = p.b_data = None
     t0 = time.time()
+    nv = max(1, args.n_vectors)                               # > 1: batched apply (hpsi_apply_multi), value counts all vectors
+    if nv > 1:
+        plan_kw = dict(plan_kw, n_vectors=nv)
     plan = H.plan_problem(p, a, b, **plan_kw)
     plan_s = time.time() - t0
     q = lambda w: H.hpsi_query(plan, w)  # noqa: E731
@@ -492,6 +495,7 @@ def run_ours(args, rank, world, local_rank):
     if world > 1:
         dist.all_reduce(sums)
     useful_flops, operator_bytes, n_tasks, arena_total = (int(v) for v in sums.tolist())
+    useful_flops *= nv                                        # one step = H psi_v for every vector of the batch
     log(f"[rank {rank}] {cfg}: gen {gen_s:.1f}s plan {plan_s:.2f}s tasks {q(H.HPSI_Q_N_TASKS)} "
         f"useful {q(H.HPSI_Q_USEFUL_FLOPS) / 1e9:.1f} GF issued {q(H.HPSI_Q_ISSUED_FLOPS) / 1e9:.1f} GF "
         f"operators {q(H.HPSI_Q_OPERATOR_BYTES) / 1e9:.2f} GB workspace {q(H.HPSI_Q_WORKSPACE_BYTES) / 1e9:.2f} GB")
@@ -502,12 +506,20 @@ def run_ours(args, rank, world, local_rank):
 
     stream = torch.cuda.current_stream()
     n_psi = 10 if cfg == "femoco" else 1                      # A17: 10 different psi's for the FeMoco config
-    psis = [torch.from_numpy(workloads.make_psi(p, k)).to(dev) for k in range(n_psi)]
-    out = torch.empty(n, dtype=torch.float64, device=dev)
+    if nv > 1:
+        assert world == 1, "--n-vectors is a single-GPU measurement"
+        psis = [torch.from_numpy(np.stack([workloads.make_psi(p, k * nv + v) for v in range(nv)])).to(dev) for k in range(n_psi)]
+        out = torch.empty(nv * n, dtype=torch.float64, device=dev)
+    else:
+        psis = [torch.from_numpy(workloads.make_psi(p, k)).to(dev) for k in range(n_psi)]
+        out = torch.empty(n, dtype=torch.float64, device=dev)
     parts = torch.empty(world * n, dtype=torch.float64, device=dev) if world > 1 else None
     mine = parts[rank * n:(rank + 1) * n] if world > 1 else out
 
     def step(i):
+        if nv > 1:
+            H.hpsi_apply_multi(plan, psis[i % n_psi], out, nv, stream)
+            return
         H.hpsi_apply(plan, psis[i % n_psi], mine, stream)
         if world > 1:                                         # exchange step: all-gather + rank-ordered sum
             dist.all_gather_into_tensor(parts, mine)
@@ -556,12 +568,17 @@ def run_ours(args, rank, world, local_rank):
         apply_ms = [x / args.steps for x in per_rank_apply]
 
     # ---- end to end: pinned HOST psi / out, H2D + D2H inside the timed region
-    hpsi_in = [torch.from_numpy(workloads.make_psi(p, k)).pin_memory() for k in range(n_psi)]
-    hout = torch.empty(n, dtype=torch.float64).pin_memory()
-    xdev = torch.empty(n, dtype=torch.float64, device=dev)
+    hpsi_in = [(psis[k].cpu() if nv > 1 else torch.from_numpy(workloads.make_psi(p, k))).pin_memory() for k in range(n_psi)]
+    hout = torch.empty(nv * n, dtype=torch.float64).pin_memory()
+    xdev = torch.empty(nv * n, dtype=torch.float64, device=dev)
 
     def e2e_step(i):
-        if world == 1:
+        if nv > 1:                                            # no host-buffer entry point for a batch: copies + hpsi_apply_multi
+            xdev.copy_(hpsi_in[i % n_psi].reshape(-1), non_blocking=True)
+            H.hpsi_apply_multi(plan, xdev, out, nv, stream)
+            hout.copy_(out, non_blocking=True)
+            torch.cuda.synchronize()
+        elif world == 1:
             H.hpsi_apply_host(plan, hpsi_in[i % n_psi], hout, stream)       # the C-ABI call with HOST buffers
         else:
             xdev.copy_(hpsi_in[i % n_psi], non_blocking=True)
@@ -578,8 +595,8 @@ def run_ours(args, rank, world, local_rank):
 
     # ---- roofline of the dominant kernel (live CUDA events between the kernels of an apply)
     prof = np.zeros(4)
-    for i in range(3):
-        prof += np.array(H.hpsi_apply_profiled(plan, psis[0], mine, stream))
+    for i in range(3):                                        # (one vector's worth of work, also for a batched plan)
+        prof += np.array(H.hpsi_apply_profiled(plan, psis[0][:n] if nv > 1 else psis[0], mine[:n], stream))
     prof /= 3
     names = ["prep_kernel", "p1_kernel (first GEMM)", "p2_kernel (second GEMM)", "reduce_kernel"]
     fl_p1 = q(H.HPSI_Q_USEFUL_FLOPS_P1)
@@ -616,10 +633,11 @@ def run_ours(args, rank, world, local_rank):
                    "l2": "inputs larger than L2 (operators streamed once per step)",
                    "operator_storage": "adjoint terms share their partner's blocks (read transposed)" if args.share_adjoint
                    else "every block materialised", "operator_arena_bytes": arena_total,
-                   "schedule": dict(zip(("p1_stages_per_unit", "p2_waves", "p2_min_unit_dmma"), q(H.HPSI_Q_TUNING)))},
+                   "schedule": dict(zip(("p1_stages_per_unit", "p2_waves", "p2_min_unit_dmma"), q(H.HPSI_Q_TUNING))),
+                   "vectors_per_step": nv},
         "calibration": {"fp64_tc_peak_tflops": dgemm_peak, **calib},
         "clocks": clk.summary(),
-        "e2e": {"value": e2e_value, "unit": "TFLOPS", "h2d_bytes_per_step": 8 * n * world, "d2h_bytes_per_step": 8 * n * world},
+        "e2e": {"value": e2e_value, "unit": "TFLOPS", "h2d_bytes_per_step": 8 * n * world * nv, "d2h_bytes_per_step": 8 * n * world * nv},
         "gpu_launches": (int(q(H.HPSI_Q_LAUNCHES_PER_APPLY)) + (1 if world > 1 else 0)) * args.steps * world,
         "roofline": roofline,
     }
@@ -635,7 +653,9 @@ def run_ours(args, rank, world, local_rank):
     if rank == 0:
         sl, sx, sy, idx = sample_points(p, 32)
         psi0 = workloads.make_psi(p, 0)
-        got = out.cpu().numpy()[idx]
+        got = out.cpu().numpy()[idx]                    # (batched: the first vector of the batch)
+        if nv > 1:
+            psi0 = psis[0][0].cpu().numpy()
         del a, b
         if keep_host:
             import oracle
@@ -758,6 +778,8 @@ def main():
                     help="override the config's bond dimension per side (sweep over D as in the paper's Fig. 1-2; 1 GPU)")
     ap.add_argument("--site-update", action="store_true",
                     help="time the steps after the eigen-solve instead: hpsi_truncate + hpsi_rotate_apply (SURVEY 8(f)-4)")
+    ap.add_argument("--n-vectors", type=int, default=1,
+                    help="batched apply: hpsi_apply_multi on this many vectors per step (plan built with n_vectors; 1 GPU)")
     ap.add_argument("--davidson", action="store_true",
                     help="time the eigensolver drivers (hpsi_davidson, hpsi_lanczos) and their overhead over a bare hpsi_apply")
     args = ap.parse_args()

@@ -459,13 +459,17 @@ int build_schedule(const hpsi_sectors_t* s, const hpsi_terms_t* t, uint32_t flag
       for (int pass = 0; pass < 2; ++pass) total_cost[pass] += di.cost[pass] * (int64_t)(di.rt.size() * di.ct.size());
     }
   }
-  const int waves = opt.p2_waves > 0 ? opt.p2_waves : 48;
+  // Fewer waves for smaller problems: the partials a launch writes (and reduce_kernel reads back) grow with the number of
+  // units, not with the problem - 48 waves are ~0.9 GB whatever D is, 0.14 ms of a 2.7 ms apply at D = 2048 (measured
+  // there: 12-24 waves 25.3-25.7 TFLOPS, 48 waves 24.7; at D = 4096 48 waves are still best).
+  const int auto_waves = (int)std::max<int64_t>(8, std::min<int64_t>(48, total_cost[0] / 3400000));
+  const int waves = opt.p2_waves > 0 ? opt.p2_waves : auto_waves;
   // 4 resident CTAs per SM, ~48 waves: small units keep the tail of the launch short and the operand segments of a
   // (block, K-chunk) bundle L2-resident while its tiles pass over them.  Measured A/B/A/B on B200, 32 -> 48 waves:
   // cyp 31.6 -> 32.0 TFLOPS, stress 32.2 -> 32.5, femoco 31.7 -> 32.0, small unchanged (p2 -2 %, reduce +0.035 ms);
   // 64 waves gain nothing more (the ordered reduce grows as fast as p2 shrinks).
   const int64_t slots = std::max<int64_t>(1, (int64_t)std::max(n_sm, 1) * 4 * waves / nvec);   // every unit exists once per vector
-  const int64_t min_target = opt.p2_min_unit_dmma > 0 ? opt.p2_min_unit_dmma : 1536;   // DMMA per unit at least (~10 us of a CTA)
+  const int64_t min_target = opt.p2_min_unit_dmma > 0 ? opt.p2_min_unit_dmma : 3072;   // DMMA per unit at least (~20 us of a CTA; D = 1024: 17.9 -> 18.9 TFLOPS against 1536)
   sc->tuning[1] = waves;
   sc->tuning[2] = min_target;
   const int64_t target_of[2] = {std::max<int64_t>(min_target, total_cost[0] / slots),

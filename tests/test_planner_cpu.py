@@ -66,7 +66,7 @@ def test_plan_options_change_the_schedule_not_the_result(small):
     ref = oracle.apply(small, psi)
     base = host_plan(small)
     t0 = H.hpsi_query(base, H.HPSI_Q_TUNING)
-    assert t0[1] == 48 and t0[2] == 1536 and 12 <= t0[0] <= 96
+    assert 8 <= t0[1] <= 48 and t0[2] == 3072 and 12 <= t0[0] <= 96
     for kw in (dict(p1_stages_per_unit=7), dict(p2_waves=3), dict(p2_min_unit_dmma=200000), dict(p1_stages_per_unit=500, p2_waves=100)):
         plan = H.plan_problem(small, flags=H.HPSI_PLAN_HOST_ONLY, **kw)
         t = H.hpsi_query(plan, H.HPSI_Q_TUNING)
