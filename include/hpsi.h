@@ -233,11 +233,16 @@ int hpsi_lanczos(hpsi_plan_t* plan, double* psi_inout_dev, double* eig_host,
 
 /* Operator streaming from HOST memory ("host-device datacommunication ... due to memory
  * limitations"): for operators that do not fit HBM.  terms->a_data / b_data are pinned HOST arenas here
- * (BORROWED, must outlive the object).  The term list is cut into windows of consecutive terms whose arena ranges fit
- * `window_doubles` (A + B together); the object owns two device staging slots of that size and one plan per window.
- * hpsi_stream_apply copies window w+1 on an internal copy stream while window w computes on `cuda_stream`; the windows'
- * results add up in window order (deterministic).  out = H psi (overwrite); psi_dev / out_dev: DEVICE.  Enqueue only,
- * but uses a second stream and events, so it is not CUDA-graph capturable.  Transposed blocks are not supported. */
+ * (BORROWED, must outlive the object).  The term list is cut, in the order of the terms' arena positions, into windows
+ * whose arena ranges fit `window_doubles` (A + B together); the object owns two device staging slots of that size and one
+ * plan per window.  hpsi_stream_apply copies window w+1 on an internal copy stream while window w computes on
+ * `cuda_stream`; the windows' results add up in window order (deterministic).  out = H psi (overwrite); psi_dev /
+ * out_dev: DEVICE.  Enqueue only, but uses a second stream and events, so it is not CUDA-graph capturable.
+ * Blocks stored transposed (a_transposed / b_transposed) are supported: an adjoint term that reads its partner's storage
+ * lands in its partner's window, so with shared adjoint storage every operator byte crosses the host link once per apply
+ * - half the bytes of the materialised form, the one "compression" a Hermitian H offers without touching the FP64
+ * entries (PAPER.md:84 names "data compression techniques" without giving one; synthetic N(0,1) entries have no other
+ * redundancy). */
 typedef struct hpsi_stream hpsi_stream_t;
 int hpsi_stream_create(const hpsi_sectors_t* sectors, const hpsi_terms_t* terms_with_host_arenas, int64_t window_doubles,
                        uint32_t flags, hpsi_stream_t** out);

@@ -368,6 +368,13 @@ def hpsi_stream_create(p, a_host, b_host, window_doubles: int, flags: int = 0) -
     trm = hpsi_terms_t(coef.shape[0], coef.ctypes.data, a_blocks.shape[0], a_blocks.ctypes.data,
                        b_blocks.shape[0], b_blocks.ctypes.data, _ptr(a_host), _ptr(b_host), int(p.a_len), int(p.b_len),
                        None, None)
+    a_tr, b_tr = getattr(p, "a_trans", None), getattr(p, "b_trans", None)
+    if a_tr is not None:
+        a_tr = np.ascontiguousarray(a_tr, np.uint8)
+        trm.a_transposed = a_tr.ctypes.data
+    if b_tr is not None:
+        b_tr = np.ascontiguousarray(b_tr, np.uint8)
+        trm.b_transposed = b_tr.ctypes.data
     out = ctypes.c_void_p()
     _check(lib().hpsi_stream_create(ctypes.byref(sec), ctypes.byref(trm), int(window_doubles), flags, ctypes.byref(out)))
     return StreamPlan(out.value, (a_host, b_host))

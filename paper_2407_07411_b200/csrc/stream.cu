@@ -49,25 +49,25 @@ extern "C" int hpsi_stream_create(const hpsi_sectors_t* sectors, const hpsi_term
   if (flags & HPSI_PLAN_HOST_ONLY) { set_error("a streamed plan needs a device"); return HPSI_EINVAL; }
   if (!terms->a_data || !terms->b_data) { set_error("hpsi_stream_create needs the HOST arenas"); return HPSI_EINVAL; }
   if (window_doubles < 2) { set_error("window too small"); return HPSI_EINVAL; }
-  if (terms->a_transposed || terms->b_transposed) { set_error("transposed blocks are not supported in streamed plans"); return HPSI_EINVAL; }
   const int T = terms->n_terms;
   // arena range of every term (its blocks need not be contiguous; the range is what gets copied)
   struct Range { int64_t a_lo, a_hi, b_lo, b_hi; };
   std::vector<Range> rg(T, Range{INT64_MAX, 0, INT64_MAX, 0});
-  auto extent = [&](const hpsi_opblock_t& e, const int32_t* d, int nsec) -> int64_t {
+  auto extent = [&](const hpsi_opblock_t& e, const int32_t* d, int nsec, bool tr) -> int64_t {
     if (e.row < 0 || e.row >= nsec || e.col < 0 || e.col >= nsec) return -1;
-    return e.offset + (int64_t)(d[e.row] - 1) * e.ld + d[e.col];
+    const int64_t srows = tr ? d[e.col] : d[e.row], scols = tr ? d[e.row] : d[e.col];     // a transposed block stores d[col] x d[row]
+    return e.offset + (srows - 1) * e.ld + scols;
   };
   for (int64_t i = 0; i < terms->n_a; ++i) {
     const hpsi_opblock_t& e = terms->a_blocks[i];
-    const int64_t hi = extent(e, sectors->d_left, sectors->n_left);
+    const int64_t hi = extent(e, sectors->d_left, sectors->n_left, terms->a_transposed && terms->a_transposed[i]);
     if (e.term < 0 || e.term >= T || hi < 0 || e.offset < 0) { set_error("bad A block descriptor"); return HPSI_EINVAL; }
     rg[e.term].a_lo = std::min(rg[e.term].a_lo, e.offset & ~(int64_t)3);      // keep 32-byte alignment of the rows
     rg[e.term].a_hi = std::max(rg[e.term].a_hi, hi);
   }
   for (int64_t i = 0; i < terms->n_b; ++i) {
     const hpsi_opblock_t& e = terms->b_blocks[i];
-    const int64_t hi = extent(e, sectors->d_right, sectors->n_right);
+    const int64_t hi = extent(e, sectors->d_right, sectors->n_right, terms->b_transposed && terms->b_transposed[i]);
     if (e.term < 0 || e.term >= T || hi < 0 || e.offset < 0) { set_error("bad B block descriptor"); return HPSI_EINVAL; }
     rg[e.term].b_lo = std::min(rg[e.term].b_lo, e.offset & ~(int64_t)3);
     rg[e.term].b_hi = std::max(rg[e.term].b_hi, hi);
@@ -76,30 +76,43 @@ extern "C" int hpsi_stream_create(const hpsi_sectors_t* sectors, const hpsi_term
   if (!s) { set_error("out of host memory"); return HPSI_ENOMEM; }
   s->a_host = terms->a_data;
   s->b_host = terms->b_data;
-  // windows of consecutive terms whose A + B ranges fit window_doubles
+  // windows of terms whose A + B ranges fit window_doubles.  The terms are taken in the order of their arena position
+  // (ties: term number), so that terms which share storage - an adjoint reading its partner's blocks transposed - fall
+  // into the same window and their bytes cross the host link once.  `order[cuts[w].first .. cuts[w].second)` = window w.
+  std::vector<int> order(T);
+  for (int t = 0; t < T; ++t) order[t] = t;
+  std::stable_sort(order.begin(), order.end(), [&](int x, int y) {
+    if (rg[x].a_lo != rg[y].a_lo) return rg[x].a_lo < rg[y].a_lo;
+    return rg[x].b_lo < rg[y].b_lo;
+  });
   std::vector<std::pair<int, int>> cuts;
   {
     int t0 = 0;
     Range cur{INT64_MAX, 0, INT64_MAX, 0};
     auto size = [](const Range& r) { return std::max<int64_t>(0, r.a_hi - std::min(r.a_lo, r.a_hi)) + std::max<int64_t>(0, r.b_hi - std::min(r.b_lo, r.b_hi)); };
-    for (int t = 0; t < T; ++t) {
-      Range nx{std::min(cur.a_lo, rg[t].a_lo), std::max(cur.a_hi, rg[t].a_hi), std::min(cur.b_lo, rg[t].b_lo), std::max(cur.b_hi, rg[t].b_hi)};
-      if (size(nx) > window_doubles && t > t0) {
-        cuts.push_back({t0, t});
-        t0 = t;
-        nx = rg[t];
+    for (int i = 0; i < T; ++i) {
+      const Range& rt = rg[order[i]];
+      Range nx{std::min(cur.a_lo, rt.a_lo), std::max(cur.a_hi, rt.a_hi), std::min(cur.b_lo, rt.b_lo), std::max(cur.b_hi, rt.b_hi)};
+      if (size(nx) > window_doubles && i > t0) {
+        cuts.push_back({t0, i});
+        t0 = i;
+        nx = rt;
       }
       if (size(nx) > window_doubles) { set_error("one term's blocks do not fit the window"); hpsi_stream_destroy(s); return HPSI_EINVAL; }
       cur = nx;
     }
     if (T > t0 || T == 0) cuts.push_back({t0, T});
   }
+  std::vector<int> window_of(T, 0);
+  for (size_t w = 0; w < cuts.size(); ++w)
+    for (int i = cuts[w].first; i < cuts[w].second; ++i) window_of[order[i]] = (int)w;
   int rc = HPSI_OK;
   auto fail = [&](int code) { hpsi_stream_destroy(s); return code; };
   // staging capacity = the largest window of each side
   std::vector<Range> wr(cuts.size(), Range{INT64_MAX, 0, INT64_MAX, 0});
   for (size_t w = 0; w < cuts.size(); ++w)
-    for (int t = cuts[w].first; t < cuts[w].second; ++t) {
+    for (int i = cuts[w].first; i < cuts[w].second; ++i) {
+      const int t = order[i];
       wr[w].a_lo = std::min(wr[w].a_lo, rg[t].a_lo); wr[w].a_hi = std::max(wr[w].a_hi, rg[t].a_hi);
       wr[w].b_lo = std::min(wr[w].b_lo, rg[t].b_lo); wr[w].b_hi = std::max(wr[w].b_hi, rg[t].b_hi);
     }
@@ -122,19 +135,24 @@ extern "C" int hpsi_stream_create(const hpsi_sectors_t* sectors, const hpsi_term
   // one plan per window: only that window's blocks, offsets rebased to the staging slot
   for (size_t w = 0; w < cuts.size(); ++w) {
     std::vector<hpsi_opblock_t> ab, bb;
+    std::vector<uint8_t> atr, btr;
     for (int64_t i = 0; i < terms->n_a; ++i)
-      if (terms->a_blocks[i].term >= cuts[w].first && terms->a_blocks[i].term < cuts[w].second) {
+      if (window_of[terms->a_blocks[i].term] == (int)w) {
         ab.push_back(terms->a_blocks[i]);
         ab.back().offset -= wr[w].a_lo;
+        atr.push_back(terms->a_transposed ? terms->a_transposed[i] : 0);
       }
     for (int64_t i = 0; i < terms->n_b; ++i)
-      if (terms->b_blocks[i].term >= cuts[w].first && terms->b_blocks[i].term < cuts[w].second) {
+      if (window_of[terms->b_blocks[i].term] == (int)w) {
         bb.push_back(terms->b_blocks[i]);
         bb.back().offset -= wr[w].b_lo;
+        btr.push_back(terms->b_transposed ? terms->b_transposed[i] : 0);
       }
     hpsi_terms_t sub = *terms;
     sub.n_a = (int64_t)ab.size(); sub.a_blocks = ab.data();
     sub.n_b = (int64_t)bb.size(); sub.b_blocks = bb.data();
+    sub.a_transposed = terms->a_transposed ? atr.data() : nullptr;
+    sub.b_transposed = terms->b_transposed ? btr.data() : nullptr;
     double* slot = s->stage[w & 1];
     sub.a_data = slot; sub.b_data = slot + s->a_cap;
     sub.a_len = s->a_cap; sub.b_len = s->b_cap;

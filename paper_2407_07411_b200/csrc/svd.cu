@@ -81,8 +81,8 @@ __device__ __forceinline__ double warp_sum(double v) {
 
 constexpr int SV_B = 16;             // rows per chunk
 constexpr int SV_M = 2 * SV_B;       // rows one CTA orthogonalises per visit (a chunk pair)
-constexpr int SV_KC = 32;            // columns of the psi part staged per Gram step
-constexpr int SV_THREADS = 256;
+constexpr int SV_KC = 32;            // columns of the psi part staged per Gram step (512 threads x 2 doubles)
+constexpr int SV_THREADS = 512;      // 16 warps: one Gram fragment, one row pair of a rotation step, one (row half, column block) each
 
 __device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double b) {
   asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
@@ -101,11 +101,13 @@ struct SvdSmem {
 //   1. G = X_psi X_psi^T for the 32 rows of the chunk pair (DMMA, the rows streamed once through shared memory);
 //   2. one cyclic pass of plane rotations over the row pairs of the visit, applied to G from both sides (32-long vectors
 //      in shared memory instead of the rows themselves) and accumulated in Q - same pairs, same order, same rotation
-//      formula and threshold as rotating the rows one pair at a time;
+//      formula and threshold as rotating the rows one pair at a time.  One warp per pair: the chain square root ->
+//      division -> reciprocal square root of a rotation is ~600 clk, and 16 (cross pairs) or 31 (all pairs) such steps
+//      in sequence are the critical path of a visit;
 //   3. X <- Q X over all L columns (DMMA, every element read and written once).
 // Shared-memory traffic per visit drops from ~93 passes over the 32 rows (31 inner rounds x 3) to 2 passes through
-// global memory / L2; measured on cyp: 9.7 ms -> see DESIGN.md section 9.
-__global__ void __launch_bounds__(SV_THREADS) svd_round_kernel(const SvdBlk* __restrict__ blk, const int32_t* __restrict__ cta_blk,
+// global memory / L2.
+__global__ void __launch_bounds__(SV_THREADS, 2) svd_round_kernel(const SvdBlk* __restrict__ blk, const int32_t* __restrict__ cta_blk,
                                                                int round, double* __restrict__ w, int* __restrict__ flag) {
   __shared__ SvdSmem sm;
   const SvdBlk B = blk[cta_blk[blockIdx.x]];
@@ -128,44 +130,38 @@ __global__ void __launch_bounds__(SV_THREADS) svd_round_kernel(const SvdBlk* __r
     return w + B.w_off + (int64_t)row * L;
   };
 
-  // ---- 1. Gram matrix: warp wid owns fragments (i, j) = (wid / 2, 2 (wid % 2) + {0, 1}) of the 4 x 4 grid of 8 x 8 fragments
+  // ---- 1. Gram matrix: warp wid owns fragment (i, j) = (wid / 4, wid % 4) of the 4 x 4 grid of 8 x 8 fragments
   {
-    const int fi = wid >> 1, fj = (wid & 1) * 2;
-    double acc[2][2] = {{0.0, 0.0}, {0.0, 0.0}};
-    const int lrow = tid >> 3, lc = (tid & 7) * 4;       // this thread stages 4 consecutive columns of one row
+    const int fi = wid >> 2, fj = wid & 3;
+    double acc0 = 0.0, acc1 = 0.0;
+    const int lrow = tid >> 4, lc = (tid & 15) * 2;      // this thread stages 2 consecutive columns of one row
     const bool lvalid = valid(lrow);
     const double* lsrc = grow(lrow);
-    double v[4];
+    double v0, v1;
     auto fetch = [&](int kc) {
-#pragma unroll
-      for (int e = 0; e < 4; ++e) { const int c = kc + lc + e; v[e] = (lvalid && c < B.vlen) ? lsrc[c] : 0.0; }
+      const int c = kc + lc;
+      v0 = (lvalid && c < B.vlen) ? lsrc[c] : 0.0;
+      v1 = (lvalid && c + 1 < B.vlen) ? lsrc[c + 1] : 0.0;
     };
     const int nchunk = (B.vlen + SV_KC - 1) / SV_KC;
     fetch(0);
     for (int ch = 0; ch < nchunk; ++ch) {
       double (*st)[SV_KC + 4] = sm.stage[ch & 1];
-#pragma unroll
-      for (int e = 0; e < 4; ++e) st[lrow][lc + e] = v[e];
+      st[lrow][lc] = v0;
+      st[lrow][lc + 1] = v1;
       __syncthreads();                                   // chunk ch staged; everybody is past the DMMAs of chunk ch - 2
       if (ch + 1 < nchunk) fetch((ch + 1) * SV_KC);
 #pragma unroll
-      for (int ks = 0; ks < SV_KC / 4; ++ks) {
-        const double a = st[8 * fi + g][4 * ks + q];
-        const double b0 = st[8 * fj + g][4 * ks + q], b1 = st[8 * fj + 8 + g][4 * ks + q];
-        dmma884(acc[0][0], acc[0][1], a, b0);
-        dmma884(acc[1][0], acc[1][1], a, b1);
-      }
+      for (int ks = 0; ks < SV_KC / 4; ++ks)
+        dmma884(acc0, acc1, st[8 * fi + g][4 * ks + q], st[8 * fj + g][4 * ks + q]);
     }
-#pragma unroll
-    for (int f = 0; f < 2; ++f) {
-      sm.G[8 * fi + g][8 * (fj + f) + 2 * q] = acc[f][0];
-      sm.G[8 * fi + g][8 * (fj + f) + 2 * q + 1] = acc[f][1];
-    }
+    sm.G[8 * fi + g][8 * fj + 2 * q] = acc0;
+    sm.G[8 * fi + g][8 * fj + 2 * q + 1] = acc1;
     for (int e = tid; e < SV_M * SV_M; e += SV_THREADS) sm.Q[e >> 5][e & 31] = ((e >> 5) == (e & 31)) ? 1.0 : 0.0;
   }
   __syncthreads();
 
-  // ---- 2. one pass over the row pairs of the visit, on G (two-sided) and Q
+  // ---- 2. one pass over the row pairs of the visit, on G (two-sided) and Q: warp wid = pair wid of the step
   // rotate when |<x_p,x_q>| > tol |x_p||x_q| with tol = cols * 2^-53, the threshold LAPACK's Jacobi SVD (dgesvj) uses:
   // a dot product of `cols` terms cannot resolve angles below ~sqrt(cols) * 2^-53, and a tighter test only makes
   // rounding noise trigger further sweeps
@@ -174,90 +170,80 @@ __global__ void __launch_bounds__(SV_THREADS) svd_round_kernel(const SvdBlk* __r
   const int np = SV_M - 1;
   const int inner = full ? np : SV_B;
   for (int s = 0; s < inner; ++s) {
-#pragma unroll
-    for (int h = 0; h < 2; ++h) {                        // 16 pairs per step, two per warp
-      const int pp = wid + 8 * h;
-      int p, qq;
-      if (full) {
-        if (pp == 0) { p = np; qq = s; }
-        else { p = (s + pp) % np; qq = (s - pp + np) % np; }
-      } else {
-        p = pp; qq = SV_B + (pp + s) % SV_B;
-      }
-      double cs = 1.0, sn = 0.0;
-      if (valid(p) && valid(qq)) {
-        const double a = sm.G[p][p], b = sm.G[qq][qq], gg = sm.G[p][qq];
-        if (a > B.floor2 && b > B.floor2 && gg * gg > tol * tol * a * b) {
-          // tan of the smaller rotation angle: t = sign(zeta) / (|zeta| + sqrt(1 + zeta^2)) with zeta = (b - a) / 2g
-          const double d = b - a;
-          const double t = 2.0 * gg / (d + copysign(sqrt(d * d + 4.0 * gg * gg), d));
-          cs = rsqrt(1.0 + t * t);
-          sn = cs * t;
-          ++rotated;
-        }
-      }
-      __syncwarp();
-      if (lane == 0) { sm.cs[pp][0] = cs; sm.cs[pp][1] = sn; }
-      if (sn != 0.0) {                                   // rows p, q of G and of Q (this pair's alone)
-        const double gp = sm.G[p][lane], gq = sm.G[qq][lane];
-        sm.G[p][lane] = cs * gp - sn * gq;
-        sm.G[qq][lane] = sn * gp + cs * gq;
-        const double qp = sm.Q[p][lane], qv = sm.Q[qq][lane];
-        sm.Q[p][lane] = cs * qp - sn * qv;
-        sm.Q[qq][lane] = sn * qp + cs * qv;
+    int p, qq;
+    if (full) {
+      if (wid == 0) { p = np; qq = s; }
+      else { p = (s + wid) % np; qq = (s - wid + np) % np; }
+    } else {
+      p = wid; qq = SV_B + (wid + s) % SV_B;
+    }
+    double cs = 1.0, sn = 0.0;
+    if (valid(p) && valid(qq)) {
+      const double a = sm.G[p][p], b = sm.G[qq][qq], gg = sm.G[p][qq];
+      if (a > B.floor2 && b > B.floor2 && gg * gg > tol * tol * a * b) {
+        // tan of the smaller rotation angle: t = sign(zeta) / (|zeta| + sqrt(1 + zeta^2)) with zeta = (b - a) / 2g
+        const double d = b - a;
+        const double t = 2.0 * gg / (d + copysign(sqrt(d * d + 4.0 * gg * gg), d));
+        cs = rsqrt(1.0 + t * t);
+        sn = cs * t;
+        ++rotated;
       }
     }
+    __syncwarp();
+    if (lane == 0) { sm.cs[wid][0] = cs; sm.cs[wid][1] = sn; }
+    if (sn != 0.0) {                                     // rows p, q of G and of Q (this pair's alone)
+      const double gp = sm.G[p][lane], gq = sm.G[qq][lane];
+      sm.G[p][lane] = cs * gp - sn * gq;
+      sm.G[qq][lane] = sn * gp + cs * gq;
+      const double qp = sm.Q[p][lane], qv = sm.Q[qq][lane];
+      sm.Q[p][lane] = cs * qp - sn * qv;
+      sm.Q[qq][lane] = sn * qp + cs * qv;
+    }
     __syncthreads();
-#pragma unroll
-    for (int h = 0; h < 2; ++h) {                        // columns p, q of G
-      const int pp = wid + 8 * h;
-      int p, qq;
-      if (full) {
-        if (pp == 0) { p = np; qq = s; }
-        else { p = (s + pp) % np; qq = (s - pp + np) % np; }
-      } else {
-        p = pp; qq = SV_B + (pp + s) % SV_B;
-      }
-      const double cs = sm.cs[pp][0], sn = sm.cs[pp][1];
-      if (sn != 0.0) {
-        const double gp = sm.G[lane][p], gq = sm.G[lane][qq];
-        sm.G[lane][p] = cs * gp - sn * gq;
-        sm.G[lane][qq] = sn * gp + cs * gq;
-      }
+    if (sn != 0.0) {                                     // columns p, q of G (same warp: its cs / sn are still in registers)
+      const double gp = sm.G[lane][p], gq = sm.G[lane][qq];
+      sm.G[lane][p] = cs * gp - sn * gq;
+      sm.G[lane][qq] = sn * gp + cs * gq;
     }
     __syncthreads();
   }
   const int any = __syncthreads_or(rotated);
   if (!any) return;                                      // nothing rotated: the rows stay as they are
 
-  // ---- 3. X <- Q X over all L columns: warp wid owns the 8-column blocks wid, wid + 8, ...
-  double qa[4][SV_M / 4];                                // A fragments of Q: row block i, k-step ks
+  // ---- 3. X <- Q X over all L columns: warp wid owns row blocks 2h, 2h+1 (h = wid / 8) of the 8-column blocks
+  // wid % 8, wid % 8 + 8, ...
+  const int h = wid >> 3, wc = wid & 7;
+  double qa[2][SV_M / 4];                                // A fragments of Q: row block 2h + i, k-step ks
 #pragma unroll
-  for (int i = 0; i < 4; ++i)
+  for (int i = 0; i < 2; ++i)
 #pragma unroll
-    for (int ks = 0; ks < SV_M / 4; ++ks) qa[i][ks] = sm.Q[8 * i + g][4 * ks + q];
+    for (int ks = 0; ks < SV_M / 4; ++ks) qa[i][ks] = sm.Q[8 * (2 * h + i) + g][4 * ks + q];
   const double* brow[SV_M / 4];                          // row 4 ks + q of the visit (B fragment: k = q, n = g)
   bool bval[SV_M / 4];
 #pragma unroll
   for (int ks = 0; ks < SV_M / 4; ++ks) { bval[ks] = valid(4 * ks + q); brow[ks] = grow(4 * ks + q); }
-  for (int col0 = 8 * wid; col0 < L; col0 += 64) {
+  // The two warps that share a column block (wid and wid ^ 8) read all 32 rows of it and write 16 each, so both must have
+  // read before either writes: a named barrier of those 64 threads between the loads and the stores.
+  const int nblk = (L + 7) / 8, nround = (nblk + 7) / 8;
+  for (int rd = 0; rd < nround; ++rd) {
+    const int col0 = 8 * (wc + 8 * rd);
     double bf[SV_M / 4];
     const bool cok = col0 + g < L;
 #pragma unroll
     for (int ks = 0; ks < SV_M / 4; ++ks) bf[ks] = (bval[ks] && cok) ? brow[ks][col0 + g] : 0.0;
-    double acc[4][2];
-#pragma unroll
-    for (int i = 0; i < 4; ++i) acc[i][0] = acc[i][1] = 0.0;
+    double acc[2][2] = {{0.0, 0.0}, {0.0, 0.0}};
 #pragma unroll
     for (int ks = 0; ks < SV_M / 4; ++ks)
 #pragma unroll
-      for (int i = 0; i < 4; ++i) dmma884(acc[i][0], acc[i][1], qa[i][ks], bf[ks]);
-    __syncwarp();                                        // every lane has read its part of the column block
+      for (int i = 0; i < 2; ++i) dmma884(acc[i][0], acc[i][1], qa[i][ks], bf[ks]);
+    asm volatile("bar.sync %0, 64;\n" ::"r"(1 + wc) : "memory");   // the two warps of this column block have both read it
     const int c = col0 + 2 * q;
     if (c < L) {                                         // L is even: the pair (c, c + 1) is inside the row or outside it
 #pragma unroll
-      for (int i = 0; i < 4; ++i)
-        if (valid(8 * i + g)) *reinterpret_cast<double2*>(grow(8 * i + g) + c) = make_double2(acc[i][0], acc[i][1]);
+      for (int i = 0; i < 2; ++i) {
+        const int slot = 8 * (2 * h + i) + g;
+        if (valid(slot)) *reinterpret_cast<double2*>(grow(slot) + c) = make_double2(acc[i][0], acc[i][1]);
+      }
     }
   }
   if (lane == 0 && rotated) atomicAdd(flag, rotated);    // rotations of the sweep (control only, not data)
