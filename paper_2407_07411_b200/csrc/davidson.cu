@@ -134,10 +134,12 @@ __device__ void small_eig_block(const double* __restrict__ G, int j, double* the
         if (q < j) {                                     // not the dummy player
           const double apq = sm.A[p][q];
           if (fabs(apq) >= 1e-300) {
-            const double app = sm.A[p][p], aqq = sm.A[q][q];
-            const double tau = (aqq - app) / (2.0 * apq);
-            const double tt = (tau >= 0 ? 1.0 : -1.0) / (fabs(tau) + sqrt(1.0 + tau * tau));
-            c = 1.0 / sqrt(1.0 + tt * tt);
+            // tan of the smaller rotation angle, t = sign(tau) / (|tau| + sqrt(1 + tau^2)) with tau = (aqq - app) / (2 apq),
+            // written with one division, one square root and one reciprocal square root (the chain of three divisions and
+            // two square roots was most of a round's latency, and the rounds are the critical path of the iteration)
+            const double d = sm.A[q][q] - sm.A[p][p];
+            const double tt = 2.0 * apq / (d + copysign(sqrt(d * d + 4.0 * apq * apq), d));
+            c = rsqrt(1.0 + tt * tt);
             sn = tt * c;
           }
         }
