@@ -665,9 +665,9 @@ def run_ours(args, rank, world, local_rank):
         else:                                   # the oracle only knows fully materialised, unsharded operators
             ref = oracle_samples(cfg, psi0, sl, sx, sy, D=args.D)
         res["parity_sample_rel_err"] = float(np.linalg.norm(got - ref) / np.linalg.norm(ref))
-        if args.D is None:
+        if args.D is None and world == 1:           # the timed oracle: rank 0 at N = 1 only
             res["cpu_baseline"], _, _ = cpu_baseline(cfg)
-        else:
+        elif args.D is not None:
             res["config"]["workload"] += f" with D overridden to {args.D} (bond-dimension sweep, not a BASELINE config)"
         print(json.dumps(res), flush=True)
     if world > 1:

@@ -452,3 +452,43 @@ def test_batched_schedule_interpreter(toy, flags):
         H.plan_problem(toy, flags=H.HPSI_PLAN_HOST_ONLY | H.HPSI_PLAN_FUSE_ALL, n_vectors=2)
     with pytest.raises(H.HpsiError):
         H.plan_problem(toy, flags=H.HPSI_PLAN_HOST_ONLY, n_vectors=65)
+
+
+# --------------------------------------------------------------------- argument checks of the round-2 entry points
+def test_new_entry_points_refuse_bad_arguments(toy):
+    """No device is needed to be refused: host-only plans answer ESTATE to every compute call (no CPU fallback), bad
+    arguments EINVAL, and hpsi_plan_options_t is versioned by its size."""
+    plan = host_plan(toy)
+    n = H.hpsi_query(plan, H.HPSI_Q_PSI_LENGTH)
+    x = np.zeros(2 * n)
+    L = H.lib()
+    st = ctypes.c_void_p
+    # batched apply on a single-vector plan / a host-only plan
+    assert L.hpsi_apply_multi(plan.handle, x.ctypes.data, n, x.ctypes.data + 8 * n, n, 2, None) == H.HPSI_EINVAL
+    plan2 = H.plan_problem(toy, flags=H.HPSI_PLAN_HOST_ONLY, n_vectors=2)
+    y = np.zeros(2 * n)
+    assert L.hpsi_apply_multi(plan2.handle, x.ctypes.data, n, y.ctypes.data, n, 2, None) == H.HPSI_ESTATE
+    assert L.hpsi_apply_multi(plan2.handle, x.ctypes.data, n - 1, y.ctypes.data, n, 2, None) == H.HPSI_EINVAL     # stride < psi_length
+    assert L.hpsi_apply_multi(plan2.handle, x.ctypes.data, n, x.ctypes.data + 8, n, 2, None) == H.HPSI_EINVAL     # overlap
+    # eigensolvers
+    eig = (ctypes.c_double * 4)()
+    prm = H.binding.hpsi_davidson_params_t(1e-8, 10, 16, 1)
+    assert L.hpsi_davidson_multi(plan2.handle, x.ctypes.data, n, 2, eig, None, ctypes.byref(prm), None, None) == H.HPSI_ESTATE
+    assert L.hpsi_davidson_multi(None, x.ctypes.data, n, 2, eig, None, ctypes.byref(prm), None, None) == H.HPSI_EINVAL
+    # hpsi_sum_shards: argument checks come before any CUDA call
+    assert L.hpsi_sum_shards(x.ctypes.data, 0, n, y.ctypes.data, None) == H.HPSI_EINVAL
+    assert L.hpsi_sum_shards(None, 2, n, y.ctypes.data, None) == H.HPSI_EINVAL
+    assert L.hpsi_sum_shards(x.ctypes.data, 2, n, x.ctypes.data + 8, None) == H.HPSI_EINVAL                       # overlapping, not in place
+    assert L.hpsi_sum_shards(x.ctypes.data, 2, 0, y.ctypes.data, None) == H.HPSI_OK                               # nothing to do
+    # options struct smaller than the library's: refused, not misread
+    sec, trm, keep = H.binding._marshal(toy.q_left, toy.q_right, toy.d_left, toy.d_right, toy.target, toy.coef, toy.a_desc,
+                                        toy.b_desc, None, None, toy.a_len, toy.b_len, None, None)
+    opt = H.binding.hpsi_plan_options_t(8, 0, None, 0, 0, 0, 0)
+    out = ctypes.c_void_p()
+    assert L.hpsi_plan_ex(ctypes.byref(sec), ctypes.byref(trm), H.HPSI_PLAN_HOST_ONLY, ctypes.byref(opt), ctypes.byref(out)) == H.HPSI_EINVAL
+    assert out.value is None and b"struct_bytes" in L.hpsi_last_error()
+    # layout helper
+    bad = toy.a_desc.copy(); bad["row"][0] = 99
+    with pytest.raises(H.HpsiError):
+        H.hpsi_layout_blocks(toy.d_left, bad)
+    del st
