@@ -83,7 +83,8 @@ typedef struct {
    * says the arena holds the TRANSPOSE of that block: element (x, x') of the block is arena[offset + x' * ld + x] with
    * ld >= d[row].  A Hermitian H pairs every term with its adjoint (same c, A^T, B^T): the adjoint term's descriptors
    * can then point at the base term's storage and the operator arenas halve (80 -> 40 GB at D=8192).  Such blocks are
-   * staged K-major (TMA boxes of 8 rows x 16 k, 64-byte swizzle); tiles stay padded to 8 rows as in plain plans. */
+   * staged K-major (TMA boxes of 8 rows x 16 k, 64-byte swizzle); tiles stay padded to 8 rows as in plain plans.
+   * The flags are per block and independent: any mix of plain and transposed A / B blocks inside a term is legal. */
   const uint8_t* a_transposed;
   const uint8_t* b_transposed;
 } hpsi_terms_t;

@@ -28,8 +28,9 @@ void interpret_schedule(const Schedule& sc, const double* a, const double* b, co
     const double* y = ws + g.y1_off + (int64_t)u.vec * g.N1 * g.ldy1;     // vector v: rows [v N1, (v + 1) N1) of the stacked operand
     for (int t = u.t0; t < u.t1; ++t) {
       const Seg& sg = sc.segs[g.seg0 + t];
-      // element (i, k) of the operator block: plain storage [i][k], transposed storage [k][i]
-      const int64_t xsi = sg.p1_trans ? 1 : sg.p1_ld, xsk = sg.p1_trans ? sg.p1_ld : 1;
+      // element (i, k) of the operator block: plain storage [i][k], transposed storage [k][i]; the layout is the UNIT's
+      // flag, as in the kernels (one layout per unit), not the seg's
+      const int64_t xsi = u.xtrans ? 1 : sg.p1_ld, xsk = u.xtrans ? sg.p1_ld : 1;
       for (int r = 0; r < u.rows_valid; ++r) {
         const double* xr = xbase + sg.p1_off + (int64_t)(u.i0 + r) * xsi;
         for (int c = 0; c < u.cols_valid; ++c) {
@@ -53,7 +54,7 @@ void interpret_schedule(const Schedule& sc, const double* a, const double* b, co
           for (int si = run.seg_begin; si < run.seg_end; ++si) {
             const Seg& sg = sc.segs[si];
             const int64_t t_off = run.ws_off + (int64_t)(si - run.seg0) * run.rows * run.ldw + u.vec * run.Kp;
-            const int64_t osi = sg.p2_trans ? 1 : sg.p2_ld, osk = sg.p2_trans ? sg.p2_ld : 1;   // operator block strides
+            const int64_t osi = run.trans ? 1 : sg.p2_ld, osk = run.trans ? sg.p2_ld : 1;   // operator block strides: the RUN's layout flag, as in the kernels
             const double *xr, *yr;
             int64_t xsk = 1, ysk = 1;
             if (run.order == 1) {

@@ -294,6 +294,14 @@ int build_schedule(const hpsi_sectors_t* s, const hpsi_terms_t* t, uint32_t flag
     int order = (f2 < f1) ? 2 : 1;
     if (flags & HPSI_PLAN_FIXED_ORDER1) order = 1;
     if (flags & HPSI_PLAN_FIXED_ORDER2) order = 2;
+    // the first GEMM's units take [plain | transposed] halves of the group, so its operand's layout is the primary key
+    // (the sort above put A's first: right for order 1 only); the second GEMM's runs split at every layout change
+    if (order == 2 && paired)
+      std::stable_sort(raw.begin() + i, raw.begin() + j, [](const RawTask& x, const RawTask& y) {
+        if (x.tb != y.tb) return x.tb < y.tb;
+        if (x.ta != y.ta) return x.ta < y.ta;
+        return x.term < y.term;
+      });
     Group g{};
     g.order = order;
     g.tcount = (int32_t)(j - i);
@@ -511,15 +519,16 @@ int build_schedule(const hpsi_sectors_t* s, const hpsi_terms_t* t, uint32_t flag
           if (sp == nsplit - 1) take = g.tcount - ti;
           else take = (int)std::min<int64_t>(g.tcount - ti, std::max<int64_t>(1, (want - cum + per - 1) / per));
           if (take > 0) {
-            // a run has one storage layout of its operator blocks: split [ti, ti + take) at the group's layout boundary
-            int tbnd = ti;
-            while (tbnd < ti + take && !sc->segs[g.seg0 + tbnd].p2_trans) ++tbnd;
-            Run r{g.seg0 + ti, g.seg0 + tbnd, g.N1, g.ldw, g.order, g.rows, g.seg0, g.ws_map, g.ws_off, 0, 0, 0, 0, g.N1p, 0};
-            if (g.fused) { r.K1 = g.K1; r.y1_map = g.y1_map; r.ldy1 = g.ldy1; r.y1_off = g.y1_off; }
-            if (tbnd > ti) sc->runs.push_back(r);
-            if (tbnd < ti + take) {
-              r.seg_begin = g.seg0 + tbnd; r.seg_end = g.seg0 + ti + take; r.trans = 1;
+            // a run has one storage layout of its operator blocks: split [ti, ti + take) at every layout change
+            // (adjoint-pair sharing gives one boundary per group; arbitrary flags may alternate)
+            for (int s0 = ti; s0 < ti + take;) {
+              const int32_t tr = sc->segs[g.seg0 + s0].p2_trans;
+              int s1 = s0 + 1;
+              while (s1 < ti + take && sc->segs[g.seg0 + s1].p2_trans == tr) ++s1;
+              Run r{g.seg0 + s0, g.seg0 + s1, g.N1, g.ldw, g.order, g.rows, g.seg0, g.ws_map, g.ws_off, tr, 0, 0, 0, g.N1p, 0};
+              if (g.fused) { r.K1 = g.K1; r.y1_map = g.y1_map; r.ldy1 = g.ldy1; r.y1_off = g.y1_off; }
               sc->runs.push_back(r);
+              s0 = s1;
             }
             cum += per * take;
             chunk_ksteps += (int64_t)((g.N1 + 3) / 4) * take;

@@ -101,3 +101,32 @@ def fill_device_arenas(torch, full, chunk_terms=48, workers=6, on_chunk=None):
             del sub
     torch.cuda.synchronize()
     return a, b
+
+
+def store_randomly_transposed(p, seed, prob=0.5):
+    """A copy of Problem ``p`` (materialised arenas) whose operator blocks are re-stored, each with probability ``prob``
+    as its transpose (d[col] x d[row], flagged in a_trans / b_trans).  Even leading dimensions are kept when ``p`` has
+    them.  The values of every block are unchanged, so the oracle's result for ``p`` is the expected one."""
+    import copy
+    rng = np.random.default_rng(seed)
+    q = copy.copy(p)
+
+    def restore(desc, data, d):
+        even = all(int(e["ld"]) % 2 == 0 for e in desc)
+        out, tr, chunks, off = desc.copy(), np.zeros(desc.shape[0], np.uint8), [], 0
+        for i, e in enumerate(desc):
+            r, c, ld, o = int(d[e["row"]]), int(d[e["col"]]), int(e["ld"]), int(e["offset"])
+            blk = data[o:o + r * ld].reshape(r, ld)[:, :c]
+            if rng.random() < prob:
+                blk, tr[i] = blk.T, 1
+            nld = blk.shape[1] + (blk.shape[1] % 2 if even else 0)
+            buf = np.zeros((blk.shape[0], nld))
+            buf[:, :blk.shape[1]] = blk
+            out[i]["ld"], out[i]["offset"] = nld, off
+            chunks.append(buf.ravel())
+            off += buf.size
+        return out, tr, (np.concatenate(chunks) if chunks else np.zeros(1)), off
+
+    q.a_desc, q.a_trans, q.a_data, q.a_len = restore(p.a_desc, p.a_data, p.d_left)
+    q.b_desc, q.b_trans, q.b_data, q.b_len = restore(p.b_desc, p.b_data, p.d_right)
+    return q

@@ -1,15 +1,17 @@
 """Randomised structures through the C ABI against the oracle: irregular label sets, partner-less sectors, sector dims
 from 1 to 200 mixed in one problem, sparse and dense block patterns, odd leading dimensions, misaligned arenas, forced
 contraction orders; every case runs hpsi_apply, hpsi_rotate_apply (random kept dims, some zero) and hpsi_truncate
-(either side, by count or by discarded weight); odd seeds send the narrow groups through the fused kernel.  (7000 seeds
-of this generator were run on a B200 with no failure; the committed test keeps 60.)"""
+(either side, by count or by discarded weight); odd seeds send the narrow groups through the fused kernel; every seed
+also re-stores a random half of the operator blocks transposed (A and B flags independent) and runs a batched plan of
+2 .. 4 vectors.  (7000 seeds of this generator were run on a B200 in each round with no failure; the committed test
+keeps 60.)"""
 import numpy as np
 import pytest
 
 import oracle
 import workloads
 from oracle import site_update as su
-from gpu_util import GpuProblem
+from gpu_util import GpuProblem, store_randomly_transposed
 
 pytestmark = pytest.mark.gpu
 
@@ -121,3 +123,23 @@ def test_random_structure(seed):
         row0 += cc if side else rr
         if k:
             np.testing.assert_allclose(O @ M, (sig ** 2)[:, None] * O, atol=1e-11 * max(smax ** 2, 1e-300))
+
+    # the same operator with a random half of its blocks stored transposed (both staging variants)
+    q = store_randomly_transposed(p, seed)
+    for mis in (False, True):
+        out = GpuProblem(q, flags & ~H.HPSI_PLAN_FUSE_ALL, misalign=mis).apply(psi)
+        assert np.linalg.norm(out - ref) <= 1e-12 * max(np.linalg.norm(ref), 1.0), ("mixed storage", mis)
+
+    # a batched plan: every vector against the oracle
+    nv = 2 + seed % 3
+    gb = GpuProblem(p, flags & ~H.HPSI_PLAN_FUSE_ALL, misalign=bool(seed & 4), n_vectors=nv)
+    psis = rng.standard_normal((nv, p.psi_len))
+    psis[0] = psi
+    x = torch.from_numpy(psis).cuda()
+    y = torch.full_like(x, float("nan"))
+    H.hpsi_apply_multi(gb.plan, x, y, nv, st)
+    torch.cuda.synchronize()
+    yh = y.cpu().numpy()
+    for k in range(nv):
+        rk = oracle.apply(p, psis[k])
+        assert np.linalg.norm(yh[k] - rk) <= 1e-12 * max(np.linalg.norm(rk), 1.0), ("batched", k)

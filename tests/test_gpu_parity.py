@@ -556,6 +556,33 @@ def test_shared_adjoint_ragged_multi_tile(H):
         assert rel_l2(GpuProblem(shared, misalign=misalign).apply(psi), ref) <= TOL
 
 
+@pytest.mark.parametrize("seed", range(6))
+def test_mixed_storage_irregular(H, seed):
+    """Plain and transposed blocks mixed at random inside one term, on irregular structures (dims 1 .. 4, partner-less
+    sectors, odd or even leading dimensions, 16-byte or 8-byte aligned arenas) and on the multi-tile ragged blocks."""
+    from gpu_util import store_randomly_transposed
+    rng = np.random.default_rng(100 + seed)
+    if seed < 4:
+        p = random_custom(seed, grid=(seed < 2))
+    else:
+        dL, dR = [150, 70, 9], [131, 9, 77]
+        terms = []
+        for _ in range(6):
+            ab = {(r, c): rng.standard_normal((dL[r], dL[c])) for r in range(3) for c in range(3) if rng.random() < 0.7}
+            bb = {(r, c): rng.standard_normal((dR[r], dR[c])) for r in range(3) for c in range(3) if rng.random() < 0.7}
+            terms.append((float(rng.standard_normal()), ab, bb))
+        p = workloads.custom_problem([(i, 0) for i in range(3)], dL, [(3 - i, 0) for i in range(3)], dR, (3, 0), terms,
+                                     pad_even=(seed == 4))
+    psi = rng.standard_normal(p.psi_len)
+    ref = oracle.apply(p, psi)
+    for k in range(2):
+        q = store_randomly_transposed(p, 10 * seed + k)
+        assert q.a_trans.any() or q.b_trans.any()
+        for misalign in (False, True):
+            out = GpuProblem(q, misalign=misalign).apply(psi)
+            assert np.linalg.norm(out - ref) <= TOL * max(np.linalg.norm(ref), 1.0), (seed, k, misalign)
+
+
 def test_davidson_trajectory_matches_oracle(H, small):
     """Step-by-step parity of the driver: without the (ill-conditioned) diagonal preconditioner the Ritz value and
     the residual after k mat-vecs agree with the oracle's textbook Davidson (A21) to rounding."""

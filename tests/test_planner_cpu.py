@@ -414,6 +414,23 @@ def test_shared_adjoint_storage_interpreter(name, kw):
         assert rel(H.hpsi_debug_interpret(plan, shared.a_data, shared.b_data, psi), ref) <= 1e-13
 
 
+@pytest.mark.parametrize("seed", range(6))
+def test_mixed_storage_interpreter(seed):
+    """Plain and transposed blocks mixed at random inside one term (irregular structures, odd and even leading dimensions,
+    every order): the A and B flags of a task are independent, so neither GEMM may assume the other's layout boundary."""
+    from gpu_util import store_randomly_transposed
+    for grid in (True, False):
+        p = random_custom(seed, grid=grid)
+        psi = np.random.default_rng(seed).standard_normal(p.psi_len)
+        ref = oracle.apply(p, psi)
+        for k in range(3):
+            q = store_randomly_transposed(p, 10 * seed + k)
+            assert q.a_trans.any() or q.b_trans.any()
+            for flags in (0, H.HPSI_PLAN_FIXED_ORDER1, H.HPSI_PLAN_FIXED_ORDER2):
+                got = H.hpsi_debug_interpret(host_plan(q, flags), q.a_data, q.b_data, psi)
+                assert np.linalg.norm(got - ref) <= 1e-13 * max(np.linalg.norm(ref), 1.0), (grid, k, flags)
+
+
 def test_transposed_block_validation(toy):
     shared = workloads.make_problem("toy", share_adjoint=True)
     bad = shared.a_desc.copy()
