@@ -143,3 +143,63 @@ def test_random_structure(seed):
     for k in range(nv):
         rk = oracle.apply(p, psis[k])
         assert np.linalg.norm(yh[k] - rk) <= 1e-12 * max(np.linalg.norm(rk), 1.0), ("batched", k)
+
+
+def _term_doubles(q, t):
+    """doubles term t occupies in the two arenas (stored rows x ld of each of its blocks)"""
+    tot = 0
+    for desc, tr, d, rng_ in ((q.a_desc, q.a_trans, q.d_left, q.term_a_range), (q.b_desc, q.b_trans, q.d_right, q.term_b_range)):
+        for i in range(int(rng_[t][0]), int(rng_[t][1])):
+            e = desc[i]
+            rows = d[e["col"]] if (tr is not None and tr[i]) else d[e["row"]]
+            tot += int(rows) * int(e["ld"])
+    return tot
+
+
+@pytest.mark.parametrize("seed", range(3000, 3024))
+def test_random_structure_other_entry_points(seed):
+    """The same generator through hpsi_diagonal, hpsi_set_task_coefficients, term shards (hpsi_shard_terms + hpsi_plan_ex +
+    hpsi_sum_shards) and the streamed apply (1 window ... 1 term per window); odd seeds with a random half of the blocks
+    stored transposed.  (3000 seeds of this test were run on a B200 with no failure.)"""
+    import torch
+    import paper_2407_07411_b200 as H
+    from gpu_util import shard_sum
+    from test_planner_cpu import exploded_problem
+    p, rng = rand_problem(seed)
+    redraw = 0
+    while p.psi_len == 0:
+        redraw += 1
+        p, rng = rand_problem(seed + 100000 * redraw)
+    st = torch.cuda.current_stream()
+    psi = rng.standard_normal(p.psi_len)
+    ref = oracle.apply(p, psi)
+    nref = max(np.linalg.norm(ref), 1.0)
+    q = store_randomly_transposed(p, seed) if seed % 2 else p
+    g = GpuProblem(q)
+    x = torch.from_numpy(psi).cuda()
+
+    d = torch.empty(g.n, dtype=torch.float64, device="cuda")
+    H.hpsi_diagonal(g.plan, d)
+    torch.cuda.synchronize()
+    dref = oracle.diagonal(p)
+    assert np.linalg.norm(d.cpu().numpy() - dref) <= 1e-12 * max(np.linalg.norm(dref), 1.0)
+
+    world = 2 + seed % 3
+    shard, _fl = H.hpsi_shard_terms(q, world)
+    parts = [GpuProblem(q, arenas=(g.a, g.b), shard_of_term=shard, shard_index=r).apply_dev(x) for r in range(world)]
+    assert np.linalg.norm(shard_sum(H, torch, parts) - ref) <= 1e-12 * nref
+
+    per_term = max(_term_doubles(q, t) for t in range(len(q.coef)))
+    a_host, b_host = torch.from_numpy(q.a_data).pin_memory(), torch.from_numpy(q.b_data).pin_memory()
+    for window in (q.a_len + q.b_len + 16, 3 * per_term + 64, per_term + 64):
+        sp = H.hpsi_stream_create(q, a_host, b_host, window)
+        y = torch.full_like(x, float("nan"))
+        H.hpsi_stream_apply(sp, x, y, st)
+        torch.cuda.synchronize()
+        assert np.linalg.norm(y.cpu().numpy() - ref) <= 1e-12 * nref, (window, H.hpsi_stream_query(sp, H.HPSI_SQ_N_WINDOWS))
+        del sp
+
+    f = rng.standard_normal(g.q(H.HPSI_Q_N_TASKS))                # last: it changes the plan's operator
+    H.hpsi_set_task_coefficients(g.plan, f, st)
+    r2 = oracle.apply(exploded_problem(p, g.plan, f), psi)
+    assert np.linalg.norm(g.apply(psi) - r2) <= 1e-12 * max(np.linalg.norm(r2), 1.0)
