@@ -198,7 +198,8 @@ def davidson(p, v0: np.ndarray, tol: float = 1e-8, max_iter: int = 200, m_max: i
 
     V=[v0/|v0|]; loop: W=H V (one new column per iteration), G=V^T W, smallest Ritz pair (theta,y), x=V y,
     r=W y - theta x; stop if |r|<=tol; s=r/(diag(H)-theta) with small-denominator guard (or s=r); orthogonalise
-    s against V twice (classical Gram-Schmidt, applied twice); append; when dim V == m_max restart with V=[x].
+    s against V twice (classical Gram-Schmidt, applied twice); if the preconditioned s vanishes (|s| < 1e-14) retry with
+    s=r (reading A21c); append; when dim V == m_max restart with V=[x].
     Returns (theta, x, n_matvec, residual_norm)."""
     mv = (lambda x: apply(p, x)) if matvec is None else matvec
     d = diagonal(p) if precondition else None
@@ -233,6 +234,13 @@ def davidson(p, v0: np.ndarray, tol: float = 1e-8, max_iter: int = 200, m_max: i
         for _pass in range(2):
             s = s - Vm @ (Vm.T @ s)
         ns = np.linalg.norm(s)
+        if ns < 1e-14 and d is not None:
+            # reading A21c: the preconditioned correction lies in span(V) (e.g. H diagonal, where r/(diag - theta) is the
+            # Ritz vector itself) although |r| > tol: take the residual itself as the new direction
+            s = r.copy()
+            for _pass in range(2):
+                s = s - Vm @ (Vm.T @ s)
+            ns = np.linalg.norm(s)
         if ns < 1e-14:
             break
         s = s / ns
@@ -300,6 +308,12 @@ def davidson_block(p, V0: np.ndarray, tol: float = 1e-8, max_iter: int = 200, m_
                 Vm = np.stack(V, axis=1)
                 s = s - Vm @ (Vm.T @ s)
             ns = np.linalg.norm(s)
+            if ns < 1e-14 and d is not None:             # reading A21c: fall back to the residual itself
+                s = r.copy()
+                for _pass in range(2):
+                    Vm = np.stack(V, axis=1)
+                    s = s - Vm @ (Vm.T @ s)
+                ns = np.linalg.norm(s)
             if ns < 1e-14:
                 continue
             V.append(s / ns)

@@ -343,6 +343,30 @@ def test_davidson_block_vs_dense_eigensolver(toy, k, precondition):
     assert k <= nmv <= 800
 
 
+def test_davidson_diagonal_operator_needs_the_residual_fallback():
+    """Reading A21c, pinned against LAPACK: for a diagonal H the preconditioned correction r/(diag - theta) is the Ritz
+    vector itself, so it vanishes under Gram-Schmidt with |r| > tol; the residual is taken instead and the solver still
+    reaches the lowest eigenvalue (a block-diagonal H with one diagonal and one dense block does the same in one block).
+    An exact start vector (r = 0) is a converged run after one mat-vec."""
+    rng = np.random.default_rng(12)
+    dvals = np.array([-2.0, 1.0, 3.0, 0.5])
+    diag = workloads.custom_problem([(0, 0)], [4], [(1, 0)], [1], (1, 0), [(1.0, {(0, 0): np.diag(dvals)}, {(0, 0): np.ones((1, 1))})])
+    S = rng.standard_normal((3, 3))
+    mixed = workloads.custom_problem([(0, 0), (1, 0)], [4, 3], [(1, 0), (0, 0)], [1, 1], (1, 0),
+                                     [(1.0, {(0, 0): np.diag(dvals), (1, 1): S + S.T}, {(0, 0): np.ones((1, 1)), (1, 1): np.ones((1, 1))})])
+    for p in (diag, mixed):
+        ev = np.linalg.eigvalsh(oracle.dense_hamiltonian(p))
+        v0 = rng.standard_normal(p.psi_len)
+        for pre in (True, False):
+            th, x, nmv, rn = oracle.davidson(p, v0, tol=1e-10, max_iter=100, precondition=pre)
+            assert rn <= 1e-10 and abs(th - ev[0]) <= 1e-12, (pre, th, ev[0], nmv)
+            thb, X, nb, rb = oracle.davidson_block(p, rng.standard_normal((p.psi_len, 2)), tol=1e-10, max_iter=200, precondition=pre)
+            assert rb.max() <= 1e-10 and np.max(np.abs(thb - ev[:2])) <= 1e-12, (pre, thb, ev[:2])
+    e0 = np.array([1.0, 0.0, 0.0, 0.0])
+    th, x, nmv, rn = oracle.davidson(diag, 3.0 * e0, tol=1e-10)
+    assert nmv == 1 and rn == 0.0 and th == -2.0 and np.array_equal(x, e0)
+
+
 def test_davidson_block_single_root_is_davidson(toy):
     """k = 1 is the single-root method of reading A21, mat-vec for mat-vec."""
     v0 = workloads.make_psi(toy)
