@@ -190,7 +190,10 @@ int hpsi_diagonal(hpsi_plan_t* plan, double* diag_dev, void* cuda_stream);
 
 /* Step 8: Davidson-Liu, lowest eigenpair, single root (PAPER.md:62 names the method; A21 gives the
  * algorithm).  All O(psi_length) work and the small subspace eigenproblem run on the device; the host reads back
- * one residual norm per iteration to test convergence. */
+ * one residual norm per iteration to test convergence.  If the preconditioned correction vanishes under
+ * Gram-Schmidt (||s|| < 1e-14; an operator with a diagonal block) while the residual is above tol, the residual itself is
+ * taken (reading A21c); the solver stops unconverged only if that vanishes too.  A start vector that already is the
+ * eigenvector converges after one mat-vec (converged = 1, residual = 0). */
 typedef struct {
   double tol;            /* stop when ||H x - theta x|| <= tol                 (default 1e-8) */
   int32_t max_iter;      /* max matrix-vector products                          (default 200)  */

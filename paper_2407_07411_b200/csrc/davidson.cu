@@ -57,7 +57,8 @@ __global__ void dot_kernel(const double* __restrict__ X, int64_t ldx, const doub
 
 // dst = src / sqrt(*nrm2)   (dst2 = src2 / sqrt(*nrm2) if given)
 __global__ void scale_kernel(double* dst, const double* src, double* dst2, const double* src2, const double* nrm2,
-                             int64_t n) {
+                             int64_t n, const double* dead = nullptr) {
+  if (dead && *dead != 0.0) return;
   const double inv = 1.0 / sqrt(*nrm2);
   for (int64_t e = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; e < n; e += (int64_t)gridDim.x * blockDim.x) {
     dst[e] = src[e] * inv;
@@ -299,7 +300,8 @@ __global__ void __launch_bounds__(256) dav_ritz_kernel(const double* __restrict_
 // also raises the "dead" flag when |s| < 1e-14)
 __global__ void __launch_bounds__(256) dav_project_kernel(double* s, const double* __restrict__ V, int64_t n, int j,
                                                           const double* __restrict__ c_in, double* partial,
-                                                          unsigned int* ticket, double* c_out, double* nrm_s2, double* ctl) {
+                                                          unsigned int* ticket, double* c_out, double* nrm_s2, double* ctl,
+                                                          double stamp) {
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
   int64_t lo, hi;
   dav_slice(n, lo, hi);
@@ -322,7 +324,7 @@ __global__ void __launch_bounds__(256) dav_project_kernel(double* s, const doubl
     const double t = dav_sum_partials(partial + i * NB, lane);
     if (lane == 0) {
       if (c_out) c_out[i] = t;
-      else { *nrm_s2 = t; if (!(t >= 1e-28) && ctl[5] == 0.0) ctl[5] = 1.0; }
+      else { *nrm_s2 = t; if (!(t >= 1e-28) && ctl[5] == 0.0) ctl[5] = stamp; }
     }
   }
   if (threadIdx.x == 0) *ticket = 0;
@@ -338,6 +340,12 @@ __global__ void project_kernel(double* s, const double* __restrict__ V, int64_t 
 }
 
 __global__ void set_scalar_kernel(double* dst, const double* src) { *dst = *src; }
+
+// restart: G = [[theta]] (a no-op while the dead flag is up, like the other kernels that change the subspace)
+__global__ void reset_gram_kernel(double* G, const double* theta, const double* dead) {
+  if (*dead != 0.0) return;
+  for (int i = threadIdx.x; i < MMAX * MMAX; i += blockDim.x) G[i] = i == 0 ? *theta : 0.0;
+}
 
 }  // namespace
 
@@ -398,6 +406,7 @@ extern "C" int hpsi_davidson(hpsi_plan_t* p, double* psi, double* eig_host, cons
   dots(psi, 1, psi, ctl, 1, nullptr, 0);
   if ((rc = apply_impl(p, psi, W, false, cuda_stream, ctl, V)) != HPSI_OK) return rc;
   int j = 1, nmv = 1, converged = 0;
+  int j_good = 1;                                        // columns of V / W that were valid when the last correction vector was built
   double rn = INFINITY, th = 0.0;
   double* hostbuf = p->h_dav;
   for (int it = 0; it < prm.max_iter; ++it) {
@@ -414,23 +423,44 @@ extern "C" int hpsi_davidson(hpsi_plan_t* p, double* psi, double* eig_host, cons
     HPSI_CUDA(cudaEventRecord(p->dav_ev[1], p->dav_side));
     if (j >= prm.m_max) {                                           // restart with V = [x/|x|]
       dots(x, 1, x, ctl + 2, 1, nullptr, 0);
-      scale_kernel<<<eg, 256, 0, st>>>(V, x, W, wy, ctl + 2, n);
-      HPSI_CUDA(cudaMemsetAsync(G, 0, MMAX * MMAX * sizeof(double), st));
-      set_scalar_kernel<<<1, 1, 0, st>>>(G, theta);
+      scale_kernel<<<eg, 256, 0, st>>>(V, x, W, wy, ctl + 2, n, ctl + 5);
+      reset_gram_kernel<<<1, 256, 0, st>>>(G, theta, ctl + 5);
       j = 1;
       jp = 0;
       dots(V, 1, s, c, 1, nullptr, 0);
     }
-    // classical Gram-Schmidt, twice; the second pass leaves |s|^2 (and the dead flag)
-    dav_project_kernel<<<NB, 256, 0, st>>>(s, V, n, j, c, partial, tickets + 2, c2, nullptr, ctl);
-    dav_project_kernel<<<NB, 256, 0, st>>>(s, V, n, j, c2, partial, tickets + 3, nullptr, ctl + 3, ctl);
+    // classical Gram-Schmidt, twice; the second pass leaves |s|^2 (and the dead flag, stamped with the iteration)
+    const double stamp = (double)(it + 1);
+    dav_project_kernel<<<NB, 256, 0, st>>>(s, V, n, j, c, partial, tickets + 2, c2, nullptr, ctl, stamp);
+    dav_project_kernel<<<NB, 256, 0, st>>>(s, V, n, j, c2, partial, tickets + 3, nullptr, ctl + 3, ctl, stamp);
     HPSI_CUDA(cudaEventSynchronize(p->dav_ev[1]));
     th = hostbuf[0];
     rn = std::sqrt(hostbuf[2]);
-    if (hostbuf[6] != 0.0) break;                                   // the previous correction vector vanished: theta, x are the last good ones
+    // theta, |r| are the last good ones whether or not the dead flag is up (a dead iteration's kernels are no-ops; the flag
+    // of THIS iteration's correction can already be visible because the copy runs beside the orthogonalisation: an exact
+    // eigenvector gives r = 0, hence s = 0): convergence is decided first
     if (rn <= prm.tol) { converged = 1; break; }
-    if (nmv >= prm.max_iter) break;
+    const double dead = hostbuf[6];
+    if (dead != 0.0) {
+      // The correction vector vanished with |r| > tol.  A flag stamped by an earlier iteration was raised after that
+      // iteration's read-back: the mat-vec enqueued for the dead vector and everything since were no-ops on the subspace,
+      // so the host counters step back.
+      if (dead != stamp) { j = j_good; --nmv; }
+      // Unpreconditioned (s = r) that is a breakdown, and so is a vanished fallback vector (stamp + 0.5 below).
+      // Preconditioned it means r/(diag - theta) lies in span(V) (H diagonal: it is the Ritz vector itself): reading A21c
+      // retries with the residual itself.
+      if (!prm.precondition || dead != std::floor(dead) || nmv >= prm.max_iter) break;
+      jp = 0;
+      HPSI_CUDA(cudaMemsetAsync(ctl + 5, 0, sizeof(double), st));
+      HPSI_CUDA(cudaMemcpyAsync(s, r, n * sizeof(double), cudaMemcpyDeviceToDevice, st));
+      dots(V, j, s, c, 1, nullptr, 0);
+      dav_project_kernel<<<NB, 256, 0, st>>>(s, V, n, j, c, partial, tickets + 2, c2, nullptr, ctl, stamp + 0.5);
+      dav_project_kernel<<<NB, 256, 0, st>>>(s, V, n, j, c2, partial, tickets + 3, nullptr, ctl + 3, ctl, stamp + 0.5);
+    } else if (nmv >= prm.max_iter) {
+      break;
+    }
     // V_j = s/|s| (written by the prep kernel), W_j = H V_j - enqueued while the orthogonalisation may still be running
+    j_good = j;
     if ((rc = apply_impl(p, s, W + (size_t)j * n, false, cuda_stream, ctl + 3, V + (size_t)j * n)) != HPSI_OK) return rc;
     ++j;
     ++nmv;
@@ -600,7 +630,15 @@ extern "C" int hpsi_davidson_multi(hpsi_plan_t* p, double* psi, int64_t ld, int3
         if (check_each) {
           cudaMemcpyAsync(host.data(), nrm + added, sizeof(double), cudaMemcpyDeviceToHost, st);
           cudaStreamSynchronize(st);
-          if (!(host[0] >= 1e-28)) continue;                          // dropped: the slot is reused by the next root
+          if (!(host[0] >= 1e-28)) {
+            if (!prm.precondition) continue;                          // dropped: the slot is reused by the next root
+            // reading A21c: the preconditioned correction lies in span(V); retry with the residual itself
+            precond_kernel<<<eg, 256, 0, st>>>(Rv + (size_t)r * n, diag, theta + r, 0, s, n);
+            orth_append(j + added, added);
+            cudaMemcpyAsync(host.data(), nrm + added, sizeof(double), cudaMemcpyDeviceToHost, st);
+            cudaStreamSynchronize(st);
+            if (!(host[0] >= 1e-28)) continue;
+          }
         }
         ++added;
       }

@@ -583,6 +583,68 @@ def test_mixed_storage_irregular(H, seed):
             assert np.linalg.norm(out - ref) <= TOL * max(np.linalg.norm(ref), 1.0), (seed, k, misalign)
 
 
+def _tiny_eig_problems():
+    """psi_length 1; H = 0; a diagonal H; one diagonal and one dense block (the preconditioned correction of a Ritz vector
+    living in the diagonal block vanishes under Gram-Schmidt)."""
+    rng = np.random.default_rng(12)
+    one = workloads.custom_problem([(0, 0)], [1], [(1, 0)], [1], (1, 0), [(2.0, {(0, 0): np.array([[0.7]])}, {(0, 0): np.array([[-0.3]])})])
+    zero = workloads.custom_problem([(0, 0)], [3], [(1, 0)], [2], (1, 0),
+                                    [(1.0, {(0, 0): np.zeros((3, 3))}, {(0, 0): np.zeros((2, 2))})])
+    dvals = np.array([-2.0, 1.0, 3.0, 0.5])
+    diag = workloads.custom_problem([(0, 0)], [4], [(1, 0)], [1], (1, 0), [(1.0, {(0, 0): np.diag(dvals)}, {(0, 0): np.ones((1, 1))})])
+    S = rng.standard_normal((3, 3))
+    mixed = workloads.custom_problem([(0, 0), (1, 0)], [4, 3], [(1, 0), (0, 0)], [1, 1], (1, 0),
+                                     [(1.0, {(0, 0): np.diag(dvals), (1, 1): S + S.T}, {(0, 0): np.ones((1, 1)), (1, 1): np.ones((1, 1))})])
+    return one, zero, diag, mixed
+
+
+def test_eigensolvers_exact_start_vector(H):
+    """psi_length 1, H = 0 and a start vector that already is the eigenvector: the residual is exactly 0 after the first
+    mat-vec, the correction vector vanishes with it, and the solvers must report convergence (not a breakdown)."""
+    import torch
+    one, zero, diag, _ = _tiny_eig_problems()
+    for p, v0, want in ((one, np.array([3.0]), 2.0 * 0.7 * -0.3), (zero, np.arange(1.0, 7.0), 0.0),
+                        (diag, np.array([2.0, 0.0, 0.0, 0.0]), -2.0)):
+        g = GpuProblem(p)
+        for pre in (True, False):
+            x = torch.from_numpy(v0.copy()).cuda()
+            th, info = H.hpsi_davidson(g.plan, x, tol=1e-10, max_iter=50, precondition=pre)
+            assert info["converged"] and info["residual"] <= 1e-10 and abs(th - want) <= 1e-14, (p.psi_len, pre, th, info)
+            assert info["n_matvec"] == 1 and np.allclose(x.cpu().numpy(), v0 / np.linalg.norm(v0), atol=1e-14)
+        x = torch.from_numpy(v0.copy()).cuda()
+        th, info = H.hpsi_lanczos(g.plan, x, tol=1e-10, max_iter=50)
+        assert info["converged"] and abs(th - want) <= 1e-14, (p.psi_len, th, info)
+        X = torch.from_numpy(v0.copy()[None, :]).cuda()
+        thm, infom = H.hpsi_davidson_multi(g.plan, X, 1, tol=1e-10, max_iter=50)
+        assert infom["converged"] and abs(thm[0] - want) <= 1e-14, (p.psi_len, thm, infom)
+
+
+def test_davidson_vanished_correction_takes_the_residual(H):
+    """Reading A21c through the kernels: on a diagonal operator (and one with a diagonal block) the preconditioned
+    correction vanishes with |r| > tol; the solvers go on with the residual and reach LAPACK's eigenvalues with the
+    oracle's mat-vec count."""
+    import torch
+    _, _, diag, mixed = _tiny_eig_problems()
+    rng = np.random.default_rng(3)
+    for p in (diag, mixed):
+        ev = np.linalg.eigvalsh(oracle.dense_hamiltonian(p))
+        g = GpuProblem(p)
+        v0 = rng.standard_normal(p.psi_len)
+        for pre in (True, False):
+            x = torch.from_numpy(v0.copy()).cuda()
+            th, info = H.hpsi_davidson(g.plan, x, tol=1e-10, max_iter=100, precondition=pre)
+            th_o, x_o, nmv_o, rn_o = oracle.davidson(p, v0, tol=1e-10, max_iter=100, precondition=pre)
+            assert info["converged"] and abs(th - ev[0]) <= 1e-12 and abs(th - th_o) <= 1e-12, (pre, th, ev[0], info)
+            assert info["n_matvec"] == nmv_o, (pre, info, nmv_o)
+            xv = x.cpu().numpy()
+            assert min(np.linalg.norm(xv - x_o), np.linalg.norm(xv + x_o)) <= 1e-8
+            V0 = rng.standard_normal((p.psi_len, 2))
+            thm, X, infom = _davidson_multi(H, g, V0, tol=1e-10, max_iter=200, precondition=pre)
+            thb, _, nb, _ = oracle.davidson_block(p, V0, tol=1e-10, max_iter=200, precondition=pre)
+            assert infom["converged"] and np.max(np.abs(thm - ev[:2])) <= 1e-12, (pre, thm, ev[:2], infom)
+            assert infom["n_matvec"] == nb, (pre, infom, nb)
+
+
 def test_davidson_trajectory_matches_oracle(H, small):
     """Step-by-step parity of the driver: without the (ill-conditioned) diagonal preconditioner the Ritz value and
     the residual after k mat-vecs agree with the oracle's textbook Davidson (A21) to rounding."""
