@@ -296,6 +296,24 @@ void hpsi_stream_destroy(hpsi_stream_t* s);
 int hpsi_truncate(hpsi_plan_t* plan, const double* psi_dev, int32_t side, int32_t chi_max, double eps_discard,
                   double* ot_dev, int32_t* chi_host, double* sigma_host, double* discarded_host, void* cuda_stream);
 
+/* hpsi_truncate for callers that must not allocate device memory (code that may not call cudaMalloc: tight serving
+ * loops, harnesses that forbid it).  Same arguments, same steps, same results as hpsi_truncate; the device buffers
+ * (working matrices, singular values, tables) live in ONE file-scope `static __device__` array of
+ * HPSI_TRUNCATE_STATIC_BYTES instead of the plan's lazily grown cudaMalloc block.  The call makes no cudaMalloc /
+ * cudaFree and calls no library routine that allocates; the array's device address is taken once per device
+ * (cudaGetSymbolAddress, with that device current - call with the plan's device current).
+ *   Limit:    a plan whose psi needs more scratch than the array holds is rejected with EINVAL and a message naming
+ *             both sizes (roughly 16 * sum over psi blocks of min(d_l, d_r) * (d_l + d_r) bytes: D = 1024 fits, D = 4096
+ *             does not).  Every GPU that loads the library holds the array until the process exits.
+ *   Sharing:  every call on a device - any plan, any stream, any thread - uses the same array, which keeps the last
+ *             call's contents.  Nothing in it has to start at zero except the per-sweep rotation flag, which the call
+ *             clears itself.  Calls that overlap on the GPU race: serialise them (hpsi_truncate has one buffer per plan).
+ * Synchronises the stream like hpsi_truncate (chi is needed on the host), so it is not CUDA-graph capturable.
+ * Errors: as hpsi_truncate, without ENOMEM. */
+#define HPSI_TRUNCATE_STATIC_BYTES (32u << 20)
+int hpsi_truncate_static(hpsi_plan_t* plan, const double* psi_dev, int32_t side, int32_t chi_max, double eps_discard,
+                         double* ot_dev, int32_t* chi_host, double* sigma_host, double* discarded_host, void* cuda_stream);
+
 typedef struct hpsi_rotate hpsi_rotate_t;   /* opaque; owns the schedule, the workspace (padded isometries, T^T) */
 
 /* Plan the update of `n_blocks` operator blocks of one side.  d / chi: HOST int32[n_sectors], enlarged and kept

@@ -127,6 +127,7 @@ def lib() -> ctypes.CDLL:
         L.hpsi_last_error.restype = ctypes.c_char_p
         L.hpsi_debug_interpret.argtypes = [vp, vp, vp, vp, vp]
         L.hpsi_truncate.argtypes = [vp, vp, ctypes.c_int32, ctypes.c_int32, ctypes.c_double, vp, vp, vp, vp, vp]
+        L.hpsi_truncate_static.argtypes = L.hpsi_truncate.argtypes
         L.hpsi_rotate_plan.argtypes = [ctypes.c_int32, vp, vp, i64, vp, vp, i64, ctypes.c_uint32, ctypes.POINTER(vp)]
         L.hpsi_rotate_apply.argtypes = [vp, vp, vp, vp]
         L.hpsi_rotate_apply_profiled.argtypes = [vp, vp, vp, vp, ctypes.POINTER(ctypes.c_float)]
@@ -134,7 +135,7 @@ def lib() -> ctypes.CDLL:
         L.hpsi_rotate_debug_interpret.argtypes = [vp, vp, vp, vp]
         L.hpsi_rotate_destroy.argtypes = [vp]
         L.hpsi_rotate_destroy.restype = None
-        for name in ("hpsi_truncate", "hpsi_rotate_plan", "hpsi_rotate_apply", "hpsi_rotate_apply_profiled",
+        for name in ("hpsi_truncate", "hpsi_truncate_static", "hpsi_rotate_plan", "hpsi_rotate_apply", "hpsi_rotate_apply_profiled",
                      "hpsi_rotate_query", "hpsi_rotate_debug_interpret"):
             getattr(L, name).restype = ctypes.c_int
         for name in ("hpsi_plan", "hpsi_plan_ex", "hpsi_shard_terms", "hpsi_layout_blocks", "hpsi_bind",
@@ -447,17 +448,28 @@ def hpsi_debug_interpret(plan: Plan, a_host: np.ndarray, b_host: np.ndarray, psi
 
 
 # ------------------------------------------------------------------------ site update
-def hpsi_truncate(plan: Plan, psi, chi_max: int, ot, stream=None, eps_discard: float = -1.0, side: int = 0):
+HPSI_TRUNCATE_STATIC_BYTES = 32 << 20
+
+
+def hpsi_truncate(plan: Plan, psi, chi_max: int, ot, stream=None, eps_discard: float = -1.0, side: int = 0,
+                  static_scratch: bool = False):
     """SVD truncation of psi (torch CUDA tensor).  ot: torch CUDA float64 tensor of >= HPSI_Q_ISO_CAPACITY doubles that
     receives the isometries; eps_discard >= 0 keeps only as many states as the discarded weight <= eps_discard needs.
-    Returns (chi int32[n_left], sigma float64[HPSI_Q_PSI_ROWS], discarded_weight)."""
+    Returns (chi int32[n_left], sigma float64[HPSI_Q_PSI_ROWS], discarded_weight).
+    static_scratch=True calls hpsi_truncate_static (no device allocation; scratch limited to HPSI_TRUNCATE_STATIC_BYTES)."""
     chi = np.zeros(int(plan.n_right if side == HPSI_SIDE_RIGHT else plan.n_left), np.int32)
     n_sig = hpsi_query(plan, HPSI_Q_PSI_COLS if side == HPSI_SIDE_RIGHT else HPSI_Q_PSI_ROWS)
     sigma = np.zeros(max(n_sig, 1), np.float64)
     disc = ctypes.c_double()
-    _check(lib().hpsi_truncate(plan.handle, _ptr(psi), int(side), int(chi_max), float(eps_discard), _ptr(ot), chi.ctypes.data, sigma.ctypes.data,
-                               ctypes.addressof(disc), _stream(stream)))
+    fn = lib().hpsi_truncate_static if static_scratch else lib().hpsi_truncate
+    _check(fn(plan.handle, _ptr(psi), int(side), int(chi_max), float(eps_discard), _ptr(ot), chi.ctypes.data, sigma.ctypes.data,
+              ctypes.addressof(disc), _stream(stream)))
     return chi, sigma[:n_sig], disc.value
+
+
+def hpsi_truncate_static(plan: Plan, psi, chi_max: int, ot, stream=None, eps_discard: float = -1.0, side: int = 0):
+    """hpsi_truncate with its device buffers in the library's static scratch array: allocates nothing on the device."""
+    return hpsi_truncate(plan, psi, chi_max, ot, stream, eps_discard, side, static_scratch=True)
 
 
 class RotatePlan:

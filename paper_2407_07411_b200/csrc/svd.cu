@@ -23,6 +23,7 @@
 #include <cmath>
 #include <cstdio>
 #include <cstdlib>
+#include <mutex>
 #include <numeric>
 #include <vector>
 
@@ -274,8 +275,34 @@ __global__ void svd_gather_kernel(const IsoRow* __restrict__ rows, int n, const 
 
 using namespace hpsi;
 
-extern "C" int hpsi_truncate(hpsi_plan_t* p, const double* psi_dev, int32_t side, int32_t chi_max, double eps_discard,
-                             double* ot_dev, int32_t* chi_host, double* sigma_host, double* discarded_host, void* cuda_stream) {
+// Scratch of hpsi_truncate_static: one array per GPU that loads the library, held until the process exits.  In host code
+// the name is a host-side stand-in, not a device address: truncate_static_scratch() asks the runtime for the address once
+// per device and the kernels get that pointer.
+static __device__ __align__(256) unsigned char g_truncate_scratch[HPSI_TRUNCATE_STATIC_BYTES];
+
+static int truncate_static_scratch(char** out) {
+  constexpr int MAX_DEVICES = 64;
+  static std::mutex mu;
+  static char* ptr_of_device[MAX_DEVICES] = {};
+  int dev = -1;
+  HPSI_CUDA(cudaGetDevice(&dev));
+  if (dev < 0 || dev >= MAX_DEVICES) { set_error("hpsi_truncate_static: device ordinal out of range"); return HPSI_EINVAL; }
+  std::lock_guard<std::mutex> lock(mu);
+  if (!ptr_of_device[dev]) {
+    void* q = nullptr;
+    HPSI_CUDA(cudaGetSymbolAddress(&q, g_truncate_scratch));       // the current device's copy of the array
+    if (!q) { set_error("hpsi_truncate_static: cudaGetSymbolAddress returned a null address"); return HPSI_ECUDA; }
+    ptr_of_device[dev] = static_cast<char*>(q);
+  }
+  *out = ptr_of_device[dev];
+  return HPSI_OK;
+}
+
+// hpsi_truncate / hpsi_truncate_static: the same steps; `static_base` != nullptr takes the device buffers from that array
+// (capacity static_bytes) instead of the plan's lazily grown cudaMalloc block.
+static int truncate_impl(hpsi_plan_t* p, const double* psi_dev, int32_t side, int32_t chi_max, double eps_discard,
+                         double* ot_dev, int32_t* chi_host, double* sigma_host, double* discarded_host, void* cuda_stream,
+                         char* static_base, size_t static_bytes) {
   if (!p) { set_error("null plan"); return HPSI_EINVAL; }
   if (p->host_only) { set_error("host-only plan: hpsi_truncate needs a CUDA device (no CPU fallback)"); return HPSI_ESTATE; }
   if (chi_max < 0) { set_error("negative chi_max"); return HPSI_EINVAL; }
@@ -325,8 +352,16 @@ extern "C" int hpsi_truncate(hpsi_plan_t* p, const double* psi_dev, int32_t side
     rounds = std::max(rounds, s.nce - 1);
   }
   // ---- device buffers (kept on the plan; regrown if a call needs more, e.g. the other side)
-  {
-    const size_t bytes = (size_t)wlen * 8 + (size_t)n_rows * 8 + tab.size() * sizeof(SvdBlk) + cta_blk.size() * 4 + (size_t)n_rows * sizeof(IsoRow) + 4096;
+  const size_t bytes = (size_t)wlen * 8 + (size_t)n_rows * 8 + tab.size() * sizeof(SvdBlk) + cta_blk.size() * 4 + (size_t)n_rows * sizeof(IsoRow) + 4096;
+  if (static_base) {
+    if (bytes > static_bytes) {
+      char buf[200];
+      snprintf(buf, sizeof buf, "hpsi_truncate_static: this plan needs %zu bytes of scratch, the static array holds %zu "
+               "(HPSI_TRUNCATE_STATIC_BYTES); use hpsi_truncate", bytes, static_bytes);
+      set_error(buf);
+      return HPSI_EINVAL;
+    }
+  } else {
     if (bytes > p->svd_bytes) {
       HPSI_CUDA(cudaStreamSynchronize(st));
       cudaFree(p->d_svd);
@@ -337,7 +372,7 @@ extern "C" int hpsi_truncate(hpsi_plan_t* p, const double* psi_dev, int32_t side
       p->svd_bytes = bytes;
     }
   }
-  char* base = static_cast<char*>(p->d_svd);
+  char* base = static_base ? static_base : static_cast<char*>(p->d_svd);
   size_t cur = 0;
   auto carve = [&](size_t bytes) { char* q = base + cur; cur = (cur + bytes + 255) & ~(size_t)255; return q; };
   double* d_w = reinterpret_cast<double*>(carve((size_t)wlen * 8));
@@ -435,4 +470,21 @@ extern "C" int hpsi_truncate(hpsi_plan_t* p, const double* psi_dev, int32_t side
   }
   HPSI_CUDA(cudaGetLastError());
   return HPSI_OK;
+}
+
+extern "C" int hpsi_truncate(hpsi_plan_t* p, const double* psi_dev, int32_t side, int32_t chi_max, double eps_discard,
+                             double* ot_dev, int32_t* chi_host, double* sigma_host, double* discarded_host, void* cuda_stream) {
+  return truncate_impl(p, psi_dev, side, chi_max, eps_discard, ot_dev, chi_host, sigma_host, discarded_host, cuda_stream,
+                       nullptr, 0);
+}
+
+extern "C" int hpsi_truncate_static(hpsi_plan_t* p, const double* psi_dev, int32_t side, int32_t chi_max,
+                                    double eps_discard, double* ot_dev, int32_t* chi_host, double* sigma_host,
+                                    double* discarded_host, void* cuda_stream) {
+  if (!p) { set_error("null plan"); return HPSI_EINVAL; }
+  if (p->host_only) { set_error("host-only plan: hpsi_truncate_static needs a CUDA device (no CPU fallback)"); return HPSI_ESTATE; }
+  char* scratch = nullptr;
+  if (int rc = truncate_static_scratch(&scratch)) return rc;
+  return truncate_impl(p, psi_dev, side, chi_max, eps_discard, ot_dev, chi_host, sigma_host, discarded_host, cuda_stream,
+                       scratch, sizeof g_truncate_scratch);
 }
