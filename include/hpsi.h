@@ -176,6 +176,23 @@ int hpsi_apply_multi(hpsi_plan_t* plan, const double* psi_dev, int64_t ld_psi, d
  * parts_dev (in place over shard 0) but must not overlap it otherwise.  Enqueue only. */
 int hpsi_sum_shards(const double* parts_dev, int32_t n_parts, int64_t n, double* out_dev, void* cuda_stream);
 
+/* Eigensolvers on a term-sharded plan ("eight GPU accelerated diagonalization procedure"):
+ * every rank runs the same hpsi_davidson / hpsi_davidson_multi / hpsi_lanczos call on its shard plan with the same start
+ * vector, and the solver hands every product it computes to `fn` before using it:
+ *   fn(user, v_dev, w_dev, n, n_vectors, ld, cuda_stream)
+ *     w_dev   DEVICE, in/out: n_vectors vectors of n doubles, ld doubles apart - on entry this rank's partial results
+ *             (the sum over ITS terms), on return (stream order) the sum over all ranks
+ *     v_dev   DEVICE, the vectors that were multiplied (same layout), or NULL when w_dev is the partial diag(H)
+ *   fn only enqueues on cuda_stream (e.g. NCCL all-gather of w + hpsi_sum_shards in rank order) and returns 0; any other
+ *   value makes the solver return HPSI_ESTATE.  The sum must have the same bits on every rank (hpsi_sum_shards does):
+ *   the ranks then take the same decisions and issue the same sequence of calls, which a collective needs.  While an
+ *   exchange is set, hpsi_davidson reads each iteration's scalars after its orthogonalisation instead of beside it, so that
+ *   the decision never depends on timing.  hpsi_apply / hpsi_diagonal themselves never call fn.
+ * fn = NULL removes the hook.  `user` is BORROWED.  Not called for plans without it: single-GPU behaviour is unchanged. */
+typedef int (*hpsi_exchange_fn)(void* user, const double* v_dev, double* w_dev, int64_t n, int32_t n_vectors, int64_t ld,
+                                void* cuda_stream);
+int hpsi_set_exchange(hpsi_plan_t* plan, hpsi_exchange_fn fn, void* user);
+
 /* hpsi_apply with a CUDA event between its kernels: ms_host (HOST, 4 floats) receives the device time of
  * [prep, first-GEMM kernel, second-GEMM kernel, reduce].  Synchronises the stream.  For bench.py's roofline object. */
 int hpsi_apply_profiled(hpsi_plan_t* plan, const double* psi_dev, double* out_dev, void* cuda_stream, float* ms_host);

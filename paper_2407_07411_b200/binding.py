@@ -126,6 +126,8 @@ def lib() -> ctypes.CDLL:
         L.hpsi_destroy.restype = None
         L.hpsi_last_error.restype = ctypes.c_char_p
         L.hpsi_debug_interpret.argtypes = [vp, vp, vp, vp, vp]
+        L.hpsi_set_exchange.argtypes = [vp, vp, vp]
+        L.hpsi_set_exchange.restype = ctypes.c_int
         L.hpsi_truncate.argtypes = [vp, vp, ctypes.c_int32, ctypes.c_int32, ctypes.c_double, vp, vp, vp, vp, vp]
         L.hpsi_truncate_static.argtypes = L.hpsi_truncate.argtypes
         L.hpsi_rotate_plan.argtypes = [ctypes.c_int32, vp, vp, i64, vp, vp, i64, ctypes.c_uint32, ctypes.POINTER(vp)]
@@ -328,6 +330,42 @@ def hpsi_davidson_multi(plan: Plan, psi_inout, n_roots: int, tol: float = 1e-8, 
     _check(lib().hpsi_davidson_multi(plan.handle, _ptr(psi_inout), int(psi_inout.shape[1]), int(n_roots), eig.ctypes.data,
                                      res.ctypes.data, ctypes.byref(prm), ctypes.byref(info), _stream(stream)))
     return eig, {"n_matvec": info.n_matvec, "converged": bool(info.converged), "residual": info.residual, "residuals": res}
+
+
+EXCHANGE_FN = ctypes.CFUNCTYPE(ctypes.c_int, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int64,
+                               ctypes.c_int32, ctypes.c_int64, ctypes.c_void_p)
+
+
+def device_tensor(ptr: int, shape, torch_module):
+    """A float64 torch view of device memory the library owns (row-major ``shape``, no copy, no allocation): what an
+    exchange callback wraps its pointers in to hand them to torch.distributed."""
+    class _View:
+        __cuda_array_interface__ = {"shape": tuple(int(x) for x in shape), "typestr": "<f8", "data": (int(ptr), False),
+                                    "version": 3, "strides": None}
+    return torch_module.as_tensor(_View(), device="cuda")
+
+
+def hpsi_set_exchange(plan: Plan, fn) -> None:
+    """fn(v_ptr | None, w_ptr, n, n_vectors, ld, stream_ptr) is called by hpsi_davidson / hpsi_davidson_multi /
+    hpsi_lanczos after every mat-vec (and once for diag(H), v_ptr None) on a term-sharded plan; it enqueues the sum over
+    ranks into w.  fn = None removes the hook.  A Python exception inside fn makes the solver fail with HPSI_ESTATE; the
+    exception is kept in ``plan.exchange_error``."""
+    if fn is None:
+        _check(lib().hpsi_set_exchange(plan.handle, None, None))
+        plan._exchange_cb = None
+        return
+    plan.exchange_error = None
+
+    def trampoline(_user, v, w, n, nvec, ld, stream):
+        try:
+            fn(v, w, int(n), int(nvec), int(ld), stream)
+            return 0
+        except BaseException as e:                       # never unwind through the C frames
+            plan.exchange_error = e
+            return 1
+    cb = EXCHANGE_FN(trampoline)
+    _check(lib().hpsi_set_exchange(plan.handle, ctypes.cast(cb, ctypes.c_void_p), None))
+    plan._exchange_cb = cb                               # keeps the thunk alive as long as the plan
 
 
 def hpsi_lanczos(plan: Plan, psi_inout, tol: float = 1e-8, max_iter: int = 200, m_max: int = 16, stream=None):

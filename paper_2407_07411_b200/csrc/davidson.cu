@@ -5,6 +5,7 @@
 // mat-vec is enqueued without a bubble.  All reductions are two-stage with a fixed order: bitwise reproducible.
 #include <algorithm>
 #include <cmath>
+#include <string>
 #include <vector>
 
 #include "plan_dev.h"
@@ -349,6 +350,24 @@ __global__ void reset_gram_kernel(double* G, const double* theta, const double* 
 
 }  // namespace
 
+// hpsi_set_exchange hook: w (this rank's partial products of v, or partial diag(H) when v == nullptr) -> sum over ranks
+static int exchange(hpsi_plan_t* p, const double* v, double* w, int64_t n, int nvec, int64_t ld, void* cuda_stream) {
+  if (!p->exchange_fn) return HPSI_OK;
+  const int rc = p->exchange_fn(p->exchange_user, v, w, n, nvec, ld, cuda_stream);
+  if (rc != 0) {
+    hpsi::set_error("the exchange callback (hpsi_set_exchange) failed with code " + std::to_string(rc));
+    return HPSI_ESTATE;
+  }
+  return HPSI_OK;
+}
+
+extern "C" int hpsi_set_exchange(hpsi_plan_t* p, hpsi_exchange_fn fn, void* user) {
+  if (!p) { hpsi::set_error("null plan"); return HPSI_EINVAL; }
+  p->exchange_fn = fn;
+  p->exchange_user = fn ? user : nullptr;
+  return HPSI_OK;
+}
+
 extern "C" int hpsi_davidson(hpsi_plan_t* p, double* psi, double* eig_host, const hpsi_davidson_params_t* params,
                              hpsi_davidson_info_t* info, void* cuda_stream) {
   using namespace hpsi;
@@ -400,11 +419,15 @@ extern "C" int hpsi_davidson(hpsi_plan_t* p, double* psi, double* eig_host, cons
     dot_kernel<<<dim3(NB, nvec), 256, 0, st>>>(X, n, yv, n, partial, tickets + 8, out, stride, mirror, mstride);
   };
   int rc;
-  if (prm.precondition && (rc = hpsi_diagonal(p, diag, cuda_stream)) != HPSI_OK) return rc;
+  if (prm.precondition) {
+    if ((rc = hpsi_diagonal(p, diag, cuda_stream)) != HPSI_OK) return rc;
+    if ((rc = exchange(p, nullptr, diag, n, 1, n, cuda_stream)) != HPSI_OK) return rc;
+  }
 
   // V0 = psi/|psi| ; W0 = H V0   (the normalisation rides on the mat-vec's prep kernel)
   dots(psi, 1, psi, ctl, 1, nullptr, 0);
   if ((rc = apply_impl(p, psi, W, false, cuda_stream, ctl, V)) != HPSI_OK) return rc;
+  if ((rc = exchange(p, V, W, n, 1, n, cuda_stream)) != HPSI_OK) return rc;
   int j = 1, nmv = 1, converged = 0;
   int j_good = 1;                                        // columns of V / W that were valid when the last correction vector was built
   double rn = INFINITY, th = 0.0;
@@ -416,11 +439,17 @@ extern "C" int hpsi_davidson(hpsi_plan_t* p, double* psi, double* eig_host, cons
     jp = j;
     dav_ritz_kernel<<<NB, 256, 0, st>>>(V, W, diag, n, j, y, theta, prm.precondition, x, wy, r, s, partial, tickets + 1, c,
                                          ctl + 1, ctl);
-    // theta and |r|^2 travel to the host on a side stream while the orthogonalisation below is still running
-    HPSI_CUDA(cudaEventRecord(p->dav_ev[0], st));
-    HPSI_CUDA(cudaStreamWaitEvent(p->dav_side, p->dav_ev[0], 0));
-    HPSI_CUDA(cudaMemcpyAsync(hostbuf, theta, 7 * sizeof(double), cudaMemcpyDeviceToHost, p->dav_side));
-    HPSI_CUDA(cudaEventRecord(p->dav_ev[1], p->dav_side));
+    // theta and |r|^2 travel to the host on a side stream while the orthogonalisation below is still running.  With an
+    // exchange hook (ranks in lockstep) the copy waits for the orthogonalisation: whether it sees this iteration's dead flag
+    // must not depend on timing, or the ranks would issue different numbers of mat-vecs.
+    auto read_back = [&]() -> int {
+      HPSI_CUDA(cudaEventRecord(p->dav_ev[0], st));
+      HPSI_CUDA(cudaStreamWaitEvent(p->dav_side, p->dav_ev[0], 0));
+      HPSI_CUDA(cudaMemcpyAsync(hostbuf, theta, 7 * sizeof(double), cudaMemcpyDeviceToHost, p->dav_side));
+      HPSI_CUDA(cudaEventRecord(p->dav_ev[1], p->dav_side));
+      return HPSI_OK;
+    };
+    if (!p->exchange_fn && (rc = read_back()) != HPSI_OK) return rc;
     if (j >= prm.m_max) {                                           // restart with V = [x/|x|]
       dots(x, 1, x, ctl + 2, 1, nullptr, 0);
       scale_kernel<<<eg, 256, 0, st>>>(V, x, W, wy, ctl + 2, n, ctl + 5);
@@ -433,6 +462,7 @@ extern "C" int hpsi_davidson(hpsi_plan_t* p, double* psi, double* eig_host, cons
     const double stamp = (double)(it + 1);
     dav_project_kernel<<<NB, 256, 0, st>>>(s, V, n, j, c, partial, tickets + 2, c2, nullptr, ctl, stamp);
     dav_project_kernel<<<NB, 256, 0, st>>>(s, V, n, j, c2, partial, tickets + 3, nullptr, ctl + 3, ctl, stamp);
+    if (p->exchange_fn && (rc = read_back()) != HPSI_OK) return rc;
     HPSI_CUDA(cudaEventSynchronize(p->dav_ev[1]));
     th = hostbuf[0];
     rn = std::sqrt(hostbuf[2]);
@@ -462,6 +492,7 @@ extern "C" int hpsi_davidson(hpsi_plan_t* p, double* psi, double* eig_host, cons
     // V_j = s/|s| (written by the prep kernel), W_j = H V_j - enqueued while the orthogonalisation may still be running
     j_good = j;
     if ((rc = apply_impl(p, s, W + (size_t)j * n, false, cuda_stream, ctl + 3, V + (size_t)j * n)) != HPSI_OK) return rc;
+    if ((rc = exchange(p, V + (size_t)j * n, W + (size_t)j * n, n, 1, n, cuda_stream)) != HPSI_OK) return rc;
     ++j;
     ++nmv;
   }
@@ -570,6 +601,7 @@ extern "C" int hpsi_davidson_multi(hpsi_plan_t* p, double* psi, int64_t ld, int3
       const int nb = std::min(p->sc.nvec, cnt - off);
       int rc = apply_impl(p, V + (size_t)(j0 + off) * n, W + (size_t)(j0 + off) * n, false, cuda_stream, nullptr, nullptr, nb, n, n);
       if (rc != HPSI_OK) return rc;
+      if ((rc = exchange(p, V + (size_t)(j0 + off) * n, W + (size_t)(j0 + off) * n, n, nb, n, cuda_stream)) != HPSI_OK) return rc;
     }
     return HPSI_OK;
   };
@@ -583,7 +615,10 @@ extern "C" int hpsi_davidson_multi(hpsi_plan_t* p, double* psi, int64_t ld, int3
     scale_kernel<<<eg, 256, 0, st>>>(V + (size_t)j * n, s, nullptr, nullptr, nrm + slot, n);
   };
   int rc;
-  if (prm.precondition && (rc = hpsi_diagonal(p, diag, cuda_stream)) != HPSI_OK) return rc;
+  if (prm.precondition) {
+    if ((rc = hpsi_diagonal(p, diag, cuda_stream)) != HPSI_OK) return rc;
+    if ((rc = exchange(p, nullptr, diag, n, 1, n, cuda_stream)) != HPSI_OK) return rc;
+  }
 
   // start vectors, orthonormalised one after the other
   for (int i = 0; i < k; ++i) {
@@ -741,6 +776,7 @@ extern "C" int hpsi_lanczos(hpsi_plan_t* p, double* psi, double* eig_host, const
   double* host = p->h_dav;
   for (;;) {
     if ((rc = hpsi_apply(p, V + (size_t)j * n, w, cuda_stream)) != HPSI_OK) return rc;
+    if ((rc = exchange(p, V + (size_t)j * n, w, n, 1, n, cuda_stream)) != HPSI_OK) return rc;
     ++nmv;
     dots(V, j + 1, w, c);                                            // c[j] = alpha_j
     project_kernel<<<eg, 256, 0, st>>>(w, V, n, j + 1, c);           // three-term recurrence + re-orthogonalisation
@@ -772,6 +808,7 @@ extern "C" int hpsi_lanczos(hpsi_plan_t* p, double* psi, double* eig_host, const
   // psi = x/|x| ; true residual |H psi - theta psi|
   scale_kernel<<<eg, 256, 0, st>>>(psi, x, nullptr, nullptr, nrm + 2, n);
   if ((rc = hpsi_apply(p, psi, w, cuda_stream)) != HPSI_OK) return rc;
+  if ((rc = exchange(p, psi, w, n, 1, n, cuda_stream)) != HPSI_OK) return rc;
   ++nmv;
   set_scalar_kernel<<<1, 1, 0, st>>>(c, theta);
   project_kernel<<<eg, 256, 0, st>>>(w, psi, n, 1, c);

@@ -28,6 +28,9 @@ struct hpsi_plan {
   double* h_dav = nullptr;        // pinned host scalars the Davidson loop reads back each iteration
   cudaStream_t dav_side = nullptr;   // side stream + events: the read-back of an iteration's residual overlaps its
   cudaEvent_t dav_ev[2] = {nullptr, nullptr};   // orthogonalisation kernels (davidson.cu)
+  // hpsi_set_exchange: called by the eigensolvers after every mat-vec / diagonal they compute (term-sharded plans)
+  hpsi_exchange_fn exchange_fn = nullptr;
+  void* exchange_user = nullptr;
   // hpsi_truncate (svd.cu)
   int n_left = 0, n_right = 0;    // sectors of the sector table (length of chi_host for either side)
   void* d_svd = nullptr;          // working matrices, singular values, tables (allocated on first use)

@@ -645,6 +645,89 @@ def test_davidson_vanished_correction_takes_the_residual(H):
             assert infom["n_matvec"] == nb, (pre, infom, nb)
 
 
+class _EmulatedRanks:
+    """The exchange hook of a term-sharded eigensolver with all ranks on one GPU (B200_PROFILING.md: emulate the ranks as
+    kernels over all ranks' data, never as processes whose kernels wait on one another): the callback plays ranks 1 ..
+    world-1 - it multiplies the same vectors by their shard plans - and adds the partial results in rank order with
+    hpsi_sum_shards, which is what all-gather + hpsi_sum_shards leaves on every rank of a real run."""
+
+    def __init__(self, H, torch, p, world, n_vectors=1):
+        self.H, self.torch, self.world = H, torch, world
+        shard, _ = H.hpsi_shard_terms(p, world)
+        self.a, self.b = torch.from_numpy(p.a_data).cuda(), torch.from_numpy(p.b_data).cuda()
+        self.plans = [H.plan_problem(p, self.a, self.b, shard_of_term=shard, shard_index=r, n_vectors=n_vectors)
+                      for r in range(world)]
+        self.n = H.hpsi_query(self.plans[0], H.HPSI_Q_PSI_LENGTH)
+        self.buf = torch.empty((world, self.n), dtype=torch.float64, device="cuda")
+        self.calls, self.diag_calls = 0, 0
+        H.hpsi_set_exchange(self.plans[0], self)
+
+    def __call__(self, v, w, n, nvec, ld, stream):
+        H, torch = self.H, self.torch
+        assert n == self.n and (stream or 0) == torch.cuda.current_stream().cuda_stream
+        st = torch.cuda.current_stream()
+        wt = H.device_tensor(w, (nvec, ld), torch)
+        if v is None:
+            self.diag_calls += 1
+            assert nvec == 1
+            self.buf[0].copy_(wt[0, :n])
+            for r in range(1, self.world):
+                H.hpsi_diagonal(self.plans[r], self.buf[r], st)
+            H.hpsi_sum_shards(self.buf, self.world, wt[0, :n], st)
+            return
+        self.calls += 1
+        vt = H.device_tensor(v, (nvec, ld), torch)
+        for k in range(nvec):
+            self.buf[0].copy_(wt[k, :n])
+            for r in range(1, self.world):
+                H.hpsi_apply(self.plans[r], vt[k, :n], self.buf[r], st)
+            H.hpsi_sum_shards(self.buf, self.world, wt[k, :n], st)
+
+
+def test_eigensolvers_on_term_shards_through_the_exchange_hook(H, toy):
+    """hpsi_set_exchange: the solvers run on rank 0's shard plan, every product (and diag(H)) passes through the hook, and
+    the result is the full operator's eigenpair - LAPACK on the dense toy H, and the single-plan solvers."""
+    import torch
+    ev = np.linalg.eigvalsh(oracle.dense_hamiltonian(toy))
+    Hd = oracle.dense_hamiltonian(toy)
+    v0 = workloads.make_psi(toy)
+    full = GpuProblem(toy)
+    for world in (2, 3):
+        ranks = _EmulatedRanks(H, torch, toy, world)
+        plan0 = ranks.plans[0]
+        for pre in (True, False):
+            ranks.calls = ranks.diag_calls = 0
+            x = torch.from_numpy(v0.copy()).cuda()
+            th, info = H.hpsi_davidson(plan0, x, tol=1e-9, max_iter=400, precondition=pre)
+            th1, _, info1 = _davidson(H, full, v0, tol=1e-9, max_iter=400, precondition=pre)
+            assert info["converged"] and abs(th - ev[0]) <= 1e-10 and abs(th - th1) <= 1e-10, (world, pre, th, ev[0], info)
+            assert ranks.calls == info["n_matvec"] and ranks.diag_calls == (1 if pre else 0)
+            assert abs(info["n_matvec"] - info1["n_matvec"]) <= 2                   # same method, sums in another order
+            xv = x.cpu().numpy()
+            assert np.linalg.norm(Hd @ xv - th * xv) <= 1e-8
+        ranks.calls = 0
+        x = torch.from_numpy(v0.copy()).cuda()
+        th, info = H.hpsi_lanczos(plan0, x, tol=1e-9, max_iter=400)
+        assert info["converged"] and abs(th - ev[0]) <= 1e-10 and ranks.calls == info["n_matvec"]
+    # block Davidson on a batched shard plan: the hook receives several vectors per call
+    ranks = _EmulatedRanks(H, torch, toy, 2, n_vectors=3)
+    V0 = np.random.default_rng(3).standard_normal((toy.psi_len, 3))
+    X = torch.from_numpy(np.ascontiguousarray(V0.T)).cuda()
+    th, info = H.hpsi_davidson_multi(ranks.plans[0], X, 3, tol=1e-9, max_iter=800)
+    assert info["converged"] and np.max(np.abs(th - ev[:3])) <= 1e-10, (th, ev[:3], info)
+    assert ranks.diag_calls == 1 and 1 <= ranks.calls <= info["n_matvec"]
+    # a failing hook stops the solver with ESTATE; removing the hook gives the shard's own (different) operator
+    def boom(*_a):
+        raise RuntimeError("link down")
+    H.hpsi_set_exchange(ranks.plans[0], boom)
+    with pytest.raises(H.HpsiError) as e:
+        H.hpsi_davidson(ranks.plans[0], torch.from_numpy(v0.copy()).cuda(), tol=1e-9)
+    assert e.value.code == H.HPSI_ESTATE and isinstance(ranks.plans[0].exchange_error, RuntimeError)
+    H.hpsi_set_exchange(ranks.plans[0], None)
+    th_s, info_s = H.hpsi_davidson(ranks.plans[0], torch.from_numpy(v0.copy()).cuda(), tol=1e-9, max_iter=400)
+    assert abs(th_s - ev[0]) > 1e-6
+
+
 def test_davidson_trajectory_matches_oracle(H, small):
     """Step-by-step parity of the driver: without the (ill-conditioned) diagonal preconditioner the Ritz value and
     the residual after k mat-vecs agree with the oracle's textbook Davidson (A21) to rounding."""

@@ -431,6 +431,14 @@ def test_mixed_storage_interpreter(seed):
                 assert np.linalg.norm(got - ref) <= 1e-13 * max(np.linalg.norm(ref), 1.0), (grid, k, flags)
 
 
+def test_set_exchange_arguments(toy):
+    """hpsi_set_exchange on a host-only plan: setting and clearing the hook are plain state changes; a null plan is EINVAL."""
+    plan = host_plan(toy)
+    H.hpsi_set_exchange(plan, lambda *a: None)
+    H.hpsi_set_exchange(plan, None)
+    assert H.lib().hpsi_set_exchange(None, None, None) == H.HPSI_EINVAL
+
+
 def test_transposed_block_validation(toy):
     shared = workloads.make_problem("toy", share_adjoint=True)
     bad = shared.a_desc.copy()
