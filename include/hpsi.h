@@ -370,6 +370,14 @@ void hpsi_rotate_destroy(hpsi_rotate_t* r);
  * ot_host: isometries, out_host: HPSI_RQ_OUT_LENGTH doubles) */
 int hpsi_rotate_debug_interpret(const hpsi_rotate_t* r, const double* a_host, const double* ot_host, double* out_host);
 
+/* test entry point: the subspace eigensolver of hpsi_davidson / hpsi_lanczos (k = 1: tridiagonalisation + bisection +
+ * inverse iteration by one warp, with the Jacobi solver as fallback; k > 1: the Jacobi solver) on ONE symmetric matrix.
+ * g_host: HOST, j x j row-major, 1 <= j <= 32; theta_host: HOST, k values ascending; y_host: HOST, k x j (row r = the
+ * r-th eigenvector); fell_back_host: HOST or NULL, 1 if the k = 1 path failed its own check and the Jacobi solver ran.
+ * Allocates and frees device memory, synchronises the device. */
+int hpsi_debug_small_eig(const double* g_host, int32_t j, int32_t k, double* theta_host, double* y_host,
+                         int32_t* fell_back_host);
+
 /* hpsi_query items.  `out` is HOST; `bytes` must be >= the item's size (else EINVAL). */
 enum {
   HPSI_Q_PSI_LENGTH = 0,     /* int64: doubles in psi / out                                                  */

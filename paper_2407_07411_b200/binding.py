@@ -489,6 +489,19 @@ def hpsi_debug_interpret(plan: Plan, a_host: np.ndarray, b_host: np.ndarray, psi
 HPSI_TRUNCATE_STATIC_BYTES = 32 << 20
 
 
+def hpsi_debug_small_eig(g: np.ndarray, k: int = 1):
+    """The drivers' subspace eigensolver on one symmetric matrix: (theta[k], y[k, j], fell_back)."""
+    g = np.ascontiguousarray(g, np.float64)
+    j = g.shape[0]
+    theta, y, fb = np.zeros(k), np.zeros((k, j)), ctypes.c_int32()
+    L = lib()
+    L.hpsi_debug_small_eig.argtypes = [ctypes.c_void_p, ctypes.c_int32, ctypes.c_int32, ctypes.c_void_p, ctypes.c_void_p,
+                                       ctypes.c_void_p]
+    L.hpsi_debug_small_eig.restype = ctypes.c_int
+    _check(L.hpsi_debug_small_eig(g.ctypes.data, j, int(k), theta.ctypes.data, y.ctypes.data, ctypes.addressof(fb)))
+    return theta, y, bool(fb.value)
+
+
 def hpsi_truncate(plan: Plan, psi, chi_max: int, ot, stream=None, eps_discard: float = -1.0, side: int = 0,
                   static_scratch: bool = False):
     """SVD truncation of psi (torch CUDA tensor).  ot: torch CUDA float64 tensor of >= HPSI_Q_ISO_CAPACITY doubles that

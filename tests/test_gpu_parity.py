@@ -728,6 +728,71 @@ def test_eigensolvers_on_term_shards_through_the_exchange_hook(H, toy):
     assert abs(th_s - ev[0]) > 1e-6
 
 
+def _small_eig_cases(n, seed=0):
+    """Symmetric matrices of order 1 .. 32: dense Gaussian, diagonal, zero, a degenerate lowest eigenvalue, an arrowhead
+    with 1e-9 coupling (a Davidson subspace matrix near convergence), scaled by 1e+150 / 1e-150, a lowest pair 1e-13
+    apart, and a Lanczos tridiagonal whose lowest Ritz value has converged."""
+    rng = np.random.default_rng(seed)
+    for trial in range(n):
+        j, kind = int(rng.integers(1, 33)), trial % 9
+        if kind == 0:
+            A = rng.standard_normal((j, j))
+        elif kind == 1:
+            A = np.diag(rng.standard_normal(j))
+        elif kind == 2:
+            A = np.zeros((j, j))
+        elif kind in (3, 7):
+            Q, _ = np.linalg.qr(rng.standard_normal((j, j)))
+            lam = np.sort(rng.standard_normal(j))
+            if kind == 3:
+                lam[:min(3, j)] = lam[0]
+            else:
+                lam = np.concatenate([[-1.0, -1.0 + 1e-13], rng.random(max(j - 2, 0))])[:j]
+            A = Q @ np.diag(lam) @ Q.T
+        elif kind == 4:
+            A = np.diag(np.sort(rng.standard_normal(j)) * 10)
+            A[-1, :] = A[:, -1] = rng.standard_normal(j) * 1e-9
+            A[-1, -1] = rng.standard_normal()
+        elif kind in (5, 6):
+            A = rng.standard_normal((j, j)) * (1e-150 if kind == 5 else 1e150)
+        else:
+            n_big = 200
+            M = rng.standard_normal((n_big, n_big))
+            M, q, qp, b, V, al, be = M + M.T, rng.standard_normal(n_big), np.zeros(n_big), 0.0, [], [], []
+            q /= np.linalg.norm(q)
+            for _ in range(j):
+                w = M @ q - b * qp
+                a = q @ w
+                w -= a * q
+                for u in V:
+                    w -= u * (u @ w)
+                V.append(q)
+                al.append(a)
+                b = np.linalg.norm(w)
+                be.append(b)
+                qp, q = q, w / b
+            A = np.diag(al) + np.diag(be[:-1], 1) + np.diag(be[:-1], -1)
+        yield kind, 0.5 * (A + A.T)
+
+
+def test_subspace_eigensolver_vs_lapack(H):
+    """hpsi_debug_small_eig: the drivers' subspace solver on its own.  k = 1 (tridiagonalisation, multisection on the Sturm
+    count, inverse iteration): lowest eigenvalue against LAPACK, residual of the vector, and the solver must not have
+    needed its Jacobi fallback; k = 3 (the Jacobi solver of hpsi_davidson_multi): the three lowest pairs."""
+    for kind, A in _small_eig_cases(1500):
+        j = A.shape[0]
+        ev = np.linalg.eigvalsh(A)
+        sc = max(np.abs(ev).max(), 1e-300)
+        th, y, fell_back = H.hpsi_debug_small_eig(A, 1)
+        assert abs(th[0] - ev[0]) <= 1e-13 * sc and not fell_back, (kind, j, th[0], ev[0], fell_back)
+        assert np.linalg.norm(A @ y[0] - th[0] * y[0]) <= 1e-12 * sc and abs(np.linalg.norm(y[0]) - 1.0) <= 1e-12, (kind, j)
+        if j >= 3 and kind in (0, 1, 3, 4, 8):           # (the Jacobi solver's thresholds are absolute: not for 1e+-150 scales)
+            th3, y3, _ = H.hpsi_debug_small_eig(A, 3)
+            assert np.max(np.abs(th3 - ev[:3])) <= 1e-12 * sc, (kind, j, th3, ev[:3])
+            assert np.max(np.abs(y3 @ y3.T - np.eye(3))) <= 1e-12
+            assert np.max(np.linalg.norm(A @ y3.T - y3.T * th3[None, :], axis=0)) <= 1e-11 * sc
+
+
 def test_davidson_trajectory_matches_oracle(H, small):
     """Step-by-step parity of the driver: without the (ill-conditioned) diagonal preconditioner the Ritz value and
     the residual after k mat-vecs agree with the oracle's textbook Davidson (A21) to rounding."""
