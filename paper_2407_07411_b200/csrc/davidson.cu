@@ -12,6 +12,9 @@
 
 namespace {
 
+using hpsi::launch_dependent;   // kernels.cuh: every kernel of this file starts with pdl_wait() and is launched as a dependent
+using hpsi::pdl_wait;           // of the kernel before it in the stream (launch latency of ~9 boundaries per iteration)
+
 constexpr int NB = 256;       // partial blocks per dot product
 constexpr int MMAX = 32;
 
@@ -22,6 +25,7 @@ constexpr int MMAX = 32;
 __global__ void dot_kernel(const double* __restrict__ X, int64_t ldx, const double* __restrict__ y, int64_t n,
                            double* __restrict__ partial, unsigned int* __restrict__ counters, double* out, int stride,
                            double* mirror, int mstride) {
+  pdl_wait();
   __shared__ double red[256];
   __shared__ bool last;
   const int v = blockIdx.y;
@@ -59,6 +63,7 @@ __global__ void dot_kernel(const double* __restrict__ X, int64_t ldx, const doub
 // dst = src / sqrt(*nrm2)   (dst2 = src2 / sqrt(*nrm2) if given)
 __global__ void scale_kernel(double* dst, const double* src, double* dst2, const double* src2, const double* nrm2,
                              int64_t n, const double* dead = nullptr) {
+  pdl_wait();
   if (dead && *dead != 0.0) return;
   const double inv = 1.0 / sqrt(*nrm2);
   for (int64_t e = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; e < n; e += (int64_t)gridDim.x * blockDim.x) {
@@ -406,6 +411,7 @@ __device__ void small_eig_lowest_or_jacobi(const double* __restrict__ G, int j, 
 
 __global__ void small_eig_kernel(const double* __restrict__ G, int j, double* theta, double* y, int k,
                                  int* fell_back = nullptr) {
+  pdl_wait();
   __shared__ EigSmem sm;
   if (threadIdx.x == 0) sm.ok = 0;
   __syncthreads();
@@ -452,6 +458,7 @@ __global__ void __launch_bounds__(256) dav_gram_eig_kernel(const double* __restr
                                                            int j, double* partial, unsigned int* ticket, double* G,
                                                            double* theta, double* y, const double* ctl, double* Qp,
                                                            double* Lp, int warm) {
+  pdl_wait();
   __shared__ EigSmem sm;
   if (ctl[5] != 0.0) return;
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
@@ -482,6 +489,7 @@ __global__ void __launch_bounds__(256) dav_ritz_kernel(const double* __restrict_
                                                        int precondition, double* x, double* wy, double* r, double* s,
                                                        double* partial, unsigned int* ticket, double* c, double* nrm_r2,
                                                        const double* ctl) {
+  pdl_wait();
   if (ctl[5] != 0.0) return;
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
   const double th = *theta;
@@ -522,6 +530,7 @@ __global__ void __launch_bounds__(256) dav_project_kernel(double* s, const doubl
                                                           const double* __restrict__ c_in, double* partial,
                                                           unsigned int* ticket, double* c_out, double* nrm_s2, double* ctl,
                                                           double stamp) {
+  pdl_wait();
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
   int64_t lo, hi;
   dav_slice(n, lo, hi);
@@ -552,6 +561,7 @@ __global__ void __launch_bounds__(256) dav_project_kernel(double* s, const doubl
 
 // s -= sum_i c_i V_i
 __global__ void project_kernel(double* s, const double* __restrict__ V, int64_t n, int j, const double* __restrict__ c) {
+  pdl_wait();
   for (int64_t e = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; e < n; e += (int64_t)gridDim.x * blockDim.x) {
     double acc = s[e];
     for (int i = 0; i < j; ++i) acc -= c[i] * V[i * n + e];
@@ -559,10 +569,14 @@ __global__ void project_kernel(double* s, const double* __restrict__ V, int64_t 
   }
 }
 
-__global__ void set_scalar_kernel(double* dst, const double* src) { *dst = *src; }
+__global__ void set_scalar_kernel(double* dst, const double* src) {
+  pdl_wait();
+  *dst = *src;
+}
 
 // restart: G = [[theta]] (a no-op while the dead flag is up, like the other kernels that change the subspace)
 __global__ void reset_gram_kernel(double* G, const double* theta, const double* dead) {
+  pdl_wait();
   if (*dead != 0.0) return;
   for (int i = threadIdx.x; i < MMAX * MMAX; i += blockDim.x) G[i] = i == 0 ? *theta : 0.0;
 }
@@ -666,7 +680,7 @@ extern "C" int hpsi_davidson(hpsi_plan_t* p, double* psi, double* eig_host, cons
 
   const int eg = (int)std::min<int64_t>((n + 255) / 256, 2048);
   auto dots = [&](const double* X, int nvec, const double* yv, double* out, int stride, double* mirror, int mstride) {
-    dot_kernel<<<dim3(NB, nvec), 256, 0, st>>>(X, n, yv, n, partial, tickets + 8, out, stride, mirror, mstride);
+    launch_dependent(dot_kernel, dim3(dim3(NB, nvec)), dim3(256), 0, st, X, n, yv, n, partial, tickets + 8, out, stride, mirror, mstride);
   };
   int rc;
   if (prm.precondition) {
@@ -684,10 +698,10 @@ extern "C" int hpsi_davidson(hpsi_plan_t* p, double* psi, double* eig_host, cons
   double* hostbuf = p->h_dav;
   for (int it = 0; it < prm.max_iter; ++it) {
     // new column of G = V^T W and its smallest Ritz pair; Ritz vector, residual, correction vector and its overlaps with V
-    dav_gram_eig_kernel<<<NB, 256, 0, st>>>(V, W + (size_t)(j - 1) * n, n, j, partial, tickets, G, theta, y, ctl, Qp, Lp,
+    launch_dependent(dav_gram_eig_kernel, dim3(NB), dim3(256), 0, st, V, W + (size_t)(j - 1) * n, n, j, partial, tickets, G, theta, y, ctl, Qp, Lp,
                                             jp == j - 1 && jp >= 1);
     jp = j;
-    dav_ritz_kernel<<<NB, 256, 0, st>>>(V, W, diag, n, j, y, theta, prm.precondition, x, wy, r, s, partial, tickets + 1, c,
+    launch_dependent(dav_ritz_kernel, dim3(NB), dim3(256), 0, st, V, W, diag, n, j, y, theta, prm.precondition, x, wy, r, s, partial, tickets + 1, c,
                                          ctl + 1, ctl);
     // theta and |r|^2 travel to the host on a side stream while the orthogonalisation below is still running.  With an
     // exchange hook (ranks in lockstep) the copy waits for the orthogonalisation: whether it sees this iteration's dead flag
@@ -702,16 +716,16 @@ extern "C" int hpsi_davidson(hpsi_plan_t* p, double* psi, double* eig_host, cons
     if (!p->exchange_fn && (rc = read_back()) != HPSI_OK) return rc;
     if (j >= prm.m_max) {                                           // restart with V = [x/|x|]
       dots(x, 1, x, ctl + 2, 1, nullptr, 0);
-      scale_kernel<<<eg, 256, 0, st>>>(V, x, W, wy, ctl + 2, n, ctl + 5);
-      reset_gram_kernel<<<1, 256, 0, st>>>(G, theta, ctl + 5);
+      launch_dependent(scale_kernel, dim3(eg), dim3(256), 0, st, V, x, W, wy, ctl + 2, n, ctl + 5);
+      launch_dependent(reset_gram_kernel, dim3(1), dim3(256), 0, st, G, theta, ctl + 5);
       j = 1;
       jp = 0;
       dots(V, 1, s, c, 1, nullptr, 0);
     }
     // classical Gram-Schmidt, twice; the second pass leaves |s|^2 (and the dead flag, stamped with the iteration)
     const double stamp = (double)(it + 1);
-    dav_project_kernel<<<NB, 256, 0, st>>>(s, V, n, j, c, partial, tickets + 2, c2, nullptr, ctl, stamp);
-    dav_project_kernel<<<NB, 256, 0, st>>>(s, V, n, j, c2, partial, tickets + 3, nullptr, ctl + 3, ctl, stamp);
+    launch_dependent(dav_project_kernel, dim3(NB), dim3(256), 0, st, s, V, n, j, c, partial, tickets + 2, c2, nullptr, ctl, stamp);
+    launch_dependent(dav_project_kernel, dim3(NB), dim3(256), 0, st, s, V, n, j, c2, partial, tickets + 3, nullptr, ctl + 3, ctl, stamp);
     if (p->exchange_fn && (rc = read_back()) != HPSI_OK) return rc;
     HPSI_CUDA(cudaEventSynchronize(p->dav_ev[1]));
     th = hostbuf[0];
@@ -734,8 +748,8 @@ extern "C" int hpsi_davidson(hpsi_plan_t* p, double* psi, double* eig_host, cons
       HPSI_CUDA(cudaMemsetAsync(ctl + 5, 0, sizeof(double), st));
       HPSI_CUDA(cudaMemcpyAsync(s, r, n * sizeof(double), cudaMemcpyDeviceToDevice, st));
       dots(V, j, s, c, 1, nullptr, 0);
-      dav_project_kernel<<<NB, 256, 0, st>>>(s, V, n, j, c, partial, tickets + 2, c2, nullptr, ctl, stamp + 0.5);
-      dav_project_kernel<<<NB, 256, 0, st>>>(s, V, n, j, c2, partial, tickets + 3, nullptr, ctl + 3, ctl, stamp + 0.5);
+      launch_dependent(dav_project_kernel, dim3(NB), dim3(256), 0, st, s, V, n, j, c, partial, tickets + 2, c2, nullptr, ctl, stamp + 0.5);
+      launch_dependent(dav_project_kernel, dim3(NB), dim3(256), 0, st, s, V, n, j, c2, partial, tickets + 3, nullptr, ctl + 3, ctl, stamp + 0.5);
     } else if (nmv >= prm.max_iter) {
       break;
     }
@@ -748,7 +762,7 @@ extern "C" int hpsi_davidson(hpsi_plan_t* p, double* psi, double* eig_host, cons
   }
   // psi = x/|x|
   dots(x, 1, x, ctl + 2, 1, nullptr, 0);
-  scale_kernel<<<eg, 256, 0, st>>>(psi, x, nullptr, nullptr, ctl + 2, n);
+  launch_dependent(scale_kernel, dim3(eg), dim3(256), 0, st, psi, x, nullptr, nullptr, ctl + 2, n, nullptr);
   HPSI_CUDA(cudaGetLastError());
   HPSI_CUDA(cudaStreamSynchronize(st));
   *eig_host = th;
@@ -766,6 +780,7 @@ namespace {
 __global__ void ritz_multi_kernel(const double* __restrict__ V, const double* __restrict__ W, int64_t n, int j,
                                   const double* __restrict__ Y, const double* __restrict__ theta, double* X, double* WY,
                                   double* Rv) {
+  pdl_wait();
   const int r = blockIdx.y;
   const double* y = Y + r * MMAX;
   const double th = theta[r];
@@ -779,6 +794,7 @@ __global__ void ritz_multi_kernel(const double* __restrict__ V, const double* __
 // s = r / (diag - theta) with |den| clamped to >= 1e-8 keeping its sign; or s = r
 __global__ void precond_kernel(const double* __restrict__ r, const double* __restrict__ diag,
                                const double* __restrict__ theta, int precondition, double* s, int64_t n) {
+  pdl_wait();
   const double th = *theta;
   for (int64_t e = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; e < n; e += (int64_t)gridDim.x * blockDim.x) {
     double v = r[e];
@@ -792,6 +808,7 @@ __global__ void precond_kernel(const double* __restrict__ r, const double* __res
 }
 
 __global__ void set_diag_kernel(double* G, const double* theta, int k) {
+  pdl_wait();
   if ((int)threadIdx.x < k) G[threadIdx.x * MMAX + threadIdx.x] = theta[threadIdx.x];
 }
 
@@ -843,7 +860,7 @@ extern "C" int hpsi_davidson_multi(hpsi_plan_t* p, double* psi, int64_t ld, int3
   HPSI_CUDA(cudaMemsetAsync(G, 0, small * sizeof(double), st));
   const int eg = (int)std::min<int64_t>((n + 255) / 256, 2048);
   auto dots = [&](const double* Xv, int nvec, const double* yv, double* out, int stride, double* mirror, int mstride) {
-    dot_kernel<<<dim3(NB, nvec), 256, 0, st>>>(Xv, n, yv, n, partial, counters, out, stride, mirror, mstride);
+    launch_dependent(dot_kernel, dim3(dim3(NB, nvec)), dim3(256), 0, st, Xv, n, yv, n, partial, counters, out, stride, mirror, mstride);
   };
   // W[j0 .. j0 + cnt) = H V[j0 .. j0 + cnt): as few passes over the operators as the plan's batch width allows
   auto apply_block = [&](int j0, int cnt) -> int {
@@ -859,10 +876,10 @@ extern "C" int hpsi_davidson_multi(hpsi_plan_t* p, double* psi, int64_t ld, int3
   auto orth_append = [&](int j, int slot) {
     for (int pass = 0; pass < 2 && j > 0; ++pass) {
       dots(V, j, s, c, 1, nullptr, 0);
-      project_kernel<<<eg, 256, 0, st>>>(s, V, n, j, c);
+      launch_dependent(project_kernel, dim3(eg), dim3(256), 0, st, s, V, n, j, c);
     }
     dots(s, 1, s, nrm + slot, 1, nullptr, 0);
-    scale_kernel<<<eg, 256, 0, st>>>(V + (size_t)j * n, s, nullptr, nullptr, nrm + slot, n);
+    launch_dependent(scale_kernel, dim3(eg), dim3(256), 0, st, V + (size_t)j * n, s, nullptr, nullptr, nrm + slot, n, nullptr);
   };
   int rc;
   if (prm.precondition) {
@@ -882,8 +899,8 @@ extern "C" int hpsi_davidson_multi(hpsi_plan_t* p, double* psi, int64_t ld, int3
     for (int col = g0; col < j; ++col)                                // new columns (and rows) of G = V^T W
       dots(V, j, W + (size_t)col * n, G + col, MMAX, G + (size_t)col * MMAX, 1);
     g0 = j;
-    small_eig_kernel<<<1, 32 * std::min(8, std::max(1, (j + 1) / 2)), 0, st>>>(G, j, theta, Y, k);
-    ritz_multi_kernel<<<dim3(eg, k), 256, 0, st>>>(V, W, n, j, Y, theta, X, WY, Rv);
+    launch_dependent(small_eig_kernel, dim3(1), dim3(32 * std::min(8, std::max(1, (j + 1) / 2))), 0, st, G, j, theta, Y, k, nullptr);
+    launch_dependent(ritz_multi_kernel, dim3(dim3(eg, k)), dim3(256), 0, st, V, W, n, j, Y, theta, X, WY, Rv);
     for (int r = 0; r < k; ++r) dots(Rv + (size_t)r * n, 1, Rv + (size_t)r * n, nrm + r, 1, nullptr, 0);
     HPSI_CUDA(cudaMemcpyAsync(host.data(), theta, k * sizeof(double), cudaMemcpyDeviceToHost, st));
     HPSI_CUDA(cudaMemcpyAsync(host.data() + MMAX, nrm, k * sizeof(double), cudaMemcpyDeviceToHost, st));
@@ -900,7 +917,7 @@ extern "C" int hpsi_davidson_multi(hpsi_plan_t* p, double* psi, int64_t ld, int3
       HPSI_CUDA(cudaMemcpyAsync(V, X, (size_t)k * n * sizeof(double), cudaMemcpyDeviceToDevice, st));
       HPSI_CUDA(cudaMemcpyAsync(W, WY, (size_t)k * n * sizeof(double), cudaMemcpyDeviceToDevice, st));
       HPSI_CUDA(cudaMemsetAsync(G, 0, MMAX * MMAX * sizeof(double), st));
-      set_diag_kernel<<<1, 32, 0, st>>>(G, theta, k);
+      launch_dependent(set_diag_kernel, dim3(1), dim3(32), 0, st, G, theta, k);
       j = g0 = k;
     }
     // correction vectors of the unconverged roots, each orthogonalised against V and the ones appended before it.  Fast
@@ -910,7 +927,7 @@ extern "C" int hpsi_davidson_multi(hpsi_plan_t* p, double* psi, int64_t ld, int3
       int added = 0;
       for (int r : todo) {
         if (nmv + added >= prm.max_iter) break;
-        precond_kernel<<<eg, 256, 0, st>>>(Rv + (size_t)r * n, diag, theta + r, prm.precondition, s, n);
+        launch_dependent(precond_kernel, dim3(eg), dim3(256), 0, st, Rv + (size_t)r * n, diag, theta + r, prm.precondition, s, n);
         orth_append(j + added, added);
         if (check_each) {
           cudaMemcpyAsync(host.data(), nrm + added, sizeof(double), cudaMemcpyDeviceToHost, st);
@@ -918,7 +935,7 @@ extern "C" int hpsi_davidson_multi(hpsi_plan_t* p, double* psi, int64_t ld, int3
           if (!(host[0] >= 1e-28)) {
             if (!prm.precondition) continue;                          // dropped: the slot is reused by the next root
             // reading A21c: the preconditioned correction lies in span(V); retry with the residual itself
-            precond_kernel<<<eg, 256, 0, st>>>(Rv + (size_t)r * n, diag, theta + r, 0, s, n);
+            launch_dependent(precond_kernel, dim3(eg), dim3(256), 0, st, Rv + (size_t)r * n, diag, theta + r, 0, s, n);
             orth_append(j + added, added);
             cudaMemcpyAsync(host.data(), nrm + added, sizeof(double), cudaMemcpyDeviceToHost, st);
             cudaStreamSynchronize(st);
@@ -965,6 +982,7 @@ namespace {
 
 // x = sum_i y_i V_i
 __global__ void combine_kernel(const double* __restrict__ V, int64_t n, int j, const double* __restrict__ y, double* x) {
+  pdl_wait();
   for (int64_t e = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; e < n; e += (int64_t)gridDim.x * blockDim.x) {
     double s = 0.0;
     for (int i = 0; i < j; ++i) s += y[i] * V[i * n + e];
@@ -973,6 +991,7 @@ __global__ void combine_kernel(const double* __restrict__ V, int64_t n, int j, c
 }
 // T[j][j] = alpha_j, T[j][j+1] = T[j+1][j] = beta_j = sqrt(|w|^2)   (T stored with leading dimension MMAX)
 __global__ void lanczos_set_kernel(double* T, int j, const double* alpha, const double* beta2) {
+  pdl_wait();
   T[j * MMAX + j] = *alpha;
   if (j + 1 < MMAX) { const double b = sqrt(*beta2); T[j * MMAX + j + 1] = b; T[(j + 1) * MMAX + j] = b; }
 }
@@ -1016,11 +1035,11 @@ extern "C" int hpsi_lanczos(hpsi_plan_t* p, double* psi, double* eig_host, const
   HPSI_CUDA(cudaMemsetAsync(T, 0, small * sizeof(double), st));
   const int eg = (int)std::min<int64_t>((n + 255) / 256, 2048);
   auto dots = [&](const double* X, int nvec, const double* yv, double* out) {
-    dot_kernel<<<dim3(NB, nvec), 256, 0, st>>>(X, n, yv, n, partial, counters, out, 1, nullptr, 0);
+    launch_dependent(dot_kernel, dim3(dim3(NB, nvec)), dim3(256), 0, st, X, n, yv, n, partial, counters, out, 1, nullptr, 0);
   };
   int rc;
   dots(psi, 1, psi, nrm);
-  scale_kernel<<<eg, 256, 0, st>>>(V, psi, nullptr, nullptr, nrm, n);
+  launch_dependent(scale_kernel, dim3(eg), dim3(256), 0, st, V, psi, nullptr, nullptr, nrm, n, nullptr);
   int j = 0, nmv = 0, converged = 0;
   double th = 0.0;
   double* host = p->h_dav;
@@ -1029,12 +1048,12 @@ extern "C" int hpsi_lanczos(hpsi_plan_t* p, double* psi, double* eig_host, const
     if ((rc = exchange(p, V + (size_t)j * n, w, n, 1, n, cuda_stream)) != HPSI_OK) return rc;
     ++nmv;
     dots(V, j + 1, w, c);                                            // c[j] = alpha_j
-    project_kernel<<<eg, 256, 0, st>>>(w, V, n, j + 1, c);           // three-term recurrence + re-orthogonalisation
+    launch_dependent(project_kernel, dim3(eg), dim3(256), 0, st, w, V, n, j + 1, c);           // three-term recurrence + re-orthogonalisation
     dots(V, j + 1, w, c2);
-    project_kernel<<<eg, 256, 0, st>>>(w, V, n, j + 1, c2);          // second Gram-Schmidt pass
+    launch_dependent(project_kernel, dim3(eg), dim3(256), 0, st, w, V, n, j + 1, c2);          // second Gram-Schmidt pass
     dots(w, 1, w, nrm + 3);                                          // beta_j^2
-    lanczos_set_kernel<<<1, 1, 0, st>>>(T, j, c + j, nrm + 3);
-    small_eig_kernel<<<1, 32 * std::max(1, (j + 2) / 2), 0, st>>>(T, j + 1, theta, y, 1);
+    launch_dependent(lanczos_set_kernel, dim3(1), dim3(1), 0, st, T, j, c + j, nrm + 3);
+    launch_dependent(small_eig_kernel, dim3(1), dim3(32 * std::max(1, (j + 2) / 2)), 0, st, T, j + 1, theta, y, 1, nullptr);
     HPSI_CUDA(cudaMemcpyAsync(host, theta, sizeof(double), cudaMemcpyDeviceToHost, st));
     HPSI_CUDA(cudaMemcpyAsync(host + 1, y + j, sizeof(double), cudaMemcpyDeviceToHost, st));
     HPSI_CUDA(cudaMemcpyAsync(host + 2, nrm + 3, sizeof(double), cudaMemcpyDeviceToHost, st));
@@ -1044,24 +1063,24 @@ extern "C" int hpsi_lanczos(hpsi_plan_t* p, double* psi, double* eig_host, const
     const double est = beta * std::fabs(host[1]);
     const bool done = est <= prm.tol || !(beta >= 1e-14) || nmv >= prm.max_iter;
     if (done || j + 1 >= prm.m_max) {
-      combine_kernel<<<eg, 256, 0, st>>>(V, n, j + 1, y, x);         // Ritz vector
+      launch_dependent(combine_kernel, dim3(eg), dim3(256), 0, st, V, n, j + 1, y, x);         // Ritz vector
       dots(x, 1, x, nrm + 2);
       if (done) break;
-      scale_kernel<<<eg, 256, 0, st>>>(V, x, nullptr, nullptr, nrm + 2, n);   // restart from the Ritz vector
+      launch_dependent(scale_kernel, dim3(eg), dim3(256), 0, st, V, x, nullptr, nullptr, nrm + 2, n, nullptr);   // restart from the Ritz vector
       HPSI_CUDA(cudaMemsetAsync(T, 0, MMAX * MMAX * sizeof(double), st));
       j = 0;
       continue;
     }
-    scale_kernel<<<eg, 256, 0, st>>>(V + (size_t)(j + 1) * n, w, nullptr, nullptr, nrm + 3, n);
+    launch_dependent(scale_kernel, dim3(eg), dim3(256), 0, st, V + (size_t)(j + 1) * n, w, nullptr, nullptr, nrm + 3, n, nullptr);
     ++j;
   }
   // psi = x/|x| ; true residual |H psi - theta psi|
-  scale_kernel<<<eg, 256, 0, st>>>(psi, x, nullptr, nullptr, nrm + 2, n);
+  launch_dependent(scale_kernel, dim3(eg), dim3(256), 0, st, psi, x, nullptr, nullptr, nrm + 2, n, nullptr);
   if ((rc = hpsi_apply(p, psi, w, cuda_stream)) != HPSI_OK) return rc;
   if ((rc = exchange(p, psi, w, n, 1, n, cuda_stream)) != HPSI_OK) return rc;
   ++nmv;
-  set_scalar_kernel<<<1, 1, 0, st>>>(c, theta);
-  project_kernel<<<eg, 256, 0, st>>>(w, psi, n, 1, c);
+  launch_dependent(set_scalar_kernel, dim3(1), dim3(1), 0, st, c, theta);
+  launch_dependent(project_kernel, dim3(eg), dim3(256), 0, st, w, psi, n, 1, c);
   dots(w, 1, w, nrm + 1);
   HPSI_CUDA(cudaMemcpyAsync(host, nrm + 1, sizeof(double), cudaMemcpyDeviceToHost, st));
   HPSI_CUDA(cudaGetLastError());

@@ -100,6 +100,7 @@ __device__ __forceinline__ void idle_consume(const SmemLayout& sm, int nstages, 
 
 template <bool TMA, bool ROT>
 __global__ void __maxnreg__(136) p1_kernel(DevSchedule d) {
+  pdl_wait();
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const P1Unit u = d.p1[blockIdx.x];
   if (!ROT && u.vec >= d.nvec_active) return;            // batched plan applied to fewer vectors than it was laid out for
@@ -207,6 +208,7 @@ __device__ __forceinline__ void p2_consume(const DevSchedule& d, const P2Unit& u
 
 template <bool TMA>
 __global__ void __maxnreg__(136) p2_kernel(DevSchedule d) {
+  pdl_wait();
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const P2Unit u = d.p2[blockIdx.x];
   if (u.vec >= d.nvec_active) return;                    // batched plan applied to fewer vectors than it was laid out for
@@ -292,6 +294,7 @@ __global__ void __maxnreg__(136) p2_kernel(DevSchedule d) {
 // eigensolver drivers hand over a new basis vector unnormalised: one launch fewer per iteration).
 __global__ void prep_kernel(DevSchedule d, const double* __restrict__ psi, const double* __restrict__ nrm2,
                             double* __restrict__ normalized) {
+  pdl_wait();
   const ElemCta c = d.elem[blockIdx.x];
   const PsiBlk B = d.blocks[c.blk];
   const int e = c.e0 + threadIdx.x;
@@ -312,6 +315,7 @@ __global__ void prep_kernel(DevSchedule d, const double* __restrict__ psi, const
 // reduce_plain_kernel below; the launcher picks by size.  Partials: split-major, vector-minor.
 constexpr int RED_LANES = 8;
 __global__ void reduce_kernel(DevSchedule d, double* __restrict__ out, int accumulate) {
+  pdl_wait();
   const ElemCta c = d.elem[blockIdx.x >> 3];                   // eight CTAs per granule: 32 elements each (lanes x 8 = 256 threads)
   const PsiBlk B = d.blocks[c.blk];
   const int n = B.rows * B.cols;
@@ -348,6 +352,7 @@ __global__ void reduce_kernel(DevSchedule d, double* __restrict__ out, int accum
 
 // the plain form: one thread per element, rows fully coalesced (large vectors; bandwidth-bound)
 __global__ void reduce_plain_kernel(DevSchedule d, double* __restrict__ out, int accumulate) {
+  pdl_wait();
   const ElemCta c = d.elem[blockIdx.x];
   const PsiBlk B = d.blocks[c.blk];
   const int e = c.e0 + threadIdx.x;
@@ -371,6 +376,7 @@ __global__ void reduce_plain_kernel(DevSchedule d, double* __restrict__ out, int
 
 // diag(H): diag[l][x,y] = sum over sector-diagonal tasks of c_t A[x,x] B[y,y]   (reading A21)
 __global__ void diag_kernel(DevSchedule d, double* __restrict__ diag) {
+  pdl_wait();
   const ElemCta c = d.elem[blockIdx.x];
   const PsiBlk B = d.blocks[c.blk];
   const int e = c.e0 + threadIdx.x;
@@ -387,6 +393,7 @@ __global__ void diag_kernel(DevSchedule d, double* __restrict__ diag) {
 // out[e] = parts[0][e] + parts[1][e] + ... in that order (term-sharded apply: the ranks' partial H psi, gathered, are added
 // in rank order - bitwise the same on every rank and every run, whatever the transport did)
 __global__ void sum_shards_kernel(const double* __restrict__ parts, int n_parts, int64_t n, double* __restrict__ out) {
+  pdl_wait();
   for (int64_t e = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; e < n; e += (int64_t)gridDim.x * blockDim.x) {
     double s = parts[e];
     for (int r = 1; r < n_parts; ++r) s += parts[(int64_t)r * n + e];
@@ -413,33 +420,33 @@ cudaError_t kernels_init() {
 }
 
 void launch_prep(const DevSchedule& d, const double* psi, const double* nrm2, double* normalized, cudaStream_t st) {
-  if (d.n_elem > 0) prep_kernel<<<dim3(d.n_elem, d.nvec_active), 256, 0, st>>>(d, psi, nrm2, normalized);
+  if (d.n_elem > 0) launch_dependent(prep_kernel, dim3(dim3(d.n_elem, d.nvec_active)), dim3(256), 0, st, d, psi, nrm2, normalized);
 }
 void launch_p1(const DevSchedule& d, bool tma, cudaStream_t st) {
   if (d.n_p1 == 0) return;
   if (d.paired) { launch_p1_paired(d, tma, st); return; }
-  if (tma) p1_kernel<true, false><<<d.n_p1, NTHREADS, SMEM_BYTES, st>>>(d);
-  else p1_kernel<false, false><<<d.n_p1, NTHREADS, SMEM_BYTES, st>>>(d);
+  if (tma) launch_dependent(p1_kernel<true, false>, dim3(d.n_p1), dim3(NTHREADS), SMEM_BYTES, st, d);
+  else launch_dependent(p1_kernel<false, false>, dim3(d.n_p1), dim3(NTHREADS), SMEM_BYTES, st, d);
 }
 void launch_p1_rot(const DevSchedule& d, bool tma, cudaStream_t st) {
   if (d.n_p1 == 0) return;
-  if (tma) p1_kernel<true, true><<<d.n_p1, NTHREADS, SMEM_BYTES, st>>>(d);
-  else p1_kernel<false, true><<<d.n_p1, NTHREADS, SMEM_BYTES, st>>>(d);
+  if (tma) launch_dependent(p1_kernel<true, true>, dim3(d.n_p1), dim3(NTHREADS), SMEM_BYTES, st, d);
+  else launch_dependent(p1_kernel<false, true>, dim3(d.n_p1), dim3(NTHREADS), SMEM_BYTES, st, d);
 }
 void launch_p2(const DevSchedule& d, bool tma, cudaStream_t st) {
   if (d.n_p2 == 0) return;
   if (d.paired) { launch_p2_paired(d, tma, st); return; }
-  if (tma) p2_kernel<true><<<d.n_p2, NTHREADS, SMEM_BYTES, st>>>(d);
-  else p2_kernel<false><<<d.n_p2, NTHREADS, SMEM_BYTES, st>>>(d);
+  if (tma) launch_dependent(p2_kernel<true>, dim3(d.n_p2), dim3(NTHREADS), SMEM_BYTES, st, d);
+  else launch_dependent(p2_kernel<false>, dim3(d.n_p2), dim3(NTHREADS), SMEM_BYTES, st, d);
 }
 void launch_reduce(const DevSchedule& d, double* out, bool accumulate, cudaStream_t st) {
   if (d.n_elem == 0) return;
   const bool small_vec = (int64_t)d.n_elem * 256 <= 500000;     // latency-bound sizes (D <~ 1500)
-  if (small_vec) reduce_kernel<<<dim3(d.n_elem * 8, d.nvec_active), 256, 0, st>>>(d, out, accumulate ? 1 : 0);
-  else reduce_plain_kernel<<<dim3(d.n_elem, d.nvec_active), 256, 0, st>>>(d, out, accumulate ? 1 : 0);
+  if (small_vec) launch_dependent(reduce_kernel, dim3(dim3(d.n_elem * 8, d.nvec_active)), dim3(256), 0, st, d, out, accumulate ? 1 : 0);
+  else launch_dependent(reduce_plain_kernel, dim3(dim3(d.n_elem, d.nvec_active)), dim3(256), 0, st, d, out, accumulate ? 1 : 0);
 }
 void launch_diag(const DevSchedule& d, double* diag, cudaStream_t st) {
-  if (d.n_elem > 0) diag_kernel<<<d.n_elem, 256, 0, st>>>(d, diag);
+  if (d.n_elem > 0) launch_dependent(diag_kernel, dim3(d.n_elem), dim3(256), 0, st, d, diag);
 }
 
 }  // namespace hpsi

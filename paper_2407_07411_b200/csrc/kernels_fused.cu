@@ -40,6 +40,7 @@ __device__ __forceinline__ void mma_stage_rt(const double* px, const double* py,
 
 template <bool TMA>
 __global__ void __launch_bounds__(NTHREADS, 2) pf_kernel(DevSchedule d) {
+  pdl_wait();
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const P2Unit u = d.pf[blockIdx.x];
   const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
@@ -193,8 +194,8 @@ cudaError_t kernels_fused_init() {
 
 void launch_pf(const DevSchedule& d, bool tma, cudaStream_t st) {
   if (d.n_pf == 0) return;
-  if (tma) pf_kernel<true><<<d.n_pf, NTHREADS, SMEM_FUSED, st>>>(d);
-  else pf_kernel<false><<<d.n_pf, NTHREADS, SMEM_FUSED, st>>>(d);
+  if (tma) launch_dependent(pf_kernel<true>, dim3(d.n_pf), dim3(NTHREADS), SMEM_FUSED, st, d);
+  else launch_dependent(pf_kernel<false>, dim3(d.n_pf), dim3(NTHREADS), SMEM_FUSED, st, d);
 }
 
 }  // namespace hpsi

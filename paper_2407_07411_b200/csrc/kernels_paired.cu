@@ -193,6 +193,7 @@ __device__ __forceinline__ void p1p_consume(const DevSchedule& d, const P1Unit& 
 
 template <bool TMA>
 __global__ void __maxnreg__(136) p1p_kernel(DevSchedule d) {
+  pdl_wait();
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const P1Unit u = d.p1[blockIdx.x];
   const Group g = d.groups[u.group];
@@ -258,6 +259,7 @@ __device__ __forceinline__ void p2p_consume(const DevSchedule& d, const P2Unit& 
 
 template <bool TMA>
 __global__ void __maxnreg__(136) p2p_kernel(DevSchedule d) {
+  pdl_wait();
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const P2Unit u = d.p2[blockIdx.x];
   const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
@@ -322,12 +324,12 @@ cudaError_t kernels_paired_init() {
   return cudaSuccess;
 }
 void launch_p1_paired(const DevSchedule& d, bool tma, cudaStream_t st) {
-  if (tma) p1p_kernel<true><<<d.n_p1, NTHREADS, SMEM_BYTES, st>>>(d);
-  else p1p_kernel<false><<<d.n_p1, NTHREADS, SMEM_BYTES, st>>>(d);
+  if (tma) launch_dependent(p1p_kernel<true>, dim3(d.n_p1), dim3(NTHREADS), SMEM_BYTES, st, d);
+  else launch_dependent(p1p_kernel<false>, dim3(d.n_p1), dim3(NTHREADS), SMEM_BYTES, st, d);
 }
 void launch_p2_paired(const DevSchedule& d, bool tma, cudaStream_t st) {
-  if (tma) p2p_kernel<true><<<d.n_p2, NTHREADS, SMEM_BYTES, st>>>(d);
-  else p2p_kernel<false><<<d.n_p2, NTHREADS, SMEM_BYTES, st>>>(d);
+  if (tma) launch_dependent(p2p_kernel<true>, dim3(d.n_p2), dim3(NTHREADS), SMEM_BYTES, st, d);
+  else launch_dependent(p2p_kernel<false>, dim3(d.n_p2), dim3(NTHREADS), SMEM_BYTES, st, d);
 }
 
 }  // namespace hpsi

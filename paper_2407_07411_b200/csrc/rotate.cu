@@ -23,6 +23,7 @@ struct IsoCopy {              // O_l^T: dense chi x d at src_off of the caller's
 };
 
 __global__ void rot_prep_kernel(const IsoCopy* iso, const double* __restrict__ ot, double* __restrict__ ws) {
+  pdl_wait();
   const IsoCopy c = iso[blockIdx.y];
   const int n = c.rows * c.cols;
   for (int e = blockIdx.x * blockDim.x + threadIdx.x; e < n; e += gridDim.x * blockDim.x) {
@@ -338,7 +339,7 @@ static int rotate_launch(hpsi_rotate* r, const double* ot_dev, double* out_dev, 
   if (ev) HPSI_CUDA(cudaEventRecord(ev[0], st));
   if (!r->iso.empty()) {
     int gx = std::min(64, std::max(1, (r->max_iso_elems + 255) / 256));
-    rot_prep_kernel<<<dim3(gx, (unsigned)r->iso.size()), 256, 0, st>>>(r->d_iso, ot_dev, p.d_ws);
+    launch_dependent(rot_prep_kernel, dim3(dim3(gx, (unsigned)r->iso.size())), dim3(256), 0, st, r->d_iso, ot_dev, p.d_ws);
   }
   if (ev) HPSI_CUDA(cudaEventRecord(ev[1], st));
   DevSchedule d1 = p.dev;

@@ -47,6 +47,7 @@ struct SvdBlk {
 
 // working matrix <- [psi block | identity]; floor2 of the block from its Frobenius norm (one CTA per block row range)
 __global__ void svd_init_kernel(SvdBlk* blk, const double* __restrict__ psi, double* __restrict__ w) {
+  pdl_wait();
   const SvdBlk B = blk[blockIdx.y];
   for (int i = blockIdx.x; i < B.nv; i += gridDim.x) {
     double* row = w + B.w_off + (int64_t)i * B.L;
@@ -60,6 +61,7 @@ __global__ void svd_init_kernel(SvdBlk* blk, const double* __restrict__ psi, dou
 }
 // squared Frobenius norm of each block in a fixed order (one CTA per block, tree reduction)
 __global__ void svd_norm_kernel(SvdBlk* blk, const double* __restrict__ psi) {
+  pdl_wait();
   __shared__ double red[256];
   SvdBlk& B = blk[blockIdx.x];
   const int64_t n = (int64_t)B.rows * B.cols;
@@ -110,6 +112,7 @@ struct SvdSmem {
 // global memory / L2.
 __global__ void __launch_bounds__(SV_THREADS, 2) svd_round_kernel(const SvdBlk* __restrict__ blk, const int32_t* __restrict__ cta_blk,
                                                                int round, double* __restrict__ w, int* __restrict__ flag) {
+  pdl_wait();
   __shared__ SvdSmem sm;
   const SvdBlk B = blk[cta_blk[blockIdx.x]];
   const int k = blockIdx.x - B.cta0;
@@ -252,6 +255,7 @@ __global__ void __launch_bounds__(SV_THREADS, 2) svd_round_kernel(const SvdBlk* 
 
 // singular value of every row = norm of its psi part (one warp per row)
 __global__ void svd_sigma_kernel(const SvdBlk* __restrict__ blk, const double* __restrict__ w, double* __restrict__ sigma) {
+  pdl_wait();
   const SvdBlk B = blk[blockIdx.y];
   const int lane = threadIdx.x & 31, wpb = blockDim.x >> 5;
   for (int i = blockIdx.x * wpb + (threadIdx.x >> 5); i < B.nv; i += gridDim.x * wpb) {
@@ -265,6 +269,7 @@ __global__ void svd_sigma_kernel(const SvdBlk* __restrict__ blk, const double* _
 
 struct IsoRow { int64_t src, dst; double scale; int32_t len, pad; };   // kept vector (R part, or row / sigma) -> one row of O_l^T
 __global__ void svd_gather_kernel(const IsoRow* __restrict__ rows, int n, const double* __restrict__ w, double* __restrict__ ot) {
+  pdl_wait();
   for (int i = blockIdx.x; i < n; i += gridDim.x) {
     const IsoRow r = rows[i];
     for (int j = threadIdx.x; j < r.len; j += blockDim.x) ot[r.dst + j] = w[r.src + j] * r.scale;
@@ -384,21 +389,21 @@ static int truncate_impl(hpsi_plan_t* p, const double* psi_dev, int32_t side, in
   HPSI_CUDA(cudaMemcpyAsync(d_tab, tab.data(), tab.size() * sizeof(SvdBlk), cudaMemcpyHostToDevice, st));
   HPSI_CUDA(cudaMemcpyAsync(d_cta, cta_blk.data(), cta_blk.size() * 4, cudaMemcpyHostToDevice, st));
 
-  svd_norm_kernel<<<nB, 256, 0, st>>>(d_tab, psi_dev);
-  svd_init_kernel<<<dim3(64, nB), 128, 0, st>>>(d_tab, psi_dev, d_w);
+  launch_dependent(svd_norm_kernel, dim3(nB), dim3(256), 0, st, d_tab, psi_dev);
+  launch_dependent(svd_init_kernel, dim3(dim3(64, nB)), dim3(128), 0, st, d_tab, psi_dev, d_w);
   constexpr int MAX_SWEEPS = 60;
   int sweeps = 0, flag = 1;
   for (; sweeps < MAX_SWEEPS && flag; ++sweeps) {
     HPSI_CUDA(cudaMemsetAsync(d_flag, 0, sizeof(int), st));
     for (int r = 0; r < rounds; ++r)
-      svd_round_kernel<<<n_cta, SV_THREADS, 0, st>>>(d_tab, d_cta, sweeps * rounds + r, d_w, d_flag);
+      launch_dependent(svd_round_kernel, dim3(n_cta), dim3(SV_THREADS), 0, st, d_tab, d_cta, sweeps * rounds + r, d_w, d_flag);
     HPSI_CUDA(cudaMemcpyAsync(&flag, d_flag, sizeof(int), cudaMemcpyDeviceToHost, st));
     HPSI_CUDA(cudaStreamSynchronize(st));
   }
   if (flag) { set_error("hpsi_truncate: Jacobi SVD did not converge"); return HPSI_ESTATE; }
   p->svd_sweeps = sweeps;
   p->svd_launches = sweeps * rounds + 4;
-  svd_sigma_kernel<<<dim3(16, nB), 256, 0, st>>>(d_tab, d_w, d_sigma);
+  launch_dependent(svd_sigma_kernel, dim3(dim3(16, nB)), dim3(256), 0, st, d_tab, d_w, d_sigma);
   std::vector<double> sig(n_rows);
   HPSI_CUDA(cudaMemcpyAsync(sig.data(), d_sigma, (size_t)n_rows * 8, cudaMemcpyDeviceToHost, st));
   HPSI_CUDA(cudaStreamSynchronize(st));
@@ -465,7 +470,7 @@ static int truncate_impl(hpsi_plan_t* p, const double* psi_dev, int32_t side, in
   }
   if (!rows.empty()) {
     HPSI_CUDA(cudaMemcpyAsync(d_rows, rows.data(), rows.size() * sizeof(IsoRow), cudaMemcpyHostToDevice, st));
-    svd_gather_kernel<<<std::min<int>((int)rows.size(), 1024), 128, 0, st>>>(d_rows, (int)rows.size(), d_w, ot_dev);
+    launch_dependent(svd_gather_kernel, dim3(std::min<int>((int)rows.size(), 1024)), dim3(128), 0, st, d_rows, (int)rows.size(), d_w, ot_dev);
     HPSI_CUDA(cudaStreamSynchronize(st));              // `rows` must outlive the copy
   }
   HPSI_CUDA(cudaGetLastError());
