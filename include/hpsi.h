@@ -159,7 +159,11 @@ int hpsi_set_task_coefficients(hpsi_plan_t* plan, const double* coef_host, int64
 /* Steps 5-7: out = H psi (overwrite).  psi_dev / out_dev: DEVICE, psi_length doubles each, must not alias.
  * cuda_stream: a cudaStream_t cast to void* (NULL = default stream).  Enqueue only: no host sync, no
  * allocation, CUDA-graph capturable.  A plan owns one workspace: do not run it on two streams at once.
- * Repeated applies on the same inputs are bitwise identical (no atomics on data). */
+ * Repeated applies on the same inputs are bitwise identical (no atomics on data).
+ * Launch form (all entry points): every kernel is enqueued as a programmatic dependent of the operation before it in
+ * the stream and waits on the device (griddepcontrol.wait) before its first memory access, which hides its launch latency
+ * (~2 us per kernel boundary).  Stream order and visibility are those of plain launches: the caller's own work before
+ * and after a call needs no change. */
 int hpsi_apply(hpsi_plan_t* plan, const double* psi_dev, double* out_dev, void* cuda_stream);
 
 /* Batched apply: out_v = H psi_v for v = 0 .. n_vectors-1 in one pass over the operators (plan built with
