@@ -97,34 +97,12 @@ struct EigSmem {
   double d[MMAX], e[MMAX], beta[MMAX], v[MMAX], w[MMAX], l[MMAX], rq[MMAX], z[MMAX];
   int ok;
 };
-// Warm start (Davidson): G grows by one row and column per iteration, so with the eigenvectors Qp and eigenvalues Lp of
-// the previous (j-1) x (j-1) matrix the new one is, in the basis [Qp, e_j], diagonal plus one row and column ("arrowhead":
-// diag(Lp), z = Qp^T g, gamma) - two Jacobi sweeps instead of six to eight.  `warm` = Qp / Lp describe G[0..j-1, 0..j-1).
-// The eigen-decomposition found is left in Qp / Lp for the next call.
-__device__ void small_eig_block(const double* __restrict__ G, int j, double* theta, double* y, EigSmem& sm, int k = 1,
-                                double* Qp = nullptr, double* Lp = nullptr, bool warm = false) {
+__device__ void small_eig_block(const double* __restrict__ G, int j, double* theta, double* y, EigSmem& sm, int k = 1) {
   const int t = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
   const int m = (j + 1) & ~1;                            // players of the round-robin (a dummy one if j is odd)
   const int np = m > 1 ? m / 2 : 1;                      // pairs per round
-  if (warm && j >= 2) {
-    const int jp = j - 1;
-    for (int c = wid; c <= jp; c += nw)
-      if (t <= jp) {
-        double a = 0.0, qv = (t == c) ? 1.0 : 0.0;
-        if (t < jp && c < jp) { a = (t == c) ? Lp[t] : 0.0; qv = Qp[t * MMAX + c]; }
-        else if (t == jp && c == jp) a = G[jp * MMAX + jp];
-        else {                                           // z_u = sum_i Qp[i][u] g_i with g = new column of G, u = the index < jp
-          const int u = t < jp ? t : c;
-          for (int i = 0; i < jp; ++i) a += Qp[i * MMAX + u] * 0.5 * (G[i * MMAX + jp] + G[jp * MMAX + i]);
-          qv = 0.0;
-        }
-        sm.A[t][c] = a;
-        sm.Q[t][c] = qv;
-      }
-  } else {
-    for (int c = wid; c < j; c += nw)
-      if (t < j) { sm.A[t][c] = 0.5 * (G[t * MMAX + c] + G[c * MMAX + t]); sm.Q[t][c] = (t == c) ? 1.0 : 0.0; }
-  }
+  for (int c = wid; c < j; c += nw)
+    if (t < j) { sm.A[t][c] = 0.5 * (G[t * MMAX + c] + G[c * MMAX + t]); sm.Q[t][c] = (t == c) ? 1.0 : 0.0; }
   __syncthreads();
   double prev_off = 0.0;
   for (int sweep = 0; sweep < 30 && j > 1; ++sweep) {
@@ -193,11 +171,6 @@ __device__ void small_eig_block(const double* __restrict__ G, int j, double* the
     }
   }
   __syncthreads();
-  if (Qp) {                                              // keep the decomposition for the next (warm) call
-    for (int c = wid; c < j; c += nw)
-      if (t < j) Qp[t * MMAX + c] = sm.Q[t][c];
-    if (wid == 0 && t < j) Lp[t] = sm.A[t][t];
-  }
   if (wid == 0) {                                        // the k lowest Ritz pairs, ascending: theta[r], y[r * MMAX + t]
     unsigned taken = 0u;
     for (int r = 0; r < k && r < j; ++r) {
@@ -456,8 +429,7 @@ __device__ __forceinline__ void dav_slice(int64_t n, int64_t& lo, int64_t& hi) {
 // G[:, j-1] = G[j-1, :] = V^T W_{j-1};  then (last block) the smallest Ritz pair of G -> theta, y
 __global__ void __launch_bounds__(256) dav_gram_eig_kernel(const double* __restrict__ V, const double* __restrict__ wl, int64_t n,
                                                            int j, double* partial, unsigned int* ticket, double* G,
-                                                           double* theta, double* y, const double* ctl, double* Qp,
-                                                           double* Lp, int warm) {
+                                                           double* theta, double* y, const double* ctl) {
   pdl_wait();
   __shared__ EigSmem sm;
   if (ctl[5] != 0.0) return;
@@ -478,7 +450,6 @@ __global__ void __launch_bounds__(256) dav_gram_eig_kernel(const double* __restr
   }
   if (threadIdx.x == 0) *ticket = 0;
   __syncthreads();
-  (void)Qp; (void)Lp; (void)warm;                         // the Jacobi solver's warm start: only its fallback role is left
   small_eig_lowest_or_jacobi(G, j, theta, y, sm, 1);
 }
 
@@ -645,8 +616,8 @@ extern "C" int hpsi_davidson(hpsi_plan_t* p, double* psi, double* eig_host, cons
   if (n == 0) { set_error("empty target sector"); return HPSI_EINVAL; }
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
 
-  // buffers: V[m][n] W[m][n] diag x wy r s | G[MMAX*MMAX] y[MMAX] c[MMAX] c2[MMAX] theta ctl[7] partial[(MMAX+1)*NB] tickets Qp Lp
-  const size_t small = MMAX * MMAX + 3 * MMAX + 8 + (MMAX + 1) * NB + MMAX + MMAX * MMAX + MMAX;
+  // buffers: V[m][n] W[m][n] diag x wy r s | G[MMAX*MMAX] y[MMAX] c[MMAX] c2[MMAX] theta ctl[7] partial[(MMAX+1)*NB] tickets
+  const size_t small = MMAX * MMAX + 3 * MMAX + 8 + (MMAX + 1) * NB + MMAX;
   const size_t need = (size_t)(2 * prm.m_max + 5) * n + small;
   if (p->dav_doubles < need) {
     HPSI_CUDA(cudaStreamSynchronize(st));
@@ -672,9 +643,6 @@ extern "C" int hpsi_davidson(hpsi_plan_t* p, double* psi, double* eig_host, cons
   double* G = s + n;
   double *y = G + MMAX * MMAX, *c = y + MMAX, *c2 = c + MMAX, *theta = c2 + MMAX, *ctl = theta + 1, *partial = ctl + 7;
   unsigned int* tickets = reinterpret_cast<unsigned int*>(partial + (MMAX + 1) * NB);
-  double* Qp = partial + (MMAX + 1) * NB + MMAX;         // eigenvectors / eigenvalues of the previous subspace matrix
-  double* Lp = Qp + MMAX * MMAX;
-  int jp = 0;                                            // dimension Qp / Lp describe (0: none - cold start)
   // ctl: [0] |psi|^2  [1] |r|^2  [2] |x|^2  [3] |s|^2  [5] dead flag   (theta, ctl[0..5] are read back together)
   HPSI_CUDA(cudaMemsetAsync(G, 0, small * sizeof(double), st));
 
@@ -698,9 +666,7 @@ extern "C" int hpsi_davidson(hpsi_plan_t* p, double* psi, double* eig_host, cons
   double* hostbuf = p->h_dav;
   for (int it = 0; it < prm.max_iter; ++it) {
     // new column of G = V^T W and its smallest Ritz pair; Ritz vector, residual, correction vector and its overlaps with V
-    launch_dependent(dav_gram_eig_kernel, dim3(NB), dim3(256), 0, st, V, W + (size_t)(j - 1) * n, n, j, partial, tickets, G, theta, y, ctl, Qp, Lp,
-                                            jp == j - 1 && jp >= 1);
-    jp = j;
+    launch_dependent(dav_gram_eig_kernel, dim3(NB), dim3(256), 0, st, V, W + (size_t)(j - 1) * n, n, j, partial, tickets, G, theta, y, ctl);
     launch_dependent(dav_ritz_kernel, dim3(NB), dim3(256), 0, st, V, W, diag, n, j, y, theta, prm.precondition, x, wy, r, s, partial, tickets + 1, c,
                                          ctl + 1, ctl);
     // theta and |r|^2 travel to the host on a side stream while the orthogonalisation below is still running.  With an
@@ -719,7 +685,6 @@ extern "C" int hpsi_davidson(hpsi_plan_t* p, double* psi, double* eig_host, cons
       launch_dependent(scale_kernel, dim3(eg), dim3(256), 0, st, V, x, W, wy, ctl + 2, n, ctl + 5);
       launch_dependent(reset_gram_kernel, dim3(1), dim3(256), 0, st, G, theta, ctl + 5);
       j = 1;
-      jp = 0;
       dots(V, 1, s, c, 1, nullptr, 0);
     }
     // classical Gram-Schmidt, twice; the second pass leaves |s|^2 (and the dead flag, stamped with the iteration)
@@ -744,7 +709,6 @@ extern "C" int hpsi_davidson(hpsi_plan_t* p, double* psi, double* eig_host, cons
       // Preconditioned it means r/(diag - theta) lies in span(V) (H diagonal: it is the Ritz vector itself): reading A21c
       // retries with the residual itself.
       if (!prm.precondition || dead != std::floor(dead) || nmv >= prm.max_iter) break;
-      jp = 0;
       HPSI_CUDA(cudaMemsetAsync(ctl + 5, 0, sizeof(double), st));
       HPSI_CUDA(cudaMemcpyAsync(s, r, n * sizeof(double), cudaMemcpyDeviceToDevice, st));
       dots(V, j, s, c, 1, nullptr, 0);
