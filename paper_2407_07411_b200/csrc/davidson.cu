@@ -255,7 +255,7 @@ __device__ bool lowest_eig_warp(const double* __restrict__ G, int j, double* the
   // The counts run on the determinant form of the Sturm sequence, p_i = (d_i - x) p_{i-1} - e_{i-1}^2 p_{i-2} (sign
   // changes = negative pivots q_i = p_i / p_{i-1}): one FMA per step on the critical path instead of a division (~130 clk),
   // which made the counts 2/3 of this routine.  T is scaled by a power of two (exact) to norm [1, 2), so p cannot
-  // overflow in 32 steps; it is re-scaled when it shrinks.  A vanishing p_i is replaced as the pivot form replaces q_i.
+  // overflow in 32 steps; it is re-scaled when it shrinks.
   const int ex = ilogb(tn);
   const double pm = scalbn(pivmin, -ex);
   if (in) {
@@ -268,28 +268,31 @@ __device__ bool lowest_eig_warp(const double* __restrict__ G, int j, double* the
   hi = scalbn(hi, -ex);
   for (int round = 0; round < 40; ++round) {
     const double x = lo + (hi - lo) * ((t + 1) * (1.0 / 33.0));
+    // neg = "p_i is negative", an exact zero taking the sign opposite to p_{i-1} (the pivot form would make q_i = -pivmin);
+    // the recurrence itself has no division, so a vanishing p_i needs no replacement: the only arithmetic on the critical
+    // path is one FMA per step.  The magnitude is checked every fourth step (p changes by 2^-106 .. 2^3 per step).
     double pp = 1.0, p = sm.v[0] - x;
-    if (fabs(p) < pm) p = -pm;
-    int cnt = p < 0.0;
+    bool neg = p <= 0.0;
+    int cnt = neg;
     for (int i = 1; i < j; ++i) {
-      double pn = fma(sm.v[i] - x, p, -sm.w[i - 1] * pp);
-      if (fabs(pn) < pm * fabs(p)) pn = -pm * p;
-      cnt += (pn < 0.0) != (p < 0.0);
+      const double pn = fma(sm.v[i] - x, p, -sm.w[i - 1] * pp);
+      const bool nneg = pn < 0.0 || (pn == 0.0 && !neg);
+      cnt += nneg != neg;
+      neg = nneg;
       pp = p;
       p = pn;
-      const double mag = fmax(fabs(p), fabs(pp));
-      if (mag < 1e-100) { p *= 0x1p400; pp *= 0x1p400; }
-      else if (mag > 1e100) { p *= 0x1p-400; pp *= 0x1p-400; }
+      if ((i & 3) == 0) {
+        const double mag = fmax(fabs(p), fabs(pp));
+        if (mag < 1e-100) { p *= 0x1p400; pp *= 0x1p400; }
+        else if (mag > 1e100) { p *= 0x1p-400; pp *= 0x1p-400; }
+      }
     }
+    // the first lane whose shift has an eigenvalue below it closes the bracket from above, the lane before it from below;
+    // every lane recomputes those two shifts from the lane number (same expression, same bits: no shuffle needed)
     const unsigned below = __ballot_sync(FULL, cnt >= 1);
-    double nlo, nhi;
-    if (below == 0u) { nlo = __shfl_sync(FULL, x, 31); nhi = hi; }
-    else {
-      const int l = __ffs(below) - 1;
-      nhi = __shfl_sync(FULL, x, l);
-      const double xm = __shfl_sync(FULL, x, l > 0 ? l - 1 : 0);
-      nlo = l > 0 ? xm : lo;
-    }
+    const int l = below ? __ffs(below) - 1 : 32;
+    const double nhi = l < 32 ? lo + (hi - lo) * ((l + 1) * (1.0 / 33.0)) : hi;
+    const double nlo = l > 0 ? lo + (hi - lo) * (l * (1.0 / 33.0)) : lo;
     const bool conv = (nhi - nlo) <= 2.0 * EPS * fmax(fabs(nlo), fabs(nhi)) + 2.0 * pm || !(nlo > lo || nhi < hi);
     lo = nlo; hi = nhi;
     if (conv) break;
