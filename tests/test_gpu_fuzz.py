@@ -3,8 +3,8 @@ from 1 to 200 mixed in one problem, sparse and dense block patterns, odd leading
 contraction orders; every case runs hpsi_apply, hpsi_rotate_apply (random kept dims, some zero) and hpsi_truncate
 (either side, by count or by discarded weight); odd seeds send the narrow groups through the fused kernel; every seed
 also re-stores a random half of the operator blocks transposed (A and B flags independent) and runs a batched plan of
-2 .. 4 vectors.  (7000 seeds of this generator were run on a B200 in each round, and 8440 seeds of both tests of this
-file at the round's last kernel change, with no failure; the committed tests keep 60 + 24.)"""
+2 .. 4 vectors.  (7000 seeds of this generator were run on a B200 in each round, and 8440 + 13424 seeds of both tests of this
+file after the round's last kernel changes, with no failure; the committed tests keep 60 + 24.)"""
 import numpy as np
 import pytest
 
