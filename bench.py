@@ -137,17 +137,35 @@ def git_head():
         return None
 
 
+KERNEL_SOURCES = ("kernels.cu", "kernels.cuh", "kernels_common.cuh", "kernels_paired.cu", "kernels_fused.cu", "plan.h")
+
+
+def kernel_sources_digest():
+    """sha1 over the sources of the GEMM kernels: what tells whether a committed ncu capture still describes the kernels
+    being timed (there is no .git on the GPU box, so the commit id alone cannot)."""
+    import hashlib
+    h = hashlib.sha1()
+    for name in KERNEL_SOURCES:
+        with open(os.path.join(ROOT, "paper_2407_07411_b200", "csrc", name), "rb") as fh:
+            h.update(fh.read())
+    return h.hexdigest()[:16]
+
+
 def ncu_traffic(key, kernel):
-    """DRAM bytes per launch of ``kernel`` from the committed ncu --set full capture (profiles/ncu_traffic.json.txt),
-    with the commit the capture was taken at, so that a reader can tell whether it describes the kernels being timed."""
+    """DRAM bytes per launch of ``kernel`` from the committed ncu --set full capture (profiles/ncu_traffic.json.txt).
+    The file records the digest of the kernel sources the capture was taken with; if today's sources differ the figure is
+    withheld (None) - a stale capture says nothing about the kernels being timed."""
     try:
         with open(os.path.join(ROOT, "profiles", "ncu_traffic.json.txt")) as fh:
             tab = json.load(fh)
     except (OSError, ValueError):
         return None, None
-    val = tab.get(key, {}).get(kernel)
+    now = kernel_sources_digest()
     src = {"file": "profiles/ncu_traffic.json.txt", "capture": tab.get("_capture"), "capture_commit": tab.get("_commit"),
-           "bench_commit": git_head()}
+           "capture_kernels_digest": tab.get("_kernels_digest"), "kernels_digest": now, "bench_commit": git_head()}
+    val = tab.get(key, {}).get(kernel)
+    if tab.get("_kernels_digest") != now:
+        val = None
     return val, src
 
 

@@ -127,3 +127,15 @@ def test_term_sharded_site_update_world2():
     assert int(nblk) == len(full.a_desc) and int(flops) == su.rotate_flops(full.d_left, chi, full.a_desc)
     alive = sum(1 for e in full.a_desc if chi[e["row"]] > 0 and chi[e["col"]] > 0)
     assert int(nalive) == alive                                                   # the shards partition the surviving blocks
+
+
+def test_bench_withholds_stale_traffic(monkeypatch):
+    """roofline.traffic comes from a committed ncu capture: bench.py reports it only while the digest of the kernel
+    sources equals the one recorded with the capture (profiles/ncu_traffic.json.txt), and null otherwise."""
+    import bench
+    val, src = bench.ncu_traffic("cyp", "p1_kernel")
+    assert src["capture_kernels_digest"] == src["kernels_digest"] == bench.kernel_sources_digest()
+    assert isinstance(val, int) and val > 10 ** 10          # the committed capture describes the committed kernels
+    monkeypatch.setattr(bench, "kernel_sources_digest", lambda: "0" * 16)
+    val, src = bench.ncu_traffic("cyp", "p1_kernel")
+    assert val is None and src["kernels_digest"] != src["capture_kernels_digest"]
